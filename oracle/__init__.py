@@ -1,0 +1,213 @@
+"""ctypes front-end of the CPU oracle (oracle/tmpc_oracle.cpp).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package; the product path (paper_2606_24039_b200) never does.  This file marshals numpy arrays
+into the C entry points and holds none of the method's arithmetic.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from .build import build as _build
+
+_LIB = None
+MAXR = 64
+
+
+class Cfg(C.Structure):
+    _fields_ = [
+        ("N", C.c_int32), ("nx", C.c_int32), ("nu", C.c_int32), ("ng", C.c_int32),
+        ("band", C.c_int32), ("g_sel", C.c_int32), ("zg_given", C.c_int32), ("model", C.c_int32),
+        ("sigma", C.c_double), ("rho_bar", C.c_double), ("rho_eq_scale", C.c_double), ("alpha", C.c_double),
+        ("gamma", C.c_double), ("lam", C.c_double), ("eps_abs", C.c_double), ("eps_rel", C.c_double),
+        ("wheelbase", C.c_double), ("dt", C.c_double),
+        ("g_lo", C.c_double * MAXR), ("g_hi", C.c_double * MAXR),
+        ("g_col", C.c_int32 * MAXR), ("soft", C.c_uint8 * MAXR),
+    ]
+
+
+def lib():
+    global _LIB
+    if _LIB is None:
+        _LIB = C.CDLL(_build())
+        assert _LIB.orc_sizeof_cfg() == C.sizeof(Cfg), "oracle Cfg layout mismatch"
+        _LIB.orc_project.argtypes = [C.c_int] + [C.c_double] * 6 + [C.POINTER(C.c_double)] * 2
+        _LIB.orc_project.restype = None
+    return _LIB
+
+
+def _p(a):
+    if a is None:
+        return None
+    assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _c(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+
+
+def make_cfg(w, band=None, zg_given=0, eps_abs=1e-8, eps_rel=1e-8, **over) -> Cfg:
+    """Cfg from a workloads.QPData (plus overrides such as rho_bar=..., lam=...)."""
+    c = Cfg()
+    c.N, c.nx, c.nu, c.ng = w.N, w.nx, w.nu, w.ng
+    nz = (w.N + 1) * (w.nx + w.nu)
+    c.band = int(nz > 512) if band is None else int(band)
+    c.g_sel = int(w.g_col is not None and w.G is None and w.model == 0)
+    c.zg_given = zg_given
+    c.model = w.model
+    c.sigma, c.rho_bar, c.rho_eq_scale, c.alpha = w.sigma, w.rho_bar, w.rho_eq_scale, w.alpha
+    c.gamma, c.lam = w.gamma, w.lam
+    c.eps_abs, c.eps_rel = eps_abs, eps_rel
+    c.wheelbase, c.dt = w.wheelbase, w.dt
+    for r in range(w.ng):
+        c.soft[r] = int(w.soft[r])
+        if c.g_sel:
+            c.g_col[r] = int(w.g_col[r])
+        if w.g_lo is not None:
+            c.g_lo[r], c.g_hi[r] = w.g_lo[r], w.g_hi[r]
+    for k, v in over.items():
+        setattr(c, k, v)
+    return c
+
+
+def _dims(w):
+    n = w.nx + w.nu
+    T = w.N + 1
+    return n, T, T * n, w.nx + w.N * w.nx, T * w.ng
+
+
+def _bs(a, b):
+    """Per-problem view of a [B|1,...] array."""
+    return a[b if a.shape[0] > 1 else 0]
+
+
+def assemble_S(w, cfg, b=0) -> np.ndarray:
+    n, T, nz, mf, mg = _dims(w)
+    S = np.zeros((nz, nz))
+    D, E, Am, Ap = _c(_bs(w.D, b)), _c(_bs(w.E, b)), _c(w.Am[b]), _c(w.Ap[b])
+    G = None if cfg.g_sel else _c(_bs(w.G, b))
+    lib().orc_assemble_S(C.byref(cfg), _p(D), _p(E), _p(Am), _p(Ap), _p(G), _p(S))
+    return S
+
+
+def solve_S(w, cfg, eta, b=0) -> np.ndarray:
+    n, T, nz, mf, mg = _dims(w)
+    xt = np.zeros(nz)
+    D, E, Am, Ap = _c(_bs(w.D, b)), _c(_bs(w.E, b)), _c(w.Am[b]), _c(w.Ap[b])
+    G = None if cfg.g_sel else _c(_bs(w.G, b))
+    rc = lib().orc_solve_S(C.byref(cfg), _p(D), _p(E), _p(Am), _p(Ap), _p(G), _p(_c(eta)), _p(xt))
+    assert rc == 0
+    return xt
+
+
+def project(soft, v, lo, hi, rho, gamma, lam):
+    z, xi = C.c_double(), C.c_double()
+    lib().orc_project(int(soft), v, lo, hi, rho, gamma, lam, C.byref(z), C.byref(xi))
+    return z.value, xi.value
+
+
+def new_state(w, B=None):
+    n, T, nz, mf, mg = _dims(w)
+    B = w.B if B is None else B
+    return dict(x=np.zeros((B, T, n)), zg=np.zeros((B, T, w.ng)), yf=np.zeros((B, mf)), yg=np.zeros((B, T, w.ng)),
+                xi=np.zeros((B, T, w.ng)))
+
+
+def admm(w, cfg, iters=None, state=None, nthreads=1):
+    """Alg. 3 on every problem of the batch.  Returns (state dict, info [B,4] = r_prim, r_dual, objective, min pivot)."""
+    n, T, nz, mf, mg = _dims(w)
+    iters = w.iters if iters is None else iters
+    st = new_state(w) if state is None else {k: _c(v).copy() for k, v in state.items()}
+    info = np.zeros((w.B, 4))
+    D, E, G = _c(w.D), _c(w.E), (None if cfg.g_sel else _c(w.G))
+    sD = 0 if D.shape[0] == 1 else D[0].size
+    sE = 0 if E.shape[0] == 1 else E[0].size
+    sG = 0 if (G is None or G.shape[0] == 1) else G[0].size
+    q, Am, Ap, b, xi0, lo, hi = _c(w.q), _c(w.Am), _c(w.Ap), _c(w.b), _c(w.x_init), _c(w.lo), _c(w.hi)
+    f = lib().orc_admm_batch
+    f.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int64, C.c_void_p, C.c_int64] + [C.c_void_p] * 6 + \
+                 [C.c_int64] + [C.c_void_p] * 7 + [C.c_int, C.c_void_p]
+    rc = f(C.byref(cfg), w.B, nthreads, _p(D), sD, _p(E), sE, _p(q), _p(Am), _p(Ap), _p(b), _p(xi0), _p(G), sG, _p(lo), _p(hi),
+           _p(st["x"]), _p(st["zg"]), _p(st["yf"]), _p(st["yg"]), _p(st["xi"]), iters, _p(info))
+    return st, info, rc
+
+
+def backward(w, cfg, state, dLdx, dLdxi=None):
+    """O-5 on every problem.  Returns dq [B,T,n], dxinit [B,nx], counts [B,2], rc [B]."""
+    n, T, nz, mf, mg = _dims(w)
+    dq = np.zeros((w.B, T, n))
+    dxi = np.zeros((w.B, w.nx))
+    counts = np.zeros((w.B, 2), dtype=np.int32)
+    rcs = np.zeros(w.B, dtype=np.int32)
+    f = lib().orc_backward
+    f.argtypes = [C.c_void_p] * 20
+    for b in range(w.B):
+        D, E = _c(_bs(w.D, b)), _c(_bs(w.E, b))
+        G = None if cfg.g_sel else _c(_bs(w.G, b))
+        args = [_c(w.q[b]), _c(w.Am[b]), _c(w.Ap[b]), _c(w.b[b]), _c(w.x_init[b])]
+        lo, hi = _c(w.lo[b]), _c(w.hi[b])
+        x, yg, xi = _c(state["x"][b]), _c(state["yg"][b]), _c(state["xi"][b])
+        gx = _c(dLdx[b])
+        gxi = None if dLdxi is None else _c(dLdxi[b])
+        rcs[b] = f(C.byref(cfg), _p(D), _p(E), *[_p(a) for a in args], _p(G), _p(lo), _p(hi), _p(x), _p(yg), _p(xi), _p(gx), _p(gxi),
+                   _p(dq[b]), _p(dxi[b]), counts[b].ctypes.data_as(C.c_void_p))
+    return dq, dxi, counts, rcs
+
+
+def classify(w, cfg, state, b=0):
+    n, T, nz, mf, mg = _dims(w)
+    cls = np.zeros(mg, dtype=np.int32)
+    f = lib().orc_classify
+    f.argtypes = [C.c_void_p] * 15
+    D, E = _c(_bs(w.D, b)), _c(_bs(w.E, b))
+    G = None if cfg.g_sel else _c(_bs(w.G, b))
+    f(C.byref(cfg), _p(D), _p(E), _p(_c(w.q[b])), _p(_c(w.Am[b])), _p(_c(w.Ap[b])), _p(_c(w.b[b])), _p(_c(w.x_init[b])), _p(G),
+      _p(_c(w.lo[b])), _p(_c(w.hi[b])), _p(_c(state["x"][b])), _p(_c(state["yg"][b])), _p(_c(state["xi"][b])), cls.ctypes.data_as(C.c_void_p))
+    return cls.reshape(T, w.ng)
+
+
+def bicycle_residual(cfg, vk, vk1):
+    f = np.zeros(4)
+    fn = lib().orc_bicycle_residual
+    fn.argtypes = [C.c_void_p] * 4
+    fn(C.byref(cfg), _p(_c(vk)), _p(_c(vk1)), _p(f))
+    return f
+
+
+def bicycle_linearize(w, cfg, xbar, b=0):
+    n, T, nz, mf, mg = _dims(w)
+    Am = np.zeros((w.N, 4, 6)); Ap = np.zeros((w.N, 4, 6)); bb = np.zeros((w.N, 4))
+    G = np.zeros((T, 3, 6)); lo = np.zeros((T, 3)); hi = np.zeros((T, 3))
+    fn = lib().orc_bicycle_linearize
+    fn.argtypes = [C.c_void_p] * 9
+    fn(C.byref(cfg), _p(_c(xbar)), _p(_c(w.stage_ref[b])), _p(Am), _p(Ap), _p(bb), _p(G), _p(lo), _p(hi))
+    return Am, Ap, bb, G, lo, hi
+
+
+def sqp_bicycle(w, cfg, n_sqp=None, iters=None, nthreads=1, with_fnorm=False):
+    """O-4 on every problem.  Returns (state dict with x = final xbar, info [B,4], rc[, fnorm [B,n_sqp+1]])."""
+    n, T, nz, mf, mg = _dims(w)
+    n_sqp = w.sqp_iters if n_sqp is None else n_sqp
+    iters = w.iters if iters is None else iters
+    st = new_state(w)
+    st["x"] = _c(w.xbar0).copy()
+    info = np.zeros((w.B, 4))
+    D, E, q, x0, ref = _c(w.D[0]), _c(w.E[0]), _c(w.q), _c(w.x_init), _c(w.stage_ref)
+    if with_fnorm:
+        fn = lib().orc_sqp_bicycle
+        fn.argtypes = [C.c_void_p] * 11 + [C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        fnorm = np.zeros((w.B, n_sqp + 1))
+        rc = 0
+        for b in range(w.B):
+            rc |= fn(C.byref(cfg), _p(D), _p(E), _p(q[b]), _p(x0[b]), _p(ref[b]), _p(st["x"][b]), _p(st["zg"][b]), _p(st["yf"][b]),
+                     _p(st["yg"][b]), _p(st["xi"][b]), n_sqp, iters, _p(info[b]), _p(fnorm[b]))
+        return st, info, rc, fnorm
+    fn = lib().orc_sqp_bicycle_batch
+    fn.argtypes = [C.c_void_p, C.c_int, C.c_int] + [C.c_void_p] * 10 + [C.c_int, C.c_int, C.c_void_p]
+    rc = fn(C.byref(cfg), w.B, nthreads, _p(D), _p(E), _p(q), _p(x0), _p(ref), _p(st["x"]), _p(st["zg"]), _p(st["yf"]), _p(st["yg"]),
+            _p(st["xi"]), n_sqp, iters, _p(info))
+    return st, info, rc

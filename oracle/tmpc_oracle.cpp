@@ -1,0 +1,414 @@
+// tmpc_oracle.cpp — TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, slow, single-threaded-per-problem fp64 CPU implementation of what the TurboMPC hot path
+// computes (arxiv/paper_2606_24039; citations are /root/reference/PAPER.md lines).  Only tests/,
+// __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call it.  It shares
+// no code, header, table or helper with paper_2606_24039_b200/csrc (the CUDA path) and neither
+// includes the other.  No BLAS/LAPACK/Eigen: scalar loops only, so it can be checked against the
+// paper by eye.
+//
+//   O-1  assemble   P, C, G from the stage blocks (eq. 1, 612-621 eq. 29-31) and
+//                   S = P + sigma I + rho_f C'C + rho_g G'G from THOSE matrices, never
+//                   from the Theta/Phi block formulas that the CUDA path uses.
+//   O-2  factor     hand-written Cholesky S = L L' (jik scalar loops) + two triangular solves.
+//                   Storage is a symmetric band of half-bandwidth bw: bw = n_z-1 is the literal dense
+//                   matrix (cfg.band = 0); bw = 2n-1 (cfg.band = 1) skips structural zeros only
+//                   (reading O-7) and is tested equal to the dense path.
+//   O-3  ADMM       Alg. 3 with eq. 8-16, 42-45, 51, in the paper's order.
+//   O-4  SQP        fixed-count full-step driver around O-1..O-3 with the bicycle model linearised
+//                   by eq. 36-38.
+//   O-5  backward   the definition: dense active-set KKT system eq. 62 / 65 solved by
+//                   Gaussian elimination with partial pivoting; dL/dq = -eta_x, dL/dx_init = +eta_f[0:nx].
+//
+// Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): Theta/Phi block formulas, LQR Riccati, brute-force
+// active-set enumeration, projection closed forms and invariants, residual convergence, central finite
+// differences for backward and for the bicycle Jacobians, dense == band.  Nothing is "parity unpinned".
+
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <thread>
+#include <vector>
+#include <algorithm>
+#include <limits>
+
+namespace {
+
+typedef std::vector<double> vec;
+
+struct Cfg {              // mirrored field-by-field by oracle/__init__.py (ctypes.Structure)
+  int32_t N, nx, nu, ng;
+  int32_t band;           // 0: dense storage (bw = n_z-1); 1: banded (bw = 2n-1)
+  int32_t g_sel;          // 1: G_t rows are unit vectors e_{g_col[r]} and G == nullptr
+  int32_t zg_given;       // 0: z_g^0 = clip(G x^0, lo, hi) (reading A-12); 1: use zg as passed (resume)
+  int32_t model;          // 0 none, 1 kinematic bicycle + implicit midpoint (reading A-24)
+  double sigma, rho_bar, rho_eq_scale, alpha;
+  double gamma, lam;      // gamma_xi and the L1 slack weight lambda (reading A-14)
+  double eps_abs, eps_rel;  // active-set classification (reading A-16)
+  double wheelbase, dt;   // bicycle
+  double g_lo[64], g_hi[64];  // un-shifted bounds of g_t (model != 0)
+  int32_t g_col[64];
+  uint8_t soft[64];       // per-row delta_xi (reading A-13)
+};
+
+// ---- symmetric band matrix, lower storage: element (i,j), i-bw <= j <= i, at a[i*(bw+1) + (j-i+bw)]
+struct Band {
+  int n, bw; vec a;
+  Band(int n_, int bw_) : n(n_), bw(std::min(bw_, n_ - 1 < 0 ? 0 : n_ - 1)), a((size_t)n_ * (std::min(bw_, n_ - 1 < 0 ? 0 : n_ - 1) + 1), 0.0) {}
+  inline double& lo(int i, int j) { return a[(size_t)i * (bw + 1) + (j - i + bw)]; }     // needs j <= i
+  inline double get(int i, int j) const { if (j > i) std::swap(i, j); if (i - j > bw) return 0.0; return a[(size_t)i * (bw + 1) + (j - i + bw)]; }
+  inline void add_sym(int i, int j, double v) { if (j > i) return; lo(i, j) += v; }      // caller passes both (i,j),(j,i); keep lower
+};
+
+// ---- a matrix whose every row is dense on a window of columns [c0, c0+len)  (C and G, eq. 30-31)
+struct Rows {
+  int m = 0, stride = 0; std::vector<int> c0, len; vec v;
+  void init(int m_, int stride_) { m = m_; stride = stride_; c0.assign(m, 0); len.assign(m, 0); v.assign((size_t)m * stride, 0.0); }
+  double* row(int r) { return &v[(size_t)r * stride]; }
+  const double* row(int r) const { return &v[(size_t)r * stride]; }
+  void mul(const vec& x, vec& z) const {           // z = M x
+    for (int r = 0; r < m; ++r) { double s = 0; const double* a = row(r); for (int k = 0; k < len[r]; ++k) s += a[k] * x[c0[r] + k]; z[r] = s; }
+  }
+  void mulT_add(const vec& y, vec& out) const {    // out += M' y
+    for (int r = 0; r < m; ++r) { const double* a = row(r); for (int k = 0; k < len[r]; ++k) out[c0[r] + k] += a[k] * y[r]; }
+  }
+  void add_AtA(Band& S, double w) const {          // S += w M'M   (row by row: w * row' row)
+    for (int r = 0; r < m; ++r) { const double* a = row(r);
+      for (int i = 0; i < len[r]; ++i) { if (a[i] == 0.0) continue; for (int j = 0; j <= i; ++j) S.lo(c0[r] + i, c0[r] + j) += w * a[i] * a[j]; } }
+  }
+  void add_AtWA(Band& S, const vec& w) const {     // S += M' diag(w) M
+    for (int r = 0; r < m; ++r) { if (w[r] == 0.0) continue; const double* a = row(r);
+      for (int i = 0; i < len[r]; ++i) { if (a[i] == 0.0) continue; for (int j = 0; j <= i; ++j) S.lo(c0[r] + i, c0[r] + j) += w[r] * a[i] * a[j]; } }
+  }
+};
+
+struct QP {               // one problem, assembled per O-1
+  int N, T, nx, nu, n, ng, nz, mf, mg;
+  Band P; Rows C, G; vec q, c, lo, hi;
+  QP(int N_, int nx_, int nu_, int ng_, int bw) : N(N_), T(N_ + 1), nx(nx_), nu(nu_), n(nx_ + nu_), ng(ng_), nz((N_ + 1) * (nx_ + nu_)),
+      mf(nx_ + N_ * nx_), mg((N_ + 1) * ng_), P((N_ + 1) * (nx_ + nu_), bw) {}
+};
+
+int half_bandwidth(const Cfg& c) { int n = c.nx + c.nu; int nz = (c.N + 1) * n; return c.band ? std::min(2 * n - 1, nz - 1) : nz - 1; }
+
+// O-1.  D [T][n][n], E [N][n][n] (block (t+1,t) of P), q [T][n], Am/Ap [N][nx][n], b [N][nx], x_init [nx],
+//       G [T][ng][n] or nullptr with cfg.g_sel, lo/hi [T][ng].
+QP assemble(const Cfg& cf, const double* D, const double* E, const double* q, const double* Am, const double* Ap, const double* b,
+            const double* x_init, const double* G, const double* lo, const double* hi) {
+  QP p(cf.N, cf.nx, cf.nu, cf.ng, half_bandwidth(cf));
+  const int n = p.n, nx = p.nx, N = p.N, T = p.T, ng = p.ng;
+  for (int t = 0; t < T; ++t)                                    // P: D_t on the diagonal (eq. 29)
+    for (int i = 0; i < n; ++i) for (int j = 0; j <= i; ++j) p.P.lo(t * n + i, t * n + j) += D[((size_t)t * n + i) * n + j];   // D_t symmetric by contract: lower part taken
+  for (int t = 0; t < N; ++t)                                    // E_t at block (t+1, t)
+    for (int i = 0; i < n; ++i) for (int j = 0; j < n; ++j) p.P.lo((t + 1) * n + i, t * n + j) += E[((size_t)t * n + i) * n + j];
+  p.q.assign(q, q + p.nz);
+  p.C.init(p.mf, 2 * n); p.c.assign(p.mf, 0.0);                  // C: eq. 30; rows 0..nx-1: A_init = [I 0], rhs x_init
+  for (int i = 0; i < nx; ++i) { p.C.c0[i] = 0; p.C.len[i] = n; p.C.row(i)[i] = 1.0; p.c[i] = x_init[i]; }
+  for (int t = 0; t < N; ++t) for (int i = 0; i < nx; ++i) {     // dynamics row: [A_t^- | A_t^+] on stages t, t+1 (eq. 36)
+    int r = nx + t * nx + i; p.C.c0[r] = t * n; p.C.len[r] = 2 * n;
+    for (int j = 0; j < n; ++j) { p.C.row(r)[j] = Am[((size_t)t * nx + i) * n + j]; p.C.row(r)[n + j] = Ap[((size_t)t * nx + i) * n + j]; }
+    p.c[r] = b[(size_t)t * nx + i];
+  }
+  p.G.init(p.mg, n); p.lo.assign(p.mg, 0.0); p.hi.assign(p.mg, 0.0);   // G: eq. 31, block diagonal
+  for (int t = 0; t < T; ++t) for (int r = 0; r < ng; ++r) {
+    int row = t * ng + r; p.G.c0[row] = t * n; p.G.len[row] = n;
+    if (cf.g_sel) p.G.row(row)[cf.g_col[r]] = 1.0; else for (int j = 0; j < n; ++j) p.G.row(row)[j] = G[((size_t)t * ng + r) * n + j];
+    p.lo[row] = lo[(size_t)t * ng + r]; p.hi[row] = hi[(size_t)t * ng + r];
+  }
+  return p;
+}
+
+// S = P + sigma I + C' diag(wf) C + G' diag(wg) G   (PAPER.md:172, 788 with rho = diag(rho_f I, rho_g I))
+Band build_S(const QP& p, double sigma, const vec& wf, const vec& wg) {
+  Band S = p.P;
+  for (int i = 0; i < p.nz; ++i) S.lo(i, i) += sigma;
+  p.C.add_AtWA(S, wf); p.G.add_AtWA(S, wg);
+  return S;
+}
+
+// O-2.  In-place Cholesky of the band (lower factor overwrites S).  Returns the smallest pivot seen (<=0: failure).
+double cholesky(Band& S) {
+  const int n = S.n, bw = S.bw; double minpiv = std::numeric_limits<double>::infinity();
+  for (int j = 0; j < n; ++j) {
+    for (int i = j; i <= std::min(n - 1, j + bw); ++i) {
+      double s = S.lo(i, j);
+      for (int k = std::max(0, i - bw); k < j; ++k) s -= S.lo(i, k) * S.lo(j, k);
+      if (i == j) { minpiv = std::min(minpiv, s); S.lo(j, j) = std::sqrt(s); }
+      else S.lo(i, j) = s / S.lo(j, j);
+    }
+  }
+  return minpiv;
+}
+void chol_solve(Band& L, vec& x) {            // x <- (L L')^{-1} x
+  const int n = L.n, bw = L.bw;
+  for (int i = 0; i < n; ++i) { double s = x[i]; for (int k = std::max(0, i - bw); k < i; ++k) s -= L.lo(i, k) * x[k]; x[i] = s / L.lo(i, i); }
+  for (int i = n - 1; i >= 0; --i) { double s = x[i]; for (int k = i + 1; k <= std::min(n - 1, i + bw); ++k) s -= L.lo(k, i) * x[k]; x[i] = s / L.lo(i, i); }
+}
+
+void band_mul(const Band& A, const vec& x, vec& y) {   // y = A x (symmetric)
+  for (int i = 0; i < A.n; ++i) { double s = 0; for (int j = std::max(0, i - A.bw); j <= std::min(A.n - 1, i + A.bw); ++j) s += A.get(i, j) * x[j]; y[i] = s; }
+}
+
+inline double clip(double v, double lo, double hi) { return std::min(std::max(v, lo), hi); }
+
+// O-3 step 5.  Hard row: eq. 13.  Soft row: eq. 15a/15b generalised with the L1 weight lambda (reading A-14);
+// lambda = 0 is exactly eq. 15 == the 3-case formula at PAPER.md:836.
+inline void project_row(bool soft, double v, double lo, double hi, double rho, double gamma, double lam, double& z, double& xi) {
+  if (!soft) { z = clip(v, lo, hi); xi = 0.0; return; }
+  double sp = std::max(0.0, (rho * (v - hi) - lam) / (rho + gamma));
+  double sm = std::max(0.0, (rho * (lo - v) - lam) / (rho + gamma));
+  z = clip(v, lo, hi) + sp - sm; xi = sm - sp;
+}
+
+struct Info { double r_prim, r_dual, objective, min_pivot; };
+
+// O-3.  K iterations of Alg. 3.  x [nz], zg [mg], yf [mf], yg [mg], xi [mg] in/out.
+Info admm(const Cfg& cf, const QP& p, double* x_, double* zg_, double* yf_, double* yg_, double* xi_, int K) {
+  const double rho_g = cf.rho_bar, rho_f = cf.rho_eq_scale * cf.rho_bar, sigma = cf.sigma, alpha = cf.alpha;
+  vec x(x_, x_ + p.nz), zg(p.mg), yf(yf_, yf_ + p.mf), yg(yg_, yg_ + p.mg), xi(p.mg, 0.0);
+  vec tmp(p.mg);
+  if (cf.zg_given) { zg.assign(zg_, zg_ + p.mg); xi.assign(xi_, xi_ + p.mg); }
+  else { p.G.mul(x, tmp); for (int i = 0; i < p.mg; ++i) zg[i] = clip(tmp[i], p.lo[i], p.hi[i]); }
+  Band L = build_S(p, sigma, vec(p.mf, rho_f), vec(p.mg, rho_g));
+  Info info; info.min_pivot = cholesky(L);
+  vec eta(p.nz), xt(p.nz), ztf(p.mf), ztg(p.mg), rf(p.mf), rg(p.mg);
+  for (int k = 0; k < K; ++k) {
+    // 1. eta = sigma x - q + C'(rho_f c - y_f) + G'(rho_g z_g - y_g)              (eq. 51, z_f == c)
+    for (int i = 0; i < p.nz; ++i) eta[i] = sigma * x[i] - p.q[i];
+    for (int i = 0; i < p.mf; ++i) rf[i] = rho_f * p.c[i] - yf[i];
+    for (int i = 0; i < p.mg; ++i) rg[i] = rho_g * zg[i] - yg[i];
+    p.C.mulT_add(rf, eta); p.G.mulT_add(rg, eta);
+    // 2. x~ = S^{-1} eta (eq. 8);  z~ = A x~ (eq. 9)
+    xt = eta; chol_solve(L, xt); p.C.mul(xt, ztf); p.G.mul(xt, ztg);
+    // 3. x^{k+1} = alpha x~ + (1-alpha) x^k                                         (eq. 10-11)
+    for (int i = 0; i < p.nz; ++i) x[i] = alpha * xt[i] + (1.0 - alpha) * x[i];
+    // 4.-6. z^_g, v, projection (eq. 12-15), dual updates (eq. 44-45)
+    for (int i = 0; i < p.mg; ++i) {
+      double zh = alpha * ztg[i] + (1.0 - alpha) * zg[i];
+      double v = zh + yg[i] / rho_g, z, s;
+      project_row(cf.soft[i % p.ng] != 0, v, p.lo[i], p.hi[i], rho_g, cf.gamma, cf.lam, z, s);
+      zg[i] = z; xi[i] = s; yg[i] = yg[i] + rho_g * (zh - z);
+    }
+    for (int i = 0; i < p.mf; ++i) yf[i] = yf[i] + rho_f * alpha * (ztf[i] - p.c[i]);
+  }
+  // residuals (eq. 3) and objective at the K-th iterate
+  p.C.mul(x, ztf); p.G.mul(x, ztg);
+  double rp = 0; for (int i = 0; i < p.mf; ++i) rp = std::max(rp, std::fabs(ztf[i] - p.c[i]));
+  for (int i = 0; i < p.mg; ++i) rp = std::max(rp, std::fabs(ztg[i] - zg[i]));
+  vec g(p.nz), Px(p.nz); band_mul(p.P, x, Px);
+  for (int i = 0; i < p.nz; ++i) g[i] = Px[i] + p.q[i];
+  p.C.mulT_add(yf, g); p.G.mulT_add(yg, g);
+  double rd = 0; for (int i = 0; i < p.nz; ++i) rd = std::max(rd, std::fabs(g[i]));
+  double obj = 0; for (int i = 0; i < p.nz; ++i) obj += 0.5 * x[i] * Px[i] + p.q[i] * x[i];
+  for (int i = 0; i < p.mg; ++i) if (cf.soft[i % p.ng] && xi[i] != 0.0) {
+    double sg = xi[i] > 0 ? 1.0 : -1.0;
+    rd = std::max(rd, std::fabs(cf.gamma * xi[i] + cf.lam * sg + yg[i]));
+    obj += cf.lam * std::fabs(xi[i]) + 0.5 * cf.gamma * xi[i] * xi[i];
+  }
+  info.r_prim = rp; info.r_dual = rd; info.objective = obj;
+  std::copy(x.begin(), x.end(), x_); std::copy(zg.begin(), zg.end(), zg_); std::copy(yf.begin(), yf.end(), yf_);
+  std::copy(yg.begin(), yg.end(), yg_); std::copy(xi.begin(), xi.end(), xi_);
+  return info;
+}
+
+// dense Gaussian elimination with partial pivoting, A [m][m] row-major, rhs in/out.  Returns min |pivot|.
+double gauss_solve(vec& A, vec& rhs, int m) {
+  double minpiv = std::numeric_limits<double>::infinity();
+  for (int k = 0; k < m; ++k) {
+    int piv = k; double best = std::fabs(A[(size_t)k * m + k]);
+    for (int i = k + 1; i < m; ++i) { double a = std::fabs(A[(size_t)i * m + k]); if (a > best) { best = a; piv = i; } }
+    minpiv = std::min(minpiv, best);
+    if (best == 0.0) return 0.0;
+    if (piv != k) { for (int j = 0; j < m; ++j) std::swap(A[(size_t)k * m + j], A[(size_t)piv * m + j]); std::swap(rhs[k], rhs[piv]); }
+    double d = A[(size_t)k * m + k];
+    for (int i = k + 1; i < m; ++i) { double f = A[(size_t)i * m + k] / d; if (f == 0.0) continue;
+      for (int j = k; j < m; ++j) A[(size_t)i * m + j] -= f * A[(size_t)k * m + j]; rhs[i] -= f * rhs[k]; }
+  }
+  for (int i = m - 1; i >= 0; --i) { double s = rhs[i]; for (int j = i + 1; j < m; ++j) s -= A[(size_t)i * m + j] * rhs[j]; rhs[i] = s / A[(size_t)i * m + i]; }
+  return minpiv;
+}
+
+// Row classification (readings A-16): 0 inactive, 1 hard-active, 2 soft-active.
+void classify(const Cfg& cf, const QP& p, const double* x, const double* yg, const double* xi, std::vector<int>& cls) {
+  vec xv(x, x + p.nz), gx(p.mg); p.G.mul(xv, gx);
+  double ymax = 0; for (int i = 0; i < p.mg; ++i) ymax = std::max(ymax, std::fabs(yg[i]));
+  const double eps_y = cf.eps_abs + cf.eps_rel * ymax;
+  cls.assign(p.mg, 0);
+  for (int i = 0; i < p.mg; ++i) {
+    bool soft = cf.soft[i % p.ng] != 0;
+    if (soft && std::fabs(xi[i]) > cf.eps_abs) { cls[i] = 2; continue; }
+    if (std::fabs(yg[i]) > eps_y) { cls[i] = 1; continue; }
+    double dl = gx[i] - p.lo[i], du = p.hi[i] - gx[i];
+    bool near_lo = std::isfinite(p.lo[i]) && dl <= cf.eps_abs + cf.eps_rel * std::fabs(p.lo[i]);
+    bool near_hi = std::isfinite(p.hi[i]) && du <= cf.eps_abs + cf.eps_rel * std::fabs(p.hi[i]);
+    if (near_lo || near_hi) cls[i] = 1;
+  }
+}
+
+// O-5.  Backward by the definition (eq. 62 / 65).  Returns min |pivot| of the elimination.
+double backward(const Cfg& cf, const QP& p, const double* x, const double* yg, const double* xi, const double* dLdx, const double* dLdxi,
+                double* dq, double* dxinit, int* n_hard, int* n_soft) {
+  std::vector<int> cls; classify(cf, p, x, yg, xi, cls);
+  std::vector<int> hard; int ns = 0;
+  for (int i = 0; i < p.mg; ++i) { if (cls[i] == 1) hard.push_back(i); if (cls[i] == 2) ++ns; }
+  const int nh = (int)hard.size(), m = p.nz + p.mf + nh;
+  vec K((size_t)m * m, 0.0), rhs(m, 0.0);
+  for (int i = 0; i < p.nz; ++i) for (int j = std::max(0, i - p.P.bw); j <= std::min(p.nz - 1, i + p.P.bw); ++j) K[(size_t)i * m + j] = p.P.get(i, j);
+  for (int i = 0; i < p.nz; ++i) rhs[i] = dLdx[i];
+  for (int r = 0; r < p.mg; ++r) if (cls[r] == 2) {              // + gamma G_s' G_s ;  rhs -= G_s' Sigma_s dL/dxi_s  (eq. 65)
+    const double* a = p.G.row(r); int c0 = p.G.c0[r];
+    for (int i = 0; i < p.G.len[r]; ++i) for (int j = 0; j < p.G.len[r]; ++j) K[(size_t)(c0 + i) * m + c0 + j] += cf.gamma * a[i] * a[j];
+    if (dLdxi) { double sg = xi[r] > 0 ? 1.0 : -1.0; for (int i = 0; i < p.G.len[r]; ++i) rhs[c0 + i] -= a[i] * sg * dLdxi[r]; }
+  }
+  for (int r = 0; r < p.mf; ++r) { const double* a = p.C.row(r); for (int k = 0; k < p.C.len[r]; ++k) { K[(size_t)(p.nz + r) * m + p.C.c0[r] + k] = a[k]; K[(size_t)(p.C.c0[r] + k) * m + p.nz + r] = a[k]; } }
+  for (int h = 0; h < nh; ++h) { int r = hard[h]; const double* a = p.G.row(r); for (int k = 0; k < p.G.len[r]; ++k) { K[(size_t)(p.nz + p.mf + h) * m + p.G.c0[r] + k] = a[k]; K[(size_t)(p.G.c0[r] + k) * m + p.nz + p.mf + h] = a[k]; } }
+  double piv = gauss_solve(K, rhs, m);
+  for (int i = 0; i < p.nz; ++i) dq[i] = -rhs[i];                 // dL/dq = -eta_x         (eq. 59, dF/dq = [I;0;0])
+  for (int i = 0; i < p.nx; ++i) dxinit[i] = rhs[p.nz + i];       // dL/dx_init = +eta_f[0:nx] (dF/dx_init = -I on init rows)
+  *n_hard = nh; *n_soft = ns;
+  return piv;
+}
+
+// ---- kinematic bicycle, implicit midpoint (reading A-24).  v = (px, py, psi, vel, a, delta).
+// residual f_k = x_k + dt F((x_k + x_{k+1})/2, u_k) - x_{k+1},  F = (v cos psi, v sin psi, v/L tan delta, a)
+void bicycle_residual(double Lwb, double dt, const double* vk, const double* vk1, double* f) {
+  double psi = 0.5 * (vk[2] + vk1[2]), vel = 0.5 * (vk[3] + vk1[3]), a = vk[4], del = vk[5];
+  double F[4] = { vel * std::cos(psi), vel * std::sin(psi), vel / Lwb * std::tan(del), a };
+  for (int i = 0; i < 4; ++i) f[i] = vk[i] + dt * F[i] - vk1[i];
+}
+// eq. 36-38 for the bicycle: Am = df/dv_k, Ap = df/dv_{k+1}, b = Am v_k + Ap v_{k+1} - f (eq. 37);
+// g_t(v) = (a, delta, lateral error e = -sin(psi_ref)(px - px_ref) + cos(psi_ref)(py - py_ref)) is linear in v,
+// so G_t is its constant Jacobian and the shifted bounds (eq. 38) are g_lo - g(v) + G v = g_lo + G_lat . p_ref on row 2.
+void bicycle_linearize(const Cfg& cf, const double* xbar, const double* ref, double* Am, double* Ap, double* b, double* G, double* lo, double* hi) {
+  const int N = cf.N, n = 6, nx = 4; const double dt = cf.dt, L = cf.wheelbase;
+  for (int t = 0; t < N; ++t) {
+    const double* vk = xbar + (size_t)t * n; const double* vk1 = vk + n;
+    double psi = 0.5 * (vk[2] + vk1[2]), vel = 0.5 * (vk[3] + vk1[3]), del = vk[5];
+    double Fx[4][4] = {{0, 0, -vel * std::sin(psi), std::cos(psi)}, {0, 0, vel * std::cos(psi), std::sin(psi)}, {0, 0, 0, std::tan(del) / L}, {0, 0, 0, 0}};
+    double Fu[4][2] = {{0, 0}, {0, 0}, {0, vel / (L * std::cos(del) * std::cos(del))}, {1, 0}};
+    double* am = Am + (size_t)t * nx * n; double* ap = Ap + (size_t)t * nx * n;
+    for (int i = 0; i < nx; ++i) {
+      for (int j = 0; j < nx; ++j) { am[i * n + j] = (i == j ? 1.0 : 0.0) + 0.5 * dt * Fx[i][j]; ap[i * n + j] = (i == j ? -1.0 : 0.0) + 0.5 * dt * Fx[i][j]; }
+      for (int j = 0; j < 2; ++j) { am[i * n + nx + j] = dt * Fu[i][j]; ap[i * n + nx + j] = 0.0; }
+    }
+    double f[4]; bicycle_residual(L, dt, vk, vk1, f);
+    for (int i = 0; i < nx; ++i) { double s = -f[i]; for (int j = 0; j < n; ++j) s += am[i * n + j] * vk[j] + ap[i * n + j] * vk1[j]; b[(size_t)t * nx + i] = s; }
+  }
+  for (int t = 0; t <= N; ++t) {
+    const double* r = ref + (size_t)t * n; double* g = G + (size_t)t * 3 * n;
+    for (int k = 0; k < 3 * n; ++k) g[k] = 0.0;
+    g[0 * n + 4] = 1.0; g[1 * n + 5] = 1.0; g[2 * n + 0] = -std::sin(r[2]); g[2 * n + 1] = std::cos(r[2]);
+    double off = g[2 * n + 0] * r[0] + g[2 * n + 1] * r[1];
+    for (int k = 0; k < 3; ++k) { double o = (k == 2) ? off : 0.0; lo[(size_t)t * 3 + k] = cf.g_lo[k] + o; hi[(size_t)t * 3 + k] = cf.g_hi[k] + o; }
+  }
+}
+
+}  // namespace
+
+extern "C" {
+
+// Dense S [nz][nz] (full symmetric) for the Theta/Phi pin.
+int orc_assemble_S(const Cfg* cf, const double* D, const double* E, const double* Am, const double* Ap, const double* G, double* S_out) {
+  int n = cf->nx + cf->nu, nz = (cf->N + 1) * n, T = cf->N + 1;
+  vec q(nz, 0.0), b((size_t)cf->N * cf->nx, 0.0), xi(cf->nx, 0.0), lo((size_t)T * cf->ng, 0.0);
+  QP p = assemble(*cf, D, E, q.data(), Am, Ap, b.data(), xi.data(), G, lo.data(), lo.data());
+  Band S = build_S(p, cf->sigma, vec(p.mf, cf->rho_eq_scale * cf->rho_bar), vec(p.mg, cf->rho_bar));
+  for (int i = 0; i < nz; ++i) for (int j = 0; j < nz; ++j) S_out[(size_t)i * nz + j] = S.get(i, j);
+  return 0;
+}
+
+// x~ = S^{-1} eta by O-2 (pin for the block factor, the solves and the cyclic reduction).  Returns 0, or 1 on a non-positive pivot.
+int orc_solve_S(const Cfg* cf, const double* D, const double* E, const double* Am, const double* Ap, const double* G, const double* eta, double* xt) {
+  int n = cf->nx + cf->nu, nz = (cf->N + 1) * n, T = cf->N + 1;
+  vec q(nz, 0.0), b((size_t)cf->N * cf->nx, 0.0), xi(cf->nx, 0.0), lo((size_t)T * cf->ng, 0.0);
+  QP p = assemble(*cf, D, E, q.data(), Am, Ap, b.data(), xi.data(), G, lo.data(), lo.data());
+  Band L = build_S(p, cf->sigma, vec(p.mf, cf->rho_eq_scale * cf->rho_bar), vec(p.mg, cf->rho_bar));
+  double piv = cholesky(L); vec x(eta, eta + nz); chol_solve(L, x); std::copy(x.begin(), x.end(), xt);
+  return piv > 0 ? 0 : 1;
+}
+
+void orc_project(int soft, double v, double lo, double hi, double rho, double gamma, double lam, double* z, double* xi) { project_row(soft != 0, v, lo, hi, rho, gamma, lam, *z, *xi); }
+
+// One problem, K iterations of Alg. 3.  info_out[4] = r_prim, r_dual, objective, min Cholesky pivot.
+int orc_admm(const Cfg* cf, const double* D, const double* E, const double* q, const double* Am, const double* Ap, const double* b, const double* x_init,
+             const double* G, const double* lo, const double* hi, double* x, double* zg, double* yf, double* yg, double* xi, int K, double* info_out) {
+  QP p = assemble(*cf, D, E, q, Am, Ap, b, x_init, G, lo, hi);
+  Info i = admm(*cf, p, x, zg, yf, yg, xi, K);
+  info_out[0] = i.r_prim; info_out[1] = i.r_dual; info_out[2] = i.objective; info_out[3] = i.min_pivot;
+  return i.min_pivot > 0 ? 0 : 1;
+}
+
+// Batch of independent problems spread over nthreads std::threads (each problem stays single-threaded).  Strides in elements; 0 = shared.
+int orc_admm_batch(const Cfg* cf, int B, int nthreads, const double* D, int64_t sD, const double* E, int64_t sE, const double* q, const double* Am,
+                   const double* Ap, const double* b, const double* x_init, const double* G, int64_t sG, const double* lo, const double* hi,
+                   double* x, double* zg, double* yf, double* yg, double* xi, int K, double* info_out) {
+  const int n = cf->nx + cf->nu, T = cf->N + 1, nz = T * n, mf = cf->nx + cf->N * cf->nx, mg = T * cf->ng;
+  std::vector<int> fail(std::max(1, nthreads), 0);
+  auto work = [&](int tid) {
+    for (int p = tid; p < B; p += nthreads)
+      fail[tid] |= orc_admm(cf, D + sD * p, E + sE * p, q + (size_t)nz * p, Am + (size_t)cf->N * cf->nx * n * p, Ap + (size_t)cf->N * cf->nx * n * p,
+                            b + (size_t)cf->N * cf->nx * p, x_init + (size_t)cf->nx * p, G ? G + sG * p : nullptr, lo + (size_t)mg * p, hi + (size_t)mg * p,
+                            x + (size_t)nz * p, zg + (size_t)mg * p, yf + (size_t)mf * p, yg + (size_t)mg * p, xi + (size_t)mg * p, K, info_out + 4 * (size_t)p);
+  };
+  if (nthreads <= 1) { nthreads = 1; work(0); }
+  else { std::vector<std::thread> th; for (int t = 0; t < nthreads; ++t) th.emplace_back(work, t); for (auto& t : th) t.join(); }
+  int f = 0; for (int v : fail) f |= v; return f;
+}
+
+// O-5 for one problem.  counts_out[2] = #hard-active, #soft-active.  Returns 0, or 2 when the KKT system is (numerically) singular (reading A-18).
+int orc_backward(const Cfg* cf, const double* D, const double* E, const double* q, const double* Am, const double* Ap, const double* b, const double* x_init,
+                 const double* G, const double* lo, const double* hi, const double* x, const double* yg, const double* xi, const double* dLdx,
+                 const double* dLdxi, double* dq, double* dxinit, int* counts_out) {
+  Cfg c = *cf;
+  QP p = assemble(c, D, E, q, Am, Ap, b, x_init, G, lo, hi);
+  double piv = backward(c, p, x, yg, xi, dLdx, dLdxi, dq, dxinit, &counts_out[0], &counts_out[1]);
+  return piv > 1e-12 ? 0 : 2;
+}
+
+int orc_classify(const Cfg* cf, const double* D, const double* E, const double* q, const double* Am, const double* Ap, const double* b, const double* x_init,
+                 const double* G, const double* lo, const double* hi, const double* x, const double* yg, const double* xi, int32_t* cls_out) {
+  QP p = assemble(*cf, D, E, q, Am, Ap, b, x_init, G, lo, hi);
+  std::vector<int> cls; classify(*cf, p, x, yg, xi, cls); for (int i = 0; i < p.mg; ++i) cls_out[i] = cls[i];
+  return 0;
+}
+
+void orc_bicycle_residual(const Cfg* cf, const double* vk, const double* vk1, double* f) { bicycle_residual(cf->wheelbase, cf->dt, vk, vk1, f); }
+void orc_bicycle_linearize(const Cfg* cf, const double* xbar, const double* ref, double* Am, double* Ap, double* b, double* G, double* lo, double* hi) {
+  bicycle_linearize(*cf, xbar, ref, Am, Ap, b, G, lo, hi);
+}
+
+// O-4.  n_sqp x (linearise at xbar -> K ADMM iterations warm-started with x^0 = xbar, y carried, z_g re-projected -> full step), reading A-26.
+// xbar [T][n] in/out (final iterate), yf/yg in/out, xi/zg out.  fnorm_out[n_sqp+1]: ||f(xbar)||_inf before each step and after the last.
+int orc_sqp_bicycle(const Cfg* cf, const double* D, const double* E, const double* q, const double* x_init, const double* ref, double* xbar, double* zg,
+                    double* yf, double* yg, double* xi, int n_sqp, int K, double* info_out, double* fnorm_out) {
+  const int N = cf->N, T = N + 1, n = 6, nx = 4, ng = 3;
+  vec Am((size_t)N * nx * n), Ap((size_t)N * nx * n), b((size_t)N * nx), G((size_t)T * ng * n), lo((size_t)T * ng), hi((size_t)T * ng);
+  Cfg c = *cf; c.g_sel = 0; c.zg_given = 0; int fail = 0;
+  auto fnorm = [&]() { double m = 0, f[4]; for (int t = 0; t < N; ++t) { bicycle_residual(c.wheelbase, c.dt, xbar + (size_t)t * n, xbar + (size_t)(t + 1) * n, f); for (int i = 0; i < 4; ++i) m = std::max(m, std::fabs(f[i])); } return m; };
+  for (int s = 0; s < n_sqp; ++s) {
+    if (fnorm_out) fnorm_out[s] = fnorm();
+    bicycle_linearize(c, xbar, ref, Am.data(), Ap.data(), b.data(), G.data(), lo.data(), hi.data());
+    fail |= orc_admm(&c, D, E, q, Am.data(), Ap.data(), b.data(), x_init, G.data(), lo.data(), hi.data(), xbar, zg, yf, yg, xi, K, info_out);
+  }
+  if (fnorm_out) fnorm_out[n_sqp] = fnorm();
+  return fail;
+}
+
+int orc_sqp_bicycle_batch(const Cfg* cf, int B, int nthreads, const double* D, const double* E, const double* q, const double* x_init, const double* ref,
+                          double* xbar, double* zg, double* yf, double* yg, double* xi, int n_sqp, int K, double* info_out) {
+  const int T = cf->N + 1, n = 6, nz = T * n, mf = 4 + cf->N * 4, mg = T * 3;
+  std::vector<int> fail(std::max(1, nthreads), 0);
+  auto work = [&](int tid) {
+    for (int p = tid; p < B; p += nthreads)
+      fail[tid] |= orc_sqp_bicycle(cf, D, E, q + (size_t)nz * p, x_init + (size_t)4 * p, ref + (size_t)nz * p, xbar + (size_t)nz * p, zg + (size_t)mg * p,
+                                   yf + (size_t)mf * p, yg + (size_t)mg * p, xi + (size_t)mg * p, n_sqp, K, info_out + 4 * (size_t)p, nullptr);
+  };
+  if (nthreads <= 1) { nthreads = 1; work(0); }
+  else { std::vector<std::thread> th; for (int t = 0; t < nthreads; ++t) th.emplace_back(work, t); for (auto& t : th) t.join(); }
+  int f = 0; for (int v : fail) f |= v; return f;
+}
+
+int orc_sizeof_cfg() { return (int)sizeof(Cfg); }
+
+}  // extern "C"
