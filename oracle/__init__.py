@@ -144,7 +144,7 @@ def backward(w, cfg, state, dLdx, dLdxi=None):
     counts = np.zeros((w.B, 2), dtype=np.int32)
     rcs = np.zeros(w.B, dtype=np.int32)
     f = lib().orc_backward
-    f.argtypes = [C.c_void_p] * 20
+    f.argtypes = [C.c_void_p] * 19
     for b in range(w.B):
         D, E = _c(_bs(w.D, b)), _c(_bs(w.E, b))
         G = None if cfg.g_sel else _c(_bs(w.G, b))
