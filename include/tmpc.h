@@ -1,0 +1,123 @@
+/* tmpc.h — C ABI of the B200-native batched ADMM-QP hot path of TurboMPC (arxiv/paper_2606_24039).
+ *
+ * Citations are lines of the paper text with the equation / algorithm they fall in.
+ * The library solves, for a batch of B independent stage-structured QPs (eq. 1 / 28-31)
+ *
+ *     min 1/2 x'Px + q'x + gamma/2 |xi|^2 + lambda |xi|_1   s.t.  Cx = c,  lo <= Gx + delta.xi <= hi,
+ *
+ * with x = (x_t,u_t)_{t=0..N} (n = nx+nu per stage, T = N+1 stages), P block-tridiagonal (D_t, E_t),
+ * C block-bidiagonal (A_init = [I 0], A_t^-, A_t^+), G block-diagonal, by the OSQP-style ADMM of Alg. 3
+ * (PAPER.md:207-224): per iteration a solve with the block-tridiagonal S = P + sigma I + A' diag(rho) A
+ * (eq. 8), over-relaxation (eq. 10), the (slack-smoothed) projection (eq. 12-15)
+ * and the dual update (eq. 16).  tmpc_backward gives implicit-differentiation gradients (Alg. 2, eq. 59-65).
+ *
+ * Conventions
+ *  - every array pointer is DEVICE memory owned by the caller (e.g. torch tensors), contiguous, in the working
+ *    dtype of the handle (float for TMPC_F32, double for TMPC_F64); int32 for status.  Layouts are problem-major,
+ *    row-major blocks, as written beside each field.  A batch stride of 0 means "one copy shared by the batch".
+ *  - the library allocates no device memory: the caller passes a workspace of tmpc_workspace_bytes() bytes to
+ *    tmpc_setup; the factor lives there from tmpc_factor until the next tmpc_factor / tmpc_destroy.
+ *  - all calls enqueue on the stream given to tmpc_setup and return without synchronising
+ *    (tmpc_admm_solve_host is the exception: it takes HOST buffers and synchronises before returning).
+ *  - errors: bad arguments / shapes / call order -> a tmpc_status code and nothing is enqueued.  Numerical
+ *    trouble never aborts the batch: bits are set in info.status[b] (TMPC_ST_*).
+ *  - there is no CPU fallback: without a CUDA device every compute entry point returns TMPC_E_CUDA.
+ */
+#ifndef TMPC_H_
+#define TMPC_H_
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TMPC_MAX_NG 32
+
+typedef struct tmpc_ctx* tmpc_handle; /* opaque; owns nothing the caller passed in */
+
+typedef enum { TMPC_OK = 0, TMPC_E_BADARG, TMPC_E_DIM, TMPC_E_UNSUPPORTED, TMPC_E_STATE, TMPC_E_WORKSPACE, TMPC_E_CUDA } tmpc_status;
+typedef enum { TMPC_F32 = 0, TMPC_F64 = 1 } tmpc_dtype;
+typedef enum { TMPC_MODEL_NONE = 0, TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT = 1 } tmpc_model;
+typedef enum { TMPC_LIN_SEQUENTIAL = 0, TMPC_LIN_CYCLIC_REDUCTION = 1, TMPC_LIN_AUTO = 2 } tmpc_linsolve;
+typedef enum { TMPC_BWD_REFACTOR_REFINE = 0, TMPC_BWD_ADMM_REUSE_FACTOR = 1 } tmpc_bwd_mode;
+
+/* info.status[b] bits */
+#define TMPC_ST_PIVOT 1  /* a non-positive pivot was met while factoring S (replaced by a tiny positive one) */
+#define TMPC_ST_NAN 2    /* a non-finite value appeared in the iterate */
+/* tmpc_admm_solve flags */
+#define TMPC_SOLVE_ZG_GIVEN 1 /* use state.zg / state.xi as passed (resume); default z_g^0 = clip(G x^0, lo, hi) */
+
+typedef struct { /* POD, copied at tmpc_setup */
+  int32_t batch, N, nx, nu, ng; /* n_init = nx: the rows x_0 = x_init are implicit (A_init = [I 0]) */
+  int32_t dtype;                /* tmpc_dtype */
+  int32_t model;                /* tmpc_model, used by tmpc_linearize only */
+  int32_t linsolve;             /* tmpc_linsolve */
+  double sigma, rho_bar, rho_eq_scale, alpha; /* sigma=1e-6, rho_g=rho_bar, rho_f=rho_eq_scale*rho_bar, alpha in (0,2) */
+  double slack_gamma, slack_lambda;           /* gamma_xi and an L1 slack weight lambda >= 0 (0 = the paper's scheme) */
+  double eps_active_abs, eps_active_rel;      /* active-set classification of tmpc_backward */
+  double wheelbase, dt;                       /* bicycle model */
+  double g_lo[TMPC_MAX_NG], g_hi[TMPC_MAX_NG]; /* un-shifted bounds of g_t(x,u) for tmpc_linearize (eq. 38) */
+  int32_t g_is_selection;                     /* 1: row r of every G_t is the unit vector e_{g_col[r]} and qp.G is NULL */
+  int32_t g_col[TMPC_MAX_NG];
+  uint8_t soft_row[TMPC_MAX_NG];              /* per-row delta_xi, same for every stage and problem */
+} tmpc_config;
+
+typedef struct {
+  const void* D; int64_t D_bstride; /* [B|1][T][n][n]   symmetric diagonal blocks of P (eq. 29), full storage            */
+  const void* E; int64_t E_bstride; /* [B|1][N][n][n]   block (t+1,t) of P                                               */
+  const void* q;                    /* [B][T][n]                                                                         */
+  const void* Am; const void* Ap;   /* [B][N][nx][n]    A_t^-, A_t^+ (eq. 36): Am v_t + Ap v_{t+1} = b_t                   */
+  const void* b;                    /* [B][N][nx]                                                                        */
+  const void* x_init;               /* [B][nx]                                                                           */
+  const void* G; int64_t G_bstride; /* [B|1][T][ng][n]  or NULL with g_is_selection (eq. 31)                             */
+  const void* lo; const void* hi;   /* [B][T][ng]       +-INFINITY allowed (eq. 38)                                      */
+} tmpc_qp; /* tmpc_linearize WRITES Am, Ap, b, G, lo, hi (the caller passes writable buffers there) */
+
+typedef struct { /* ADMM state, in/out = warm start (Alg. 3 'Initial guess') */
+  void* x;  /* [B][T][n]   */
+  void* zg; /* [B][T][ng]  */
+  void* yf; /* [B][nx+N*nx] multipliers of (x_0 = x_init ; dynamics rows) */
+  void* yg; /* [B][T][ng]  */
+  void* xi; /* [B][T][ng]  slack, out (in with TMPC_SOLVE_ZG_GIVEN) */
+} tmpc_state;
+
+typedef struct { /* per-problem outputs at the last iterate (eq. 3); any pointer may be NULL */
+  void* r_prim; void* r_dual; void* objective; /* [B] working dtype */
+  int32_t* status;                             /* [B] TMPC_ST_* bits (written by tmpc_factor and tmpc_admm_solve) */
+} tmpc_info;
+
+/* Bytes of device workspace tmpc_setup needs for this config. */
+tmpc_status tmpc_workspace_bytes(const tmpc_config* cfg, size_t* bytes);
+/* Creates a handle. workspace: device memory of >= tmpc_workspace_bytes() bytes, 256-byte aligned, caller-owned and
+ * alive until tmpc_destroy.  cuda_stream: a cudaStream_t (NULL = default stream). */
+tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, void* cuda_stream, tmpc_handle* out);
+/* a1 (eq. 36-38): linearise the built-in model at xbar [B][T][n] against stage_ref [B][T][n]
+ * (x_ref,u_ref per stage); writes qp->Am, Ap, b, G, lo, hi.  TMPC_E_UNSUPPORTED for TMPC_MODEL_NONE. */
+tmpc_status tmpc_linearize(tmpc_handle h, const void* xbar, const void* stage_ref, tmpc_qp* qp);
+/* a2+a3: assemble Theta_t, Phi_t and factor S block by block into the workspace. */
+tmpc_status tmpc_factor(tmpc_handle h, const tmpc_qp* qp);
+/* a4-a9 (Alg. 3): exactly `iters` ADMM iterations on every problem, no early exit; needs tmpc_factor first. */
+tmpc_status tmpc_admm_solve(tmpc_handle h, const tmpc_qp* qp, tmpc_state* st, int32_t iters, int32_t flags, tmpc_info* info);
+/* a10 (Alg. 2, eq. 59-65): dL/dq [B][T][n] and dL/dx_init [B][nx] from dL/dx [B][T][n] (and dL/dxi [B][T][ng] or NULL)
+ * at the state st.  REFACTOR_REFINE factors the adjoint-weighted S and runs `iters` refinement sweeps of the
+ * active-set KKT system; ADMM_REUSE_FACTOR runs `iters` ADMM iterations on the adjoint QP (eq. 67) with the
+ * forward factor.  Overwrites the factor in the workspace in REFACTOR_REFINE mode. */
+tmpc_status tmpc_backward(tmpc_handle h, const tmpc_qp* qp, const tmpc_state* st, const void* dL_dx, const void* dL_dxi,
+                          int32_t mode, int32_t iters, void* dL_dq, void* dL_dxinit);
+/* Applies the current factor: xt [B][T][n] = S^{-1} eta [B][T][n] (eq. 8).  Test/diagnostic entry. */
+tmpc_status tmpc_kkt_solve(tmpc_handle h, const void* eta, void* xt);
+/* Same as tmpc_factor + tmpc_admm_solve but every pointer in qp/st/info is HOST memory (pinned for speed); the
+ * library stages through `staging` (device, >= tmpc_host_staging_bytes()), copies results back and synchronises. */
+tmpc_status tmpc_host_staging_bytes(const tmpc_config* cfg, size_t* bytes);
+tmpc_status tmpc_admm_solve_host(tmpc_handle h, const tmpc_qp* host_qp, tmpc_state* host_st, int32_t iters, int32_t flags,
+                                 tmpc_info* host_info, void* staging, size_t staging_bytes);
+tmpc_status tmpc_destroy(tmpc_handle h);
+const char* tmpc_status_string(tmpc_status s);
+/* Number of kernels this handle has launched so far (for bench.py's gpu_launches). */
+int64_t tmpc_launch_count(tmpc_handle h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TMPC_H_ */

@@ -1,0 +1,371 @@
+// tmpc_api.cu — the C ABI of include/tmpc.h: argument checking, workspace layout, kernel-family dispatch.
+// No CPU fallback: every compute entry point needs a CUDA device and returns TMPC_E_CUDA otherwise.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include "tmpc_common.cuh"
+#include "tmpc_factor.cuh"
+#include "tmpc_admm.cuh"
+#include "tmpc_misc.cuh"
+#include "tmpc_backward.cuh"
+#include "tmpc_cr.cuh"
+
+using namespace tmpc;
+
+namespace {
+
+constexpr size_t kMaxSmem = 227 * 1024;
+inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+inline size_t esize(int dtype) { return dtype == TMPC_F64 ? 8 : 4; }
+
+struct Layout {   // byte offsets into the workspace
+  size_t Lam, Sinv, cls, soft_adj, rhs, w_rows, lo_adj, hi_adj, q_adj, ax, azg, ayf, ayg, axi, zero_xinit, zero_b, cr, total;
+};
+
+Dims make_dims(const tmpc_config& c) {
+  Dims d; memset(&d, 0, sizeof(d));
+  d.B = c.batch; d.N = c.N; d.T = c.N + 1; d.nx = c.nx; d.nu = c.nu; d.n = c.nx + c.nu; d.ng = c.ng;
+  d.nz = d.T * d.n; d.mf = c.nx + c.N * c.nx; d.mg = d.T * c.ng; d.g_sel = c.g_is_selection;
+  for (int r = 0; r < c.ng && r < TMPC_MAX_NG; ++r) { d.g_col[r] = c.g_col[r]; if (c.soft_row[r]) d.soft_mask |= 1u << r; }
+  return d;
+}
+
+Layout make_layout(const tmpc_config& c) {
+  const Dims d = make_dims(c); const size_t es = esize(c.dtype), B = d.B, nn = (size_t)d.n * d.n;
+  Layout L; size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+  L.Lam = take(B * d.N * nn * es); L.Sinv = take(B * d.T * nn * es);
+  L.cls = take(B * d.mg); L.soft_adj = take(B * d.mg);
+  L.rhs = take(B * d.nz * es); L.w_rows = take(B * d.mg * es); L.lo_adj = take(B * d.mg * es); L.hi_adj = take(B * d.mg * es);
+  L.q_adj = take(B * d.nz * es); L.ax = take(B * d.nz * es); L.azg = take(B * d.mg * es); L.ayf = take(B * d.mf * es);
+  L.ayg = take(B * d.mg * es); L.axi = take(B * d.mg * es); L.zero_xinit = take(B * d.nx * es); L.zero_b = take(B * (size_t)d.N * d.nx * es);
+  L.cr = take(cr_workspace_bytes(d, es));
+  L.total = o;
+  return L;
+}
+
+tmpc_status check_cfg(const tmpc_config* c) {
+  if (!c) return TMPC_E_BADARG;
+  if (c->batch < 1 || c->N < 1 || c->nx < 1 || c->nu < 0 || c->ng < 0) return TMPC_E_DIM;
+  if (c->ng > TMPC_MAX_NG) return TMPC_E_DIM;
+  if (c->dtype != TMPC_F32 && c->dtype != TMPC_F64) return TMPC_E_BADARG;
+  if (!(c->sigma > 0) || !(c->rho_bar > 0) || !(c->rho_eq_scale > 0) || !(c->alpha > 0 && c->alpha < 2)) return TMPC_E_BADARG;
+  if (!(c->slack_gamma >= 0) || !(c->slack_lambda >= 0)) return TMPC_E_BADARG;
+  if (c->g_is_selection) for (int r = 0; r < c->ng; ++r) if (c->g_col[r] < 0 || c->g_col[r] >= c->nx + c->nu) return TMPC_E_BADARG;
+  if (c->model == TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT && (c->nx != 4 || c->nu != 2 || c->ng != 3 || c->g_is_selection)) return TMPC_E_DIM;
+  if (c->model != TMPC_MODEL_NONE && c->model != TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT) return TMPC_E_BADARG;
+  return TMPC_OK;
+}
+
+}  // namespace
+
+struct tmpc_ctx {
+  tmpc_config cfg; Dims d; Layout lay; unsigned char* ws; cudaStream_t stream; bool factored; bool cr; int64_t launches;
+};
+
+namespace {
+
+template <typename T> QpView<T> view(const tmpc_qp* q) {
+  QpView<T> v;
+  v.D = (const T*)q->D; v.sD = q->D_bstride; v.E = (const T*)q->E; v.sE = q->E_bstride; v.q = (const T*)q->q;
+  v.Am = (const T*)q->Am; v.Ap = (const T*)q->Ap; v.b = (const T*)q->b; v.x_init = (const T*)q->x_init;
+  v.G = (const T*)q->G; v.sG = q->G_bstride; v.lo = (const T*)q->lo; v.hi = (const T*)q->hi;
+  return v;
+}
+template <typename T> Params<T> params(const tmpc_config& c) {
+  Params<T> p; p.sigma = (T)c.sigma; p.rho_g = (T)c.rho_bar; p.rho_f = (T)(c.rho_eq_scale * c.rho_bar); p.alpha = (T)c.alpha;
+  p.gamma = (T)c.slack_gamma; p.lam = (T)c.slack_lambda; return p;
+}
+inline bool cuda_ok() { return cudaGetLastError() == cudaSuccess; }
+
+bool use_cr(const tmpc_config& c) {
+  if (c.linsolve == TMPC_LIN_CYCLIC_REDUCTION) return true;
+  if (c.linsolve == TMPC_LIN_AUTO) return c.batch <= 4 && c.N >= 1024;
+  return false;
+}
+
+// ---- factor launch (a2 + a3)
+template <typename T>
+tmpc_status launch_factor(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_in, const T* w_rows, int32_t* status) {
+  FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = w_rows;
+  a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
+  const int nn = h->d.n * h->d.n;
+  int nt = ((nn + 31) / 32) * 32; if (nt > 1024) nt = 1024; if (nt < 32) nt = 32;
+  const size_t smem = 3 * (size_t)nn * sizeof(double);
+  if (smem > kMaxSmem) return TMPC_E_UNSUPPORTED;
+  auto k = factor_kernel<T, double>;
+  if (smem > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return TMPC_E_CUDA;
+  k<<<h->d.B, nt, smem, h->stream>>>(a); h->launches++;
+  return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+}
+
+// ---- ADMM launch (a4..a9); also serves tmpc_kkt_solve and the REUSE backward mode
+template <typename T, int NC, bool RES>
+tmpc_status launch_admm_inst(tmpc_ctx* h, const AdmmArgs<T>& a, int nt, size_t smem) {
+  auto k = admm_kernel<T, NC, RES>;
+  if (smem > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return TMPC_E_CUDA;
+  k<<<h->d.B, nt, smem, h->stream>>>(a); h->launches++;
+  return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+}
+template <typename T>
+tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
+  const Dims& d = h->d;
+  size_t smem_res = admm_smem_elems(d, true) * sizeof(T), smem_str = admm_smem_elems(d, false) * sizeof(T);
+  const bool res = smem_res <= kMaxSmem;
+  if (!res && smem_str > kMaxSmem) return TMPC_E_UNSUPPORTED;
+  int nt = ((d.nz + 31) / 32) * 32; if (nt > 1024) nt = 1024; if (nt < 64) nt = 64;
+  if (res) {
+    if (d.n == 6) return launch_admm_inst<T, 6, true>(h, a, nt, smem_res);
+    if (d.n == 8) return launch_admm_inst<T, 8, true>(h, a, nt, smem_res);
+    return launch_admm_inst<T, 0, true>(h, a, nt, smem_res);
+  }
+  return launch_admm_inst<T, 0, false>(h, a, nt, smem_str);
+}
+
+template <typename T>
+tmpc_status do_factor(tmpc_ctx* h, const tmpc_qp* qp) {
+  const double rho_f = h->cfg.rho_eq_scale * h->cfg.rho_bar, rho_g = h->cfg.rho_bar;
+  if (h->cr) return cr_factor<T>(h->d, view<T>(qp), h->cfg.sigma, rho_f, rho_g, h->ws + h->lay.cr, h->stream, &h->launches);
+  return launch_factor<T>(h, qp, rho_f, rho_g, nullptr, nullptr);
+}
+
+template <typename T>
+tmpc_status do_solve(tmpc_ctx* h, const tmpc_qp* qp, tmpc_state* st, int iters, int flags, tmpc_info* info) {
+  if (h->cr) {
+    return cr_admm<T>(h->d, params<T>(h->cfg), view<T>(qp), h->ws + h->lay.cr, (T*)st->x, (T*)st->zg, (T*)st->yf, (T*)st->yg, (T*)st->xi,
+                      info ? (T*)info->r_prim : nullptr, info ? (T*)info->r_dual : nullptr, info ? (T*)info->objective : nullptr,
+                      info ? info->status : nullptr, iters, (flags & TMPC_SOLVE_ZG_GIVEN) != 0, h->stream, &h->launches);
+  }
+  AdmmArgs<T> a; memset(&a, 0, sizeof(a));
+  a.d = h->d; a.prm = params<T>(h->cfg); a.qp = view<T>(qp);
+  a.Lam = (const T*)(h->ws + h->lay.Lam); a.Sinv = (const T*)(h->ws + h->lay.Sinv);
+  a.x = (T*)st->x; a.zg = (T*)st->zg; a.yf = (T*)st->yf; a.yg = (T*)st->yg; a.xi = (T*)st->xi;
+  if (info) { a.r_prim = (T*)info->r_prim; a.r_dual = (T*)info->r_dual; a.objective = (T*)info->objective; a.status = info->status; }
+  a.iters = iters; a.zg_given = (flags & TMPC_SOLVE_ZG_GIVEN) ? 1 : 0;
+  return launch_admm<T>(h, a);
+}
+
+template <typename T>
+tmpc_status kkt_solve_t(tmpc_handle h, const void* eta, void* xt) {
+  AdmmArgs<T> a; memset(&a, 0, sizeof(a));
+  a.d = h->d; a.prm = params<T>(h->cfg);
+  a.Lam = (const T*)(h->ws + h->lay.Lam); a.Sinv = (const T*)(h->ws + h->lay.Sinv);
+  a.x = (T*)eta; a.xi = (T*)xt; a.kkt_only = 1;
+  return launch_admm<T>(h, a);
+}
+}  // namespace
+
+// =================================================================================================== C ABI
+extern "C" {
+
+const char* tmpc_status_string(tmpc_status s) {
+  switch (s) {
+    case TMPC_OK: return "ok";
+    case TMPC_E_BADARG: return "bad argument";
+    case TMPC_E_DIM: return "bad dimension";
+    case TMPC_E_UNSUPPORTED: return "unsupported configuration";
+    case TMPC_E_STATE: return "call order: tmpc_factor must precede tmpc_admm_solve / tmpc_backward / tmpc_kkt_solve";
+    case TMPC_E_WORKSPACE: return "workspace missing, misaligned or too small";
+    case TMPC_E_CUDA: return "CUDA error (or no CUDA device: there is no CPU fallback)";
+  }
+  return "unknown";
+}
+
+tmpc_status tmpc_workspace_bytes(const tmpc_config* cfg, size_t* bytes) {
+  tmpc_status s = check_cfg(cfg); if (s != TMPC_OK) return s;
+  if (!bytes) return TMPC_E_BADARG;
+  *bytes = make_layout(*cfg).total;
+  return TMPC_OK;
+}
+
+tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, void* cuda_stream, tmpc_handle* out) {
+  tmpc_status s = check_cfg(cfg); if (s != TMPC_OK) return s;
+  if (!out) return TMPC_E_BADARG;
+  Layout L = make_layout(*cfg);
+  if (!workspace || ((uintptr_t)workspace & 255) || bytes < L.total) return TMPC_E_WORKSPACE;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return TMPC_E_CUDA; }
+  tmpc_ctx* h = new (std::nothrow) tmpc_ctx;
+  if (!h) return TMPC_E_BADARG;
+  h->cfg = *cfg; h->d = make_dims(*cfg); h->lay = L; h->ws = (unsigned char*)workspace; h->stream = (cudaStream_t)cuda_stream;
+  h->factored = false; h->cr = use_cr(*cfg); h->launches = 0;
+  // zero buffers of the adjoint QP (x_init = 0, b = 0)
+  if (cudaMemsetAsync(h->ws + L.zero_xinit, 0, L.zero_b - L.zero_xinit, h->stream) != cudaSuccess ||
+      cudaMemsetAsync(h->ws + L.zero_b, 0, L.cr - L.zero_b, h->stream) != cudaSuccess) { delete h; return TMPC_E_CUDA; }
+  *out = h;
+  return TMPC_OK;
+}
+
+tmpc_status tmpc_destroy(tmpc_handle h) { delete h; return TMPC_OK; }
+int64_t tmpc_launch_count(tmpc_handle h) { return h ? h->launches : 0; }
+
+tmpc_status tmpc_linearize(tmpc_handle h, const void* xbar, const void* stage_ref, tmpc_qp* qp) {
+  if (!h || !xbar || !stage_ref || !qp || !qp->Am || !qp->Ap || !qp->b || !qp->G || !qp->lo || !qp->hi) return TMPC_E_BADARG;
+  if (h->cfg.model != TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT) return TMPC_E_UNSUPPORTED;
+  if (qp->G_bstride != (int64_t)h->d.T * 3 * 6 && h->d.B > 1) return TMPC_E_BADARG;
+  const long long total = (long long)h->d.B * h->d.T; const int nt = 128; const unsigned nb = (unsigned)((total + nt - 1) / nt);
+  const tmpc_config& c = h->cfg;
+  if (c.dtype == TMPC_F32) {
+    LinArgs<float> a; a.B = h->d.B; a.N = h->d.N; a.Lwb = (float)c.wheelbase; a.dt = (float)c.dt; a.xbar = (const float*)xbar; a.ref = (const float*)stage_ref;
+    for (int k = 0; k < 3; ++k) { a.glo[k] = (float)c.g_lo[k]; a.ghi[k] = (float)c.g_hi[k]; }
+    a.Am = (float*)qp->Am; a.Ap = (float*)qp->Ap; a.b = (float*)qp->b; a.G = (float*)qp->G; a.lo = (float*)qp->lo; a.hi = (float*)qp->hi;
+    bicycle_linearize_kernel<float><<<nb, nt, 0, h->stream>>>(a);
+  } else {
+    LinArgs<double> a; a.B = h->d.B; a.N = h->d.N; a.Lwb = c.wheelbase; a.dt = c.dt; a.xbar = (const double*)xbar; a.ref = (const double*)stage_ref;
+    for (int k = 0; k < 3; ++k) { a.glo[k] = c.g_lo[k]; a.ghi[k] = c.g_hi[k]; }
+    a.Am = (double*)qp->Am; a.Ap = (double*)qp->Ap; a.b = (double*)qp->b; a.G = (double*)qp->G; a.lo = (double*)qp->lo; a.hi = (double*)qp->hi;
+    bicycle_linearize_kernel<double><<<nb, nt, 0, h->stream>>>(a);
+  }
+  h->launches++;
+  return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+}
+
+static tmpc_status check_qp(tmpc_handle h, const tmpc_qp* qp) {
+  if (!h || !qp || !qp->D || !qp->E || !qp->q || !qp->Am || !qp->Ap || !qp->b || !qp->x_init) return TMPC_E_BADARG;
+  if (h->d.ng > 0 && (!qp->lo || !qp->hi)) return TMPC_E_BADARG;
+  if (h->d.ng > 0 && !h->cfg.g_is_selection && !qp->G) return TMPC_E_BADARG;
+  return TMPC_OK;
+}
+
+tmpc_status tmpc_factor(tmpc_handle h, const tmpc_qp* qp) {
+  tmpc_status s = check_qp(h, qp); if (s != TMPC_OK) return s;
+  s = h->cfg.dtype == TMPC_F32 ? do_factor<float>(h, qp) : do_factor<double>(h, qp);
+  if (s == TMPC_OK) h->factored = true;
+  return s;
+}
+
+tmpc_status tmpc_admm_solve(tmpc_handle h, const tmpc_qp* qp, tmpc_state* st, int32_t iters, int32_t flags, tmpc_info* info) {
+  tmpc_status s = check_qp(h, qp); if (s != TMPC_OK) return s;
+  if (!st || !st->x || !st->zg || !st->yf || !st->yg || !st->xi || iters < 0) return TMPC_E_BADARG;
+  if (!h->factored) return TMPC_E_STATE;
+  return h->cfg.dtype == TMPC_F32 ? do_solve<float>(h, qp, st, iters, flags, info) : do_solve<double>(h, qp, st, iters, flags, info);
+}
+
+tmpc_status tmpc_kkt_solve(tmpc_handle h, const void* eta, void* xt) {
+  if (!h || !eta || !xt) return TMPC_E_BADARG;
+  if (!h->factored) return TMPC_E_STATE;
+  if (h->cr) return h->cfg.dtype == TMPC_F32 ? cr_kkt_solve<float>(h->d, h->ws + h->lay.cr, (const float*)eta, (float*)xt, h->stream, &h->launches)
+                                             : cr_kkt_solve<double>(h->d, h->ws + h->lay.cr, (const double*)eta, (double*)xt, h->stream, &h->launches);
+  return h->cfg.dtype == TMPC_F32 ? kkt_solve_t<float>(h, eta, xt) : kkt_solve_t<double>(h, eta, xt);
+}
+
+}  // extern "C"
+
+// =================================================================================================== backward + host entry
+namespace {
+
+template <typename T>
+tmpc_status do_backward(tmpc_ctx* h, const tmpc_qp* qp, const tmpc_state* st, const void* dLdx, const void* dLdxi, int mode, int iters, void* dq, void* dxinit) {
+  const Dims& d = h->d; const Layout& L = h->lay; unsigned char* ws = h->ws;
+  if (h->cr) return TMPC_E_UNSUPPORTED;
+  BwdArgs<T> a; memset(&a, 0, sizeof(a));
+  a.d = d; a.qp = view<T>(qp); a.x = (const T*)st->x; a.yg = (const T*)st->yg; a.xi = (const T*)st->xi;
+  a.dLdx = (const T*)dLdx; a.dLdxi = (const T*)dLdxi;
+  a.eps_abs = (T)h->cfg.eps_active_abs; a.eps_rel = (T)h->cfg.eps_active_rel; a.gamma = (T)h->cfg.slack_gamma; a.sigma = (T)h->cfg.sigma;
+  a.rho_adj = sizeof(T) == 8 ? (T)1e6 : (T)1e4;
+  a.cls = (int8_t*)(ws + L.cls); a.rhs = (T*)(ws + L.rhs);
+  a.dq = (T*)dq; a.dxinit = (T*)dxinit; a.sweeps = iters;
+  int ntp = ((d.nz + 31) / 32) * 32; if (ntp > 512) ntp = 512; if (ntp < 64) ntp = 64;
+  if (mode == TMPC_BWD_REFACTOR_REFINE) {
+    a.w_rows = (T*)(ws + L.w_rows);
+    bwd_prepare_kernel<T><<<d.B, ntp, 0, h->stream>>>(a); h->launches++;
+    if (!cuda_ok()) return TMPC_E_CUDA;
+    tmpc_status s = launch_factor<T>(h, qp, (double)a.rho_adj, 0.0, a.w_rows, nullptr);
+    h->factored = false;                       // the forward factor has been overwritten
+    if (s != TMPC_OK) return s;
+    a.Lam = (const T*)(ws + L.Lam); a.Sinv = (const T*)(ws + L.Sinv);
+    const size_t smem = (3 * (size_t)d.nz + 2 * (size_t)d.mf + 2 * (size_t)d.mg) * sizeof(T);
+    if (smem > kMaxSmem) return TMPC_E_UNSUPPORTED;
+    int nt = ((d.nz + 31) / 32) * 32; if (nt > 1024) nt = 1024; if (nt < 64) nt = 64;
+    auto launch = [&](auto k) -> tmpc_status {
+      if (smem > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return TMPC_E_CUDA;
+      k<<<d.B, nt, smem, h->stream>>>(a); h->launches++;
+      return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+    };
+    if (d.n == 6) return launch(bwd_refine_kernel<T, 6>);
+    if (d.n == 8) return launch(bwd_refine_kernel<T, 8>);
+    return launch(bwd_refine_kernel<T, 0>);
+  }
+  // ---- ADMM on the adjoint QP (eq. 67) with the forward factor
+  if (!h->factored) return TMPC_E_STATE;
+  a.lo_adj = (T*)(ws + L.lo_adj); a.hi_adj = (T*)(ws + L.hi_adj); a.soft_adj = (int8_t*)(ws + L.soft_adj); a.q_adj = (T*)(ws + L.q_adj);
+  bwd_prepare_kernel<T><<<d.B, ntp, 0, h->stream>>>(a); h->launches++;
+  if (!cuda_ok()) return TMPC_E_CUDA;
+  if (cudaMemsetAsync(ws + L.ax, 0, L.zero_xinit - L.ax, h->stream) != cudaSuccess) return TMPC_E_CUDA;
+  AdmmArgs<T> s; memset(&s, 0, sizeof(s));
+  s.d = d; s.prm = params<T>(h->cfg); s.prm.lam = T(0); s.qp = view<T>(qp);
+  s.qp.q = a.q_adj; s.qp.b = (const T*)(ws + L.zero_b); s.qp.x_init = (const T*)(ws + L.zero_xinit); s.qp.lo = a.lo_adj; s.qp.hi = a.hi_adj;
+  s.Lam = (const T*)(ws + L.Lam); s.Sinv = (const T*)(ws + L.Sinv);
+  s.x = (T*)(ws + L.ax); s.zg = (T*)(ws + L.azg); s.yf = (T*)(ws + L.ayf); s.yg = (T*)(ws + L.ayg); s.xi = (T*)(ws + L.axi);
+  s.iters = iters; s.soft_rows = a.soft_adj;
+  tmpc_status rc = launch_admm<T>(h, s);
+  if (rc != TMPC_OK) return rc;
+  const long long tot = (long long)d.B * d.nz;
+  bwd_reuse_finish_kernel<T><<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(d.B, d.nz, d.nx, d.mf, s.x, s.yf, (T*)dq, (T*)dxinit); h->launches++;
+  return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+}
+
+struct HostPlan { size_t off[20]; size_t bytes[20]; size_t total; };
+// order: D E q Am Ap b x_init G lo hi | x zg yf yg xi | r_prim r_dual objective status
+HostPlan host_plan(const tmpc_config& c, int64_t sD, int64_t sE, int64_t sG, bool haveG) {
+  const Dims d = make_dims(c); const size_t es = esize(c.dtype), B = d.B, nn = (size_t)d.n * d.n;
+  HostPlan P; memset(&P, 0, sizeof(P));
+  size_t sz[20] = { (sD ? B : 1) * d.T * nn * es, (sE ? B : 1) * d.N * nn * es, B * d.nz * es, B * d.N * d.nx * d.n * es, B * d.N * d.nx * d.n * es,
+                    B * d.N * d.nx * es, B * d.nx * es, haveG ? (sG ? B : 1) * (size_t)d.T * d.ng * d.n * es : 0, B * d.mg * es, B * d.mg * es,
+                    B * d.nz * es, B * d.mg * es, B * d.mf * es, B * d.mg * es, B * d.mg * es, B * es, B * es, B * es, B * 4, 0 };
+  size_t o = 0;
+  for (int i = 0; i < 20; ++i) { P.off[i] = o; P.bytes[i] = sz[i]; o = align_up(o + sz[i]); }
+  P.total = o;
+  return P;
+}
+
+}  // namespace
+
+extern "C" {
+
+tmpc_status tmpc_backward(tmpc_handle h, const tmpc_qp* qp, const tmpc_state* st, const void* dL_dx, const void* dL_dxi,
+                          int32_t mode, int32_t iters, void* dL_dq, void* dL_dxinit) {
+  tmpc_status s = check_qp(h, qp); if (s != TMPC_OK) return s;
+  if (!st || !st->x || !st->yg || !st->xi || !dL_dx || !dL_dq || !dL_dxinit || iters < 0) return TMPC_E_BADARG;
+  if (mode != TMPC_BWD_REFACTOR_REFINE && mode != TMPC_BWD_ADMM_REUSE_FACTOR) return TMPC_E_BADARG;
+  return h->cfg.dtype == TMPC_F32 ? do_backward<float>(h, qp, st, dL_dx, dL_dxi, mode, iters, dL_dq, dL_dxinit)
+                                  : do_backward<double>(h, qp, st, dL_dx, dL_dxi, mode, iters, dL_dq, dL_dxinit);
+}
+
+tmpc_status tmpc_host_staging_bytes(const tmpc_config* cfg, size_t* bytes) {
+  tmpc_status s = check_cfg(cfg); if (s != TMPC_OK) return s;
+  if (!bytes) return TMPC_E_BADARG;
+  *bytes = host_plan(*cfg, 1, 1, 1, true).total;   // upper bound: nothing shared
+  return TMPC_OK;
+}
+
+tmpc_status tmpc_admm_solve_host(tmpc_handle h, const tmpc_qp* hq, tmpc_state* hs, int32_t iters, int32_t flags, tmpc_info* hi_, void* staging, size_t staging_bytes) {
+  tmpc_status s = check_qp(h, hq); if (s != TMPC_OK) return s;
+  if (!hs || !hs->x || !hs->zg || !hs->yf || !hs->yg || !hs->xi || !staging || iters < 0) return TMPC_E_BADARG;
+  const HostPlan P = host_plan(h->cfg, hq->D_bstride, hq->E_bstride, hq->G_bstride, hq->G != nullptr);
+  if (staging_bytes < P.total || ((uintptr_t)staging & 255)) return TMPC_E_WORKSPACE;
+  unsigned char* dv = (unsigned char*)staging;
+  const void* src[15] = { hq->D, hq->E, hq->q, hq->Am, hq->Ap, hq->b, hq->x_init, hq->G, hq->lo, hq->hi, hs->x, hs->zg, hs->yf, hs->yg, hs->xi };
+  for (int i = 0; i < 15; ++i) {
+    if (!src[i] || !P.bytes[i]) continue;
+    if ((i == 11 || i == 14) && !(flags & TMPC_SOLVE_ZG_GIVEN)) continue;      // zg, xi are outputs only
+    if (cudaMemcpyAsync(dv + P.off[i], src[i], P.bytes[i], cudaMemcpyHostToDevice, h->stream) != cudaSuccess) return TMPC_E_CUDA;
+  }
+  tmpc_qp dq = *hq;
+  dq.D = dv + P.off[0]; dq.E = dv + P.off[1]; dq.q = dv + P.off[2]; dq.Am = dv + P.off[3]; dq.Ap = dv + P.off[4]; dq.b = dv + P.off[5];
+  dq.x_init = dv + P.off[6]; dq.G = hq->G ? dv + P.off[7] : nullptr; dq.lo = dv + P.off[8]; dq.hi = dv + P.off[9];
+  tmpc_state ds = { dv + P.off[10], dv + P.off[11], dv + P.off[12], dv + P.off[13], dv + P.off[14] };
+  tmpc_info di = { dv + P.off[15], dv + P.off[16], dv + P.off[17], (int32_t*)(dv + P.off[18]) };
+  if (cudaMemsetAsync(di.status, 0, P.bytes[18], h->stream) != cudaSuccess) return TMPC_E_CUDA;
+  s = tmpc_factor(h, &dq); if (s != TMPC_OK) return s;
+  s = tmpc_admm_solve(h, &dq, &ds, iters, flags, &di); if (s != TMPC_OK) return s;
+  void* dst[5] = { hs->x, hs->zg, hs->yf, hs->yg, hs->xi };
+  for (int i = 0; i < 5; ++i) if (cudaMemcpyAsync(dst[i], dv + P.off[10 + i], P.bytes[10 + i], cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) return TMPC_E_CUDA;
+  if (hi_) {
+    void* idst[4] = { hi_->r_prim, hi_->r_dual, hi_->objective, hi_->status };
+    for (int i = 0; i < 4; ++i) if (idst[i] && cudaMemcpyAsync(idst[i], dv + P.off[15 + i], P.bytes[15 + i], cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) return TMPC_E_CUDA;
+  }
+  return cudaStreamSynchronize(h->stream) == cudaSuccess ? TMPC_OK : TMPC_E_CUDA;
+}
+
+}  // extern "C"
