@@ -113,3 +113,95 @@ def test_kkt_solve_matches_oracle_cholesky(dtype):
         ref = np.stack([O.solve_S(wr, cfg, eta[b].ravel(), b).reshape(w.T, w.n) for b in range(w.B)])
         assert rel_err(xt, ref) <= (1e-10 if dtype == "f64" else 2e-3)
         s.close()
+
+
+# ----------------------------------------------------------------------------------------------- a10 backward
+def _backward_case(dtype, soft_bound, rho_bar, iters, B=6, N=20):
+    """Oracle forward output is fed to BOTH sides (reading A-20) so the classification cannot diverge by rounding."""
+    import torch
+    from paper_2606_24039_b200.solver import Solver
+    w = W.config2(B=B, N=N, soft_bound=soft_bound)
+    w.rho_bar = rho_bar
+    if soft_bound < 1.0:
+        w.lam = 0.05       # lambda = 100 makes the stress instance degenerate (more rows at their bound than free directions)
+    w.q = w.q + 0.3 * np.random.default_rng(5).standard_normal(w.q.shape)
+    wr = w.rounded(np.float32) if dtype == "f32" else w
+    eps = 1e-8 if dtype == "f64" else 1e-4
+    cfg = O.make_cfg(wr, eps_abs=eps, eps_rel=eps)
+    ref, info, rc = O.admm(wr, cfg, iters=iters)
+    if dtype == "f32":
+        ref = {k: v.astype(np.float32).astype(np.float64) for k, v in ref.items()}
+    dq_o, dxi_o, counts, rcs = O.backward(wr, cfg, ref, 2.0 * ref["x"])
+    ok = rcs == 0                      # degenerate active sets are skipped (reading A-18)
+    assert ok.sum() >= (w.B + 1) // 2
+    s = Solver(wr, dtype=dtype)
+    s.set_state(ref)
+    return w, s, ref, dq_o, dxi_o, counts, ok
+
+
+@pytest.mark.parametrize("dtype,soft_bound", [("f64", 2.0), ("f64", 0.3), ("f32", 2.0), ("f32", 0.3)])
+def test_backward_refine_matches_oracle_definition(dtype, soft_bound):
+    from paper_2606_24039_b200 import binding as Bd
+    w, s, ref, dq_o, dxi_o, counts, ok = _backward_case(dtype, soft_bound, 2.0, 3000)
+    assert counts.sum() > 0
+    dq, dxi = s.backward(2.0 * s.s["x"], mode=Bd.TMPC_BWD_REFACTOR_REFINE)
+    tol = 1e-9 if dtype == "f64" else 2e-3
+    assert rel_err(dq.cpu().double().numpy()[ok], dq_o[ok]) <= tol
+    assert rel_err(dxi.cpu().double().numpy()[ok], dxi_o[ok]) <= tol
+    s.close()
+
+
+def test_backward_admm_reuse_factor_converges_to_definition():
+    """eq. 67 mode: biased by its tolerance -> loose check after many iterations."""
+    from paper_2606_24039_b200 import binding as Bd
+    w, s, ref, dq_o, dxi_o, counts, ok = _backward_case("f64", 0.3, 2.0, 3000)
+    s.factor()
+    dq, dxi = s.backward(2.0 * s.s["x"], mode=Bd.TMPC_BWD_ADMM_REUSE_FACTOR, iters=4000)
+    assert rel_err(dq.cpu().double().numpy()[ok], dq_o[ok]) <= 1e-5
+    assert rel_err(dxi.cpu().double().numpy()[ok], dxi_o[ok]) <= 1e-5
+    s.close()
+
+
+# ----------------------------------------------------------------------------------------------- a1 + SQP (config 4)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_linearize_matches_oracle(dtype):
+    from paper_2606_24039_b200.solver import Solver
+    w = W.config4(B=5, N=37, dtype=dtype)
+    wr = w.rounded(np.float32) if dtype == "f32" else w
+    s = Solver(wr, dtype=dtype)
+    s.reset_state(wr.xbar0)
+    s.linearize()
+    cfg = O.make_cfg(wr)
+    tol = 1e-12 if dtype == "f64" else 2e-5
+    for b in range(w.B):
+        ref = O.bicycle_linearize(wr, cfg, wr.xbar0[b], b)
+        for name, r in zip(("Am", "Ap", "b", "G", "lo", "hi"), ref):
+            g = s.t[name][b].cpu().double().numpy()
+            assert np.abs(g - r).max() <= tol * max(1.0, np.abs(r).max()), name
+    s.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config4_sqp_subset(dtype):
+    from paper_2606_24039_b200.solver import Solver
+    w = W.config4(B=12, dtype=dtype)
+    wr = w.rounded(np.float32) if dtype == "f32" else w
+    s = Solver(wr, dtype=dtype)
+    s.reset_state(wr.xbar0)
+    s.sqp()
+    got = s.state_numpy()
+    ref, info, rc = O.sqp_bicycle(wr, O.make_cfg(wr), nthreads=8)
+    assert rc == 0
+    compare_states(got, ref, TOL[dtype])
+    s.close()
+
+
+# ----------------------------------------------------------------------------------------------- config 3 (streamed class)
+def test_config3_subset_fp32():
+    w = W.config3(B=3, N=6)
+    run_pair(w, "f32", iters=40, band=1)
+
+
+def test_config3_shape_fp64():
+    w = W.config3(B=2, N=4)
+    run_pair(w, "f64", iters=25, band=1)
