@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the batched ADMM-QP hot path on B200 (BASELINE.json metric).
+
+  python bench.py --gpus N --steps K --warmup W [--config 2] [--dtype f32] [--impl reference]
+
+A step = one pass of the hot path over one batch of synthetic QPs: configs 1-3: tmpc_factor + tmpc_admm_solve
+(fixed iteration count); configs 4-5: n_sqp x (tmpc_linearize + tmpc_factor + tmpc_admm_solve).  Default workload
+(N=1): BASELINE.json configs[1] = random LTV QP batch, B=1024, N=50, nx=6, nu=2, rate cost + slack, fp32,
+100 ADMM iterations; its backward pass is timed separately and reported as `backward_ms`.
+value = QP solves per second over all ranks (each rank solves its own batch: weak scaling, no collective on the
+data path; NCCL only carries the barrier and the max-over-ranks reduction of the timings).
+`--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+# algorithmic flops per problem per ADMM iteration (a4-a8, selection-type G, compact C) — SURVEY.md 8(a)/(d), DESIGN.md 6
+FLOPS_PER_ITER = {1: 7.6e3, 2: 36.1e3, 3: 2.75e6, 4: 37.7e3, 5: 3.1e6}
+# algorithmic HBM bytes per problem per ADMM iteration for the streamed class (config 3) — SURVEY.md 8(d)
+BYTES_PER_ITER = {3: 4.33e6}
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 FMA lanes x 2 flop x 1965 MHz
+FP64_PEAK_TFLOPS = FP32_PEAK_TFLOPS / 2               # 64 FP64 FMA lanes per SM
+
+
+def make_workload(cfg_id, dtype, batch=None):
+    from paper_2606_24039_b200 import workloads as W
+    if cfg_id == 1:
+        w = W.config1()
+    elif cfg_id == 2:
+        w = W.config2(dtype=dtype, **({"B": batch} if batch else {}))
+    elif cfg_id == 3:
+        w = W.config3(**({"B": batch} if batch else {}))
+    elif cfg_id == 4:
+        w = W.config4(dtype=dtype, **({"B": batch} if batch else {}))
+    elif cfg_id == 5:
+        w = W.config5(dtype=dtype)
+    else:
+        raise SystemExit("config must be 1..5")
+    return w.rounded(np.float32) if dtype == "f32" else w
+
+
+def workload_name(w, dtype):
+    s = f"{w.name}: B={w.B} N={w.N} nx={w.nx} nu={w.nu} ng={w.ng} {dtype} iters={w.iters}"
+    return s + (f" sqp={w.sqp_iters}" if w.sqp_iters else "")
+
+
+def total_iters(w):
+    return w.iters * max(1, w.sqp_iters)
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        self.stop_flag = True
+        self.join(timeout=6)
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        sm = sorted(float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit())
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[2 + i].lower().startswith("active") for r in self.rows if len(r) > 2 + i)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": float(self.rows[0][1]) if self.rows[0][1].replace(".", "").isdigit() else None,
+                "reasons": reasons, "samples": len(self.rows)}
+
+
+def oracle_rate(w, cfg_id, nthreads, budget_problems):
+    """Times the oracle as it stands on a bounded sample; returns (solves/s, sample description, seconds)."""
+    import oracle as O
+    nb = min(w.B, budget_problems)
+    ws = w.subset(np.arange(nb)) if nb < w.B else w
+    cfg = O.make_cfg(ws)
+    t0 = time.perf_counter()
+    if w.model:
+        O.sqp_bicycle(ws, cfg, nthreads=nthreads)
+    else:
+        O.admm(ws, cfg, nthreads=nthreads)
+    dt = time.perf_counter() - t0
+    return nb / dt, f"first {nb} of {w.B} problems, {total_iters(w)} ADMM iterations each, {nthreads} threads (one problem per thread)", dt
+
+
+def oracle_sample_size(cfg_id):
+    return {1: 1, 2: 256, 3: 16, 4: 256, 5: 1}[cfg_id]
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = make_workload(args.config, args.dtype, args.batch)
+    cores = len(os.sched_getaffinity(0))
+    nb = oracle_sample_size(args.config)
+    for _ in range(args.warmup):
+        oracle_rate(w, args.config, cores, nb)
+    t, desc = 0.0, ""
+    for _ in range(args.steps):
+        r, desc, dt = oracle_rate(w, args.config, cores, nb)
+        t += dt
+    rate = min(w.B, nb) * args.steps / t
+    line = {"impl": "reference", "metric": "batched QP solves/s", "value": rate, "unit": "QP solves/s", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": workload_name(w, args.dtype)},
+            "cpu_baseline": {"value": rate, "unit": "QP solves/s", "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": rate, "unit": "QP solves/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_24039_b200 import binding as Bd
+    from paper_2606_24039_b200.solver import Solver
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = torch.device(f"cuda:{local}")
+    w = make_workload(args.config, args.dtype, args.batch)
+    linsolve = Bd.TMPC_LIN_CYCLIC_REDUCTION if args.config == 5 else Bd.TMPC_LIN_SEQUENTIAL
+    s = Solver(w, dtype=args.dtype, device=dev, linsolve=linsolve)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    x0 = s._up(w.xbar0) if w.model else None
+
+    def reset():
+        for k, v in s.s.items():
+            if k == "x" and x0 is not None:
+                v.copy_(x0)
+            else:
+                v.zero_()
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    solve_ms = []
+
+    def step(timed):
+        """one pass of the hot path; returns (start, end, [(a,b) events around each tmpc_admm_solve])."""
+        a, b, inner = ev(), ev(), []
+        a.record()
+        for _ in range(max(1, w.sqp_iters)):
+            if w.model:
+                s.linearize()
+            s.factor()
+            c, d = ev(), ev()
+            c.record(); s.admm_solve(); d.record()
+            inner.append((c, d))
+        b.record()
+        return a, b, inner
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(max(3, args.warmup)):
+        reset(); step(False)
+    barrier()
+    sampler = ClockSampler(local); sampler.start()
+    l0 = s.launches()
+    recs = []
+    for _ in range(args.steps):
+        reset(); flush.zero_()
+        recs.append(step(True))
+    barrier()
+    launches = s.launches() - l0
+    clocks = sampler.summary()
+    step_ms = [a.elapsed_time(b) for a, b, _ in recs]
+    kern_ms = [sum(c.elapsed_time(d) for c, d in inner) for _, _, inner in recs]
+    n_admm_launch = sum(len(inner) for _, _, inner in recs)
+    tot = torch.tensor([sum(step_ms)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tot, op=dist.ReduceOp.MAX)
+    total_ms = float(tot.item())
+    info = s.info_numpy()
+
+    # ---- backward (config 2), separately
+    backward_ms = None
+    if args.config == 2:
+        dLdx = 2.0 * s.s["x"]
+        ts = []
+        for _ in range(3 + args.steps):
+            s.factor(); flush.zero_()
+            a, b = ev(), ev(); a.record(); s.backward(dLdx); b.record(); torch.cuda.synchronize(dev); ts.append(a.elapsed_time(b))
+        backward_ms = float(np.median(ts[3:]))
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not w.model and args.config != 5:
+        hp = lambda t: t.detach().cpu().pin_memory()
+        ht = {k: (hp(v) if v is not None else None) for k, v in s.t.items()}
+        hs = {k: hp(torch.zeros_like(v)) for k, v in s.s.items()}
+        hi = {k: hp(v) for k, v in s.info.items()}
+        hq = s.make_qp(ht)
+        hst = Bd.TmpcState(*[hs[k].data_ptr() for k in ("x", "zg", "yf", "yg", "xi")])
+        hin = Bd.TmpcInfo(hi["r_prim"].data_ptr(), hi["r_dual"].data_ptr(), hi["objective"].data_ptr(), hi["status"].data_ptr())
+        nst = Bd.tmpc_host_staging_bytes(s.cfg)
+        staging = torch.empty(nst + 256, dtype=torch.uint8, device=dev)
+        sp = (staging.data_ptr() + 255) // 256 * 256
+        h2d = sum(v.numel() * v.element_size() for v in ht.values() if v is not None) + sum(hs[k].numel() * hs[k].element_size() for k in ("x", "yf", "yg"))
+        d2h = sum(v.numel() * v.element_size() for v in hs.values()) + sum(v.numel() * v.element_size() for v in hi.values())
+        ts = []
+        for i in range(3 + args.steps):
+            for v in hs.values():
+                v.zero_()
+            torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            Bd.tmpc_admm_solve_host(s.h, hq, hst, w.iters, 0, hin, sp, nst)
+            ts.append(time.perf_counter() - t0)
+        t_e2e = torch.tensor([sum(ts[3:])], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
+        e2e = {"value": w.B * world * args.steps / float(t_e2e.item()), "unit": "QP solves/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "ms_per_step": 1e3 * float(t_e2e.item()) / args.steps}
+        assert np.abs(hs["x"].double().numpy() - s.state_numpy()["x"]).max() < 1e-3, "host path disagrees with device path"
+    else:
+        # model configs: the same public calls with pinned host inputs copied in and the result copied out every step
+        hx0 = x0.cpu().pin_memory(); href = s.t["stage_ref"].cpu().pin_memory(); hq_ = s.t["q"].cpu().pin_memory(); hxi = s.t["x_init"].cpu().pin_memory()
+        hout = torch.empty_like(hx0).pin_memory()
+        ts = []
+        for i in range(2 + args.steps):
+            reset(); torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            s.s["x"].copy_(hx0, non_blocking=True); s.t["stage_ref"].copy_(href, non_blocking=True)
+            s.t["q"].copy_(hq_, non_blocking=True); s.t["x_init"].copy_(hxi, non_blocking=True)
+            step(False)
+            hout.copy_(s.s["x"], non_blocking=True); torch.cuda.synchronize(dev)
+            ts.append(time.perf_counter() - t0)
+        t_e2e = torch.tensor([sum(ts[2:])], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
+        nb = lambda t: t.numel() * t.element_size()
+        e2e = {"value": w.B * world * args.steps / float(t_e2e.item()), "unit": "QP solves/s", "h2d_bytes_per_step": int(nb(hx0) + nb(href) + nb(hq_) + nb(hxi)),
+               "d2h_bytes_per_step": int(nb(hout)), "ms_per_step": 1e3 * float(t_e2e.item()) / args.steps}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    ms_per_step = total_ms / args.steps
+    value = w.B * world / (ms_per_step * 1e-3)
+    iters = total_iters(w)
+    kern_avg_ms = sum(kern_ms) / max(1, n_admm_launch)
+    if args.config == 3:
+        alg = BYTES_PER_ITER[3] * w.B * w.iters
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else None
+        peak = peaks["hbm_gbs"] if peaks else 6650.0
+        roof = {"bound": "hbm", "achieved": alg / (kern_avg_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s", "peak_source": "measured" if peaks else "fallback"}
+    else:
+        alg = FLOPS_PER_ITER[args.config] * w.B * w.iters
+        peak = FP64_PEAK_TFLOPS if args.dtype == "f64" else FP32_PEAK_TFLOPS
+        roof = {"bound": "alu", "achieved": alg / (kern_avg_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s", "peak_source": "derived: 148 SMs x 128 (fp32) / 64 (fp64) FMA lanes x 2 x 1965 MHz"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"] = None
+    roof["kernel"] = "admm_kernel (tmpc_admm_solve)" if args.config != 5 else "cr_admm_kernel (tmpc_admm_solve)"
+    roof["kernel_ms_per_launch"] = kern_avg_ms
+    roof["kernel_share_of_step"] = sum(kern_ms) / sum(step_ms)
+    line = {"metric": "batched QP solves/s", "value": value, "unit": "QP solves/s", "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+            "config": {"workload": workload_name(w, args.dtype), "l2": "256 MB flush write between timed steps", "step": "tmpc_factor + tmpc_admm_solve" if not w.model else "n_sqp x (tmpc_linearize + tmpc_factor + tmpc_admm_solve)"},
+            "admm_iters_per_s": value * iters, "ms_per_batched_solve": ms_per_step, "us_per_admm_iteration": 1e3 * ms_per_step / iters,
+            "backward_ms": backward_ms, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "roofline": roof,
+            "parity_snapshot": {"max_r_prim": float(np.max(info["r_prim"])), "max_r_dual": float(np.max(info["r_dual"])), "status_nonzero": int((info["status"] != 0).sum())}}
+    if world == 1 and not args.no_cpu_baseline:
+        cores = len(os.sched_getaffinity(0))
+        r, desc, dt = oracle_rate(w, args.config, cores, oracle_sample_size(args.config))
+        line["cpu_baseline"] = {"value": r, "unit": "QP solves/s", "cores": cores, "kind": "oracle", "sample": desc, "seconds": dt}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="tmpc", choices=["tmpc", "reference"])
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--dtype", default=None, choices=[None, "f32", "f64"])
+    ap.add_argument("--batch", type=int, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.dtype is None:
+        args.dtype = {1: "f64", 2: "f32", 3: "f32", 4: "f32", 5: "f64"}[args.config]
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()
