@@ -1,22 +1,432 @@
-// tmpc_cr.cuh — a11: parallel-in-time (block cyclic reduction) factor and solve for one long horizon (config 5).
+// tmpc_cr.cuh — a11: parallel-in-time factor and solve of the block-tridiagonal S by block cyclic reduction
+// (odd-even elimination; textbook, cited as prior art at PAPER.md:86) for a single long horizon (config 5).
+//
+// Level l (h = 2^l) eliminates the stages j = h(2k+1) < T; survivors are the multiples of 2h.  With Lo_j the
+// current block (j, j-h) and a = j-h, b = j+h the neighbours of an eliminated stage j:
+//     U_j = Theta_j^{-1},   FA_j = Lo_j' U_j,   FB_j = Lo_b U_j                      (stored for the solves)
+//     Theta_a -= FA_j Lo_j,   Theta_b -= FB_j Lo_b',   Lo_b(new, couples b and a) = -FB_j Lo_j
+//     down-sweep  eta_a -= FA_j eta_j,  eta_b -= FB_j eta_j ;  root x_0 = U_0 eta_0
+//     up-sweep    x_j = U_j eta_j - FA_j' x_a - FB_j' x_b.
+// Every Theta met is a Schur complement of the SPD matrix S, hence SPD: each pivot block is inverted through its
+// Cholesky factor.  ceil(log2 T) levels; T need not be a power of two (out-of-range neighbours simply vanish).
+// All updates are written in GATHER form (each survivor pulls from its two eliminated neighbours) so that there are
+// no write conflicts and the result is deterministic.
+//
+// v1 layout: everything in global memory (L2-resident: 5 T n^2 elements), one cooperative grid, grid-wide barrier
+// between levels.  The fused ADMM loop (Alg. 3) runs entirely inside cr_admm_kernel.
 #pragma once
+#include <cooperative_groups.h>
 #include "tmpc_common.cuh"
 
 namespace tmpc {
+namespace cg = cooperative_groups;
 
-inline size_t cr_workspace_bytes(const Dims& d, size_t es) { (void)d; (void)es; return 0; }
+template <typename T>
+struct CrBuf {         // per problem, carved from the workspace
+  T* Th; T* Lo; T* U; T* FA; T* FB;    // [T][n][n]
+  T* eta; T* xt;                       // [T][n]
+  T* rv; T* sv;                        // [mf], [mg]
+  T* part;                             // [3 * max CTAs] reduction partials
+  int32_t* flag;
+};
+
+inline size_t cr_workspace_bytes(const Dims& d, size_t es) {
+  const size_t nn = (size_t)d.n * d.n;
+  size_t per = 5 * (size_t)d.T * nn + 2 * (size_t)d.nz + d.mf + d.mg + 3 * 4096;
+  return (size_t)d.B * per * es + 256 * (size_t)d.B + 1024;
+}
+template <typename T>
+__host__ __device__ inline CrBuf<T> cr_carve(const Dims& d, unsigned char* ws, int p) {
+  const size_t nn = (size_t)d.n * d.n;
+  const size_t per = 5 * (size_t)d.T * nn + 2 * (size_t)d.nz + d.mf + d.mg + 3 * 4096;
+  T* base = reinterpret_cast<T*>(ws) + (size_t)p * per;
+  CrBuf<T> b;
+  b.Th = base; b.Lo = b.Th + d.T * nn; b.U = b.Lo + d.T * nn; b.FA = b.U + d.T * nn; b.FB = b.FA + d.T * nn;
+  b.eta = b.FB + d.T * nn; b.xt = b.eta + d.nz; b.rv = b.xt + d.nz; b.sv = b.rv + d.mf; b.part = b.sv + d.mg;
+  b.flag = reinterpret_cast<int32_t*>(ws + (size_t)d.B * per * sizeof(T)) + 64 * p;
+  return b;
+}
+__host__ __device__ inline int cr_levels(int T_) { int L = 0; while ((1 << L) < T_) ++L; return L; }
+
+// inverse of an SPD NC x NC block through its Cholesky factor, in registers/local memory.  Returns 1 on a bad pivot.
+template <typename T, int NC>
+__device__ int spd_inverse(const T* __restrict__ A, T* __restrict__ X) {
+  T L[NC * NC]; int bad = 0;
+#pragma unroll
+  for (int i = 0; i < NC * NC; ++i) L[i] = A[i];
+#pragma unroll
+  for (int k = 0; k < NC; ++k) {
+    T dk = L[k * NC + k];
+    if (!(dk > T(0)) || !isfinite(dk)) { bad = 1; dk = T(1); }
+    const T sq = sqrt(dk), inv = T(1) / sq;
+    L[k * NC + k] = sq;
+#pragma unroll
+    for (int i = k + 1; i < NC; ++i) L[i * NC + k] *= inv;
+#pragma unroll
+    for (int j = k + 1; j < NC; ++j)
+#pragma unroll
+      for (int i = j; i < NC; ++i) L[i * NC + j] -= L[i * NC + k] * L[j * NC + k];
+  }
+  T Y[NC * NC];    // Y = L^{-1} (lower)
+#pragma unroll
+  for (int j = 0; j < NC; ++j) {
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+      if (i < j) { Y[i * NC + j] = T(0); continue; }
+      T s = (i == j) ? T(1) : T(0);
+#pragma unroll
+      for (int k = 0; k < NC; ++k) if (k >= j && k < i) s -= L[i * NC + k] * Y[k * NC + j];
+      Y[i * NC + j] = s / L[i * NC + i];
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < NC; ++i)
+#pragma unroll
+    for (int j = 0; j < NC; ++j) {
+      T s = T(0);
+#pragma unroll
+      for (int k = 0; k < NC; ++k) if (k >= i && k >= j) s += Y[k * NC + i] * Y[k * NC + j];
+      X[i * NC + j] = s;
+    }
+  return bad;
+}
+
+template <typename T>
+struct CrFactorArgs { Dims d; QpView<T> qp; T sigma, rho_f, rho_g; unsigned char* ws; };
+
+// ---- factor: assemble Theta_t, Lo_t = Phi_{t-1}, then ceil(log2 T) elimination levels
+template <typename T, int NC>
+__global__ void __launch_bounds__(256) cr_factor_kernel(CrFactorArgs<T> a) {
+  cg::grid_group grid = cg::this_grid();
+  const Dims& d = a.d;
+  constexpr int n = NC, nn = NC * NC;
+  const int nx = d.nx, ng = d.ng, N = d.N, T_ = d.T, p = blockIdx.y;
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x, gsz = (long long)gridDim.x * blockDim.x;
+  CrBuf<T> b = cr_carve<T>(d, a.ws, p);
+  const T* Dp = a.qp.D + a.qp.sD * p; const T* Ep = a.qp.E + a.qp.sE * p;
+  const T* Amp = a.qp.Am + (size_t)p * N * nx * n; const T* App = a.qp.Ap + (size_t)p * N * nx * n;
+  const T* Gp = a.qp.G ? a.qp.G + a.qp.sG * p : nullptr;
+  for (long long e = gid; e < (long long)T_ * nn; e += gsz) {
+    const int t = (int)(e / nn), r_ = (int)(e - (long long)t * nn), i = r_ / n, j = r_ - i * n;
+    const T* Amt = Amp + (size_t)t * nx * n; const T* Apm = App + (size_t)(t - 1) * nx * n;
+    T s = Dp[(size_t)t * nn + r_];
+    if (i == j) s += a.sigma;
+    T acc = T(0);
+    if (t < N) for (int r = 0; r < nx; ++r) acc += Amt[r * n + i] * Amt[r * n + j];
+    if (t > 0) for (int r = 0; r < nx; ++r) acc += Apm[r * n + i] * Apm[r * n + j];
+    if (t == 0 && i == j && i < nx) acc += T(1);
+    s += a.rho_f * acc;
+    if (d.g_sel) { for (int r = 0; r < ng; ++r) if (d.g_col[r] == i && i == j) s += a.rho_g; }
+    else { const T* Gt = Gp + (size_t)t * ng * n; for (int r = 0; r < ng; ++r) s += a.rho_g * Gt[r * n + i] * Gt[r * n + j]; }
+    b.Th[e] = s;
+    T lo = T(0);
+    if (t > 0) {   // Lo_t = Phi_{t-1} = E_{t-1} + rho_f A^+_{t-1}' A^-_{t-1}
+      const T* Amm = Amp + (size_t)(t - 1) * nx * n;
+      T c = T(0);
+      for (int r = 0; r < nx; ++r) c += Apm[r * n + i] * Amm[r * n + j];
+      lo = Ep[(size_t)(t - 1) * nn + r_] + a.rho_f * c;
+    }
+    b.Lo[e] = lo;
+  }
+  if (gid == 0) *b.flag = 0;
+  grid.sync();
+  const int L = cr_levels(T_);
+  for (int l = 0; l < L; ++l) {
+    const int h = 1 << l;
+    // (1) eliminated stages j = h(2k+1): U_j, FA_j, FB_j
+    for (long long k = gid;; k += gsz) {
+      const long long j = (long long)h * (2 * k + 1);
+      if (j >= T_) break;
+      T U[nn];
+      if (spd_inverse<T, NC>(b.Th + j * nn, U)) atomicOr(b.flag, 1);
+      const T* Loj = b.Lo + j * nn;
+      T* FA = b.FA + j * nn; T* FB = b.FB + j * nn; T* Uo = b.U + j * nn;
+#pragma unroll
+      for (int e = 0; e < nn; ++e) Uo[e] = U[e];
+#pragma unroll
+      for (int i = 0; i < n; ++i)
+#pragma unroll
+        for (int c = 0; c < n; ++c) { T s = T(0);
+#pragma unroll
+          for (int m = 0; m < n; ++m) s += Loj[m * n + i] * U[m * n + c];
+          FA[i * n + c] = s; }
+      if (j + h < T_) {
+        const T* Lob = b.Lo + (j + h) * nn;
+#pragma unroll
+        for (int i = 0; i < n; ++i)
+#pragma unroll
+          for (int c = 0; c < n; ++c) { T s = T(0);
+#pragma unroll
+            for (int m = 0; m < n; ++m) s += Lob[i * n + m] * U[m * n + c];
+            FB[i * n + c] = s; }
+      }
+    }
+    grid.sync();
+    // (2) survivors s = 2hk: Theta_s -= FA_{s+h} Lo_{s+h} + FB_{s-h} Lo_s' ;  Lo_s <- -FB_{s-h} Lo_{s-h}
+    for (long long k = gid;; k += gsz) {
+      const long long s_ = 2LL * h * k;
+      if (s_ >= T_) break;
+      T* Th = b.Th + s_ * nn; T* Los = b.Lo + s_ * nn;
+      T nlo[nn];
+#pragma unroll
+      for (int e = 0; e < nn; ++e) nlo[e] = T(0);
+      if (s_ + h < T_) {
+        const T* FA = b.FA + (s_ + h) * nn; const T* Loj = b.Lo + (s_ + h) * nn;
+#pragma unroll
+        for (int i = 0; i < n; ++i)
+#pragma unroll
+          for (int c = 0; c < n; ++c) { T acc = T(0);
+#pragma unroll
+            for (int m = 0; m < n; ++m) acc += FA[i * n + m] * Loj[m * n + c];
+            Th[i * n + c] -= acc; }
+      }
+      if (s_ - h >= 0) {
+        const T* FB = b.FB + (s_ - h) * nn; const T* Loj = b.Lo + (s_ - h) * nn;
+#pragma unroll
+        for (int i = 0; i < n; ++i)
+#pragma unroll
+          for (int c = 0; c < n; ++c) { T acc = T(0), acc2 = T(0);
+#pragma unroll
+            for (int m = 0; m < n; ++m) { acc += FB[i * n + m] * Los[c * n + m]; acc2 += FB[i * n + m] * Loj[m * n + c]; }
+            Th[i * n + c] -= acc; nlo[i * n + c] = -acc2; }
+      }
+#pragma unroll
+      for (int e = 0; e < nn; ++e) Los[e] = nlo[e];
+    }
+    grid.sync();
+  }
+  if (gid == 0) { T U[nn]; if (spd_inverse<T, NC>(b.Th, U)) atomicOr(b.flag, 1);
+#pragma unroll
+    for (int e = 0; e < nn; ++e) b.U[e] = U[e]; }
+}
+
+}  // namespace tmpc
+
+namespace tmpc {
+
+// ---- the solve with the CR factor, all threads of the grid, gather form; eta is consumed, x written to xt.
+template <typename T, int NC>
+__device__ void cr_solve(cg::grid_group& grid, const CrBuf<T>& b, int T_, long long gid, long long gsz) {
+  constexpr int n = NC, nn = NC * NC;
+  const int L = cr_levels(T_);
+  for (int l = 0; l < L; ++l) {                       // down-sweep: survivors s = 2hk pull from s+h and s-h
+    const long long h = 1LL << l;
+    for (long long w = gid;; w += gsz) {
+      const long long k = w / n; const int i = (int)(w - k * n);
+      const long long s_ = 2 * h * k;
+      if (s_ >= T_) break;
+      T acc = T(0);
+      if (s_ + h < T_) { const T* F = b.FA + (s_ + h) * nn + i * n; const T* e = b.eta + (s_ + h) * n;
+#pragma unroll
+        for (int m = 0; m < n; ++m) acc += F[m] * e[m]; }
+      if (s_ - h >= 0) { const T* F = b.FB + (s_ - h) * nn + i * n; const T* e = b.eta + (s_ - h) * n;
+#pragma unroll
+        for (int m = 0; m < n; ++m) acc += F[m] * e[m]; }
+      b.eta[s_ * n + i] -= acc;
+    }
+    grid.sync();
+  }
+  if (gid < n) { T acc = T(0);
+#pragma unroll
+    for (int m = 0; m < n; ++m) acc += b.U[gid * n + m] * b.eta[m];
+    b.xt[gid] = acc; }
+  grid.sync();
+  for (int l = L - 1; l >= 0; --l) {                  // up-sweep: eliminated j = h(2k+1)
+    const long long h = 1LL << l;
+    for (long long w = gid;; w += gsz) {
+      const long long k = w / n; const int i = (int)(w - k * n);
+      const long long j = h * (2 * k + 1);
+      if (j >= T_) break;
+      const T* U = b.U + j * nn + i * n; const T* e = b.eta + j * n;
+      T acc = T(0);
+#pragma unroll
+      for (int m = 0; m < n; ++m) acc += U[m] * e[m];
+      { const T* F = b.FA + j * nn + i; const T* xa = b.xt + (j - h) * n;
+#pragma unroll
+        for (int m = 0; m < n; ++m) acc -= F[m * n] * xa[m]; }
+      if (j + h < T_) { const T* F = b.FB + j * nn + i; const T* xb = b.xt + (j + h) * n;
+#pragma unroll
+        for (int m = 0; m < n; ++m) acc -= F[m * n] * xb[m]; }
+      b.xt[j * n + i] = acc;
+    }
+    grid.sync();
+  }
+}
+
+template <typename T>
+struct CrAdmmArgs {
+  Dims d; Params<T> prm; QpView<T> qp; unsigned char* ws;
+  T* x; T* zg; T* yf; T* yg; T* xi; T* r_prim; T* r_dual; T* objective; int32_t* status;
+  int iters, zg_given, kkt_only;
+  const T* eta_in; T* xt_out;
+};
+
+// ---- fused ADMM loop (Alg. 3) on the CR factor: one cooperative grid, blockIdx.y = problem
+template <typename T, int NC>
+__global__ void __launch_bounds__(256) cr_admm_kernel(CrAdmmArgs<T> a) {
+  cg::grid_group grid = cg::this_grid();
+  __shared__ T red[64];
+  const Dims& d = a.d;
+  constexpr int n = NC, nn = NC * NC;
+  const int nx = d.nx, ng = d.ng, N = d.N, T_ = d.T, nz = d.nz, mf = d.mf, mg = d.mg, p = blockIdx.y;
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x, gsz = (long long)gridDim.x * blockDim.x;
+  CrBuf<T> b = cr_carve<T>(d, a.ws, p);
+  if (a.kkt_only) {
+    for (long long e = gid; e < nz; e += gsz) b.eta[e] = a.eta_in[(size_t)p * nz + e];
+    grid.sync();
+    cr_solve<T, NC>(grid, b, T_, gid, gsz);
+    for (long long e = gid; e < nz; e += gsz) a.xt_out[(size_t)p * nz + e] = b.xt[e];
+    return;
+  }
+  const T sigma = a.prm.sigma, rho_f = a.prm.rho_f, rho_g = a.prm.rho_g, alpha = a.prm.alpha;
+  const T inv_rho_g = T(1) / rho_g, inv_rg = T(1) / (rho_g + a.prm.gamma), lam = a.prm.lam, gam = a.prm.gamma;
+  T* x = a.x + (size_t)p * nz; T* zg = a.zg + (size_t)p * mg; T* yf = a.yf + (size_t)p * mf; T* yg = a.yg + (size_t)p * mg; T* xi = a.xi + (size_t)p * mg;
+  const T* q = a.qp.q + (size_t)p * nz; const T* lo = a.qp.lo + (size_t)p * mg; const T* hi = a.qp.hi + (size_t)p * mg;
+  const T* Am = a.qp.Am + (size_t)p * N * nx * n; const T* Ap = a.qp.Ap + (size_t)p * N * nx * n;
+  const T* G = a.qp.G ? a.qp.G + a.qp.sG * p : nullptr;
+  const T* xin = a.qp.x_init + (size_t)p * nx; const T* bb = a.qp.b + (size_t)p * N * nx;
+  auto cval = [&](long long e) -> T { return e < nx ? xin[e] : bb[e - nx]; };
+  auto g_dot = [&](int t, int r, const T* vec) -> T {
+    if (d.g_sel) return vec[(size_t)t * n + d.g_col[r]];
+    const T* g = G + ((size_t)t * ng + r) * n; const T* vt = vec + (size_t)t * n; T s = T(0);
+#pragma unroll
+    for (int j = 0; j < n; ++j) s += g[j] * vt[j];
+    return s;
+  };
+  auto c_row = [&](long long e, const T* v) -> T {
+    if (e < nx) return v[e];
+    const long long t = (e - nx) / nx; const int i = (int)((e - nx) - t * nx);
+    const T* am = Am + ((size_t)t * nx + i) * n; const T* ap = Ap + ((size_t)t * nx + i) * n; T s = T(0);
+#pragma unroll
+    for (int j = 0; j < n; ++j) s += am[j] * v[t * n + j] + ap[j] * v[(t + 1) * n + j];
+    return s;
+  };
+  for (long long e = gid; e < mg; e += gsz) {
+    const int t = (int)(e / ng), r = (int)(e - (long long)t * ng);
+    if (!a.zg_given) { zg[e] = tmin(tmax(g_dot(t, r, x), lo[e]), hi[e]); xi[e] = T(0); }
+    b.sv[e] = rho_g * zg[e] - yg[e];
+  }
+  for (long long e = gid; e < mf; e += gsz) b.rv[e] = rho_f * cval(e) - yf[e];
+  grid.sync();
+  for (int it = 0; it < a.iters; ++it) {
+    for (long long e = gid; e < nz; e += gsz) {       // a4 (eq. 51)
+      const long long t = e / n; const int i = (int)(e - t * n);
+      T s = sigma * x[e] - q[e];
+      if (t == 0 && i < nx) s += b.rv[i];
+      if (t < N) { const T* A_ = Am + (size_t)t * nx * n + i; const T* r = b.rv + nx + t * nx; for (int k = 0; k < nx; ++k) s += A_[k * n] * r[k]; }
+      if (t > 0) { const T* A_ = Ap + (size_t)(t - 1) * nx * n + i; const T* r = b.rv + nx + (t - 1) * nx; for (int k = 0; k < nx; ++k) s += A_[k * n] * r[k]; }
+      if (d.g_sel) { for (int r = 0; r < ng; ++r) if (d.g_col[r] == i) s += b.sv[t * ng + r]; }
+      else { const T* g = G + (size_t)t * ng * n + i; for (int r = 0; r < ng; ++r) s += g[r * n] * b.sv[t * ng + r]; }
+      b.eta[e] = s;
+    }
+    grid.sync();
+    cr_solve<T, NC>(grid, b, T_, gid, gsz);          // a11 (eq. 8)
+    for (long long e = gid; e < mf; e += gsz) {       // a7 + a8
+      const T c = cval(e);
+      const T y = yf[e] + rho_f * alpha * (c_row(e, b.xt) - c);
+      yf[e] = y; b.rv[e] = rho_f * c - y;
+    }
+    for (long long e = gid; e < mg; e += gsz) {
+      const int t = (int)(e / ng), r = (int)(e - (long long)t * ng);
+      const T zh = alpha * g_dot(t, r, b.xt) + (T(1) - alpha) * zg[e];
+      const T v = zh + yg[e] * inv_rho_g;
+      T z, s;
+      project_row<T>(((d.soft_mask >> r) & 1u) != 0, v, lo[e], hi[e], rho_g, inv_rg, lam, z, s);
+      const T y = yg[e] + rho_g * (zh - z);
+      zg[e] = z; xi[e] = s; yg[e] = y; b.sv[e] = rho_g * z - y;
+    }
+    for (long long e = gid; e < nz; e += gsz) x[e] = alpha * b.xt[e] + (T(1) - alpha) * x[e];
+    grid.sync();
+  }
+  // ---- a9 residuals / objective: per-CTA partials, then CTA 0 reduces in a fixed order
+  if (a.r_prim || a.r_dual || a.objective || a.status) {
+    const T* Dp = a.qp.D + a.qp.sD * p; const T* Ep = a.qp.E + a.qp.sE * p;
+    T rp = T(0), rd = T(0), ob = T(0);
+    for (long long e = gid; e < mf; e += gsz) rp = tmax(rp, tabs(c_row(e, x) - cval(e)));
+    for (long long e = gid; e < mg; e += gsz) {
+      const int t = (int)(e / ng), r = (int)(e - (long long)t * ng);
+      rp = tmax(rp, tabs(g_dot(t, r, x) - zg[e]));
+      if (((d.soft_mask >> r) & 1u) && xi[e] != T(0)) {
+        const T sg = xi[e] > T(0) ? T(1) : T(-1);
+        rd = tmax(rd, tabs(gam * xi[e] + lam * sg + yg[e]));
+        ob += lam * tabs(xi[e]) + T(0.5) * gam * xi[e] * xi[e];
+      }
+    }
+    for (long long e = gid; e < nz; e += gsz) {
+      const long long t = e / n; const int i = (int)(e - t * n);
+      T px = T(0);
+      const T* Dt = Dp + (size_t)t * nn + i * n;
+      for (int j = 0; j < n; ++j) px += Dt[j] * x[t * n + j];
+      if (t > 0) { const T* Et = Ep + (size_t)(t - 1) * nn + i * n; for (int j = 0; j < n; ++j) px += Et[j] * x[(t - 1) * n + j]; }
+      if (t < N) { const T* Et = Ep + (size_t)t * nn + i; for (int j = 0; j < n; ++j) px += Et[j * n] * x[(t + 1) * n + j]; }
+      T g = px + q[e];
+      if (t == 0 && i < nx) g += yf[i];
+      if (t < N) { const T* A_ = Am + (size_t)t * nx * n + i; for (int k = 0; k < nx; ++k) g += A_[k * n] * yf[nx + t * nx + k]; }
+      if (t > 0) { const T* A_ = Ap + (size_t)(t - 1) * nx * n + i; for (int k = 0; k < nx; ++k) g += A_[k * n] * yf[nx + (t - 1) * nx + k]; }
+      if (d.g_sel) { for (int r = 0; r < ng; ++r) if (d.g_col[r] == i) g += yg[t * ng + r]; }
+      else { const T* gg = G + (size_t)t * ng * n + i; for (int r = 0; r < ng; ++r) g += gg[r * n] * yg[t * ng + r]; }
+      rd = tmax(rd, tabs(g));
+      ob += T(0.5) * x[e] * px + q[e] * x[e];
+    }
+    rp = block_max(rp, red); rd = block_max(rd, red); ob = block_sum(ob, red);
+    if (threadIdx.x == 0) { b.part[3 * blockIdx.x] = rp; b.part[3 * blockIdx.x + 1] = rd; b.part[3 * blockIdx.x + 2] = ob; }
+    grid.sync();
+    if (gid == 0) {
+      T RP = T(0), RD = T(0), OB = T(0);
+      for (unsigned c = 0; c < gridDim.x; ++c) { RP = tmax(RP, b.part[3 * c]); RD = tmax(RD, b.part[3 * c + 1]); OB += b.part[3 * c + 2]; }
+      if (a.r_prim) a.r_prim[p] = RP;
+      if (a.r_dual) a.r_dual[p] = RD;
+      if (a.objective) a.objective[p] = OB;
+      if (a.status) { int st = (*b.flag ? TMPC_ST_PIVOT : 0) | (isfinite(OB) ? 0 : TMPC_ST_NAN); if (st) atomicOr(&a.status[p], st); }
+    }
+  }
+}
+
+// ---- host launchers
+template <typename K, typename A>
+inline tmpc_status cr_launch(K kern, A& args, const Dims& d, cudaStream_t s, int64_t* launches) {
+  int dev = 0, sms = 0, per_sm = 0, coop = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+  if (!coop) return TMPC_E_UNSUPPORTED;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 256, 0) != cudaSuccess || per_sm < 1) return TMPC_E_CUDA;
+  long long want = ((long long)d.nz + 255) / 256;
+  long long cap = (long long)sms * per_sm / d.B;
+  if (cap < 1) return TMPC_E_UNSUPPORTED;
+  if (want > cap) want = cap;
+  if (want > 4096) want = 4096;
+  dim3 grid((unsigned)want, (unsigned)d.B), block(256);
+  void* params[] = { (void*)&args };
+  if (cudaLaunchCooperativeKernel((void*)kern, grid, block, params, 0, s) != cudaSuccess) { cudaGetLastError(); return TMPC_E_CUDA; }
+  if (launches) ++*launches;
+  return TMPC_OK;
+}
 
 template <typename T>
 tmpc_status cr_factor(const Dims& d, const QpView<T>& qp, double sigma, double rho_f, double rho_g, unsigned char* ws, cudaStream_t s, int64_t* launches) {
+  CrFactorArgs<T> a; a.d = d; a.qp = qp; a.sigma = (T)sigma; a.rho_f = (T)rho_f; a.rho_g = (T)rho_g; a.ws = ws;
+  if (d.n == 6) return cr_launch(cr_factor_kernel<T, 6>, a, d, s, launches);
+  if (d.n == 8) return cr_launch(cr_factor_kernel<T, 8>, a, d, s, launches);
   return TMPC_E_UNSUPPORTED;
 }
 template <typename T>
 tmpc_status cr_admm(const Dims& d, const Params<T>& prm, const QpView<T>& qp, unsigned char* ws, T* x, T* zg, T* yf, T* yg, T* xi, T* r_prim, T* r_dual,
                     T* objective, int32_t* status, int iters, bool zg_given, cudaStream_t s, int64_t* launches) {
+  CrAdmmArgs<T> a; memset(&a, 0, sizeof(a));
+  a.d = d; a.prm = prm; a.qp = qp; a.ws = ws; a.x = x; a.zg = zg; a.yf = yf; a.yg = yg; a.xi = xi;
+  a.r_prim = r_prim; a.r_dual = r_dual; a.objective = objective; a.status = status; a.iters = iters; a.zg_given = zg_given;
+  if (d.n == 6) return cr_launch(cr_admm_kernel<T, 6>, a, d, s, launches);
+  if (d.n == 8) return cr_launch(cr_admm_kernel<T, 8>, a, d, s, launches);
   return TMPC_E_UNSUPPORTED;
 }
-
 template <typename T>
-tmpc_status cr_kkt_solve(const Dims& d, unsigned char* ws, const T* eta, T* xt, cudaStream_t s, int64_t* launches) { return TMPC_E_UNSUPPORTED; }
+tmpc_status cr_kkt_solve(const Dims& d, unsigned char* ws, const T* eta, T* xt, cudaStream_t s, int64_t* launches) {
+  CrAdmmArgs<T> a; memset(&a, 0, sizeof(a));
+  a.d = d; a.ws = ws; a.kkt_only = 1; a.eta_in = eta; a.xt_out = xt;
+  if (d.n == 6) return cr_launch(cr_admm_kernel<T, 6>, a, d, s, launches);
+  if (d.n == 8) return cr_launch(cr_admm_kernel<T, 8>, a, d, s, launches);
+  return TMPC_E_UNSUPPORTED;
+}
 
 }  // namespace tmpc

@@ -205,3 +205,51 @@ def test_config3_subset_fp32():
 def test_config3_shape_fp64():
     w = W.config3(B=2, N=4)
     run_pair(w, "f64", iters=25, band=1)
+
+
+# ----------------------------------------------------------------------------------------------- a11 cyclic reduction
+@pytest.mark.parametrize("N", [1, 2, 4, 20, 63, 64, 100])
+def test_cyclic_reduction_solve_equals_sequential_and_oracle(N):
+    """T = N+1 in {2,3,5,21,64,65,101}: CR solve == oracle band Cholesky == sequential block factor (reading O-6)."""
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    w = W.random_ltv(40 + N, 2, N, 4, 2, [4, 5], [0, 0, 1], implicit=True, dense_g_rows=1)
+    eta = np.random.default_rng(N).standard_normal((w.B, w.T, w.n))
+    cfg = O.make_cfg(w)
+    ref = np.stack([O.solve_S(w, cfg, eta[b].ravel(), b).reshape(w.T, w.n) for b in range(w.B)])
+    for lin in (Bd.TMPC_LIN_CYCLIC_REDUCTION, Bd.TMPC_LIN_SEQUENTIAL):
+        s = Solver(w, dtype="f64", linsolve=lin)
+        s.factor()
+        xt = s.kkt_solve(s._up(eta)).cpu().double().numpy()
+        assert rel_err(xt, ref) <= 1e-10, lin
+        s.close()
+
+
+def test_cyclic_reduction_admm_matches_oracle():
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    w = W.random_ltv(51, 2, 37, 4, 2, [4, 5], [0, 0, 1], implicit=True, dense_g_rows=1, q_scale=0.3)
+    s = Solver(w, dtype="f64", linsolve=Bd.TMPC_LIN_CYCLIC_REDUCTION)
+    s.solve(80)
+    got, info = s.state_numpy(), s.info_numpy()
+    ref, rinfo, rc = O.admm(w, O.make_cfg(w), iters=80)
+    compare_states(got, ref, 1e-9)
+    assert (np.abs(info["objective"] - rinfo[:, 2]) <= 1e-9 * np.maximum(1, np.abs(rinfo[:, 2]))).all()
+    assert (np.abs(info["r_prim"] - rinfo[:, 0]) <= 1e-9).all() and (np.abs(info["r_dual"] - rinfo[:, 1]) <= 1e-7).all()
+    s.close()
+
+
+@pytest.mark.parametrize("N,n_sqp,iters", [(300, 3, 100), (8192, 3, 100)])
+def test_config5_long_horizon_sqp(N, n_sqp, iters):
+    """BASELINE configs[4]: bicycle, B=1, fp64, cyclic reduction, 3 SQP x 100 ADMM, against the banded oracle."""
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    w = W.config5(N=N)
+    s = Solver(w, dtype="f64", linsolve=Bd.TMPC_LIN_CYCLIC_REDUCTION)
+    s.reset_state(w.xbar0)
+    s.sqp(n_sqp, iters)
+    got = s.state_numpy()
+    ref, info, rc = O.sqp_bicycle(w, O.make_cfg(w, band=1), n_sqp=n_sqp, iters=iters)
+    assert rc == 0
+    compare_states(got, ref, 1e-9)
+    s.close()
