@@ -32,16 +32,20 @@ FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 FMA lan
 FP64_PEAK_TFLOPS = FP32_PEAK_TFLOPS / 2               # 64 FP64 FMA lanes per SM
 
 
-def make_workload(cfg_id, dtype, batch=None):
+def make_workload(cfg_id, dtype, batch=None, rank=0):
     from paper_2606_24039_b200 import workloads as W
+    from paper_2606_24039_b200.sharding import rank_problem_range
+    kw = {"B": batch} if batch else {}
+    B = batch or {1: 1, 2: 1024, 3: 512, 4: 4096, 5: 1}[cfg_id]
+    first = rank_problem_range(B, max(1, rank + 1), rank)[0]      # rank r owns problems [r*B, (r+1)*B) of the generator
     if cfg_id == 1:
-        w = W.config1()
+        w = W.config1(seed=rank)
     elif cfg_id == 2:
-        w = W.config2(dtype=dtype, **({"B": batch} if batch else {}))
+        w = W.config2(dtype=dtype, first_problem=first, **kw)
     elif cfg_id == 3:
-        w = W.config3(**({"B": batch} if batch else {}))
+        w = W.config3(first_problem=first, **kw)
     elif cfg_id == 4:
-        w = W.config4(dtype=dtype, **({"B": batch} if batch else {}))
+        w = W.config4(dtype=dtype, first_problem=first, **kw)
     elif cfg_id == 5:
         w = W.config5(dtype=dtype)
     else:
@@ -105,7 +109,7 @@ def oracle_rate(w, cfg_id, nthreads, budget_problems):
 
 
 def oracle_sample_size(cfg_id):
-    return {1: 1, 2: 256, 3: 16, 4: 256, 5: 1}[cfg_id]
+    return {1: 1, 2: 1024, 3: 64, 4: 1024, 5: 1}[cfg_id]
 
 
 def run_reference(args):
@@ -144,7 +148,7 @@ def run_gpu(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     dev = torch.device(f"cuda:{local}")
-    w = make_workload(args.config, args.dtype, args.batch)
+    w = make_workload(args.config, args.dtype, args.batch, rank)
     linsolve = Bd.TMPC_LIN_CYCLIC_REDUCTION if args.config == 5 else Bd.TMPC_LIN_SEQUENTIAL
     s = Solver(w, dtype=args.dtype, device=dev, linsolve=linsolve)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)   # > 126 MB L2
