@@ -6,6 +6,7 @@
 #include "tmpc_common.cuh"
 #include "tmpc_factor.cuh"
 #include "tmpc_admm.cuh"
+#include "tmpc_admm2.cuh"
 #include "tmpc_misc.cuh"
 #include "tmpc_backward.cuh"
 #include "tmpc_cr.cuh"
@@ -34,7 +35,7 @@ Layout make_layout(const tmpc_config& c) {
   const Dims d = make_dims(c); const size_t es = esize(c.dtype), B = d.B, nn = (size_t)d.n * d.n;
   Layout L; size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
-  L.Lam = take(B * d.N * nn * es); L.Sinv = take(B * d.T * nn * es);
+  L.Lam = take(B * d.T * nn * es); L.Sinv = take(B * d.T * nn * es);
   L.cls = take(B * d.mg); L.soft_adj = take(B * d.mg);
   L.rhs = take(B * d.nz * es); L.w_rows = take(B * d.mg * es); L.lo_adj = take(B * d.mg * es); L.hi_adj = take(B * d.mg * es);
   L.q_adj = take(B * d.nz * es); L.ax = take(B * d.nz * es); L.azg = take(B * d.mg * es); L.ayf = take(B * d.mf * es);
@@ -60,7 +61,7 @@ tmpc_status check_cfg(const tmpc_config* c) {
 }  // namespace
 
 struct tmpc_ctx {
-  tmpc_config cfg; Dims d; Layout lay; unsigned char* ws; cudaStream_t stream; bool factored; bool cr; int64_t launches;
+  tmpc_config cfg; Dims d; Layout lay; unsigned char* ws; cudaStream_t stream; bool factored; bool cr; bool twisted; int64_t launches;
 };
 
 namespace {
@@ -107,9 +108,18 @@ tmpc_status launch_admm_inst(tmpc_ctx* h, const AdmmArgs<T>& a, int nt, size_t s
   k<<<h->d.B, nt, smem, h->stream>>>(a); h->launches++;
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
 }
+struct FastPlan { bool ok; int pg, nt, ctas_per_sm; size_t smem; };
+template <typename T> FastPlan fast_plan(const Dims& d);
+template <typename T> tmpc_status launch_admm2(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f);
+template <typename T> tmpc_status launch_residual(tmpc_ctx* h, const AdmmArgs<T>& s);
 template <typename T>
 tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
   const Dims& d = h->d;
+  if (h->twisted) {                      // the factor in the workspace is the twisted one: only admm2_kernel reads it
+    tmpc_status s = launch_admm2<T>(h, a, fast_plan<T>(d));
+    if (s != TMPC_OK || a.kkt_only) return s;
+    return launch_residual<T>(h, a);
+  }
   size_t smem_res = admm_smem_elems(d, true) * sizeof(T), smem_str = admm_smem_elems(d, false) * sizeof(T);
   const bool res = smem_res <= kMaxSmem;
   if (!res && smem_str > kMaxSmem) return TMPC_E_UNSUPPORTED;
@@ -122,10 +132,77 @@ tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
   return launch_admm_inst<T, 0, false>(h, a, nt, smem_str);
 }
 
+// ---- resident fast path (tmpc_admm2.cuh): eligibility and launch shape
+constexpr size_t kSmemPerSM = 228 * 1024;
+template <typename T>
+FastPlan fast_plan(const Dims& d) {
+  FastPlan f; f.ok = false; f.pg = 1; f.nt = 0; f.ctas_per_sm = 0; f.smem = 0;
+  const bool shape = (d.n == 8 && d.nx == 6) || (d.n == 6 && d.nx == 4);
+  if (!shape || d.ng > d.n || d.T < 2) return f;
+  const size_t s1 = d.n == 8 ? admm2_smem_bytes<T, 8, 6>(d, 1) : admm2_smem_bytes<T, 6, 4>(d, 1), s2 = d.n == 8 ? admm2_smem_bytes<T, 8, 6>(d, 2) : admm2_smem_bytes<T, 6, 4>(d, 2);
+  if (s1 > kMaxSmem) return f;
+  const int c1 = (int)(kSmemPerSM / (s1 + 1024)), c2 = s2 <= kMaxSmem ? (int)(kSmemPerSM / (s2 + 1024)) : 0;
+  f.pg = (d.B >= 2 && c2 >= 2 && 2 * c2 >= c1) ? 2 : 1;
+  auto threads = [&](int pg) { int t = ((pg * d.nz + 1) / 2 + 31) / 32 * 32; return t < 32 ? 32 : t; };
+  const int tmax = sizeof(T) == 8 ? 512 : 1024;
+  if (threads(f.pg) > tmax) f.pg = 1;
+  f.nt = threads(f.pg);
+  if (f.nt > tmax) return f;
+  f.smem = f.pg == 2 ? s2 : s1; f.ctas_per_sm = f.pg == 2 ? c2 : c1; f.ok = true;
+  return f;
+}
+
+template <typename T, int NC, int NX, int PG, int MAXT, int MINB>
+tmpc_status launch_admm2_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
+  auto k = admm2_kernel<T, NC, NX, PG, MAXT, MINB>;
+  if (f.smem > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem) != cudaSuccess) return TMPC_E_CUDA;
+  const unsigned grid = (unsigned)((h->d.B + PG - 1) / PG);
+  Admm2Args<T> A; A.a = a; A.pl = admm2_plan<T, NC, NX>(h->d, PG);
+  A.rfa = a.prm.rho_f * a.prm.alpha; A.oma = T(1) - a.prm.alpha; A.inv_rho_g = T(1) / a.prm.rho_g; A.inv_rg = T(1) / (a.prm.rho_g + a.prm.gamma);
+  k<<<grid, f.nt, f.smem, h->stream>>>(A); h->launches++;
+  return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+}
+template <typename T, int NC, int NX, int PG>
+tmpc_status launch_admm2_shape(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
+  if constexpr (sizeof(T) == 8) return launch_admm2_inst<T, NC, NX, PG, 512, 1>(h, a, f);
+  else {
+    if (f.nt <= 448 && f.ctas_per_sm <= 2) return launch_admm2_inst<T, NC, NX, PG, 448, 2>(h, a, f);
+    return launch_admm2_inst<T, NC, NX, PG, 1024, 1>(h, a, f);
+  }
+}
+template <typename T>
+tmpc_status launch_admm2(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
+  const Dims& d = h->d;
+  if (d.n == 8 && d.nx == 6) return f.pg == 2 ? launch_admm2_shape<T, 8, 6, 2>(h, a, f) : launch_admm2_shape<T, 8, 6, 1>(h, a, f);
+  if (d.n == 6 && d.nx == 4) return f.pg == 2 ? launch_admm2_shape<T, 6, 4, 2>(h, a, f) : launch_admm2_shape<T, 6, 4, 1>(h, a, f);
+  return TMPC_E_UNSUPPORTED;
+}
+template <typename T>
+tmpc_status launch_factor_tw(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_in, int32_t* status) {
+  FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = nullptr;
+  a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
+  const int nn = h->d.n * h->d.n;
+  int hn = ((nn + 31) / 32) * 32; if (hn > 512) hn = 512;
+  const size_t smem = 6 * (size_t)nn * sizeof(double);
+  factor_tw_kernel<T, double><<<h->d.B, 2 * hn, smem, h->stream>>>(a); h->launches++;
+  return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+}
+template <typename T>
+tmpc_status launch_residual(tmpc_ctx* h, const AdmmArgs<T>& s) {
+  if (!s.r_prim && !s.r_dual && !s.objective && !s.status) return TMPC_OK;
+  ResidualArgs<T> r; r.d = h->d; r.prm = s.prm; r.qp = s.qp; r.x = s.x; r.zg = s.zg; r.yf = s.yf; r.yg = s.yg; r.xi = s.xi;
+  r.r_prim = s.r_prim; r.r_dual = s.r_dual; r.objective = s.objective; r.status = s.status;
+  int nt = ((h->d.nz + 31) / 32) * 32; if (nt > 256) nt = 256;
+  residual_kernel<T><<<h->d.B, nt, 0, h->stream>>>(r); h->launches++;
+  return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+}
+
 template <typename T>
 tmpc_status do_factor(tmpc_ctx* h, const tmpc_qp* qp) {
   const double rho_f = h->cfg.rho_eq_scale * h->cfg.rho_bar, rho_g = h->cfg.rho_bar;
   if (h->cr) return cr_factor<T>(h->d, view<T>(qp), h->cfg.sigma, rho_f, rho_g, h->ws + h->lay.cr, h->stream, &h->launches);
+  h->twisted = fast_plan<T>(h->d).ok;
+  if (h->twisted) return launch_factor_tw<T>(h, qp, rho_f, rho_g, nullptr);
   return launch_factor<T>(h, qp, rho_f, rho_g, nullptr, nullptr);
 }
 
@@ -188,7 +265,7 @@ tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, vo
   tmpc_ctx* h = new (std::nothrow) tmpc_ctx;
   if (!h) return TMPC_E_BADARG;
   h->cfg = *cfg; h->d = make_dims(*cfg); h->lay = L; h->ws = (unsigned char*)workspace; h->stream = (cudaStream_t)cuda_stream;
-  h->factored = false; h->cr = use_cr(*cfg); h->launches = 0;
+  h->factored = false; h->cr = use_cr(*cfg); h->twisted = false; h->launches = 0;
   // zero buffers of the adjoint QP (x_init = 0, b = 0)
   if (cudaMemsetAsync(h->ws + L.zero_xinit, 0, L.zero_b - L.zero_xinit, h->stream) != cudaSuccess ||
       cudaMemsetAsync(h->ws + L.zero_b, 0, L.cr - L.zero_b, h->stream) != cudaSuccess) { delete h; return TMPC_E_CUDA; }
@@ -271,7 +348,7 @@ tmpc_status do_backward(tmpc_ctx* h, const tmpc_qp* qp, const tmpc_state* st, co
     bwd_prepare_kernel<T><<<d.B, ntp, 0, h->stream>>>(a); h->launches++;
     if (!cuda_ok()) return TMPC_E_CUDA;
     tmpc_status s = launch_factor<T>(h, qp, (double)a.rho_adj, 0.0, a.w_rows, nullptr);
-    h->factored = false;                       // the forward factor has been overwritten
+    h->factored = false; h->twisted = false;   // the forward factor has been overwritten (one-directional form)
     if (s != TMPC_OK) return s;
     a.Lam = (const T*)(ws + L.Lam); a.Sinv = (const T*)(ws + L.Sinv);
     const size_t smem = (3 * (size_t)d.nz + 2 * (size_t)d.mf + 2 * (size_t)d.mg) * sizeof(T);
