@@ -63,16 +63,17 @@ template <int L> __device__ __forceinline__ double dotv(const double (&a)[L], co
 
 // ---- shared-memory layout.  One RECORD per stage holds everything that multiplies or belongs to the stage variable
 // v_t, at compile-time offsets from the record base (so a thread needs one address register per stage it touches):
-//   AM  A^-_t             [nx][n]   (zero for t = N)
-//   AP  A^+_{t-1}         [nx][n]   (A_init = [I 0] for t = 0: the rows x_0 = x_init are "dynamics block -1")
+//   AM  A~^-_t = A^-_t X_t'     [nx][n]   (zero for t = N)
+//   AP  A~^+_{t-1} = A^+_{t-1} X_t' [nx][n] (A_init = [I 0] for t = 0: the rows x_0 = x_init are "dynamics block -1")
 //   RM  r of block t      [nx]      r = rho_f c - y_f of the rows that AM belongs to
 //   RP  r of block t-1    [nx]      (r_init for t = 0); written by the owner of that row together with RM of its own stage
-//   S   s_t = rho_g z_g - y_g [n slots, ng used]
-//   E0  eta_t -> w_t      [n]
-//   E1  v_t -> x~_t       [n]
-//   LAM Lambda_t          [n][n]    twisted factor, tmpc_factor.cuh
-//   SINV Sigma_t^{-1}     [n][n]
-//   G   G_t               [ng][n]   only when G is not a selection
+//   E0  y_t               [n]       solution of the scaled system (x~_t = X_t' y_t)
+//   E1  eta~_t -> w_t     [n]
+//   D   sigma x - q + G's [n]       exchanged inside the stage for the X_t product
+//   LAM -B_t              [n][n]    twisted factor, tmpc_factor.cuh
+//   SINV X_t = L_t^{-1}   [n][n]
+//   S   s_t = rho_g z_g - y_g [n slots, ng used]   only when G is not a selection
+//   G   G~_t = G_t X_t'   [ng][n]                  only when G is not a selection
 // Rows of AM, AP, LAM, SINV are XOR-swizzled by 16-byte chunks for n = 8 (conflict-free row-wise vector loads AND
 // column-wise scalar loads); the record stride is padded to 8 (mod 32) words so that the four stages a warp touches
 // fall into distinct banks, records of the down chain are skewed by 8 words and the second problem by 16.
@@ -80,8 +81,8 @@ template <typename T, int NC, int NX>
 struct Rec {
   static constexpr int V = 16 / (int)sizeof(T);
   static constexpr int up(int v) { return (v + V - 1) / V * V; }
-  static constexpr int AM = 0, AP = AM + up(NX * NC), RM = AP + up(NX * NC), RP = RM + up(NX), S = RP + up(NX), E0 = S + up(NC),
-                       E1 = E0 + up(NC), LAM = E1 + up(NC), SINV = LAM + up(NC * NC), G = SINV + up(NC * NC);
+  static constexpr int AM = 0, AP = AM + up(NX * NC), RM = AP + up(NX * NC), RP = RM + up(NX), E0 = RP + up(NX),
+                       E1 = E0 + up(NC), D = E1 + up(NC), LAM = D + up(NC), SINV = LAM + up(NC * NC), S = SINV + up(NC * NC), G = S + up(NC);   // S, G: dense G only
   static constexpr int SKEW = NC == 8 ? 8 : 0;
 };
 struct Admm2Plan { int R, per_problem; };
@@ -90,7 +91,7 @@ template <typename T, int NC, int NX>
 __host__ __device__ inline Admm2Plan admm2_plan(const Dims& d, int pg) {
   using RC = Rec<T, NC, NX>;
   Admm2Plan P;
-  int R = RC::G + (d.g_sel ? 0 : RC::up(d.ng * NC));
+  int R = d.g_sel ? RC::S : RC::G + RC::up(d.ng * NC);
   if (NC == 8) { const int mod = 128 / (int)sizeof(T), want = sizeof(T) == 4 ? 8 : 8; while (R % (sizeof(T) == 4 ? 32 : 16) != want) R += RC::V; (void)mod; }
   P.R = R;
   int pp = d.T * R + RC::SKEW;
@@ -107,6 +108,36 @@ template <typename T, int NC> __device__ __forceinline__ constexpr int swz_x(int
   return sizeof(T) == 4 ? ((row >> 2) & 1) * 4 : ((row >> 1) & 3) * 2;
 }
 
+
+// ---- explicit shared-state-space accesses on 32-bit addresses (byte units).  Going through generic pointers makes the
+// compiler rebuild the shared window base (S2UR SR_CgaCtaId + ULEA, ~25 cycles) inside every chain step.
+__device__ __forceinline__ void lds_vec8(unsigned a0, unsigned a1, float (&r)[8]) {   // two 16-byte chunks, issued together
+  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%8];\n\tld.shared.v4.f32 {%4,%5,%6,%7}, [%9];"
+               : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]), "=f"(r[4]), "=f"(r[5]), "=f"(r[6]), "=f"(r[7]) : "r"(a0), "r"(a1));
+}
+__device__ __forceinline__ void lds_vec8(unsigned a0, unsigned a1, unsigned a2, unsigned a3, double (&r)[8]) {
+  asm volatile("ld.shared.v2.f64 {%0,%1}, [%8];\n\tld.shared.v2.f64 {%2,%3}, [%9];\n\tld.shared.v2.f64 {%4,%5}, [%10];\n\tld.shared.v2.f64 {%6,%7}, [%11];"
+               : "=d"(r[0]), "=d"(r[1]), "=d"(r[2]), "=d"(r[3]), "=d"(r[4]), "=d"(r[5]), "=d"(r[6]), "=d"(r[7]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3));
+}
+__device__ __forceinline__ void lds_vec6(unsigned a, float (&r)[6]) {
+  asm volatile("ld.shared.v2.f32 {%0,%1}, [%6];\n\tld.shared.v2.f32 {%2,%3}, [%6+8];\n\tld.shared.v2.f32 {%4,%5}, [%6+16];"
+               : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]), "=f"(r[4]), "=f"(r[5]) : "r"(a));
+}
+__device__ __forceinline__ void lds_vec6(unsigned a, double (&r)[6]) {
+  asm volatile("ld.shared.v2.f64 {%0,%1}, [%6];\n\tld.shared.v2.f64 {%2,%3}, [%6+16];\n\tld.shared.v2.f64 {%4,%5}, [%6+32];"
+               : "=d"(r[0]), "=d"(r[1]), "=d"(r[2]), "=d"(r[3]), "=d"(r[4]), "=d"(r[5]) : "r"(a));
+}
+__device__ __forceinline__ float lds_1(unsigned a, float) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
+__device__ __forceinline__ double lds_1(unsigned a, double) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
+__device__ __forceinline__ void sts_1(unsigned a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ void sts_1(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+// contiguous NC-vector at byte address a; for NC = 8 the 16-byte chunks are taken in the order of a row swizzled by swb bytes
+template <typename T, int NC> __device__ __forceinline__ void lds_row(unsigned a, unsigned swb, T (&r)[NC]) {
+  if constexpr (NC == 8 && sizeof(T) == 4) lds_vec8(a + (0u ^ swb), a + (16u ^ swb), r);
+  else if constexpr (NC == 8) lds_vec8(a + (0u ^ swb), a + (16u ^ swb), a + (32u ^ swb), a + (48u ^ swb), r);
+  else lds_vec6(a, r);
+}
+
 template <typename T>
 struct Admm2Args {
   AdmmArgs<T> a;
@@ -115,7 +146,99 @@ struct Admm2Args {
 };
 
 // item flag bits
-enum : unsigned { F_VALID = 1u, F_DYN = 2u, F_INEQ = 4u, F_SOFT = 8u, F_GMASK_SH = 8, F_GCOL_SH = 16 };
+enum : unsigned { F_VALID = 1u, F_DYN = 2u, F_INEQ = 4u, F_SOFT = 8u, F_ROW_SH = 8 };
+
+// named barriers: 1 = right-hand side ready (item warps arrive, chain warp waits), 2 = solution ready (chain warp
+// arrives, item warps wait), 3 = item warps only
+__device__ __forceinline__ void bar_sync(int id, int cnt) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(cnt) : "memory"); }
+__device__ __forceinline__ void bar_arrive(int id, int cnt) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(cnt) : "memory"); }
+
+template <int L> __device__ __forceinline__ float dotv_from(const float (&a)[L], const float (&b)[L], float init) {
+  // two independent FFMA2 chains, one per half of the vectors: the second instruction already needs the second half, so
+  // ptxas issues all operand loads back to back instead of serialising load - use - load - use on recycled registers
+  static_assert(L % 2 == 0, "even length");
+  constexpr int H = (L / 4) * 2;                       // first half length (even)
+  float2 p = make_float2(init, 0.f), q = make_float2(0.f, 0.f);
+#pragma unroll
+  for (int j = 0; j < H; j += 2) {
+    p = __ffma2_rn(make_float2(a[j], a[j + 1]), make_float2(b[j], b[j + 1]), p);
+    if (H + j + 1 < L) q = __ffma2_rn(make_float2(a[H + j], a[H + j + 1]), make_float2(b[H + j], b[H + j + 1]), q);
+  }
+  if constexpr (L - 2 * H > 0) q = __ffma2_rn(make_float2(a[L - 2], a[L - 1]), make_float2(b[L - 2], b[L - 1]), q);
+  return (p.x + q.x) + (p.y + q.y);
+}
+template <int L> __device__ __forceinline__ double dotv_from(const double (&a)[L], const double (&b)[L], double init) {
+  double acc[2] = {init, 0.0};
+#pragma unroll
+  for (int j = 0; j < L; ++j) acc[j & 1] += a[j] * b[j];
+  return acc[0] + acc[1];
+}
+
+// ---- x~ = S^{-1} eta on the scaled variables (tmpc_factor.cuh): E1 holds eta~ on entry and w on exit, E0 receives y.
+// One warp; lanes = (problem, direction, row), 8 lanes per slot.  Every step is: publish my component (STS), read the
+// 8-vector back as a broadcast vector load, one row (forward) or column (outward) of -B_t, one FFMA2 dot.
+template <typename T, int NC, int NX, int PG>
+__device__ __forceinline__ void chain_warp_solve(T* sm, int R, int PP, int T_, int lane) {
+  static_assert(NC == 8 || NC == 6, "chain lanes are written for n = 6 and n = 8");
+  using RC = Rec<T, NC, NX>;
+  constexpr int n = NC;
+  constexpr unsigned ES = sizeof(T);
+  const unsigned sb = (unsigned)__cvta_generic_to_shared(sm);
+  const int N = T_ - 1, m = T_ / 2;
+  const int slot = lane >> 3, i8 = lane & 7;
+  const int g = PG == 2 ? (slot >> 1) : 0, dir = slot & 1;
+  const bool act = (PG == 2 || slot < 2) && i8 < n;
+  const int ii = i8 < n ? i8 : 0;
+  const unsigned swb = (unsigned)swz_x<T, NC>(ii) * ES;                 // my row's chunk swizzle, bytes
+  const int cnt = act ? (dir ? T_ - 1 - m : m) : 0, t0 = dir ? N : 0;
+  const int dRb = (dir ? -R : R) * (int)ES;
+  auto rec = [&](int t) { return t * R + (t > m ? RC::SKEW : 0); };
+  const unsigned pb = sb + (unsigned)(g * PP) * ES, bm = pb + (unsigned)rec(m) * ES;
+  constexpr unsigned oE0 = RC::E0 * ES, oE1 = RC::E1 * ES, oLAM = RC::LAM * ES;
+  const unsigned me = (unsigned)ii * ES, myrow = oLAM + (unsigned)(ii * n) * ES;
+  unsigned bt = cnt > 0 ? pb + (unsigned)rec(t0) * ES : bm;
+  T wv = cnt > 0 ? lds_1(bt + oE1 + me, T(0)) : T(0);
+  T Br[n];
+  lds_row<T, NC>(bt + myrow, 0u, Br);
+#pragma unroll 1
+  for (int k = 0; k < m; ++k) {                        // w_next = eta~_next + (-B_t) w_t
+    const bool on = k < cnt, last = k == cnt - 1;
+    if (on) sts_1(bt + oE1 + me, wv);
+    __syncwarp();
+    T W[n];
+    lds_row<T, NC>(bt + oE1, swb, W);
+    const unsigned bnext = last ? bm : bt + dRb;
+    const T eta = (on && !(last && dir)) ? lds_1(bnext + oE1 + me, T(0)) : T(0);
+    if (on) bt = bnext;
+    T Bn[n];
+    lds_row<T, NC>(bt + myrow, 0u, Bn);                // next step's row (record m holds zeros: harmless)
+    const T nw = dotv_from<n>(Br, W, eta);
+    if (on) wv = nw;
+#pragma unroll
+    for (int j = 0; j < n; ++j) Br[j] = Bn[j];
+  }
+  // middle stage: w_m = eta~_m + both contributions; y_m = w_m
+  const T wm = wv + __shfl_xor_sync(0xffffffffu, wv, 8);
+  if (act) { sts_1(bm + oE1 + me, wm); sts_1(bm + oE0 + me, wm); }
+  __syncwarp();
+  // outward sweep: y_t = w_t + (-B_t)' y_next
+  unsigned bc = cnt > 0 ? pb + (unsigned)rec(t0 + (cnt - 1) * (dir ? -1 : 1)) * ES : bm, bp = bm;
+  unsigned colo[n];
+#pragma unroll
+  for (int j = 0; j < n; ++j) colo[j] = oLAM + (unsigned)(j * n + (ii ^ swz_x<T, NC>(j))) * ES;
+#pragma unroll 1
+  for (int k = m - 1; k >= 0; --k) {
+    const bool on = k < cnt;
+    T Y[n], col[n];
+    lds_row<T, NC>(bp + oE0, 0u, Y);
+#pragma unroll
+    for (int j = 0; j < n; ++j) col[j] = lds_1(bc + colo[j], T(0));
+    const T w = lds_1(bc + oE1 + me, T(0));
+    const T y = dotv_from<n>(col, Y, w);
+    if (on) { sts_1(bc + oE0 + me, y); bp = bc; bc -= dRb; }
+    __syncwarp();
+  }
+}
 
 template <typename T, int NC, int NX, int PG, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant__ Admm2Args<T> A) {
@@ -127,11 +250,12 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
   constexpr int n = NC, nx = NX, nn = NC * NC, V = RC::V;
   const int R = A.pl.R, PP = A.pl.per_problem;
   const int ng = d.ng, N = d.N, T_ = d.T, nz = T_ * n, mf = d.mf, mg = d.mg;
-  const int tid = threadIdx.x, nt = blockDim.x;
+  const int tid = threadIdx.x, nt = blockDim.x, nti = nt - 32, it_tid = tid - 32;
   const int m = T_ / 2;
   auto rec = [&](int t) { return t * R + (t > m ? RC::SKEW : 0); };
+  auto sw = [&](int row, int col) { return row * n + (col ^ swz_x<T, NC>(row)); };
 
-  // ---- stage the factor and the constraint blocks of every problem of this CTA into the records
+  // ---- stage 1: X_t and -B_t of every problem of this CTA into the records (all threads)
 #pragma unroll 1
   for (int g = 0; g < PG; ++g) {
     const int p = blockIdx.x * PG + g;
@@ -140,112 +264,112 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
     __syncthreads();
     if (p >= d.B) continue;
     const T* gLam = a.Lam + (size_t)p * T_ * nn;
-    const T* gSinv = a.Sinv + (size_t)p * T_ * nn;
+    const T* gX = a.Sinv + (size_t)p * T_ * nn;
     for (int e = tid; e < T_ * nn; e += nt) {
       const int t = e / nn, rc = e - t * nn, row = rc / n, col = rc - row * n;
-      const int o = rec(t) + row * n + (col ^ swz_x<T, NC>(row));
-      if (t != m) P[o + RC::LAM] = gLam[e];
-      P[o + RC::SINV] = gSinv[e];
-    }
-    if (!a.kkt_only) {
-      const T* gAm = a.qp.Am + (size_t)p * N * nx * n; const T* gAp = a.qp.Ap + (size_t)p * N * nx * n;
-      for (int e = tid; e < N * nx * n; e += nt) {
-        const int t = e / (nx * n), rc = e - t * nx * n, row = rc / n, col = rc - row * n;
-        const int o = row * n + (col ^ swz_x<T, NC>(row));
-        P[rec(t) + RC::AM + o] = gAm[e];
-        P[rec(t + 1) + RC::AP + o] = gAp[e];
-      }
-      for (int e = tid; e < nx; e += nt) P[rec(0) + RC::AP + e * n + (e ^ swz_x<T, NC>(e))] = T(1);   // A_init = [I 0]
-      if (!d.g_sel) { const T* gG = a.qp.G + a.qp.sG * p; for (int e = tid; e < T_ * ng * n; e += nt) { const int t = e / (ng * n); P[rec(t) + RC::G + (e - t * ng * n)] = gG[e]; } }
+      const int o = rec(t) + sw(row, col);
+      if (t != m) P[o + RC::LAM] = -gLam[e];
+      P[o + RC::SINV] = gX[e];
     }
   }
-
-  // ---- x~ = S^{-1} eta on warp 0: E0 (eta) -> E1 (x~)                                                    (eq. 8)
-  // lanes = (problem, direction, row); the operand vector of every step is written to the record by its 8 owners and
-  // read back as a broadcast vector load (3 instructions instead of 8 shuffles; in-order issue makes count = time).
-  auto chain_solve = [&]() {
-    const int lane = tid & 31, slot = lane >> 3, i8 = lane & 7;
-    const int g = PG == 2 ? (slot >> 1) : 0, dir = slot & 1;
-    const bool act = (PG == 2 || slot < 2) && i8 < n;
-    const int ii = i8 < n ? i8 : 0, swx = swz_x<T, NC>(ii);
-    const int cnt = act ? (dir ? T_ - 1 - m : m) : 0, t0 = dir ? N : 0, dR = dir ? -R : R;
-    const int pb = g * PP, bm = pb + rec(m);
-    int bt = cnt > 0 ? pb + rec(t0) : bm;
-    T wv = cnt > 0 ? sm[bt + RC::E0 + ii] : T(0);
-    // physical chunk c of a swizzled row holds logical columns (c*V) ^ swx ...: load the operand vector in the same order
-    auto ld_operand = [&](int base, T (&w)[n]) {
-      if constexpr (NC == 8) {
-#pragma unroll
-        for (int c = 0; c < n / V; ++c) { T part[V]; ld_vec<V>(sm + base + ((c * V) ^ swx), part);
-#pragma unroll
-          for (int e = 0; e < V; ++e) w[c * V + e] = part[e]; }
-      } else ld_vec<n>(sm + base, w);
-    };
+  __syncthreads();
+  // ---- stage 2: constraint blocks in the scaled variables: A~^-_t = A^-_t X_t', A~^+_{t-1} = A^+_{t-1} X_t', G~_t = G_t X_t'
+  if (!a.kkt_only) {
 #pragma unroll 1
-    for (int k = 0; k < m; ++k) {                      // consumes the blocks of the current stage, produces w of the next
-      const bool on = k < cnt, last = k == cnt - 1;
-      if (on) sm[bt + RC::E0 + ii] = wv;
-      __syncwarp();
-      T W[n], Lr[n], Sr[n];
-      ld_operand(bt + RC::E0, W);
-      ld_vec<n>(sm + bt + RC::LAM + ii * n, Lr); ld_vec<n>(sm + bt + RC::SINV + ii * n, Sr);
-      const int bnext = last ? bm : bt + dR;
-      const T eta = (on && !(last && dir)) ? sm[bnext + RC::E0 + ii] : T(0);
-      const T aL = dotv<n>(Lr, W), aS = dotv<n>(Sr, W);
-      if (on) { sm[bt + RC::E1 + ii] = aS; wv = eta - aL; bt = bnext; }   // v = Sigma^{-1} w ; w_next = eta_next - Lambda w
-    }
-    // middle stage: w_m = eta_m - Lam_{m-1} w_{m-1} - Lam_{m+1} w_{m+1} ; x_m = Sigma_m^{-1} w_m (both slots redundantly)
-    const T wm = wv + __shfl_xor_sync(0xffffffffu, wv, 8);
-    if (act) sm[bm + RC::E0 + ii] = wm;
-    __syncwarp();
-    {
-      T W[n], Sr[n];
-      ld_operand(bm + RC::E0, W); ld_vec<n>(sm + bm + RC::SINV + ii * n, Sr);
-      const T xm = dotv<n>(Sr, W);
-      if (act) sm[bm + RC::E1 + ii] = xm;
-    }
-    __syncwarp();
-    // outward sweep: x_t = v_t - Lam_t' x_prev, prev = the neighbour towards the middle
-    int bc = cnt > 0 ? pb + rec(t0 + (cnt - 1) * (dir ? -1 : 1)) : bm, bp = bm;
-#pragma unroll 1
-    for (int k = m - 1; k >= 0; --k) {
-      const bool on = k < cnt;
-      T X[n], col[n];
-      ld_vec<n>(sm + bp + RC::E1, X);
-#pragma unroll
-      for (int j = 0; j < n; ++j) col[j] = sm[bc + RC::LAM + j * n + (ii ^ swz_x<T, NC>(j))];
-      const T v = sm[bc + RC::E1 + ii];
-      const T xn = v - dotv<n>(col, X);
-      if (on) { sm[bc + RC::E1 + ii] = xn; bp = bc; bc -= dR; }
-      __syncwarp();
-    }
-  };
-
-  // ---- tmpc_kkt_solve: xt <- S^{-1} eta
-  if (a.kkt_only) {
-    for (int e = tid; e < PG * nz; e += nt) {
-      const int g = e / nz, el = e - g * nz, t = el / n, i = el - t * n, p = blockIdx.x * PG + g;
-      sm[g * PP + rec(t) + RC::E0 + i] = p < d.B ? a.x[(size_t)p * nz + el] : T(0);
+    for (int g = 0; g < PG; ++g) {
+      const int p = blockIdx.x * PG + g;
+      if (p >= d.B) continue;
+      T* P = sm + g * PP;
+      const T* gAm = a.qp.Am + (size_t)p * N * nx * n; const T* gAp = a.qp.Ap + (size_t)p * N * nx * n;
+      for (int e = tid; e < T_ * nx * n; e += nt) {    // (t, row k, col j): sum_l M[k][l] X_t[j][l], l <= j
+        const int t = e / (nx * n), rc = e - t * nx * n, k = rc / n, j = rc - k * n;
+        const T* Xj = P + rec(t) + RC::SINV;
+        T sa = T(0), sp = T(0);
+        if (t < N) { const T* Mr = gAm + ((size_t)t * nx + k) * n; for (int l = 0; l <= j; ++l) sa += Mr[l] * Xj[sw(j, l)]; }
+        if (t > 0) { const T* Mr = gAp + ((size_t)(t - 1) * nx + k) * n; for (int l = 0; l <= j; ++l) sp += Mr[l] * Xj[sw(j, l)]; }
+        else if (k <= j) sp = Xj[sw(j, k)];             // A_init = [I 0]
+        P[rec(t) + RC::AM + sw(k, j)] = sa;
+        P[rec(t) + RC::AP + sw(k, j)] = sp;
+      }
+      if (!d.g_sel) {
+        const T* gG = a.qp.G + a.qp.sG * p;
+        for (int e = tid; e < T_ * ng * n; e += nt) {
+          const int t = e / (ng * n), rc = e - t * ng * n, k = rc / n, j = rc - k * n;
+          const T* Xj = P + rec(t) + RC::SINV; const T* Mr = gG + ((size_t)t * ng + k) * n;
+          T sg = T(0);
+          for (int l = 0; l <= j; ++l) sg += Mr[l] * Xj[sw(j, l)];
+          P[rec(t) + RC::G + k * n + j] = sg;
+        }
+      }
     }
     __syncthreads();
-    if (tid < 32) chain_solve();
-    __syncthreads();
-    for (int e = tid; e < PG * nz; e += nt) {
-      const int g = e / nz, el = e - g * nz, t = el / n, i = el - t * n, p = blockIdx.x * PG + g;
-      if (p < d.B) a.xi[(size_t)p * nz + el] = sm[g * PP + rec(t) + RC::E1 + i];
+  }
+
+  // ================================================================ chain warp
+  if (tid < 32) {
+    const int iters = a.kkt_only ? 1 : a.iters;
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+      bar_sync(1, nt);
+      chain_warp_solve<T, NC, NX, PG>(sm, R, PP, T_, tid);
+      __syncwarp();
+      bar_arrive(2, nt);
     }
     return;
   }
 
+  // ================================================================ item warps
+  // group exchange of a per-stage vector: the NC owners of a stage sit in one warp when NC = 8, else use the item barrier
+  auto group_sync = [&]() { if constexpr (NC == 8) __syncwarp(); else bar_sync(3, nti); };
+  // operand vector of stage record `base`, field `f`, in the chunk order of swizzled row `row`
+  auto ld_operand = [&](int base, int f, int row, T (&w)[n]) {
+    if constexpr (NC == 8) {
+      const int swx = swz_x<T, NC>(row);
+#pragma unroll
+      for (int c = 0; c < n / V; ++c) { T part[V]; ld_vec<V>(sm + base + f + ((c * V) ^ swx), part);
+#pragma unroll
+        for (int e = 0; e < V; ++e) w[c * V + e] = part[e]; }
+    } else ld_vec<n>(sm + base + f, w);
+  };
+
+  if (a.kkt_only) {                                    // xt <- S^{-1} eta : eta~ = X eta, solve, x = X' y
+    for (int e = it_tid; e < PG * nz; e += nti) {
+      const int g = e / nz, el = e - g * nz, t = el / n, i = el - t * n, p = blockIdx.x * PG + g;
+      sm[g * PP + rec(t) + RC::D + i] = p < d.B ? a.x[(size_t)p * nz + el] : T(0);
+    }
+    bar_sync(3, nti);
+    for (int e = it_tid; e < PG * nz; e += nti) {
+      const int g = e / nz, el = e - g * nz, t = el / n, i = el - t * n, b = g * PP + rec(t);
+      T xr[n], dv[n];
+      ld_vec<n>(sm + b + RC::SINV + i * n, xr); ld_operand(b, RC::D, i, dv);
+      sm[b + RC::E1 + i] = dotv<n>(xr, dv);
+    }
+    bar_arrive(1, nt);
+    bar_sync(2, nt);
+    for (int e = it_tid; e < PG * nz; e += nti) {
+      const int g = e / nz, el = e - g * nz, t = el / n, i = el - t * n, b = g * PP + rec(t), p = blockIdx.x * PG + g;
+      T xc[n], yv[n];
+#pragma unroll
+      for (int j = 0; j < n; ++j) xc[j] = sm[b + RC::SINV + sw(j, i)];
+      ld_vec<n>(sm + b + RC::E0, yv);
+      if (p < d.B) a.xi[(size_t)p * nz + el] = dotv<n>(xc, yv);
+    }
+    return;
+  }
   // ---- per-thread items: (problem g, stage t, row i), two per thread, state in registers.
   // Item (t, i < nx) owns the equality row i of dynamics block t (t < N) or of the init block (t = N: A^- = 0 in record N,
-  // A^+ = A_init in record 0); item (t, i < ng) owns inequality row i of stage t.
+  // A^+ = A_init in record 0).  Inequality row r of stage t is owned by item (t, g_col[r]) for a selection G (so that
+  // G'(.) and G x~ touch only the owner's own component) and by item (t, r) for a dense G.
   constexpr int IPT = 2;
   unsigned fl[IPT]; int bt[IPT], bn[IPT], it_i[IPT];
   T x[IPT], q[IPT], yf[IPT], cv[IPT], zg[IPT], yg[IPT], lo[IPT], hi[IPT];
+  auto g_row = [&](int u) -> size_t {                    // global index of the inequality row of item u (recomputed: not kept live)
+    const int e = it_tid + u * nti, g = e / nz, el = e - g * nz, t = el / n;
+    return (size_t)(blockIdx.x * PG + g) * mg + t * ng + (int)((fl[u] >> F_ROW_SH) & 31u);
+  };
 #pragma unroll
   for (int u = 0; u < IPT; ++u) {
-    const int e = tid + u * nt;
+    const int e = it_tid + u * nti;
     const int g = e / nz, el = e - g * nz, t = el / n, i = el - t * n, p = blockIdx.x * PG + g;
     const bool valid = g < PG && p < d.B;
     fl[u] = 0u; it_i[u] = i; bt[u] = bn[u] = 0;
@@ -259,112 +383,116 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
         if (t < N) { yf[u] = a.yf[(size_t)p * mf + nx + t * nx + i]; cv[u] = a.qp.b[((size_t)p * N + t) * nx + i]; }
         else { yf[u] = a.yf[(size_t)p * mf + i]; cv[u] = a.qp.x_init[(size_t)p * nx + i]; }
       }
-      if (i < ng) {
-        const size_t row = (size_t)p * mg + t * ng + i;
-        fl[u] |= F_INEQ;
+      int r = -1;
+      if (d.g_sel) {
+#pragma unroll
+        for (int rr = 0; rr < NC; ++rr) if (rr < ng && d.g_col[rr] == i) r = rr;   // static indices: no local copy of the array
+      } else if (i < ng) r = i;
+      if (r >= 0) {
+        const size_t row = (size_t)p * mg + t * ng + r;
+        fl[u] |= F_INEQ | ((unsigned)r << F_ROW_SH);
         lo[u] = a.qp.lo[row]; hi[u] = a.qp.hi[row]; yg[u] = a.yg[row];
         if (a.zg_given) zg[u] = a.zg[row];
         else if (a.iters == 0) a.xi[row] = T(0);
-        if (a.soft_rows ? (a.soft_rows[row] != 0) : (((d.soft_mask >> i) & 1u) != 0)) fl[u] |= F_SOFT;
-      }
-      if (d.g_sel) {
-#pragma unroll
-        for (int r = 0; r < NC; ++r) if (r < ng) {       // static indices: no local copy of the parameter array
-          if (r == i) fl[u] |= (unsigned)d.g_col[r] << F_GCOL_SH;
-          if (d.g_col[r] == i) fl[u] |= 1u << (F_GMASK_SH + r);
-        }
+        if (a.soft_rows ? (a.soft_rows[row] != 0) : (((d.soft_mask >> r) & 1u) != 0)) fl[u] |= F_SOFT;
       }
     }
   }
-  // (G_t vec_t)[row i] for the owner of inequality row (t, i); field = RC::E1 (or wherever vec_t sits in the record)
-  auto g_dot_item = [&](int u, int field) -> T {
-    if (d.g_sel) return sm[bt[u] + field + (int)((fl[u] >> F_GCOL_SH) & 15u)];
-    T gr[n], vt[n];
-    ld_vec<n>(sm + bt[u] + RC::G + it_i[u] * n, gr); ld_vec<n>(sm + bt[u] + field, vt);
-    return dotv<n>(gr, vt);
-  };
-  auto g_row = [&](int u) -> size_t {                    // global index of the inequality row of item u (recomputed: not kept live)
-    const int e = tid + u * nt, g = e / nz, el = e - g * nz, t = el / n;
-    return (size_t)(blockIdx.x * PG + g) * mg + t * ng + it_i[u];
-  };
   auto put_r = [&](int u) {                              // r = rho_f c - y_f, for both records that read it
     const T r = a.prm.rho_f * cv[u] - yf[u];
     sm[bt[u] + RC::RM + it_i[u]] = r; sm[bn[u] + RC::RP + it_i[u]] = r;
   };
-  // z_g^0 = clip(G x^0, lo, hi) unless given; r = rho_f c - y_f ; s = rho_g z_g - y_g
+  // z_g^0 = clip(G x^0, lo, hi) unless given (x-space, straight from the problem data); r, s
 #pragma unroll
-  for (int u = 0; u < IPT; ++u) if (fl[u] & F_VALID) sm[bt[u] + RC::E1 + it_i[u]] = x[u];
-  __syncthreads();
+  for (int u = 0; u < IPT; ++u) if (fl[u] & F_VALID) sm[bt[u] + RC::D + it_i[u]] = x[u];
+  bar_sync(3, nti);
 #pragma unroll
   for (int u = 0; u < IPT; ++u) {
     if (fl[u] & F_INEQ) {
-      if (!a.zg_given) zg[u] = tmin(tmax(g_dot_item(u, RC::E1), lo[u]), hi[u]);
-      sm[bt[u] + RC::S + it_i[u]] = a.prm.rho_g * zg[u] - yg[u];
+      if (!a.zg_given) {
+        T gx;
+        if (d.g_sel) gx = x[u];
+        else {
+          const int e = it_tid + u * nti, g = e / nz, el = e - g * nz, t = el / n;
+          const T* gr = a.qp.G + a.qp.sG * (blockIdx.x * PG + g) + ((size_t)t * ng + it_i[u]) * n;
+          gx = T(0);
+          for (int j = 0; j < n; ++j) gx += gr[j] * sm[bt[u] + RC::D + j];
+        }
+        zg[u] = tmin(tmax(gx, lo[u]), hi[u]);
+      }
+      if (!d.g_sel) sm[bt[u] + RC::S + it_i[u]] = a.prm.rho_g * zg[u] - yg[u];
     }
     if (fl[u] & F_DYN) put_r(u);
   }
-  __syncthreads();
+  bar_sync(3, nti);
 
 #pragma unroll 1
   for (int it = 0; it < a.iters; ++it) {
-    // a4: eta = sigma x - q + C'(rho_f c - y_f) + G'(rho_g z_g - y_g)                                       (eq. 51)
+    // a4 in scaled variables: eta~ = X (sigma x - q + G's) + A~^-' r_t + A~^+' r_{t-1}   [+ G~' s for a dense G]   (eq. 51)
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
       if (!(fl[u] & F_VALID)) continue;
-      const int b = bt[u], i = it_i[u];
-      T am[nx], ap[nx], rm[nx], rp[nx];
-#pragma unroll
-      for (int k = 0; k < nx; ++k) { am[k] = sm[b + RC::AM + k * n + (i ^ swz_x<T, NC>(k))]; ap[k] = sm[b + RC::AP + k * n + (i ^ swz_x<T, NC>(k))]; }
-      ld_vec<nx>(sm + b + RC::RM, rm); ld_vec<nx>(sm + b + RC::RP, rp);
-      T s = a.prm.sigma * x[u] - q[u];
-      s += dotv<nx>(am, rm) + dotv<nx>(ap, rp);
-      if (d.g_sel) { unsigned mk = (fl[u] >> F_GMASK_SH) & 255u; while (mk) { const int r = __ffs(mk) - 1; mk &= mk - 1; s += sm[b + RC::S + r]; } }
-      else { for (int r = 0; r < ng; ++r) s += sm[b + RC::G + r * n + i] * sm[b + RC::S + r]; }
-      sm[b + RC::E0 + i] = s;
+      T dd = a.prm.sigma * x[u] - q[u];
+      if (d.g_sel && (fl[u] & F_INEQ)) dd += a.prm.rho_g * zg[u] - yg[u];
+      sm[bt[u] + RC::D + it_i[u]] = dd;
     }
-    __syncthreads();
-    if (tid < 32) chain_solve();
-    __syncthreads();
-    // a7 + a8: z~ = A x~ (eq. 9), relaxation (eq. 10), projection (eq. 12-15), duals (eq. 16 / 44-45)
+    group_sync();
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
       if (!(fl[u] & F_VALID)) continue;
       const int b = bt[u], i = it_i[u];
+      T xr[n], dv[n], am[nx], ap[nx], rm[nx], rp[nx];
+      ld_vec<n>(sm + b + RC::SINV + i * n, xr); ld_operand(b, RC::D, i, dv);
+#pragma unroll
+      for (int k = 0; k < nx; ++k) { am[k] = sm[b + RC::AM + sw(k, i)]; ap[k] = sm[b + RC::AP + sw(k, i)]; }
+      ld_vec<nx>(sm + b + RC::RM, rm); ld_vec<nx>(sm + b + RC::RP, rp);
+      T s = dotv<n>(xr, dv) + (dotv<nx>(am, rm) + dotv<nx>(ap, rp));
+      if (!d.g_sel) for (int r = 0; r < ng; ++r) s += sm[b + RC::G + r * n + i] * sm[b + RC::S + r];
+      sm[b + RC::E1 + i] = s;
+    }
+    bar_arrive(1, nt);
+    bar_sync(2, nt);
+    // a7 + a8 on y: z~_f = A~^- y_t + A~^+ y_{t+1}, x~_i = X(:,i)' y_t, z~_g = x~_i or G~ y_t; relaxation (eq. 10),
+    // projection (eq. 12-15), duals (eq. 16 / 44-45)
+#pragma unroll
+    for (int u = 0; u < IPT; ++u) {
+      if (!(fl[u] & F_VALID)) continue;
+      const int b = bt[u], i = it_i[u];
+      T xc[n], yv[n];
+#pragma unroll
+      for (int j = 0; j < n; ++j) xc[j] = sm[b + RC::SINV + sw(j, i)];
+      ld_vec<n>(sm + b + RC::E0, yv);
+      const T xt = dotv<n>(xc, yv);
       if (fl[u] & F_DYN) {
-        T am[n], ap[n], xa[n], xb[n];
+        T am[n], ap[n], ya[n], yb[n];
         ld_vec<n>(sm + b + RC::AM + i * n, am); ld_vec<n>(sm + bn[u] + RC::AP + i * n, ap);
-        const int swx = swz_x<T, NC>(i);
-        if constexpr (NC == 8) {
-#pragma unroll
-          for (int c = 0; c < n / V; ++c) { T pa[V], pb2[V]; ld_vec<V>(sm + b + RC::E1 + ((c * V) ^ swx), pa); ld_vec<V>(sm + bn[u] + RC::E1 + ((c * V) ^ swx), pb2);
-#pragma unroll
-            for (int e = 0; e < V; ++e) { xa[c * V + e] = pa[e]; xb[c * V + e] = pb2[e]; } }
-        } else { ld_vec<n>(sm + b + RC::E1, xa); ld_vec<n>(sm + bn[u] + RC::E1, xb); }
-        const T zt = dotv<n>(am, xa) + dotv<n>(ap, xb);
+        ld_operand(b, RC::E0, i, ya); ld_operand(bn[u], RC::E0, i, yb);
+        const T zt = dotv<n>(am, ya) + dotv<n>(ap, yb);
         yf[u] += A.rfa * (zt - cv[u]);
         put_r(u);
       }
       if (fl[u] & F_INEQ) {
-        const T ztg = g_dot_item(u, RC::E1);
+        T ztg = xt;
+        if (!d.g_sel) { T gr[n]; ld_vec<n>(sm + b + RC::G + i * n, gr); ztg = dotv<n>(gr, yv); }
         const T zh = a.prm.alpha * ztg + A.oma * zg[u];
         const T v = zh + yg[u] * A.inv_rho_g;
         T z, s;
         project_row<T>((fl[u] & F_SOFT) != 0, v, lo[u], hi[u], a.prm.rho_g, A.inv_rg, a.prm.lam, z, s);
         yg[u] += a.prm.rho_g * (zh - z);
         zg[u] = z;
-        sm[b + RC::S + i] = a.prm.rho_g * z - yg[u];
+        if (!d.g_sel) sm[b + RC::S + i] = a.prm.rho_g * z - yg[u];
         if (it == a.iters - 1) a.xi[g_row(u)] = s;
       }
-      x[u] = a.prm.alpha * sm[b + RC::E1 + i] + A.oma * x[u];
+      x[u] = a.prm.alpha * xt + A.oma * x[u];
     }
-    __syncthreads();
+    bar_sync(3, nti);
   }
 
   // ---- write back the state
 #pragma unroll
   for (int u = 0; u < IPT; ++u) {
     if (!(fl[u] & F_VALID)) continue;
-    const int e = tid + u * nt, g = e / nz, el = e - g * nz, t = el / n, i = it_i[u], p = blockIdx.x * PG + g;
+    const int e = it_tid + u * nti, g = e / nz, el = e - g * nz, t = el / n, i = it_i[u], p = blockIdx.x * PG + g;
     a.x[(size_t)p * nz + el] = x[u];
     if (fl[u] & F_DYN) a.yf[(size_t)p * mf + (t < N ? nx + t * nx + i : i)] = yf[u];
     if (fl[u] & F_INEQ) { const size_t row = g_row(u); a.zg[row] = zg[u]; a.yg[row] = yg[u]; }

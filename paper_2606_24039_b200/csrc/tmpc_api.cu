@@ -139,11 +139,12 @@ FastPlan fast_plan(const Dims& d) {
   FastPlan f; f.ok = false; f.pg = 1; f.nt = 0; f.ctas_per_sm = 0; f.smem = 0;
   const bool shape = (d.n == 8 && d.nx == 6) || (d.n == 6 && d.nx == 4);
   if (!shape || d.ng > d.n || d.T < 2) return f;
+  if (d.g_sel) for (int r = 0; r < d.ng; ++r) for (int q = 0; q < r; ++q) if (d.g_col[r] == d.g_col[q]) return f;   // one selection row per column
   const size_t s1 = d.n == 8 ? admm2_smem_bytes<T, 8, 6>(d, 1) : admm2_smem_bytes<T, 6, 4>(d, 1), s2 = d.n == 8 ? admm2_smem_bytes<T, 8, 6>(d, 2) : admm2_smem_bytes<T, 6, 4>(d, 2);
   if (s1 > kMaxSmem) return f;
   const int c1 = (int)(kSmemPerSM / (s1 + 1024)), c2 = s2 <= kMaxSmem ? (int)(kSmemPerSM / (s2 + 1024)) : 0;
   f.pg = (d.B >= 2 && c2 >= 2 && 2 * c2 >= c1) ? 2 : 1;
-  auto threads = [&](int pg) { int t = ((pg * d.nz + 1) / 2 + 31) / 32 * 32; return t < 32 ? 32 : t; };
+  auto threads = [&](int pg) { int t = ((pg * d.nz + 1) / 2 + 31) / 32 * 32; return 32 + (t < 32 ? 32 : t); };   // + the chain warp
   const int tmax = sizeof(T) == 8 ? 512 : 1024;
   if (threads(f.pg) > tmax) f.pg = 1;
   f.nt = threads(f.pg);
@@ -166,7 +167,8 @@ template <typename T, int NC, int NX, int PG>
 tmpc_status launch_admm2_shape(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
   if constexpr (sizeof(T) == 8) return launch_admm2_inst<T, NC, NX, PG, 512, 1>(h, a, f);
   else {
-    if (f.nt <= 448 && f.ctas_per_sm <= 2) return launch_admm2_inst<T, NC, NX, PG, 448, 2>(h, a, f);
+    if (f.nt <= 384 && f.ctas_per_sm >= 3) return launch_admm2_inst<T, NC, NX, PG, 384, 3>(h, a, f);
+    if (f.nt <= 448) return launch_admm2_inst<T, NC, NX, PG, 448, 2>(h, a, f);
     return launch_admm2_inst<T, NC, NX, PG, 1024, 1>(h, a, f);
   }
 }

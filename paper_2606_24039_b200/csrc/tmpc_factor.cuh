@@ -143,14 +143,17 @@ __global__ void __launch_bounds__(1024) factor_kernel(FactorArgs<T> a) {
 // The block-tridiagonal S is eliminated from BOTH ends towards the middle stage m = T/2: the up chain runs over
 // stages 0,1,..,m-1 and the down chain over N,N-1,..,m+1, independently; the middle pivot collects both Schur
 // contributions.  With  Psi_t = block(next stage of the chain, t) of S  (up: Phi_t; down: Phi_{t-1}'),
-//     Sigma_first = Theta_first,  Lambda_t = Psi_t Sigma_t^{-1},  Sigma_next = Theta_next - Lambda_t Psi_t',
-//     Sigma_m = Theta_m - Lambda_{m-1} Phi_{m-1}' - Lambda_{m+1} Phi_m.
+//     Sigma_first = Theta_first,  L_t L_t' = Sigma_t,  W_t = Psi_t L_t^{-T},  Sigma_next = Theta_next - W_t W_t',
+//     Sigma_m = Theta_m - W_{m-1} W_{m-1}' - W_{m+1} W_{m+1}'   (block Cholesky with the middle stage eliminated last).
+// Stored with explicit inverses of the diagonal Cholesky blocks, X_t = L_t^{-1}, and the off-diagonal blocks pre- and
+// post-multiplied by them, B_t = X_next W_t, so that the two sequential sweeps are pure mat-vecs on scaled variables:
+//     eta~_t = X_t eta_t (stage-parallel),  w_next = eta~_next - B_t w_t,  w_m = eta~_m - B_{m-1} w_{m-1} - B_{m+1} w_{m+1},
+//     y_m = w_m,  y_t = w_t - B_t' y_next (outwards from m),  x_t = X_t' y_t (stage-parallel).
 // It is an exact factorisation of the same S (P A P' = L D L' for the permutation that orders stages
 // 0, N, 1, N-1, ...), same flops and same storage as the one-directional form, but both substitution sweeps of a
-// solve are two independent chains of half the length:
-//     w_t = eta_t - Lambda_prev w_prev  (both chains),  w_m = eta_m - Lambda_{m-1} w_{m-1} - Lambda_{m+1} w_{m+1},
-//     x_m = Sigma_m^{-1} w_m,  x_t = Sigma_t^{-1} w_t - Lambda_t' x_next  (outwards from m).
-// Layout: Lam [B][T][n][n] indexed by the stage t the multiplier belongs to (slot m unused), Sinv [B][T][n][n].
+// solve are two independent chains of half the length.
+// Layout: Lam [B][T][n][n] holds B_t, indexed by the stage t the block belongs to (slot m unused); Sinv [B][T][n][n]
+// holds X_t (lower triangular, zeros stored).
 // One CTA per problem, two halves of blockDim/2 threads, each with its own named barrier and shared buffers.
 struct HalfBar {
   int id, cnt;
@@ -238,21 +241,27 @@ __global__ void __launch_bounds__(1024) factor_tw_kernel(FactorArgs<T> a) {
       dst[e] = s;
     }
   };
-  auto sinv_out = [&](int t, const TA* X, int tt, int tn) {     // Sigma_t^{-1} = X'X
+  // X (lower triangular, zeros above) -> Sinv slot of stage t
+  auto x_out = [&](int t, const TA* X, int tt, int tn) {
+    for (int e = tt; e < nn; e += tn) Sinvp[(size_t)t * nn + e] = (T)X[e];
+  };
+  // B = X_next W_prev -> Lam slot of the stage W belongs to (coupling prev -> next)
+  auto b_out = [&](int tprev, const TA* X, const TA* W, int tt, int tn) {
     for (int e = tt; e < nn; e += tn) {
       const int i = e / n, j = e - i * n;
       TA s = 0;
-      for (int k = (i > j ? i : j); k < n; ++k) s += X[k * n + i] * X[k * n + j];
-      Sinvp[(size_t)t * nn + e] = (T)s;
+      for (int kk = 0; kk <= i; ++kk) s += X[i * n + kk] * W[kk * n + j];
+      Lamp[(size_t)tprev * nn + e] = (T)s;
     }
   };
-
   for (int k = 0; k < cnt; ++k) {
     const int t = half ? N - k : k;
     theta(t, A, k > 0 ? C : nullptr, nullptr, ht, hn);
     bar.sync();
     bad |= chol_and_inverse<TA>(A, Bm, n, ht, hn, bar);
-    sinv_out(t, Bm, ht, hn);
+    if (k > 0) b_out(half ? t + 1 : t - 1, Bm, C, ht, hn);
+    x_out(t, Bm, ht, hn);
+    bar.sync();
     // A <- Psi_t: up Phi_t = E_t + w A^+_t' A^-_t ; down Phi_{t-1}' = E_{t-1}' + w A^-_{t-1}' A^+_{t-1}
     {
       const int tc = half ? t - 1 : t;                  // index of the coupling block Phi_tc
@@ -266,23 +275,16 @@ __global__ void __launch_bounds__(1024) factor_tw_kernel(FactorArgs<T> a) {
       }
     }
     bar.sync();
-    for (int e = ht; e < nn; e += hn) {                 // C <- W = Psi X'
+    for (int e = ht; e < nn; e += hn) {                 // C <- W = Psi X'  (the Cholesky block L_{next,t})
       const int i = e / n, j = e - i * n;
       TA s = 0;
       for (int kk = 0; kk <= j; ++kk) s += A[i * n + kk] * Bm[j * n + kk];
       C[e] = s;
     }
     bar.sync();
-    for (int e = ht; e < nn; e += hn) {                 // Lambda_t = W X
-      const int i = e / n, j = e - i * n;
-      TA s = 0;
-      for (int kk = j; kk < n; ++kk) s += C[i * n + kk] * Bm[kk * n + j];
-      Lamp[(size_t)t * nn + e] = (T)s;
-    }
-    bar.sync();
   }
   __syncthreads();
-  // ---- middle stage m: both halves' last W (if any) feed Sigma_m; half 0 finishes
+  // ---- middle stage m: both halves' last W (if any) feed Sigma_m
   {
     TA* base = reinterpret_cast<TA*>(smem_raw);
     TA* A0 = base; TA* B0 = base + nn; const TA* Wup = base + 2 * nn; const TA* Wdn = base + 5 * nn;
@@ -290,7 +292,9 @@ __global__ void __launch_bounds__(1024) factor_tw_kernel(FactorArgs<T> a) {
     theta(m, A0, m > 0 ? Wup : nullptr, (T_ - 1 - m) > 0 ? Wdn : nullptr, threadIdx.x, blockDim.x);
     __syncthreads();
     bad |= chol_and_inverse<TA>(A0, B0, n, threadIdx.x, blockDim.x, all);
-    sinv_out(m, B0, threadIdx.x, blockDim.x);
+    if (m > 0) b_out(m - 1, B0, Wup, threadIdx.x, blockDim.x);
+    if (T_ - 1 - m > 0) b_out(m + 1, B0, Wdn, threadIdx.x, blockDim.x);
+    x_out(m, B0, threadIdx.x, blockDim.x);
   }
   bad = __syncthreads_or(bad);
   if (a.status && threadIdx.x == 0 && bad) atomicOr(&a.status[p], TMPC_ST_PIVOT);
