@@ -5,6 +5,7 @@
 #include <new>
 #include "tmpc_common.cuh"
 #include "tmpc_factor.cuh"
+#include "tmpc_factor2.cuh"
 #include "tmpc_admm.cuh"
 #include "tmpc_admm2.cuh"
 #include "tmpc_misc.cuh"
@@ -183,10 +184,15 @@ template <typename T>
 tmpc_status launch_factor_tw(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_in, int32_t* status) {
   FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = nullptr;
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
-  const int nn = h->d.n * h->d.n;
-  int hn = ((nn + 31) / 32) * 32; if (hn > 512) hn = 512;
-  const size_t smem = 6 * (size_t)nn * sizeof(double);
-  factor_tw_kernel<T, double><<<h->d.B, 2 * hn, smem, h->stream>>>(a); h->launches++;
+  if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) factor_tw2_kernel<T, 8, 6><<<h->d.B, 64, 0, h->stream>>>(a);
+  else if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) factor_tw2_kernel<T, 6, 4><<<h->d.B, 64, 0, h->stream>>>(a);
+  else {
+    const int nn = h->d.n * h->d.n;
+    int hn = ((nn + 31) / 32) * 32; if (hn > 512) hn = 512;
+    const size_t smem = 6 * (size_t)nn * sizeof(double);
+    factor_tw_kernel<T, double><<<h->d.B, 2 * hn, smem, h->stream>>>(a);
+  }
+  h->launches++;
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
 }
 template <typename T>

@@ -1,0 +1,195 @@
+// tmpc_factor2.cuh — a2 + a3 for the resident fast path: the twisted block Cholesky of tmpc_factor.cuh (same math,
+// same output X_t / B_t), one WARP per half chain with compile-time block sizes.
+//
+// factor_tw_kernel (tmpc_factor.cuh) spends its time in CTA barriers, run-time integer divisions and dependent global
+// loads; here a CTA is two warps (the up chain and the down chain of one problem), every phase of a stage is separated
+// by __syncwarp only, the raw stage data (D_t, E_t, A^-_t, A^+_{t-1}, G_t) of the NEXT stage is prefetched into
+// registers while the current stage is factored, and all index arithmetic is compile-time.  Arithmetic in double.
+#pragma once
+#include "tmpc_factor.cuh"
+
+namespace tmpc {
+
+template <typename T, int NC, int NX>
+__global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
+  constexpr int n = NC, nx = NX, nn = NC * NC, an = NX * NC;
+  constexpr int EPL = (nn + 31) / 32;                   // matrix elements per lane
+  constexpr int GMAX = NC * NC;                         // room for ng <= n rows of G
+  constexpr int RAW = 2 * nn + 2 * an + GMAX;           // D, E, Am, Ap, G
+  constexpr int RPL = (RAW + 31) / 32;
+  __shared__ double sm[2][3 * nn + RAW];
+  const Dims& d = a.d;
+  const int ng = d.ng, N = d.N, T_ = d.T;
+  const int half = threadIdx.x >> 5, lane = threadIdx.x & 31, p = blockIdx.x;
+  double* A = sm[half]; double* Bm = A + nn; double* C = Bm + nn;
+  double* rD = C + nn; double* rE = rD + nn; double* rAm = rE + nn; double* rAp = rAm + an; double* rG = rAp + an;
+  const T* Dp = a.qp.D + a.qp.sD * p;
+  const T* Ep = a.qp.E + a.qp.sE * p;
+  const T* Amp = a.qp.Am + (size_t)p * N * an;
+  const T* App = a.qp.Ap + (size_t)p * N * an;
+  const T* Gp = a.qp.G ? a.qp.G + a.qp.sG * p : nullptr;
+  T* Lamp = a.Lam + (size_t)p * T_ * nn;
+  T* Xp = a.Sinv + (size_t)p * T_ * nn;
+  const int m = T_ / 2, cnt = half ? T_ - 1 - m : m;
+  const double w_eq = a.w_eq, w_in = a.w_in, sigma = a.sigma;
+  int bad = 0;
+
+  // raw data of stage t for this chain: D_t, the coupling block E_tc (tc = t for up, t-1 for down), A^-_t, A^+_{t-1}, G_t
+  auto raw_src = [&](int t, int e) -> T {
+    if (e < nn) return Dp[(size_t)t * nn + e];
+    e -= nn;
+    if (e < nn) { const int tc = half ? t - 1 : t; return (tc >= 0 && tc < N) ? Ep[(size_t)tc * nn + e] : T(0); }
+    e -= nn;
+    if (e < an) return t < N ? Amp[(size_t)t * an + e] : T(0);
+    e -= an;
+    if (e < an) return t > 0 ? App[(size_t)(t - 1) * an + e] : T(0);
+    e -= an;
+    return (Gp && e < ng * n) ? Gp[(size_t)t * ng * n + e] : T(0);
+  };
+  T pre[RPL];
+  auto prefetch = [&](int t) {
+#pragma unroll
+    for (int u = 0; u < RPL; ++u) { const int e = lane + 32 * u; pre[u] = e < RAW ? raw_src(t, e) : T(0); }
+  };
+  auto commit = [&]() {
+#pragma unroll
+    for (int u = 0; u < RPL; ++u) { const int e = lane + 32 * u; if (e < RAW) rD[e] = (double)pre[u]; }
+  };
+  // Theta_t (lower triangle) minus W W' of up to two finished neighbours, from the raw data in shared memory
+  auto theta = [&](int t, double* dst, const double* W1, const double* W2) {
+#pragma unroll
+    for (int u = 0; u < EPL; ++u) {
+      const int e = lane + 32 * u;
+      if (e >= nn) continue;
+      const int i = e / n, j = e % n;
+      if (j > i) continue;
+      double s = rD[e];
+      if (i == j) s += sigma;
+      double acc = 0;
+#pragma unroll
+      for (int r = 0; r < nx; ++r) acc += rAm[r * n + i] * rAm[r * n + j] + rAp[r * n + i] * rAp[r * n + j];
+      if (t == 0 && i == j && i < nx) acc += 1;        // A_init' A_init = blkdiag(I_nx, 0)
+      s += w_eq * acc;
+      if (d.g_sel) { for (int r = 0; r < ng; ++r) if (d.g_col[r] == i && i == j) s += w_in; }
+      else { for (int r = 0; r < ng; ++r) s += w_in * rG[r * n + i] * rG[r * n + j]; }
+      if (W1) { double c = 0;
+#pragma unroll
+        for (int k = 0; k < n; ++k) c += W1[i * n + k] * W1[j * n + k];
+        s -= c; }
+      if (W2) { double c = 0;
+#pragma unroll
+        for (int k = 0; k < n; ++k) c += W2[i * n + k] * W2[j * n + k];
+        s -= c; }
+      dst[e] = s;
+    }
+  };
+  // in-place Cholesky of the lower triangle of Am_ (right-looking), then Xo <- L^{-1}
+  auto chol_inv = [&](double* Am_, double* Xo) {
+#pragma unroll
+    for (int k = 0; k < n; ++k) {
+      double dk = Am_[k * n + k];
+      if (!(dk > 0) || !isfinite(dk)) { bad = 1; dk = 1; }
+      const double inv = 1.0 / dk, sq = sqrt(dk), rs = 1.0 / sq;
+#pragma unroll
+      for (int u = 0; u < EPL; ++u) {
+        const int e = lane + 32 * u, i = e / n, j = e % n;
+        if (e < nn && j > k && j <= i) Am_[e] -= Am_[i * n + k] * Am_[j * n + k] * inv;
+      }
+      __syncwarp();
+      if (lane < n && lane >= k) Am_[lane * n + k] = lane == k ? sq : Am_[lane * n + k] * rs;
+      __syncwarp();
+    }
+#pragma unroll
+    for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u; if (e < nn) Xo[e] = (e / n == e % n) ? 1.0 : 0.0; }
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < n - 1; ++k) {
+      const double inv = 1.0 / Am_[k * n + k];
+#pragma unroll
+      for (int u = 0; u < EPL; ++u) {
+        const int e = lane + 32 * u, i = e / n, j = e % n;
+        if (e < nn && i > k && j <= k) Xo[e] -= Am_[i * n + k] * Xo[k * n + j] * inv;
+      }
+      __syncwarp();
+    }
+#pragma unroll
+    for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u; if (e < nn) Xo[e] = Xo[e] / Am_[(e / n) * n + (e / n)]; }
+    __syncwarp();
+  };
+  auto x_out = [&](int t, const double* X) {
+#pragma unroll
+    for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u; if (e < nn) Xp[(size_t)t * nn + e] = (T)X[e]; }
+  };
+  auto b_out = [&](int tprev, const double* X, const double* W) {      // B = X_next W_prev
+#pragma unroll
+    for (int u = 0; u < EPL; ++u) {
+      const int e = lane + 32 * u;
+      if (e >= nn) continue;
+      const int i = e / n, j = e % n;
+      double s = 0;
+#pragma unroll
+      for (int k = 0; k < n; ++k) if (k <= i) s += X[i * n + k] * W[k * n + j];
+      Lamp[(size_t)tprev * nn + e] = (T)s;
+    }
+  };
+
+  if (cnt > 0) prefetch(half ? N : 0);
+  for (int k = 0; k < cnt; ++k) {
+    const int t = half ? N - k : k;
+    commit();
+    __syncwarp();
+    if (k + 1 < cnt) prefetch(half ? t - 1 : t + 1);
+    theta(t, A, k > 0 ? C : nullptr, nullptr);
+    __syncwarp();
+    chol_inv(A, Bm);
+    if (k > 0) b_out(half ? t + 1 : t - 1, Bm, C);
+    x_out(t, Bm);
+    __syncwarp();
+    // A <- Psi_t: up Phi_t = E_t + w A^+_t' A^-_t ; down Phi_{t-1}' = E_{t-1}' + w A^-_{t-1}' A^+_{t-1}.
+    // up needs A^+_t (not in this stage's raw data): read it from global; down has A^+_{t-1} (rAp) and needs A^-_{t-1}.
+    {
+      const int tc = half ? t - 1 : t;
+      const T* other = half ? Amp + (size_t)tc * an : App + (size_t)tc * an;
+#pragma unroll
+      for (int u = 0; u < EPL; ++u) {
+        const int e = lane + 32 * u;
+        if (e >= nn) continue;
+        const int i = e / n, j = e % n;
+        const int ii = half ? j : i, jj = half ? i : j; // Phi[ii][jj] = E[ii][jj] + w sum_r A^+[r][ii] A^-[r][jj]
+        double acc = 0;
+#pragma unroll
+        for (int r = 0; r < nx; ++r) acc += half ? rAp[r * n + ii] * (double)other[r * n + jj] : (double)other[r * n + ii] * rAm[r * n + jj];
+        A[e] = rE[ii * n + jj] + w_eq * acc;
+      }
+    }
+    __syncwarp();
+#pragma unroll
+    for (int u = 0; u < EPL; ++u) {                     // C <- W = Psi X'
+      const int e = lane + 32 * u;
+      if (e >= nn) continue;
+      const int i = e / n, j = e % n;
+      double s = 0;
+#pragma unroll
+      for (int kk = 0; kk < n; ++kk) if (kk <= j) s += A[i * n + kk] * Bm[j * n + kk];
+      C[e] = s;
+    }
+    __syncwarp();
+  }
+  __syncthreads();
+  // ---- middle stage m (warp 0): both chains' last W feed Sigma_m
+  if (half == 0) {
+    const double* Wup = sm[0] + 2 * nn; const double* Wdn = sm[1] + 2 * nn;
+    prefetch(m); commit();
+    __syncwarp();
+    theta(m, A, m > 0 ? Wup : nullptr, (T_ - 1 - m) > 0 ? Wdn : nullptr);
+    __syncwarp();
+    chol_inv(A, Bm);
+    if (m > 0) b_out(m - 1, Bm, Wup);
+    if (T_ - 1 - m > 0) b_out(m + 1, Bm, Wdn);
+    x_out(m, Bm);
+  }
+  bad = __syncthreads_or(bad);
+  if (a.status && threadIdx.x == 0 && bad) atomicOr(&a.status[p], TMPC_ST_PIVOT);
+}
+
+}  // namespace tmpc
