@@ -8,6 +8,7 @@
 #include "tmpc_factor2.cuh"
 #include "tmpc_admm.cuh"
 #include "tmpc_admm2.cuh"
+#include "tmpc_stream.cuh"
 #include "tmpc_misc.cuh"
 #include "tmpc_backward.cuh"
 #include "tmpc_cr.cuh"
@@ -123,6 +124,18 @@ tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
   }
   size_t smem_res = admm_smem_elems(d, true) * sizeof(T), smem_str = admm_smem_elems(d, false) * sizeof(T);
   const bool res = smem_res <= kMaxSmem;
+  if (!res) {                            // streamed class: bulk-copy ring (tmpc_stream.cuh) when the shape allows it
+    const StreamPlan sp = stream_plan<T>(d, kMaxSmem);
+    const int V = 16 / (int)sizeof(T);
+    if ((d.n * d.n) % V == 0 && (d.nx * d.n) % V == 0 && d.n % V == 0 && 4 * d.ng <= sp.nthreads - 32 && sp.slots >= 3 && sp.nthreads <= 1024) {
+      StreamArgs<T> S; S.a = a; S.LD = sp.LD; S.slots = sp.slots; S.tile_elems = sp.tile_elems;
+      auto k = admm_stream_kernel<T>;
+      if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp.smem) != cudaSuccess) return TMPC_E_CUDA;
+      k<<<d.B, sp.nthreads, sp.smem, h->stream>>>(S); h->launches++;
+      if (!cuda_ok()) return TMPC_E_CUDA;
+      return a.kkt_only ? TMPC_OK : launch_residual<T>(h, a);
+    }
+  }
   if (!res && smem_str > kMaxSmem) return TMPC_E_UNSUPPORTED;
   int nt = ((d.nz + 31) / 32) * 32; if (nt > 1024) nt = 1024; if (nt < 64) nt = 64;
   if (res) {
