@@ -127,7 +127,7 @@ tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
   if (!res) {                            // streamed class: bulk-copy ring (tmpc_stream.cuh) when the shape allows it
     const StreamPlan sp = stream_plan<T>(d, kMaxSmem);
     const int V = 16 / (int)sizeof(T);
-    if ((d.n * d.n) % V == 0 && (d.nx * d.n) % V == 0 && d.n % V == 0 && 4 * d.ng <= sp.nthreads - 32 && sp.slots >= 3 && sp.nthreads <= 1024) {
+    if ((d.n * d.n) % V == 0 && (d.nx * d.n) % V == 0 && d.n % V == 0 && 4 * d.ng <= sp.nthreads - 32 && sp.slots >= 2 && sp.nthreads <= 1024) {
       StreamArgs<T> S; S.a = a; S.LD = sp.LD; S.slots = sp.slots; S.tile_elems = sp.tile_elems;
       auto k = admm_stream_kernel<T>;
       if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp.smem) != cudaSuccess) return TMPC_E_CUDA;

@@ -12,6 +12,7 @@
 // next right-hand side eta (eq. 51) while A^-_t / A^+_t are resident, so the constraint blocks are read once.
 // Factor format: the one-directional block LDL' of factor_kernel (Lam [N][n][n], Sinv [T][n][n]).
 #pragma once
+#include <cstdlib>
 #include "tmpc_common.cuh"
 #include "tmpc_admm.cuh"
 
@@ -47,6 +48,10 @@ __host__ inline StreamPlan stream_plan(const Dims& d, size_t max_smem) {
   const size_t tile = (size_t)P.tile_elems * sizeof(T);
   long s = ((long)max_smem - (long)fixed) / (long)tile;
   P.slots = s > 6 ? 6 : (int)s;
+  // the consumers are latency bound (dependent dots + CTA barriers), so two co-resident CTAs with a 2-deep ring each beat
+  // one CTA with a deep ring (measured at config 3: 116 ms vs 144 ms per 200 iterations)
+  if (P.slots >= 2 && 2 * (fixed + 2 * tile + 1024) <= (size_t)228 * 1024) P.slots = 2;
+  if (const char* e = getenv("TMPC_STREAM_SLOTS")) { const int v = atoi(e); if (v >= 2 && v <= P.slots) P.slots = v; }   // tuning knob
   P.smem = fixed + (size_t)(P.slots > 0 ? P.slots : 0) * tile;
   return P;
 }
@@ -201,7 +206,17 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
       release(1);
     }
     cons_bar();
-    // ---- outward sweep: x~_t = v_t - Lambda_t' x~_{t+1}, then everything local to stage t and dynamics block t
+    // ---- outward sweep: x~_t = v_t - Lambda_t' x~_{t+1}, then everything local to stage t and dynamics block t.
+    // The per-row state of stage t-1 (z_g, y_g, lo, hi, y_f, c, q: global memory, L2 resident) is prefetched into
+    // registers while stage t is processed, so no global-load latency sits on the dependent path.
+    T pzg = T(0), pyg = T(0), plo = T(0), phi = T(0), pyf = T(0), pc = T(0), pq = T(0);
+    auto prefetch_state = [&](int t) {
+      if (a.kkt_only || t < 0) return;
+      if (own_g) { const size_t row = gg + t * ng + ci; pzg = a.zg[row]; pyg = a.yg[row]; plo = a.qp.lo[row]; phi = a.qp.hi[row]; }
+      if (own_f && t < N) { pyf = a.yf[gf + nx + t * nx + ci]; pc = a.qp.b[((size_t)p * N + t) * nx + ci]; }
+      if (own_x) pq = a.qp.q[gx + t * n + ci];
+    };
+    prefetch_state(N);
     for (int t = N; t >= 0; --t) {
       if (t < N) {
         const T* L = acquire(0);
@@ -211,14 +226,15 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
         cons_bar();
       }
       if (a.kkt_only) continue;
+      const T zgo = pzg, ygo = pyg, lo_ = plo, hi_ = phi, yfo = pyf, cval = pc, qv = pq;
+      prefetch_state(t - 1);
       if (own_g) {                                     // eq. 9-16 on inequality row (t, ci)
         const size_t row = gg + t * ng + ci;
-        const T zgo = a.zg[row], ygo = a.yg[row];
         const T zh = alpha * g_row_dot(t, e1) + (T(1) - alpha) * zgo;
         const T v = zh + ygo * inv_rho_g;
         const bool soft = a.soft_rows ? (a.soft_rows[row] != 0) : (((d.soft_mask >> ci) & 1u) != 0);
         T z, s;
-        project_row<T>(soft, v, a.qp.lo[row], a.qp.hi[row], rho_g, inv_rg, lam, z, s);
+        project_row<T>(soft, v, lo_, hi_, rho_g, inv_rg, lam, z, s);
         const T y = ygo + rho_g * (zh - z);
         a.zg[row] = z; a.yg[row] = y; sbuf[ci] = rho_g * z - y;
         if (lastit) a.xi[row] = s;
@@ -230,17 +246,15 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
         Am = acquire(0); Ap = acquire(1);
         const T ztf = row_dot(Am, e1 + t * n, nx) + row_dot(Ap, e1 + (t + 1) * n, nx);
         if (own_f) {
-          const size_t fr = gf + nx + t * nx + ci;
-          const T cval = a.qp.b[((size_t)p * N + t) * nx + ci];
-          const T y = a.yf[fr] + rho_f * alpha * (ztf - cval);
-          a.yf[fr] = y; rbuf[ci] = rho_f * cval - y;
+          const T y = yfo + rho_f * alpha * (ztf - cval);
+          a.yf[gf + nx + t * nx + ci] = y; rbuf[ci] = rho_f * cval - y;
         }
       }
       cons_bar();
       T da = T(0), dp = T(0);
       if (t < N) { da = col_dot(Am, rbuf, nx); dp = col_dot(Ap, rbuf, nx); }
       if (own_x) {
-        T eta = sigma * xn - a.qp.q[gx + t * n + ci] + gts(t, sbuf);
+        T eta = sigma * xn - qv + gts(t, sbuf);
         if (t < N) { eta += da; e0[(t + 1) * n + ci] += dp; }
         if (t == 0 && own_f) {                         // rows x_0 = x_init (A_init = [I 0])
           const T xi0 = a.qp.x_init[(size_t)p * nx + ci];
