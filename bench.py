@@ -282,8 +282,19 @@ def run_gpu(args):
         peak = FP64_PEAK_TFLOPS if args.dtype == "f64" else FP32_PEAK_TFLOPS
         roof = {"bound": "alu", "achieved": alg / (kern_avg_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s", "peak_source": "derived: 148 SMs x 128 (fp32) / 64 (fp64) FMA lanes x 2 x 1965 MHz"}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None
-    roof["kernel"] = "admm_kernel (tmpc_admm_solve)" if args.config != 5 else "cr_admm_kernel (tmpc_admm_solve)"
+    # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed `ncu --set full` captures
+    # (profiles/r01_v2_ncu_full_*.md); only valid for the workload the capture was taken on
+    ncu_traffic = {(2, "f32", 1024): 57.11e6 + 0.43e6, (3, "f32", 512): 440.47e9 + 1.53e9}
+    roof["traffic"] = ncu_traffic.get((args.config, args.dtype, w.B))
+    roof["kernel"] = {1: "admm2_kernel", 2: "admm2_kernel", 3: "admm_stream_kernel", 4: "admm2_kernel", 5: "cr_admm_kernel"}[args.config] + " (tmpc_admm_solve)"
+    if args.config in (1, 2, 4):
+        # supplementary: the resident class reads every factor / constraint element from SHARED memory once per use, so the
+        # binding on-chip resource is LDS bandwidth (148 SMs x 128 B/clk x 1965 MHz), not the FMA pipe
+        es = 8 if args.dtype == "f64" else 4
+        lds_bytes = (2 * w.N * w.n * w.n + 2 * w.T * w.n * w.n + 4 * w.N * w.nx * w.n) * es * w.B * w.iters
+        lds_peak = 148 * 128 * 1.965e9 / 1e9
+        roof["lds"] = {"achieved": lds_bytes / (kern_avg_ms * 1e-3) / 1e9, "peak": lds_peak, "unit": "GB/s", "frac": lds_bytes / (kern_avg_ms * 1e-3) / 1e9 / lds_peak,
+                       "note": "algorithmic shared-memory bytes (B twice, X twice, A~-/A~+ twice per iteration) / kernel time"}
     roof["kernel_ms_per_launch"] = kern_avg_ms
     roof["kernel_share_of_step"] = sum(kern_ms) / sum(step_ms)
     line = {"metric": "batched QP solves/s", "value": value, "unit": "QP solves/s", "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),

@@ -1,20 +1,20 @@
 // tmpc_admm2.cuh — a4..a8 for the RESIDENT class (configs 1, 2, 4): the fused ADMM loop of Alg. 3
 // on the twisted block factor of tmpc_factor.cuh, all iterations in one launch.
 //
-// Design (DESIGN.md section 5):
-//  * a CTA owns PG problems (1 or 2).  Factor (Lam, Sinv) and constraint blocks (Am, Ap, G) are copied into shared
-//    memory once and stay there for all iterations; the per-row ADMM state (x, q, y_f, c, z_g, y_g, lo, hi, xi) lives
-//    in REGISTERS of the thread that owns the row: two (problem, stage, row) items per thread, fixed for the launch.
-//  * x~ = S^{-1} eta (eq. 8) runs on warp 0: lanes = (problem, direction, row), 8 lanes per slot, so the up chain and
-//    the down chain of the twisted factor of up to two problems advance together; a step is one n x n mat-vec whose
-//    operand vector is exchanged with width-8 shuffles, and v_t = Sigma_t^{-1} w_t is folded into the forward step
-//    (same shuffled values), so a solve is 2 * (T/2) dependent steps instead of 2T + a barrier-separated pass.
+// Design (DESIGN.md section 5.1):
+//  * a CTA owns PG problems (1 or 2).  The factor (X_t, -B_t) and the constraint blocks carried into the scaled
+//    variables (A~^- = A^- X', A~^+ = A^+ X_next', G~ = G X') sit in shared memory for all iterations; the per-row ADMM
+//    state (x, q, y_f, c, z_g, y_g, lo, hi) lives in REGISTERS of the thread that owns the row: two (problem, stage,
+//    row) items per thread, fixed for the launch.
+//  * x~ = S^{-1} eta (eq. 8) runs on a dedicated chain warp (warp 0): lanes = (problem, direction, row), 8 lanes per
+//    slot, so the up chain and the down chain of the twisted factor of up to two problems advance together; a step is
+//    one n x n mat-vec whose operand vector is published with one STS and read back as a broadcast vector load.
 //  * everything local to a stage (eta eq. 51, z~ = A x~ eq. 9, relaxation eq. 10, projection eq. 12-15, duals eq. 16)
-//    is done by all threads between three CTA barriers per iteration; several CTAs per SM overlap one CTA's chain
-//    phase with another's stage-parallel phase.
-//  * shared-memory layout is bank-conflict free for n = 8: rows of the factor blocks are XOR-swizzled by 16-byte
-//    chunks (row-wise vector loads in the forward sweep, column-wise scalar loads in the backward sweep), and the
-//    down-chain blocks / second problem are skewed by 8 / 16 elements so the four slots hit distinct banks.
+//    is done by the item warps; chain warp and item warps hand over through named barriers (arrive / sync), and
+//    several CTAs per SM overlap one CTA's chain phase with another's stage-parallel phase.
+//  * shared-memory layout is bank-conflict free for n = 8: rows of the blocks are XOR-swizzled by 16-byte chunks
+//    (row-wise vector loads AND column-wise scalar loads), the record stride is 8 (mod 32) words, the down-chain
+//    records are skewed by 8 words and the second problem by 16 so the four slots hit distinct banks.
 // Residuals (a9) are computed by residual_kernel below from the state written back to global memory.
 #pragma once
 #include "tmpc_common.cuh"
