@@ -133,9 +133,19 @@ __device__ __forceinline__ void sts_1(unsigned a, float v) { asm volatile("st.sh
 __device__ __forceinline__ void sts_1(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
 // contiguous NC-vector at byte address a; for NC = 8 the 16-byte chunks are taken in the order of a row swizzled by swb bytes
 template <typename T, int NC> __device__ __forceinline__ void lds_row(unsigned a, unsigned swb, T (&r)[NC]) {
-  if constexpr (NC == 8 && sizeof(T) == 4) lds_vec8(a + (0u ^ swb), a + (16u ^ swb), r);
+  if constexpr (NC == 8 && sizeof(T) == 4) lds_vec8(a + swb, a + 16u - swb, r);     // swb in {0,16}: chunks (0,16) or (16,0), one add each
   else if constexpr (NC == 8) lds_vec8(a + (0u ^ swb), a + (16u ^ swb), a + (32u ^ swb), a + (48u ^ swb), r);
   else lds_vec6(a, r);
+}
+
+// empty asm that "uses" a whole register vector: keeps ptxas from splitting a multi-chunk load into load - use - load - use
+template <int L> __device__ __forceinline__ void pin_vec(float (&r)[L]) {
+  if constexpr (L == 8) asm volatile("" : "+f"(r[0]), "+f"(r[1]), "+f"(r[2]), "+f"(r[3]), "+f"(r[4]), "+f"(r[5]), "+f"(r[6]), "+f"(r[7]));
+  else if constexpr (L == 6) asm volatile("" : "+f"(r[0]), "+f"(r[1]), "+f"(r[2]), "+f"(r[3]), "+f"(r[4]), "+f"(r[5]));
+}
+template <int L> __device__ __forceinline__ void pin_vec(double (&r)[L]) {
+  if constexpr (L == 8) asm volatile("" : "+d"(r[0]), "+d"(r[1]), "+d"(r[2]), "+d"(r[3]), "+d"(r[4]), "+d"(r[5]), "+d"(r[6]), "+d"(r[7]));
+  else if constexpr (L == 6) asm volatile("" : "+d"(r[0]), "+d"(r[1]), "+d"(r[2]), "+d"(r[3]), "+d"(r[4]), "+d"(r[5]));
 }
 
 template <typename T>
@@ -207,6 +217,7 @@ __device__ __forceinline__ void chain_warp_solve(T* sm, int R, int PP, int T_, i
     __syncwarp();
     T W[n];
     lds_row<T, NC>(bt + oE1, swb, W);
+    pin_vec<n>(W);
     const unsigned bnext = last ? bm : bt + dRb;
     const T eta = (on && !(last && dir)) ? lds_1(bnext + oE1 + me, T(0)) : T(0);
     if (on) bt = bnext;

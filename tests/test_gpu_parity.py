@@ -253,3 +253,67 @@ def test_config5_long_horizon_sqp(N, n_sqp, iters):
     assert rc == 0
     compare_states(got, ref, 1e-9)
     s.close()
+
+
+# ----------------------------------------------------------------------------------------------- full BASELINE sizes
+# The batch sizes, horizons and iteration counts of BASELINE.json, i.e. the launch configuration bench.py times
+# (CTAs per SM, problems per CTA, waves, ring depth); compared on SAMPLED problems the oracle solves one by one.
+def _sample(B, k=6, seed=7):
+    idx = set(range(min(3, B))) | {B - 1} | set(np.random.default_rng(seed).integers(0, B, size=k).tolist())
+    return np.array(sorted(idx))
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_config2_full_batch_sampled(dtype):
+    from paper_2606_24039_b200.solver import Solver
+    w = W.config2()
+    assert w.B == 1024 and w.N == 50 and w.iters == 100
+    wr = w.rounded(np.float32) if dtype == "f32" else w
+    s = Solver(wr, dtype=dtype)
+    s.solve()
+    got, info = s.state_numpy(), s.info_numpy()
+    assert (info["status"] == 0).all() and all(np.isfinite(got[k]).all() for k in KEYS)
+    idx = _sample(w.B)
+    ws = wr.subset(idx)
+    ref, rinfo, rc = O.admm(ws, O.make_cfg(ws), nthreads=8)
+    assert rc == 0
+    compare_states({k: got[k][idx] for k in KEYS}, ref, TOL[dtype])
+    otol = 1e-4 if dtype == "f32" else 1e-9
+    assert (np.abs(info["objective"][idx] - rinfo[:, 2]) <= otol * np.maximum(np.abs(rinfo[:, 2]), 1.0)).all()
+    s.close()
+
+
+def test_config3_full_batch_sampled_fp32():
+    from paper_2606_24039_b200.solver import Solver
+    w = W.config3()
+    assert w.B == 512 and w.N == 32 and w.n == 88 and w.iters == 200
+    wr = w.rounded(np.float32)
+    s = Solver(wr, dtype="f32")
+    s.solve()
+    got, info = s.state_numpy(), s.info_numpy()
+    assert (info["status"] == 0).all() and all(np.isfinite(got[k]).all() for k in KEYS)
+    idx = _sample(w.B, k=3)
+    ws = wr.subset(idx)
+    ref, rinfo, rc = O.admm(ws, O.make_cfg(ws, band=1), nthreads=8)
+    assert rc == 0
+    compare_states({k: got[k][idx] for k in KEYS}, ref, TOL["f32"])
+    assert (np.abs(info["objective"][idx] - rinfo[:, 2]) <= 1e-4 * np.maximum(np.abs(rinfo[:, 2]), 1.0)).all()
+    s.close()
+
+
+def test_config4_full_batch_sampled_fp32():
+    from paper_2606_24039_b200.solver import Solver
+    w = W.config4(dtype="f32")
+    assert w.B == 4096 and w.N == 100 and w.iters == 50 and w.sqp_iters == 5
+    wr = w.rounded(np.float32)
+    s = Solver(wr, dtype="f32")
+    s.reset_state(wr.xbar0)
+    s.sqp()
+    got = s.state_numpy()
+    assert all(np.isfinite(got[k]).all() for k in KEYS)
+    idx = _sample(w.B)
+    ws = wr.subset(idx)
+    ref, info, rc = O.sqp_bicycle(ws, O.make_cfg(ws), nthreads=8)
+    assert rc == 0
+    compare_states({k: got[k][idx] for k in KEYS}, ref, TOL["f32"])
+    s.close()
