@@ -6,6 +6,7 @@
 #include "tmpc_common.cuh"
 #include "tmpc_factor.cuh"
 #include "tmpc_factor2.cuh"
+#include "tmpc_factor3.cuh"
 #include "tmpc_admm.cuh"
 #include "tmpc_admm2.cuh"
 #include "tmpc_stream.cuh"
@@ -93,6 +94,15 @@ tmpc_status launch_factor(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_
   FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = w_rows;
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
   const int nn = h->d.n * h->d.n;
+  {                                      // large blocks: register-tiled products (tmpc_factor3.cuh)
+    const int nt4 = f3_ld(h->d.n) / 4; const size_t smem3 = factor3_smem<T>(h->d.n);
+    if (h->d.n >= 32 && nt4 * nt4 <= 512 && smem3 <= kMaxSmem) {
+      auto k3 = factor3_kernel<T>;
+      if (cudaFuncSetAttribute(k3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3) != cudaSuccess) return TMPC_E_CUDA;
+      k3<<<h->d.B, 512, smem3, h->stream>>>(a); h->launches++;
+      return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+    }
+  }
   int nt = ((nn + 31) / 32) * 32; if (nt > 1024) nt = 1024; if (nt < 32) nt = 32;
   const size_t smem = 3 * (size_t)nn * sizeof(double);
   if (smem > kMaxSmem) return TMPC_E_UNSUPPORTED;

@@ -1,0 +1,209 @@
+// tmpc_factor3.cuh — a2 + a3 for the STREAMED class (n ~ 88): the one-directional block LDL' of factor_kernel
+// (same outputs: Lam_t = Phi_t Sigma_t^{-1}, Sinv_t = Sigma_t^{-1}), restructured as register-tiled shared-memory
+// matrix products.  factor_kernel spends its time on dependent global loads and two shared loads per FMA; here every
+// product has the form  out(i,j) = sum_k A[k][i] B[k][j]  with BOTH operands contiguous along the tile (so a thread's
+// 4 x 4 tile costs 4 vector loads per 16 DFMA), operands are staged in shared memory, and three n x n buffers suffice:
+//   P: Sigma_t -> L (in-place Cholesky) -> Sigma_t^{-1} -> (next stage) Sigma_{t+1}
+//   Q: X = L^{-1} -> Phi_t' (transposed)
+//   R: Lambda_t' (transposed)
+// with  Sigma^{-1} = X'X,  Lambda = Phi Sigma^{-1}  (out(j... ) from Q = Phi', P),  Sigma_{t+1} = Theta_{t+1} - Lambda Phi'
+// (from R = Lambda', Q = Phi').  Arithmetic in double for both working dtypes.  One CTA per problem.
+#pragma once
+#include "tmpc_factor.cuh"
+
+namespace tmpc {
+
+template <typename T> __host__ __device__ constexpr int f3_ch() { return sizeof(T) == 4 ? 32 : 16; }   // rows of A^-/A^+/G staged per chunk (in the working dtype)
+
+__host__ __device__ inline int f3_ld(int n) { return (n + 3) / 4 * 4; }
+template <typename T> __host__ inline size_t factor3_smem(int n) { const int ld = f3_ld(n); return (size_t)3 * ld * ld * sizeof(double) + (size_t)2 * f3_ch<T>() * ld * sizeof(T) + 64; }
+
+template <typename T>
+__global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const Dims& d = a.d;
+  const int n = d.n, nx = d.nx, ng = d.ng, N = d.N, T_ = d.T, nn = n * n, ld = f3_ld(n), nt4 = ld / 4;
+  double* P = reinterpret_cast<double*>(smem_raw);
+  double* Q = P + (size_t)ld * ld;
+  double* R = Q + (size_t)ld * ld;
+  constexpr int F3_CH = f3_ch<T>();
+  T* S1 = reinterpret_cast<T*>(R + (size_t)ld * ld);              // staged chunk, [F3_CH][ld], working dtype (exact copy)
+  T* S2 = S1 + (size_t)F3_CH * ld;
+  const int p = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
+  const T* Dp = a.qp.D + a.qp.sD * p;
+  const T* Ep = a.qp.E + a.qp.sE * p;
+  const T* Amp = a.qp.Am + (size_t)p * N * nx * n;
+  const T* App = a.qp.Ap + (size_t)p * N * nx * n;
+  const T* Gp = a.qp.G ? a.qp.G + a.qp.sG * p : nullptr;
+  const T* wr = a.w_rows ? a.w_rows + (size_t)p * T_ * ng : nullptr;
+  T* Lamp = a.Lam + (size_t)p * N * nn;
+  T* Sinvp = a.Sinv + (size_t)p * T_ * nn;
+  const int tiles = nt4 * nt4;
+  int bad = 0;
+  for (int e = tid; e < 3 * ld * ld; e += nt) P[e] = 0.0;          // pads stay zero
+  __syncthreads();
+
+  // stage rows [r0, r0+rows) of a row-major [*][n] global matrix into S (float), zero padded; optional per-row scale
+  auto stage = [&](T* S, const T* src, int r0, int rows, const T* scale, double scale_all) {
+    for (int e = tid; e < F3_CH * ld; e += nt) {
+      const int r = e / ld, c = e - r * ld;
+      T v = T(0);
+      if (r < rows && c < n && src) { double x = (double)src[(size_t)(r0 + r) * n + c]; if (scale) x *= (double)scale[r0 + r]; v = (T)(x * scale_all); }
+      S[e] = v;
+    }
+  };
+  // acc(i,j) += sum_k A[k][i0+i] B[k][j0+j]  for this thread's 4 x 4 tile; A, B row-major with leading dimension ld
+  auto mm_d = [&](double (&acc)[4][4], const double* A, const double* B, int k0, int k1, int i0, int j0) {
+    for (int k = k0; k < k1; ++k) {
+      const double2 a0 = *reinterpret_cast<const double2*>(A + (size_t)k * ld + i0), a1 = *reinterpret_cast<const double2*>(A + (size_t)k * ld + i0 + 2);
+      const double2 b0 = *reinterpret_cast<const double2*>(B + (size_t)k * ld + j0), b1 = *reinterpret_cast<const double2*>(B + (size_t)k * ld + j0 + 2);
+      const double av[4] = {a0.x, a0.y, a1.x, a1.y}, bv[4] = {b0.x, b0.y, b1.x, b1.y};
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] += av[i] * bv[j];
+    }
+  };
+  auto mm_f = [&](double (&acc)[4][4], const T* A, const T* B, int rows, int i0, int j0) {
+    for (int k = 0; k < rows; ++k) {
+      double av[4], bv[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { av[i] = (double)A[(size_t)k * ld + i0 + i]; bv[i] = (double)B[(size_t)k * ld + j0 + i]; }
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] += av[i] * bv[j];
+    }
+  };
+  const bool has_tile = tid < tiles;
+  const int ti = has_tile ? tid / nt4 : 0, tj = has_tile ? tid - ti * nt4 : 0, i0 = 4 * ti, j0 = 4 * tj;
+
+  for (int t = 0; t < T_; ++t) {
+    // ---- P <- Theta_t - Lambda_{t-1} Phi_{t-1}'   (R = Lambda', Q = Phi' of the previous stage)
+    {
+      double accS[4][4] = {}, accA[4][4] = {}, accG[4][4] = {};
+      if (t > 0 && has_tile) mm_d(accS, R, Q, 0, n, i0, j0);
+      for (int which = 0; which < 2; ++which) {       // A^-_t' A^-_t  and  A^+_{t-1}' A^+_{t-1}
+        const T* src = which == 0 ? (t < N ? Amp + (size_t)t * nx * n : nullptr) : (t > 0 ? App + (size_t)(t - 1) * nx * n : nullptr);
+        if (!src) continue;
+        for (int r0 = 0; r0 < nx; r0 += F3_CH) {
+          const int rows = nx - r0 < F3_CH ? nx - r0 : F3_CH;
+          __syncthreads();
+          stage(S1, src, r0, rows, nullptr, 1.0);
+          __syncthreads();
+          if (has_tile) mm_f(accA, S1, S1, rows, i0, j0);
+        }
+      }
+      if (!d.g_sel && Gp) for (int r0 = 0; r0 < ng; r0 += F3_CH) {   // G' diag(w) G
+        const int rows = ng - r0 < F3_CH ? ng - r0 : F3_CH;
+        __syncthreads();
+        stage(S1, Gp + (size_t)t * ng * n, r0, rows, nullptr, 1.0);
+        stage(S2, Gp + (size_t)t * ng * n, r0, rows, wr ? wr + (size_t)t * ng : nullptr, wr ? 1.0 : a.w_in);
+        __syncthreads();
+        if (has_tile) mm_f(accG, S1, S2, rows, i0, j0);
+      }
+      __syncthreads();                                 // everyone is done reading R, Q, S before P is rewritten
+      if (has_tile) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const int gi = i0 + i, gj = j0 + j;
+            double s = 0.0;
+            if (gi < n && gj < n) {
+              s = (double)Dp[(size_t)t * nn + gi * n + gj] + a.w_eq * accA[i][j] + accG[i][j] - accS[i][j];
+              if (gi == gj) {
+                s += a.sigma;
+                if (t == 0 && gi < nx) s += a.w_eq;      // A_init' A_init = blkdiag(I_nx, 0)
+                if (d.g_sel) for (int r = 0; r < ng; ++r) if (d.g_col[r] == gi) s += wr ? (double)wr[(size_t)t * ng + r] : a.w_in;
+              }
+            } else if (gi == gj) s = 1.0;              // identity on the padding keeps the factor well defined
+            P[(size_t)gi * ld + gj] = s;
+          }
+      }
+      __syncthreads();
+    }
+    // ---- in-place Cholesky of P (lower), then Q <- X = L^{-1}  (X[k][i] row-major: row k of L^{-1})
+    for (int k = 0; k < n; ++k) {
+      double dk = P[(size_t)k * ld + k];
+      if (!(dk > 0) || !isfinite(dk)) { bad = 1; dk = 1; }
+      const double inv = 1.0 / dk;
+      const int m = n - 1 - k;
+      for (int e = tid; e < m * m; e += nt) {
+        const int i = k + 1 + e / m, j = k + 1 + e % m;
+        if (j <= i) P[(size_t)i * ld + j] -= P[(size_t)i * ld + k] * P[(size_t)j * ld + k] * inv;
+      }
+      __syncthreads();
+      const double sq = sqrt(dk), rs = 1.0 / sq;
+      for (int i = k + tid; i < n; i += nt) P[(size_t)i * ld + k] = (i == k) ? sq : P[(size_t)i * ld + k] * rs;
+    }
+    for (int e = tid; e < ld * ld; e += nt) { const int i = e / ld, j = e - i * ld; Q[e] = (i == j && i < n) ? 1.0 : 0.0; }
+    __syncthreads();
+    for (int k = 0; k < n - 1; ++k) {
+      const double inv = 1.0 / P[(size_t)k * ld + k];
+      const int m = n - 1 - k, kk = k + 1;
+      for (int e = tid; e < m * kk; e += nt) {
+        const int i = k + 1 + e / kk, j = e % kk;
+        Q[(size_t)i * ld + j] -= P[(size_t)i * ld + k] * Q[(size_t)k * ld + j] * inv;
+      }
+      __syncthreads();
+    }
+    for (int e = tid; e < n * n; e += nt) { const int i = e / n, j = e - i * n; Q[(size_t)i * ld + j] /= P[(size_t)i * ld + i]; }
+    __syncthreads();
+    // ---- P <- Sigma^{-1} = X'X  (sum over k >= max(i,j): X lower triangular), also to global
+    if (has_tile) {
+      double acc[4][4] = {};
+      mm_d(acc, Q, Q, i0 > j0 ? i0 : j0, n, i0, j0);
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int gi = i0 + i, gj = j0 + j;
+          P[(size_t)gi * ld + gj] = (gi < n && gj < n) ? acc[i][j] : 0.0;
+          if (gi < n && gj < n) Sinvp[(size_t)t * nn + gi * n + gj] = (T)acc[i][j];
+        }
+    }
+    __syncthreads();
+    if (t == N) break;
+    // ---- Q <- Phi_t' : Q[k][i] = Phi[i][k] = E_t[i][k] + w sum_r A^+_t[r][i] A^-_t[r][k]   (tile (k-block, i-block))
+    {
+      double acc[4][4] = {};
+      for (int r0 = 0; r0 < nx; r0 += F3_CH) {
+        const int rows = nx - r0 < F3_CH ? nx - r0 : F3_CH;
+        __syncthreads();
+        stage(S1, Amp + (size_t)t * nx * n, r0, rows, nullptr, 1.0);
+        stage(S2, App + (size_t)t * nx * n, r0, rows, nullptr, 1.0);
+        __syncthreads();
+        if (has_tile) mm_f(acc, S1, S2, rows, i0, j0);   // acc(k, i) = sum_r A^-[r][k] A^+[r][i]
+      }
+      if (has_tile) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const int gk = i0 + i, gi = j0 + j;
+            Q[(size_t)gk * ld + gi] = (gk < n && gi < n) ? (double)Ep[(size_t)t * nn + gi * n + gk] + a.w_eq * acc[i][j] : 0.0;
+          }
+      }
+      __syncthreads();
+    }
+    // ---- Lambda = Phi Sigma^{-1}: Lambda(i,j) = sum_k Q[k][i] P[k][j] ; R <- Lambda' , Lambda to global
+    if (has_tile) {
+      double acc[4][4] = {};
+      mm_d(acc, Q, P, 0, n, i0, j0);
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int gi = i0 + i, gj = j0 + j;
+          R[(size_t)gj * ld + gi] = (gi < n && gj < n) ? acc[i][j] : 0.0;
+          if (gi < n && gj < n) Lamp[(size_t)t * nn + gi * n + gj] = (T)acc[i][j];
+        }
+    }
+    __syncthreads();
+  }
+  bad = __syncthreads_or(bad);
+  if (a.status && tid == 0 && bad) atomicOr(&a.status[p], TMPC_ST_PIVOT);
+}
+
+}  // namespace tmpc
