@@ -13,6 +13,7 @@
 #include "tmpc_misc.cuh"
 #include "tmpc_backward.cuh"
 #include "tmpc_cr.cuh"
+#include "tmpc_cr2.cuh"
 
 using namespace tmpc;
 
@@ -240,6 +241,30 @@ tmpc_status do_factor(tmpc_ctx* h, const tmpc_qp* qp) {
 template <typename T>
 tmpc_status do_solve(tmpc_ctx* h, const tmpc_qp* qp, tmpc_state* st, int iters, int flags, tmpc_info* info) {
   if (h->cr) {
+    // chunked form (tmpc_cr2.cuh) when the horizon is long enough and one CTA per chunk (+1) is co-resident
+    const Dims& d = h->d;
+    const int nchunks = (d.T + CR2_CS - 1) / CR2_CS, S = d.N / CR2_CS + 1;
+    int dev = 0, sms = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const bool shape = (d.n == 6 && d.nx == 4) || (d.n == 8 && d.nx == 6);
+    if (shape && d.T >= 4 * CR2_CS && (long long)(nchunks + 1) * d.B <= sms && 3 * S * d.n + S * d.nx <= 3 * 4096) {
+      const size_t smem = (d.n == 6 ? cr2_smem_elems<T, 6, 4>(d.ng, S) : cr2_smem_elems<T, 8, 6>(d.ng, S)) * sizeof(T);
+      if (smem <= kMaxSmem) {
+        CrAdmmArgs<T> a; memset(&a, 0, sizeof(a));
+        a.d = d; a.prm = params<T>(h->cfg); a.qp = view<T>(qp); a.ws = h->ws + h->lay.cr;
+        a.x = (T*)st->x; a.zg = (T*)st->zg; a.yf = (T*)st->yf; a.yg = (T*)st->yg; a.xi = (T*)st->xi;
+        a.status = info ? info->status : nullptr; a.iters = iters; a.zg_given = (flags & TMPC_SOLVE_ZG_GIVEN) != 0;
+        void* kern = d.n == 6 ? (void*)cr2_admm_kernel<T, 6, 4> : (void*)cr2_admm_kernel<T, 8, 6>;
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return TMPC_E_CUDA;
+        int nch = nchunks; void* params_[] = { (void*)&a, (void*)&nch };
+        if (cudaLaunchCooperativeKernel(kern, dim3((unsigned)nchunks + 1, (unsigned)d.B), dim3(256), params_, smem, h->stream) != cudaSuccess) { cudaGetLastError(); return TMPC_E_CUDA; }
+        h->launches++;
+        if (!info) return TMPC_OK;
+        AdmmArgs<T> r; memset(&r, 0, sizeof(r));
+        r.d = d; r.prm = a.prm; r.qp = a.qp; r.x = a.x; r.zg = a.zg; r.yf = a.yf; r.yg = a.yg; r.xi = a.xi;
+        r.r_prim = (T*)info->r_prim; r.r_dual = (T*)info->r_dual; r.objective = (T*)info->objective; r.status = info->status;
+        return launch_residual<T>(h, r);
+      }
+    }
     return cr_admm<T>(h->d, params<T>(h->cfg), view<T>(qp), h->ws + h->lay.cr, (T*)st->x, (T*)st->zg, (T*)st->yf, (T*)st->yg, (T*)st->xi,
                       info ? (T*)info->r_prim : nullptr, info ? (T*)info->r_dual : nullptr, info ? (T*)info->objective : nullptr,
                       info ? info->status : nullptr, iters, (flags & TMPC_SOLVE_ZG_GIVEN) != 0, h->stream, &h->launches);
@@ -300,6 +325,10 @@ tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, vo
   // zero buffers of the adjoint QP (x_init = 0, b = 0)
   if (cudaMemsetAsync(h->ws + L.zero_xinit, 0, L.zero_b - L.zero_xinit, h->stream) != cudaSuccess ||
       cudaMemsetAsync(h->ws + L.zero_b, 0, L.cr - L.zero_b, h->stream) != cudaSuccess) { delete h; return TMPC_E_CUDA; }
+  {                                      // barrier words of the cyclic-reduction kernels (tmpc_cr.cuh GridBar) start at zero
+    const size_t crb = cr_workspace_bytes(h->d, esize(cfg->dtype)), flags = 256 * (size_t)h->d.B + 1024;
+    if (cudaMemsetAsync(h->ws + L.cr + crb - flags, 0, flags, h->stream) != cudaSuccess) { delete h; return TMPC_E_CUDA; }
+  }
   *out = h;
   return TMPC_OK;
 }

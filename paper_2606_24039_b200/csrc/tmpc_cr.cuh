@@ -91,18 +91,38 @@ __device__ int spd_inverse(const T* __restrict__ A, T* __restrict__ X) {
   return bad;
 }
 
+// Light-weight barrier over the gridDim.x CTAs of ONE problem (cooperative launch guarantees co-residency): one atomic
+// per CTA on a counter, release by bumping a generation word; a gpu-scope fence on both sides orders global memory
+// (and invalidates L1 on the waiting side).  About 1 us per barrier against ~2.5 us for cooperative_groups grid.sync.
+struct GridBar {
+  unsigned* cnt; unsigned* gen; unsigned nblocks;
+  __device__ __forceinline__ void sync() const {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      const unsigned g = *reinterpret_cast<volatile unsigned*>(gen);
+      __threadfence();
+      if (atomicAdd(cnt, 1u) == nblocks - 1) { *reinterpret_cast<volatile unsigned*>(cnt) = 0u; __threadfence(); atomicAdd(gen, 1u); }
+      else { while (*reinterpret_cast<volatile unsigned*>(gen) == g) {} }
+      __threadfence();
+    }
+    __syncthreads();
+  }
+};
+template <typename T>
+__device__ __forceinline__ GridBar cr_gridbar(const CrBuf<T>& b) { return GridBar{reinterpret_cast<unsigned*>(b.flag) + 16, reinterpret_cast<unsigned*>(b.flag) + 32, gridDim.x}; }
+
 template <typename T>
 struct CrFactorArgs { Dims d; QpView<T> qp; T sigma, rho_f, rho_g; unsigned char* ws; };
 
 // ---- factor: assemble Theta_t, Lo_t = Phi_{t-1}, then ceil(log2 T) elimination levels
 template <typename T, int NC>
 __global__ void __launch_bounds__(256) cr_factor_kernel(CrFactorArgs<T> a) {
-  cg::grid_group grid = cg::this_grid();
   const Dims& d = a.d;
   constexpr int n = NC, nn = NC * NC;
   const int nx = d.nx, ng = d.ng, N = d.N, T_ = d.T, p = blockIdx.y;
   const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x, gsz = (long long)gridDim.x * blockDim.x;
   CrBuf<T> b = cr_carve<T>(d, a.ws, p);
+  const GridBar grid = cr_gridbar<T>(b);
   const T* Dp = a.qp.D + a.qp.sD * p; const T* Ep = a.qp.E + a.qp.sE * p;
   const T* Amp = a.qp.Am + (size_t)p * N * nx * n; const T* App = a.qp.Ap + (size_t)p * N * nx * n;
   const T* Gp = a.qp.G ? a.qp.G + a.qp.sG * p : nullptr;
@@ -204,53 +224,65 @@ __global__ void __launch_bounds__(256) cr_factor_kernel(CrFactorArgs<T> a) {
 
 namespace tmpc {
 
-// ---- the solve with the CR factor, all threads of the grid, gather form; eta is consumed, x written to xt.
+// ---- the solve with the CR factor, gather form; eta is consumed, x written to xt.
+// Levels with many stages run grid-wide (one barrier per level); once at most CR_SMALL stages survive, CTA 0 finishes
+// the down-sweep, the root and the first up-sweep levels alone with __syncthreads, the other CTAs wait at one barrier.
+constexpr int CR_SMALL = 512;
 template <typename T, int NC>
-__device__ void cr_solve(cg::grid_group& grid, const CrBuf<T>& b, int T_, long long gid, long long gsz) {
+__device__ __forceinline__ void cr_down_level(const CrBuf<T>& b, int T_, long long h, long long w0, long long wstep) {
   constexpr int n = NC, nn = NC * NC;
+  for (long long w = w0;; w += wstep) {               // survivors s = 2hk pull from s+h and s-h
+    const long long k = w / n; const int i = (int)(w - k * n);
+    const long long s_ = 2 * h * k;
+    if (s_ >= T_) break;
+    T acc = T(0);
+    if (s_ + h < T_) { const T* F = b.FA + (s_ + h) * nn + i * n; const T* e = b.eta + (s_ + h) * n;
+#pragma unroll
+      for (int m = 0; m < n; ++m) acc += F[m] * e[m]; }
+    if (s_ - h >= 0) { const T* F = b.FB + (s_ - h) * nn + i * n; const T* e = b.eta + (s_ - h) * n;
+#pragma unroll
+      for (int m = 0; m < n; ++m) acc += F[m] * e[m]; }
+    b.eta[s_ * n + i] -= acc;
+  }
+}
+template <typename T, int NC>
+__device__ __forceinline__ void cr_up_level(const CrBuf<T>& b, int T_, long long h, long long w0, long long wstep) {
+  constexpr int n = NC, nn = NC * NC;
+  for (long long w = w0;; w += wstep) {               // eliminated j = h(2k+1)
+    const long long k = w / n; const int i = (int)(w - k * n);
+    const long long j = h * (2 * k + 1);
+    if (j >= T_) break;
+    const T* U = b.U + j * nn + i * n; const T* e = b.eta + j * n;
+    T acc = T(0);
+#pragma unroll
+    for (int m = 0; m < n; ++m) acc += U[m] * e[m];
+    { const T* F = b.FA + j * nn + i; const T* xa = b.xt + (j - h) * n;
+#pragma unroll
+      for (int m = 0; m < n; ++m) acc -= F[m * n] * xa[m]; }
+    if (j + h < T_) { const T* F = b.FB + j * nn + i; const T* xb = b.xt + (j + h) * n;
+#pragma unroll
+      for (int m = 0; m < n; ++m) acc -= F[m * n] * xb[m]; }
+    b.xt[j * n + i] = acc;
+  }
+}
+template <typename T, int NC>
+__device__ void cr_solve(const GridBar& gb, const CrBuf<T>& b, int T_, long long gid, long long gsz) {
+  constexpr int n = NC;
   const int L = cr_levels(T_);
-  for (int l = 0; l < L; ++l) {                       // down-sweep: survivors s = 2hk pull from s+h and s-h
-    const long long h = 1LL << l;
-    for (long long w = gid;; w += gsz) {
-      const long long k = w / n; const int i = (int)(w - k * n);
-      const long long s_ = 2 * h * k;
-      if (s_ >= T_) break;
-      T acc = T(0);
-      if (s_ + h < T_) { const T* F = b.FA + (s_ + h) * nn + i * n; const T* e = b.eta + (s_ + h) * n;
+  int LS = 0;                                          // levels run grid-wide
+  while (LS < L && ((T_ + (1 << LS) - 1) >> LS) > CR_SMALL) ++LS;
+  for (int l = 0; l < LS; ++l) { cr_down_level<T, NC>(b, T_, 1LL << l, gid, gsz); gb.sync(); }
+  if (blockIdx.x == 0) {
+    for (int l = LS; l < L; ++l) { cr_down_level<T, NC>(b, T_, 1LL << l, threadIdx.x, blockDim.x); __syncthreads(); }
+    if (threadIdx.x < n) { T acc = T(0);
 #pragma unroll
-        for (int m = 0; m < n; ++m) acc += F[m] * e[m]; }
-      if (s_ - h >= 0) { const T* F = b.FB + (s_ - h) * nn + i * n; const T* e = b.eta + (s_ - h) * n;
-#pragma unroll
-        for (int m = 0; m < n; ++m) acc += F[m] * e[m]; }
-      b.eta[s_ * n + i] -= acc;
-    }
-    grid.sync();
+      for (int m = 0; m < n; ++m) acc += b.U[threadIdx.x * n + m] * b.eta[m];
+      b.xt[threadIdx.x] = acc; }
+    __syncthreads();
+    for (int l = L - 1; l >= LS; --l) { cr_up_level<T, NC>(b, T_, 1LL << l, threadIdx.x, blockDim.x); __syncthreads(); }
   }
-  if (gid < n) { T acc = T(0);
-#pragma unroll
-    for (int m = 0; m < n; ++m) acc += b.U[gid * n + m] * b.eta[m];
-    b.xt[gid] = acc; }
-  grid.sync();
-  for (int l = L - 1; l >= 0; --l) {                  // up-sweep: eliminated j = h(2k+1)
-    const long long h = 1LL << l;
-    for (long long w = gid;; w += gsz) {
-      const long long k = w / n; const int i = (int)(w - k * n);
-      const long long j = h * (2 * k + 1);
-      if (j >= T_) break;
-      const T* U = b.U + j * nn + i * n; const T* e = b.eta + j * n;
-      T acc = T(0);
-#pragma unroll
-      for (int m = 0; m < n; ++m) acc += U[m] * e[m];
-      { const T* F = b.FA + j * nn + i; const T* xa = b.xt + (j - h) * n;
-#pragma unroll
-        for (int m = 0; m < n; ++m) acc -= F[m * n] * xa[m]; }
-      if (j + h < T_) { const T* F = b.FB + j * nn + i; const T* xb = b.xt + (j + h) * n;
-#pragma unroll
-        for (int m = 0; m < n; ++m) acc -= F[m * n] * xb[m]; }
-      b.xt[j * n + i] = acc;
-    }
-    grid.sync();
-  }
+  gb.sync();
+  for (int l = LS - 1; l >= 0; --l) { cr_up_level<T, NC>(b, T_, 1LL << l, gid, gsz); gb.sync(); }
 }
 
 template <typename T>
@@ -264,13 +296,13 @@ struct CrAdmmArgs {
 // ---- fused ADMM loop (Alg. 3) on the CR factor: one cooperative grid, blockIdx.y = problem
 template <typename T, int NC>
 __global__ void __launch_bounds__(256) cr_admm_kernel(CrAdmmArgs<T> a) {
-  cg::grid_group grid = cg::this_grid();
   __shared__ T red[64];
   const Dims& d = a.d;
   constexpr int n = NC, nn = NC * NC;
   const int nx = d.nx, ng = d.ng, N = d.N, T_ = d.T, nz = d.nz, mf = d.mf, mg = d.mg, p = blockIdx.y;
   const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x, gsz = (long long)gridDim.x * blockDim.x;
   CrBuf<T> b = cr_carve<T>(d, a.ws, p);
+  const GridBar grid = cr_gridbar<T>(b);
   if (a.kkt_only) {
     for (long long e = gid; e < nz; e += gsz) b.eta[e] = a.eta_in[(size_t)p * nz + e];
     grid.sync();
