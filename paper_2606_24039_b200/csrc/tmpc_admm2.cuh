@@ -516,6 +516,7 @@ struct ResidualArgs {
   Dims d; Params<T> prm; QpView<T> qp;
   const T* x; const T* zg; const T* yf; const T* yg; const T* xi;
   T* r_prim; T* r_dual; T* objective; int32_t* status;
+  double* partial; int nparts;          // nparts > 1: gridDim.y CTAs per problem write partials, residual_finish_kernel reduces them in a fixed order
 };
 
 template <typename T>
@@ -523,7 +524,7 @@ __global__ void __launch_bounds__(256) residual_kernel(ResidualArgs<T> a) {
   __shared__ T red[64];
   const Dims& d = a.d;
   const int n = d.n, nx = d.nx, ng = d.ng, N = d.N, nn = n * n, nz = d.nz, mf = d.mf, mg = d.mg;
-  const int p = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
+  const int p = blockIdx.x, nt = blockDim.x * gridDim.y, tid = blockIdx.y * blockDim.x + threadIdx.x;   // parts interleave
   const T gam = a.prm.gamma, lam = a.prm.lam;
   const T* x = a.x + (size_t)p * nz; const T* zg = a.zg + (size_t)p * mg; const T* yf = a.yf + (size_t)p * mf;
   const T* yg = a.yg + (size_t)p * mg; const T* xi = a.xi + (size_t)p * mg; const T* q = a.qp.q + (size_t)p * nz;
@@ -574,12 +575,25 @@ __global__ void __launch_bounds__(256) residual_kernel(ResidualArgs<T> a) {
   }
   rp = block_max(rp, red); rd = block_max(rd, red); ob = block_sum(ob, red);
   bad = __syncthreads_or(bad);
-  if (tid == 0) {
+  if (threadIdx.x == 0) {
+    if (a.nparts > 1) { double* o = a.partial + ((size_t)p * a.nparts + blockIdx.y) * 4; o[0] = (double)rp; o[1] = (double)rd; o[2] = (double)ob; o[3] = bad ? 1.0 : 0.0; return; }
     if (a.r_prim) a.r_prim[p] = rp;
     if (a.r_dual) a.r_dual[p] = rd;
     if (a.objective) a.objective[p] = ob;
     if (a.status && bad) atomicOr(&a.status[p], TMPC_ST_NAN);
   }
+}
+
+template <typename T>
+__global__ void residual_finish_kernel(ResidualArgs<T> a) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= a.d.B) return;
+  double rp = 0, rd = 0, ob = 0; bool bad = false;
+  for (int k = 0; k < a.nparts; ++k) { const double* o = a.partial + ((size_t)p * a.nparts + k) * 4; rp = fmax(rp, o[0]); rd = fmax(rd, o[1]); ob += o[2]; bad |= o[3] != 0.0; }
+  if (a.r_prim) a.r_prim[p] = (T)rp;
+  if (a.r_dual) a.r_dual[p] = (T)rd;
+  if (a.objective) a.objective[p] = (T)ob;
+  if (a.status && bad) atomicOr(&a.status[p], TMPC_ST_NAN);
 }
 
 }  // namespace tmpc

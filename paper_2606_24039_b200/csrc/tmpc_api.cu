@@ -24,7 +24,7 @@ inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 inline size_t esize(int dtype) { return dtype == TMPC_F64 ? 8 : 4; }
 
 struct Layout {   // byte offsets into the workspace
-  size_t Lam, Sinv, cls, soft_adj, rhs, w_rows, lo_adj, hi_adj, q_adj, ax, azg, ayf, ayg, axi, zero_xinit, zero_b, cr, total;
+  size_t Lam, Sinv, cls, soft_adj, rhs, w_rows, lo_adj, hi_adj, q_adj, ax, azg, ayf, ayg, axi, zero_xinit, zero_b, res, cr, total;
 };
 
 Dims make_dims(const tmpc_config& c) {
@@ -44,6 +44,7 @@ Layout make_layout(const tmpc_config& c) {
   L.rhs = take(B * d.nz * es); L.w_rows = take(B * d.mg * es); L.lo_adj = take(B * d.mg * es); L.hi_adj = take(B * d.mg * es);
   L.q_adj = take(B * d.nz * es); L.ax = take(B * d.nz * es); L.azg = take(B * d.mg * es); L.ayf = take(B * d.mf * es);
   L.ayg = take(B * d.mg * es); L.axi = take(B * d.mg * es); L.zero_xinit = take(B * d.nx * es); L.zero_b = take(B * (size_t)d.N * d.nx * es);
+  L.res = take(B * 64 * 4 * sizeof(double));
   L.cr = take(cr_workspace_bytes(d, es));
   L.total = o;
   return L;
@@ -225,7 +226,11 @@ tmpc_status launch_residual(tmpc_ctx* h, const AdmmArgs<T>& s) {
   ResidualArgs<T> r; r.d = h->d; r.prm = s.prm; r.qp = s.qp; r.x = s.x; r.zg = s.zg; r.yf = s.yf; r.yg = s.yg; r.xi = s.xi;
   r.r_prim = s.r_prim; r.r_dual = s.r_dual; r.objective = s.objective; r.status = s.status;
   int nt = ((h->d.nz + 31) / 32) * 32; if (nt > 256) nt = 256;
-  residual_kernel<T><<<h->d.B, nt, 0, h->stream>>>(r); h->launches++;
+  int nparts = 1;                        // few long problems: several CTAs per problem, partials reduced in a fixed order
+  if (h->d.B < 64) { nparts = (h->d.nz + 2047) / 2048; if (nparts > 64) nparts = 64; if (nparts < 1) nparts = 1; }
+  r.partial = (double*)(h->ws + h->lay.res); r.nparts = nparts;
+  residual_kernel<T><<<dim3(h->d.B, nparts), nt, 0, h->stream>>>(r); h->launches++;
+  if (nparts > 1) { residual_finish_kernel<T><<<(h->d.B + 63) / 64, 64, 0, h->stream>>>(r); h->launches++; }
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
 }
 

@@ -151,73 +151,86 @@ __global__ void __launch_bounds__(256) cr_factor_kernel(CrFactorArgs<T> a) {
   if (gid == 0) *b.flag = 0;
   grid.sync();
   const int L = cr_levels(T_);
+  // One WARP per stage from here on: lane e owns matrix element e (and e + 32 when nn > 32); the small products go
+  // through a per-warp shared scratch, the pivot block is inverted in place by Gauss-Jordan (no pivoting: SPD).
+  __shared__ T scr[8][6 * NC * NC];
+  constexpr int EPL = (nn + 31) / 32;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const long long gw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
+  T* M0 = scr[wib]; T* M1 = M0 + nn; T* M2 = M1 + nn; T* M3 = M2 + nn; T* M4 = M3 + nn;
+  auto ld_mat = [&](T* dst, const T* src) {
+#pragma unroll
+    for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u; if (e < nn) dst[e] = src ? src[e] : T(0); }
+  };
+  auto gj_inverse = [&](T* A) -> int {                 // in-place inverse of an SPD block; returns 1 on a bad pivot
+    int bad = 0;
+#pragma unroll 1
+    for (int k = 0; k < n; ++k) {
+      T dk = A[k * n + k];
+      if (!(dk > T(0)) || !isfinite(dk)) { bad = 1; dk = T(1); }
+      const T pinv = T(1) / dk;
+      __syncwarp();
+#pragma unroll
+      for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u, i = e / n, j = e % n; if (e < nn && i == k && j != k) A[e] *= pinv; }
+      __syncwarp();
+#pragma unroll
+      for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u, i = e / n, j = e % n; if (e < nn && i != k && j != k) A[e] -= A[i * n + k] * A[k * n + j]; }
+      __syncwarp();
+#pragma unroll
+      for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u, i = e / n, j = e % n; if (e < nn && j == k) A[e] = (i == k) ? pinv : -A[e] * pinv; }
+      __syncwarp();
+    }
+    return bad;
+  };
   for (int l = 0; l < L; ++l) {
     const int h = 1 << l;
-    // (1) eliminated stages j = h(2k+1): U_j, FA_j, FB_j
-    for (long long k = gid;; k += gsz) {
+    // (1) eliminated stages j = h(2k+1): U_j = Theta_j^{-1}, FA_j = Lo_j' U_j, FB_j = Lo_b U_j
+    for (long long k = gw;; k += nw) {
       const long long j = (long long)h * (2 * k + 1);
       if (j >= T_) break;
-      T U[nn];
-      if (spd_inverse<T, NC>(b.Th + j * nn, U)) atomicOr(b.flag, 1);
-      const T* Loj = b.Lo + j * nn;
-      T* FA = b.FA + j * nn; T* FB = b.FB + j * nn; T* Uo = b.U + j * nn;
+      const bool hb = j + h < T_;
+      ld_mat(M0, b.Th + j * nn); ld_mat(M1, b.Lo + j * nn); ld_mat(M2, hb ? b.Lo + (j + h) * nn : nullptr);
+      __syncwarp();
+      if (gj_inverse(M0) && lane == 0) atomicOr(b.flag, 1);
 #pragma unroll
-      for (int e = 0; e < nn; ++e) Uo[e] = U[e];
+      for (int u = 0; u < EPL; ++u) {
+        const int e = lane + 32 * u, i = e / n, c = e % n;
+        if (e >= nn) continue;
+        T fa = T(0), fb = T(0);
 #pragma unroll
-      for (int i = 0; i < n; ++i)
-#pragma unroll
-        for (int c = 0; c < n; ++c) { T s = T(0);
-#pragma unroll
-          for (int m = 0; m < n; ++m) s += Loj[m * n + i] * U[m * n + c];
-          FA[i * n + c] = s; }
-      if (j + h < T_) {
-        const T* Lob = b.Lo + (j + h) * nn;
-#pragma unroll
-        for (int i = 0; i < n; ++i)
-#pragma unroll
-          for (int c = 0; c < n; ++c) { T s = T(0);
-#pragma unroll
-            for (int m = 0; m < n; ++m) s += Lob[i * n + m] * U[m * n + c];
-            FB[i * n + c] = s; }
+        for (int m = 0; m < n; ++m) { fa += M1[m * n + i] * M0[m * n + c]; fb += M2[i * n + m] * M0[m * n + c]; }
+        b.U[j * nn + e] = M0[e]; b.FA[j * nn + e] = fa; if (hb) b.FB[j * nn + e] = fb;
       }
+      __syncwarp();
     }
     grid.sync();
     // (2) survivors s = 2hk: Theta_s -= FA_{s+h} Lo_{s+h} + FB_{s-h} Lo_s' ;  Lo_s <- -FB_{s-h} Lo_{s-h}
-    for (long long k = gid;; k += gsz) {
+    for (long long k = gw;; k += nw) {
       const long long s_ = 2LL * h * k;
       if (s_ >= T_) break;
-      T* Th = b.Th + s_ * nn; T* Los = b.Lo + s_ * nn;
-      T nlo[nn];
+      const bool hp = s_ + h < T_, hm = s_ - h >= 0;
+      ld_mat(M0, hp ? b.FA + (s_ + h) * nn : nullptr); ld_mat(M1, hp ? b.Lo + (s_ + h) * nn : nullptr);
+      ld_mat(M2, hm ? b.FB + (s_ - h) * nn : nullptr); ld_mat(M3, b.Lo + s_ * nn); ld_mat(M4, hm ? b.Lo + (s_ - h) * nn : nullptr);
+      __syncwarp();
 #pragma unroll
-      for (int e = 0; e < nn; ++e) nlo[e] = T(0);
-      if (s_ + h < T_) {
-        const T* FA = b.FA + (s_ + h) * nn; const T* Loj = b.Lo + (s_ + h) * nn;
+      for (int u = 0; u < EPL; ++u) {
+        const int e = lane + 32 * u, i = e / n, c = e % n;
+        if (e >= nn) continue;
+        T acc = T(0), nlo = T(0);
 #pragma unroll
-        for (int i = 0; i < n; ++i)
-#pragma unroll
-          for (int c = 0; c < n; ++c) { T acc = T(0);
-#pragma unroll
-            for (int m = 0; m < n; ++m) acc += FA[i * n + m] * Loj[m * n + c];
-            Th[i * n + c] -= acc; }
+        for (int m = 0; m < n; ++m) { acc += M0[i * n + m] * M1[m * n + c] + M2[i * n + m] * M3[c * n + m]; nlo -= M2[i * n + m] * M4[m * n + c]; }
+        b.Th[s_ * nn + e] -= acc; b.Lo[s_ * nn + e] = nlo;
       }
-      if (s_ - h >= 0) {
-        const T* FB = b.FB + (s_ - h) * nn; const T* Loj = b.Lo + (s_ - h) * nn;
-#pragma unroll
-        for (int i = 0; i < n; ++i)
-#pragma unroll
-          for (int c = 0; c < n; ++c) { T acc = T(0), acc2 = T(0);
-#pragma unroll
-            for (int m = 0; m < n; ++m) { acc += FB[i * n + m] * Los[c * n + m]; acc2 += FB[i * n + m] * Loj[m * n + c]; }
-            Th[i * n + c] -= acc; nlo[i * n + c] = -acc2; }
-      }
-#pragma unroll
-      for (int e = 0; e < nn; ++e) Los[e] = nlo[e];
+      __syncwarp();
     }
     grid.sync();
   }
-  if (gid == 0) { T U[nn]; if (spd_inverse<T, NC>(b.Th, U)) atomicOr(b.flag, 1);
+  if (gw == 0) {
+    ld_mat(M0, b.Th); __syncwarp();
+    if (gj_inverse(M0) && lane == 0) atomicOr(b.flag, 1);
 #pragma unroll
-    for (int e = 0; e < nn; ++e) b.U[e] = U[e]; }
+    for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u; if (e < nn) b.U[e] = M0[e]; }
+  }
 }
 
 }  // namespace tmpc
