@@ -319,13 +319,28 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
   // ================================================================ chain warp
   if (tid < 32) {
     const int iters = a.kkt_only ? 1 : a.iters;
+#ifdef TMPC_TIMING
+    long long tw = 0, ts = 0;
+#endif
 #pragma unroll 1
     for (int it = 0; it < iters; ++it) {
+#ifdef TMPC_TIMING
+      const long long c0 = clock64();
+#endif
       bar_sync(1, nt);
+#ifdef TMPC_TIMING
+      const long long c1 = clock64();
+#endif
       chain_warp_solve<T, NC, NX, PG>(sm, R, PP, T_, tid);
       __syncwarp();
+#ifdef TMPC_TIMING
+      tw += c1 - c0; ts += clock64() - c1;
+#endif
       bar_arrive(2, nt);
     }
+#ifdef TMPC_TIMING
+    if (blockIdx.x == 0 && tid == 0) printf("chain warp: wait %lld solve %lld cycles per iteration\n", tw / iters, ts / iters);
+#endif
     return;
   }
 
@@ -437,8 +452,14 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
   }
   bar_sync(3, nti);
 
+#ifdef TMPC_TIMING
+  long long t_eta = 0, t_wait = 0, t_proj = 0, t_bar3 = 0;
+#endif
 #pragma unroll 1
   for (int it = 0; it < a.iters; ++it) {
+#ifdef TMPC_TIMING
+    const long long c0 = clock64();
+#endif
     // a4 in scaled variables: eta~ = X (sigma x - q + G's) + A~^-' r_t + A~^+' r_{t-1}   [+ G~' s for a dense G]   (eq. 51)
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
@@ -461,8 +482,14 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
       if (!d.g_sel) for (int r = 0; r < ng; ++r) s += sm[b + RC::G + r * n + i] * sm[b + RC::S + r];
       sm[b + RC::E1 + i] = s;
     }
+#ifdef TMPC_TIMING
+    const long long c1 = clock64();
+#endif
     bar_arrive(1, nt);
     bar_sync(2, nt);
+#ifdef TMPC_TIMING
+    const long long c2 = clock64();
+#endif
     // a7 + a8 on y: z~_f = A~^- y_t + A~^+ y_{t+1}, x~_i = X(:,i)' y_t, z~_g = x~_i or G~ y_t; relaxation (eq. 10),
     // projection (eq. 12-15), duals (eq. 16 / 44-45)
 #pragma unroll
@@ -496,8 +523,17 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
       }
       x[u] = a.prm.alpha * xt + A.oma * x[u];
     }
+#ifdef TMPC_TIMING
+    const long long c3 = clock64();
+#endif
     bar_sync(3, nti);
+#ifdef TMPC_TIMING
+    t_eta += c1 - c0; t_wait += c2 - c1; t_proj += c3 - c2; t_bar3 += clock64() - c3;
+#endif
   }
+#ifdef TMPC_TIMING
+  if (blockIdx.x == 0 && (tid == 32 || tid == nt - 32)) printf("item warp %d: eta %lld wait %lld proj %lld bar3 %lld cycles per iteration\n", tid >> 5, t_eta / a.iters, t_wait / a.iters, t_proj / a.iters, t_bar3 / a.iters);
+#endif
 
   // ---- write back the state
 #pragma unroll
