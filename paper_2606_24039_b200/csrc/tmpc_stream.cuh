@@ -130,9 +130,19 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
   auto row_dot = [&](const T* M, const T* vec, int rows) -> T {
     const T* row = M + (size_t)(ci < rows ? ci : 0) * LD;
     T acc[2] = {T(0), T(0)};
-    for (int j = cq * V; j < n; j += 4 * V) {
-#pragma unroll
-      for (int e = 0; e < V; ++e) acc[e & 1] += row[j + e] * vec[j + e];
+    if constexpr (sizeof(T) == 4) {                    // explicit 16-byte loads (rows and vectors are 16-byte aligned: n % 4 == 0)
+      float2 p2 = make_float2(0.f, 0.f);
+      for (int j = cq * 4; j < n; j += 16) {
+        const float4 m4 = *reinterpret_cast<const float4*>(row + j), v4 = *reinterpret_cast<const float4*>(vec + j);
+        p2 = __ffma2_rn(make_float2(m4.x, m4.y), make_float2(v4.x, v4.y), p2);
+        p2 = __ffma2_rn(make_float2(m4.z, m4.w), make_float2(v4.z, v4.w), p2);
+      }
+      acc[0] = p2.x; acc[1] = p2.y;
+    } else {
+      for (int j = cq * 2; j < n; j += 8) {
+        const double2 m2 = *reinterpret_cast<const double2*>(row + j), v2 = *reinterpret_cast<const double2*>(vec + j);
+        acc[0] += m2.x * v2.x; acc[1] += m2.y * v2.y;
+      }
     }
     return quad_sum(acc[0] + acc[1]);
   };
