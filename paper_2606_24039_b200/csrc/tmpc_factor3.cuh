@@ -67,8 +67,14 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
   auto mm_f = [&](double (&acc)[4][4], const T* A, const T* B, int rows, int i0, int j0) {
     for (int k = 0; k < rows; ++k) {
       double av[4], bv[4];
-#pragma unroll
-      for (int i = 0; i < 4; ++i) { av[i] = (double)A[(size_t)k * ld + i0 + i]; bv[i] = (double)B[(size_t)k * ld + j0 + i]; }
+      if constexpr (sizeof(T) == 4) {
+        const float4 a4 = *reinterpret_cast<const float4*>(A + (size_t)k * ld + i0), b4 = *reinterpret_cast<const float4*>(B + (size_t)k * ld + j0);
+        av[0] = a4.x; av[1] = a4.y; av[2] = a4.z; av[3] = a4.w; bv[0] = b4.x; bv[1] = b4.y; bv[2] = b4.z; bv[3] = b4.w;
+      } else {
+        const double2 a0 = *reinterpret_cast<const double2*>(A + (size_t)k * ld + i0), a1 = *reinterpret_cast<const double2*>(A + (size_t)k * ld + i0 + 2);
+        const double2 b0 = *reinterpret_cast<const double2*>(B + (size_t)k * ld + j0), b1 = *reinterpret_cast<const double2*>(B + (size_t)k * ld + j0 + 2);
+        av[0] = a0.x; av[1] = a0.y; av[2] = a1.x; av[3] = a1.y; bv[0] = b0.x; bv[1] = b0.y; bv[2] = b1.x; bv[3] = b1.y;
+      }
 #pragma unroll
       for (int i = 0; i < 4; ++i)
 #pragma unroll
