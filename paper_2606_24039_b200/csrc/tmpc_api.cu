@@ -95,6 +95,9 @@ template <typename T>
 tmpc_status launch_factor(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_in, const T* w_rows, int32_t* status) {
   FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = w_rows;
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
+  // small compile-time shapes: the warp-level kernel in its one-directional form (tmpc_factor2.cuh)
+  if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) { factor_tw2_kernel<T, 8, 6, false><<<h->d.B, 32, 0, h->stream>>>(a); h->launches++; return cuda_ok() ? TMPC_OK : TMPC_E_CUDA; }
+  if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) { factor_tw2_kernel<T, 6, 4, false><<<h->d.B, 32, 0, h->stream>>>(a); h->launches++; return cuda_ok() ? TMPC_OK : TMPC_E_CUDA; }
   const int nn = h->d.n * h->d.n;
   {                                      // large blocks: register-tiled products (tmpc_factor3.cuh)
     const int nt4 = f3_ld(h->d.n) / 4; const size_t smem3 = factor3_smem<T>(h->d.n);
@@ -209,8 +212,8 @@ template <typename T>
 tmpc_status launch_factor_tw(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_in, int32_t* status) {
   FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = nullptr;
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
-  if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) factor_tw2_kernel<T, 8, 6><<<h->d.B, 64, 0, h->stream>>>(a);
-  else if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) factor_tw2_kernel<T, 6, 4><<<h->d.B, 64, 0, h->stream>>>(a);
+  if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) factor_tw2_kernel<T, 8, 6, true><<<h->d.B, 64, 0, h->stream>>>(a);
+  else if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) factor_tw2_kernel<T, 6, 4, true><<<h->d.B, 64, 0, h->stream>>>(a);
   else {
     const int nn = h->d.n * h->d.n;
     int hn = ((nn + 31) / 32) * 32; if (hn > 512) hn = 512;

@@ -10,7 +10,9 @@
 
 namespace tmpc {
 
-template <typename T, int NC, int NX>
+// TW = true: twisted factor (X_t, B_t) for admm2_kernel.  TW = false: the one-directional block LDL' of factor_kernel
+// (Lam_t = Phi_t Sigma_t^{-1}, Sinv_t = Sigma_t^{-1}; per-row weights w_rows supported) for the backward pass; one warp.
+template <typename T, int NC, int NX, bool TW>
 __global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
   constexpr int n = NC, nx = NX, nn = NC * NC, an = NX * NC;
   constexpr int EPL = (nn + 31) / 32;                   // matrix elements per lane
@@ -28,9 +30,10 @@ __global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
   const T* Amp = a.qp.Am + (size_t)p * N * an;
   const T* App = a.qp.Ap + (size_t)p * N * an;
   const T* Gp = a.qp.G ? a.qp.G + a.qp.sG * p : nullptr;
-  T* Lamp = a.Lam + (size_t)p * T_ * nn;
+  T* Lamp = a.Lam + (size_t)p * (TW ? T_ : N) * nn;
   T* Xp = a.Sinv + (size_t)p * T_ * nn;
-  const int m = T_ / 2, cnt = half ? T_ - 1 - m : m;
+  const int m = TW ? T_ / 2 : T_, cnt = half ? T_ - 1 - m : m;      // !TW: the up chain covers every stage, no middle
+  const T* wr = a.w_rows ? a.w_rows + (size_t)p * T_ * ng : nullptr;
   const double w_eq = a.w_eq, w_in = a.w_in, sigma = a.sigma;
   int bad = 0;
 
@@ -70,8 +73,8 @@ __global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
       for (int r = 0; r < nx; ++r) acc += rAm[r * n + i] * rAm[r * n + j] + rAp[r * n + i] * rAp[r * n + j];
       if (t == 0 && i == j && i < nx) acc += 1;        // A_init' A_init = blkdiag(I_nx, 0)
       s += w_eq * acc;
-      if (d.g_sel) { for (int r = 0; r < ng; ++r) if (d.g_col[r] == i && i == j) s += w_in; }
-      else { for (int r = 0; r < ng; ++r) s += w_in * rG[r * n + i] * rG[r * n + j]; }
+      if (d.g_sel) { for (int r = 0; r < ng; ++r) if (d.g_col[r] == i && i == j) s += wr ? (double)wr[t * ng + r] : w_in; }
+      else { for (int r = 0; r < ng; ++r) s += (wr ? (double)wr[t * ng + r] : w_in) * rG[r * n + i] * rG[r * n + j]; }
       if (W1) { double c = 0;
 #pragma unroll
         for (int k = 0; k < n; ++k) c += W1[i * n + k] * W1[j * n + k];
@@ -142,8 +145,20 @@ __global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
     theta(t, A, k > 0 ? C : nullptr, nullptr);
     __syncwarp();
     chol_inv(A, Bm);
-    if (k > 0) b_out(half ? t + 1 : t - 1, Bm, C);
-    x_out(t, Bm);
+    if constexpr (TW) { if (k > 0) b_out(half ? t + 1 : t - 1, Bm, C); x_out(t, Bm); }
+    else {                                             // Sinv_t = X'X
+#pragma unroll
+      for (int u = 0; u < EPL; ++u) {
+        const int e = lane + 32 * u;
+        if (e >= nn) continue;
+        const int i = e / n, j = e % n;
+        double s = 0;
+#pragma unroll
+        for (int kk = 0; kk < n; ++kk) if (kk >= i && kk >= j) s += Bm[kk * n + i] * Bm[kk * n + j];
+        Xp[(size_t)t * nn + e] = (T)s;
+      }
+      if (t == N) break;
+    }
     __syncwarp();
     // A <- Psi_t: up Phi_t = E_t + w A^+_t' A^-_t ; down Phi_{t-1}' = E_{t-1}' + w A^-_{t-1}' A^+_{t-1}.
     // up needs A^+_t (not in this stage's raw data): read it from global; down has A^+_{t-1} (rAp) and needs A^-_{t-1}.
@@ -174,10 +189,22 @@ __global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
       C[e] = s;
     }
     __syncwarp();
+    if constexpr (!TW) {                                // Lambda_t = W X
+#pragma unroll
+      for (int u = 0; u < EPL; ++u) {
+        const int e = lane + 32 * u;
+        if (e >= nn) continue;
+        const int i = e / n, j = e % n;
+        double s = 0;
+#pragma unroll
+        for (int kk = 0; kk < n; ++kk) if (kk >= j) s += C[i * n + kk] * Bm[kk * n + j];
+        Lamp[(size_t)t * nn + e] = (T)s;
+      }
+    }
   }
   __syncthreads();
   // ---- middle stage m (warp 0): both chains' last W feed Sigma_m
-  if (half == 0) {
+  if (TW && half == 0) {
     const double* Wup = sm[0] + 2 * nn; const double* Wdn = sm[1] + 2 * nn;
     prefetch(m); commit();
     __syncwarp();
