@@ -317,3 +317,18 @@ def test_config4_full_batch_sampled_fp32():
     assert rc == 0
     compare_states({k: got[k][idx] for k in KEYS}, ref, TOL["f32"])
     s.close()
+
+
+# ----------------------------------------------------------------------------------------------- launch-shape edge cases
+@pytest.mark.parametrize("B", [1, 7])
+def test_resident_odd_batch_fp32(B):
+    """Odd batches leave the second problem slot of the last CTA empty (PG = 2); B = 1 takes the one-problem-per-CTA shape."""
+    run_pair(W.config2(B=B, N=9), "f32", iters=40)
+    run_pair(W.config2(B=B, N=10, soft_bound=0.5), "f64", iters=40)
+
+
+def test_duplicate_selection_column_falls_back_fp64():
+    """Two inequality rows on the same column are outside the fast path's one-row-per-column ownership: generic kernels."""
+    w = W.random_ltv(77, 3, 11, 6, 2, [6, 6, 7], [0, 1, 0], q_scale=0.3)
+    w.lo[..., 1] = -0.6; w.hi[..., 1] = 0.6          # a second, tighter (soft) bound on the same control
+    run_pair(w, "f64", iters=60)
