@@ -1,5 +1,5 @@
 // tmpc_admm2.cuh — a4..a8 for the RESIDENT class (configs 1, 2, 4): the fused ADMM loop of Alg. 3
-// on the twisted block factor of tmpc_factor.cuh, all iterations in one launch.
+// on the twisted block factor of tmpc_factor2.cuh, all iterations in one launch.
 //
 // Design:
 //  * a CTA owns PG problems (1 or 2).  The factor (X_t, -B_t) and the constraint blocks carried into the scaled
@@ -70,7 +70,7 @@ template <int L> __device__ __forceinline__ double dotv(const double (&a)[L], co
 //   E0  y_t               [n]       solution of the scaled system (x~_t = X_t' y_t)
 //   E1  eta~_t -> w_t     [n]
 //   D   sigma x - q + G's [n]       exchanged inside the stage for the X_t product
-//   LAM -B_t              [n][n]    twisted factor, tmpc_factor.cuh
+//   LAM -B_t              [n][n]    twisted factor, tmpc_factor2.cuh
 //   SINV X_t = L_t^{-1}   [n][n]
 //   S   s_t = rho_g z_g - y_g [n slots, ng used]   only when G is not a selection
 //   G   G~_t = G_t X_t'   [ng][n]                  only when G is not a selection
@@ -184,7 +184,7 @@ template <int L> __device__ __forceinline__ double dotv_from(const double (&a)[L
   return acc[0] + acc[1];
 }
 
-// ---- x~ = S^{-1} eta on the scaled variables (tmpc_factor.cuh): E1 holds eta~ on entry and w on exit, E0 receives y.
+// ---- x~ = S^{-1} eta on the scaled variables (tmpc_factor2.cuh): E1 holds eta~ on entry and w on exit, E0 receives y.
 // One warp; lanes = (problem, direction, row), 8 lanes per slot.  Every step is: publish my component (STS), read the
 // 8-vector back as a broadcast vector load, one row (forward) or column (outward) of -B_t, one FFMA2 dot.
 template <typename T, int NC, int NX, int PG>

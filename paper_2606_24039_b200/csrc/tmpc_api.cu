@@ -214,12 +214,7 @@ tmpc_status launch_factor_tw(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
   if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) factor_tw2_kernel<T, 8, 6, true><<<h->d.B, 64, 0, h->stream>>>(a);
   else if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) factor_tw2_kernel<T, 6, 4, true><<<h->d.B, 64, 0, h->stream>>>(a);
-  else {
-    const int nn = h->d.n * h->d.n;
-    int hn = ((nn + 31) / 32) * 32; if (hn > 512) hn = 512;
-    const size_t smem = 6 * (size_t)nn * sizeof(double);
-    factor_tw_kernel<T, double><<<h->d.B, 2 * hn, smem, h->stream>>>(a);
-  }
+  else return TMPC_E_UNSUPPORTED;      // fast_plan() only admits the shapes above
   h->launches++;
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
 }

@@ -48,49 +48,6 @@ __host__ __device__ inline CrBuf<T> cr_carve(const Dims& d, unsigned char* ws, i
 }
 __host__ __device__ inline int cr_levels(int T_) { int L = 0; while ((1 << L) < T_) ++L; return L; }
 
-// inverse of an SPD NC x NC block through its Cholesky factor, in registers/local memory.  Returns 1 on a bad pivot.
-template <typename T, int NC>
-__device__ int spd_inverse(const T* __restrict__ A, T* __restrict__ X) {
-  T L[NC * NC]; int bad = 0;
-#pragma unroll
-  for (int i = 0; i < NC * NC; ++i) L[i] = A[i];
-#pragma unroll
-  for (int k = 0; k < NC; ++k) {
-    T dk = L[k * NC + k];
-    if (!(dk > T(0)) || !isfinite(dk)) { bad = 1; dk = T(1); }
-    const T sq = sqrt(dk), inv = T(1) / sq;
-    L[k * NC + k] = sq;
-#pragma unroll
-    for (int i = k + 1; i < NC; ++i) L[i * NC + k] *= inv;
-#pragma unroll
-    for (int j = k + 1; j < NC; ++j)
-#pragma unroll
-      for (int i = j; i < NC; ++i) L[i * NC + j] -= L[i * NC + k] * L[j * NC + k];
-  }
-  T Y[NC * NC];    // Y = L^{-1} (lower)
-#pragma unroll
-  for (int j = 0; j < NC; ++j) {
-#pragma unroll
-    for (int i = 0; i < NC; ++i) {
-      if (i < j) { Y[i * NC + j] = T(0); continue; }
-      T s = (i == j) ? T(1) : T(0);
-#pragma unroll
-      for (int k = 0; k < NC; ++k) if (k >= j && k < i) s -= L[i * NC + k] * Y[k * NC + j];
-      Y[i * NC + j] = s / L[i * NC + i];
-    }
-  }
-#pragma unroll
-  for (int i = 0; i < NC; ++i)
-#pragma unroll
-    for (int j = 0; j < NC; ++j) {
-      T s = T(0);
-#pragma unroll
-      for (int k = 0; k < NC; ++k) if (k >= i && k >= j) s += Y[k * NC + i] * Y[k * NC + j];
-      X[i * NC + j] = s;
-    }
-  return bad;
-}
-
 // Light-weight barrier over the gridDim.x CTAs of ONE problem (cooperative launch guarantees co-residency): one atomic
 // per CTA on a counter, release by bumping a generation word; a gpu-scope fence on both sides orders global memory
 // (and invalidates L1 on the waiting side).  About 1 us per barrier against ~2.5 us for cooperative_groups grid.sync.

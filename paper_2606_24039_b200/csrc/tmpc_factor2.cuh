@@ -1,8 +1,25 @@
-// tmpc_factor2.cuh — a2 + a3 for the resident fast path: the twisted block Cholesky of tmpc_factor.cuh (same math,
-// same output X_t / B_t), one WARP per half chain with compile-time block sizes.
+// tmpc_factor2.cuh — a2 + a3 for the resident fast path: twisted block Cholesky, one WARP per half chain with
+// compile-time block sizes.
 //
-// factor_tw_kernel (tmpc_factor.cuh) spends its time in CTA barriers, run-time integer divisions and dependent global
-// loads; here a CTA is two warps (the up chain and the down chain of one problem), every phase of a stage is separated
+// Twisted ("burn at both ends") block LDL' factor for the resident fast path (tmpc_admm2.cuh).
+//
+// The block-tridiagonal S is eliminated from BOTH ends towards the middle stage m = T/2: the up chain runs over
+// stages 0,1,..,m-1 and the down chain over N,N-1,..,m+1, independently; the middle pivot collects both Schur
+// contributions.  With  Psi_t = block(next stage of the chain, t) of S  (up: Phi_t; down: Phi_{t-1}'),
+//     Sigma_first = Theta_first,  L_t L_t' = Sigma_t,  W_t = Psi_t L_t^{-T},  Sigma_next = Theta_next - W_t W_t',
+//     Sigma_m = Theta_m - W_{m-1} W_{m-1}' - W_{m+1} W_{m+1}'   (block Cholesky with the middle stage eliminated last).
+// Stored with explicit inverses of the diagonal Cholesky blocks, X_t = L_t^{-1}, and the off-diagonal blocks pre- and
+// post-multiplied by them, B_t = X_next W_t, so that the two sequential sweeps are pure mat-vecs on scaled variables:
+//     eta~_t = X_t eta_t (stage-parallel),  w_next = eta~_next - B_t w_t,  w_m = eta~_m - B_{m-1} w_{m-1} - B_{m+1} w_{m+1},
+//     y_m = w_m,  y_t = w_t - B_t' y_next (outwards from m),  x_t = X_t' y_t (stage-parallel).
+// It is an exact factorisation of the same S (P A P' = L D L' for the permutation that orders stages
+// 0, N, 1, N-1, ...), same flops and same storage as the one-directional form, but both substitution sweeps of a
+// solve are two independent chains of half the length.
+// Layout: Lam [B][T][n][n] holds B_t, indexed by the stage t the block belongs to (slot m unused); Sinv [B][T][n][n]
+// holds X_t (lower triangular, zeros stored).
+//
+// The generic CTA-level factor_kernel (tmpc_factor.cuh) spends its time in CTA barriers, run-time integer divisions and
+// dependent global loads; here a CTA is two warps (the up chain and the down chain of one problem), every phase of a stage is separated
 // by __syncwarp only, the raw stage data (D_t, E_t, A^-_t, A^+_{t-1}, G_t) of the NEXT stage is prefetched into
 // registers while the current stage is factored, and all index arithmetic is compile-time.  Arithmetic in double.
 #pragma once
