@@ -48,25 +48,36 @@ __host__ __device__ inline CrBuf<T> cr_carve(const Dims& d, unsigned char* ws, i
 }
 __host__ __device__ inline int cr_levels(int T_) { int L = 0; while ((1 << L) < T_) ++L; return L; }
 
-// Light-weight barrier over the gridDim.x CTAs of ONE problem (cooperative launch guarantees co-residency): one atomic
-// per CTA on a counter, release by bumping a generation word; a gpu-scope fence on both sides orders global memory
-// (and invalidates L1 on the waiting side).  About 1 us per barrier against ~2.5 us for cooperative_groups grid.sync.
+// Light-weight barrier over the gridDim.x CTAs of ONE problem (cooperative launch guarantees co-residency): one
+// acq_rel atomic per CTA on a counter; the last arriver resets the counter and bumps a generation word with release
+// semantics; the others poll the generation word with acquire loads.  Each CTA counts its own barriers (the expected
+// generation lives in a register), so a barrier costs one atomic round trip plus the release/acquire hand-over.
 struct GridBar {
-  unsigned* cnt; unsigned* gen; unsigned nblocks;
-  __device__ __forceinline__ void sync() const {
+  unsigned* cnt; unsigned* gen; unsigned nblocks; unsigned expect;      // expect: generation value that ends my next barrier
+  __device__ __forceinline__ void sync() {
     __syncthreads();
     if (threadIdx.x == 0) {
-      const unsigned g = *reinterpret_cast<volatile unsigned*>(gen);
-      __threadfence();
-      if (atomicAdd(cnt, 1u) == nblocks - 1) { *reinterpret_cast<volatile unsigned*>(cnt) = 0u; __threadfence(); atomicAdd(gen, 1u); }
-      else { while (*reinterpret_cast<volatile unsigned*>(gen) == g) {} }
-      __threadfence();
+      unsigned old;
+      asm volatile("atom.add.acq_rel.gpu.u32 %0, [%1], 1;" : "=r"(old) : "l"(cnt) : "memory");
+      if (old == nblocks - 1) {
+        asm volatile("st.relaxed.gpu.u32 [%0], %1;" ::"l"(cnt), "r"(0u) : "memory");
+        asm volatile("red.release.gpu.add.u32 [%0], 1;" ::"l"(gen) : "memory");
+      } else {
+        unsigned g;
+        do { asm volatile("ld.acquire.gpu.u32 %0, [%1];" : "=r"(g) : "l"(gen) : "memory"); } while ((int)(g - expect) < 0);
+      }
     }
+    ++expect;
     __syncthreads();
   }
 };
 template <typename T>
-__device__ __forceinline__ GridBar cr_gridbar(const CrBuf<T>& b) { return GridBar{reinterpret_cast<unsigned*>(b.flag) + 16, reinterpret_cast<unsigned*>(b.flag) + 32, gridDim.x}; }
+__device__ __forceinline__ GridBar cr_gridbar(const CrBuf<T>& b) {
+  unsigned* gen = reinterpret_cast<unsigned*>(b.flag) + 32;
+  unsigned g0;                                          // every CTA reads the generation before anyone can have passed a barrier of this launch
+  asm volatile("ld.acquire.gpu.u32 %0, [%1];" : "=r"(g0) : "l"(gen) : "memory");
+  return GridBar{reinterpret_cast<unsigned*>(b.flag) + 16, gen, gridDim.x, g0 + 1};
+}
 
 template <typename T>
 struct CrFactorArgs { Dims d; QpView<T> qp; T sigma, rho_f, rho_g; unsigned char* ws; };
@@ -79,7 +90,7 @@ __global__ void __launch_bounds__(256) cr_factor_kernel(CrFactorArgs<T> a) {
   const int nx = d.nx, ng = d.ng, N = d.N, T_ = d.T, p = blockIdx.y;
   const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x, gsz = (long long)gridDim.x * blockDim.x;
   CrBuf<T> b = cr_carve<T>(d, a.ws, p);
-  const GridBar grid = cr_gridbar<T>(b);
+  GridBar grid = cr_gridbar<T>(b);
   const T* Dp = a.qp.D + a.qp.sD * p; const T* Ep = a.qp.E + a.qp.sE * p;
   const T* Amp = a.qp.Am + (size_t)p * N * nx * n; const T* App = a.qp.Ap + (size_t)p * N * nx * n;
   const T* Gp = a.qp.G ? a.qp.G + a.qp.sG * p : nullptr;
@@ -236,7 +247,7 @@ __device__ __forceinline__ void cr_up_level(const CrBuf<T>& b, int T_, long long
   }
 }
 template <typename T, int NC>
-__device__ void cr_solve(const GridBar& gb, const CrBuf<T>& b, int T_, long long gid, long long gsz) {
+__device__ void cr_solve(GridBar& gb, const CrBuf<T>& b, int T_, long long gid, long long gsz) {
   constexpr int n = NC;
   const int L = cr_levels(T_);
   int LS = 0;                                          // levels run grid-wide
@@ -272,7 +283,7 @@ __global__ void __launch_bounds__(256) cr_admm_kernel(CrAdmmArgs<T> a) {
   const int nx = d.nx, ng = d.ng, N = d.N, T_ = d.T, nz = d.nz, mf = d.mf, mg = d.mg, p = blockIdx.y;
   const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x, gsz = (long long)gridDim.x * blockDim.x;
   CrBuf<T> b = cr_carve<T>(d, a.ws, p);
-  const GridBar grid = cr_gridbar<T>(b);
+  GridBar grid = cr_gridbar<T>(b);
   if (a.kkt_only) {
     for (long long e = gid; e < nz; e += gsz) b.eta[e] = a.eta_in[(size_t)p * nz + e];
     grid.sync();

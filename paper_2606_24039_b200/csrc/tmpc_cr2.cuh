@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(256) cr2_admm_kernel(CrAdmmArgs<T> a, int nchu
   constexpr int n = NC, nn = NC * NC, nx = NX, CS = CR2_CS;
   const int ng = d.ng, N = d.N, T_ = d.T, nz = d.nz, mf = d.mf, mg = d.mg, p = blockIdx.y, tid = threadIdx.x, nt = blockDim.x;
   CrBuf<T> b = cr_carve<T>(d, a.ws, p);
-  const GridBar grid = cr_gridbar<T>(b);
+  GridBar grid = cr_gridbar<T>(b);
   const int S = N / CS + 1;                             // separators 0, 64, .., 64 (S-1)
   T* gEta = b.part; T* gPart = gEta + S * n; T* gX = gPart + S * n; T* gR = gX + S * n;   // exchange through global memory
   const int L = cr_levels(T_);
@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(256) cr2_admm_kernel(CrAdmmArgs<T> a, int nchu
     if (!a.kkt_only) grid.sync();                       // pairs with the chunks' set-up barrier
     for (int it = 0; it < iters; ++it) {
       grid.sync();
-      for (int e = tid; e < S * n; e += nt) { const int k = e / n; eta[e] = gEta[e] + (k > 0 ? gPart[e - n] : T(0)); }
+      for (int e = tid; e < S * n; e += nt) { const int k = e / n; eta[e] = __ldcg(gEta + e) + (k > 0 ? __ldcg(gPart + e - n) : T(0)); }
       __syncthreads();
       for (int l = CR2_LV; l < L; ++l) { cr2_down<T, NC>(FA, FB, eta, S - 1, 1 << (l - CR2_LV), tid, nt); __syncthreads(); }
       if (tid < n) { T acc = T(0);
@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(256) cr2_admm_kernel(CrAdmmArgs<T> a, int nchu
     if (tid < n) { gEta[c * n + tid] = eta[tid]; if (nl == CS) gPart[c * n + tid] = eta[CS * n + tid]; }
   };
   auto fetch_x = [&]() {
-    if (tid < n) { xt[tid] = gX[c * n + tid]; if (nl == CS) xt[CS * n + tid] = gX[(c + 1) * n + tid]; }
+    if (tid < n) { xt[tid] = __ldcg(gX + c * n + tid); if (nl == CS) xt[CS * n + tid] = __ldcg(gX + (c + 1) * n + tid); }
     __syncthreads();
   };
 
@@ -171,7 +171,7 @@ __global__ void __launch_bounds__(256) cr2_admm_kernel(CrAdmmArgs<T> a, int nchu
 
   for (int it = 0; it < a.iters; ++it) {
     // ---- a4 (eq. 51) for my stages; rows of the block before the chunk come through gR
-    if (c > 0 && tid < nx) rv[tid] = gR[(c - 1) * nx + tid];
+    if (c > 0 && tid < nx) rv[tid] = __ldcg(gR + (c - 1) * nx + tid);
     __syncthreads();
     for (int e = tid; e < (nl + 1) * n; e += nt) {
       const int ls = e / n, i = e - ls * n;
