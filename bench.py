@@ -284,7 +284,7 @@ def run_gpu(args):
     roof["frac"] = roof["achieved"] / roof["peak"]
     # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed `ncu --set full` captures
     # (profiles/r01_v2_ncu_full_*.md); only valid for the workload the capture was taken on
-    ncu_traffic = {(2, "f32", 1024): 57.11e6 + 0.43e6, (3, "f32", 512): 440.47e9 + 1.53e9}
+    ncu_traffic = {(2, "f32", 1024): 57.11e6 + 0.43e6, (3, "f32", 512): 441.74e9 + 1.53e9}
     roof["traffic"] = ncu_traffic.get((args.config, args.dtype, w.B))
     roof["kernel"] = {1: "admm2_kernel", 2: "admm2_kernel", 3: "admm_stream_kernel", 4: "admm2_kernel", 5: "cr2_admm_kernel"}[args.config] + " (tmpc_admm_solve)"
     if args.config in (1, 2, 4):
