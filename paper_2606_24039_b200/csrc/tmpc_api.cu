@@ -24,7 +24,7 @@ inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 inline size_t esize(int dtype) { return dtype == TMPC_F64 ? 8 : 4; }
 
 struct Layout {   // byte offsets into the workspace
-  size_t Lam, Sinv, cls, soft_adj, rhs, w_rows, lo_adj, hi_adj, q_adj, ax, azg, ayf, ayg, axi, zero_xinit, zero_b, res, cr, total;
+  size_t Lam, Sinv, eta, cls, soft_adj, rhs, w_rows, lo_adj, hi_adj, q_adj, ax, azg, ayf, ayg, axi, zero_xinit, zero_b, res, cr, total;
 };
 
 Dims make_dims(const tmpc_config& c) {
@@ -39,7 +39,7 @@ Layout make_layout(const tmpc_config& c) {
   const Dims d = make_dims(c); const size_t es = esize(c.dtype), B = d.B, nn = (size_t)d.n * d.n;
   Layout L; size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
-  L.Lam = take(B * d.T * nn * es); L.Sinv = take(B * d.T * nn * es);
+  L.Lam = take(B * d.T * nn * es); L.Sinv = take(B * d.T * nn * es); L.eta = take(B * d.nz * es);
   L.cls = take(B * d.mg); L.soft_adj = take(B * d.mg);
   L.rhs = take(B * d.nz * es); L.w_rows = take(B * d.mg * es); L.lo_adj = take(B * d.mg * es); L.hi_adj = take(B * d.mg * es);
   L.q_adj = take(B * d.nz * es); L.ax = take(B * d.nz * es); L.azg = take(B * d.mg * es); L.ayf = take(B * d.mf * es);
@@ -143,7 +143,7 @@ tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
     const StreamPlan sp = stream_plan<T>(d, kMaxSmem);
     const int V = 16 / (int)sizeof(T);
     if ((d.n * d.n) % V == 0 && (d.nx * d.n) % V == 0 && d.n % V == 0 && 4 * d.ng <= sp.nthreads - 32 && sp.slots >= 2 && sp.nthreads <= 1024) {
-      StreamArgs<T> S; S.a = a; S.LD = sp.LD; S.slots = sp.slots; S.tile_elems = sp.tile_elems;
+      StreamArgs<T> S; S.a = a; S.LD = sp.LD; S.slots = sp.slots; S.tile_elems = sp.tile_elems; S.eta = (T*)(h->ws + h->lay.eta);
       auto k = admm_stream_kernel<T>;
       if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp.smem) != cudaSuccess) return TMPC_E_CUDA;
       k<<<d.B, sp.nthreads, sp.smem, h->stream>>>(S); h->launches++;

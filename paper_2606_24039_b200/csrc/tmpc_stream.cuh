@@ -44,20 +44,22 @@ __host__ inline StreamPlan stream_plan(const Dims& d, size_t max_smem) {
   StreamPlan P; P.LD = stream_ld<T>(d.n); P.tile_elems = d.n * P.LD;
   const int nc = (4 * (d.n > d.nx ? d.n : d.nx) + 31) / 32 * 32;    // a quad of threads per row
   P.nthreads = 32 + nc;
-  const size_t fixed = (size_t)(3 * d.nz + 2 * d.nx + 2 * d.ng + 64) * sizeof(T) + 256;
+  const size_t fixed = (size_t)(d.nz + 2 * d.n + 2 * d.nx + 2 * d.ng + 64) * sizeof(T) + 256;   // x~/v, w window, r, s
   const size_t tile = (size_t)P.tile_elems * sizeof(T);
   long s = ((long)max_smem - (long)fixed) / (long)tile;
-  P.slots = s > 6 ? 6 : (int)s;
-  // the consumers are latency bound (dependent dots + CTA barriers), so two co-resident CTAs with a 2-deep ring each beat
-  // one CTA with a deep ring (measured at config 3: 116 ms vs 144 ms per 200 iterations)
-  if (P.slots >= 2 && 2 * (fixed + 2 * tile + 1024) <= (size_t)228 * 1024) P.slots = 2;
-  if (const char* e = getenv("TMPC_STREAM_SLOTS")) { const int v = atoi(e); if (v >= 2 && v <= P.slots) P.slots = v; }   // tuning knob
+  const int smax = s > 6 ? 6 : (int)s;
+  P.slots = smax;
+  // the consumers are latency bound (dependent dots + CTA barriers): co-resident CTAs hide that better than a deep ring
+  // (measured at config 3: two CTAs per SM with 2 slots 116 ms, one CTA with 6 slots 144 ms), so take the deepest ring
+  // that still lets two CTAs share an SM
+  for (int k = smax; k >= 2; --k) if (2 * (fixed + k * tile + 1024) <= (size_t)228 * 1024) { P.slots = k; break; }
+  if (const char* e = getenv("TMPC_STREAM_SLOTS")) { const int v = atoi(e); if (v >= 2 && v <= smax) P.slots = v; }   // tuning knob
   P.smem = fixed + (size_t)(P.slots > 0 ? P.slots : 0) * tile;
   return P;
 }
 
 template <typename T>
-struct StreamArgs { AdmmArgs<T> a; int LD, slots, tile_elems; };
+struct StreamArgs { AdmmArgs<T> a; int LD, slots, tile_elems; T* eta; };   // eta: global scratch [B][nz] (right-hand side, L2 resident)
 
 // block sequence of one launch, identical in the producer and the consumers:
 //   [eta pass]   t = N-1..0 : A^-_t, A^+_t                         (skipped for kkt_only)
@@ -73,10 +75,12 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
   const int LD = S.LD, KS = S.slots, p = blockIdx.x, tid = threadIdx.x;
   unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_raw);            // full[KS], empty[KS]
   T* ring = reinterpret_cast<T*>(smem_raw + 256);
-  T* xs = ring + (size_t)KS * S.tile_elems;      // x   [nz]
-  T* e0 = xs + nz;                                // eta / w, then the next eta   [nz]
-  T* e1 = e0 + nz;                                // v / x~   [nz]
-  T* rbuf = e1 + nz;                              // r_t [nx], then z~ partials [nx]
+  // Only v / x~ is kept whole in shared memory.  The right-hand side eta lives in global memory (each element is written
+  // once and read once per iteration by the SAME thread, prefetched a step ahead), x is updated in place in global
+  // memory, and w_t only needs a two-stage window: the small footprint leaves room for a deeper ring / more CTAs.
+  T* e1 = ring + (size_t)KS * S.tile_elems;       // v / x~   [nz]
+  T* wwin = e1 + nz;                              // w_{t-1}, w_t   [2][n]
+  T* rbuf = wwin + 2 * n;                         // r_t [nx]
   T* sbuf = rbuf + 2 * nx;                        // s_t [ng]
   const unsigned bar0 = smem_u32(bars);
   auto full_bar = [&](int s) { return bar0 + 8u * s; };
@@ -176,57 +180,66 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
     return s;
   };
 
-  for (int e = ct; e < nz; e += ncons) { const T v = a.x[gx + e]; if (a.kkt_only) e0[e] = v; else xs[e] = v; }
-  cons_bar();
+  T* geta = S.eta + gx;                                                 // my problem's right-hand side (global)
+  const T* eta_rd = a.kkt_only ? a.x + gx : geta;                       // tmpc_kkt_solve: eta is the caller's vector
+  T* gxs = a.x + gx;                                                    // x, updated in place
   if (!a.kkt_only) {
     if (own_g) for (int t = 0; t < T_; ++t) {
       const size_t row = gg + t * ng + ci;
-      if (!a.zg_given) a.zg[row] = tmin(tmax(g_row_dot(t, xs), a.qp.lo[row]), a.qp.hi[row]);
+      if (!a.zg_given) a.zg[row] = tmin(tmax(g_row_dot(t, gxs), a.qp.lo[row]), a.qp.hi[row]);
       if (!a.zg_given && a.iters == 0) a.xi[row] = T(0);
     }
     cons_bar();
     __threadfence_block();
-    // ---- eta pass: eta = sigma x - q + C'(rho_f c - y_f) + G'(rho_g z_g - y_g)                              (eq. 51)
-    if (own_x) for (int t = 0; t < T_; ++t) e0[t * n + ci] = sigma * xs[t * n + ci] - a.qp.q[gx + t * n + ci] + gts(t, nullptr);
+    // ---- eta pass: eta = sigma x - q + C'(rho_f c - y_f) + G'(rho_g z_g - y_g)  (eq. 51).  Thread ci carries the
+    // partial eta of the stage above in a register until block t has added A^+_t' r_t, then stores it once.
+    T pend = own_x ? sigma * gxs[N * n + ci] - a.qp.q[gx + N * n + ci] + gts(N, nullptr) : T(0);
     for (int t = N - 1; t >= 0; --t) {
       if (own_f) rbuf[ci] = rho_f * a.qp.b[((size_t)p * N + t) * nx + ci] - a.yf[gf + nx + t * nx + ci];
+      const T base = own_x ? sigma * gxs[t * n + ci] - a.qp.q[gx + t * n + ci] + gts(t, nullptr) : T(0);
       const T* Am = acquire(0); const T* Ap = acquire(1);
       cons_bar();
-      { const T da = col_dot(Am, rbuf, nx), dp = col_dot(Ap, rbuf, nx); if (own_x) { e0[t * n + ci] += da; e0[(t + 1) * n + ci] += dp; } }
+      const T da = col_dot(Am, rbuf, nx), dp = col_dot(Ap, rbuf, nx);
+      if (own_x) { geta[(t + 1) * n + ci] = pend + dp; pend = base + da; }
       release(2);
       cons_bar();
     }
-    if (own_f) e0[ci] += rho_f * a.qp.x_init[(size_t)p * nx + ci] - a.yf[gf + ci];
+    if (own_f) pend += rho_f * a.qp.x_init[(size_t)p * nx + ci] - a.yf[gf + ci];
+    if (own_x) geta[ci] = pend;
   }
 
   for (int it = 0; it < iters; ++it) {
     const bool lastit = it == iters - 1;
-    cons_bar();
     // ---- forward sweep: w_t = eta_t - Lambda_{t-1} w_{t-1},  v_t = Sigma_t^{-1} w_t                         (eq. 8)
+    T eta_nx = own_x ? eta_rd[ci] : T(0);
     for (int t = 0; t < T_; ++t) {
+      const T eta_t = eta_nx;
+      if (t + 1 < T_ && own_x) eta_nx = eta_rd[(t + 1) * n + ci];       // prefetch
+      T* wt = wwin + (t & 1) * n;
       if (t > 0) {
         const T* L = acquire(0);
-        const T lw = row_dot(L, e0 + (t - 1) * n, n);
+        const T lw = row_dot(L, wwin + ((t - 1) & 1) * n, n);
         release(1);
-        if (own_x) e0[t * n + ci] -= lw;
-        cons_bar();
-      }
+        if (own_x) wt[ci] = eta_t - lw;
+      } else if (own_x) wt[ci] = eta_t;
+      cons_bar();
       const T* Si = acquire(0);
-      { const T v = row_dot(Si, e0 + t * n, n); if (own_x) e1[t * n + ci] = v; }
+      { const T v = row_dot(Si, wt, n); if (own_x) e1[t * n + ci] = v; }
       release(1);
     }
     cons_bar();
     // ---- outward sweep: x~_t = v_t - Lambda_t' x~_{t+1}, then everything local to stage t and dynamics block t.
-    // The per-row state of stage t-1 (z_g, y_g, lo, hi, y_f, c, q: global memory, L2 resident) is prefetched into
+    // The per-row state of stage t-1 (x, z_g, y_g, lo, hi, y_f, c, q: global memory, L2 resident) is prefetched into
     // registers while stage t is processed, so no global-load latency sits on the dependent path.
-    T pzg = T(0), pyg = T(0), plo = T(0), phi = T(0), pyf = T(0), pc = T(0), pq = T(0);
+    T pzg = T(0), pyg = T(0), plo = T(0), phi = T(0), pyf = T(0), pc = T(0), pq = T(0), px = T(0);
     auto prefetch_state = [&](int t) {
       if (a.kkt_only || t < 0) return;
       if (own_g) { const size_t row = gg + t * ng + ci; pzg = a.zg[row]; pyg = a.yg[row]; plo = a.qp.lo[row]; phi = a.qp.hi[row]; }
       if (own_f && t < N) { pyf = a.yf[gf + nx + t * nx + ci]; pc = a.qp.b[((size_t)p * N + t) * nx + ci]; }
-      if (own_x) pq = a.qp.q[gx + t * n + ci];
+      if (own_x) { pq = a.qp.q[gx + t * n + ci]; px = gxs[t * n + ci]; }
     };
     prefetch_state(N);
+    T pend = T(0);                                     // partial next eta of stage t+1 (see the eta pass)
     for (int t = N; t >= 0; --t) {
       if (t < N) {
         const T* L = acquire(0);
@@ -236,7 +249,7 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
         cons_bar();
       }
       if (a.kkt_only) continue;
-      const T zgo = pzg, ygo = pyg, lo_ = plo, hi_ = phi, yfo = pyf, cval = pc, qv = pq;
+      const T zgo = pzg, ygo = pyg, lo_ = plo, hi_ = phi, yfo = pyf, cval = pc, qv = pq, xo = px;
       prefetch_state(t - 1);
       if (own_g) {                                     // eq. 9-16 on inequality row (t, ci)
         const size_t row = gg + t * ng + ci;
@@ -250,7 +263,7 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
         if (lastit) a.xi[row] = s;
       }
       T xn = T(0);
-      if (own_x) { xn = alpha * e1[t * n + ci] + (T(1) - alpha) * xs[t * n + ci]; xs[t * n + ci] = xn; }
+      if (own_x) { xn = alpha * e1[t * n + ci] + (T(1) - alpha) * xo; gxs[t * n + ci] = xn; }
       const T* Am = nullptr; const T* Ap = nullptr;
       if (t < N) {
         Am = acquire(0); Ap = acquire(1);
@@ -264,21 +277,22 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
       T da = T(0), dp = T(0);
       if (t < N) { da = col_dot(Am, rbuf, nx); dp = col_dot(Ap, rbuf, nx); }
       if (own_x) {
-        T eta = sigma * xn - qv + gts(t, sbuf);
-        if (t < N) { eta += da; e0[(t + 1) * n + ci] += dp; }
-        if (t == 0 && own_f) {                         // rows x_0 = x_init (A_init = [I 0])
-          const T xi0 = a.qp.x_init[(size_t)p * nx + ci];
-          const T y = a.yf[gf + ci] + rho_f * alpha * (e1[ci] - xi0);
-          a.yf[gf + ci] = y; eta += rho_f * xi0 - y;
+        if (t < N) geta[(t + 1) * n + ci] = pend + dp;  // stage t+1 is complete
+        pend = sigma * xn - qv + gts(t, sbuf) + da;
+        if (t == 0) {
+          if (own_f) {                                 // rows x_0 = x_init (A_init = [I 0])
+            const T xi0 = a.qp.x_init[(size_t)p * nx + ci];
+            const T y = a.yf[gf + ci] + rho_f * alpha * (e1[ci] - xi0);
+            a.yf[gf + ci] = y; pend += rho_f * xi0 - y;
+          }
+          geta[ci] = pend;
         }
-        e0[t * n + ci] = eta;
       }
       if (t < N) release(2);
     }
   }
   cons_bar();
   if (a.kkt_only) { for (int e = ct; e < nz; e += ncons) a.xi[gx + e] = e1[e]; }
-  else for (int e = ct; e < nz; e += ncons) a.x[gx + e] = xs[e];
 }
 
 }  // namespace tmpc
