@@ -129,28 +129,31 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
       }
       __syncthreads();
     }
-    // ---- in-place Cholesky of P (lower), then Q <- X = L^{-1}  (X[k][i] row-major: row k of L^{-1})
+    // ---- in-place Cholesky of P (lower), then Q <- X = L^{-1}  (X[k][i] row-major: row k of L^{-1}).
+    // Right-looking; the scaled pivot column is first copied to a contiguous vector so that the rank-1 update reads it
+    // conflict free; a warp owns rows i, its lanes run along j (no index divisions).
+    double* colk = reinterpret_cast<double*>(S1);      // n doubles of scratch (the staging chunk is idle here)
+    const int lane = tid & 31, wid = tid >> 5, nwarp = nt >> 5;
     for (int k = 0; k < n; ++k) {
       double dk = P[(size_t)k * ld + k];
       if (!(dk > 0) || !isfinite(dk)) { bad = 1; dk = 1; }
-      const double inv = 1.0 / dk;
-      const int m = n - 1 - k;
-      for (int e = tid; e < m * m; e += nt) {
-        const int i = k + 1 + e / m, j = k + 1 + e % m;
-        if (j <= i) P[(size_t)i * ld + j] -= P[(size_t)i * ld + k] * P[(size_t)j * ld + k] * inv;
-      }
-      __syncthreads();
       const double sq = sqrt(dk), rs = 1.0 / sq;
-      for (int i = k + tid; i < n; i += nt) P[(size_t)i * ld + k] = (i == k) ? sq : P[(size_t)i * ld + k] * rs;
+      for (int i = k + tid; i < n; i += nt) { const double v = (i == k) ? sq : P[(size_t)i * ld + k] * rs; colk[i] = v; }
+      __syncthreads();
+      for (int i = k + 1 + wid; i < n; i += nwarp) {
+        const double lik = colk[i];
+        for (int j = k + 1 + lane; j <= i; j += 32) P[(size_t)i * ld + j] -= lik * colk[j];
+      }
+      for (int i = k + tid; i < n; i += nt) P[(size_t)i * ld + k] = colk[i];
+      __syncthreads();
     }
     for (int e = tid; e < ld * ld; e += nt) { const int i = e / ld, j = e - i * ld; Q[e] = (i == j && i < n) ? 1.0 : 0.0; }
     __syncthreads();
-    for (int k = 0; k < n - 1; ++k) {
+    for (int k = 0; k < n - 1; ++k) {                  // Y[i][0..k] -= (L[i][k] / L[k][k]) Y[k][0..k] for rows i > k
       const double inv = 1.0 / P[(size_t)k * ld + k];
-      const int m = n - 1 - k, kk = k + 1;
-      for (int e = tid; e < m * kk; e += nt) {
-        const int i = k + 1 + e / kk, j = e % kk;
-        Q[(size_t)i * ld + j] -= P[(size_t)i * ld + k] * Q[(size_t)k * ld + j] * inv;
+      for (int i = k + 1 + wid; i < n; i += nwarp) {
+        const double lik = P[(size_t)i * ld + k] * inv;
+        for (int j = lane; j <= k; j += 32) Q[(size_t)i * ld + j] -= lik * Q[(size_t)k * ld + j];
       }
       __syncthreads();
     }
