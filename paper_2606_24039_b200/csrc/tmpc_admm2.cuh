@@ -331,7 +331,9 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
 #ifdef TMPC_TIMING
       const long long c1 = clock64();
 #endif
+#ifndef TMPC_NO_CHAIN                                    // debug builds: measure the stage-parallel phases alone
       chain_warp_solve<T, NC, NX, PG>(sm, R, PP, T_, tid);
+#endif
       __syncwarp();
 #ifdef TMPC_TIMING
       tw += c1 - c0; ts += clock64() - c1;
@@ -504,7 +506,12 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
       if (fl[u] & F_DYN) {
         T am[n], ap[n], ya[n], yb[n];
         ld_vec<n>(sm + b + RC::AM + i * n, am); ld_vec<n>(sm + bn[u] + RC::AP + i * n, ap);
-        ld_operand(b, RC::E0, i, ya); ld_operand(bn[u], RC::E0, i, yb);
+        if constexpr (NC == 8 && sizeof(T) == 4) {      // y_t is already in registers (yv): permute instead of reloading
+          const bool sw4 = swz_x<T, NC>(i) != 0;
+#pragma unroll
+          for (int j = 0; j < n; ++j) ya[j] = sw4 ? yv[j ^ 4] : yv[j];
+        } else ld_operand(b, RC::E0, i, ya);
+        ld_operand(bn[u], RC::E0, i, yb);
         const T zt = dotv<n>(am, ya) + dotv<n>(ap, yb);
         yf[u] += A.rfa * (zt - cv[u]);
         put_r(u);
