@@ -92,7 +92,9 @@ __host__ __device__ inline Admm2Plan admm2_plan(const Dims& d, int pg) {
   using RC = Rec<T, NC, NX>;
   Admm2Plan P;
   int R = d.g_sel ? RC::S : RC::G + RC::up(d.ng * NC);
-  if (NC == 8) { const int mod = 128 / (int)sizeof(T), want = sizeof(T) == 4 ? 8 : 8; while (R % (sizeof(T) == 4 ? 32 : 16) != want) R += RC::V; (void)mod; }
+  // four lanes per stage, eight stages per warp: a stride of 4 (mod 32) words (fp32) puts the eight stages' rows in distinct banks
+  // (any stride = 4 mod 8 words: k R mod 32 runs through all multiples of 4 for k = 0..7)
+  if (NC == 8) { const int mod = sizeof(T) == 4 ? 8 : 16, want = sizeof(T) == 4 ? 4 : 8; while (R % mod != want) R += RC::V; }
   P.R = R;
   int pp = d.T * R + RC::SKEW;
   if (pg == 2 && NC == 8) { const int half = 64 / (int)sizeof(T); while (pp % (2 * half) != half) pp += RC::V; }
@@ -388,17 +390,27 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
   // Item (t, i < nx) owns the equality row i of dynamics block t (t < N) or of the init block (t = N: A^- = 0 in record N,
   // A^+ = A_init in record 0).  Inequality row r of stage t is owned by item (t, g_col[r]) for a selection G (so that
   // G'(.) and G x~ touch only the owner's own component) and by item (t, r) for a dense G.
-  constexpr int IPT = 2;
+  // The two items of a thread are rows i0 and i0 + n/2 of the SAME stage, so the stage's operand vectors (y_t, y_{t+1},
+  // r_t, r_{t-1}, the exchange vector) are loaded once per thread and serve both rows: the stage-parallel phases are bound
+  // by shared-memory wavefronts (measured: 0.69 of 1.22 ms at config 2 with the chain switched off), not by issue.
+  // PAIR needs a row's chunk swizzle to be undone on registers at compile time (not so for fp64 n = 8) and registers for
+  // the shared vectors (not so for fp32 n = 6 under the 56-register cap of three CTAs per SM: measured 4.72 vs 4.44 ms at
+  // config 4); those two shapes keep two rows of different stages per thread and load their operands per row.
+  constexpr int IPT = 2, HALF = NC / 2;
+  constexpr bool PAIR = (NC == 8 && sizeof(T) == 4) || (NC != 8 && sizeof(T) == 8);
+  static_assert(NC % 2 == 0, "two rows per thread");
+  const int per_p = T_ * HALF;                           // PAIR: threads per problem
+  const int pr_g = it_tid / per_p, pr_rem = it_tid - pr_g * per_p, pr_t = pr_rem / HALF, pr_i0 = pr_rem - pr_t * HALF;
+  auto item_g = [&](int u) { return PAIR ? pr_g : (it_tid + u * nti) / nz; };
+  auto item_el = [&](int u) { return PAIR ? pr_t * n + pr_i0 + u * HALF : (it_tid + u * nti) - item_g(u) * nz; };
   unsigned fl[IPT]; int bt[IPT], bn[IPT], it_i[IPT];
   T x[IPT], q[IPT], yf[IPT], cv[IPT], zg[IPT], yg[IPT], lo[IPT], hi[IPT];
   auto g_row = [&](int u) -> size_t {                    // global index of the inequality row of item u (recomputed: not kept live)
-    const int e = it_tid + u * nti, g = e / nz, el = e - g * nz, t = el / n;
-    return (size_t)(blockIdx.x * PG + g) * mg + t * ng + (int)((fl[u] >> F_ROW_SH) & 31u);
+    return (size_t)(blockIdx.x * PG + item_g(u)) * mg + (item_el(u) / n) * ng + (int)((fl[u] >> F_ROW_SH) & 31u);
   };
 #pragma unroll
   for (int u = 0; u < IPT; ++u) {
-    const int e = it_tid + u * nti;
-    const int g = e / nz, el = e - g * nz, t = el / n, i = el - t * n, p = blockIdx.x * PG + g;
+    const int g = item_g(u), el = item_el(u), t = el / n, i = el - t * n, p = blockIdx.x * PG + g;
     const bool valid = g < PG && p < d.B;
     fl[u] = 0u; it_i[u] = i; bt[u] = bn[u] = 0;
     x[u] = q[u] = yf[u] = cv[u] = zg[u] = yg[u] = lo[u] = hi[u] = T(0);
@@ -441,8 +453,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
         T gx;
         if (d.g_sel) gx = x[u];
         else {
-          const int e = it_tid + u * nti, g = e / nz, el = e - g * nz, t = el / n;
-          const T* gr = a.qp.G + a.qp.sG * (blockIdx.x * PG + g) + ((size_t)t * ng + it_i[u]) * n;
+          const T* gr = a.qp.G + a.qp.sG * (blockIdx.x * PG + item_g(u)) + ((size_t)(item_el(u) / n) * ng + it_i[u]) * n;
           gx = T(0);
           for (int j = 0; j < n; ++j) gx += gr[j] * sm[bt[u] + RC::D + j];
         }
@@ -471,18 +482,30 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
       sm[bt[u] + RC::D + it_i[u]] = dd;
     }
     group_sync();
+    // operand vectors of my stage, once for both rows (natural order; a row's chunk swizzle is undone on the registers)
+    auto for_row = [&](int u, const T (&nat)[n], T (&out)[n]) {       // NC = 8 fp32: rows >= 4 (u = 1) take the halves swapped
 #pragma unroll
-    for (int u = 0; u < IPT; ++u) {
-      if (!(fl[u] & F_VALID)) continue;
-      const int b = bt[u], i = it_i[u];
-      T xr[n], dv[n], am[nx], ap[nx], rm[nx], rp[nx];
-      ld_vec<n>(sm + b + RC::SINV + i * n, xr); ld_operand(b, RC::D, i, dv);
+      for (int j = 0; j < n; ++j) out[j] = (PAIR && NC == 8 && u == 1) ? nat[j ^ 4] : nat[j];
+    };
+    if (!PAIR || (fl[0] & F_VALID)) {                 // PAIR: both rows belong to the same (valid or padding) stage
+      T dop[n], rm[nx], rp[nx];
 #pragma unroll
-      for (int k = 0; k < nx; ++k) { am[k] = sm[b + RC::AM + sw(k, i)]; ap[k] = sm[b + RC::AP + sw(k, i)]; }
-      ld_vec<nx>(sm + b + RC::RM, rm); ld_vec<nx>(sm + b + RC::RP, rp);
-      T s = dotv<n>(xr, dv) + (dotv<nx>(am, rm) + dotv<nx>(ap, rp));
-      if (!d.g_sel) for (int r = 0; r < ng; ++r) s += sm[b + RC::G + r * n + i] * sm[b + RC::S + r];
-      sm[b + RC::E1 + i] = s;
+      for (int u = 0; u < IPT; ++u) {
+        if (!PAIR && !(fl[u] & F_VALID)) continue;
+        const int b = bt[u], i = it_i[u];
+        if (!PAIR || u == 0) {
+          if constexpr (PAIR) ld_vec<n>(sm + b + RC::D, dop); else ld_operand(b, RC::D, i, dop);
+          ld_vec<nx>(sm + b + RC::RM, rm); ld_vec<nx>(sm + b + RC::RP, rp);
+        }
+        T xr[n], dv[n], am[nx], ap[nx];
+        ld_vec<n>(sm + b + RC::SINV + i * n, xr);
+        for_row(u, dop, dv);
+#pragma unroll
+        for (int k = 0; k < nx; ++k) { am[k] = sm[b + RC::AM + sw(k, i)]; ap[k] = sm[b + RC::AP + sw(k, i)]; }
+        T s = dotv<n>(xr, dv) + (dotv<nx>(am, rm) + dotv<nx>(ap, rp));
+        if (!d.g_sel) for (int r = 0; r < ng; ++r) s += sm[b + RC::G + r * n + i] * sm[b + RC::S + r];
+        sm[b + RC::E1 + i] = s;
+      }
     }
 #ifdef TMPC_TIMING
     const long long c1 = clock64();
@@ -494,41 +517,43 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
 #endif
     // a7 + a8 on y: z~_f = A~^- y_t + A~^+ y_{t+1}, x~_i = X(:,i)' y_t, z~_g = x~_i or G~ y_t; relaxation (eq. 10),
     // projection (eq. 12-15), duals (eq. 16 / 44-45)
+    if (!PAIR || (fl[0] & F_VALID)) {
+      T yv[n], ybn[n];
 #pragma unroll
-    for (int u = 0; u < IPT; ++u) {
-      if (!(fl[u] & F_VALID)) continue;
-      const int b = bt[u], i = it_i[u];
-      T xc[n], yv[n];
+      for (int u = 0; u < IPT; ++u) {
+        if (!PAIR && !(fl[u] & F_VALID)) continue;
+        const int b = bt[u], i = it_i[u];
+        if (!PAIR || u == 0) {
+          ld_vec<n>(sm + b + RC::E0, yv);
+          if constexpr (PAIR) { if ((fl[0] | fl[1]) & F_DYN) ld_vec<n>(sm + bn[0] + RC::E0, ybn); }
+        }
+        T xc[n];
 #pragma unroll
-      for (int j = 0; j < n; ++j) xc[j] = sm[b + RC::SINV + sw(j, i)];
-      ld_vec<n>(sm + b + RC::E0, yv);
-      const T xt = dotv<n>(xc, yv);
-      if (fl[u] & F_DYN) {
-        T am[n], ap[n], ya[n], yb[n];
-        ld_vec<n>(sm + b + RC::AM + i * n, am); ld_vec<n>(sm + bn[u] + RC::AP + i * n, ap);
-        if constexpr (NC == 8 && sizeof(T) == 4) {      // y_t is already in registers (yv): permute instead of reloading
-          const bool sw4 = swz_x<T, NC>(i) != 0;
-#pragma unroll
-          for (int j = 0; j < n; ++j) ya[j] = sw4 ? yv[j ^ 4] : yv[j];
-        } else ld_operand(b, RC::E0, i, ya);
-        ld_operand(bn[u], RC::E0, i, yb);
-        const T zt = dotv<n>(am, ya) + dotv<n>(ap, yb);
-        yf[u] += A.rfa * (zt - cv[u]);
-        put_r(u);
+        for (int j = 0; j < n; ++j) xc[j] = sm[b + RC::SINV + sw(j, i)];
+        const T xt = dotv<n>(xc, yv);
+        if (fl[u] & F_DYN) {
+          T am[n], ap[n], ya[n], yb[n];
+          ld_vec<n>(sm + b + RC::AM + i * n, am); ld_vec<n>(sm + bn[u] + RC::AP + i * n, ap);
+          if constexpr (PAIR) { for_row(u, yv, ya); for_row(u, ybn, yb); }
+          else { ld_operand(b, RC::E0, i, ya); ld_operand(bn[u], RC::E0, i, yb); }
+          const T zt = dotv<n>(am, ya) + dotv<n>(ap, yb);
+          yf[u] += A.rfa * (zt - cv[u]);
+          put_r(u);
+        }
+        if (fl[u] & F_INEQ) {
+          T ztg = xt;
+          if (!d.g_sel) { T gr[n]; ld_vec<n>(sm + b + RC::G + i * n, gr); ztg = dotv<n>(gr, yv); }
+          const T zh = a.prm.alpha * ztg + A.oma * zg[u];
+          const T v = zh + yg[u] * A.inv_rho_g;
+          T z, s;
+          project_row<T>((fl[u] & F_SOFT) != 0, v, lo[u], hi[u], a.prm.rho_g, A.inv_rg, a.prm.lam, z, s);
+          yg[u] += a.prm.rho_g * (zh - z);
+          zg[u] = z;
+          if (!d.g_sel) sm[b + RC::S + i] = a.prm.rho_g * z - yg[u];
+          if (it == a.iters - 1) a.xi[g_row(u)] = s;
+        }
+        x[u] = a.prm.alpha * xt + A.oma * x[u];
       }
-      if (fl[u] & F_INEQ) {
-        T ztg = xt;
-        if (!d.g_sel) { T gr[n]; ld_vec<n>(sm + b + RC::G + i * n, gr); ztg = dotv<n>(gr, yv); }
-        const T zh = a.prm.alpha * ztg + A.oma * zg[u];
-        const T v = zh + yg[u] * A.inv_rho_g;
-        T z, s;
-        project_row<T>((fl[u] & F_SOFT) != 0, v, lo[u], hi[u], a.prm.rho_g, A.inv_rg, a.prm.lam, z, s);
-        yg[u] += a.prm.rho_g * (zh - z);
-        zg[u] = z;
-        if (!d.g_sel) sm[b + RC::S + i] = a.prm.rho_g * z - yg[u];
-        if (it == a.iters - 1) a.xi[g_row(u)] = s;
-      }
-      x[u] = a.prm.alpha * xt + A.oma * x[u];
     }
 #ifdef TMPC_TIMING
     const long long c3 = clock64();
@@ -546,7 +571,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
 #pragma unroll
   for (int u = 0; u < IPT; ++u) {
     if (!(fl[u] & F_VALID)) continue;
-    const int e = it_tid + u * nti, g = e / nz, el = e - g * nz, t = el / n, i = it_i[u], p = blockIdx.x * PG + g;
+    const int el = item_el(u), t = el / n, i = it_i[u], p = blockIdx.x * PG + item_g(u);
     a.x[(size_t)p * nz + el] = x[u];
     if (fl[u] & F_DYN) a.yf[(size_t)p * mf + (t < N ? nx + t * nx + i : i)] = yf[u];
     if (fl[u] & F_INEQ) { const size_t row = g_row(u); a.zg[row] = zg[u]; a.yg[row] = yg[u]; }
