@@ -405,6 +405,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
   auto item_el = [&](int u) { return PAIR ? pr_t * n + pr_i0 + u * HALF : (it_tid + u * nti) - item_g(u) * nz; };
   unsigned fl[IPT]; int bt[IPT], bn[IPT], it_i[IPT];
   T x[IPT], q[IPT], yf[IPT], cv[IPT], zg[IPT], yg[IPT], lo[IPT], hi[IPT];
+  T xi_last[IPT] = {T(0), T(0)};                         // slack of the last iteration, written back after the loop
   auto g_row = [&](int u) -> size_t {                    // global index of the inequality row of item u (recomputed: not kept live)
     return (size_t)(blockIdx.x * PG + item_g(u)) * mg + (item_el(u) / n) * ng + (int)((fl[u] >> F_ROW_SH) & 31u);
   };
@@ -485,23 +486,36 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
     // operand vectors of my stage, once for both rows (natural order; a row's chunk swizzle is undone on the registers)
     auto for_row = [&](int u, const T (&nat)[n], T (&out)[n]) {       // NC = 8 fp32: rows >= 4 (u = 1) take the halves swapped
 #pragma unroll
-      for (int j = 0; j < n; ++j) out[j] = (PAIR && NC == 8 && u == 1) ? nat[j ^ 4] : nat[j];
+      for (int j = 0; j < n; ++j) out[j] = (NC == 8 && u == 1) ? nat[j ^ 4] : nat[j];
     };
-    if (!PAIR || (fl[0] & F_VALID)) {                 // PAIR: both rows belong to the same (valid or padding) stage
-      T dop[n], rm[nx], rp[nx];
+    if constexpr (PAIR) {
+      if (fl[0] & F_VALID) {                           // both rows belong to the same (valid or padding) stage
+        const int b = bt[0];
+        T dnat[n], rm[nx], rp[nx];
+        ld_vec<n>(sm + b + RC::D, dnat); ld_vec<nx>(sm + b + RC::RM, rm); ld_vec<nx>(sm + b + RC::RP, rp);
+#pragma unroll
+        for (int u = 0; u < IPT; ++u) {
+          const int i = it_i[u];
+          T xr[n], dv[n], am[nx], ap[nx];
+          ld_vec<n>(sm + b + RC::SINV + i * n, xr);
+          for_row(u, dnat, dv);
+#pragma unroll
+          for (int k = 0; k < nx; ++k) { am[k] = sm[b + RC::AM + sw(k, i)]; ap[k] = sm[b + RC::AP + sw(k, i)]; }
+          T s = dotv<n>(xr, dv) + (dotv<nx>(am, rm) + dotv<nx>(ap, rp));
+          if (!d.g_sel) for (int r = 0; r < ng; ++r) s += sm[b + RC::G + r * n + i] * sm[b + RC::S + r];
+          sm[b + RC::E1 + i] = s;
+        }
+      }
+    } else {
 #pragma unroll
       for (int u = 0; u < IPT; ++u) {
-        if (!PAIR && !(fl[u] & F_VALID)) continue;
+        if (!(fl[u] & F_VALID)) continue;
         const int b = bt[u], i = it_i[u];
-        if (!PAIR || u == 0) {
-          if constexpr (PAIR) ld_vec<n>(sm + b + RC::D, dop); else ld_operand(b, RC::D, i, dop);
-          ld_vec<nx>(sm + b + RC::RM, rm); ld_vec<nx>(sm + b + RC::RP, rp);
-        }
-        T xr[n], dv[n], am[nx], ap[nx];
-        ld_vec<n>(sm + b + RC::SINV + i * n, xr);
-        for_row(u, dop, dv);
+        T xr[n], dv[n], am[nx], ap[nx], rm[nx], rp[nx];
+        ld_vec<n>(sm + b + RC::SINV + i * n, xr); ld_operand(b, RC::D, i, dv);
 #pragma unroll
         for (int k = 0; k < nx; ++k) { am[k] = sm[b + RC::AM + sw(k, i)]; ap[k] = sm[b + RC::AP + sw(k, i)]; }
+        ld_vec<nx>(sm + b + RC::RM, rm); ld_vec<nx>(sm + b + RC::RP, rp);
         T s = dotv<n>(xr, dv) + (dotv<nx>(am, rm) + dotv<nx>(ap, rp));
         if (!d.g_sel) for (int r = 0; r < ng; ++r) s += sm[b + RC::G + r * n + i] * sm[b + RC::S + r];
         sm[b + RC::E1 + i] = s;
@@ -517,25 +531,61 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
 #endif
     // a7 + a8 on y: z~_f = A~^- y_t + A~^+ y_{t+1}, x~_i = X(:,i)' y_t, z~_g = x~_i or G~ y_t; relaxation (eq. 10),
     // projection (eq. 12-15), duals (eq. 16 / 44-45)
-    if (!PAIR || (fl[0] & F_VALID)) {
-      T yv[n], ybn[n];
+    if constexpr (PAIR) {
+      if (fl[0] & F_VALID) {
+        const int b = bt[0];
+        T yv[n], ybn[n];
+        ld_vec<n>(sm + b + RC::E0, yv);
+        if ((fl[0] | fl[1]) & F_DYN) ld_vec<n>(sm + bn[0] + RC::E0, ybn);
+#pragma unroll
+        for (int u = 0; u < IPT; ++u) {
+          const int i = it_i[u];
+          T xc[n];
+#pragma unroll
+          for (int j = 0; j < n; ++j) xc[j] = sm[b + RC::SINV + sw(j, i)];
+          const T xt = dotv<n>(xc, yv);
+          if (fl[u] & F_DYN) {
+            T am[n], ap[n], ya[n], yb[n];
+            ld_vec<n>(sm + b + RC::AM + i * n, am); ld_vec<n>(sm + bn[u] + RC::AP + i * n, ap);
+            for_row(u, yv, ya); for_row(u, ybn, yb);
+            const T zt = dotv<n>(am, ya) + dotv<n>(ap, yb);
+            yf[u] += A.rfa * (zt - cv[u]);
+            put_r(u);
+          }
+          if (fl[u] & F_INEQ) {
+            T ztg = xt;
+            if (!d.g_sel) { T gr[n]; ld_vec<n>(sm + b + RC::G + i * n, gr); ztg = dotv<n>(gr, yv); }
+            const T zh = a.prm.alpha * ztg + A.oma * zg[u];
+            const T v = zh + yg[u] * A.inv_rho_g;
+            T z, s;
+            project_row<T>((fl[u] & F_SOFT) != 0, v, lo[u], hi[u], a.prm.rho_g, A.inv_rg, a.prm.lam, z, s);
+            yg[u] += a.prm.rho_g * (zh - z);
+            zg[u] = z;
+            if (!d.g_sel) sm[b + RC::S + i] = a.prm.rho_g * z - yg[u];
+            xi_last[u] = s;
+          }
+          x[u] = a.prm.alpha * xt + A.oma * x[u];
+        }
+      }
+    } else {
 #pragma unroll
       for (int u = 0; u < IPT; ++u) {
-        if (!PAIR && !(fl[u] & F_VALID)) continue;
+        if (!(fl[u] & F_VALID)) continue;
         const int b = bt[u], i = it_i[u];
-        if (!PAIR || u == 0) {
-          ld_vec<n>(sm + b + RC::E0, yv);
-          if constexpr (PAIR) { if ((fl[0] | fl[1]) & F_DYN) ld_vec<n>(sm + bn[0] + RC::E0, ybn); }
-        }
-        T xc[n];
+        T xc[n], yv[n];
 #pragma unroll
         for (int j = 0; j < n; ++j) xc[j] = sm[b + RC::SINV + sw(j, i)];
+        ld_vec<n>(sm + b + RC::E0, yv);
         const T xt = dotv<n>(xc, yv);
         if (fl[u] & F_DYN) {
           T am[n], ap[n], ya[n], yb[n];
           ld_vec<n>(sm + b + RC::AM + i * n, am); ld_vec<n>(sm + bn[u] + RC::AP + i * n, ap);
-          if constexpr (PAIR) { for_row(u, yv, ya); for_row(u, ybn, yb); }
-          else { ld_operand(b, RC::E0, i, ya); ld_operand(bn[u], RC::E0, i, yb); }
+          if constexpr (NC == 8 && sizeof(T) == 4) {      // y_t is already in registers (yv): permute instead of reloading
+            const bool sw4 = swz_x<T, NC>(i) != 0;
+#pragma unroll
+            for (int j = 0; j < n; ++j) ya[j] = sw4 ? yv[j ^ 4] : yv[j];
+          } else ld_operand(b, RC::E0, i, ya);
+          ld_operand(bn[u], RC::E0, i, yb);
           const T zt = dotv<n>(am, ya) + dotv<n>(ap, yb);
           yf[u] += A.rfa * (zt - cv[u]);
           put_r(u);
@@ -550,7 +600,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
           yg[u] += a.prm.rho_g * (zh - z);
           zg[u] = z;
           if (!d.g_sel) sm[b + RC::S + i] = a.prm.rho_g * z - yg[u];
-          if (it == a.iters - 1) a.xi[g_row(u)] = s;
+          xi_last[u] = s;
         }
         x[u] = a.prm.alpha * xt + A.oma * x[u];
       }
@@ -574,7 +624,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
     const int el = item_el(u), t = el / n, i = it_i[u], p = blockIdx.x * PG + item_g(u);
     a.x[(size_t)p * nz + el] = x[u];
     if (fl[u] & F_DYN) a.yf[(size_t)p * mf + (t < N ? nx + t * nx + i : i)] = yf[u];
-    if (fl[u] & F_INEQ) { const size_t row = g_row(u); a.zg[row] = zg[u]; a.yg[row] = yg[u]; }
+    if (fl[u] & F_INEQ) { const size_t row = g_row(u); a.zg[row] = zg[u]; a.yg[row] = yg[u]; if (a.iters > 0) a.xi[row] = xi_last[u]; }
   }
 }
 
