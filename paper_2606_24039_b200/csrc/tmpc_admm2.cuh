@@ -94,7 +94,7 @@ __host__ __device__ inline Admm2Plan admm2_plan(const Dims& d, int pg) {
   int R = d.g_sel ? RC::S : RC::G + RC::up(d.ng * NC);
   // four lanes per stage, eight stages per warp: a stride of 4 (mod 32) words (fp32) puts the eight stages' rows in distinct banks
   // (any stride = 4 mod 8 words: k R mod 32 runs through all multiples of 4 for k = 0..7)
-  if (NC == 8) { const int mod = sizeof(T) == 4 ? 8 : 16, want = sizeof(T) == 4 ? 4 : 8; while (R % mod != want) R += RC::V; }
+  if (NC == 8) { while (R % 8 != 4) R += RC::V; }
   P.R = R;
   int pp = d.T * R + RC::SKEW;
   if (pg == 2 && NC == 8) { const int half = 64 / (int)sizeof(T); while (pp % (2 * half) != half) pp += RC::V; }
@@ -393,11 +393,11 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
   // The two items of a thread are rows i0 and i0 + n/2 of the SAME stage, so the stage's operand vectors (y_t, y_{t+1},
   // r_t, r_{t-1}, the exchange vector) are loaded once per thread and serve both rows: the stage-parallel phases are bound
   // by shared-memory wavefronts (measured: 0.69 of 1.22 ms at config 2 with the chain switched off), not by issue.
-  // PAIR needs a row's chunk swizzle to be undone on registers at compile time (not so for fp64 n = 8) and registers for
-  // the shared vectors (not so for fp32 n = 6 under the 56-register cap of three CTAs per SM: measured 4.72 vs 4.44 ms at
-  // config 4); those two shapes keep two rows of different stages per thread and load their operands per row.
+  // A row's chunk swizzle is undone on the registers (compile-time half swap for rows >= n/2, plus one select level for
+  // fp64 n = 8).  PAIR needs registers for the shared vectors: not so for fp32 n = 6 under the 56-register cap of three
+  // CTAs per SM (measured 4.72 vs 4.44 ms at config 4), which keeps two rows of different stages per thread.
   constexpr int IPT = 2, HALF = NC / 2;
-  constexpr bool PAIR = (NC == 8 && sizeof(T) == 4) || (NC != 8 && sizeof(T) == 8);
+  constexpr bool PAIR = NC == 8 || sizeof(T) == 8;
   static_assert(NC % 2 == 0, "two rows per thread");
   const int per_p = T_ * HALF;                           // PAIR: threads per problem
   const int pr_g = it_tid / per_p, pr_rem = it_tid - pr_g * per_p, pr_t = pr_rem / HALF, pr_i0 = pr_rem - pr_t * HALF;
@@ -484,9 +484,13 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
     }
     group_sync();
     // operand vectors of my stage, once for both rows (natural order; a row's chunk swizzle is undone on the registers)
-    auto for_row = [&](int u, const T (&nat)[n], T (&out)[n]) {       // NC = 8 fp32: rows >= 4 (u = 1) take the halves swapped
+    auto for_row = [&](int u, const T (&nat)[n], T (&out)[n]) {       // natural order -> chunk order of row it_i[u] (see Rec)
 #pragma unroll
-      for (int j = 0; j < n; ++j) out[j] = (NC == 8 && u == 1) ? nat[j ^ 4] : nat[j];
+      for (int j = 0; j < n; ++j) {
+        if constexpr (NC != 8) out[j] = nat[j];
+        else if constexpr (sizeof(T) == 4) out[j] = nat[j ^ (4 * u)];
+        else out[j] = ((it_i[u] >> 1) & 1) ? nat[j ^ (4 * u) ^ 2] : nat[j ^ (4 * u)];      // fp64: chunks of two, swizzle (row >> 1) & 3
+      }
     };
     if constexpr (PAIR) {
       if (fl[0] & F_VALID) {                           // both rows belong to the same (valid or padding) stage
