@@ -150,6 +150,10 @@ template <int L> __device__ __forceinline__ void pin_vec(double (&r)[L]) {
   else if constexpr (L == 6) asm volatile("" : "+d"(r[0]), "+d"(r[1]), "+d"(r[2]), "+d"(r[3]), "+d"(r[4]), "+d"(r[5]));
 }
 
+// rows of one stage handled by a thread: 3 for fp32 n = 6 (three CTAs per SM leave 80 registers per thread only with
+// 256-thread CTAs), else 2
+template <typename T, int NC> __host__ __device__ constexpr int admm2_ipt() { return (NC == 6 && sizeof(T) == 4) ? 3 : 2; }
+
 template <typename T>
 struct Admm2Args {
   AdmmArgs<T> a;
@@ -396,16 +400,18 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
   // A row's chunk swizzle is undone on the registers (compile-time half swap for rows >= n/2, plus one select level for
   // fp64 n = 8).  PAIR needs registers for the shared vectors: not so for fp32 n = 6 under the 56-register cap of three
   // CTAs per SM (measured 4.72 vs 4.44 ms at config 4), which keeps two rows of different stages per thread.
-  constexpr int IPT = 2, HALF = NC / 2;
-  constexpr bool PAIR = NC == 8 || sizeof(T) == 8;
-  static_assert(NC % 2 == 0, "two rows per thread");
+  constexpr int IPT = admm2_ipt<T, NC>(), HALF = NC / IPT;     // rows i0, i0 + HALF, .. of one stage per thread
+  constexpr bool PAIR = true;
+  static_assert(NC % IPT == 0 && (NC != 8 || IPT == 2), "rows per thread");
   const int per_p = T_ * HALF;                           // PAIR: threads per problem
   const int pr_g = it_tid / per_p, pr_rem = it_tid - pr_g * per_p, pr_t = pr_rem / HALF, pr_i0 = pr_rem - pr_t * HALF;
   auto item_g = [&](int u) { return PAIR ? pr_g : (it_tid + u * nti) / nz; };
   auto item_el = [&](int u) { return PAIR ? pr_t * n + pr_i0 + u * HALF : (it_tid + u * nti) - item_g(u) * nz; };
   unsigned fl[IPT]; int bt[IPT], bn[IPT], it_i[IPT];
   T x[IPT], q[IPT], yf[IPT], cv[IPT], zg[IPT], yg[IPT], lo[IPT], hi[IPT];
-  T xi_last[IPT] = {T(0), T(0)};                         // slack of the last iteration, written back after the loop
+  T xi_last[IPT];                                        // slack of the last iteration, written back after the loop
+#pragma unroll
+  for (int u = 0; u < IPT; ++u) xi_last[u] = T(0);
   auto g_row = [&](int u) -> size_t {                    // global index of the inequality row of item u (recomputed: not kept live)
     return (size_t)(blockIdx.x * PG + item_g(u)) * mg + (item_el(u) / n) * ng + (int)((fl[u] >> F_ROW_SH) & 31u);
   };
@@ -540,7 +546,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm2_kernel(const __grid_constant
         const int b = bt[0];
         T yv[n], ybn[n];
         ld_vec<n>(sm + b + RC::E0, yv);
-        if ((fl[0] | fl[1]) & F_DYN) ld_vec<n>(sm + bn[0] + RC::E0, ybn);
+        if (fl[0] & F_DYN) ld_vec<n>(sm + bn[0] + RC::E0, ybn);     // row i0 < n / IPT <= nx is a dynamics row whenever any is
 #pragma unroll
         for (int u = 0; u < IPT; ++u) {
           const int i = it_i[u];

@@ -173,7 +173,8 @@ FastPlan fast_plan(const Dims& d) {
   if (s1 > kMaxSmem) return f;
   const int c1 = (int)(kSmemPerSM / (s1 + 1024)), c2 = s2 <= kMaxSmem ? (int)(kSmemPerSM / (s2 + 1024)) : 0;
   f.pg = (d.B >= 2 && c2 >= 2 && 2 * c2 >= c1) ? 2 : 1;
-  auto threads = [&](int pg) { int t = ((pg * d.nz + 1) / 2 + 31) / 32 * 32; return 32 + (t < 32 ? 32 : t); };   // + the chain warp
+  const int ipt = d.n == 8 ? admm2_ipt<T, 8>() : admm2_ipt<T, 6>();
+  auto threads = [&](int pg) { int t = ((pg * d.nz + ipt - 1) / ipt + 31) / 32 * 32; return 32 + (t < 32 ? 32 : t); };   // + the chain warp
   const int tmax = sizeof(T) == 8 ? 512 : 1024;
   if (threads(f.pg) > tmax) f.pg = 1;
   f.nt = threads(f.pg);
@@ -196,6 +197,7 @@ template <typename T, int NC, int NX, int PG>
 tmpc_status launch_admm2_shape(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
   if constexpr (sizeof(T) == 8) return launch_admm2_inst<T, NC, NX, PG, 512, 1>(h, a, f);
   else {
+    if (f.nt <= 256 && f.ctas_per_sm >= 3) return launch_admm2_inst<T, NC, NX, PG, 256, 3>(h, a, f);
     if (f.nt <= 384 && f.ctas_per_sm >= 3) return launch_admm2_inst<T, NC, NX, PG, 384, 3>(h, a, f);
     if (f.nt <= 448) return launch_admm2_inst<T, NC, NX, PG, 448, 2>(h, a, f);
     return launch_admm2_inst<T, NC, NX, PG, 1024, 1>(h, a, f);
