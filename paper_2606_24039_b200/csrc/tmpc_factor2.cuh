@@ -36,7 +36,7 @@ __global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
   constexpr int GMAX = NC * NC;                         // room for ng <= n rows of G
   constexpr int RAW = 2 * nn + 2 * an + GMAX;           // D, E, Am, Ap, G
   constexpr int RPL = (RAW + 31) / 32;
-  __shared__ double sm[2][3 * nn + RAW];
+  __shared__ double sm[2][3 * nn + RAW + NC];
   const Dims& d = a.d;
   const int ng = d.ng, N = d.N, T_ = d.T;
   const int half = threadIdx.x >> 5, lane = threadIdx.x & 31, p = blockIdx.x;
@@ -103,13 +103,17 @@ __global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
       dst[e] = s;
     }
   };
-  // in-place Cholesky of the lower triangle of Am_ (right-looking), then Xo <- L^{-1}
+  // in-place Cholesky of the lower triangle of Am_ (right-looking), then Xo <- L^{-1}.  One rsqrt per pivot and no
+  // division: 1 / L_kk is kept in registers (compile-time k) and in `rsd` for the final row scaling.
+  double* rsd = sm[half] + 3 * nn + RAW;
   auto chol_inv = [&](double* Am_, double* Xo) {
+    double rsk[n];
 #pragma unroll
     for (int k = 0; k < n; ++k) {
       double dk = Am_[k * n + k];
       if (!(dk > 0) || !isfinite(dk)) { bad = 1; dk = 1; }
-      const double inv = 1.0 / dk, sq = sqrt(dk), rs = 1.0 / sq;
+      const double rs = rsqrt(dk), sq = dk * rs, inv = rs * rs;
+      rsk[k] = rs;
 #pragma unroll
       for (int u = 0; u < EPL; ++u) {
         const int e = lane + 32 * u, i = e / n, j = e % n;
@@ -117,6 +121,7 @@ __global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
       }
       __syncwarp();
       if (lane < n && lane >= k) Am_[lane * n + k] = lane == k ? sq : Am_[lane * n + k] * rs;
+      if (lane == 0) rsd[k] = rs;
       __syncwarp();
     }
 #pragma unroll
@@ -124,7 +129,7 @@ __global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
     __syncwarp();
 #pragma unroll
     for (int k = 0; k < n - 1; ++k) {
-      const double inv = 1.0 / Am_[k * n + k];
+      const double inv = rsk[k];
 #pragma unroll
       for (int u = 0; u < EPL; ++u) {
         const int e = lane + 32 * u, i = e / n, j = e % n;
@@ -133,7 +138,7 @@ __global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
       __syncwarp();
     }
 #pragma unroll
-    for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u; if (e < nn) Xo[e] = Xo[e] / Am_[(e / n) * n + (e / n)]; }
+    for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u; if (e < nn) Xo[e] = Xo[e] * rsd[e / n]; }
     __syncwarp();
   };
   auto x_out = [&](int t, const double* X) {
