@@ -4,8 +4,9 @@
 // Design:
 //  * a CTA owns PG problems (1 or 2).  The factor (X_t, -B_t) and the constraint blocks carried into the scaled
 //    variables (A~^- = A^- X', A~^+ = A^+ X_next', G~ = G X') sit in shared memory for all iterations; the per-row ADMM
-//    state (x, q, y_f, c, z_g, y_g, lo, hi) lives in REGISTERS of the thread that owns the row: two (problem, stage,
-//    row) items per thread, fixed for the launch.
+//    state (x, q, y_f, c, z_g, y_g, lo, hi) lives in REGISTERS of the thread that owns the row: two or three rows of
+//    ONE stage per thread, fixed for the launch, so the stage's operand vectors are loaded once per thread (the
+//    stage-parallel phases are bound by shared-memory wavefronts).
 //  * x~ = S^{-1} eta (eq. 8) runs on a dedicated chain warp (warp 0): lanes = (problem, direction, row), 8 lanes per
 //    slot, so the up chain and the down chain of the twisted factor of up to two problems advance together; a step is
 //    one n x n mat-vec whose operand vector is published with one STS and read back as a broadcast vector load.
