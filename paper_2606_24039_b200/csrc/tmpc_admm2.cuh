@@ -217,8 +217,26 @@ __device__ __forceinline__ void chain_warp_solve(T* sm, int R, int PP, int T_, i
   T wv = cnt > 0 ? lds_1(bt + oE1 + me, T(0)) : T(0);
   T Br[n];
   lds_row<T, NC>(bt + myrow, 0u, Br);
+  // steps in which every active slot is on and none is at its last stage run without per-lane predicates
+  const int cmin = T_ - 1 - m;                          // = the down chain's length <= the up chain's (m)
+  const int kmain = cmin > 1 ? cmin - 1 : 0;
+  const int dRa = act ? dRb : 0;                        // idle lanes stay on record m
 #pragma unroll 1
-  for (int k = 0; k < m; ++k) {                        // w_next = eta~_next + (-B_t) w_t
+  for (int k = 0; k < kmain; ++k) {
+    if (act) sts_1(bt + oE1 + me, wv);
+    __syncwarp();
+    T W[n];
+    lds_row<T, NC>(bt + oE1, swb, W);
+    bt += dRa;
+    const T eta = lds_1(bt + oE1 + me, T(0));
+    T Bn[n];
+    lds_row<T, NC>(bt + myrow, 0u, Bn);
+    wv = dotv_from<n>(Br, W, eta);
+#pragma unroll
+    for (int j = 0; j < n; ++j) Br[j] = Bn[j];
+  }
+#pragma unroll 1
+  for (int k = kmain; k < m; ++k) {                    // w_next = eta~_next + (-B_t) w_t
     const bool on = k < cnt, last = k == cnt - 1;
     if (on) sts_1(bt + oE1 + me, wv);
     __syncwarp();
