@@ -284,7 +284,7 @@ def run_gpu(args):
     roof["frac"] = roof["achieved"] / roof["peak"]
     # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed `ncu --set full` captures
     # (profiles/r01_v2_ncu_full_*.md); only valid for the workload the capture was taken on
-    ncu_traffic = {(2, "f32", 1024): 57.05e6 + 0.62e6, (3, "f32", 512): 445.52e9 + 3.91e9}
+    ncu_traffic = {(2, "f32", 1024): 57.05e6 + 0.29e6, (3, "f32", 512): 445.52e9 + 3.91e9}
     roof["traffic"] = ncu_traffic.get((args.config, args.dtype, w.B))
     roof["kernel"] = {1: "admm2_kernel", 2: "admm2_kernel", 3: "admm_stream_kernel", 4: "admm2_kernel", 5: "cr2_admm_kernel"}[args.config] + " (tmpc_admm_solve)"
     if args.config in (1, 2, 4):
@@ -295,7 +295,7 @@ def run_gpu(args):
         lds_peak = 148 * 128 * 1.965e9 / 1e9
         roof["lds"] = {"achieved": lds_bytes / (kern_avg_ms * 1e-3) / 1e9, "peak": lds_peak, "unit": "GB/s", "frac": lds_bytes / (kern_avg_ms * 1e-3) / 1e9 / lds_peak,
                        "note": "algorithmic shared-memory bytes (B twice, X twice, A~-/A~+ twice per iteration) / kernel time",
-                       "lsu_wavefront_util_ncu": {(2, "f32", 1024): 0.478}.get((args.config, args.dtype, w.B))}   # l1tex__data_pipe_lsu_wavefronts_mem_shared pct of peak, profiles/
+                       "lsu_wavefront_util_ncu": {(2, "f32", 1024): 0.523}.get((args.config, args.dtype, w.B))}   # l1tex__data_pipe_lsu_wavefronts_mem_shared pct of peak, profiles/
     roof["kernel_ms_per_launch"] = kern_avg_ms
     roof["kernel_share_of_step"] = sum(kern_ms) / sum(step_ms)
     line = {"metric": "batched QP solves/s", "value": value, "unit": "QP solves/s", "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
