@@ -11,7 +11,16 @@
 #pragma once
 #include "tmpc_factor.cuh"
 
+#include <type_traits>
+
 namespace tmpc {
+
+// fused Cholesky / inverse of factor3_kernel: 16 warps x F3_RMAX rows, 32 lanes x F3_CMAX chunks cover n <= 96; scratch buffer
+// = colk[96], rowk[96], d_k (+ pad) doubles
+constexpr int F3_RMAX = 6, F3_CMAX = 3, F3_SB = 2 * 96 + 2;
+template <int V> using f3_ic = std::integral_constant<int, V>;
+__device__ __forceinline__ double f3_lds(unsigned a) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
+__device__ __forceinline__ void f3_sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
 
 template <typename T> __host__ __device__ constexpr int f3_ch() { return sizeof(T) == 4 ? 32 : 16; }   // rows of A^-/A^+/G staged per chunk (in the working dtype)
 
@@ -84,6 +93,12 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
   const bool has_tile = tid < tiles;
   const int ti = has_tile ? tid / nt4 : 0, tj = has_tile ? tid - ti * nt4 : 0, i0 = 4 * ti, j0 = 4 * tj;
 
+#ifdef TMPC_F3_PROF
+  long long tk[8] = {}, tc = clock64();
+#define F3_TICK(i) { long long c_ = clock64(); tk[i] += c_ - tc; tc = c_; }
+#else
+#define F3_TICK(i)
+#endif
   for (int t = 0; t < T_; ++t) {
     // ---- P <- Theta_t - Lambda_{t-1} Phi_{t-1}'   (R = Lambda', Q = Phi' of the previous stage)
     {
@@ -129,36 +144,86 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
       }
       __syncthreads();
     }
-    // ---- in-place Cholesky of P (lower), then Q <- X = L^{-1}  (X[k][i] row-major: row k of L^{-1}).
-    // Right-looking; the scaled pivot column is first copied to a contiguous vector so that the rank-1 update reads it
-    // conflict free; a warp owns rows i, its lanes run along j (no index divisions).
-    double* colk = reinterpret_cast<double*>(S1);      // n doubles of scratch (the staging chunk is idle here)
-    const int lane = tid & 31, wid = tid >> 5, nwarp = nt >> 5;
-    for (int k = 0; k < n; ++k) {
-      double dk = P[(size_t)k * ld + k];
-      if (!(dk > 0) || !isfinite(dk)) { bad = 1; dk = 1; }
-      const double sq = sqrt(dk), rs = 1.0 / sq;
-      for (int i = k + tid; i < n; i += nt) { const double v = (i == k) ? sq : P[(size_t)i * ld + k] * rs; colk[i] = v; }
+    F3_TICK(0)
+    // ---- Cholesky of P and X = L^{-1} TOGETHER, both held in registers: warp w owns rows i = w + 16 r, lane l owns columns
+    // j = l + 32 c of P (symmetric, being reduced) and of Y (starts as I, becomes diag(L) X).  Step k: the owners publish
+    // column k of the reduced P (u_i, zero for i <= k), row k of Y and the pivot d_k in a double-buffered scratch (ONE CTA
+    // barrier per column); then every thread applies  P[i][j] -= (u_i / d_k) u_j  and  Y[i][j] -= (u_i / d_k) Y[k][j]  to its
+    // own registers (l_ik l_jk = u_i u_j / d_k and l_ik / l_kk = u_i / d_k: L itself is never formed).  The columns are
+    // walked in six compile-time groups of 16 (row slot r of the pivot row and the live 32-column chunks are constants
+    // inside a group; the only run-time conditions are warp uniform).  At the end X[i][j] = Y[i][j] / sqrt(d_i) goes to Q.
+    {
+      const int lane = tid & 31, wid = tid >> 5;
+      const unsigned scr = (unsigned)__cvta_generic_to_shared(S1);   // the staging chunks are idle here (>= 8 KB)
+      const unsigned a_row = scr + 8u * wid, a_col = scr + 8u * lane;  // colk[i] broadcast per warp / colk[j], rowk[j] per lane
+      double pv[F3_RMAX][F3_CMAX], yv[F3_RMAX][F3_CMAX];
+      for (int e = tid; e < 2 * F3_SB + 96; e += nt) f3_sts(scr + 8u * e, 0.0);       // tails (i, j >= n) stay zero
+#pragma unroll
+      for (int r = 0; r < F3_RMAX; ++r)
+#pragma unroll
+        for (int c = 0; c < F3_CMAX; ++c) {
+          const int i = wid + 16 * r, j = lane + 32 * c;
+          pv[r][c] = (i < n && j < n) ? P[(size_t)i * ld + j] : 0.0;
+          yv[r][c] = (i == j) ? 1.0 : 0.0;
+        }
       __syncthreads();
-      for (int i = k + 1 + wid; i < n; i += nwarp) {
-        const double lik = colk[i];
-        for (int j = k + 1 + lane; j <= i; j += 32) P[(size_t)i * ld + j] -= lik * colk[j];
+      auto step = [&](auto RKc, auto BUFc, int kk) {
+        constexpr int RK = decltype(RKc)::value, BUF = decltype(BUFc)::value, KC = RK / 2;
+        constexpr unsigned OC = 8u * BUF * F3_SB, OR = OC + 8u * 96, OD = OR + 8u * 96;    // colk, rowk, d_k of this buffer
+        const int k = 16 * RK + kk;
+        if (k >= n) return;                                                              // uniform
+        if (lane == 16 * (RK & 1) + kk) {                                                 // owners of column k
+#pragma unroll
+          for (int r = RK; r < F3_RMAX; ++r) {
+            const int i = wid + 16 * r;
+            if (i < n) f3_sts(a_row + OC + 128u * r, (r > RK || wid > kk) ? pv[r][KC] : 0.0);
+          }
+          if (wid == kk) { f3_sts(scr + OD, pv[RK][KC]); f3_sts(scr + 8u * (2 * F3_SB + k), pv[RK][KC]); }
+        }
+        if (wid == kk) {                                                                  // owners of row k
+#pragma unroll
+          for (int c = 0; c <= KC; ++c) f3_sts(a_col + OR + 256u * c, yv[RK][c]);
+        }
+        __syncthreads();
+        double dk = f3_lds(scr + OD);
+        if (!(dk > 0) || !isfinite(dk)) { bad = 1; dk = 1; }
+        const double inv = 1.0 / dk;
+        double uj[F3_CMAX], yk[F3_CMAX];
+#pragma unroll
+        for (int c = KC; c < F3_CMAX; ++c) uj[c] = f3_lds(a_col + OC + 256u * c);
+#pragma unroll
+        for (int c = 0; c <= KC; ++c) yk[c] = f3_lds(a_col + OR + 256u * c);
+#pragma unroll
+        for (int r = RK; r < F3_RMAX; ++r) {
+          if (r > RK || wid > kk) {                    // rows i > k (rows beyond n read u_i = 0)
+            const double f = f3_lds(a_row + OC + 128u * r) * inv;
+#pragma unroll
+            for (int c = KC; c < F3_CMAX; ++c) pv[r][c] -= f * uj[c];
+#pragma unroll
+            for (int c = 0; c <= KC; ++c) yv[r][c] -= f * yk[c];
+          }
+        }
+      };
+      auto group = [&](auto RKc) {
+        for (int kk = 0; kk < 16; kk += 2) { step(RKc, f3_ic<0>{}, kk); step(RKc, f3_ic<1>{}, kk + 1); }
+      };
+      group(f3_ic<0>{}); group(f3_ic<1>{}); group(f3_ic<2>{}); group(f3_ic<3>{}); group(f3_ic<4>{}); group(f3_ic<5>{});
+      __syncthreads();
+      if (tid < 96) { const double di = f3_lds(scr + 8u * (2 * F3_SB + tid)); f3_sts(scr + 8u * (2 * F3_SB + tid), tid < n ? 1.0 / sqrt(di > 0 ? di : 1.0) : 0.0); }
+      __syncthreads();
+#pragma unroll
+      for (int r = 0; r < F3_RMAX; ++r) {
+        const int i = wid + 16 * r;
+        const double si = f3_lds(a_row + 8u * 2 * F3_SB + 128u * r);
+#pragma unroll
+        for (int c = 0; c < F3_CMAX; ++c) {
+          const int j = lane + 32 * c;
+          if (i < ld && j < ld) Q[(size_t)i * ld + j] = (i < n && j < n) ? yv[r][c] * si : 0.0;
+        }
       }
-      for (int i = k + tid; i < n; i += nt) P[(size_t)i * ld + k] = colk[i];
       __syncthreads();
     }
-    for (int e = tid; e < ld * ld; e += nt) { const int i = e / ld, j = e - i * ld; Q[e] = (i == j && i < n) ? 1.0 : 0.0; }
-    __syncthreads();
-    for (int k = 0; k < n - 1; ++k) {                  // Y[i][0..k] -= (L[i][k] / L[k][k]) Y[k][0..k] for rows i > k
-      const double inv = 1.0 / P[(size_t)k * ld + k];
-      for (int i = k + 1 + wid; i < n; i += nwarp) {
-        const double lik = P[(size_t)i * ld + k] * inv;
-        for (int j = lane; j <= k; j += 32) Q[(size_t)i * ld + j] -= lik * Q[(size_t)k * ld + j];
-      }
-      __syncthreads();
-    }
-    for (int e = tid; e < n * n; e += nt) { const int i = e / n, j = e - i * n; Q[(size_t)i * ld + j] /= P[(size_t)i * ld + i]; }
-    __syncthreads();
+    F3_TICK(2)
     // ---- P <- Sigma^{-1} = X'X  (sum over k >= max(i,j): X lower triangular), also to global
     if (has_tile) {
       double acc[4][4] = {};
@@ -173,6 +238,7 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
         }
     }
     __syncthreads();
+    F3_TICK(3)
     if (t == N) break;
     // ---- Q <- Phi_t' : Q[k][i] = Phi[i][k] = E_t[i][k] + w sum_r A^+_t[r][i] A^-_t[r][k]   (tile (k-block, i-block))
     {
@@ -196,6 +262,7 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
       }
       __syncthreads();
     }
+    F3_TICK(4)
     // ---- Lambda = Phi Sigma^{-1}: Lambda(i,j) = sum_k Q[k][i] P[k][j] ; R <- Lambda' , Lambda to global
     if (has_tile) {
       double acc[4][4] = {};
@@ -210,7 +277,11 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
         }
     }
     __syncthreads();
+    F3_TICK(5)
   }
+#ifdef TMPC_F3_PROF
+  if (tid == 0 && p == 0) printf("f3 cycles: theta %lld chol+inv %lld - %lld xtx %lld phi %lld lam %lld\n", tk[0], tk[1], tk[2], tk[3], tk[4], tk[5]);
+#endif
   bad = __syncthreads_or(bad);
   if (a.status && tid == 0 && bad) atomicOr(&a.status[p], TMPC_ST_PIVOT);
 }
