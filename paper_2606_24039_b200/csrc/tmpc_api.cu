@@ -100,8 +100,8 @@ tmpc_status launch_factor(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_
   if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) { factor_tw2_kernel<T, 6, 4, false><<<h->d.B, 32, 0, h->stream>>>(a); h->launches++; return cuda_ok() ? TMPC_OK : TMPC_E_CUDA; }
   const int nn = h->d.n * h->d.n;
   {                                      // large blocks: register-tiled products (tmpc_factor3.cuh)
-    const int nt4 = f3_ld(h->d.n) / 4; const size_t smem3 = factor3_smem<T>(h->d.n);
-    if (h->d.n >= 32 && nt4 * nt4 <= 512 && smem3 <= kMaxSmem) {
+    const int nt8 = f3_ld(h->d.n) / 8; const size_t smem3 = factor3_smem<T>(h->d.n);   // 4 x 4 warps x (3 x 3) tiles of 8 x 8
+    if (h->d.n >= 32 && nt8 <= 12 && smem3 <= kMaxSmem) {
       auto k3 = factor3_kernel<T>;
       if (cudaFuncSetAttribute(k3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3) != cudaSuccess) return TMPC_E_CUDA;
       k3<<<h->d.B, 512, smem3, h->stream>>>(a); h->launches++;

@@ -1,8 +1,11 @@
 // tmpc_factor3.cuh — a2 + a3 for the STREAMED class (n ~ 88): the one-directional block LDL' of factor_kernel
 // (same outputs: Lam_t = Phi_t Sigma_t^{-1}, Sinv_t = Sigma_t^{-1}), restructured as register-tiled shared-memory
 // matrix products.  factor_kernel spends its time on dependent global loads and two shared loads per FMA; here every
-// product has the form  out(i,j) = sum_k A[k][i] B[k][j]  with BOTH operands contiguous along the tile (so a thread's
-// 4 x 4 tile costs 4 vector loads per 16 DFMA), operands are staged in shared memory, and three n x n buffers suffice:
+// product has the form  out(i,j) = sum_k A[k][i] B[k][j]  and runs on the FP64 tensor cores (DMMA m8n8k4: the A fragment
+// of a lane is A[k + lane%4][i0 + lane/4], 8 contiguous doubles per k-row, two wavefronts per fragment load for ld = 88):
+// 16 warps in a 4 x 4 grid, each owning up to 3 x 3 tiles of 8 x 8 (6 fragment loads per 9 DMMA; the 4 x 4 DFMA register
+// tile it replaces needed 4 vector loads per 16 DFMA and was shared-memory bound).  Operands are staged in shared
+// memory, and three n x n buffers suffice:
 //   P: Sigma_t -> L (in-place Cholesky) -> Sigma_t^{-1} -> (next stage) Sigma_{t+1}
 //   Q: X = L^{-1} -> Phi_t' (transposed)
 //   R: Lambda_t' (transposed)
@@ -24,14 +27,18 @@ __device__ __forceinline__ void f3_sts(unsigned a, double v) { asm volatile("st.
 
 template <typename T> __host__ __device__ constexpr int f3_ch() { return sizeof(T) == 4 ? 32 : 16; }   // rows of A^-/A^+/G staged per chunk (in the working dtype)
 
-__host__ __device__ inline int f3_ld(int n) { return (n + 3) / 4 * 4; }
+__host__ __device__ inline int f3_ld(int n) { return (n + 7) / 8 * 8; }
+// D (8 x 8) += A (8 x 4, row) B (4 x 8, col): lane holds A[lane/4][lane%4], B[lane%4][lane/4], D[lane/4][2 (lane%4) + {0,1}]
+__device__ __forceinline__ void f3_dmma(double (&c)[2], double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
 template <typename T> __host__ inline size_t factor3_smem(int n) { const int ld = f3_ld(n); return (size_t)3 * ld * ld * sizeof(double) + (size_t)2 * f3_ch<T>() * ld * sizeof(T) + 64; }
 
 template <typename T>
 __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const Dims& d = a.d;
-  const int n = d.n, nx = d.nx, ng = d.ng, N = d.N, T_ = d.T, nn = n * n, ld = f3_ld(n), nt4 = ld / 4;
+  const int n = d.n, nx = d.nx, ng = d.ng, N = d.N, T_ = d.T, nn = n * n, ld = f3_ld(n), nt8 = ld / 8, n4 = (n + 3) & ~3;
   double* P = reinterpret_cast<double*>(smem_raw);
   double* Q = P + (size_t)ld * ld;
   double* R = Q + (size_t)ld * ld;
@@ -44,10 +51,9 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
   const T* Amp = a.qp.Am + (size_t)p * N * nx * n;
   const T* App = a.qp.Ap + (size_t)p * N * nx * n;
   const T* Gp = a.qp.G ? a.qp.G + a.qp.sG * p : nullptr;
-  const T* wr = a.w_rows ? a.w_rows + (size_t)p * T_ * ng : nullptr;
+  const T* wrow = a.w_rows ? a.w_rows + (size_t)p * T_ * ng : nullptr;
   T* Lamp = a.Lam + (size_t)p * N * nn;
   T* Sinvp = a.Sinv + (size_t)p * T_ * nn;
-  const int tiles = nt4 * nt4;
   int bad = 0;
   for (int e = tid; e < 3 * ld * ld; e += nt) P[e] = 0.0;          // pads stay zero
   __syncthreads();
@@ -61,37 +67,40 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
       S[e] = v;
     }
   };
-  // acc(i,j) += sum_k A[k][i0+i] B[k][j0+j]  for this thread's 4 x 4 tile; A, B row-major with leading dimension ld
-  auto mm_d = [&](double (&acc)[4][4], const double* A, const double* B, int k0, int k1, int i0, int j0) {
-    for (int k = k0; k < k1; ++k) {
-      const double2 a0 = *reinterpret_cast<const double2*>(A + (size_t)k * ld + i0), a1 = *reinterpret_cast<const double2*>(A + (size_t)k * ld + i0 + 2);
-      const double2 b0 = *reinterpret_cast<const double2*>(B + (size_t)k * ld + j0), b1 = *reinterpret_cast<const double2*>(B + (size_t)k * ld + j0 + 2);
-      const double av[4] = {a0.x, a0.y, a1.x, a1.y}, bv[4] = {b0.x, b0.y, b1.x, b1.y};
+  // acc(i,j) += sum_k A[k][i] B[k][j], k in [k0, k1) (multiples of 4; pad rows are zero): warp (wr, wc) owns the 8 x 8 tiles
+  // (3 wr + x, 3 wc + y); TRI skips the k-steps above the diagonal block of a tile (X lower triangular in X'X)
+  const int lane = tid & 31, wid = tid >> 5, wr = wid >> 2, wc = wid & 3, lq = lane >> 2, lr = lane & 3;
+  bool va[3], vb[3];
 #pragma unroll
-      for (int i = 0; i < 4; ++i)
+  for (int x = 0; x < 3; ++x) { va[x] = 3 * wr + x < nt8; vb[x] = 3 * wc + x < nt8; }
+  auto mm = [&](double (&acc)[3][3][2], const auto* A, const auto* B, int k0, int k1, auto TRIc) {
+    constexpr bool TRI = decltype(TRIc)::value != 0;
+    for (int k = k0; k < k1; k += 4) {
+      const auto* Ar = A + (size_t)(k + lr) * ld + 24 * wr + lq;
+      const auto* Br = B + (size_t)(k + lr) * ld + 24 * wc + lq;
+      double af[3], bf[3];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] += av[i] * bv[j];
+      for (int x = 0; x < 3; ++x) { af[x] = va[x] ? (double)Ar[8 * x] : 0.0; bf[x] = vb[x] ? (double)Br[8 * x] : 0.0; }
+#pragma unroll
+      for (int x = 0; x < 3; ++x)
+#pragma unroll
+        for (int y = 0; y < 3; ++y) {
+          const int tmax = 3 * wr + x > 3 * wc + y ? 3 * wr + x : 3 * wc + y;
+          if (va[x] && vb[y] && (!TRI || k >= 8 * tmax)) f3_dmma(acc[x][y], af[x], bf[y]);
+        }
     }
   };
-  auto mm_f = [&](double (&acc)[4][4], const T* A, const T* B, int rows, int i0, int j0) {
-    for (int k = 0; k < rows; ++k) {
-      double av[4], bv[4];
-      if constexpr (sizeof(T) == 4) {
-        const float4 a4 = *reinterpret_cast<const float4*>(A + (size_t)k * ld + i0), b4 = *reinterpret_cast<const float4*>(B + (size_t)k * ld + j0);
-        av[0] = a4.x; av[1] = a4.y; av[2] = a4.z; av[3] = a4.w; bv[0] = b4.x; bv[1] = b4.y; bv[2] = b4.z; bv[3] = b4.w;
-      } else {
-        const double2 a0 = *reinterpret_cast<const double2*>(A + (size_t)k * ld + i0), a1 = *reinterpret_cast<const double2*>(A + (size_t)k * ld + i0 + 2);
-        const double2 b0 = *reinterpret_cast<const double2*>(B + (size_t)k * ld + j0), b1 = *reinterpret_cast<const double2*>(B + (size_t)k * ld + j0 + 2);
-        av[0] = a0.x; av[1] = a0.y; av[2] = a1.x; av[3] = a1.y; bv[0] = b0.x; bv[1] = b0.y; bv[2] = b1.x; bv[3] = b1.y;
-      }
+  // visit this lane's accumulator elements: fn(v, gi, gj), v = acc[x][y][e], (gi, gj) = (row, column) in the padded block
+  auto for_acc = [&](double (&acc)[3][3][2], auto fn) {
 #pragma unroll
-      for (int i = 0; i < 4; ++i)
+    for (int x = 0; x < 3; ++x)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] += av[i] * bv[j];
-    }
+      for (int y = 0; y < 3; ++y)
+        if (va[x] && vb[y]) {
+#pragma unroll
+          for (int e = 0; e < 2; ++e) fn(acc[x][y][e], 8 * (3 * wr + x) + lq, 8 * (3 * wc + y) + 2 * lr + e);
+        }
   };
-  const bool has_tile = tid < tiles;
-  const int ti = has_tile ? tid / nt4 : 0, tj = has_tile ? tid - ti * nt4 : 0, i0 = 4 * ti, j0 = 4 * tj;
 
 #ifdef TMPC_F3_PROF
   long long tk[8] = {}, tc = clock64();
@@ -102,8 +111,11 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
   for (int t = 0; t < T_; ++t) {
     // ---- P <- Theta_t - Lambda_{t-1} Phi_{t-1}'   (R = Lambda', Q = Phi' of the previous stage)
     {
-      double accS[4][4] = {}, accA[4][4] = {}, accG[4][4] = {};
-      if (t > 0 && has_tile) mm_d(accS, R, Q, 0, n, i0, j0);
+      double acc[3][3][2] = {}, accA[3][3][2] = {};   // acc = G' w G - Lambda Phi' ; accA = A^-' A^- + A^+' A^+
+      if (t > 0) {
+        mm(acc, R, Q, 0, n4, f3_ic<0>{});
+        for_acc(acc, [&](double& v, int, int) { v = -v; });
+      }
       for (int which = 0; which < 2; ++which) {       // A^-_t' A^-_t  and  A^+_{t-1}' A^+_{t-1}
         const T* src = which == 0 ? (t < N ? Amp + (size_t)t * nx * n : nullptr) : (t > 0 ? App + (size_t)(t - 1) * nx * n : nullptr);
         if (!src) continue;
@@ -112,36 +124,38 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
           __syncthreads();
           stage(S1, src, r0, rows, nullptr, 1.0);
           __syncthreads();
-          if (has_tile) mm_f(accA, S1, S1, rows, i0, j0);
+          mm(accA, S1, S1, 0, (rows + 3) & ~3, f3_ic<0>{});
         }
       }
       if (!d.g_sel && Gp) for (int r0 = 0; r0 < ng; r0 += F3_CH) {   // G' diag(w) G
         const int rows = ng - r0 < F3_CH ? ng - r0 : F3_CH;
         __syncthreads();
         stage(S1, Gp + (size_t)t * ng * n, r0, rows, nullptr, 1.0);
-        stage(S2, Gp + (size_t)t * ng * n, r0, rows, wr ? wr + (size_t)t * ng : nullptr, wr ? 1.0 : a.w_in);
+        stage(S2, Gp + (size_t)t * ng * n, r0, rows, wrow ? wrow + (size_t)t * ng : nullptr, wrow ? 1.0 : a.w_in);
         __syncthreads();
-        if (has_tile) mm_f(accG, S1, S2, rows, i0, j0);
+        mm(acc, S1, S2, 0, (rows + 3) & ~3, f3_ic<0>{});
       }
       __syncthreads();                                 // everyone is done reading R, Q, S before P is rewritten
-      if (has_tile) {
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+      for (int x = 0; x < 3; ++x)
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const int gi = i0 + i, gj = j0 + j;
-            double s = 0.0;
-            if (gi < n && gj < n) {
-              s = (double)Dp[(size_t)t * nn + gi * n + gj] + a.w_eq * accA[i][j] + accG[i][j] - accS[i][j];
-              if (gi == gj) {
-                s += a.sigma;
-                if (t == 0 && gi < nx) s += a.w_eq;      // A_init' A_init = blkdiag(I_nx, 0)
-                if (d.g_sel) for (int r = 0; r < ng; ++r) if (d.g_col[r] == gi) s += wr ? (double)wr[(size_t)t * ng + r] : a.w_in;
-              }
-            } else if (gi == gj) s = 1.0;              // identity on the padding keeps the factor well defined
-            P[(size_t)gi * ld + gj] = s;
+        for (int y = 0; y < 3; ++y)
+          if (va[x] && vb[y]) {
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+              const int gi = 8 * (3 * wr + x) + lq, gj = 8 * (3 * wc + y) + 2 * lr + e;
+              double s = 0.0;
+              if (gi < n && gj < n) {
+                s = (double)Dp[(size_t)t * nn + gi * n + gj] + a.w_eq * accA[x][y][e] + acc[x][y][e];
+                if (gi == gj) {
+                  s += a.sigma;
+                  if (t == 0 && gi < nx) s += a.w_eq;      // A_init' A_init = blkdiag(I_nx, 0)
+                  if (d.g_sel) for (int r = 0; r < ng; ++r) if (d.g_col[r] == gi) s += wrow ? (double)wrow[(size_t)t * ng + r] : a.w_in;
+                }
+              } else if (gi == gj) s = 1.0;              // identity on the padding keeps the factor well defined
+              P[(size_t)gi * ld + gj] = s;
+            }
           }
-      }
       __syncthreads();
     }
     F3_TICK(0)
@@ -153,7 +167,6 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
     // walked in six compile-time groups of 16 (row slot r of the pivot row and the live 32-column chunks are constants
     // inside a group; the only run-time conditions are warp uniform).  At the end X[i][j] = Y[i][j] / sqrt(d_i) goes to Q.
     {
-      const int lane = tid & 31, wid = tid >> 5;
       const unsigned scr = (unsigned)__cvta_generic_to_shared(S1);   // the staging chunks are idle here (>= 8 KB)
       const unsigned a_row = scr + 8u * wid, a_col = scr + 8u * lane;  // colk[i] broadcast per warp / colk[j], rowk[j] per lane
       double pv[F3_RMAX][F3_CMAX], yv[F3_RMAX][F3_CMAX];
@@ -225,56 +238,42 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
     }
     F3_TICK(2)
     // ---- P <- Sigma^{-1} = X'X  (sum over k >= max(i,j): X lower triangular), also to global
-    if (has_tile) {
-      double acc[4][4] = {};
-      mm_d(acc, Q, Q, i0 > j0 ? i0 : j0, n, i0, j0);
-#pragma unroll
-      for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int gi = i0 + i, gj = j0 + j;
-          P[(size_t)gi * ld + gj] = (gi < n && gj < n) ? acc[i][j] : 0.0;
-          if (gi < n && gj < n) Sinvp[(size_t)t * nn + gi * n + gj] = (T)acc[i][j];
-        }
+    {
+      double acc[3][3][2] = {};
+      mm(acc, Q, Q, 0, n4, f3_ic<1>{});
+      for_acc(acc, [&](double& v, int gi, int gj) {
+        P[(size_t)gi * ld + gj] = (gi < n && gj < n) ? v : 0.0;
+        if (gi < n && gj < n) Sinvp[(size_t)t * nn + gi * n + gj] = (T)v;
+      });
     }
     __syncthreads();
     F3_TICK(3)
     if (t == N) break;
     // ---- Q <- Phi_t' : Q[k][i] = Phi[i][k] = E_t[i][k] + w sum_r A^+_t[r][i] A^-_t[r][k]   (tile (k-block, i-block))
     {
-      double acc[4][4] = {};
+      double acc[3][3][2] = {};
       for (int r0 = 0; r0 < nx; r0 += F3_CH) {
         const int rows = nx - r0 < F3_CH ? nx - r0 : F3_CH;
         __syncthreads();
         stage(S1, Amp + (size_t)t * nx * n, r0, rows, nullptr, 1.0);
         stage(S2, App + (size_t)t * nx * n, r0, rows, nullptr, 1.0);
         __syncthreads();
-        if (has_tile) mm_f(acc, S1, S2, rows, i0, j0);   // acc(k, i) = sum_r A^-[r][k] A^+[r][i]
+        mm(acc, S1, S2, 0, (rows + 3) & ~3, f3_ic<0>{});   // acc(k, i) = sum_r A^-[r][k] A^+[r][i]
       }
-      if (has_tile) {
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const int gk = i0 + i, gi = j0 + j;
-            Q[(size_t)gk * ld + gi] = (gk < n && gi < n) ? (double)Ep[(size_t)t * nn + gi * n + gk] + a.w_eq * acc[i][j] : 0.0;
-          }
-      }
+      for_acc(acc, [&](double& v, int gk, int gi) {
+        Q[(size_t)gk * ld + gi] = (gk < n && gi < n) ? (double)Ep[(size_t)t * nn + gi * n + gk] + a.w_eq * v : 0.0;
+      });
       __syncthreads();
     }
     F3_TICK(4)
     // ---- Lambda = Phi Sigma^{-1}: Lambda(i,j) = sum_k Q[k][i] P[k][j] ; R <- Lambda' , Lambda to global
-    if (has_tile) {
-      double acc[4][4] = {};
-      mm_d(acc, Q, P, 0, n, i0, j0);
-#pragma unroll
-      for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int gi = i0 + i, gj = j0 + j;
-          R[(size_t)gj * ld + gi] = (gi < n && gj < n) ? acc[i][j] : 0.0;
-          if (gi < n && gj < n) Lamp[(size_t)t * nn + gi * n + gj] = (T)acc[i][j];
-        }
+    {
+      double acc[3][3][2] = {};
+      mm(acc, Q, P, 0, n4, f3_ic<0>{});
+      for_acc(acc, [&](double& v, int gi, int gj) {
+        R[(size_t)gj * ld + gi] = (gi < n && gj < n) ? v : 0.0;
+        if (gi < n && gj < n) Lamp[(size_t)t * nn + gi * n + gj] = (T)v;
+      });
     }
     __syncthreads();
     F3_TICK(5)
