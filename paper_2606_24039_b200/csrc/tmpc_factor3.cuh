@@ -25,6 +25,9 @@ template <int V> using f3_ic = std::integral_constant<int, V>;
 __device__ __forceinline__ double f3_lds(unsigned a) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
 __device__ __forceinline__ void f3_sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
 
+__device__ __forceinline__ void f3_cp16(unsigned dst, const void* src) { asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory"); }
+__device__ __forceinline__ void f3_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void f3_cp_wait() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 template <typename T> __host__ __device__ constexpr int f3_ch() { return sizeof(T) == 4 ? 32 : 16; }   // rows of A^-/A^+/G staged per chunk (in the working dtype)
 
 __host__ __device__ inline int f3_ld(int n) { return (n + 7) / 8 * 8; }
@@ -67,6 +70,23 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
       S[e] = v;
     }
   };
+  // asynchronous staging (LDGSTS, 16 bytes per copy, L2 only) of rows [r0, r0+rows) when a chunk is contiguous and aligned in
+  // global AND shared memory (ld == n, 16-byte rows): the copies of the next chunk are in flight while the tensor cores work
+  // on the current product; without it every chunk exposes a chain of dependent global-load latencies (measured: the staged
+  // phases took 3-5x their DMMA time).  The tail rows of the chunk are zeroed.  Other shapes keep the synchronous path.
+  constexpr int VE = 16 / (int)sizeof(T);
+  const bool fast = ld == n && ((uintptr_t)Amp % 16 == 0) && ((uintptr_t)App % 16 == 0) && (((size_t)nx * n * sizeof(T)) % 16 == 0);
+  auto stage_async = [&](T* S, const T* src, int r0, int rows) {
+    const int nvec = rows * ld / VE, tot = F3_CH * ld / VE;
+    const unsigned s0 = (unsigned)__cvta_generic_to_shared(S);
+    const T* g0 = src + (size_t)r0 * n;
+    for (int v = tid; v < tot; v += nt) {
+      if (v < nvec) f3_cp16(s0 + 16u * v, g0 + (size_t)v * VE);
+      else *reinterpret_cast<float4*>(reinterpret_cast<unsigned char*>(S) + 16 * (size_t)v) = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+  };
+  auto clampr = [&](int r) { return r < 0 ? 0 : (r > F3_CH ? F3_CH : r); };
+
   // acc(i,j) += sum_k A[k][i] B[k][j], k in [k0, k1) (multiples of 4; pad rows are zero): warp (wr, wc) owns the 8 x 8 tiles
   // (3 wr + x, 3 wc + y); TRI skips the k-steps above the diagonal block of a tile (X lower triangular in X'X)
   const int lane = tid & 31, wid = tid >> 5, wr = wid >> 2, wc = wid & 3, lq = lane >> 2, lr = lane & 3;
@@ -112,20 +132,39 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
     // ---- P <- Theta_t - Lambda_{t-1} Phi_{t-1}'   (R = Lambda', Q = Phi' of the previous stage)
     {
       double acc[3][3][2] = {}, accA[3][3][2] = {};   // acc = G' w G - Lambda Phi' ; accA = A^-' A^- + A^+' A^+
+      const int nps = (nx + 2 * F3_CH - 1) / (2 * F3_CH);
+      auto pair_src = [&](int q_, int& r0) -> const T* {
+        const int which = q_ / nps; r0 = (q_ - which * nps) * 2 * F3_CH;
+        return which == 0 ? (t < N ? Amp + (size_t)t * nx * n : nullptr) : (t > 0 ? App + (size_t)(t - 1) * nx * n : nullptr);
+      };
+      auto next_valid = [&](int q_) { int r0; while (q_ < 2 * nps && !pair_src(q_, r0)) ++q_; return q_; };
+      auto issue_pair = [&](int q_) {
+        int r0; const T* src = pair_src(q_, r0);
+        stage_async(S1, src, r0, clampr(nx - r0));
+        if (nx - r0 - F3_CH > 0) stage_async(S2, src, r0 + F3_CH, clampr(nx - r0 - F3_CH));
+        f3_cp_commit();
+      };
+      int q = next_valid(0);
+      if (fast && q < 2 * nps) issue_pair(q);          // S1, S2 are idle since the barrier that ended the previous phase
       if (t > 0) {
         mm(acc, R, Q, 0, n4, f3_ic<0>{});
         for_acc(acc, [&](double& v, int, int) { v = -v; });
       }
-      for (int which = 0; which < 2; ++which) {       // A^-_t' A^-_t  and  A^+_{t-1}' A^+_{t-1}
-        const T* src = which == 0 ? (t < N ? Amp + (size_t)t * nx * n : nullptr) : (t > 0 ? App + (size_t)(t - 1) * nx * n : nullptr);
-        if (!src) continue;
-        for (int r0 = 0; r0 < nx; r0 += F3_CH) {
-          const int rows = nx - r0 < F3_CH ? nx - r0 : F3_CH;
+      // A^-_t' A^-_t  and  A^+_{t-1}' A^+_{t-1}, two chunks (S1, S2) per step; step q = (which, r0)
+      while (q < 2 * nps) {
+        int r0; const T* src = pair_src(q, r0);
+        const int rows1 = clampr(nx - r0), rows2 = clampr(nx - r0 - F3_CH);
+        if (fast) { f3_cp_wait(); __syncthreads(); }
+        else {
           __syncthreads();
-          stage(S1, src, r0, rows, nullptr, 1.0);
+          stage(S1, src, r0, rows1, nullptr, 1.0);
+          if (rows2 > 0) stage(S2, src, r0 + F3_CH, rows2, nullptr, 1.0);
           __syncthreads();
-          mm(accA, S1, S1, 0, (rows + 3) & ~3, f3_ic<0>{});
         }
+        mm(accA, S1, S1, 0, (rows1 + 3) & ~3, f3_ic<0>{});
+        if (rows2 > 0) mm(accA, S2, S2, 0, (rows2 + 3) & ~3, f3_ic<0>{});
+        q = next_valid(q + 1);
+        if (fast && q < 2 * nps) { __syncthreads(); issue_pair(q); }
       }
       if (!d.g_sel && Gp) for (int r0 = 0; r0 < ng; r0 += F3_CH) {   // G' diag(w) G
         const int rows = ng - r0 < F3_CH ? ng - r0 : F3_CH;
@@ -238,6 +277,12 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
     }
     F3_TICK(2)
     // ---- P <- Sigma^{-1} = X'X  (sum over k >= max(i,j): X lower triangular), also to global
+    auto issue_phi = [&](int r0) {
+      stage_async(S1, Amp + (size_t)t * nx * n, r0, clampr(nx - r0));
+      stage_async(S2, App + (size_t)t * nx * n, r0, clampr(nx - r0));
+      f3_cp_commit();
+    };
+    if (fast && t < N) issue_phi(0);                     // the Cholesky scratch in S1 is dead since the barrier above
     {
       double acc[3][3][2] = {};
       mm(acc, Q, Q, 0, n4, f3_ic<1>{});
@@ -254,11 +299,15 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
       double acc[3][3][2] = {};
       for (int r0 = 0; r0 < nx; r0 += F3_CH) {
         const int rows = nx - r0 < F3_CH ? nx - r0 : F3_CH;
-        __syncthreads();
-        stage(S1, Amp + (size_t)t * nx * n, r0, rows, nullptr, 1.0);
-        stage(S2, App + (size_t)t * nx * n, r0, rows, nullptr, 1.0);
-        __syncthreads();
+        if (fast) { f3_cp_wait(); __syncthreads(); }
+        else {
+          __syncthreads();
+          stage(S1, Amp + (size_t)t * nx * n, r0, rows, nullptr, 1.0);
+          stage(S2, App + (size_t)t * nx * n, r0, rows, nullptr, 1.0);
+          __syncthreads();
+        }
         mm(acc, S1, S2, 0, (rows + 3) & ~3, f3_ic<0>{});   // acc(k, i) = sum_r A^-[r][k] A^+[r][i]
+        if (fast && r0 + F3_CH < nx) { __syncthreads(); issue_phi(r0 + F3_CH); }
       }
       for_acc(acc, [&](double& v, int gk, int gi) {
         Q[(size_t)gk * ld + gi] = (gk < n && gi < n) ? (double)Ep[(size_t)t * nn + gi * n + gk] + a.w_eq * v : 0.0;
