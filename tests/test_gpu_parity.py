@@ -207,6 +207,15 @@ def test_config3_shape_fp64():
     run_pair(w, "f64", iters=25, band=1)
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_tensor_core_factor_ragged_block_sizes(dtype):
+    """factor3_kernel (DMMA tiles of 8 x 8) on block sizes that are NOT a multiple of 8 or 4: n = 37 (padded to 40, the
+    synchronous staging path, 5 x 5 tiles on a 4 x 4 warp grid) with a dense G row (G' w G product), implicit E_k, and
+    n = 48 (aligned: the cp.async path, nx = 40 spans a full and a ragged chunk of staged rows)."""
+    run_pair(W.random_ltv(61, 3, 5, 30, 7, [30, 33, 36], [0, 0, 1, 0], implicit=True, dense_g_rows=1, q_scale=0.3), dtype, iters=40)
+    run_pair(W.random_ltv(62, 2, 4, 40, 8, [40, 47], [0, 0], implicit=True, q_scale=0.3), dtype, iters=40)
+
+
 # ----------------------------------------------------------------------------------------------- a11 cyclic reduction
 @pytest.mark.parametrize("N", [1, 2, 4, 20, 63, 64, 100])
 def test_cyclic_reduction_solve_equals_sequential_and_oracle(N):
