@@ -144,9 +144,35 @@ tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
     const int V = 16 / (int)sizeof(T);
     if ((d.n * d.n) % V == 0 && (d.nx * d.n) % V == 0 && d.n % V == 0 && 4 * d.ng <= sp.nthreads - 32 && sp.slots >= 2 && sp.nthreads <= 1024) {
       StreamArgs<T> S; S.a = a; S.LD = sp.LD; S.slots = sp.slots; S.tile_elems = sp.tile_elems; S.eta = (T*)(h->ws + h->lay.eta);
+      S.g0 = 0; S.chunks = 1;
       auto k = admm_stream_kernel<T>;
       if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp.smem) != cudaSuccess) return TMPC_E_CUDA;
-      k<<<d.B, sp.nthreads, sp.smem, h->stream>>>(S); h->launches++;
+      // Wave quantisation: a CTA runs at a fixed rate (measured: B = 296 = one full wave of 2 CTAs x 148 SMs takes 44.6 ms,
+      // B = 512 takes 87.4 ms, B = 592 89.4 ms), so a partial last wave costs a whole one.  The ADMM state between two
+      // iterations is complete in global memory (warm start = resume), hence the solve is cut into `chunks` iteration
+      // ranges per problem and the B x chunks jobs, ordered (chunk, problem), are run `cslots` at a time in successive
+      // launches: consecutive jobs of a launch are distinct problems and a problem's previous chunk sits >= one launch
+      // earlier (B > cslots).  Cost model: launches x iterations per chunk, plus the eta pass each launch repeats.
+      int per_sm = 0, dev = 0, sms = 0;
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, sp.nthreads, sp.smem) != cudaSuccess || cudaGetDevice(&dev) != cudaSuccess ||
+          cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return TMPC_E_CUDA;
+      const long long cslots = (long long)per_sm * sms;
+      int best_c = 1;
+      if (!a.kkt_only && cslots > 0 && d.B > cslots && a.iters >= 32) {
+        double best = (double)((d.B + cslots - 1) / cslots) * (a.iters + 0.3);
+        for (int c = 2; c <= 8 && a.iters / c >= 16; ++c) {
+          const long long rounds = ((long long)d.B * c + cslots - 1) / cslots;
+          const double cost = (double)rounds * ((a.iters + c - 1) / c + 0.3);
+          if (cost < 0.97 * best) { best = cost; best_c = c; }
+        }
+      }
+      S.chunks = best_c;
+      const long long jobs = (long long)d.B * best_c, per = best_c > 1 ? cslots : jobs;
+      for (long long g0 = 0; g0 < jobs; g0 += per) {
+        S.g0 = (int)g0;
+        const long long grid = jobs - g0 < per ? jobs - g0 : per;
+        k<<<(unsigned)grid, sp.nthreads, sp.smem, h->stream>>>(S); h->launches++;
+      }
       if (!cuda_ok()) return TMPC_E_CUDA;
       return a.kkt_only ? TMPC_OK : launch_residual<T>(h, a);
     }

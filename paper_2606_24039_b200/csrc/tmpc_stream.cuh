@@ -59,7 +59,9 @@ __host__ inline StreamPlan stream_plan(const Dims& d, size_t max_smem) {
 }
 
 template <typename T>
-struct StreamArgs { AdmmArgs<T> a; int LD, slots, tile_elems; T* eta; };   // eta: global scratch [B][nz] (right-hand side, L2 resident)
+// g0, chunks: iteration-chunk scheduling (launch_admm): CTA b of a launch runs chunk (g0 + b) / B of problem (g0 + b) % B,
+// i.e. iterations [iters k / chunks, iters (k+1) / chunks); chunks = 1, g0 = 0 is the plain one-CTA-per-problem launch.
+struct StreamArgs { AdmmArgs<T> a; int LD, slots, tile_elems; T* eta; int g0, chunks; };   // eta: global scratch [B][nz] (right-hand side, L2 resident)
 
 // block sequence of one launch, identical in the producer and the consumers:
 //   [eta pass]   t = N-1..0 : A^-_t, A^+_t                         (skipped for kkt_only)
@@ -72,7 +74,9 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
   const Dims& d = a.d;
   constexpr int V = 16 / (int)sizeof(T);
   const int n = d.n, nx = d.nx, ng = d.ng, N = d.N, T_ = d.T, nn = n * n, an = nx * n, nz = d.nz, mf = d.mf, mg = d.mg;
-  const int LD = S.LD, KS = S.slots, p = blockIdx.x, tid = threadIdx.x;
+  const int LD = S.LD, KS = S.slots, tid = threadIdx.x;
+  const int gjob = S.g0 + (int)blockIdx.x, chunk = gjob / d.B, p = gjob - chunk * d.B;
+  const int zg_given = chunk > 0 ? 1 : a.zg_given;                   // later chunks resume from the stored state
   unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_raw);            // full[KS], empty[KS]
   T* ring = reinterpret_cast<T*>(smem_raw + 256);
   // Only v / x~ is kept whole in shared memory.  The right-hand side eta lives in global memory (each element is written
@@ -95,7 +99,7 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
   const T* gSinv = a.Sinv + (size_t)p * T_ * nn;
   const T* gAm = a.kkt_only ? nullptr : a.qp.Am + (size_t)p * N * an;
   const T* gAp = a.kkt_only ? nullptr : a.qp.Ap + (size_t)p * N * an;
-  const int iters = a.kkt_only ? 1 : a.iters;
+  const int iters = a.kkt_only ? 1 : (int)(((long long)a.iters * (chunk + 1)) / S.chunks - ((long long)a.iters * chunk) / S.chunks);
 
   // ======================================================================= producer warp
   if (tid < 32) {
@@ -186,8 +190,8 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
   if (!a.kkt_only) {
     if (own_g) for (int t = 0; t < T_; ++t) {
       const size_t row = gg + t * ng + ci;
-      if (!a.zg_given) a.zg[row] = tmin(tmax(g_row_dot(t, gxs), a.qp.lo[row]), a.qp.hi[row]);
-      if (!a.zg_given && a.iters == 0) a.xi[row] = T(0);
+      if (!zg_given) a.zg[row] = tmin(tmax(g_row_dot(t, gxs), a.qp.lo[row]), a.qp.hi[row]);
+      if (!zg_given && a.iters == 0) a.xi[row] = T(0);
     }
     cons_bar();
     __threadfence_block();
