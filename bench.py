@@ -283,8 +283,10 @@ def run_gpu(args):
         roof = {"bound": "alu", "achieved": alg / (kern_avg_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s", "peak_source": "derived: 148 SMs x 128 (fp32) / 64 (fp64) FMA lanes x 2 x 1965 MHz"}
     roof["frac"] = roof["achieved"] / roof["peak"]
     # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed `ncu --set full` captures
-    # (profiles/r01_v2_ncu_full_*.md); only valid for the workload the capture was taken on
-    ncu_traffic = {(2, "f32", 1024): 57.05e6 + 0.29e6, (3, "f32", 512): 445.52e9 + 3.91e9}
+    # (profiles/r01_v2_ncu_full_admm2_*.md, profiles/r01_v3_ncu_full_admm_stream_*.md); only valid for the workload the capture was taken on
+    # config 3: one tmpc_admm_solve = 7 chunk launches; the capture is ONE full-wave launch (296 CTAs x 50
+    # iterations: 65.42 GB read + 0.57 GB written), scaled to the 2048 chunk jobs of a call, like `achieved` (whole call)
+    ncu_traffic = {(2, "f32", 1024): 57.05e6 + 0.29e6, (3, "f32", 512): (65.42e9 + 0.572e9) * 2048 / 296}
     roof["traffic"] = ncu_traffic.get((args.config, args.dtype, w.B))
     roof["kernel"] = {1: "admm2_kernel", 2: "admm2_kernel", 3: "admm_stream_kernel", 4: "admm2_kernel", 5: "cr2_admm_kernel"}[args.config] + " (tmpc_admm_solve)"
     if args.config in (1, 2, 4):
