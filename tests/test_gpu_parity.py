@@ -202,6 +202,14 @@ def test_config3_subset_fp32():
     run_pair(w, "f32", iters=40, band=1)
 
 
+def test_streamed_chunk_scheduling_uneven_split_fp32():
+    """B = 300 is just above one wave of co-resident CTAs (2 x 148), so tmpc_admm_solve cuts the 33 iterations into 2 chunks
+    of 16 and 17 and runs the 600 chunk jobs 296 per launch (a launch mixes chunk 0 and chunk 1 of different problems).
+    EVERY problem must still match the oracle's uninterrupted 33 iterations."""
+    w = W.config3(B=300, N=2)
+    run_pair(w, "f32", iters=33, band=1)
+
+
 def test_config3_shape_fp64():
     w = W.config3(B=2, N=4)
     run_pair(w, "f64", iters=25, band=1)
