@@ -97,7 +97,11 @@ tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, vo
 tmpc_status tmpc_linearize(tmpc_handle h, const void* xbar, const void* stage_ref, tmpc_qp* qp);
 /* a2+a3: assemble Theta_t, Phi_t and factor S block by block into the workspace. */
 tmpc_status tmpc_factor(tmpc_handle h, const tmpc_qp* qp);
-/* a4-a9 (Alg. 3): exactly `iters` ADMM iterations on every problem, no early exit; needs tmpc_factor first. */
+/* a4-a9 (Alg. 3): exactly `iters` ADMM iterations on every problem, no early exit; needs tmpc_factor first.
+ * Enqueues one fused kernel for all iterations, or, for the streamed class with more problems than co-resident CTAs,
+ * several launches of it over iteration chunks (same arithmetic, bit-identical state), plus the residual kernel (a9)
+ * when `info` has a non-NULL pointer.  The state in `st` is complete between calls: a later call with
+ * TMPC_SOLVE_ZG_GIVEN continues where this one stopped. */
 tmpc_status tmpc_admm_solve(tmpc_handle h, const tmpc_qp* qp, tmpc_state* st, int32_t iters, int32_t flags, tmpc_info* info);
 /* a10 (Alg. 2, eq. 59-65): dL/dq [B][T][n] and dL/dx_init [B][nx] from dL/dx [B][T][n] (and dL/dxi [B][T][ng] or NULL)
  * at the state st.  REFACTOR_REFINE factors the adjoint-weighted S and runs `iters` refinement sweeps of the
