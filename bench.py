@@ -288,7 +288,7 @@ def run_gpu(args):
     # iterations: 65.42 GB read + 0.57 GB written), scaled to the 2048 chunk jobs of a call, like `achieved` (whole call)
     ncu_traffic = {(2, "f32", 1024): 57.05e6 + 0.29e6, (3, "f32", 512): (65.42e9 + 0.572e9) * 2048 / 296}
     roof["traffic"] = ncu_traffic.get((args.config, args.dtype, w.B))
-    roof["kernel"] = {1: "admm2_kernel", 2: "admm2_kernel", 3: "admm_stream_kernel", 4: "admm2_kernel", 5: "cr2_admm_kernel"}[args.config] + " (tmpc_admm_solve)"
+    roof["kernel"] = {1: "admm2_kernel", 2: "admm2_kernel", 3: "admm_stream_kernel x chunk launches", 4: "admm2_kernel", 5: "cr2_admm_kernel"}[args.config] + " (tmpc_admm_solve)"
     if args.config in (1, 2, 4):
         # supplementary: the resident class reads every factor / constraint element from SHARED memory once per use, so the
         # binding on-chip resource is LDS bandwidth (148 SMs x 128 B/clk x 1965 MHz), not the FMA pipe
