@@ -104,7 +104,9 @@ tmpc_status tmpc_factor(tmpc_handle h, const tmpc_qp* qp);
  * TMPC_SOLVE_ZG_GIVEN continues where this one stopped. */
 tmpc_status tmpc_admm_solve(tmpc_handle h, const tmpc_qp* qp, tmpc_state* st, int32_t iters, int32_t flags, tmpc_info* info);
 /* a10 (Alg. 2, eq. 59-65): dL/dq [B][T][n] and dL/dx_init [B][nx] from dL/dx [B][T][n] (and dL/dxi [B][T][ng] or NULL)
- * at the state st.  REFACTOR_REFINE factors the adjoint-weighted S and runs `iters` refinement sweeps of the
+ * at the state st.  dL/dxi is the gradient with respect to the SIGNED slack st.xi that tmpc_admm_solve returns
+ * (lo <= Gx + xi <= hi; App. E's xi_A of eq. 54 is |xi| = sign(xi) xi, so eq. 65's S dL/dxi_A is dL/dxi); only its
+ * entries on soft-active rows (xi != 0) are read.  REFACTOR_REFINE factors the adjoint-weighted S and runs `iters` refinement sweeps of the
  * active-set KKT system; ADMM_REUSE_FACTOR runs `iters` ADMM iterations on the adjoint QP (eq. 67) with the
  * forward factor.  Overwrites the factor in the workspace in REFACTOR_REFINE mode. */
 tmpc_status tmpc_backward(tmpc_handle h, const tmpc_qp* qp, const tmpc_state* st, const void* dL_dx, const void* dL_dxi,

@@ -22,7 +22,10 @@
 //
 // Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): Theta/Phi block formulas, LQR Riccati, brute-force
 // active-set enumeration, projection closed forms and invariants, residual convergence, central finite
-// differences for backward and for the bicycle Jacobians, dense == band.  Nothing is "parity unpinned".
+// differences for backward (hard-active, soft-active, L1 dead-zone rows, with and without a dL/dxi term) and for the
+// bicycle Jacobians, the row classification on hand-built states, the slack terms of r_dual / objective recomputed in
+// numpy, every iterate against the un-reduced KKT form eq. 7 (large sigma, alpha != 1), equality rows re-posed as
+// two-sided inequality rows (z_f == c), three SQP steps driven by hand, dense == band.  Nothing is "parity unpinned".
 
 #include <cmath>
 #include <cstdint>
@@ -256,10 +259,15 @@ double backward(const Cfg& cf, const QP& p, const double* x, const double* yg, c
   vec K((size_t)m * m, 0.0), rhs(m, 0.0);
   for (int i = 0; i < p.nz; ++i) for (int j = std::max(0, i - p.P.bw); j <= std::min(p.nz - 1, i + p.P.bw); ++j) K[(size_t)i * m + j] = p.P.get(i, j);
   for (int i = 0; i < p.nz; ++i) rhs[i] = dLdx[i];
-  for (int r = 0; r < p.mg; ++r) if (cls[r] == 2) {              // + gamma G_s' G_s ;  rhs -= G_s' Sigma_s dL/dxi_s  (eq. 65)
+  // + gamma G_s' G_s ;  rhs -= G_s' dL/dxi_s  (eq. 65).  dLdxi is the gradient w.r.t. the SIGNED slack xi of the OCP / of Alg. 3
+  // (lo <= Gx + xi <= hi), i.e. the `xi` this solver returns.  App. E writes the active rows as
+  // g_A + S xi_A = 0 with S = sign(xi) (eq. 54), which is the same row Gx + xi = bound in the variable xi_A = S xi = |xi|;
+  // eq. 65's right-hand side -G_s' S dL/dxi_A then equals -G_s' S (S dL/dxi) = -G_s' dL/dxi  (reading A-31,
+  // pinned by central finite differences in tests/test_oracle_pins.py).
+  for (int r = 0; r < p.mg; ++r) if (cls[r] == 2) {
     const double* a = p.G.row(r); int c0 = p.G.c0[r];
     for (int i = 0; i < p.G.len[r]; ++i) for (int j = 0; j < p.G.len[r]; ++j) K[(size_t)(c0 + i) * m + c0 + j] += cf.gamma * a[i] * a[j];
-    if (dLdxi) { double sg = xi[r] > 0 ? 1.0 : -1.0; for (int i = 0; i < p.G.len[r]; ++i) rhs[c0 + i] -= a[i] * sg * dLdxi[r]; }
+    if (dLdxi) for (int i = 0; i < p.G.len[r]; ++i) rhs[c0 + i] -= a[i] * dLdxi[r];
   }
   for (int r = 0; r < p.mf; ++r) { const double* a = p.C.row(r); for (int k = 0; k < p.C.len[r]; ++k) { K[(size_t)(p.nz + r) * m + p.C.c0[r] + k] = a[k]; K[(size_t)(p.C.c0[r] + k) * m + p.nz + r] = a[k]; } }
   for (int h = 0; h < nh; ++h) { int r = hard[h]; const double* a = p.G.row(r); for (int k = 0; k < p.G.len[r]; ++k) { K[(size_t)(p.nz + p.mf + h) * m + p.G.c0[r] + k] = a[k]; K[(size_t)(p.G.c0[r] + k) * m + p.nz + p.mf + h] = a[k]; } }

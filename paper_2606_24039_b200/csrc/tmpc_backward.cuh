@@ -2,7 +2,7 @@
 //
 //  bwd_prepare_kernel : classify each inequality row (reading A-16) into
 //                       0 inactive / 1 hard-active / 2 soft-active, and build
-//                         rhs_x = dL/dx - G_s' Sigma_s dL/dxi_s                                   (eq. 65 right-hand side)
+//                         rhs_x = dL/dx - G_s' dL/dxi_s      (eq. 65 right-hand side in the signed slack xi = S xi_A of eq. 54)
 //                       plus, per mode: adjoint row weights (REFINE) or the adjoint QP's data (REUSE, eq. 67).
 //  bwd_refine_kernel  : iterative refinement of the active-set KKT system (eq. 62 / 65)
 //                         [H A_a'; A_a 0][e_x; e_y] = [rhs_x; 0],  H = P + gamma G_s'G_s,  A_a = [C; G_h],
@@ -83,8 +83,7 @@ __global__ void bwd_prepare_kernel(BwdArgs<T> a) {
         const int row = t * ng + r;
         if (cls[row] != 2) continue;
         const T gi = d.g_sel ? (d.g_col[r] == i ? T(1) : T(0)) : G[((size_t)t * ng + r) * n + i];
-        const T sg = xi[row] > T(0) ? T(1) : T(-1);
-        s -= gi * sg * a.dLdxi[(size_t)p * mg + row];
+        s -= gi * a.dLdxi[(size_t)p * mg + row];     // dL/dxi is w.r.t. the signed slack this library returns: no sign factor (tmpc.h)
       }
     }
     a.rhs[(size_t)p * nz + e] = s;

@@ -259,30 +259,152 @@ def test_config1_converges_below_eps():
     assert (np.abs(yg) > 1e-6).sum() > 0   # bounds are active: the instance tests the projection
 
 
+def test_info_slack_terms_recomputed_in_numpy():
+    """r_dual's soft-row block  gamma xi + lam sgn(xi) + y_g  (eq. 3 second block with the L1 term of reading A-14) and the
+    slack penalty  lam |xi| + gamma/2 xi^2  of the objective, recomputed from numpy-built matrices on the slack-stress
+    instance where xi != 0.  The soft-row block is an exact identity of the prox (zero up to rounding), so the objective and
+    the x-block are what move; the test also perturbs xi to show the oracle's r_dual sees that block."""
+    w = W.config2(B=2, N=12, soft_bound=0.5)
+    w.rho_bar = 20.0
+    cfg = O.make_cfg(w)
+    st, info, rc = O.admm(w, cfg, iters=60)
+    assert (st["xi"] != 0).sum() > 10
+    for b in range(w.B):
+        P, C, c, G = dense_PCG(w, b)
+        x, yf, yg, zg, xi = st["x"][b].ravel(), st["yf"][b], st["yg"][b].ravel(), st["zg"][b].ravel(), st["xi"][b].ravel()
+        soft = np.tile(np.array(w.soft, dtype=bool), w.T)
+        m = soft & (xi != 0)
+        rd = max(np.abs(P @ x + w.q[b].ravel() + C.T @ yf + G.T @ yg).max(), np.abs(w.gamma * xi[m] + w.lam * np.sign(xi[m]) + yg[m]).max(initial=0))
+        obj = 0.5 * x @ P @ x + w.q[b].ravel() @ x + (w.lam * np.abs(xi[m]) + 0.5 * w.gamma * xi[m] ** 2).sum()
+        rp = max(np.abs(C @ x - c).max(), np.abs(G @ x - zg).max())
+        assert abs(rp - info[b, 0]) < 1e-12 and abs(rd - info[b, 1]) < 1e-11 * max(1, rd) and abs(obj - info[b, 2]) < 1e-10 * abs(obj)
+        assert (w.lam * np.abs(xi[m]) + 0.5 * w.gamma * xi[m] ** 2).sum() > 1e-3 * abs(obj)       # the penalty is visible in the objective
+    # the soft-row block of r_dual: resume with zero further iterations from a state whose xi was scaled by 100 -> that block dominates
+    st2 = {k: v.copy() for k, v in st.items()}
+    st2["xi"] = 100.0 * st["xi"]
+    _, info2, _ = O.admm(w, O.make_cfg(w, zg_given=1), iters=0, state=st2)
+    for b in range(w.B):
+        xi, yg = st2["xi"][b].ravel(), st2["yg"][b].ravel()
+        m = np.tile(np.array(w.soft, dtype=bool), w.T) & (xi != 0)
+        blk = np.abs(w.gamma * xi[m] + w.lam * np.sign(xi[m]) + yg[m]).max()
+        assert blk > 2 * info[b, 1] and abs(info2[b, 1] - blk) < 1e-12 * blk
+
+
+def _kkt_form_iteration(P, q, A, lo, hi, soft, sigma, rho, alpha, gamma, lam, x, z, y):
+    """One iteration of Alg. 3 in the paper's ORIGINAL form: the quasi-definite KKT system eq. 7 solved
+    with numpy for (x~, nu), z~ = z + rho^-1 (nu - y) (OSQP's recovery, equivalent to eq. 9), then eq. 10-16."""
+    nz, m = P.shape[0], A.shape[0]
+    K = np.block([[P + sigma * np.eye(nz), A.T], [A, -np.diag(1.0 / rho)]])
+    sol = np.linalg.solve(K, np.concatenate([sigma * x - q, z - y / rho]))
+    xt, nu = sol[:nz], sol[nz:]
+    zt = z + (nu - y) / rho
+    xn = alpha * xt + (1 - alpha) * x
+    zh = alpha * zt + (1 - alpha) * z
+    v = zh + y / rho
+    pv = np.clip(v, lo, hi)
+    sp = np.maximum(0.0, (rho * (v - hi) - lam) / (rho + gamma)); sm = np.maximum(0.0, (rho * (lo - v) - lam) / (rho + gamma))
+    zn = np.where(soft, pv + sp - sm, pv)
+    xin = np.where(soft, sm - sp, 0.0)
+    yn = y + rho * (zh - zn)
+    return xn, zn, yn, xin
+
+
+@pytest.mark.parametrize("sigma,alpha", [(1e-6, 1.6), (0.3, 1.6), (0.3, 0.7)])
+def test_iterates_equal_kkt_form_of_eq7_every_iteration(sigma, alpha):
+    """Trajectory pin (not a fixed-point pin): after EVERY iteration the oracle's (x, z_g, y_f, y_g, xi) equal the iteration
+    written in the paper's un-reduced form — eq. 7 with the full stacked A = [C; G], l = [c; lo], u = [c; hi] (eq. 2), i.e.
+    equality rows treated like any other row (z_f is projected onto [c, c]) — with a LARGE sigma so that the relaxation of x
+    (eq. 10-11) is visible in eta, and alpha != 1 so that its placement in both dual updates matters."""
+    w = W.random_ltv(5, 1, 4, 3, 2, [3, 4, 0], [0, 0, 1], bound=0.3, implicit=True, dense_g_rows=1, q_scale=0.6)
+    w.soft = [0, 0, 1, 1]; w.lam = 0.05; w.sigma = sigma; w.alpha = alpha; w.rho_bar = 0.7; w.rho_eq_scale = 13.0
+    P, C, c, G = dense_PCG(w, 0)
+    A = np.vstack([C, G]); mf = C.shape[0]
+    lo = np.concatenate([c, w.lo[0].ravel()]); hi = np.concatenate([c, w.hi[0].ravel()])
+    soft = np.concatenate([np.zeros(mf, bool), np.tile(np.array(w.soft, bool), w.T)])
+    rho = np.concatenate([np.full(mf, w.rho_eq_scale * w.rho_bar), np.full(G.shape[0], w.rho_bar)])
+    rng = np.random.default_rng(3)
+    st = O.new_state(w)
+    st["x"] = 0.2 * rng.standard_normal(st["x"].shape); st["yf"] = 0.1 * rng.standard_normal(st["yf"].shape); st["yg"] = 0.1 * rng.standard_normal(st["yg"].shape)
+    x, y = st["x"][0].ravel().copy(), np.concatenate([st["yf"][0], st["yg"][0].ravel()])
+    z = np.concatenate([c, np.clip(G @ x, w.lo[0].ravel(), w.hi[0].ravel())])        # z_f == c, z_g^0 = clip(G x^0) (reading A-12)
+    seen_xi = 0
+    for k in range(25):
+        st, info, rc = O.admm(w, O.make_cfg(w, zg_given=int(k > 0)), iters=1, state=st)
+        x, z, y, xi = _kkt_form_iteration(P, w.q[0].ravel(), A, lo, hi, soft, sigma, rho, alpha, w.gamma, w.lam, x, z, y)
+        assert np.abs(z[:mf] - c).max() == 0                                        # z_f == c (PAPER.md:287-290)
+        for got, ref in ((st["x"][0].ravel(), x), (st["zg"][0].ravel(), z[mf:]), (st["yf"][0], y[:mf]), (st["yg"][0].ravel(), y[mf:]), (st["xi"][0].ravel(), xi[mf:])):
+            assert np.abs(got - ref).max() <= 1e-10 * max(1.0, np.abs(ref).max()), k
+        seen_xi += int((xi != 0).sum())
+    assert seen_xi > 0
+
+
+def test_equality_rows_posed_as_inequality_rows_give_the_same_iterates():
+    """z_f == c / y_f pin: a two-stage problem (N = 1) is re-posed as ONE fat stage (N = 0) whose
+    inequality block holds the original G rows AND the dynamics rows [A^- A^+] v = b as two-sided rows lo = hi = b.  With
+    rho_eq_scale = 1 both problems have the same S, and the general row update y += rho(z^ - clip(.)) must reproduce the
+    native equality update y_f += rho_f alpha (z~_f - c) after every iteration."""
+    import copy
+    w = W.random_ltv(8, 1, 1, 2, 1, [2, 0], [0, 1], bound=0.2, implicit=True, q_scale=0.8)
+    w.rho_eq_scale = 1.0; w.rho_bar = 3.0; w.alpha = 1.7; w.sigma = 0.05
+    n, nx, ng = w.n, w.nx, w.ng
+    f = copy.copy(w)
+    f.N, f.nx, f.nu, f.ng = 0, nx, 2 * n - nx, 2 * ng + nx
+    f.D = np.zeros((1, 1, 2 * n, 2 * n)); f.D[0, 0, :n, :n] = w.D[0, 0]; f.D[0, 0, n:, n:] = w.D[0, 1]; f.D[0, 0, n:, :n] = w.E[0, 0]; f.D[0, 0, :n, n:] = w.E[0, 0].T
+    f.E = np.zeros((1, 0, 2 * n, 2 * n)); f.Am = np.zeros((1, 0, nx, 2 * n)); f.Ap = np.zeros((1, 0, nx, 2 * n)); f.b = np.zeros((1, 0, nx))
+    f.q = w.q.reshape(1, 1, 2 * n)
+    Gd = w.G_dense()[0]
+    f.G = np.zeros((1, 1, f.ng, 2 * n)); f.G[0, 0, :ng, :n] = Gd[0]; f.G[0, 0, ng:2 * ng, n:] = Gd[1]
+    f.G[0, 0, 2 * ng:, :n] = w.Am[0, 0]; f.G[0, 0, 2 * ng:, n:] = w.Ap[0, 0]
+    f.g_col = None
+    f.lo = np.concatenate([w.lo[0, 0], w.lo[0, 1], w.b[0, 0]]).reshape(1, 1, -1); f.hi = np.concatenate([w.hi[0, 0], w.hi[0, 1], w.b[0, 0]]).reshape(1, 1, -1)
+    f.soft = list(w.soft) * 2 + [0] * nx
+    sw, sf = O.new_state(w), O.new_state(f)
+    for k in range(30):
+        sw, _, rc1 = O.admm(w, O.make_cfg(w, band=0, zg_given=int(k > 0)), iters=1, state=sw)
+        sf, _, rc2 = O.admm(f, O.make_cfg(f, band=0, zg_given=int(k > 0)), iters=1, state=sf)
+        assert rc1 == 0 and rc2 == 0
+        assert np.abs(sw["x"].ravel() - sf["x"].ravel()).max() < 1e-12
+        assert np.abs(sw["yf"][0, nx:] - sf["yg"][0, 0, 2 * ng:]).max() < 1e-12 * max(1, np.abs(sw["yf"]).max())      # dynamics multipliers
+        assert np.abs(sw["yf"][0, :nx] - sf["yf"][0]).max() < 1e-12 * max(1, np.abs(sw["yf"]).max())                   # init rows stay native in both
+        assert np.abs(sw["yg"].ravel() - sf["yg"][0, 0, :2 * ng]).max() < 1e-12 and np.abs(sw["xi"].ravel() - sf["xi"][0, 0, :2 * ng]).max() < 1e-12
+        assert np.abs(sf["zg"][0, 0, 2 * ng:] - w.b[0, 0]).max() == 0                                                   # z_f == c
+    assert np.abs(sw["yf"]).max() > 1e-2 and (sw["xi"] != 0).any()
+
+
 # ----------------------------------------------------------------------------------------------- backward vs finite differences
-def _loss_of_solution(w, cfg, iters):
+def _loss_of_solution(w, cfg, iters, xi_weight=0.0):
     st, info, rc = O.admm(w, cfg, iters=iters)
-    return (st["x"] ** 2).sum(axis=(1, 2)), st, info
+    return (st["x"] ** 2).sum(axis=(1, 2)) + xi_weight * (st["xi"] ** 2).sum(axis=(1, 2)), st, info
 
 
-@pytest.mark.parametrize("soft_bound,lam", [(2.0, 100.0), (0.3, 0.0), (0.3, 0.05)], ids=["cfg2_hard_active", "soft_active", "soft_L1"])
-def test_backward_matches_central_finite_differences(soft_bound, lam):
-    """dL/dq and dL/dx_init for L = ||x||^2 (reading A-19) vs central differences of tightly converged solves: 1e-6 relative."""
+@pytest.mark.parametrize("soft_bound,lam,xi_weight", [(2.0, 100.0, 0.0), (0.3, 0.0, 0.0), (0.3, 0.05, 0.0), (0.4, 2.0, 0.0), (0.3, 0.0, 1.0), (0.4, 2.0, 3.0)],
+                         ids=["cfg2_hard_active", "soft_active", "soft_L1", "L1_dead_zone", "soft_active_dLdxi", "L1_dead_zone_dLdxi"])
+def test_backward_matches_central_finite_differences(soft_bound, lam, xi_weight):
+    """dL/dq and dL/dx_init for L = ||x||^2 + xi_weight ||xi||^2 (reading A-19; the xi term exercises the right-hand side
+    -G_s' Sigma_s dL/dxi_s of eq. 65) vs central differences of tightly converged solves: 1e-6 relative.
+    The L1_dead_zone instances hold SOFT rows that sit on their bound with 0 < |y_g| < lambda and xi = 0: the dual-sign
+    rule must class them hard-active (the slack cannot move inside the dead zone, reading A-14)."""
     import copy
     w = W.config2(B=1, N=8, soft_bound=soft_bound)
     w.lam, w.rho_bar = lam, 2.0
     w.q = w.q + 0.3 * np.random.default_rng(5).standard_normal(w.q.shape)
     cfg = O.make_cfg(w)
     iters = 30000
-    L0, st, info = _loss_of_solution(w, cfg, iters)
+    L0, st, info = _loss_of_solution(w, cfg, iters, xi_weight)
     assert info[0, 0] < 1e-11 and info[0, 1] < 1e-11
     cls = O.classify(w, cfg, st, 0)
+    soft = np.array(w.soft, dtype=bool)
     ya = np.abs(st["yg"][0][cls == 1]); assert ya.size == 0 or ya.min() > 1e-4      # screened instance (reading A-17)
     if soft_bound < 1.0:
         assert (cls == 2).sum() > 0
     else:
         assert (cls == 1).sum() > 0
-    dq, dxi, counts, rcs = O.backward(w, cfg, st, 2.0 * st["x"])
+    if lam == 2.0:                                           # dead-zone rows present, strictly inside the dead zone
+        dead = np.abs(st["yg"][0][:, soft][cls[:, soft] == 1])
+        assert dead.size >= 2 and dead.min() > 1e-3 and dead.max() < lam - 1e-2
+        assert (st["xi"][0][:, soft][cls[:, soft] == 1] == 0).all()
+    dLdxi = 2.0 * xi_weight * st["xi"] if xi_weight else None
+    dq, dxi, counts, rcs = O.backward(w, cfg, st, 2.0 * st["x"], dLdxi)
     assert rcs[0] == 0
     rng = np.random.default_rng(6)
     h = 1e-5
@@ -290,15 +412,45 @@ def test_backward_matches_central_finite_differences(soft_bound, lam):
         dirq = rng.standard_normal(w.q.shape)
         wp, wm = copy.copy(w), copy.copy(w)
         wp.q, wm.q = w.q + h * dirq, w.q - h * dirq
-        fd = (_loss_of_solution(wp, cfg, iters)[0] - _loss_of_solution(wm, cfg, iters)[0]) / (2 * h)
+        fd = (_loss_of_solution(wp, cfg, iters, xi_weight)[0] - _loss_of_solution(wm, cfg, iters, xi_weight)[0]) / (2 * h)
         an = (dq * dirq).sum()
         assert abs(fd[0] - an) <= 1e-6 * max(1.0, abs(an))
     for i in range(w.nx):
         wp, wm = copy.copy(w), copy.copy(w)
         wp.x_init, wm.x_init = w.x_init.copy(), w.x_init.copy()
         wp.x_init[0, i] += h; wm.x_init[0, i] -= h
-        fd = (_loss_of_solution(wp, cfg, iters)[0] - _loss_of_solution(wm, cfg, iters)[0]) / (2 * h)
+        fd = (_loss_of_solution(wp, cfg, iters, xi_weight)[0] - _loss_of_solution(wm, cfg, iters, xi_weight)[0]) / (2 * h)
         assert abs(fd[0] - dxi[0, i]) <= 1e-6 * max(1.0, abs(dxi[0, i]))
+    if xi_weight:                                            # the xi term must matter: without it the gradient is visibly different
+        dq0, _, _, _ = O.backward(w, cfg, st, 2.0 * st["x"], None)
+        assert np.abs(dq0 - dq).max() > 1e-3 * np.abs(dq).max()
+
+
+def test_classification_rule_hand_built_states():
+    """Row classification of the backward pass (PAPER.md:878-888 with reading A-16), on hand-built (x, y_g, xi):
+    dual sign first (|y| > eps_y = eps_abs + eps_rel max|y|) -> active, also for soft rows with xi = 0 (L1 dead zone);
+    xi != 0 on a soft row -> soft-active; |y| <= eps_y -> active only within eps_abs + eps_rel |bound| of a bound."""
+    w = W.config2(B=1, N=3, soft_bound=0.5)                 # rows: u1,u2 hard in [-1,1]; x1..x6 soft in [-0.5,0.5]
+    eps_abs, eps_rel = 1e-3, 1e-2
+    cfg = O.make_cfg(w, eps_abs=eps_abs, eps_rel=eps_rel)
+    st = O.new_state(w)
+    x, yg, xi = st["x"][0], st["yg"][0], st["xi"][0]
+    expect = np.zeros((w.T, w.ng), dtype=int)
+    col = w.g_col
+    yg[0, 0] = 5.0; expect[0, 0] = 1                         # max|y| = 5 -> eps_y = 1e-3 + 5e-2 = 0.051
+    yg[0, 1] = -0.06; expect[0, 1] = 1                       # just above eps_y: dual sign decides, whatever x is
+    yg[1, 0] = 0.05; x[1, col[0]] = 0.0; expect[1, 0] = 0    # just below eps_y and far from both bounds
+    x[1, col[1]] = 1.0 - 0.5 * (eps_abs + eps_rel * 1.0); expect[1, 1] = 1      # y = 0, inside the proximity band of hi = 1
+    x[2, col[0]] = 1.0 - 2.0 * (eps_abs + eps_rel * 1.0); expect[2, 0] = 0      # y = 0, outside the band
+    x[2, col[1]] = -1.0 + 0.5 * (eps_abs + eps_rel * 1.0); expect[2, 1] = 1     # lower bound, inside the band
+    yg[0, 2] = 0.3; xi[0, 2] = 0.0; expect[0, 2] = 1         # SOFT row, xi = 0, |y| > eps_y: L1 dead zone -> hard-active
+    yg[0, 3] = 0.3; xi[0, 3] = -0.2; expect[0, 3] = 2        # soft row with slack: soft-active, the slack test comes first
+    xi[1, 2] = 0.5 * eps_abs; x[1, col[2]] = 0.0; expect[1, 2] = 0                # |xi| below eps_abs does not count as slack
+    x[1, col[3]] = 0.5 - 0.5 * (eps_abs + eps_rel * 0.5); expect[1, 3] = 1      # soft row, y = 0, xi = 0, on its bound
+    x[2, col[3]] = 0.5 - 2.0 * (eps_abs + eps_rel * 0.5); expect[2, 3] = 0      # relative part uses |bound| = 0.5
+    w.lo[0, 3, 4] = -np.inf; x[3, col[4]] = -7.0; expect[3, 4] = 0               # an infinite bound is never "near"
+    got = O.classify(w, cfg, st, 0)
+    assert (got == expect).all(), (got, expect)
 
 
 def test_backward_unconstrained_closed_form():
@@ -354,12 +506,20 @@ def test_sqp_driver_reduces_dynamics_residual_and_is_consistent_with_admm():
     st, info, rc, fnorm = O.sqp_bicycle(w, cfg, n_sqp=5, iters=200, with_fnorm=True)
     assert rc == 0 and (fnorm[:, -1] < 1e-3 * fnorm[:, 0]).all()
     st1, info1, rc1 = O.sqp_bicycle(w, cfg, n_sqp=1, iters=50)
+    st3, info3, rc3 = O.sqp_bicycle(w, cfg, n_sqp=3, iters=50)
     import copy
     for b in range(w.B):
-        Am, Ap, bb, G, lo, hi = O.bicycle_linearize(w, cfg, w.xbar0[b], b)
-        wq = copy.copy(w)
-        wq.B, wq.Am, wq.Ap, wq.b, wq.G, wq.lo, wq.hi = 1, Am[None], Ap[None], bb[None], G[None], lo[None], hi[None]
-        wq.q, wq.x_init, wq.model = w.q[b:b + 1], w.x_init[b:b + 1], 0
-        s0 = O.new_state(wq); s0["x"] = w.xbar0[b:b + 1].copy()
-        s, _, _ = O.admm(wq, O.make_cfg(wq), iters=50, state=s0)
-        assert np.abs(s["x"][0] - st1["x"][b]).max() < 1e-12
+        # reading A-26 by hand, three steps: linearise at xbar -> K iterations warm-started at x^0 = xbar with y_f, y_g CARRIED
+        # and z_g RE-PROJECTED (zg_given = 0: z_g^0 = clip(G xbar, lo, hi) with the NEW shifted bounds) -> full step xbar <- x^K
+        s = O.new_state(w, B=1); s["x"] = w.xbar0[b:b + 1].copy()
+        for step in range(3):
+            Am, Ap, bb, G, lo, hi = O.bicycle_linearize(w, cfg, s["x"][0], b)
+            wq = copy.copy(w)
+            wq.B, wq.Am, wq.Ap, wq.b, wq.G, wq.lo, wq.hi = 1, Am[None], Ap[None], bb[None], G[None], lo[None], hi[None]
+            wq.q, wq.x_init, wq.model = w.q[b:b + 1], w.x_init[b:b + 1], 0
+            s, _, _ = O.admm(wq, O.make_cfg(wq), iters=50, state=s)
+            if step == 0:
+                assert np.abs(s["x"][0] - st1["x"][b]).max() < 1e-12
+        for k in ("x", "zg", "yf", "yg", "xi"):
+            assert np.abs(s[k][0] - st3[k][b]).max() < 1e-12 * max(1.0, np.abs(st3[k][b]).max()), k
+        assert np.abs(st3["yf"][b]).max() > 1e-3                # the carried multipliers are not trivially zero
