@@ -1,15 +1,20 @@
 #!/usr/bin/env python
-"""bench.py — throughput of the batched ADMM-QP hot path on B200 (BASELINE.json metric).
+"""bench.py — throughput of the batched ADMM-QP hot path on B200 (BASELINE.json metric: "batched QP solves/s & ADMM iters/s,
+ms/solve; % of HBM/FP roofline" for the five configs).
 
-  python bench.py --gpus N --steps K --warmup W [--config 2] [--dtype f32] [--impl reference]
+  python bench.py --gpus N --steps K --warmup W [--config 1..5] [--dtype f32|f64] [--impl reference]
 
 A step = one pass of the hot path over one batch of synthetic QPs: configs 1-3: tmpc_factor + tmpc_admm_solve
-(fixed iteration count); configs 4-5: n_sqp x (tmpc_linearize + tmpc_factor + tmpc_admm_solve).  Default workload
-(N=1): BASELINE.json configs[1] = random LTV QP batch, B=1024, N=50, nx=6, nu=2, rate cost + slack, fp32,
-100 ADMM iterations; its backward pass is timed separately and reported as `backward_ms`.
+(fixed iteration count); configs 4-5: n_sqp x (tmpc_linearize + tmpc_factor + tmpc_admm_solve).
+Without --config the run covers ALL FIVE configs and prints ONE JSON line: the headline (value, config.workload, roofline,
+e2e, cpu_baseline) is config 4 (bicycle SQP, B = 4096, fp32: the largest batch, and the one that exercises linearise +
+factor + solve), and `per_config` carries the same fields for configs 1, 2 (fp32 and fp64, with `backward_ms`), 3 and 5.
+With --config C only that config is run (it is then the headline).
 value = QP solves per second over all ranks (each rank solves its own batch: weak scaling, no collective on the
 data path; NCCL only carries the barrier and the max-over-ranks reduction of the timings).
-`--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded sample of the same workload.
+The ALU and shared-memory roofline denominators are MEASURED in the same run with tmpc_measure_peak (FMA-chain and
+LDS.128 micro-benchmarks, include/tmpc.h); the HBM one comes from MEASURED_PEAKS.json.
+`--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded sample of the same workloads.
 """
 import argparse
 import json
@@ -28,8 +33,14 @@ sys.path.insert(0, ROOT)
 FLOPS_PER_ITER = {1: 7.6e3, 2: 36.1e3, 3: 2.75e6, 4: 37.7e3, 5: 3.1e6}
 # algorithmic HBM bytes per problem per ADMM iteration for the streamed class (config 3) — SURVEY.md 8(d)
 BYTES_PER_ITER = {3: 4.33e6}
-FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 FMA lanes x 2 flop x 1965 MHz
-FP64_PEAK_TFLOPS = FP32_PEAK_TFLOPS / 2               # 64 FP64 FMA lanes per SM
+# nominal ALU peaks, used only if the micro-benchmark entry is unavailable: 148 SMs x 128 FP32 (64 FP64) FMA lanes x 2 x 1965 MHz
+NOMINAL_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
+DEFAULT_DTYPE = {1: "f64", 2: "f32", 3: "f32", 4: "f32", 5: "f64"}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per tmpc_admm_solve call, from committed `ncu --set full`
+# captures: (bytes, profiles/ file).  Only quoted for the exact workload the capture was taken on; None otherwise.
+NCU_TRAFFIC = {}
+KERNEL_NAMES = {1: "admm2_kernel", 2: "admm2_kernel", 3: "admm_stream_kernel x chunk launches", 4: "admm2_kernel", 5: "cr2_admm_kernel"}
+STEPS_CAP = {3: 5, 5: 10}     # per_config legs of the all-configs run: the 95 ms / 6 ms steps need fewer repetitions for a stable mean
 
 
 def make_workload(cfg_id, dtype, batch=None, rank=0):
@@ -112,46 +123,71 @@ def oracle_sample_size(cfg_id):
     return {1: 1, 2: 1024, 3: 64, 4: 1024, 5: 1}[cfg_id]
 
 
+def config_list(args):
+    """(config id, dtype) pairs of this run, headline first."""
+    if args.config is not None:
+        return [(args.config, args.dtype or DEFAULT_DTYPE[args.config])]
+    return [(4, "f32"), (1, "f64"), (2, "f32"), (2, "f64"), (3, "f32"), (5, "f64")]
+
+
+def key_of(cfg_id, dtype):
+    return f"config{cfg_id}_{dtype}"
+
+
+def reference_one(cfg_id, dtype, args, cores):
+    w = make_workload(cfg_id, dtype, args.batch)
+    nb = oracle_sample_size(cfg_id)
+    for _ in range(args.warmup if args.config is not None else 0):
+        oracle_rate(w, cfg_id, cores, nb)
+    t, desc = 0.0, ""
+    steps = args.steps if args.config is not None else 1
+    for _ in range(steps):
+        r, desc, dt = oracle_rate(w, cfg_id, cores, nb)
+        t += dt
+    rate = min(w.B, nb) * steps / t
+    return {"value": rate, "unit": "QP solves/s", "ms_per_step": 1e3 * t / steps, "dtype": "f64", "config": {"workload": workload_name(w, dtype)},
+            "admm_iters_per_s": rate * total_iters(w),
+            "cpu_baseline": {"value": rate, "unit": "QP solves/s", "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": rate, "unit": "QP solves/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    w = make_workload(args.config, args.dtype, args.batch)
     cores = len(os.sched_getaffinity(0))
-    nb = oracle_sample_size(args.config)
-    for _ in range(args.warmup):
-        oracle_rate(w, args.config, cores, nb)
-    t, desc = 0.0, ""
-    for _ in range(args.steps):
-        r, desc, dt = oracle_rate(w, args.config, cores, nb)
-        t += dt
-    rate = min(w.B, nb) * args.steps / t
-    line = {"impl": "reference", "metric": "batched QP solves/s", "value": rate, "unit": "QP solves/s", "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": {"workload": workload_name(w, args.dtype)},
-            "cpu_baseline": {"value": rate, "unit": "QP solves/s", "cores": cores, "kind": "oracle", "sample": desc},
-            "e2e": {"value": rate, "unit": "QP solves/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    res = [(c, d, reference_one(c, d, args, cores)) for c, d in config_list(args)]
+    c0, d0, head = res[0]
+    line = {"impl": "reference", "metric": "batched QP solves/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "data": "synthetic"}
+    line.update(head)
+    if len(res) > 1:
+        line["per_config"] = {key_of(c, d): r for c, d, r in res[1:]}
     print(json.dumps(line))
 
 
-def run_gpu(args):
+def measure_peaks(dev, stream):
+    """FP32 / FP64 FMA and shared-memory peaks of this GPU at the clocks found, via the library's micro-benchmark entry."""
+    import torch
+    from paper_2606_24039_b200 import binding as Bd
+    scratch = torch.zeros(64, dtype=torch.float32, device=dev)
+    m = lambda what: Bd.tmpc_measure_peak(what, scratch.data_ptr(), stream.cuda_stream, 5)
+    ffma2, ffma, dfma, lds = m(Bd.TMPC_PEAK_FFMA2), m(Bd.TMPC_PEAK_FFMA), m(Bd.TMPC_PEAK_DFMA), m(Bd.TMPC_PEAK_LDS)
+    return {"f32_tflops": max(ffma2, ffma), "f32_ffma2_tflops": ffma2, "f32_ffma_tflops": ffma, "f64_tflops": dfma, "lds_gbs": lds,
+            "how": "tmpc_measure_peak: independent FMA chains (3-register FFMA2 / FFMA / DFMA) and conflict-free LDS.128, 4 CTAs x 512 threads per SM, best of 5, CUDA events"}
+
+
+def gpu_one(cfg_id, dtype, args, ctx, steps, with_cpu):
+    """Times one config; returns the dict of its metrics (rank 0: complete; other ranks: None after taking part in the reductions)."""
     import torch
     import torch.distributed as dist
     from paper_2606_24039_b200 import binding as Bd
     from paper_2606_24039_b200.solver import Solver
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
-    dev = torch.device(f"cuda:{local}")
-    w = make_workload(args.config, args.dtype, args.batch, rank)
-    linsolve = Bd.TMPC_LIN_CYCLIC_REDUCTION if args.config == 5 else Bd.TMPC_LIN_SEQUENTIAL
-    s = Solver(w, dtype=args.dtype, device=dev, linsolve=linsolve)
-    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    world, rank, local, dev, peaks = ctx["world"], ctx["rank"], ctx["local"], ctx["dev"], ctx["peaks"]
+    w = make_workload(cfg_id, dtype, args.batch, rank)
+    linsolve = Bd.TMPC_LIN_CYCLIC_REDUCTION if cfg_id == 5 else Bd.TMPC_LIN_SEQUENTIAL
+    s = Solver(w, dtype=dtype, device=dev, linsolve=linsolve)
+    flush = ctx["flush"]
     x0 = s._up(w.xbar0) if w.model else None
 
     def reset():
@@ -162,9 +198,8 @@ def run_gpu(args):
                 v.zero_()
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    solve_ms = []
 
-    def step(timed):
+    def step():
         """one pass of the hot path; returns (start, end, [(a,b) events around each tmpc_admm_solve])."""
         a, b, inner = ev(), ev(), []
         a.record()
@@ -184,15 +219,16 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    for _ in range(max(3, args.warmup)):
-        reset(); step(False)
+    warm = max(3, args.warmup)
+    for _ in range(warm):
+        reset(); step()
     barrier()
     sampler = ClockSampler(local); sampler.start()
     l0 = s.launches()
     recs = []
-    for _ in range(args.steps):
+    for _ in range(steps):
         reset(); flush.zero_()
-        recs.append(step(True))
+        recs.append(step())
     barrier()
     launches = s.launches() - l0
     clocks = sampler.summary()
@@ -205,19 +241,19 @@ def run_gpu(args):
     total_ms = float(tot.item())
     info = s.info_numpy()
 
-    # ---- backward (config 2), separately
+    # ---- backward (config 2), separately: REFACTOR_REFINE at the state the solve left
     backward_ms = None
-    if args.config == 2:
+    if cfg_id == 2:
         dLdx = 2.0 * s.s["x"]
         ts = []
-        for _ in range(3 + args.steps):
+        for _ in range(3 + steps):
             s.factor(); flush.zero_()
             a, b = ev(), ev(); a.record(); s.backward(dLdx); b.record(); torch.cuda.synchronize(dev); ts.append(a.elapsed_time(b))
         backward_ms = float(np.median(ts[3:]))
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
-    if not w.model and args.config != 5:
+    if not w.model and cfg_id != 5:
         hp = lambda t: t.detach().cpu().pin_memory()
         ht = {k: (hp(v) if v is not None else None) for k, v in s.t.items()}
         hs = {k: hp(torch.zeros_like(v)) for k, v in s.s.items()}
@@ -231,7 +267,7 @@ def run_gpu(args):
         h2d = sum(v.numel() * v.element_size() for v in ht.values() if v is not None) + sum(hs[k].numel() * hs[k].element_size() for k in ("x", "yf", "yg"))
         d2h = sum(v.numel() * v.element_size() for v in hs.values()) + sum(v.numel() * v.element_size() for v in hi.values())
         ts = []
-        for i in range(3 + args.steps):
+        for i in range(3 + steps):
             for v in hs.values():
                 v.zero_()
             torch.cuda.synchronize(dev)
@@ -241,76 +277,111 @@ def run_gpu(args):
         t_e2e = torch.tensor([sum(ts[3:])], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
-        e2e = {"value": w.B * world * args.steps / float(t_e2e.item()), "unit": "QP solves/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-               "ms_per_step": 1e3 * float(t_e2e.item()) / args.steps}
+        e2e = {"value": w.B * world * steps / float(t_e2e.item()), "unit": "QP solves/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "ms_per_step": 1e3 * float(t_e2e.item()) / steps}
         assert np.abs(hs["x"].double().numpy() - s.state_numpy()["x"]).max() < 1e-3, "host path disagrees with device path"
+        del staging
     else:
         # model configs: the same public calls with pinned host inputs copied in and the result copied out every step
         hx0 = x0.cpu().pin_memory(); href = s.t["stage_ref"].cpu().pin_memory(); hq_ = s.t["q"].cpu().pin_memory(); hxi = s.t["x_init"].cpu().pin_memory()
         hout = torch.empty_like(hx0).pin_memory()
         ts = []
-        for i in range(2 + args.steps):
+        for i in range(2 + steps):
             reset(); torch.cuda.synchronize(dev)
             t0 = time.perf_counter()
             s.s["x"].copy_(hx0, non_blocking=True); s.t["stage_ref"].copy_(href, non_blocking=True)
             s.t["q"].copy_(hq_, non_blocking=True); s.t["x_init"].copy_(hxi, non_blocking=True)
-            step(False)
+            step()
             hout.copy_(s.s["x"], non_blocking=True); torch.cuda.synchronize(dev)
             ts.append(time.perf_counter() - t0)
         t_e2e = torch.tensor([sum(ts[2:])], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
         nb = lambda t: t.numel() * t.element_size()
-        e2e = {"value": w.B * world * args.steps / float(t_e2e.item()), "unit": "QP solves/s", "h2d_bytes_per_step": int(nb(hx0) + nb(href) + nb(hq_) + nb(hxi)),
-               "d2h_bytes_per_step": int(nb(hout)), "ms_per_step": 1e3 * float(t_e2e.item()) / args.steps}
-
+        e2e = {"value": w.B * world * steps / float(t_e2e.item()), "unit": "QP solves/s", "h2d_bytes_per_step": int(nb(hx0) + nb(href) + nb(hq_) + nb(hxi)),
+               "d2h_bytes_per_step": int(nb(hout)), "ms_per_step": 1e3 * float(t_e2e.item()) / steps}
+    s.close()
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
-    ms_per_step = total_ms / args.steps
+        return None
+    ms_per_step = total_ms / steps
     value = w.B * world / (ms_per_step * 1e-3)
     iters = total_iters(w)
     kern_avg_ms = sum(kern_ms) / max(1, n_admm_launch)
-    if args.config == 3:
+    if cfg_id == 3:
         alg = BYTES_PER_ITER[3] * w.B * w.iters
-        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else None
-        peak = peaks["hbm_gbs"] if peaks else 6650.0
-        roof = {"bound": "hbm", "achieved": alg / (kern_avg_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s", "peak_source": "measured" if peaks else "fallback"}
+        mp = ctx["measured_peaks"]
+        # the kernel is timed inside a long step of back-to-back launches: the burst copy figure is the stricter denominator
+        peak = mp["hbm_gbs"] if mp else 6650.0
+        roof = {"bound": "hbm", "achieved": alg / (kern_avg_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                "peak_source": "measured: MEASURED_PEAKS.json hbm_gbs (copy bandwidth)" if mp else "fallback of B200_PROFILING.md"}
     else:
-        alg = FLOPS_PER_ITER[args.config] * w.B * w.iters
-        peak = FP64_PEAK_TFLOPS if args.dtype == "f64" else FP32_PEAK_TFLOPS
-        roof = {"bound": "alu", "achieved": alg / (kern_avg_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s", "peak_source": "derived: 148 SMs x 128 (fp32) / 64 (fp64) FMA lanes x 2 x 1965 MHz"}
+        alg = FLOPS_PER_ITER[cfg_id] * w.B * w.iters
+        if peaks:
+            peak = peaks["f64_tflops"] if dtype == "f64" else peaks["f32_tflops"]
+            src = "measured: tmpc_measure_peak FMA-chain micro-benchmark in this run (" + ("DFMA" if dtype == "f64" else "max of FFMA2, FFMA") + ")"
+        else:
+            peak, src = NOMINAL_TFLOPS[dtype], "nominal: 148 SMs x 128 (fp32) / 64 (fp64) FMA lanes x 2 x 1965 MHz"
+        roof = {"bound": "alu", "achieved": alg / (kern_avg_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s", "peak_source": src}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed `ncu --set full` captures
-    # (profiles/r01_v2_ncu_full_admm2_*.md, profiles/r01_v3_ncu_full_admm_stream_*.md); only valid for the workload the capture was taken on
-    # config 3: one tmpc_admm_solve = 7 chunk launches; the capture is ONE full-wave launch (296 CTAs x 50
-    # iterations: 65.42 GB read + 0.57 GB written), scaled to the 2048 chunk jobs of a call, like `achieved` (whole call)
-    ncu_traffic = {(2, "f32", 1024): 57.05e6 + 0.29e6, (3, "f32", 512): (65.42e9 + 0.572e9) * 2048 / 296}
-    roof["traffic"] = ncu_traffic.get((args.config, args.dtype, w.B))
-    roof["kernel"] = {1: "admm2_kernel", 2: "admm2_kernel", 3: "admm_stream_kernel x chunk launches", 4: "admm2_kernel", 5: "cr2_admm_kernel"}[args.config] + " (tmpc_admm_solve)"
-    if args.config in (1, 2, 4):
+    tr = NCU_TRAFFIC.get((cfg_id, dtype, w.B))
+    roof["traffic"] = tr[0] if tr else None
+    if tr:
+        roof["traffic_source"] = tr[1]
+    roof["kernel"] = ctx["kernel_names"][cfg_id] + " (tmpc_admm_solve)"
+    if cfg_id in (1, 2, 4) and peaks:
         # supplementary: the resident class reads every factor / constraint element from SHARED memory once per use, so the
-        # binding on-chip resource is LDS bandwidth (148 SMs x 128 B/clk x 1965 MHz), not the FMA pipe
-        es = 8 if args.dtype == "f64" else 4
+        # binding on-chip resource of its stage-parallel phases is LDS bandwidth, not the FMA pipe (DESIGN.md 5.1 / 6)
+        es = 8 if dtype == "f64" else 4
         lds_bytes = (2 * w.N * w.n * w.n + 2 * w.T * w.n * w.n + 4 * w.N * w.nx * w.n) * es * w.B * w.iters
-        lds_peak = 148 * 128 * 1.965e9 / 1e9
-        roof["lds"] = {"achieved": lds_bytes / (kern_avg_ms * 1e-3) / 1e9, "peak": lds_peak, "unit": "GB/s", "frac": lds_bytes / (kern_avg_ms * 1e-3) / 1e9 / lds_peak,
-                       "note": "algorithmic shared-memory bytes (B twice, X twice, A~-/A~+ twice per iteration) / kernel time",
-                       "lsu_wavefront_util_ncu": {(2, "f32", 1024): 0.523}.get((args.config, args.dtype, w.B))}   # l1tex__data_pipe_lsu_wavefronts_mem_shared pct of peak, profiles/
+        roof["lds"] = {"achieved": lds_bytes / (kern_avg_ms * 1e-3) / 1e9, "peak": peaks["lds_gbs"], "unit": "GB/s", "frac": lds_bytes / (kern_avg_ms * 1e-3) / 1e9 / peaks["lds_gbs"],
+                       "peak_source": "measured: tmpc_measure_peak LDS.128 micro-benchmark in this run",
+                       "note": "algorithmic shared-memory bytes (B twice, X twice, A~-/A~+ twice per iteration) / kernel time"}
     roof["kernel_ms_per_launch"] = kern_avg_ms
     roof["kernel_share_of_step"] = sum(kern_ms) / sum(step_ms)
-    line = {"metric": "batched QP solves/s", "value": value, "unit": "QP solves/s", "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
-            "config": {"workload": workload_name(w, args.dtype), "l2": "256 MB flush write between timed steps", "step": "tmpc_factor + tmpc_admm_solve" if not w.model else "n_sqp x (tmpc_linearize + tmpc_factor + tmpc_admm_solve)"},
-            "admm_iters_per_s": value * iters, "ms_per_batched_solve": ms_per_step, "us_per_admm_iteration": 1e3 * ms_per_step / iters,
-            "backward_ms": backward_ms, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "roofline": roof,
-            "parity_snapshot": {"max_r_prim": float(np.max(info["r_prim"])), "max_r_dual": float(np.max(info["r_dual"])), "status_nonzero": int((info["status"] != 0).sum())}}
-    if world == 1 and not args.no_cpu_baseline:
+    res = {"value": value, "unit": "QP solves/s", "steps": steps, "warmup": warm, "ms_per_step": ms_per_step, "dtype": dtype,
+           "config": {"workload": workload_name(w, dtype), "l2": "256 MB flush write between timed steps",
+                      "step": "tmpc_factor + tmpc_admm_solve" if not w.model else "n_sqp x (tmpc_linearize + tmpc_factor + tmpc_admm_solve)"},
+           "admm_iters_per_s": value * iters, "ms_per_batched_solve": ms_per_step, "us_per_admm_iteration": 1e3 * ms_per_step / iters,
+           "backward_ms": backward_ms, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "roofline": roof,
+           "parity_snapshot": {"max_r_prim": float(np.max(info["r_prim"])), "max_r_dual": float(np.max(info["r_dual"])), "status_nonzero": int((info["status"] != 0).sum())}}
+    if with_cpu:
         cores = len(os.sched_getaffinity(0))
-        r, desc, dt = oracle_rate(w, args.config, cores, oracle_sample_size(args.config))
-        line["cpu_baseline"] = {"value": r, "unit": "QP solves/s", "cores": cores, "kind": "oracle", "sample": desc, "seconds": dt}
-    print(json.dumps(line))
+        r, desc, dt = oracle_rate(w, cfg_id, cores, oracle_sample_size(cfg_id))
+        res["cpu_baseline"] = {"value": r, "unit": "QP solves/s", "cores": cores, "kind": "oracle", "sample": desc, "seconds": dt}
+    return res
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = torch.device(f"cuda:{local}")
+    mpath = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    ctx = {"world": world, "rank": rank, "local": local, "dev": dev,
+           "flush": torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev),   # > 126 MB L2
+           "measured_peaks": json.load(open(mpath)) if os.path.exists(mpath) else None,
+           "peaks": measure_peaks(dev, torch.cuda.current_stream(dev)),
+           "kernel_names": KERNEL_NAMES}
+    res = []
+    for i, (c, d) in enumerate(config_list(args)):
+        steps = args.steps if (args.config is not None or i == 0) else max(3, min(args.steps, STEPS_CAP.get(c, args.steps)))
+        res.append((c, d, gpu_one(c, d, args, ctx, steps, world == 1 and not args.no_cpu_baseline)))
+    if rank == 0:
+        c0, d0, head = res[0]
+        line = {"metric": "batched QP solves/s", "n_gpus": world, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "data": "synthetic"}
+        line.update(head)
+        line["measured_peaks"] = ctx["peaks"]
+        if len(res) > 1:
+            line["per_config"] = {key_of(c, d): r for c, d, r in res[1:]}
+            line["gpu_launches"] = int(sum(r["gpu_launches"] for _, _, r in res))
+        print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 
@@ -321,13 +392,11 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="tmpc", choices=["tmpc", "reference"])
-    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--config", type=int, default=None, choices=[None, 1, 2, 3, 4, 5])
     ap.add_argument("--dtype", default=None, choices=[None, "f32", "f64"])
     ap.add_argument("--batch", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
-    if args.dtype is None:
-        args.dtype = {1: "f64", 2: "f32", 3: "f32", 4: "f32", 5: "f64"}[args.config]
     if args.impl == "reference":
         run_reference(args)
     else:

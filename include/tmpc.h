@@ -43,7 +43,7 @@ typedef enum { TMPC_LIN_SEQUENTIAL = 0, TMPC_LIN_CYCLIC_REDUCTION = 1, TMPC_LIN_
 typedef enum { TMPC_BWD_REFACTOR_REFINE = 0, TMPC_BWD_ADMM_REUSE_FACTOR = 1 } tmpc_bwd_mode;
 
 /* info.status[b] bits */
-#define TMPC_ST_PIVOT 1  /* a non-positive pivot was met while factoring S (replaced by a tiny positive one) */
+#define TMPC_ST_PIVOT 1  /* a non-positive or non-finite pivot was met while factoring S (replaced by 1: the problem's result is garbage) */
 #define TMPC_ST_NAN 2    /* a non-finite value appeared in the iterate */
 /* tmpc_admm_solve flags */
 #define TMPC_SOLVE_ZG_GIVEN 1 /* use state.zg / state.xi as passed (resume); default z_g^0 = clip(G x^0, lo, hi) */
@@ -84,7 +84,8 @@ typedef struct { /* ADMM state, in/out = warm start (Alg. 3 'Initial guess', PAP
 
 typedef struct { /* per-problem outputs at the last iterate (eq. 3); any pointer may be NULL */
   void* r_prim; void* r_dual; void* objective; /* [B] working dtype */
-  int32_t* status;                             /* [B] TMPC_ST_* bits (written by tmpc_factor and tmpc_admm_solve) */
+  int32_t* status;                             /* [B] TMPC_ST_* bits, OVERWRITTEN by tmpc_admm_solve (no need to zero it): TMPC_ST_PIVOT as
+                                                  found by the last tmpc_factor (kept per problem in the workspace), TMPC_ST_NAN from the iterate */
 } tmpc_info;
 
 /* Bytes of device workspace tmpc_setup needs for this config. */
@@ -118,6 +119,15 @@ tmpc_status tmpc_kkt_solve(tmpc_handle h, const void* eta, void* xt);
 tmpc_status tmpc_host_staging_bytes(const tmpc_config* cfg, size_t* bytes);
 tmpc_status tmpc_admm_solve_host(tmpc_handle h, const tmpc_qp* host_qp, tmpc_state* host_st, int32_t iters, int32_t flags,
                                  tmpc_info* host_info, void* staging, size_t staging_bytes);
+/* Diagnostic: measures a roofline denominator of this GPU at the clocks found with a micro-benchmark kernel.
+ * what = TMPC_PEAK_FFMA2 / FFMA / DFMA -> *out in TFLOP/s (independent fused multiply-add chains, 3-register form);
+ * TMPC_PEAK_LDS -> *out in GB/s (conflict-free 16-byte shared-memory loads).  scratch: >= 16 bytes of DEVICE memory.
+ * Runs `reps` timed launches (+1 warm-up) on cuda_stream, synchronises, returns the best.  HOST pointer `out`. */
+#define TMPC_PEAK_FFMA2 0
+#define TMPC_PEAK_FFMA 1
+#define TMPC_PEAK_DFMA 2
+#define TMPC_PEAK_LDS 3
+tmpc_status tmpc_measure_peak(int32_t what, void* scratch, void* cuda_stream, int32_t reps, double* out);
 tmpc_status tmpc_destroy(tmpc_handle h);
 const char* tmpc_status_string(tmpc_status s);
 /* Number of kernels this handle has launched so far (for bench.py's gpu_launches). */

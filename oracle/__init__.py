@@ -136,6 +136,24 @@ def admm(w, cfg, iters=None, state=None, nthreads=1):
     return st, info, rc
 
 
+def admm_rows(w, cfg, soft_rows, iters, state=None):
+    """Alg. 3 with a per-row soft flag array soft_rows [B,T,ng] (uint8) instead of the per-row-type mask (adjoint QP, eq. 67)."""
+    n, T, nz, mf, mg = _dims(w)
+    st = new_state(w) if state is None else {k: _c(v).copy() for k, v in state.items()}
+    info = np.zeros((w.B, 4))
+    f = lib().orc_admm_rows
+    f.argtypes = [C.c_void_p] * 17 + [C.c_int, C.c_void_p]
+    sr = np.ascontiguousarray(soft_rows, dtype=np.uint8)
+    rc = 0
+    for b in range(w.B):
+        D, E = _c(_bs(w.D, b)), _c(_bs(w.E, b))
+        G = None if cfg.g_sel else _c(_bs(w.G, b))
+        rc |= f(C.byref(cfg), _p(D), _p(E), _p(_c(w.q[b])), _p(_c(w.Am[b])), _p(_c(w.Ap[b])), _p(_c(w.b[b])), _p(_c(w.x_init[b])), _p(G),
+                _p(_c(w.lo[b])), _p(_c(w.hi[b])), sr[b].ctypes.data_as(C.c_void_p), _p(st["x"][b]), _p(st["zg"][b]), _p(st["yf"][b]),
+                _p(st["yg"][b]), _p(st["xi"][b]), iters, _p(info[b]))
+    return st, info, rc
+
+
 def backward(w, cfg, state, dLdx, dLdxi=None):
     """O-5 on every problem.  Returns dq [B,T,n], dxinit [B,nx], counts [B,2], rc [B]."""
     n, T, nz, mf, mg = _dims(w)

@@ -167,7 +167,10 @@ inline void project_row(bool soft, double v, double lo, double hi, double rho, d
 struct Info { double r_prim, r_dual, objective, min_pivot; };
 
 // O-3.  K iterations of Alg. 3.  x [nz], zg [mg], yf [mf], yg [mg], xi [mg] in/out.
-Info admm(const Cfg& cf, const QP& p, double* x_, double* zg_, double* yf_, double* yg_, double* xi_, int K) {
+// soft_rows (optional, [mg]): per-ROW soft flag replacing the per-row-type mask cf.soft — used for the adjoint QP eq. 67, whose
+// soft rows are the soft-ACTIVE rows of one particular solution; the arithmetic is the same.
+Info admm(const Cfg& cf, const QP& p, double* x_, double* zg_, double* yf_, double* yg_, double* xi_, int K, const uint8_t* soft_rows = nullptr) {
+  auto is_soft = [&](int i) { return soft_rows ? soft_rows[i] != 0 : cf.soft[i % p.ng] != 0; };
   const double rho_g = cf.rho_bar, rho_f = cf.rho_eq_scale * cf.rho_bar, sigma = cf.sigma, alpha = cf.alpha;
   vec x(x_, x_ + p.nz), zg(p.mg), yf(yf_, yf_ + p.mf), yg(yg_, yg_ + p.mg), xi(p.mg, 0.0);
   vec tmp(p.mg);
@@ -190,7 +193,7 @@ Info admm(const Cfg& cf, const QP& p, double* x_, double* zg_, double* yf_, doub
     for (int i = 0; i < p.mg; ++i) {
       double zh = alpha * ztg[i] + (1.0 - alpha) * zg[i];
       double v = zh + yg[i] / rho_g, z, s;
-      project_row(cf.soft[i % p.ng] != 0, v, p.lo[i], p.hi[i], rho_g, cf.gamma, cf.lam, z, s);
+      project_row(is_soft(i), v, p.lo[i], p.hi[i], rho_g, cf.gamma, cf.lam, z, s);
       zg[i] = z; xi[i] = s; yg[i] = yg[i] + rho_g * (zh - z);
     }
     for (int i = 0; i < p.mf; ++i) yf[i] = yf[i] + rho_f * alpha * (ztf[i] - p.c[i]);
@@ -204,7 +207,7 @@ Info admm(const Cfg& cf, const QP& p, double* x_, double* zg_, double* yf_, doub
   p.C.mulT_add(yf, g); p.G.mulT_add(yg, g);
   double rd = 0; for (int i = 0; i < p.nz; ++i) rd = std::max(rd, std::fabs(g[i]));
   double obj = 0; for (int i = 0; i < p.nz; ++i) obj += 0.5 * x[i] * Px[i] + p.q[i] * x[i];
-  for (int i = 0; i < p.mg; ++i) if (cf.soft[i % p.ng] && xi[i] != 0.0) {
+  for (int i = 0; i < p.mg; ++i) if (is_soft(i) && xi[i] != 0.0) {
     double sg = xi[i] > 0 ? 1.0 : -1.0;
     rd = std::max(rd, std::fabs(cf.gamma * xi[i] + cf.lam * sg + yg[i]));
     obj += cf.lam * std::fabs(xi[i]) + 0.5 * cf.gamma * xi[i] * xi[i];
@@ -343,6 +346,16 @@ int orc_admm(const Cfg* cf, const double* D, const double* E, const double* q, c
              const double* G, const double* lo, const double* hi, double* x, double* zg, double* yf, double* yg, double* xi, int K, double* info_out) {
   QP p = assemble(*cf, D, E, q, Am, Ap, b, x_init, G, lo, hi);
   Info i = admm(*cf, p, x, zg, yf, yg, xi, K);
+  info_out[0] = i.r_prim; info_out[1] = i.r_dual; info_out[2] = i.objective; info_out[3] = i.min_pivot;
+  return i.min_pivot > 0 ? 0 : 1;
+}
+
+// One problem with a per-row soft flag array soft_rows [mg] (adjoint QP, eq. 67).
+int orc_admm_rows(const Cfg* cf, const double* D, const double* E, const double* q, const double* Am, const double* Ap, const double* b, const double* x_init,
+                  const double* G, const double* lo, const double* hi, const uint8_t* soft_rows, double* x, double* zg, double* yf, double* yg, double* xi, int K,
+                  double* info_out) {
+  QP p = assemble(*cf, D, E, q, Am, Ap, b, x_init, G, lo, hi);
+  Info i = admm(*cf, p, x, zg, yf, yg, xi, K, soft_rows);
   info_out[0] = i.r_prim; info_out[1] = i.r_dual; info_out[2] = i.objective; info_out[3] = i.min_pivot;
   return i.min_pivot > 0 ? 0 : 1;
 }

@@ -22,7 +22,7 @@ TMPC_BWD_REFACTOR_REFINE, TMPC_BWD_ADMM_REUSE_FACTOR = 0, 1
 TMPC_SOLVE_ZG_GIVEN = 1
 EXPORTS = ["tmpc_workspace_bytes", "tmpc_setup", "tmpc_linearize", "tmpc_factor", "tmpc_admm_solve", "tmpc_backward",
            "tmpc_kkt_solve", "tmpc_host_staging_bytes", "tmpc_admm_solve_host", "tmpc_destroy", "tmpc_status_string",
-           "tmpc_launch_count"]
+           "tmpc_launch_count", "tmpc_measure_peak"]
 
 
 class TmpcConfig(C.Structure):
@@ -74,6 +74,7 @@ def lib():
         L.tmpc_kkt_solve.argtypes = [C.c_void_p] * 3
         L.tmpc_admm_solve_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t]
         L.tmpc_destroy.argtypes = [C.c_void_p]
+        L.tmpc_measure_peak.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
         _LIB = L
     return _LIB
 
@@ -159,3 +160,12 @@ def tmpc_destroy(h):
 
 def tmpc_launch_count(h) -> int:
     return int(lib().tmpc_launch_count(h))
+
+
+TMPC_PEAK_FFMA2, TMPC_PEAK_FFMA, TMPC_PEAK_DFMA, TMPC_PEAK_LDS = 0, 1, 2, 3
+
+
+def tmpc_measure_peak(what: int, scratch_ptr: int, stream_ptr: int, reps: int = 5) -> float:
+    out = C.c_double()
+    _check(lib().tmpc_measure_peak(what, scratch_ptr, stream_ptr, reps, C.byref(out)), "tmpc_measure_peak")
+    return out.value

@@ -14,6 +14,7 @@
 #include "tmpc_backward.cuh"
 #include "tmpc_cr.cuh"
 #include "tmpc_cr2.cuh"
+#include "tmpc_peak.cuh"
 
 using namespace tmpc;
 
@@ -24,8 +25,17 @@ inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 inline size_t esize(int dtype) { return dtype == TMPC_F64 ? 8 : 4; }
 
 struct Layout {   // byte offsets into the workspace
-  size_t Lam, Sinv, eta, cls, soft_adj, rhs, w_rows, lo_adj, hi_adj, q_adj, ax, azg, ayf, ayg, axi, zero_xinit, zero_b, res, cr, total;
+  size_t Lam, Sinv, eta, fstatus, cls, soft_adj, rhs, w_rows, lo_adj, hi_adj, q_adj, ax, azg, ayf, ayg, axi, zero_xinit, zero_b, res, cr, total;
 };
+
+// Cyclic reduction (tmpc_cr.cuh) exists for n = 6 and n = 8 and pays off for a few very long horizons; TMPC_LIN_AUTO picks it
+// only there and keeps the sequential families for every other shape.
+bool use_cr(const tmpc_config& c) {
+  if (c.linsolve == TMPC_LIN_CYCLIC_REDUCTION) return true;
+  const int n = c.nx + c.nu;
+  if (c.linsolve == TMPC_LIN_AUTO) return c.batch <= 4 && c.N >= 1024 && (n == 6 || n == 8);
+  return false;
+}
 
 Dims make_dims(const tmpc_config& c) {
   Dims d; memset(&d, 0, sizeof(d));
@@ -40,12 +50,13 @@ Layout make_layout(const tmpc_config& c) {
   Layout L; size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
   L.Lam = take(B * d.T * nn * es); L.Sinv = take(B * d.T * nn * es); L.eta = take(B * d.nz * es);
+  L.fstatus = take(B * sizeof(int32_t));       // per-problem TMPC_ST_PIVOT word of the last tmpc_factor
   L.cls = take(B * d.mg); L.soft_adj = take(B * d.mg);
   L.rhs = take(B * d.nz * es); L.w_rows = take(B * d.mg * es); L.lo_adj = take(B * d.mg * es); L.hi_adj = take(B * d.mg * es);
   L.q_adj = take(B * d.nz * es); L.ax = take(B * d.nz * es); L.azg = take(B * d.mg * es); L.ayf = take(B * d.mf * es);
   L.ayg = take(B * d.mg * es); L.axi = take(B * d.mg * es); L.zero_xinit = take(B * d.nx * es); L.zero_b = take(B * (size_t)d.N * d.nx * es);
   L.res = take(B * 64 * 4 * sizeof(double));
-  L.cr = take(cr_workspace_bytes(d, es));
+  L.cr = take(use_cr(c) ? cr_workspace_bytes(d, es) : 0);   // cyclic-reduction scratch only for handles that use it
   L.total = o;
   return L;
 }
@@ -84,11 +95,6 @@ template <typename T> Params<T> params(const tmpc_config& c) {
 }
 inline bool cuda_ok() { return cudaGetLastError() == cudaSuccess; }
 
-bool use_cr(const tmpc_config& c) {
-  if (c.linsolve == TMPC_LIN_CYCLIC_REDUCTION) return true;
-  if (c.linsolve == TMPC_LIN_AUTO) return c.batch <= 4 && c.N >= 1024;
-  return false;
-}
 
 // ---- factor launch (a2 + a3)
 template <typename T>
@@ -263,14 +269,28 @@ tmpc_status launch_residual(tmpc_ctx* h, const AdmmArgs<T>& s) {
 template <typename T>
 tmpc_status do_factor(tmpc_ctx* h, const tmpc_qp* qp) {
   const double rho_f = h->cfg.rho_eq_scale * h->cfg.rho_bar, rho_g = h->cfg.rho_bar;
-  if (h->cr) return cr_factor<T>(h->d, view<T>(qp), h->cfg.sigma, rho_f, rho_g, h->ws + h->lay.cr, h->stream, &h->launches);
+  int32_t* fstatus = (int32_t*)(h->ws + h->lay.fstatus);
+  if (h->cr) {                           // the cyclic-reduction kernels keep their own per-problem pivot flag and OR it in themselves
+    if (cudaMemsetAsync(fstatus, 0, (size_t)h->d.B * sizeof(int32_t), h->stream) != cudaSuccess) return TMPC_E_CUDA;
+    return cr_factor<T>(h->d, view<T>(qp), h->cfg.sigma, rho_f, rho_g, h->ws + h->lay.cr, h->stream, &h->launches);
+  }
   h->twisted = fast_plan<T>(h->d).ok;
-  if (h->twisted) return launch_factor_tw<T>(h, qp, rho_f, rho_g, nullptr);
-  return launch_factor<T>(h, qp, rho_f, rho_g, nullptr, nullptr);
+  if (h->twisted) return launch_factor_tw<T>(h, qp, rho_f, rho_g, fstatus);
+  return launch_factor<T>(h, qp, rho_f, rho_g, nullptr, fstatus);
+}
+
+// info.status[b] <- pivot word of the last tmpc_factor (overwrites whatever the caller's buffer held); the solve kernels OR TMPC_ST_NAN in
+__global__ void status_init_kernel(int B, const int32_t* __restrict__ fstatus, int32_t* __restrict__ status) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < B) status[p] = fstatus[p];
 }
 
 template <typename T>
 tmpc_status do_solve(tmpc_ctx* h, const tmpc_qp* qp, tmpc_state* st, int iters, int flags, tmpc_info* info) {
+  if (info && info->status) {
+    status_init_kernel<<<(h->d.B + 255) / 256, 256, 0, h->stream>>>(h->d.B, (const int32_t*)(h->ws + h->lay.fstatus), info->status); h->launches++;
+    if (!cuda_ok()) return TMPC_E_CUDA;
+  }
   if (h->cr) {
     // chunked form (tmpc_cr2.cuh) when the horizon is long enough and one CTA per chunk (+1) is co-resident
     const Dims& d = h->d;
@@ -356,12 +376,19 @@ tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, vo
   // zero buffers of the adjoint QP (x_init = 0, b = 0)
   if (cudaMemsetAsync(h->ws + L.zero_xinit, 0, L.zero_b - L.zero_xinit, h->stream) != cudaSuccess ||
       cudaMemsetAsync(h->ws + L.zero_b, 0, L.cr - L.zero_b, h->stream) != cudaSuccess) { delete h; return TMPC_E_CUDA; }
-  {                                      // barrier words of the cyclic-reduction kernels (tmpc_cr.cuh GridBar) start at zero
+  if (h->cr) {                           // barrier words of the cyclic-reduction kernels (tmpc_cr.cuh GridBar) start at zero
     const size_t crb = cr_workspace_bytes(h->d, esize(cfg->dtype)), flags = 256 * (size_t)h->d.B + 1024;
     if (cudaMemsetAsync(h->ws + L.cr + crb - flags, 0, flags, h->stream) != cudaSuccess) { delete h; return TMPC_E_CUDA; }
   }
   *out = h;
   return TMPC_OK;
+}
+
+tmpc_status tmpc_measure_peak(int32_t what, void* scratch, void* cuda_stream, int32_t reps, double* out) {
+  if (what < 0 || what > 3 || !scratch || !out || reps < 1) return TMPC_E_BADARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return TMPC_E_CUDA; }
+  return measure_peak(what, (float*)scratch, (cudaStream_t)cuda_stream, reps, out);
 }
 
 tmpc_status tmpc_destroy(tmpc_handle h) { delete h; return TMPC_OK; }

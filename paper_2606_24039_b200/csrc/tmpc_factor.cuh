@@ -23,7 +23,7 @@ struct FactorArgs {
   double sigma, w_eq, w_in;     // weights: equality rows, inequality rows (scalar)
   const T* w_rows;              // optional per-inequality-row weights [B][T][ng] (overrides w_in), else null
   T* Lam; T* Sinv;              // outputs [B][N][n][n], [B][T][n][n]
-  int32_t* status;              // [B], bits OR-ed in (may be null)
+  int32_t* status;              // [B], written: TMPC_ST_PIVOT or 0 (may be null)
 };
 
 template <typename T, typename TA>
@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(1024) factor_kernel(FactorArgs<T> a) {
     }
     __syncthreads();
   }
-  if (a.status && tid == 0 && bad) atomicOr(&a.status[p], TMPC_ST_PIVOT);
+  if (a.status && tid == 0) a.status[p] = bad ? TMPC_ST_PIVOT : 0;
 }
 
 }  // namespace tmpc

@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
     x_out(m, Bm);
   }
   bad = __syncthreads_or(bad);
-  if (a.status && threadIdx.x == 0 && bad) atomicOr(&a.status[p], TMPC_ST_PIVOT);
+  if (a.status && threadIdx.x == 0) a.status[p] = bad ? TMPC_ST_PIVOT : 0;
 }
 
 }  // namespace tmpc

@@ -331,7 +331,7 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
   if (tid == 0 && p == 0) printf("f3 cycles: theta %lld chol+inv %lld - %lld xtx %lld phi %lld lam %lld\n", tk[0], tk[1], tk[2], tk[3], tk[4], tk[5]);
 #endif
   bad = __syncthreads_or(bad);
-  if (a.status && tid == 0 && bad) atomicOr(&a.status[p], TMPC_ST_PIVOT);
+  if (a.status && tid == 0) a.status[p] = bad ? TMPC_ST_PIVOT : 0;
 }
 
 }  // namespace tmpc

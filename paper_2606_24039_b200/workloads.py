@@ -385,3 +385,17 @@ def random_ltv(seed: int, B: int, N: int, nx: int, nu: int, ng_sel: list, soft: 
     hi = np.full((B, T, ng), bound)
     return QPData(f"random_ltv_nx{nx}_nu{nu}_N{N}", B, N, nx, nu, ng, "f64", D, E, qv, Am, Ap, -ck, x_init, G,
                   lo, hi, g_col=g_col, soft=list(soft), gamma=2.0, lam=0.0, iters=100)
+
+
+def with_dense_Ap(w: QPData, seed: int = 0, scale: float = 0.05) -> QPData:
+    """Copy of `w` whose A_t^+ blocks also depend on u_{t+1} (implicit integrators such as the trapezoidal rule,
+    PAPER.md:584-592 Remark A1 / eq. 36): the u-columns of Ap, zero in every BASELINE config, are filled with
+    scale * N(0,1) from a stream of its own (config id 10), so the instances without this call are unchanged."""
+    import copy
+
+    out = copy.copy(w)
+    st = Streams(seed, 10, np.arange(w.B))
+    out.Ap = w.Ap.copy()
+    out.Ap[:, :, :, w.nx:] = scale * st.normal(w.N * w.nx * w.nu).reshape(w.B, w.N, w.nx, w.nu)
+    out.name = w.name + "_denseAp"
+    return out

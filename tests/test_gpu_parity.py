@@ -281,7 +281,7 @@ def _sample(B, k=6, seed=7):
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
-def test_config2_full_batch_sampled(dtype):
+def test_config2_full_batch_every_problem(dtype):
     from paper_2606_24039_b200.solver import Solver
     w = W.config2()
     assert w.B == 1024 and w.N == 50 and w.iters == 100
@@ -290,13 +290,11 @@ def test_config2_full_batch_sampled(dtype):
     s.solve()
     got, info = s.state_numpy(), s.info_numpy()
     assert (info["status"] == 0).all() and all(np.isfinite(got[k]).all() for k in KEYS)
-    idx = _sample(w.B)
-    ws = wr.subset(idx)
-    ref, rinfo, rc = O.admm(ws, O.make_cfg(ws), nthreads=8)
+    ref, rinfo, rc = O.admm(wr, O.make_cfg(wr), nthreads=8)      # ALL 1024 problems: the oracle needs about a second for the batch
     assert rc == 0
-    compare_states({k: got[k][idx] for k in KEYS}, ref, TOL[dtype])
+    compare_states(got, ref, TOL[dtype])
     otol = 1e-4 if dtype == "f32" else 1e-9
-    assert (np.abs(info["objective"][idx] - rinfo[:, 2]) <= otol * np.maximum(np.abs(rinfo[:, 2]), 1.0)).all()
+    assert (np.abs(info["objective"] - rinfo[:, 2]) <= otol * np.maximum(np.abs(rinfo[:, 2]), 1.0)).all()
     s.close()
 
 
@@ -309,7 +307,8 @@ def test_config3_full_batch_sampled_fp32():
     s.solve()
     got, info = s.state_numpy(), s.info_numpy()
     assert (info["status"] == 0).all() and all(np.isfinite(got[k]).all() for k in KEYS)
-    idx = _sample(w.B, k=3)
+    idx = np.unique(np.concatenate([np.arange(8), np.random.default_rng(7).choice(np.arange(8, w.B), size=8, replace=False), [w.B - 1]]))   # O-7: first 8 + 8 seeded-random (+ the last)
+    assert len(idx) >= 16
     ws = wr.subset(idx)
     ref, rinfo, rc = O.admm(ws, O.make_cfg(ws, band=1), nthreads=8)
     assert rc == 0
@@ -349,3 +348,182 @@ def test_duplicate_selection_column_falls_back_fp64():
     w = W.random_ltv(77, 3, 11, 6, 2, [6, 6, 7], [0, 1, 0], q_scale=0.3)
     w.lo[..., 1] = -0.6; w.hi[..., 1] = 0.6          # a second, tighter (soft) bound on the same control
     run_pair(w, "f64", iters=60)
+
+
+# ----------------------------------------------------------------------------------------------- status bits (failure reporting)
+@pytest.mark.parametrize("family", ["resident_n8", "generic_n5", "dmma_n37"])
+def test_status_bits_indefinite_and_nan_problem(family):
+    """One indefinite problem (a D block made strongly negative: non-positive pivot) and one NaN problem (NaN in q) inside a batch:
+    exactly those two status words carry TMPC_ST_PIVOT / TMPC_ST_NAN — on every factor family (twisted warp-level, generic,
+    DMMA) —, the caller's status buffer is overwritten (pre-filled with garbage), and the other problems still match the oracle."""
+    import torch
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    if family == "resident_n8":
+        w, iters, band = W.config2(B=8, N=10), 40, None
+    elif family == "generic_n5":
+        w, iters, band = W.random_ltv(91, 8, 9, 3, 2, [3, 4], [0, 0], implicit=True, q_scale=0.3), 40, None
+    else:
+        w, iters, band = W.random_ltv(92, 4, 4, 30, 7, [30, 33, 36], [0, 0, 1], implicit=True, q_scale=0.3), 30, 1
+    bad_piv, bad_nan = 2, w.B - 1
+    w.D = np.repeat(w.D, w.B, axis=0).copy() if w.D.shape[0] == 1 else w.D.copy()
+    w.D[bad_piv, min(3, w.N)] = -500.0 * np.eye(w.n)
+    w.q = w.q.copy(); w.q[bad_nan, 1, 0] = np.nan
+    s = Solver(w, dtype="f64")
+    s.info["status"].fill_(0x7f00)                      # stale garbage in the caller's buffer
+    s.solve(iters)
+    got, info = s.state_numpy(), s.info_numpy()
+    st = info["status"]
+    good = np.array([b for b in range(w.B) if b not in (bad_piv, bad_nan)])
+    assert (st[good] == 0).all(), st
+    assert st[bad_piv] & Bd_ST_PIVOT and st[bad_nan] & Bd_ST_NAN and not (st[bad_nan] & Bd_ST_PIVOT), st
+    ws = w.subset(good)
+    ref, rinfo, rc = O.admm(ws, O.make_cfg(ws, band=band), iters=iters, nthreads=4)
+    assert rc == 0
+    compare_states({k: got[k][good] for k in KEYS}, ref, 1e-9)
+    # a second factor + solve with repaired data clears the bits (the word is rewritten by every tmpc_factor / tmpc_admm_solve)
+    w2 = w.subset(np.arange(w.B)); w2.D[bad_piv] = w.D[0]; w2.q[bad_nan, 1, 0] = 0.0
+    s.upload(w2); s.reset_state(); s.solve(iters)
+    assert (s.info_numpy()["status"] == 0).all()
+    s.close()
+
+
+Bd_ST_PIVOT, Bd_ST_NAN = 1, 2
+
+
+# ----------------------------------------------------------------------------------------------- general A^+ (u_{t+1} columns)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_dense_Ap_every_kernel_family(dtype):
+    """A_t^+ with non-zero u_{t+1} columns (implicit integrators, PAPER.md:584-592 Remark A1 / eq. 36): resident fast shapes
+    (8/6 and 6/4), ragged generic sizes, the DMMA factor + streamed class shape and cyclic reduction."""
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    run_pair(W.with_dense_Ap(W.config2(B=5, N=13, soft_bound=0.5), seed=1, scale=0.02), dtype, iters=60)
+    run_pair(W.with_dense_Ap(W.random_ltv(81, 3, 11, 4, 2, [4, 5, 0], [0, 0, 1], implicit=True, q_scale=0.3), seed=2), dtype, iters=60)
+    run_pair(W.with_dense_Ap(W.random_ltv(82, 3, 9, 3, 2, [3, 4], [0, 0, 1], implicit=True, dense_g_rows=1, q_scale=0.3), seed=3), dtype, iters=60)
+    run_pair(W.with_dense_Ap(W.config3(B=2, N=4), seed=4, scale=0.02), dtype, iters=30, band=1)
+    if dtype == "f64":
+        w = W.with_dense_Ap(W.random_ltv(83, 2, 70, 4, 2, [4, 5], [0, 0, 1], implicit=True, dense_g_rows=1, q_scale=0.3), seed=5)
+        s = Solver(w, dtype="f64", linsolve=Bd.TMPC_LIN_CYCLIC_REDUCTION)
+        s.solve(60)
+        ref, rinfo, rc = O.admm(w, O.make_cfg(w), iters=60)
+        compare_states(s.state_numpy(), ref, 1e-9)
+        s.close()
+
+
+# ----------------------------------------------------------------------------------------------- TMPC_LIN_AUTO
+def test_linsolve_auto_picks_a_path_that_exists():
+    """AUTO takes cyclic reduction for a single long horizon of a supported block size (n = 6) and must fall back to the
+    sequential families for a block size the cyclic-reduction kernels do not have (n = 3) instead of failing."""
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    for w in (W.random_ltv(84, 1, 1100, 4, 2, [4, 5], [0, 0], implicit=True, q_scale=0.3), W.random_ltv(85, 1, 1030, 2, 1, [2], [0], implicit=True, q_scale=0.3)):
+        s = Solver(w, dtype="f64", linsolve=Bd.TMPC_LIN_AUTO)
+        s.solve(40)
+        ref, rinfo, rc = O.admm(w, O.make_cfg(w, band=1), iters=40)
+        compare_states(s.state_numpy(), ref, 1e-9)
+        s.close()
+
+
+# ----------------------------------------------------------------------------------------------- backward: bench shape, dL/dxi, same-K reuse mode
+def _gpu_backward(s, ref, dLdx, dLdxi, mode, iters=None):
+    import torch
+    up = lambda a: None if a is None else s._up(a)
+    s.set_state(ref)
+    dq, dxi = s.backward(up(dLdx), up(dLdxi), mode=mode, iters=iters)
+    return dq.cpu().double().numpy(), dxi.cpu().double().numpy()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_backward_at_bench_shape(dtype):
+    """The launch shape bench.py times (B = 1024, N = 50, config 2), fed the oracle's K = 100 state (reading A-20): REFINE mode
+    against the definition on 64 sampled problems (the oracle's dense Gauss of a ~750^2 system takes ~0.3 s per problem, so the
+    full batch would take minutes), and the eq. 67 mode against the oracle's Alg. 3 on the numpy-built adjoint QP at the SAME K
+    on 16 of them."""
+    from adjoint_util import adjoint_qp
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    w = W.config2()
+    wr = w.rounded(np.float32) if dtype == "f32" else w
+    eps = 1e-8 if dtype == "f64" else 1e-4
+    cfg = O.make_cfg(wr, eps_abs=eps, eps_rel=eps)
+    ref, info, rc = O.admm(wr, cfg, nthreads=8)
+    if dtype == "f32":
+        ref = {k: v.astype(np.float32).astype(np.float64) for k, v in ref.items()}
+    s = Solver(wr, dtype=dtype)
+    dq, dxi = _gpu_backward(s, ref, 2.0 * ref["x"], None, Bd.TMPC_BWD_REFACTOR_REFINE)
+    assert np.isfinite(dq).all() and np.isfinite(dxi).all()
+    idx = np.unique(np.concatenate([np.arange(8), np.random.default_rng(11).choice(np.arange(8, w.B), size=56, replace=False)]))
+    ws = wr.subset(idx); rs = {k: v[idx] for k, v in ref.items()}
+    dq_o, dxi_o, counts, rcs = O.backward(ws, cfg, rs, 2.0 * rs["x"])
+    ok = rcs == 0
+    assert ok.sum() >= len(idx) // 2 and counts[ok, 0].sum() > 0
+    tol = 1e-9 if dtype == "f64" else 2e-3
+    assert rel_err(dq[idx][ok], dq_o[ok]) <= tol and rel_err(dxi[idx][ok], dxi_o[ok]) <= tol
+    # eq. 67 mode at the same K
+    K = 100
+    s.factor()
+    dq2, dxi2 = _gpu_backward(s, ref, 2.0 * ref["x"], None, Bd.TMPC_BWD_ADMM_REUSE_FACTOR, iters=K)
+    idx2 = idx[:16]
+    ws2 = wr.subset(idx2); rs2 = {k: v[idx2] for k, v in ref.items()}
+    wa, soft_rows, cls = adjoint_qp(ws2, cfg, rs2, 2.0 * rs2["x"])
+    sa, ia, rca = O.admm_rows(wa, O.make_cfg(wa), soft_rows, K)
+    assert rca == 0
+    assert rel_err(dq2[idx2], -sa["x"]) <= tol and rel_err(dxi2[idx2], sa["yf"][:, :w.nx]) <= tol
+    s.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_backward_with_dLdxi_and_dead_zone_rows(dtype):
+    """L = |x|^2 + 3 |xi|^2 on an instance with soft-active rows AND soft rows in the L1 dead zone (classed hard-active):
+    REFINE against the definition, the eq. 67 mode against the oracle's Alg. 3 on the adjoint QP at the same K (1e-9 / 2e-3)."""
+    from adjoint_util import adjoint_qp
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    w = W.config2(B=6, N=20, soft_bound=0.4)
+    w.rho_bar, w.lam = 2.0, 2.0
+    w.q = w.q + 0.3 * np.random.default_rng(5).standard_normal(w.q.shape)
+    wr = w.rounded(np.float32) if dtype == "f32" else w
+    eps = 1e-8 if dtype == "f64" else 1e-4
+    cfg = O.make_cfg(wr, eps_abs=eps, eps_rel=eps)
+    ref, info, rc = O.admm(wr, cfg, iters=3000)
+    if dtype == "f32":
+        ref = {k: v.astype(np.float32).astype(np.float64) for k, v in ref.items()}
+    dLdx, dLdxi = 2.0 * ref["x"], 6.0 * ref["xi"]
+    dq_o, dxi_o, counts, rcs = O.backward(wr, cfg, ref, dLdx, dLdxi)
+    ok = rcs == 0
+    assert ok.sum() >= 3 and counts[ok, 1].sum() > 0
+    cls = np.stack([O.classify(wr, cfg, ref, b) for b in range(w.B)])
+    soft = np.array(w.soft, dtype=bool)
+    assert (cls[:, :, soft] == 1).sum() > 0, "instance must hold dead-zone rows"
+    dq0, _, _, _ = O.backward(wr, cfg, ref, dLdx, None)
+    assert np.abs(dq0 - dq_o)[ok].max() > 1e-2 * np.abs(dq_o[ok]).max(), "the dL/dxi term must matter"
+    s = Solver(wr, dtype=dtype, eps_abs=eps, eps_rel=eps)
+    tol = 1e-9 if dtype == "f64" else 2e-3
+    dq, dxi = _gpu_backward(s, ref, dLdx, dLdxi, Bd.TMPC_BWD_REFACTOR_REFINE)
+    assert rel_err(dq[ok], dq_o[ok]) <= tol and rel_err(dxi[ok], dxi_o[ok]) <= tol
+    K = 300
+    s.factor()
+    dq2, dxi2 = _gpu_backward(s, ref, dLdx, dLdxi, Bd.TMPC_BWD_ADMM_REUSE_FACTOR, iters=K)
+    wa, soft_rows, _ = adjoint_qp(wr, cfg, ref, dLdx, dLdxi)
+    sa, ia, rca = O.admm_rows(wa, O.make_cfg(wa), soft_rows, K)
+    assert rel_err(dq2, -sa["x"]) <= tol and rel_err(dxi2, sa["yf"][:, :w.nx]) <= tol
+    s.close()
+
+
+def test_backward_dense_Ap_fp64():
+    """REFINE backward on a problem whose A^+ has u_{t+1} columns."""
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    w = W.with_dense_Ap(W.config2(B=4, N=12, soft_bound=0.4), seed=6, scale=0.02)
+    w.rho_bar, w.lam = 2.0, 0.05
+    w.q = w.q + 0.3 * np.random.default_rng(5).standard_normal(w.q.shape)
+    cfg = O.make_cfg(w)
+    ref, info, rc = O.admm(w, cfg, iters=3000)
+    dq_o, dxi_o, counts, rcs = O.backward(w, cfg, ref, 2.0 * ref["x"])
+    ok = rcs == 0
+    assert ok.sum() >= 2
+    s = Solver(w, dtype="f64")
+    dq, dxi = _gpu_backward(s, ref, 2.0 * ref["x"], None, Bd.TMPC_BWD_REFACTOR_REFINE)
+    assert rel_err(dq[ok], dq_o[ok]) <= 1e-9 and rel_err(dxi[ok], dxi_o[ok]) <= 1e-9
+    s.close()

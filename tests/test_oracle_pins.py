@@ -41,6 +41,7 @@ def small_family():
         W.random_ltv(1, 2, 5, 3, 2, [3, 4], [0, 0], implicit=True),
         W.random_ltv(2, 2, 4, 2, 1, [2, 0, 1], [0, 1, 1, 1], implicit=False, dense_g_rows=1),
         W.config2(B=2, N=6),
+        W.with_dense_Ap(W.random_ltv(4, 2, 5, 3, 2, [3, 4], [0, 0], implicit=True), seed=1, scale=0.3),   # A^+ with u_{t+1} columns (Remark A1)
     ]
 
 
@@ -316,6 +317,7 @@ def test_iterates_equal_kkt_form_of_eq7_every_iteration(sigma, alpha):
     equality rows treated like any other row (z_f is projected onto [c, c]) — with a LARGE sigma so that the relaxation of x
     (eq. 10-11) is visible in eta, and alpha != 1 so that its placement in both dual updates matters."""
     w = W.random_ltv(5, 1, 4, 3, 2, [3, 4, 0], [0, 0, 1], bound=0.3, implicit=True, dense_g_rows=1, q_scale=0.6)
+    w = W.with_dense_Ap(w, seed=2, scale=0.3)                                          # general A^+ (u_{t+1} columns, Remark A1)
     w.soft = [0, 0, 1, 1]; w.lam = 0.05; w.sigma = sigma; w.alpha = alpha; w.rho_bar = 0.7; w.rho_eq_scale = 13.0
     P, C, c, G = dense_PCG(w, 0)
     A = np.vstack([C, G]); mf = C.shape[0]
@@ -451,6 +453,28 @@ def test_classification_rule_hand_built_states():
     w.lo[0, 3, 4] = -np.inf; x[3, col[4]] = -7.0; expect[3, 4] = 0               # an infinite bound is never "near"
     got = O.classify(w, cfg, st, 0)
     assert (got == expect).all(), (got, expect)
+
+
+def test_adjoint_qp_of_eq67_converges_to_the_definition():
+    """eq. 67: Alg. 3 on the adjoint QP (tests/adjoint_util.py, numpy) converges to the solution of the
+    active-set system eq. 65 that backward() solves directly; per-row soft flags == per-type mask when they coincide."""
+    from adjoint_util import adjoint_qp
+    w = W.config2(B=2, N=8, soft_bound=0.4)
+    w.lam, w.rho_bar = 2.0, 2.0
+    w.q = w.q + 0.3 * np.random.default_rng(5).standard_normal(w.q.shape)
+    cfg = O.make_cfg(w)
+    st, info, rc = O.admm(w, cfg, iters=30000)
+    dLdxi = 6.0 * st["xi"]
+    dq, dxi, counts, rcs = O.backward(w, cfg, st, 2.0 * st["x"], dLdxi)
+    assert (rcs == 0).all() and counts[:, 1].min() > 0 and counts[:, 0].min() > 0
+    wa, soft_rows, cls = adjoint_qp(w, cfg, st, 2.0 * st["x"], dLdxi)
+    sa, ia, rca = O.admm_rows(wa, O.make_cfg(wa), soft_rows, 60000)
+    assert rca == 0
+    assert np.abs(-sa["x"] - dq).max() <= 1e-8 * max(1.0, np.abs(dq).max())
+    assert np.abs(sa["yf"][:, :w.nx] - dxi).max() <= 1e-8 * max(1.0, np.abs(dxi).max())
+    sr = np.tile(np.array(w.soft, np.uint8), (w.B, w.T, 1))
+    a, _, _ = O.admm(w, cfg, iters=40); b, _, _ = O.admm_rows(w, cfg, sr, 40)
+    assert all((a[k] == b[k]).all() for k in a)
 
 
 def test_backward_unconstrained_closed_form():
