@@ -9,6 +9,7 @@
 #include "tmpc_factor3.cuh"
 #include "tmpc_admm.cuh"
 #include "tmpc_admm2.cuh"
+#include "tmpc_admm3.cuh"
 #include "tmpc_stream.cuh"
 #include "tmpc_misc.cuh"
 #include "tmpc_backward.cuh"
@@ -131,7 +132,7 @@ tmpc_status launch_admm_inst(tmpc_ctx* h, const AdmmArgs<T>& a, int nt, size_t s
   k<<<h->d.B, nt, smem, h->stream>>>(a); h->launches++;
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
 }
-struct FastPlan { bool ok; int pg, nt, ctas_per_sm; size_t smem; };
+struct FastPlan { bool ok, v3; int pg, nt, ctas_per_sm; size_t smem; };   // v3: tmpc_admm3.cuh (n = 8), else tmpc_admm2.cuh (n = 6)
 template <typename T> FastPlan fast_plan(const Dims& d);
 template <typename T> tmpc_status launch_admm2(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f);
 template <typename T> tmpc_status launch_residual(tmpc_ctx* h, const AdmmArgs<T>& s);
@@ -201,13 +202,14 @@ FastPlan fast_plan(const Dims& d) {
   const bool shape = (d.n == 8 && d.nx == 6) || (d.n == 6 && d.nx == 4);
   if (!shape || d.ng > d.n || d.T < 2) return f;
   if (d.g_sel) for (int r = 0; r < d.ng; ++r) for (int q = 0; q < r; ++q) if (d.g_col[r] == d.g_col[q]) return f;   // one selection row per column
-  const size_t s1 = d.n == 8 ? admm2_smem_bytes<T, 8, 6>(d, 1) : admm2_smem_bytes<T, 6, 4>(d, 1), s2 = d.n == 8 ? admm2_smem_bytes<T, 8, 6>(d, 2) : admm2_smem_bytes<T, 6, 4>(d, 2);
+  f.v3 = d.n == 8;
+  const size_t s1 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 1) : admm2_smem_bytes<T, 6, 4>(d, 1), s2 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 2) : admm2_smem_bytes<T, 6, 4>(d, 2);
   if (s1 > kMaxSmem) return f;
   const int c1 = (int)(kSmemPerSM / (s1 + 1024)), c2 = s2 <= kMaxSmem ? (int)(kSmemPerSM / (s2 + 1024)) : 0;
   f.pg = (d.B >= 2 && c2 >= 2 && 2 * c2 >= c1) ? 2 : 1;
-  const int ipt = d.n == 8 ? admm2_ipt<T, 8>() : admm2_ipt<T, 6>();
+  const int ipt = d.n == 8 ? 4 : admm2_ipt<T, 6>();      // rows of a stage per item thread (admm3: two lanes per stage)
   auto threads = [&](int pg) { int t = ((pg * d.nz + ipt - 1) / ipt + 31) / 32 * 32; return 32 + (t < 32 ? 32 : t); };   // + the chain warp
-  const int tmax = sizeof(T) == 8 ? 512 : 1024;
+  const int tmax = (sizeof(T) == 8 && !f.v3) ? 512 : 1024;
   if (threads(f.pg) > tmax) f.pg = 1;
   f.nt = threads(f.pg);
   if (f.nt > tmax) return f;
@@ -235,9 +237,28 @@ tmpc_status launch_admm2_shape(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan
     return launch_admm2_inst<T, NC, NX, PG, 1024, 1>(h, a, f);
   }
 }
+template <typename T, int NC, int NX, int PG, int MAXT, int MINB>
+tmpc_status launch_admm3_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
+  auto k = admm3_kernel<T, NC, NX, PG, MAXT, MINB>;
+  if (f.smem > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem) != cudaSuccess) return TMPC_E_CUDA;
+  const unsigned grid = (unsigned)((h->d.B + PG - 1) / PG);
+  Admm3Args<T> A; A.a = a; A.pl = admm3_plan<T, NC, NX>(h->d, PG);
+  A.rfa = a.prm.rho_f * a.prm.alpha; A.oma = T(1) - a.prm.alpha; A.inv_rho_g = T(1) / a.prm.rho_g; A.inv_rg = T(1) / (a.prm.rho_g + a.prm.gamma);
+  k<<<grid, f.nt, f.smem, h->stream>>>(A); h->launches++;
+  return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+}
+template <typename T, int NC, int NX, int PG>
+tmpc_status launch_admm3_shape(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
+  if (f.nt <= 256) {
+    if (f.ctas_per_sm >= 2) return launch_admm3_inst<T, NC, NX, PG, 256, 2>(h, a, f);
+    return launch_admm3_inst<T, NC, NX, PG, 256, 1>(h, a, f);
+  }
+  return launch_admm3_inst<T, NC, NX, PG, 1024, 1>(h, a, f);
+}
 template <typename T>
 tmpc_status launch_admm2(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
   const Dims& d = h->d;
+  if (f.v3) return f.pg == 2 ? launch_admm3_shape<T, 8, 6, 2>(h, a, f) : launch_admm3_shape<T, 8, 6, 1>(h, a, f);
   if (d.n == 8 && d.nx == 6) return f.pg == 2 ? launch_admm2_shape<T, 8, 6, 2>(h, a, f) : launch_admm2_shape<T, 8, 6, 1>(h, a, f);
   if (d.n == 6 && d.nx == 4) return f.pg == 2 ? launch_admm2_shape<T, 6, 4, 2>(h, a, f) : launch_admm2_shape<T, 6, 4, 1>(h, a, f);
   return TMPC_E_UNSUPPORTED;
