@@ -202,14 +202,14 @@ FastPlan fast_plan(const Dims& d) {
   const bool shape = (d.n == 8 && d.nx == 6) || (d.n == 6 && d.nx == 4);
   if (!shape || d.ng > d.n || d.T < 2) return f;
   if (d.g_sel) for (int r = 0; r < d.ng; ++r) for (int q = 0; q < r; ++q) if (d.g_col[r] == d.g_col[q]) return f;   // one selection row per column
-  f.v3 = d.n == 8;
-  const size_t s1 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 1) : admm2_smem_bytes<T, 6, 4>(d, 1), s2 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 2) : admm2_smem_bytes<T, 6, 4>(d, 2);
+  f.v3 = true;
+  const size_t s1 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 1) : admm3_smem_bytes<T, 6, 4>(d, 1), s2 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 2) : admm3_smem_bytes<T, 6, 4>(d, 2);
   if (s1 > kMaxSmem) return f;
   const int c1 = (int)(kSmemPerSM / (s1 + 1024)), c2 = s2 <= kMaxSmem ? (int)(kSmemPerSM / (s2 + 1024)) : 0;
   f.pg = (d.B >= 2 && c2 >= 2 && 2 * c2 >= c1) ? 2 : 1;
-  const int ipt = d.n == 8 ? 4 : admm2_ipt<T, 6>();      // rows of a stage per item thread (admm3: two lanes per stage)
+  const int ipt = d.n / 2;                                 // rows of a stage per item thread (admm3: two lanes per stage)
   auto threads = [&](int pg) { int t = ((pg * d.nz + ipt - 1) / ipt + 31) / 32 * 32; return 32 + (t < 32 ? 32 : t); };   // + the chain warp
-  const int tmax = (sizeof(T) == 8 && !f.v3) ? 512 : 1024;
+  const int tmax = 1024;
   if (threads(f.pg) > tmax) f.pg = 1;
   f.nt = threads(f.pg);
   if (f.nt > tmax) return f;
@@ -250,6 +250,7 @@ tmpc_status launch_admm3_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan&
 template <typename T, int NC, int NX, int PG>
 tmpc_status launch_admm3_shape(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
   if (f.nt <= 256) {
+    if (f.ctas_per_sm >= 3) return launch_admm3_inst<T, NC, NX, PG, 256, 3>(h, a, f);
     if (f.ctas_per_sm >= 2) return launch_admm3_inst<T, NC, NX, PG, 256, 2>(h, a, f);
     return launch_admm3_inst<T, NC, NX, PG, 256, 1>(h, a, f);
   }
@@ -258,7 +259,8 @@ tmpc_status launch_admm3_shape(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan
 template <typename T>
 tmpc_status launch_admm2(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
   const Dims& d = h->d;
-  if (f.v3) return f.pg == 2 ? launch_admm3_shape<T, 8, 6, 2>(h, a, f) : launch_admm3_shape<T, 8, 6, 1>(h, a, f);
+  if (f.v3 && d.n == 8) return f.pg == 2 ? launch_admm3_shape<T, 8, 6, 2>(h, a, f) : launch_admm3_shape<T, 8, 6, 1>(h, a, f);
+  if (f.v3 && d.n == 6) return f.pg == 2 ? launch_admm3_shape<T, 6, 4, 2>(h, a, f) : launch_admm3_shape<T, 6, 4, 1>(h, a, f);
   if (d.n == 8 && d.nx == 6) return f.pg == 2 ? launch_admm2_shape<T, 8, 6, 2>(h, a, f) : launch_admm2_shape<T, 8, 6, 1>(h, a, f);
   if (d.n == 6 && d.nx == 4) return f.pg == 2 ? launch_admm2_shape<T, 6, 4, 2>(h, a, f) : launch_admm2_shape<T, 6, 4, 1>(h, a, f);
   return TMPC_E_UNSUPPORTED;
