@@ -154,6 +154,35 @@ def admm_rows(w, cfg, soft_rows, iters, state=None):
     return st, info, rc
 
 
+class Adaptive(C.Structure):
+    _fields_ = [("max_iters", C.c_int32), ("check_every", C.c_int32), ("adapt_rho", C.c_int32), ("pad", C.c_int32),
+                ("eps_abs", C.c_double), ("eps_rel", C.c_double), ("ratio", C.c_double), ("rho_min", C.c_double), ("rho_max", C.c_double)]
+
+
+def make_adaptive(max_iters, eps_abs=1e-3, eps_rel=1e-3, check_every=25, ratio=5.0, rho_min=1e-6, rho_max=1e6, adapt_rho=1) -> Adaptive:
+    """Defaults of PAPER.md:303 (k_rho^iter = 25, k_rho^ratio = 5, rho_bar in [1e-6, 1e6])."""
+    return Adaptive(max_iters, check_every, adapt_rho, 0, eps_abs, eps_rel, ratio, rho_min, rho_max)
+
+
+def admm_adaptive(w, cfg, ad, state=None, max_log=256):
+    """f1 on every problem.  Returns (state, info [B,8] = r_prim, r_dual, objective, min pivot, iterations, final rho_bar, converged,
+    #log rows, log [B,max_log,8] = k, r_prim, r_dual, np, nd, rho before, rho after, converged, rc)."""
+    n, T, nz, mf, mg = _dims(w)
+    assert lib().orc_sizeof_adaptive() == C.sizeof(Adaptive)
+    st = new_state(w) if state is None else {k: _c(v).copy() for k, v in state.items()}
+    info = np.zeros((w.B, 8)); log = np.zeros((w.B, max_log, 8))
+    f = lib().orc_admm_adaptive
+    f.argtypes = [C.c_void_p] * 19 + [C.c_int]
+    rc = 0
+    for b in range(w.B):
+        D, E = _c(_bs(w.D, b)), _c(_bs(w.E, b))
+        G = None if cfg.g_sel else _c(_bs(w.G, b))
+        rc |= f(C.byref(cfg), C.byref(ad), _p(D), _p(E), _p(_c(w.q[b])), _p(_c(w.Am[b])), _p(_c(w.Ap[b])), _p(_c(w.b[b])), _p(_c(w.x_init[b])), _p(G),
+                _p(_c(w.lo[b])), _p(_c(w.hi[b])), _p(st["x"][b]), _p(st["zg"][b]), _p(st["yf"][b]), _p(st["yg"][b]), _p(st["xi"][b]),
+                _p(info[b]), _p(log[b]), max_log)
+    return st, info, log, rc
+
+
 def backward(w, cfg, state, dLdx, dLdxi=None):
     """O-5 on every problem.  Returns dq [B,T,n], dxinit [B,nx], counts [B,2], rc [B]."""
     n, T, nz, mf, mg = _dims(w)

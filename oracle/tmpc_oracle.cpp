@@ -17,6 +17,7 @@
 //   O-3  ADMM       Alg. 3 with eq. 8-16, 42-45, 51, in the paper's order.
 //   O-4  SQP        fixed-count full-step driver around O-1..O-3 with the bicycle model linearised
 //                   by eq. 36-38.
+//   f1   adaptive   Alg. 3 with the adaptive step size of eq. 17 and the termination test eq. 4 (admm_adaptive).
 //   O-5  backward   the definition: dense active-set KKT system eq. 62 / 65 solved by
 //                   Gaussian elimination with partial pivoting; dL/dq = -eta_x, dL/dx_init = +eta_f[0:nx].
 //
@@ -216,6 +217,87 @@ Info admm(const Cfg& cf, const QP& p, double* x_, double* zg_, double* yf_, doub
   std::copy(x.begin(), x.end(), x_); std::copy(zg.begin(), zg.end(), zg_); std::copy(yf.begin(), yf.end(), yf_);
   std::copy(yg.begin(), yg.end(), yg_); std::copy(xi.begin(), xi.end(), xi_);
   return info;
+}
+
+// f1: Alg. 3 with the paper's adaptive step size and termination test.
+//   * every `check_every` (k_rho^iter: 25) iterations, and at iteration K_max, the residuals (eq. 3) and the
+//     scales of eq. 4 are evaluated:  np = |(Ax, z)|_inf with A = [C; G], z = (c, z_g);
+//     nd = |(Px, A'y, q, gamma xi, y_g on soft rows)|_inf   (reading A-32: the test is run at the
+//     rho schedule's cadence, not after every iteration);
+//   * converged  <=>  r_prim <= eps_abs + eps_rel np  and  r_dual <= eps_abs + eps_rel nd   (eq. 4)  ->  stop;
+//   * otherwise (eq. 17):  rho_new = clip(rho_bar sqrt((r_prim/np) / (r_dual/nd)), [rho_min, rho_max]),
+//     accepted iff max(rho_new/rho_bar, rho_bar/rho_new) > ratio; on acceptance S is re-assembled with the new rho and
+//     re-factorised; x, z, y are kept.  A zero denominator (r_dual, np or nd = 0) skips the update.
+// log_out (optional, 8 doubles per check): k, r_prim, r_dual, np, nd, rho before, rho after, converged.
+struct Adaptive { int32_t max_iters, check_every, adapt_rho, pad; double eps_abs, eps_rel, ratio, rho_min, rho_max; };
+
+int admm_adaptive(const Cfg& cf, const QP& p, const Adaptive& ad, double* x_, double* zg_, double* yf_, double* yg_, double* xi_, double* info_out,
+                  double* log_out, int max_log) {
+  const double sigma = cf.sigma, alpha = cf.alpha;
+  double rho_bar = cf.rho_bar;
+  vec x(x_, x_ + p.nz), zg(p.mg), yf(yf_, yf_ + p.mf), yg(yg_, yg_ + p.mg), xi(p.mg, 0.0), tmp(p.mg);
+  if (cf.zg_given) { zg.assign(zg_, zg_ + p.mg); xi.assign(xi_, xi_ + p.mg); }
+  else { p.G.mul(x, tmp); for (int i = 0; i < p.mg; ++i) zg[i] = clip(tmp[i], p.lo[i], p.hi[i]); }
+  double rho_g = rho_bar, rho_f = cf.rho_eq_scale * rho_bar;
+  Band L = build_S(p, sigma, vec(p.mf, rho_f), vec(p.mg, rho_g));
+  double minpiv = cholesky(L);
+  vec eta(p.nz), xt(p.nz), ztf(p.mf), ztg(p.mg), rf(p.mf), rg(p.mg), g(p.nz), Px(p.nz), Aty(p.nz);
+  int k = 0, nlog = 0, converged = 0;
+  double rp = 0, rd = 0, obj = 0;
+  while (k < ad.max_iters && !converged) {
+    for (int i = 0; i < p.nz; ++i) eta[i] = sigma * x[i] - p.q[i];
+    for (int i = 0; i < p.mf; ++i) rf[i] = rho_f * p.c[i] - yf[i];
+    for (int i = 0; i < p.mg; ++i) rg[i] = rho_g * zg[i] - yg[i];
+    p.C.mulT_add(rf, eta); p.G.mulT_add(rg, eta);
+    xt = eta; chol_solve(L, xt); p.C.mul(xt, ztf); p.G.mul(xt, ztg);
+    for (int i = 0; i < p.nz; ++i) x[i] = alpha * xt[i] + (1.0 - alpha) * x[i];
+    for (int i = 0; i < p.mg; ++i) {
+      double zh = alpha * ztg[i] + (1.0 - alpha) * zg[i];
+      double v = zh + yg[i] / rho_g, z, s;
+      project_row(cf.soft[i % p.ng] != 0, v, p.lo[i], p.hi[i], rho_g, cf.gamma, cf.lam, z, s);
+      zg[i] = z; xi[i] = s; yg[i] = yg[i] + rho_g * (zh - z);
+    }
+    for (int i = 0; i < p.mf; ++i) yf[i] = yf[i] + rho_f * alpha * (ztf[i] - p.c[i]);
+    ++k;
+    if (k % ad.check_every != 0 && k != ad.max_iters) continue;
+    // residuals (eq. 3) and the scales of eq. 4
+    p.C.mul(x, ztf); p.G.mul(x, ztg);
+    rp = 0; double np_ = 0;
+    for (int i = 0; i < p.mf; ++i) { rp = std::max(rp, std::fabs(ztf[i] - p.c[i])); np_ = std::max(np_, std::max(std::fabs(ztf[i]), std::fabs(p.c[i]))); }
+    for (int i = 0; i < p.mg; ++i) { rp = std::max(rp, std::fabs(ztg[i] - zg[i])); np_ = std::max(np_, std::max(std::fabs(ztg[i]), std::fabs(zg[i]))); }
+    band_mul(p.P, x, Px);
+    std::fill(Aty.begin(), Aty.end(), 0.0); p.C.mulT_add(yf, Aty); p.G.mulT_add(yg, Aty);
+    rd = 0; double nd_ = 0; obj = 0;
+    for (int i = 0; i < p.nz; ++i) {
+      rd = std::max(rd, std::fabs(Px[i] + p.q[i] + Aty[i]));
+      nd_ = std::max(nd_, std::max(std::fabs(Px[i]), std::max(std::fabs(Aty[i]), std::fabs(p.q[i]))));
+      obj += 0.5 * x[i] * Px[i] + p.q[i] * x[i];
+    }
+    for (int i = 0; i < p.mg; ++i) if (cf.soft[i % p.ng]) {
+      nd_ = std::max(nd_, std::max(std::fabs(cf.gamma * xi[i]), std::fabs(yg[i])));
+      if (xi[i] != 0.0) {
+        double sg = xi[i] > 0 ? 1.0 : -1.0;
+        rd = std::max(rd, std::fabs(cf.gamma * xi[i] + cf.lam * sg + yg[i]));
+        obj += cf.lam * std::fabs(xi[i]) + 0.5 * cf.gamma * xi[i] * xi[i];
+      }
+    }
+    converged = (rp <= ad.eps_abs + ad.eps_rel * np_) && (rd <= ad.eps_abs + ad.eps_rel * nd_);
+    const double rho_before = rho_bar;
+    if (!converged && ad.adapt_rho && k % ad.check_every == 0 && k < ad.max_iters && rd > 0.0 && np_ > 0.0 && nd_ > 0.0) {
+      double cand = rho_bar * std::sqrt((rp / np_) / (rd / nd_));
+      cand = std::min(std::max(cand, ad.rho_min), ad.rho_max);
+      if (std::max(cand / rho_bar, rho_bar / cand) > ad.ratio) {
+        rho_bar = cand; rho_g = rho_bar; rho_f = cf.rho_eq_scale * rho_bar;
+        L = build_S(p, sigma, vec(p.mf, rho_f), vec(p.mg, rho_g));
+        minpiv = std::min(minpiv, cholesky(L));
+      }
+    }
+    if (log_out && nlog < max_log) { double* l = log_out + 8 * nlog++; l[0] = k; l[1] = rp; l[2] = rd; l[3] = np_; l[4] = nd_; l[5] = rho_before; l[6] = rho_bar; l[7] = converged; }
+  }
+  info_out[0] = rp; info_out[1] = rd; info_out[2] = obj; info_out[3] = minpiv; info_out[4] = k; info_out[5] = rho_bar; info_out[6] = converged; info_out[7] = nlog;
+  std::copy(x.begin(), x.end(), x_); std::copy(zg.begin(), zg.end(), zg_); std::copy(yf.begin(), yf.end(), yf_);
+  std::copy(yg.begin(), yg.end(), yg_); std::copy(xi.begin(), xi.end(), xi_);
+  return minpiv > 0 ? 0 : 1;
 }
 
 // dense Gaussian elimination with partial pivoting, A [m][m] row-major, rhs in/out.  Returns min |pivot|.
@@ -429,6 +511,15 @@ int orc_sqp_bicycle_batch(const Cfg* cf, int B, int nthreads, const double* D, c
   else { std::vector<std::thread> th; for (int t = 0; t < nthreads; ++t) th.emplace_back(work, t); for (auto& t : th) t.join(); }
   int f = 0; for (int v : fail) f |= v; return f;
 }
+
+// f1: one problem, adaptive rho + termination.  info_out[8] = r_prim, r_dual, objective, min pivot, iterations, final rho_bar, converged, #log rows.
+int orc_admm_adaptive(const Cfg* cf, const Adaptive* ad, const double* D, const double* E, const double* q, const double* Am, const double* Ap, const double* b,
+                      const double* x_init, const double* G, const double* lo, const double* hi, double* x, double* zg, double* yf, double* yg, double* xi,
+                      double* info_out, double* log_out, int max_log) {
+  QP p = assemble(*cf, D, E, q, Am, Ap, b, x_init, G, lo, hi);
+  return admm_adaptive(*cf, p, *ad, x, zg, yf, yg, xi, info_out, log_out, max_log);
+}
+int orc_sizeof_adaptive() { return (int)sizeof(Adaptive); }
 
 int orc_sizeof_cfg() { return (int)sizeof(Cfg); }
 

@@ -373,6 +373,79 @@ def test_equality_rows_posed_as_inequality_rows_give_the_same_iterates():
     assert np.abs(sw["yf"]).max() > 1e-2 and (sw["xi"] != 0).any()
 
 
+# ----------------------------------------------------------------------------------------------- f1: adaptive rho + termination
+def _eq4_quantities(w, st, b=0):
+    """r_prim, r_dual (eq. 3) and the scales of eq. 4 from numpy-built matrices."""
+    P, C, c, G = dense_PCG(w, b)
+    x, yf, yg, zg, xi = st["x"][b].ravel(), st["yf"][b], st["yg"][b].ravel(), st["zg"][b].ravel(), st["xi"][b].ravel()
+    soft = np.tile(np.array(w.soft, dtype=bool), w.T)
+    m = soft & (xi != 0)
+    rp = max(np.abs(C @ x - c).max(), np.abs(G @ x - zg).max())
+    rd = max(np.abs(P @ x + w.q[b].ravel() + C.T @ yf + G.T @ yg).max(), np.abs(w.gamma * xi[m] + w.lam * np.sign(xi[m]) + yg[m]).max(initial=0))
+    npr = max(np.abs(C @ x).max(), np.abs(c).max(), np.abs(G @ x).max(), np.abs(zg).max())
+    nd = max(np.abs(P @ x).max(), np.abs(C.T @ yf + G.T @ yg).max(), np.abs(w.q[b]).max(), np.abs(w.gamma * xi[soft]).max(initial=0), np.abs(yg[soft]).max(initial=0))
+    return rp, rd, npr, nd
+
+
+def test_adaptive_off_equals_the_fixed_iteration_count():
+    """adapt_rho = 0 and eps = 0 (never converged): exactly the K iterations of Alg. 3, whatever the check cadence."""
+    w = W.config2(B=2, N=10, soft_bound=0.5)
+    w.rho_bar = 20.0
+    cfg = O.make_cfg(w)
+    ref, _, _ = O.admm(w, cfg, iters=60)
+    for every in (7, 25):
+        st, info, log, rc = O.admm_adaptive(w, cfg, O.make_adaptive(60, 0.0, 0.0, check_every=every, adapt_rho=0))
+        assert rc == 0 and (info[:, 4] == 60).all() and (info[:, 6] == 0).all()
+        assert all((st[k] == ref[k]).all() for k in ref)
+
+
+@pytest.mark.parametrize("lam,eps", [(100.0, 1e-5), (0.05, 1e-7)])
+def test_adaptive_schedule_recomputed_in_numpy(lam, eps):
+    """Every scheduled check of one adaptive run: the state at that iteration (obtained by capping max_iters there: the trajectory
+    is deterministic) gives, through numpy-built matrices, the residuals and scales of eq. 3-4, the verdict of eq. 4, the candidate
+    of eq. 17 with the clip [1e-6, 1e6] and the ratio gate 5 — all equal to what the oracle logged."""
+    w = W.config2(B=1, N=10, soft_bound=0.5)
+    w.lam = lam
+    cfg = O.make_cfg(w)
+    ad = O.make_adaptive(3000, eps, eps)
+    st, info, log, rc = O.admm_adaptive(w, cfg, ad)
+    nlog = int(info[0, 7])
+    assert rc == 0 and info[0, 6] == 1 and nlog >= 4 and int(info[0, 4]) == int(log[0, nlog - 1, 0]) and info[0, 4] % 25 == 0
+    changes = 0
+    for i in range(nlog):
+        k, rp_o, rd_o, np_o, nd_o, rho0, rho1, conv = log[0, i]
+        assert k == 25 * (i + 1)
+        sk, ik, _, _ = O.admm_adaptive(w, cfg, O.make_adaptive(int(k), eps, eps))
+        rp, rd, npr, nd = _eq4_quantities(w, sk)
+        for got, ref in ((rp_o, rp), (rd_o, rd), (np_o, npr), (nd_o, nd)):
+            assert abs(got - ref) <= 1e-10 * max(1.0, abs(ref)), (k, got, ref)
+        is_conv = rp <= eps + eps * npr and rd <= eps + eps * nd
+        assert bool(conv) == is_conv and (is_conv == (i == nlog - 1))
+        cand = min(max(rho0 * np.sqrt((rp / npr) / (rd / nd)), 1e-6), 1e6)
+        expect = cand if (not is_conv and max(cand / rho0, rho0 / cand) > 5.0) else rho0
+        assert abs(rho1 - expect) <= 1e-9 * expect, (k, rho1, expect)
+        changes += int(rho1 != rho0)
+        if i + 1 < nlog:
+            assert log[0, i + 1, 5] == rho1                      # the next interval runs with the accepted value
+    assert changes >= 1, "instance must exercise an accepted update"
+    assert abs(info[0, 5] - log[0, nlog - 1, 6]) == 0
+
+
+def test_adaptive_reaches_the_same_fixed_point_in_fewer_iterations():
+    """The step size changes the path, not the fixed point: the adaptive run and a fixed-rho run converge to the same (x, y), and
+    on the slack-stress instance (rho_bar = 0.1 makes the L1 dead zone 1000 wide, reading A-14) adaptation needs fewer iterations."""
+    w = W.config2(B=2, N=10, soft_bound=0.5)
+    cfg = O.make_cfg(w)
+    sa, ia, _, rca = O.admm_adaptive(w, cfg, O.make_adaptive(20000, 1e-9, 1e-9))
+    sf, if_, _, rcf = O.admm_adaptive(w, cfg, O.make_adaptive(20000, 1e-9, 1e-9, adapt_rho=0))
+    assert rca == 0 and (ia[:, 6] == 1).all()
+    assert (ia[:, 4] < if_[:, 4]).all()
+    ref, info, rc = O.admm(w, O.make_cfg(w, rho_bar=20.0), iters=30000)
+    assert info[:, :2].max() < 1e-10
+    for k in ("x", "yf", "yg", "xi"):
+        assert np.abs(sa[k] - ref[k]).max() <= 1e-6 * max(1.0, np.abs(ref[k]).max()), k
+
+
 # ----------------------------------------------------------------------------------------------- backward vs finite differences
 def _loss_of_solution(w, cfg, iters, xi_weight=0.0):
     st, info, rc = O.admm(w, cfg, iters=iters)
