@@ -251,6 +251,19 @@ def gpu_one(cfg_id, dtype, args, ctx, steps, with_cpu):
             a, b = ev(), ev(); a.record(); s.backward(dLdx); b.record(); torch.cuda.synchronize(dev); ts.append(a.elapsed_time(b))
         backward_ms = float(np.median(ts[3:]))
 
+    # ---- f1 (config 2): Alg. 3 as the paper runs it — adaptive step size + termination test, max 1000 iterations
+    adaptive = None
+    if cfg_id == 2:
+        adaptive = {}
+        for eps in (1e-3, 1e-5):
+            ts, out = [], None
+            for _ in range(3):
+                reset(); torch.cuda.synchronize(dev)
+                t0 = time.perf_counter(); out = s.solve_adaptive(1000, eps, eps); ts.append(time.perf_counter() - t0)
+            adaptive[f"eps_{eps:g}"] = {"ms_per_batched_solve": 1e3 * min(ts), "iterations_median": float(np.median(out["iters"])), "iterations_max": int(out["iters"].max()),
+                                        "converged_frac": float(out["converged"].mean()), "rho_bar_final_median": float(np.median(out["rho"])),
+                                        "note": "tmpc_factor + tmpc_admm_solve_adaptive, wall clock (the call synchronises once per 25-iteration round)"}
+
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
     if not w.model and cfg_id != 5:
@@ -342,7 +355,7 @@ def gpu_one(cfg_id, dtype, args, ctx, steps, with_cpu):
            "config": {"workload": workload_name(w, dtype), "l2": "256 MB flush write between timed steps",
                       "step": "tmpc_factor + tmpc_admm_solve" if not w.model else "n_sqp x (tmpc_linearize + tmpc_factor + tmpc_admm_solve)"},
            "admm_iters_per_s": value * iters, "ms_per_batched_solve": ms_per_step, "us_per_admm_iteration": 1e3 * ms_per_step / iters,
-           "backward_ms": backward_ms, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "roofline": roof,
+           "backward_ms": backward_ms, "adaptive": adaptive, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "roofline": roof,
            "parity_snapshot": {"max_r_prim": float(np.max(info["r_prim"])), "max_r_dual": float(np.max(info["r_dual"])), "status_nonzero": int((info["status"] != 0).sum())}}
     if with_cpu:
         cores = len(os.sched_getaffinity(0))

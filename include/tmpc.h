@@ -104,6 +104,26 @@ tmpc_status tmpc_factor(tmpc_handle h, const tmpc_qp* qp);
  * when `info` has a non-NULL pointer.  The state in `st` is complete between calls: a later call with
  * TMPC_SOLVE_ZG_GIVEN continues where this one stopped. */
 tmpc_status tmpc_admm_solve(tmpc_handle h, const tmpc_qp* qp, tmpc_state* st, int32_t iters, int32_t flags, tmpc_info* info);
+/* f1 — Alg. 3 as the paper runs it: adaptive step size and early termination (eq. 4, 299-303 eq. 17, 380).
+ * Every `check_every` iterations (k_rho^iter, paper default 25) and at iteration max_iters each live problem evaluates r_prim, r_dual
+ * (eq. 3) and the scales |(Ax, z)|_inf, |(Px, A'y, q, gamma xi, y_g on soft rows)|_inf; a problem that satisfies eq. 4 stops there
+ * (its state is final); otherwise, if adapt_rho, rho_new = clip(rho_bar sqrt((r_prim/|.|)/(r_dual/|.|)), [rho_min, rho_max]) replaces
+ * its rho_bar when max(rho_new/rho_bar, rho_bar/rho_new) > rho_ratio (paper: 5), and only those problems are re-factorised. */
+typedef struct {
+  int32_t max_iters;                  /* K_max >= 1 */
+  int32_t check_every;                /* k_rho^iter >= 1 */
+  int32_t adapt_rho;                  /* 0: termination test only */
+  int32_t reserved;
+  double eps_abs, eps_rel;            /* eq. 4 */
+  double rho_ratio, rho_min, rho_max; /* k_rho^ratio and the clip bounds of eq. 17 (paper: 5, 1e-6, 1e6) */
+} tmpc_adaptive;
+/* Needs tmpc_factor first (every problem starts from cfg.rho_bar) and, unlike the other calls, SYNCHRONISES: the count of live problems
+ * is read back after every round so that the call returns when all have terminated.  Outputs (DEVICE, [B], any may be NULL): iterations
+ * each problem ran, 1 if it met eq. 4, its final rho_bar (working dtype); info as in tmpc_admm_solve, at each problem's last check.
+ * Afterwards the factor in the workspace belongs to the per-problem rho_bar values: call tmpc_factor before the next solve.
+ * TMPC_E_UNSUPPORTED for the streamed class (stage blocks that do not fit in shared memory) and for cyclic reduction. */
+tmpc_status tmpc_admm_solve_adaptive(tmpc_handle h, const tmpc_qp* qp, tmpc_state* st, const tmpc_adaptive* ad, int32_t flags, tmpc_info* info,
+                                     int32_t* iters_out, int32_t* converged_out, void* rho_out);
 /* a10 (Alg. 2, eq. 59-65): dL/dq [B][T][n] and dL/dx_init [B][nx] from dL/dx [B][T][n] (and dL/dxi [B][T][ng] or NULL)
  * at the state st.  dL/dxi is the gradient with respect to the SIGNED slack st.xi that tmpc_admm_solve returns
  * (lo <= Gx + xi <= hi; App. E's xi_A of eq. 54 is |xi| = sign(xi) xi, so eq. 65's S dL/dxi_A is dL/dxi); only its

@@ -26,6 +26,10 @@ struct AdmmArgs {
   int iters, zg_given;
   int kkt_only;                           // 1: x <- S^{-1} x and return (tmpc_kkt_solve)
   const int8_t* soft_rows;                // optional [B][mg] per-row soft flag overriding d.soft_mask (adjoint QP, eq. 67)
+  // f1 (adaptive step size): optional per-problem rho_bar [B] (rho_g = rho_bar, rho_f = rho_scale rho_bar) replacing
+  // prm.rho_g / prm.rho_f, and an optional per-problem activity flag [B]: problems with active[p] == 0 (terminated by eq. 4) are left untouched
+  const T* rho_bar; T rho_scale;
+  const int32_t* active;
 };
 
 // shared-memory footprint in elements of T (host and device agree through this one function)
@@ -147,7 +151,8 @@ __global__ void __launch_bounds__(1024) admm_kernel(AdmmArgs<T> a) {
   const int n = NC ? NC : d.n;
   const int nx = d.nx, ng = d.ng, N = d.N, T_ = d.T, nn = n * n, nz = T_ * n, mf = d.mf, mg = d.mg;
   const int p = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
-  const T sigma = a.prm.sigma, rho_f = a.prm.rho_f, rho_g = a.prm.rho_g, alpha = a.prm.alpha;
+  if (a.active && !a.active[blockIdx.x]) return;        // terminated problem (f1): state stays as it is
+  const T sigma = a.prm.sigma, rho_g = a.rho_bar ? a.rho_bar[blockIdx.x] : a.prm.rho_g, rho_f = a.rho_bar ? a.rho_scale * rho_g : a.prm.rho_f, alpha = a.prm.alpha;
   const T inv_rho_g = T(1) / rho_g, inv_rg = T(1) / (rho_g + a.prm.gamma), lam = a.prm.lam, gam = a.prm.gamma;
 
   // ---- carve shared memory

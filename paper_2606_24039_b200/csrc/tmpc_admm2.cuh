@@ -664,6 +664,10 @@ struct ResidualArgs {
   const T* x; const T* zg; const T* yf; const T* yg; const T* xi;
   T* r_prim; T* r_dual; T* objective; int32_t* status;
   double* partial; int nparts;          // nparts > 1: gridDim.y CTAs per problem write partials, residual_finish_kernel reduces them in a fixed order
+  // f1: optional scales of the termination test eq. 4: norm_prim = |(Ax, z)|_inf, norm_dual = |(Px, A'y, q, gamma xi,
+  // y_g on soft rows)|_inf, [B] each (single-part launches only), and the activity flags (terminated problems keep their last values)
+  T* norm_prim; T* norm_dual;
+  const int32_t* active;
 };
 
 template <typename T>
@@ -672,7 +676,9 @@ __global__ void __launch_bounds__(256) residual_kernel(ResidualArgs<T> a) {
   const Dims& d = a.d;
   const int n = d.n, nx = d.nx, ng = d.ng, N = d.N, nn = n * n, nz = d.nz, mf = d.mf, mg = d.mg;
   const int p = blockIdx.x, nt = blockDim.x * gridDim.y, tid = blockIdx.y * blockDim.x + threadIdx.x;   // parts interleave
+  if (a.active && !a.active[p]) return;
   const T gam = a.prm.gamma, lam = a.prm.lam;
+  T nrp = T(0), nrd = T(0);
   const T* x = a.x + (size_t)p * nz; const T* zg = a.zg + (size_t)p * mg; const T* yf = a.yf + (size_t)p * mf;
   const T* yg = a.yg + (size_t)p * mg; const T* xi = a.xi + (size_t)p * mg; const T* q = a.qp.q + (size_t)p * nz;
   const T* Dp = a.qp.D + a.qp.sD * p; const T* Ep = a.qp.E + a.qp.sE * p;
@@ -689,14 +695,15 @@ __global__ void __launch_bounds__(256) residual_kernel(ResidualArgs<T> a) {
       for (int j = 0; j < n; ++j) s += am[j] * x[t * n + j] + ap[j] * x[(t + 1) * n + j];
       cx = s; c = a.qp.b[(size_t)p * N * nx + (e - nx)];
     }
-    rp = tmax(rp, tabs(cx - c));
+    rp = tmax(rp, tabs(cx - c)); nrp = tmax(nrp, tmax(tabs(cx), tabs(c)));
   }
   for (int e = tid; e < mg; e += nt) {
     const int t = e / ng, r = e - t * ng;
     T gx;
     if (d.g_sel) gx = x[t * n + d.g_col[r]];
     else { const T* g = G + ((size_t)t * ng + r) * n; gx = T(0); for (int j = 0; j < n; ++j) gx += g[j] * x[t * n + j]; }
-    rp = tmax(rp, tabs(gx - zg[e]));
+    rp = tmax(rp, tabs(gx - zg[e])); nrp = tmax(nrp, tmax(tabs(gx), tabs(zg[e])));
+    if ((d.soft_mask >> r) & 1u) nrd = tmax(nrd, tmax(tabs(gam * xi[e]), tabs(yg[e])));
     if (((d.soft_mask >> r) & 1u) && xi[e] != T(0)) {
       const T sg = xi[e] > T(0) ? T(1) : T(-1);
       rd = tmax(rd, tabs(gam * xi[e] + lam * sg + yg[e]));
@@ -710,17 +717,19 @@ __global__ void __launch_bounds__(256) residual_kernel(ResidualArgs<T> a) {
     for (int j = 0; j < n; ++j) px += Dt[j] * x[t * n + j];
     if (t > 0) { const T* Et = Ep + (size_t)(t - 1) * nn + i * n; for (int j = 0; j < n; ++j) px += Et[j] * x[(t - 1) * n + j]; }
     if (t < N) { const T* Et = Ep + (size_t)t * nn + i; for (int j = 0; j < n; ++j) px += Et[j * n] * x[(t + 1) * n + j]; }
-    T g = px + q[e];                                   // + C'y_f + G'y_g
+    T g = T(0);                                        // A'y = C'y_f + G'y_g
     if (t == 0 && i < nx) g += yf[i];
     if (t < N) { const T* A_ = Am + (size_t)t * nx * n + i; for (int k = 0; k < nx; ++k) g += A_[k * n] * yf[nx + t * nx + k]; }
     if (t > 0) { const T* A_ = Ap + (size_t)(t - 1) * nx * n + i; for (int k = 0; k < nx; ++k) g += A_[k * n] * yf[nx + (t - 1) * nx + k]; }
     if (d.g_sel) { for (int r = 0; r < ng; ++r) if (d.g_col[r] == i) g += yg[t * ng + r]; }
     else { const T* gg = G + (size_t)t * ng * n + i; for (int r = 0; r < ng; ++r) g += gg[r * n] * yg[t * ng + r]; }
-    rd = tmax(rd, tabs(g));
+    nrd = tmax(nrd, tmax(tabs(px), tmax(tabs(g), tabs(q[e]))));
+    rd = tmax(rd, tabs(px + q[e] + g));
     ob += T(0.5) * x[e] * px + q[e] * x[e];
     if (!isfinite(x[e])) bad = 1;
   }
   rp = block_max(rp, red); rd = block_max(rd, red); ob = block_sum(ob, red);
+  if (a.norm_prim) { nrp = block_max(nrp, red); nrd = block_max(nrd, red); if (threadIdx.x == 0) { a.norm_prim[p] = nrp; a.norm_dual[p] = nrd; } }
   bad = __syncthreads_or(bad);
   if (threadIdx.x == 0) {
     if (a.nparts > 1) { double* o = a.partial + ((size_t)p * a.nparts + blockIdx.y) * 4; o[0] = (double)rp; o[1] = (double)rd; o[2] = (double)ob; o[3] = bad ? 1.0 : 0.0; return; }
@@ -741,6 +750,35 @@ __global__ void residual_finish_kernel(ResidualArgs<T> a) {
   if (a.r_dual) a.r_dual[p] = (T)rd;
   if (a.objective) a.objective[p] = (T)ob;
   if (a.status && bad) atomicOr(&a.status[p], TMPC_ST_NAN);
+}
+
+// ---- f1: the decisions at a scheduled check (eq. 4 and eq. 17), one thread per problem, in double.
+struct AdaptParams { int k, last, adapt_rho; double eps_abs, eps_rel, ratio, rho_min, rho_max; };
+template <typename T>
+__global__ void adapt_kernel(int B, AdaptParams ap, const T* __restrict__ r_prim, const T* __restrict__ r_dual, const T* __restrict__ norm_prim,
+                             const T* __restrict__ norm_dual, T* __restrict__ rho_bar, int32_t* __restrict__ active, int32_t* __restrict__ mask,
+                             int32_t* __restrict__ iters, int32_t* __restrict__ converged, int32_t* __restrict__ n_active) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= B) return;
+  mask[p] = 0;
+  if (!active[p]) return;
+  iters[p] = ap.k;
+  const double rp = (double)r_prim[p], rd = (double)r_dual[p], np_ = (double)norm_prim[p], nd_ = (double)norm_dual[p];
+  if (rp <= ap.eps_abs + ap.eps_rel * np_ && rd <= ap.eps_abs + ap.eps_rel * nd_) { active[p] = 0; converged[p] = 1; return; }
+  if (ap.last) { active[p] = 0; return; }
+  atomicAdd(n_active, 1);
+  if (ap.adapt_rho && rd > 0.0 && np_ > 0.0 && nd_ > 0.0) {
+    const double rho = (double)rho_bar[p];
+    double cand = rho * sqrt((rp / np_) / (rd / nd_));
+    cand = fmin(fmax(cand, ap.rho_min), ap.rho_max);
+    if (fmax(cand / rho, rho / cand) > ap.ratio) { rho_bar[p] = (T)cand; mask[p] = 1; }
+  }
+}
+template <typename T>
+__global__ void adapt_init_kernel(int B, T rho0, T* rho_bar, int32_t* active, int32_t* mask, int32_t* iters, int32_t* converged, int32_t* n_active) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p == 0) *n_active = 0;
+  if (p < B) { rho_bar[p] = rho0; active[p] = 1; mask[p] = 0; iters[p] = 0; converged[p] = 0; }
 }
 
 }  // namespace tmpc

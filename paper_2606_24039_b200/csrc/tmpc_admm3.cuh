@@ -122,7 +122,7 @@ template <typename T, int H> __device__ __forceinline__ T dot2(const T (&a)[H], 
 // Row i >= n/2 takes its 16-byte chunks in the opposite order (`swb`; the data is not swizzled) so that the eight rows of a
 // slot cover the eight bank groups; the broadcast operand vector is read in the same order.
 template <typename T, int NC, int NX, int PG>
-__device__ __forceinline__ void chain3_solve(T* sm, int R, int PP, int T_, int lane) {
+__device__ __forceinline__ void chain3_solve(T* sm, int R, int PP, int T_, int lane, unsigned pmask) {   // pmask: bit g = problem g of the CTA is live
   static_assert(NC == 8 || NC == 6, "chain lanes are written for n = 6 and n = 8");
   using RC = Rec3<T, NC, NX>;
   constexpr int n = NC;
@@ -131,7 +131,7 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int PP, int T_, int l
   const int N = T_ - 1, m = T_ / 2;
   const int slot = lane >> 3, i8 = lane & 7;
   const int g = PG == 2 ? (slot >> 1) : 0, dir = slot & 1;
-  const bool act = (PG == 2 || slot < 2) && i8 < n;
+  const bool act = (PG == 2 || slot < 2) && i8 < n && ((pmask >> g) & 1u);
   const int ii = i8 < n ? i8 : 0;
   const unsigned swb = (unsigned)swz_x<T, NC>(ii) * ES;                 // chunk ORDER of my row (bytes)
   const int cnt = act ? (dir ? T_ - 1 - m : m) : 0, t0 = dir ? N : 0;
@@ -292,6 +292,9 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   // ================================================================ chain warp
   if (tid < 32) {
     const int iters = a.kkt_only ? 1 : a.iters;
+    unsigned pmask = 0u;
+#pragma unroll
+    for (int g = 0; g < PG; ++g) { const int p = blockIdx.x * PG + g; if (p < d.B && (!a.active || a.active[p])) pmask |= 1u << g; }
 #pragma unroll 1
 #ifdef TMPC_TIMING
     long long tch = 0; const long long tbeg = clock64();
@@ -301,7 +304,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
 #ifdef TMPC_TIMING
       __syncwarp(); const T probe = sm[tid & 7]; const long long c1 = clock64() + (probe == T(12345.678) ? 1 : 0);   // the load makes the deferred barrier block first
 #endif
-      chain3_solve<T, NC, NX, PG>(sm, R, PP, T_, tid);
+      chain3_solve<T, NC, NX, PG>(sm, R, PP, T_, tid, pmask);
       __syncwarp();
 #ifdef TMPC_TIMING
       tch += clock64() - c1;
@@ -317,7 +320,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   // ================================================================ item warps
   const int per_p = 2 * T_;                              // lanes per problem
   const int g = it_tid / per_p, rem = it_tid - g * per_p, t = rem >> 1, h = rem & 1, p = blockIdx.x * PG + g;
-  const bool valid = g < PG && p < d.B;
+  const bool valid = g < PG && p < d.B && (!a.active || a.active[p]);      // a terminated problem (f1) is left untouched
   const HalfOff mine = half_off<NC>(h), other = half_off<NC>(1 - h);
   const int b = valid ? g * PP + rec(t) : 0, bn = valid ? g * PP + (t < N ? rec(t + 1) : rec(0)) : 0;
   const T* Xb = sm + b + RC::SINV;
@@ -351,6 +354,9 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
     return;
   }
 
+  // step sizes: per problem when the adaptive schedule (f1) runs, else the handle's
+  const T rho_g = (a.rho_bar && valid) ? a.rho_bar[p] : a.prm.rho_g, rho_f = a.rho_bar ? a.rho_scale * rho_g : a.prm.rho_f;
+  const T rfa = a.rho_bar ? rho_f * a.prm.alpha : A.rfa, inv_rho_g = a.rho_bar ? T(1) / rho_g : A.inv_rho_g, inv_rg = a.rho_bar ? T(1) / (rho_g + a.prm.gamma) : A.inv_rg;
   // ---- per-lane state in registers (slot order)
   constexpr unsigned Q_VALID = 1u, Q_SOFT = 2u, Q_ROW_SH = 4;         // inequality slot flags: valid, soft, row index << 4
   T x[H], q[H], zg[H], yg[H], lo[H], hi[H], xi_last[H];
@@ -407,11 +413,11 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
 #pragma unroll
     for (int s = 0; s < H; ++s) {
       T dd = a.prm.sigma * x[s] - q[s];
-      if (d.g_sel && (qf[s] & Q_VALID)) dd += a.prm.rho_g * zg[s] - yg[s];
+      if (d.g_sel && (qf[s] & Q_VALID)) dd += rho_g * zg[s] - yg[s];
       dn[s] = dd;
     }
 #pragma unroll
-    for (int s = 0; s < KA; ++s) ro[s] = a.prm.rho_f * cv[s] - yf[s];   // r = rho_f c - y_f of my rows (0 beyond nk: c = y_f = 0)
+    for (int s = 0; s < KA; ++s) ro[s] = rho_f * cv[s] - yf[s];   // r = rho_f c - y_f of my rows (0 beyond nk: c = y_f = 0)
 #pragma unroll
     for (int s = 0; s < H; ++s) dr[s] = shfl_x1(dn[s]);                // the partner's halves
 #pragma unroll
@@ -419,7 +425,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
     T sg[H], sgr[H];
     if (!d.g_sel) {
 #pragma unroll
-      for (int s = 0; s < H; ++s) sg[s] = (qf[s] & Q_VALID) ? a.prm.rho_g * zg[s] - yg[s] : T(0);
+      for (int s = 0; s < H; ++s) sg[s] = (qf[s] & Q_VALID) ? rho_g * zg[s] - yg[s] : T(0);
 #pragma unroll
       for (int s = 0; s < H; ++s) sgr[s] = shfl_x1(sg[s]);
     }
@@ -480,7 +486,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
           T zt = dot2<T, H>(f, yo, f2, yr);
           ld_half<NC>(sm + bn + RC::AP + k * n, mine, f); ld_half<NC>(sm + bn + RC::AP + k * n, other, f2);
           zt += dot2<T, H>(f, y2o, f2, y2r);
-          yf[s] += A.rfa * (zt - cv[s]);
+          yf[s] += rfa * (zt - cv[s]);
         }
       }
 #pragma unroll
@@ -489,10 +495,10 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
           T ztg = xt[s];
           if (!d.g_sel) { const T* row = sm + b + RC::G + (int)(qf[s] >> Q_ROW_SH) * n; T f[H], f2[H]; ld_half<NC>(row, mine, f); ld_half<NC>(row, other, f2); ztg = dot2<T, H>(f, yo, f2, yr); }
           const T zh = a.prm.alpha * ztg + A.oma * zg[s];
-          const T v = zh + yg[s] * A.inv_rho_g;
+          const T v = zh + yg[s] * inv_rho_g;
           T z, sl;
-          project_row<T>((qf[s] & Q_SOFT) != 0, v, lo[s], hi[s], a.prm.rho_g, A.inv_rg, a.prm.lam, z, sl);
-          yg[s] += a.prm.rho_g * (zh - z);
+          project_row<T>((qf[s] & Q_SOFT) != 0, v, lo[s], hi[s], rho_g, inv_rg, a.prm.lam, z, sl);
+          yg[s] += rho_g * (zh - z);
           zg[s] = z;
           xi_last[s] = sl;
         }

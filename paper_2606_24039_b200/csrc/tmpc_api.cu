@@ -26,7 +26,7 @@ inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 inline size_t esize(int dtype) { return dtype == TMPC_F64 ? 8 : 4; }
 
 struct Layout {   // byte offsets into the workspace
-  size_t Lam, Sinv, eta, fstatus, cls, soft_adj, rhs, w_rows, lo_adj, hi_adj, q_adj, ax, azg, ayf, ayg, axi, zero_xinit, zero_b, res, cr, total;
+  size_t Lam, Sinv, eta, fstatus, ad_rho, ad_np, ad_nd, ad_rp, ad_rd, ad_obj, ad_active, ad_mask, ad_iters, ad_conv, ad_count, cls, soft_adj, rhs, w_rows, lo_adj, hi_adj, q_adj, ax, azg, ayf, ayg, axi, zero_xinit, zero_b, res, cr, total;
 };
 
 // Cyclic reduction (tmpc_cr.cuh) exists for n = 6 and n = 8 and pays off for a few very long horizons; TMPC_LIN_AUTO picks it
@@ -52,6 +52,10 @@ Layout make_layout(const tmpc_config& c) {
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
   L.Lam = take(B * d.T * nn * es); L.Sinv = take(B * d.T * nn * es); L.eta = take(B * d.nz * es);
   L.fstatus = take(B * sizeof(int32_t));       // per-problem TMPC_ST_PIVOT word of the last tmpc_factor
+  // f1 (tmpc_admm_solve_adaptive): per-problem rho_bar, eq. 4 scales, residuals / objective when the caller passes no info, flags, counters
+  L.ad_rho = take(B * es); L.ad_np = take(B * es); L.ad_nd = take(B * es); L.ad_rp = take(B * es); L.ad_rd = take(B * es); L.ad_obj = take(B * es);
+  L.ad_active = take(B * sizeof(int32_t)); L.ad_mask = take(B * sizeof(int32_t)); L.ad_iters = take(B * sizeof(int32_t)); L.ad_conv = take(B * sizeof(int32_t));
+  L.ad_count = take(256);
   L.cls = take(B * d.mg); L.soft_adj = take(B * d.mg);
   L.rhs = take(B * d.nz * es); L.w_rows = take(B * d.mg * es); L.lo_adj = take(B * d.mg * es); L.hi_adj = take(B * d.mg * es);
   L.q_adj = take(B * d.nz * es); L.ax = take(B * d.nz * es); L.azg = take(B * d.mg * es); L.ayf = take(B * d.mf * es);
@@ -79,6 +83,8 @@ tmpc_status check_cfg(const tmpc_config* c) {
 
 struct tmpc_ctx {
   tmpc_config cfg; Dims d; Layout lay; unsigned char* ws; cudaStream_t stream; bool factored; bool cr; bool twisted; int64_t launches;
+  // set while tmpc_admm_solve_adaptive runs (f1): per-problem rho_bar, activity flags for the solve kernels, refactor mask for the factor kernels
+  const void* cur_rho; const int32_t* cur_active; const int32_t* cur_mask;
 };
 
 namespace {
@@ -101,6 +107,7 @@ inline bool cuda_ok() { return cudaGetLastError() == cudaSuccess; }
 template <typename T>
 tmpc_status launch_factor(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_in, const T* w_rows, int32_t* status) {
   FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = w_rows;
+  a.rho_bar = w_rows ? nullptr : (const T*)h->cur_rho; a.rho_scale = h->cfg.rho_eq_scale; a.mask = w_rows ? nullptr : h->cur_mask;
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
   // small compile-time shapes: the warp-level kernel in its one-directional form (tmpc_factor2.cuh)
   if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) { factor_tw2_kernel<T, 8, 6, false><<<h->d.B, 32, 0, h->stream>>>(a); h->launches++; return cuda_ok() ? TMPC_OK : TMPC_E_CUDA; }
@@ -187,6 +194,12 @@ tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
   if (!res && smem_str > kMaxSmem) return TMPC_E_UNSUPPORTED;
   int nt = ((d.nz + 31) / 32) * 32; if (nt > 1024) nt = 1024; if (nt < 64) nt = 64;
   if (res) {
+    if (a.active) {                      // adaptive schedule (f1): the eq. 4 scales come from residual_kernel, not from the in-kernel residuals
+      AdmmArgs<T> b = a; b.r_prim = b.r_dual = b.objective = nullptr; b.status = nullptr;
+      const tmpc_status s = d.n == 6 ? launch_admm_inst<T, 6, true>(h, b, nt, smem_res) : d.n == 8 ? launch_admm_inst<T, 8, true>(h, b, nt, smem_res)
+                                                                                                    : launch_admm_inst<T, 0, true>(h, b, nt, smem_res);
+      return s != TMPC_OK ? s : launch_residual<T>(h, a);
+    }
     if (d.n == 6) return launch_admm_inst<T, 6, true>(h, a, nt, smem_res);
     if (d.n == 8) return launch_admm_inst<T, 8, true>(h, a, nt, smem_res);
     return launch_admm_inst<T, 0, true>(h, a, nt, smem_res);
@@ -268,6 +281,7 @@ tmpc_status launch_admm2(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
 template <typename T>
 tmpc_status launch_factor_tw(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_in, int32_t* status) {
   FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = nullptr;
+  a.rho_bar = (const T*)h->cur_rho; a.rho_scale = h->cfg.rho_eq_scale; a.mask = h->cur_mask;
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
   if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) factor_tw2_kernel<T, 8, 6, true><<<h->d.B, 64, 0, h->stream>>>(a);
   else if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) factor_tw2_kernel<T, 6, 4, true><<<h->d.B, 64, 0, h->stream>>>(a);
@@ -280,9 +294,11 @@ tmpc_status launch_residual(tmpc_ctx* h, const AdmmArgs<T>& s) {
   if (!s.r_prim && !s.r_dual && !s.objective && !s.status) return TMPC_OK;
   ResidualArgs<T> r; r.d = h->d; r.prm = s.prm; r.qp = s.qp; r.x = s.x; r.zg = s.zg; r.yf = s.yf; r.yg = s.yg; r.xi = s.xi;
   r.r_prim = s.r_prim; r.r_dual = s.r_dual; r.objective = s.objective; r.status = s.status;
+  r.norm_prim = nullptr; r.norm_dual = nullptr; r.active = s.active;
+  if (s.active) { r.norm_prim = (T*)(h->ws + h->lay.ad_np); r.norm_dual = (T*)(h->ws + h->lay.ad_nd); }
   int nt = ((h->d.nz + 31) / 32) * 32; if (nt > 256) nt = 256;
   int nparts = 1;                        // few long problems: several CTAs per problem, partials reduced in a fixed order
-  if (h->d.B < 64) { nparts = (h->d.nz + 2047) / 2048; if (nparts > 64) nparts = 64; if (nparts < 1) nparts = 1; }
+  if (h->d.B < 64 && !s.active) { nparts = (h->d.nz + 2047) / 2048; if (nparts > 64) nparts = 64; if (nparts < 1) nparts = 1; }
   r.partial = (double*)(h->ws + h->lay.res); r.nparts = nparts;
   residual_kernel<T><<<dim3(h->d.B, nparts), nt, 0, h->stream>>>(r); h->launches++;
   if (nparts > 1) { residual_finish_kernel<T><<<(h->d.B + 63) / 64, 64, 0, h->stream>>>(r); h->launches++; }
@@ -349,7 +365,54 @@ tmpc_status do_solve(tmpc_ctx* h, const tmpc_qp* qp, tmpc_state* st, int iters, 
   a.x = (T*)st->x; a.zg = (T*)st->zg; a.yf = (T*)st->yf; a.yg = (T*)st->yg; a.xi = (T*)st->xi;
   if (info) { a.r_prim = (T*)info->r_prim; a.r_dual = (T*)info->r_dual; a.objective = (T*)info->objective; a.status = info->status; }
   a.iters = iters; a.zg_given = (flags & TMPC_SOLVE_ZG_GIVEN) ? 1 : 0;
+  a.rho_bar = (const T*)h->cur_rho; a.rho_scale = (T)h->cfg.rho_eq_scale; a.active = h->cur_active;
   return launch_admm<T>(h, a);
+}
+
+// ---- f1: Alg. 3 with the adaptive step size (eq. 17) and the termination test (eq. 4).
+// Rounds of `check_every` iterations: [solve kernel on the live problems with their own rho_bar] -> [residuals + eq. 4 scales] ->
+// [adapt_kernel: terminate / new rho_bar / refactor mask] -> [masked refactor].  The number of live problems comes back to the host
+// after every round (4 bytes), so the call returns as soon as every problem has terminated.
+template <typename T>
+tmpc_status do_solve_adaptive(tmpc_ctx* h, const tmpc_qp* qp, tmpc_state* st, const tmpc_adaptive* ad, int flags, tmpc_info* info,
+                              int32_t* iters_out, int32_t* conv_out, void* rho_out) {
+  const Dims& d = h->d; const Layout& L = h->lay; unsigned char* ws = h->ws;
+  if (h->cr) return TMPC_E_UNSUPPORTED;
+  if (!h->twisted && admm_smem_elems(d, true) * sizeof(T) > kMaxSmem) return TMPC_E_UNSUPPORTED;     // streamed class: fixed-count solves only
+  T* rho = (T*)(ws + L.ad_rho); int32_t* active = (int32_t*)(ws + L.ad_active); int32_t* mask = (int32_t*)(ws + L.ad_mask);
+  int32_t* iters = (int32_t*)(ws + L.ad_iters); int32_t* conv = (int32_t*)(ws + L.ad_conv); int32_t* count = (int32_t*)(ws + L.ad_count);
+  tmpc_info li;
+  li.r_prim = info && info->r_prim ? info->r_prim : ws + L.ad_rp; li.r_dual = info && info->r_dual ? info->r_dual : ws + L.ad_rd;
+  li.objective = info && info->objective ? info->objective : ws + L.ad_obj; li.status = info ? info->status : nullptr;
+  const unsigned nb = (unsigned)((d.B + 255) / 256);
+  adapt_init_kernel<T><<<nb, 256, 0, h->stream>>>(d.B, (T)h->cfg.rho_bar, rho, active, mask, iters, conv, count); h->launches++;
+  if (!cuda_ok()) return TMPC_E_CUDA;
+  h->cur_rho = rho; h->cur_active = active; h->cur_mask = mask;
+  tmpc_status rc = TMPC_OK;
+  int k = 0, f = flags;
+  while (k < ad->max_iters && rc == TMPC_OK) {
+    const int chunk = ad->max_iters - k < ad->check_every ? ad->max_iters - k : ad->check_every;
+    rc = do_solve<T>(h, qp, st, chunk, f, &li);          // also runs residual_kernel with the eq. 4 scales (li is never null)
+    if (rc != TMPC_OK) break;
+    k += chunk; f |= TMPC_SOLVE_ZG_GIVEN;
+    if (cudaMemsetAsync(count, 0, sizeof(int32_t), h->stream) != cudaSuccess) { rc = TMPC_E_CUDA; break; }
+    AdaptParams ap; ap.k = k; ap.last = k >= ad->max_iters; ap.adapt_rho = ad->adapt_rho; ap.eps_abs = ad->eps_abs; ap.eps_rel = ad->eps_rel;
+    ap.ratio = ad->rho_ratio; ap.rho_min = ad->rho_min; ap.rho_max = ad->rho_max;
+    adapt_kernel<T><<<nb, 256, 0, h->stream>>>(d.B, ap, (const T*)li.r_prim, (const T*)li.r_dual, (const T*)(ws + L.ad_np), (const T*)(ws + L.ad_nd), rho, active, mask,
+                                              iters, conv, count); h->launches++;
+    int32_t live = 0;
+    if (!cuda_ok() || cudaMemcpyAsync(&live, count, sizeof(int32_t), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+        cudaStreamSynchronize(h->stream) != cudaSuccess) { rc = TMPC_E_CUDA; break; }
+    if (live == 0) break;
+    if (ad->adapt_rho) rc = do_factor<T>(h, qp);          // only the problems whose rho_bar changed (mask)
+  }
+  h->cur_rho = nullptr; h->cur_active = nullptr; h->cur_mask = nullptr;
+  h->factored = false;                                   // the factor in the workspace now belongs to the per-problem rho_bar values
+  if (rc != TMPC_OK) return rc;
+  if (iters_out && cudaMemcpyAsync(iters_out, iters, (size_t)d.B * sizeof(int32_t), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess) return TMPC_E_CUDA;
+  if (conv_out && cudaMemcpyAsync(conv_out, conv, (size_t)d.B * sizeof(int32_t), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess) return TMPC_E_CUDA;
+  if (rho_out && cudaMemcpyAsync(rho_out, rho, (size_t)d.B * sizeof(T), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess) return TMPC_E_CUDA;
+  return TMPC_OK;
 }
 
 template <typename T>
@@ -396,6 +459,7 @@ tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, vo
   if (!h) return TMPC_E_BADARG;
   h->cfg = *cfg; h->d = make_dims(*cfg); h->lay = L; h->ws = (unsigned char*)workspace; h->stream = (cudaStream_t)cuda_stream;
   h->factored = false; h->cr = use_cr(*cfg); h->twisted = false; h->launches = 0;
+  h->cur_rho = nullptr; h->cur_active = nullptr; h->cur_mask = nullptr;
   // zero buffers of the adjoint QP (x_init = 0, b = 0)
   if (cudaMemsetAsync(h->ws + L.zero_xinit, 0, L.zero_b - L.zero_xinit, h->stream) != cudaSuccess ||
       cudaMemsetAsync(h->ws + L.zero_b, 0, L.cr - L.zero_b, h->stream) != cudaSuccess) { delete h; return TMPC_E_CUDA; }
@@ -457,6 +521,17 @@ tmpc_status tmpc_admm_solve(tmpc_handle h, const tmpc_qp* qp, tmpc_state* st, in
   if (!st || !st->x || !st->zg || !st->yf || !st->yg || !st->xi || iters < 0) return TMPC_E_BADARG;
   if (!h->factored) return TMPC_E_STATE;
   return h->cfg.dtype == TMPC_F32 ? do_solve<float>(h, qp, st, iters, flags, info) : do_solve<double>(h, qp, st, iters, flags, info);
+}
+
+tmpc_status tmpc_admm_solve_adaptive(tmpc_handle h, const tmpc_qp* qp, tmpc_state* st, const tmpc_adaptive* ad, int32_t flags, tmpc_info* info,
+                                     int32_t* iters_out, int32_t* converged_out, void* rho_out) {
+  tmpc_status s = check_qp(h, qp); if (s != TMPC_OK) return s;
+  if (!st || !st->x || !st->zg || !st->yf || !st->yg || !st->xi || !ad) return TMPC_E_BADARG;
+  if (ad->max_iters < 1 || ad->check_every < 1 || !(ad->eps_abs >= 0) || !(ad->eps_rel >= 0)) return TMPC_E_BADARG;
+  if (ad->adapt_rho && (!(ad->rho_ratio >= 1) || !(ad->rho_min > 0) || !(ad->rho_max >= ad->rho_min))) return TMPC_E_BADARG;
+  if (!h->factored) return TMPC_E_STATE;
+  return h->cfg.dtype == TMPC_F32 ? do_solve_adaptive<float>(h, qp, st, ad, flags, info, iters_out, converged_out, rho_out)
+                                  : do_solve_adaptive<double>(h, qp, st, ad, flags, info, iters_out, converged_out, rho_out);
 }
 
 tmpc_status tmpc_kkt_solve(tmpc_handle h, const void* eta, void* xt) {

@@ -24,6 +24,10 @@ struct FactorArgs {
   const T* w_rows;              // optional per-inequality-row weights [B][T][ng] (overrides w_in), else null
   T* Lam; T* Sinv;              // outputs [B][N][n][n], [B][T][n][n]
   int32_t* status;              // [B], written: TMPC_ST_PIVOT or 0 (may be null)
+  // f1 (adaptive step size): optional per-problem rho_bar [B] (w_in = rho_bar, w_eq = rho_scale rho_bar) and an optional refactor
+  // mask [B]: problems with mask[p] == 0 keep their factor
+  const T* rho_bar; double rho_scale;
+  const int32_t* mask;
 };
 
 template <typename T, typename TA>
@@ -35,6 +39,8 @@ __global__ void __launch_bounds__(1024) factor_kernel(FactorArgs<T> a) {
   TA* Bm = A + nn;
   TA* C = Bm + nn;
   const int p = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
+  if (a.mask && !a.mask[p]) return;
+  const double w_in = a.rho_bar ? (double)a.rho_bar[p] : a.w_in, w_eq = a.rho_bar ? a.rho_scale * w_in : a.w_eq;
   const T* Dp = a.qp.D + a.qp.sD * p;
   const T* Ep = a.qp.E + a.qp.sE * p;
   const T* Amp = a.qp.Am + (size_t)p * N * nx * n;
@@ -60,11 +66,11 @@ __global__ void __launch_bounds__(1024) factor_kernel(FactorArgs<T> a) {
       if (t < N) for (int r = 0; r < nx; ++r) acc += (TA)Amt[r * n + i] * (TA)Amt[r * n + j];
       if (t > 0) for (int r = 0; r < nx; ++r) acc += (TA)Apm[r * n + i] * (TA)Apm[r * n + j];
       if (t == 0 && i == j && i < nx) acc += 1;        // A_init' A_init = blkdiag(I_nx, 0)
-      s += a.w_eq * acc;
+      s += (TA)w_eq * acc;
       if (d.g_sel) {
-        for (int r = 0; r < ng; ++r) if (d.g_col[r] == i && i == j) s += wr ? (TA)wr[t * ng + r] : (TA)a.w_in;
+        for (int r = 0; r < ng; ++r) if (d.g_col[r] == i && i == j) s += wr ? (TA)wr[t * ng + r] : (TA)w_in;
       } else {
-        for (int r = 0; r < ng; ++r) s += (wr ? (TA)wr[t * ng + r] : (TA)a.w_in) * (TA)Gt[r * n + i] * (TA)Gt[r * n + j];
+        for (int r = 0; r < ng; ++r) s += (wr ? (TA)wr[t * ng + r] : (TA)w_in) * (TA)Gt[r * n + i] * (TA)Gt[r * n + j];
       }
       if (t > 0) { TA c = 0; for (int k = 0; k < n; ++k) c += C[i * n + k] * C[j * n + k]; s -= c; }
       A[e] = s;
@@ -113,7 +119,7 @@ __global__ void __launch_bounds__(1024) factor_kernel(FactorArgs<T> a) {
         const int i = e / n, j = e - i * n;
         TA acc = 0;
         for (int r = 0; r < nx; ++r) acc += (TA)Apt[r * n + i] * (TA)Amt[r * n + j];
-        A[e] = (TA)Et[e] + a.w_eq * acc;
+        A[e] = (TA)Et[e] + (TA)w_eq * acc;
       }
       __syncthreads();
       // ---- C <- W_t = Phi_t X'   (X lower: sum over k <= j)

@@ -51,7 +51,8 @@ __global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
   T* Xp = a.Sinv + (size_t)p * T_ * nn;
   const int m = TW ? T_ / 2 : T_, cnt = half ? T_ - 1 - m : m;      // !TW: the up chain covers every stage, no middle
   const T* wr = a.w_rows ? a.w_rows + (size_t)p * T_ * ng : nullptr;
-  const double w_eq = a.w_eq, w_in = a.w_in, sigma = a.sigma;
+  if (a.mask && !a.mask[p]) return;
+  const double w_in = a.rho_bar ? (double)a.rho_bar[p] : a.w_in, w_eq = a.rho_bar ? a.rho_scale * w_in : a.w_eq, sigma = a.sigma;
   int bad = 0;
 
   // raw data of stage t for this chain: D_t, the coupling block E_tc (tc = t for up, t-1 for down), A^-_t, A^+_{t-1}, G_t

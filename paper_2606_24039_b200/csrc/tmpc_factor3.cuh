@@ -49,6 +49,8 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
   T* S1 = reinterpret_cast<T*>(R + (size_t)ld * ld);              // staged chunk, [F3_CH][ld], working dtype (exact copy)
   T* S2 = S1 + (size_t)F3_CH * ld;
   const int p = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
+  if (a.mask && !a.mask[p]) return;
+  const double w_in = a.rho_bar ? (double)a.rho_bar[p] : a.w_in, w_eq = a.rho_bar ? a.rho_scale * w_in : a.w_eq;
   const T* Dp = a.qp.D + a.qp.sD * p;
   const T* Ep = a.qp.E + a.qp.sE * p;
   const T* Amp = a.qp.Am + (size_t)p * N * nx * n;
@@ -170,7 +172,7 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
         const int rows = ng - r0 < F3_CH ? ng - r0 : F3_CH;
         __syncthreads();
         stage(S1, Gp + (size_t)t * ng * n, r0, rows, nullptr, 1.0);
-        stage(S2, Gp + (size_t)t * ng * n, r0, rows, wrow ? wrow + (size_t)t * ng : nullptr, wrow ? 1.0 : a.w_in);
+        stage(S2, Gp + (size_t)t * ng * n, r0, rows, wrow ? wrow + (size_t)t * ng : nullptr, wrow ? 1.0 : w_in);
         __syncthreads();
         mm(acc, S1, S2, 0, (rows + 3) & ~3, f3_ic<0>{});
       }
@@ -185,11 +187,11 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
               const int gi = 8 * (3 * wr + x) + lq, gj = 8 * (3 * wc + y) + 2 * lr + e;
               double s = 0.0;
               if (gi < n && gj < n) {
-                s = (double)Dp[(size_t)t * nn + gi * n + gj] + a.w_eq * accA[x][y][e] + acc[x][y][e];
+                s = (double)Dp[(size_t)t * nn + gi * n + gj] + w_eq * accA[x][y][e] + acc[x][y][e];
                 if (gi == gj) {
                   s += a.sigma;
-                  if (t == 0 && gi < nx) s += a.w_eq;      // A_init' A_init = blkdiag(I_nx, 0)
-                  if (d.g_sel) for (int r = 0; r < ng; ++r) if (d.g_col[r] == gi) s += wrow ? (double)wrow[(size_t)t * ng + r] : a.w_in;
+                  if (t == 0 && gi < nx) s += w_eq;      // A_init' A_init = blkdiag(I_nx, 0)
+                  if (d.g_sel) for (int r = 0; r < ng; ++r) if (d.g_col[r] == gi) s += wrow ? (double)wrow[(size_t)t * ng + r] : w_in;
                 }
               } else if (gi == gj) s = 1.0;              // identity on the padding keeps the factor well defined
               P[(size_t)gi * ld + gj] = s;
@@ -310,7 +312,7 @@ __global__ void __launch_bounds__(512) factor3_kernel(FactorArgs<T> a) {
         if (fast && r0 + F3_CH < nx) { __syncthreads(); issue_phi(r0 + F3_CH); }
       }
       for_acc(acc, [&](double& v, int gk, int gi) {
-        Q[(size_t)gk * ld + gi] = (gk < n && gi < n) ? (double)Ep[(size_t)t * nn + gi * n + gk] + a.w_eq * v : 0.0;
+        Q[(size_t)gk * ld + gi] = (gk < n && gi < n) ? (double)Ep[(size_t)t * nn + gi * n + gk] + w_eq * v : 0.0;
       });
       __syncthreads();
     }

@@ -97,6 +97,17 @@ class Solver:
         self.factor()
         self.admm_solve(iters)
 
+    def solve_adaptive(self, max_iters, eps_abs=1e-3, eps_rel=1e-3, check_every=25, ratio=5.0, rho_min=1e-6, rho_max=1e6, adapt_rho=True, flags=0):
+        """f1: tmpc_factor + tmpc_admm_solve_adaptive (paper defaults of PAPER.md:303).  Returns dict(iters, converged, rho) as numpy arrays."""
+        w = self.w
+        self.factor()
+        it = torch.zeros(w.B, dtype=torch.int32, device=self.dev); cv = torch.zeros(w.B, dtype=torch.int32, device=self.dev)
+        rho = torch.zeros(w.B, dtype=self.td, device=self.dev)
+        ad = B.TmpcAdaptive(int(max_iters), int(check_every), int(bool(adapt_rho)), 0, eps_abs, eps_rel, ratio, rho_min, rho_max)
+        B.tmpc_admm_solve_adaptive(self.h, self.qp, self.st, ad, flags, self._info(), it.data_ptr(), cv.data_ptr(), rho.data_ptr())
+        torch.cuda.synchronize(self.dev)
+        return dict(iters=it.cpu().numpy(), converged=cv.cpu().numpy(), rho=rho.cpu().double().numpy())
+
     def sqp(self, n_sqp=None, iters=None):
         """configs 4-5: n_sqp x (linearize at xbar = current x -> factor -> ADMM warm start), full steps (reading A-26)."""
         for _ in range(self.w.sqp_iters if n_sqp is None else n_sqp):
