@@ -251,19 +251,6 @@ def gpu_one(cfg_id, dtype, args, ctx, steps, with_cpu):
             a, b = ev(), ev(); a.record(); s.backward(dLdx); b.record(); torch.cuda.synchronize(dev); ts.append(a.elapsed_time(b))
         backward_ms = float(np.median(ts[3:]))
 
-    # ---- f1 (config 2): Alg. 3 as the paper runs it — adaptive step size + termination test, max 1000 iterations (PAPER.md:416, 299-303)
-    adaptive = None
-    if cfg_id == 2:
-        adaptive = {}
-        for eps in (1e-3, 1e-5):
-            ts, out = [], None
-            for _ in range(3):
-                reset(); torch.cuda.synchronize(dev)
-                t0 = time.perf_counter(); out = s.solve_adaptive(1000, eps, eps); ts.append(time.perf_counter() - t0)
-            adaptive[f"eps_{eps:g}"] = {"ms_per_batched_solve": 1e3 * min(ts), "iterations_median": float(np.median(out["iters"])), "iterations_max": int(out["iters"].max()),
-                                        "converged_frac": float(out["converged"].mean()), "rho_bar_final_median": float(np.median(out["rho"])),
-                                        "note": "tmpc_factor + tmpc_admm_solve_adaptive, wall clock (the call synchronises once per 25-iteration round)"}
-
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
     if not w.model and cfg_id != 5:
@@ -313,6 +300,19 @@ def gpu_one(cfg_id, dtype, args, ctx, steps, with_cpu):
         nb = lambda t: t.numel() * t.element_size()
         e2e = {"value": w.B * world * steps / float(t_e2e.item()), "unit": "QP solves/s", "h2d_bytes_per_step": int(nb(hx0) + nb(href) + nb(hq_) + nb(hxi)),
                "d2h_bytes_per_step": int(nb(hout)), "ms_per_step": 1e3 * float(t_e2e.item()) / steps}
+    # ---- f1 (config 2): Alg. 3 as the paper runs it — adaptive step size + termination test, max 1000 iterations (PAPER.md:416, 299-303)
+    adaptive = None
+    if cfg_id == 2:
+        adaptive = {}
+        for eps in (1e-3, 1e-5):
+            ts, out = [], None
+            for _ in range(3):
+                reset(); torch.cuda.synchronize(dev)
+                t0 = time.perf_counter(); out = s.solve_adaptive(1000, eps, eps); ts.append(time.perf_counter() - t0)
+            adaptive[f"eps_{eps:g}"] = {"ms_per_batched_solve": 1e3 * min(ts), "iterations_median": float(np.median(out["iters"])), "iterations_max": int(out["iters"].max()),
+                                        "converged_frac": float(out["converged"].mean()), "rho_bar_final_median": float(np.median(out["rho"])),
+                                        "note": "tmpc_factor + tmpc_admm_solve_adaptive, wall clock (the call synchronises once per 25-iteration round)"}
+
     s.close()
     if rank != 0:
         return None
@@ -364,6 +364,58 @@ def gpu_one(cfg_id, dtype, args, ctx, steps, with_cpu):
     return res
 
 
+def f4_rows(ctx, args):
+    """f4: the paper's linear-system RL workload at four shapes of its sweep x u_max in {1, 10}: time to
+    tolerance 1e-3 / 1e-5 with at most 1000 ADMM iterations (the paper's setting), backward pass, and an H = 50 closed-loop roll-out of
+    warm-started MPC solves at the nominal shape.  fp64 like the paper."""
+    import torch
+    from paper_2606_24039_b200 import binding as Bd
+    from paper_2606_24039_b200 import workloads as W
+    from paper_2606_24039_b200.solver import Solver
+    dev = ctx["dev"]
+    rows = []
+    for (B, N, nx, nu) in ((64, 40, 8, 4), (1024, 40, 8, 4), (64, 160, 8, 4), (64, 40, 32, 16)):
+        for u_max in (1.0, 10.0):
+            w = W.linear_rl(B=B, N=N, nx=nx, nu=nu, u_max=u_max)
+            s = Solver(w, dtype="f64", device=dev)
+            row = {"B": B, "N": N, "nx": nx, "nu": nu, "u_max": u_max, "dtype": "f64"}
+            for eps in (1e-3, 1e-5):
+                ts, out, mode = [], None, "adaptive"
+                for _ in range(3):
+                    s.reset_state(); torch.cuda.synchronize(dev)
+                    t0 = time.perf_counter()
+                    try:
+                        out = s.solve_adaptive(1000, eps, eps)
+                    except Bd.TmpcError:                 # streamed class: fixed-count solves only
+                        mode = "fixed 200 iterations (adaptive schedule not available for the streamed class)"
+                        s.solve(200); torch.cuda.synchronize(dev)
+                    ts.append(time.perf_counter() - t0)
+                row[f"tol_{eps:g}"] = {"ms_per_batched_solve": 1e3 * min(ts), "mode": mode,
+                                       "iterations_median": float(np.median(out["iters"])) if out else 200.0, "iterations_max": int(out["iters"].max()) if out else 200,
+                                       "converged_frac": float(out["converged"].mean()) if out else None}
+            dLdx = 2.0 * s.s["x"]
+            ts = []
+            for _ in range(4):
+                s.factor(); torch.cuda.synchronize(dev)
+                t0 = time.perf_counter(); s.backward(dLdx); torch.cuda.synchronize(dev); ts.append(time.perf_counter() - t0)
+            row["backward_ms"] = 1e3 * min(ts[1:])
+            if (B, N, nx, nu) == (64, 40, 8, 4):          # closed loop: H = 50 MPC solves, each warm-started from the previous solution
+                A = s.t["Am"][:, 0, :, :nx]; Bm = s.t["Am"][:, 0, :, nx:]; bv = -s.t["b"][:, 0, :]
+                s.reset_state(); s.t["x_init"].copy_(s._up(w.x_init)); torch.cuda.synchronize(dev)
+                t0 = time.perf_counter(); its = 0
+                for hstep in range(50):
+                    out = s.solve_adaptive(1000, 1e-3, 1e-3, flags=Bd.TMPC_SOLVE_ZG_GIVEN if hstep else 0)
+                    its += int(out["iters"].max())
+                    u0 = s.s["x"][:, 0, nx:]
+                    xn = torch.einsum("bij,bj->bi", A, s.t["x_init"]) + torch.einsum("bij,bj->bi", Bm, u0) + bv      # the environment step (not the solver)
+                    s.t["x_init"].copy_(xn)
+                torch.cuda.synchronize(dev)
+                row["closed_loop_H50_tol_1e-3"] = {"ms_total": 1e3 * (time.perf_counter() - t0), "max_iterations_summed": its}
+            rows.append(row)
+            s.close()
+    return rows
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -383,9 +435,14 @@ def run_gpu(args):
            "peaks": measure_peaks(dev, torch.cuda.current_stream(dev)),
            "kernel_names": KERNEL_NAMES}
     res = []
-    for i, (c, d) in enumerate(config_list(args)):
+    for i, (c, d) in enumerate([] if args.f4_only else config_list(args)):
         steps = args.steps if (args.config is not None or i == 0) else max(3, min(args.steps, STEPS_CAP.get(c, args.steps)))
         res.append((c, d, gpu_one(c, d, args, ctx, steps, world == 1 and not args.no_cpu_baseline)))
+    f4 = f4_rows(ctx, args) if (args.config is None and world == 1 and not args.no_f4) or args.f4_only else None
+    if args.f4_only:
+        if rank == 0:
+            print(json.dumps({"metric": "f4 linear-system RL workload (PAPER.md:414-416)", "rows": f4, "measured_peaks": ctx["peaks"]}))
+        return
     if rank == 0:
         c0, d0, head = res[0]
         line = {"metric": "batched QP solves/s", "n_gpus": world, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "data": "synthetic"}
@@ -394,6 +451,8 @@ def run_gpu(args):
         if len(res) > 1:
             line["per_config"] = {key_of(c, d): r for c, d, r in res[1:]}
             line["gpu_launches"] = int(sum(r["gpu_launches"] for _, _, r in res))
+        if f4 is not None:
+            line.setdefault("per_config", {})["f4_linear_rl"] = f4
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -409,6 +468,8 @@ def main():
     ap.add_argument("--dtype", default=None, choices=[None, "f32", "f64"])
     ap.add_argument("--batch", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-f4", action="store_true", help="skip the f4 linear-system RL rows of the all-configs run")
+    ap.add_argument("--f4-only", action="store_true", help="run only the f4 linear-system RL rows")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -85,6 +85,7 @@ struct tmpc_ctx {
   tmpc_config cfg; Dims d; Layout lay; unsigned char* ws; cudaStream_t stream; bool factored; bool cr; bool twisted; int64_t launches;
   // set while tmpc_admm_solve_adaptive runs (f1): per-problem rho_bar, activity flags for the solve kernels, refactor mask for the factor kernels
   const void* cur_rho; const int32_t* cur_active; const int32_t* cur_mask;
+  cudaStream_t aux[2]; cudaEvent_t ev[3];       // tmpc_admm_solve_host: two sub-batches in flight (copies of one overlap the kernels of the other)
 };
 
 namespace {
@@ -139,15 +140,15 @@ tmpc_status launch_admm_inst(tmpc_ctx* h, const AdmmArgs<T>& a, int nt, size_t s
   k<<<h->d.B, nt, smem, h->stream>>>(a); h->launches++;
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
 }
-struct FastPlan { bool ok, v3; int pg, nt, ctas_per_sm; size_t smem; };   // v3: tmpc_admm3.cuh (n = 8), else tmpc_admm2.cuh (n = 6)
+struct FastPlan { bool ok; int pg, nt, ctas_per_sm; size_t smem; };
 template <typename T> FastPlan fast_plan(const Dims& d);
-template <typename T> tmpc_status launch_admm2(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f);
+template <typename T> tmpc_status launch_resident(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f);
 template <typename T> tmpc_status launch_residual(tmpc_ctx* h, const AdmmArgs<T>& s);
 template <typename T>
 tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
   const Dims& d = h->d;
-  if (h->twisted) {                      // the factor in the workspace is the twisted one: only admm2_kernel reads it
-    tmpc_status s = launch_admm2<T>(h, a, fast_plan<T>(d));
+  if (h->twisted) {                      // the factor in the workspace is the twisted one: only admm3_kernel reads it
+    tmpc_status s = launch_resident<T>(h, a, fast_plan<T>(d));
     if (s != TMPC_OK || a.kkt_only) return s;
     return launch_residual<T>(h, a);
   }
@@ -207,7 +208,7 @@ tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
   return launch_admm_inst<T, 0, false>(h, a, nt, smem_str);
 }
 
-// ---- resident fast path (tmpc_admm2.cuh): eligibility and launch shape
+// ---- resident fast path (tmpc_admm3.cuh): eligibility and launch shape
 constexpr size_t kSmemPerSM = 228 * 1024;
 template <typename T>
 FastPlan fast_plan(const Dims& d) {
@@ -215,7 +216,6 @@ FastPlan fast_plan(const Dims& d) {
   const bool shape = (d.n == 8 && d.nx == 6) || (d.n == 6 && d.nx == 4);
   if (!shape || d.ng > d.n || d.T < 2) return f;
   if (d.g_sel) for (int r = 0; r < d.ng; ++r) for (int q = 0; q < r; ++q) if (d.g_col[r] == d.g_col[q]) return f;   // one selection row per column
-  f.v3 = true;
   const size_t s1 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 1) : admm3_smem_bytes<T, 6, 4>(d, 1), s2 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 2) : admm3_smem_bytes<T, 6, 4>(d, 2);
   if (s1 > kMaxSmem) return f;
   const int c1 = (int)(kSmemPerSM / (s1 + 1024)), c2 = s2 <= kMaxSmem ? (int)(kSmemPerSM / (s2 + 1024)) : 0;
@@ -231,26 +231,6 @@ FastPlan fast_plan(const Dims& d) {
 }
 
 template <typename T, int NC, int NX, int PG, int MAXT, int MINB>
-tmpc_status launch_admm2_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
-  auto k = admm2_kernel<T, NC, NX, PG, MAXT, MINB>;
-  if (f.smem > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem) != cudaSuccess) return TMPC_E_CUDA;
-  const unsigned grid = (unsigned)((h->d.B + PG - 1) / PG);
-  Admm2Args<T> A; A.a = a; A.pl = admm2_plan<T, NC, NX>(h->d, PG);
-  A.rfa = a.prm.rho_f * a.prm.alpha; A.oma = T(1) - a.prm.alpha; A.inv_rho_g = T(1) / a.prm.rho_g; A.inv_rg = T(1) / (a.prm.rho_g + a.prm.gamma);
-  k<<<grid, f.nt, f.smem, h->stream>>>(A); h->launches++;
-  return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
-}
-template <typename T, int NC, int NX, int PG>
-tmpc_status launch_admm2_shape(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
-  if constexpr (sizeof(T) == 8) return launch_admm2_inst<T, NC, NX, PG, 512, 1>(h, a, f);
-  else {
-    if (f.nt <= 256 && f.ctas_per_sm >= 3) return launch_admm2_inst<T, NC, NX, PG, 256, 3>(h, a, f);
-    if (f.nt <= 384 && f.ctas_per_sm >= 3) return launch_admm2_inst<T, NC, NX, PG, 384, 3>(h, a, f);
-    if (f.nt <= 448) return launch_admm2_inst<T, NC, NX, PG, 448, 2>(h, a, f);
-    return launch_admm2_inst<T, NC, NX, PG, 1024, 1>(h, a, f);
-  }
-}
-template <typename T, int NC, int NX, int PG, int MAXT, int MINB>
 tmpc_status launch_admm3_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
   auto k = admm3_kernel<T, NC, NX, PG, MAXT, MINB>;
   if (f.smem > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem) != cudaSuccess) return TMPC_E_CUDA;
@@ -263,6 +243,10 @@ tmpc_status launch_admm3_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan&
 template <typename T, int NC, int NX, int PG>
 tmpc_status launch_admm3_shape(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
   if (f.nt <= 256) {
+    // a grid that leaves SMs idle anyway (config 1: one problem) takes the variant without a register cap: the capped ones spill for double
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return TMPC_E_CUDA;
+    if ((h->d.B + PG - 1) / PG <= sms) return launch_admm3_inst<T, NC, NX, PG, 256, 1>(h, a, f);
     if (f.ctas_per_sm >= 3) return launch_admm3_inst<T, NC, NX, PG, 256, 3>(h, a, f);
     if (f.ctas_per_sm >= 2) return launch_admm3_inst<T, NC, NX, PG, 256, 2>(h, a, f);
     return launch_admm3_inst<T, NC, NX, PG, 256, 1>(h, a, f);
@@ -270,12 +254,10 @@ tmpc_status launch_admm3_shape(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan
   return launch_admm3_inst<T, NC, NX, PG, 1024, 1>(h, a, f);
 }
 template <typename T>
-tmpc_status launch_admm2(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
+tmpc_status launch_resident(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
   const Dims& d = h->d;
-  if (f.v3 && d.n == 8) return f.pg == 2 ? launch_admm3_shape<T, 8, 6, 2>(h, a, f) : launch_admm3_shape<T, 8, 6, 1>(h, a, f);
-  if (f.v3 && d.n == 6) return f.pg == 2 ? launch_admm3_shape<T, 6, 4, 2>(h, a, f) : launch_admm3_shape<T, 6, 4, 1>(h, a, f);
-  if (d.n == 8 && d.nx == 6) return f.pg == 2 ? launch_admm2_shape<T, 8, 6, 2>(h, a, f) : launch_admm2_shape<T, 8, 6, 1>(h, a, f);
-  if (d.n == 6 && d.nx == 4) return f.pg == 2 ? launch_admm2_shape<T, 6, 4, 2>(h, a, f) : launch_admm2_shape<T, 6, 4, 1>(h, a, f);
+  if (d.n == 8) return f.pg == 2 ? launch_admm3_shape<T, 8, 6, 2>(h, a, f) : launch_admm3_shape<T, 8, 6, 1>(h, a, f);
+  if (d.n == 6) return f.pg == 2 ? launch_admm3_shape<T, 6, 4, 2>(h, a, f) : launch_admm3_shape<T, 6, 4, 1>(h, a, f);
   return TMPC_E_UNSUPPORTED;
 }
 template <typename T>
@@ -460,6 +442,7 @@ tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, vo
   h->cfg = *cfg; h->d = make_dims(*cfg); h->lay = L; h->ws = (unsigned char*)workspace; h->stream = (cudaStream_t)cuda_stream;
   h->factored = false; h->cr = use_cr(*cfg); h->twisted = false; h->launches = 0;
   h->cur_rho = nullptr; h->cur_active = nullptr; h->cur_mask = nullptr;
+  h->aux[0] = h->aux[1] = nullptr; h->ev[0] = h->ev[1] = h->ev[2] = nullptr;
   // zero buffers of the adjoint QP (x_init = 0, b = 0)
   if (cudaMemsetAsync(h->ws + L.zero_xinit, 0, L.zero_b - L.zero_xinit, h->stream) != cudaSuccess ||
       cudaMemsetAsync(h->ws + L.zero_b, 0, L.cr - L.zero_b, h->stream) != cudaSuccess) { delete h; return TMPC_E_CUDA; }
@@ -478,7 +461,13 @@ tmpc_status tmpc_measure_peak(int32_t what, void* scratch, void* cuda_stream, in
   return measure_peak(what, (float*)scratch, (cudaStream_t)cuda_stream, reps, out);
 }
 
-tmpc_status tmpc_destroy(tmpc_handle h) { delete h; return TMPC_OK; }
+tmpc_status tmpc_destroy(tmpc_handle h) {
+  if (h) {
+    for (int k = 0; k < 2; ++k) if (h->aux[k]) cudaStreamDestroy(h->aux[k]);
+    for (int k = 0; k < 3; ++k) if (h->ev[k]) cudaEventDestroy(h->ev[k]);
+  }
+  delete h; return TMPC_OK;
+}
 int64_t tmpc_launch_count(tmpc_handle h) { return h ? h->launches : 0; }
 
 tmpc_status tmpc_linearize(tmpc_handle h, const void* xbar, const void* stage_ref, tmpc_qp* qp) {
@@ -632,32 +621,71 @@ tmpc_status tmpc_host_staging_bytes(const tmpc_config* cfg, size_t* bytes) {
   return TMPC_OK;
 }
 
+// One sub-batch [p0, p0 + nb) of the host entry on stream `st`: copy in, factor + solve on a handle view of nb problems whose workspace
+// is `ws`, copy out.  The staging arrays are indexed by problem, so a sub-batch is a pointer offset into each of them.
+static tmpc_status host_sub_batch(tmpc_ctx* h, const HostPlan& P, const tmpc_qp* hq, tmpc_state* hs, tmpc_info* hi_, unsigned char* dv, int iters, int flags,
+                                  int p0, int nb, unsigned char* ws, cudaStream_t st, bool copy_shared) {
+  const size_t B = h->d.B;
+  tmpc_ctx sub = *h; sub.cfg.batch = nb; sub.d.B = nb; sub.lay = make_layout(sub.cfg); sub.ws = ws; sub.stream = st; sub.factored = false; sub.launches = 0;
+  const void* src[15] = { hq->D, hq->E, hq->q, hq->Am, hq->Ap, hq->b, hq->x_init, hq->G, hq->lo, hq->hi, hs->x, hs->zg, hs->yf, hs->yg, hs->xi };
+  const int64_t bstride[15] = { hq->D_bstride, hq->E_bstride, 1, 1, 1, 1, 1, hq->G_bstride, 1, 1, 1, 1, 1, 1, 1 };
+  auto per = [&](int i) { return P.bytes[i] / B; };                       // bytes per problem of a per-problem array
+  unsigned char* d_[19];
+  for (int i = 0; i < 19; ++i) d_[i] = dv + P.off[i] + ((i < 15 && bstride[i] == 0) ? 0 : (size_t)p0 * (P.bytes[i] / B));
+  for (int i = 0; i < 15; ++i) {
+    if (!src[i] || !P.bytes[i]) continue;
+    if ((i == 11 || i == 14) && !(flags & TMPC_SOLVE_ZG_GIVEN)) continue;      // zg, xi are outputs only
+    if (bstride[i] == 0) { if (copy_shared && cudaMemcpyAsync(dv + P.off[i], src[i], P.bytes[i], cudaMemcpyHostToDevice, st) != cudaSuccess) return TMPC_E_CUDA; continue; }
+    if (cudaMemcpyAsync(d_[i], (const unsigned char*)src[i] + (size_t)p0 * per(i), (size_t)nb * per(i), cudaMemcpyHostToDevice, st) != cudaSuccess) return TMPC_E_CUDA;
+  }
+  tmpc_qp dq = *hq;
+  dq.D = d_[0]; dq.E = d_[1]; dq.q = d_[2]; dq.Am = d_[3]; dq.Ap = d_[4]; dq.b = d_[5]; dq.x_init = d_[6]; dq.G = hq->G ? d_[7] : nullptr; dq.lo = d_[8]; dq.hi = d_[9];
+  tmpc_state ds = { d_[10], d_[11], d_[12], d_[13], d_[14] };
+  tmpc_info di = { d_[15], d_[16], d_[17], (int32_t*)d_[18] };
+  tmpc_status s = tmpc_factor(&sub, &dq); if (s != TMPC_OK) return s;
+  s = tmpc_admm_solve(&sub, &dq, &ds, iters, flags, &di); if (s != TMPC_OK) return s;
+  h->launches += sub.launches;
+  void* dst[5] = { hs->x, hs->zg, hs->yf, hs->yg, hs->xi };
+  for (int i = 0; i < 5; ++i) if (cudaMemcpyAsync((unsigned char*)dst[i] + (size_t)p0 * per(10 + i), d_[10 + i], (size_t)nb * per(10 + i), cudaMemcpyDeviceToHost, st) != cudaSuccess) return TMPC_E_CUDA;
+  if (hi_) {
+    void* idst[4] = { hi_->r_prim, hi_->r_dual, hi_->objective, hi_->status };
+    for (int i = 0; i < 4; ++i) if (idst[i] && cudaMemcpyAsync((unsigned char*)idst[i] + (size_t)p0 * per(15 + i), d_[15 + i], (size_t)nb * per(15 + i), cudaMemcpyDeviceToHost, st) != cudaSuccess) return TMPC_E_CUDA;
+  }
+  return TMPC_OK;
+}
+
 tmpc_status tmpc_admm_solve_host(tmpc_handle h, const tmpc_qp* hq, tmpc_state* hs, int32_t iters, int32_t flags, tmpc_info* hi_, void* staging, size_t staging_bytes) {
   tmpc_status s = check_qp(h, hq); if (s != TMPC_OK) return s;
   if (!hs || !hs->x || !hs->zg || !hs->yf || !hs->yg || !hs->xi || !staging || iters < 0) return TMPC_E_BADARG;
   const HostPlan P = host_plan(h->cfg, hq->D_bstride, hq->E_bstride, hq->G_bstride, hq->G != nullptr);
   if (staging_bytes < P.total || ((uintptr_t)staging & 255)) return TMPC_E_WORKSPACE;
   unsigned char* dv = (unsigned char*)staging;
-  const void* src[15] = { hq->D, hq->E, hq->q, hq->Am, hq->Ap, hq->b, hq->x_init, hq->G, hq->lo, hq->hi, hs->x, hs->zg, hs->yf, hs->yg, hs->xi };
-  for (int i = 0; i < 15; ++i) {
-    if (!src[i] || !P.bytes[i]) continue;
-    if ((i == 11 || i == 14) && !(flags & TMPC_SOLVE_ZG_GIVEN)) continue;      // zg, xi are outputs only
-    if (cudaMemcpyAsync(dv + P.off[i], src[i], P.bytes[i], cudaMemcpyHostToDevice, h->stream) != cudaSuccess) return TMPC_E_CUDA;
+  h->factored = false;                                    // the workspace is re-laid out per sub-batch below
+  // Two sub-batches on two internal streams, so that the host->device copy of the second overlaps the kernels of the first and
+  // the device->host copy of the first overlaps the kernels of the second.  Each half gets its own half of the workspace.
+  const int B = h->d.B, nb0 = (B + 1) / 2;
+  tmpc_config half = h->cfg; half.batch = nb0;
+  const size_t half_bytes = make_layout(half).total;
+  const bool split = B >= 64 && !h->cr && 2 * half_bytes <= h->lay.total;
+  if (!split) {
+    s = host_sub_batch(h, P, hq, hs, hi_, dv, iters, flags, 0, B, h->ws, h->stream, true); if (s != TMPC_OK) return s;
+    return cudaStreamSynchronize(h->stream) == cudaSuccess ? TMPC_OK : TMPC_E_CUDA;
   }
-  tmpc_qp dq = *hq;
-  dq.D = dv + P.off[0]; dq.E = dv + P.off[1]; dq.q = dv + P.off[2]; dq.Am = dv + P.off[3]; dq.Ap = dv + P.off[4]; dq.b = dv + P.off[5];
-  dq.x_init = dv + P.off[6]; dq.G = hq->G ? dv + P.off[7] : nullptr; dq.lo = dv + P.off[8]; dq.hi = dv + P.off[9];
-  tmpc_state ds = { dv + P.off[10], dv + P.off[11], dv + P.off[12], dv + P.off[13], dv + P.off[14] };
-  tmpc_info di = { dv + P.off[15], dv + P.off[16], dv + P.off[17], (int32_t*)(dv + P.off[18]) };
-  if (cudaMemsetAsync(di.status, 0, P.bytes[18], h->stream) != cudaSuccess) return TMPC_E_CUDA;
-  s = tmpc_factor(h, &dq); if (s != TMPC_OK) return s;
-  s = tmpc_admm_solve(h, &dq, &ds, iters, flags, &di); if (s != TMPC_OK) return s;
-  void* dst[5] = { hs->x, hs->zg, hs->yf, hs->yg, hs->xi };
-  for (int i = 0; i < 5; ++i) if (cudaMemcpyAsync(dst[i], dv + P.off[10 + i], P.bytes[10 + i], cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) return TMPC_E_CUDA;
-  if (hi_) {
-    void* idst[4] = { hi_->r_prim, hi_->r_dual, hi_->objective, hi_->status };
-    for (int i = 0; i < 4; ++i) if (idst[i] && cudaMemcpyAsync(idst[i], dv + P.off[15 + i], P.bytes[15 + i], cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) return TMPC_E_CUDA;
+  for (int k = 0; k < 2; ++k) if (!h->aux[k] && cudaStreamCreateWithFlags(&h->aux[k], cudaStreamNonBlocking) != cudaSuccess) return TMPC_E_CUDA;
+  for (int k = 0; k < 3; ++k) if (!h->ev[k] && cudaEventCreateWithFlags(&h->ev[k], cudaEventDisableTiming) != cudaSuccess) return TMPC_E_CUDA;
+  // batch-shared arrays (D, E, G with a zero batch stride) go in once on the handle's stream; both sub-batch streams start after them
+  {
+    const void* ssrc[3] = { hq->D, hq->E, hq->G }; const int sidx[3] = { 0, 1, 7 }; const int64_t sstr[3] = { hq->D_bstride, hq->E_bstride, hq->G_bstride };
+    for (int i = 0; i < 3; ++i) if (ssrc[i] && sstr[i] == 0 && P.bytes[sidx[i]] &&
+                                    cudaMemcpyAsync(dv + P.off[sidx[i]], ssrc[i], P.bytes[sidx[i]], cudaMemcpyHostToDevice, h->stream) != cudaSuccess) return TMPC_E_CUDA;
   }
+  if (cudaEventRecord(h->ev[2], h->stream) != cudaSuccess) return TMPC_E_CUDA;           // order after whatever the caller queued
+  for (int k = 0; k < 2; ++k) if (cudaStreamWaitEvent(h->aux[k], h->ev[2], 0) != cudaSuccess) return TMPC_E_CUDA;
+  s = host_sub_batch(h, P, hq, hs, hi_, dv, iters, flags, 0, nb0, h->ws, h->aux[0], false); if (s != TMPC_OK) return s;
+  if (cudaEventRecord(h->ev[0], h->aux[0]) != cudaSuccess) return TMPC_E_CUDA;
+  s = host_sub_batch(h, P, hq, hs, hi_, dv, iters, flags, nb0, B - nb0, h->ws + half_bytes, h->aux[1], false); if (s != TMPC_OK) return s;
+  if (cudaEventRecord(h->ev[1], h->aux[1]) != cudaSuccess) return TMPC_E_CUDA;
+  for (int k = 0; k < 2; ++k) if (cudaStreamWaitEvent(h->stream, h->ev[k], 0) != cudaSuccess) return TMPC_E_CUDA;
   return cudaStreamSynchronize(h->stream) == cudaSuccess ? TMPC_OK : TMPC_E_CUDA;
 }
 

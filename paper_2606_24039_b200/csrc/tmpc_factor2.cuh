@@ -30,7 +30,7 @@ namespace tmpc {
 // TW = true: twisted factor (X_t, B_t) for admm2_kernel.  TW = false: the one-directional block LDL' of factor_kernel
 // (Lam_t = Phi_t Sigma_t^{-1}, Sinv_t = Sigma_t^{-1}; per-row weights w_rows supported) for the backward pass; one warp.
 template <typename T, int NC, int NX, bool TW>
-__global__ void __launch_bounds__(64) factor_tw2_kernel(FactorArgs<T> a) {
+__global__ void __launch_bounds__(64, 12) factor_tw2_kernel(FactorArgs<T> a) {
   constexpr int n = NC, nx = NX, nn = NC * NC, an = NX * NC;
   constexpr int EPL = (nn + 31) / 32;                   // matrix elements per lane
   constexpr int GMAX = NC * NC;                         // room for ng <= n rows of G

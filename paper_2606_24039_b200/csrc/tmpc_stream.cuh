@@ -53,7 +53,6 @@ __host__ inline StreamPlan stream_plan(const Dims& d, size_t max_smem) {
   // (measured at config 3: two CTAs per SM with 2 slots 116 ms, one CTA with 6 slots 144 ms), so take the deepest ring
   // that still lets two CTAs share an SM
   for (int k = smax; k >= 2; --k) if (2 * (fixed + k * tile + 1024) <= (size_t)228 * 1024) { P.slots = k; break; }
-  if (const char* e = getenv("TMPC_STREAM_SLOTS")) { const int v = atoi(e); if (v >= 2 && v <= smax) P.slots = v; }   // tuning knob
   P.smem = fixed + (size_t)(P.slots > 0 ? P.slots : 0) * tile;
   return P;
 }

@@ -399,3 +399,34 @@ def with_dense_Ap(w: QPData, seed: int = 0, scale: float = 0.05) -> QPData:
     out.Ap[:, :, :, w.nx:] = scale * st.normal(w.N * w.nx * w.nu).reshape(w.B, w.N, w.nx, w.nu)
     out.name = w.name + "_denseAp"
     return out
+
+
+# --------------------------------------------------------------------------- f4: the paper's linear-system RL generator
+def linear_rl(seed: int = 0, B: int = 64, N: int = 40, nx: int = 8, nu: int = 4, u_max: float = 1.0, theta: float = 1.0,
+              dtype: str = "f64", first_problem: int = 0) -> QPData:
+    """Linear-quadratic OCP batch of the paper's scaling study (Sec. IV-B): time-invariant
+    x+ = A x + B u + b per problem with A = I + 0.1 dA, vec(dA) ~ N(0, I), eigenvalues clipped to |lambda| <= 0.99,
+    vec(B) ~ N(0, I), b ~ N(0, 1e-4 I), x0 ~ N(0, 25 I); stage cost x'Qx + |u|^2 with Q = diag(theta) (all stages, u_N
+    included, reading A-10), i.e. D = 2 blkdiag(Q, I) in the 1/2-convention (A-9); hard bounds |u|_inf <= u_max.
+    Draw order per problem: dA (row-major), B, b, x0.  Nominal shape (B, N, nx, nu) = (64, 40, 8, 4)."""
+    n, T = nx + nu, N + 1
+    st = Streams(seed, 11, np.arange(first_problem, first_problem + B))
+    dA = st.normal(nx * nx).reshape(B, nx, nx)
+    Bm = st.normal(nx * nu).reshape(B, nx, nu)
+    bv = 0.01 * st.normal(nx)
+    x0 = 5.0 * st.normal(nx)
+    A = np.eye(nx) + 0.1 * dA
+    lam, V = np.linalg.eig(A)                                        # clip the spectrum: |lambda| in (0, 0.99]
+    scale = np.minimum(1.0, 0.99 / np.maximum(np.abs(lam), 1e-300))
+    A = np.real(np.einsum("bij,bj,bjk->bik", V, lam * scale, np.linalg.inv(V)))
+    Am = np.zeros((B, N, nx, n))
+    Ap = np.zeros((B, N, nx, n))
+    Am[:, :, :, :nx] = A[:, None]
+    Am[:, :, :, nx:] = Bm[:, None]
+    Ap[:, :, :, :nx] = -np.eye(nx)
+    b = np.broadcast_to(-bv[:, None, :], (B, N, nx)).copy()
+    D, E = _rate_cost_blocks(T, nx, nu, 2.0 * theta * np.eye(nx), 2.0 * np.eye(nu), None)
+    lo = np.full((B, T, nu), -u_max)
+    hi = np.full((B, T, nu), u_max)
+    return QPData(f"f4_linear_rl_umax{u_max:g}", B, N, nx, nu, nu, dtype, D, E, np.zeros((B, T, n)), Am, Ap, b, x0, None, lo, hi,
+                  g_col=list(range(nx, n)), soft=[0] * nu, iters=100)

@@ -590,3 +590,37 @@ def test_adaptive_termination_only_and_fp32():
     assert (out["iters"] == rinfo[:, 4].astype(int)).sum() >= w.B // 2, (out["iters"], rinfo[:, 4])   # a diverged accept/reject decision changes the path
     compare_states(s.state_numpy(), ref, 2e-3)
     s.close()
+
+
+# ----------------------------------------------------------------------------------------------- f4: the paper's linear-system RL workload
+@pytest.mark.parametrize("u_max", [1.0, 10.0])
+def test_f4_linear_rl_nominal_shape(u_max):
+    """PAPER.md:414-416 generator at the nominal block size (nx, nu) = (8, 4), N = 40: fixed-count iterates (both dtypes), the adaptive
+    run to tol 1e-5 with at most 1000 iterations (the paper's setting) and the backward pass against the oracle."""
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    w = W.linear_rl(B=6, N=40, u_max=u_max)
+    run_pair(w, "f64", iters=100)
+    run_pair(w, "f32", iters=100)
+    ref, rinfo, log, rc = O.admm_adaptive(w, O.make_cfg(w), O.make_adaptive(1000, 1e-5, 1e-5))
+    s = Solver(w, dtype="f64")
+    out = s.solve_adaptive(1000, 1e-5, 1e-5)
+    assert (out["iters"] == rinfo[:, 4].astype(int)).all() and (out["converged"] == 1).all()
+    compare_states(s.state_numpy(), ref, 1e-7)
+    # backward at the converged solution (tight solve first so that the active set is unambiguous)
+    cfg = O.make_cfg(w)
+    ref, info, rc = O.admm(w, O.make_cfg(w, rho_bar=5.0), iters=4000)
+    dq_o, dxi_o, counts, rcs = O.backward(w, cfg, ref, 2.0 * ref["x"])
+    ok = rcs == 0
+    assert ok.sum() >= 3
+    s.set_state(ref)
+    dq, dxi = s.backward(s._up(2.0 * ref["x"]), mode=Bd.TMPC_BWD_REFACTOR_REFINE)
+    assert rel_err(dq.cpu().double().numpy()[ok], dq_o[ok]) <= 1e-9 and rel_err(dxi.cpu().double().numpy()[ok], dxi_o[ok]) <= 1e-9
+    s.close()
+
+
+def test_f4_linear_rl_sweep_shapes_fp32():
+    """The sweep's other block sizes: (nx, nu) = (4, 2), (16, 8) and (32, 16) at short horizons, fixed iteration count."""
+    run_pair(W.linear_rl(B=5, N=12, nx=4, nu=2, u_max=1.0), "f32", iters=60)
+    run_pair(W.linear_rl(B=3, N=10, nx=16, nu=8, u_max=10.0), "f32", iters=60)
+    run_pair(W.linear_rl(B=2, N=8, nx=32, nu=16, u_max=1.0), "f32", iters=60, band=1)
