@@ -183,6 +183,28 @@ def admm_adaptive(w, cfg, ad, state=None, max_log=256):
     return st, info, log, rc
 
 
+class SqpOpt(C.Structure):
+    _fields_ = [("max_sqp", C.c_int32), ("admm_iters", C.c_int32), ("n_alpha", C.c_int32), ("pad", C.c_int32), ("eps_c", C.c_double), ("eta", C.c_double)]
+
+
+def sqp_linesearch_bicycle(w, cfg, max_sqp=10, admm_iters=50, eps_c=1e-3, n_alpha=8, eta=0.4, xbar0=None):
+    """f2 on every problem.  Returns (state with x = final iterate, info [B,5] = iterations, converged, stationarity, |f|_inf, violation,
+    log [B,max_sqp,10] = alpha, mu, phi0, phi(alpha), c1, dl, accepted, stat, |f|_inf, viol, rc)."""
+    n, T, nz, mf, mg = _dims(w)
+    assert lib().orc_sizeof_sqpopt() == C.sizeof(SqpOpt)
+    op = SqpOpt(max_sqp, admm_iters, n_alpha, 0, eps_c, eta)
+    st = new_state(w); st["x"] = _c(w.xbar0 if xbar0 is None else xbar0).copy()
+    info = np.zeros((w.B, 5)); log = np.zeros((w.B, max_sqp, 10))
+    D, E, q, x0, ref = _c(w.D[0]), _c(w.E[0]), _c(w.q), _c(w.x_init), _c(w.stage_ref)
+    fn = lib().orc_sqp_ls_bicycle
+    fn.argtypes = [C.c_void_p] * 14
+    rc = 0
+    for b in range(w.B):
+        rc |= fn(C.byref(cfg), C.byref(op), _p(D), _p(E), _p(q[b]), _p(x0[b]), _p(ref[b]), _p(st["x"][b]), _p(st["zg"][b]), _p(st["yf"][b]),
+                 _p(st["yg"][b]), _p(st["xi"][b]), _p(info[b]), _p(log[b]))
+    return st, info, log, rc
+
+
 def backward(w, cfg, state, dLdx, dLdxi=None):
     """O-5 on every problem.  Returns dq [B,T,n], dxinit [B,nx], counts [B,2], rc [B]."""
     n, T, nz, mf, mg = _dims(w)

@@ -18,6 +18,7 @@
 //   O-4  SQP        fixed-count full-step driver around O-1..O-3 with the bicycle model linearised
 //                   by eq. 36-38.
 //   f1   adaptive   Alg. 3 with the adaptive step size of eq. 17 and the termination test eq. 4 (admm_adaptive).
+//   f2   SQP + linesearch   App. D l1-merit backtracking and the convergence test eq. 18 (sqp_ls_bicycle).
 //   O-5  backward   the definition: dense active-set KKT system eq. 62 / 65 solved by
 //                   Gaussian elimination with partial pivoting; dL/dq = -eta_x, dL/dx_init = +eta_f[0:nx].
 //
@@ -397,6 +398,87 @@ void bicycle_linearize(const Cfg& cf, const double* xbar, const double* ref, dou
   }
 }
 
+// ---- f2: SQP with the l1-merit backtracking linesearch of App. D and the convergence test eq. 18
+// (PAPER.md:305-314), for the bicycle model.  Readings (A-34..A-37):
+//   x~ = (x, xi); l(x~) = 1/2 x'Px + q'x + sum_soft (lam |xi| + gamma/2 xi^2); f(x~) = (x_0 - x_init ; f_k(v_k, v_{k+1}));
+//   g(x~) = G x + xi on soft rows, G x on hard rows (g is linear for this model, so the shifted bounds of eq. 38 are exact);
+//   c1 = |f|_1 + |[g - hi]_+|_1 + |[lo - g]_+|_1;  dl = (Px + q)'dx + sum_soft (lam s_i + gamma xi_i) dxi_i with s_i = sgn(xi_i), or
+//   sgn(dxi_i) where xi_i = 0 (one-sided derivative of |.|);  mu = max(0, dl / (1/2 max(c1, eps_c)));  D_mu = dl - mu c1;
+//   candidates alpha_j = 2^-j, j = 0..J-1: the largest with phi(x~ + alpha d) <= phi(x~) + eta alpha D_mu, else the one with the smallest phi;
+//   (x, xi, y_f, y_g) <- (x, xi, y_f, y_g) + alpha ((x*, xi*, y_f*, y_g*) - (x, xi, y_f, y_g)).
+//   eq. 18 at the new iterate, with the Jacobians re-linearised there: |Px + q + C'y_f + G'y_g|_inf, |f|_inf, max bound violation, all <= eps_c.
+struct SqpOpt { int32_t max_sqp, admm_iters, n_alpha, pad; double eps_c, eta; };
+
+double merit_parts(const Cfg& c, const Band& P, const vec& q, const double* x_init, const double* x, const double* xi, const double* G, const double* lo,
+                   const double* hi, double* cost_out, double* finf_out, double* ginf_out) {
+  const int N = c.N, T = N + 1, n = 6, nx = 4, ng = 3, nz = T * n;
+  vec xv(x, x + nz), Px(nz); band_mul(P, xv, Px);
+  double cost = 0; for (int i = 0; i < nz; ++i) cost += 0.5 * x[i] * Px[i] + q[i] * x[i];
+  double c1 = 0, finf = 0, ginf = 0, f[4];
+  for (int i = 0; i < nx; ++i) { double r = x[i] - x_init[i]; c1 += std::fabs(r); finf = std::max(finf, std::fabs(r)); }
+  for (int t = 0; t < N; ++t) { bicycle_residual(c.wheelbase, c.dt, x + (size_t)t * n, x + (size_t)(t + 1) * n, f); for (int i = 0; i < 4; ++i) { c1 += std::fabs(f[i]); finf = std::max(finf, std::fabs(f[i])); } }
+  for (int t = 0; t < T; ++t) for (int r = 0; r < ng; ++r) {
+    const int e = t * ng + r; double g = 0; for (int j = 0; j < n; ++j) g += G[(size_t)e * n + j] * x[t * n + j];
+    if (c.soft[r]) { g += xi[e]; cost += c.lam * std::fabs(xi[e]) + 0.5 * c.gamma * xi[e] * xi[e]; }
+    double v = std::max(0.0, g - hi[e]) + std::max(0.0, lo[e] - g);
+    c1 += v; ginf = std::max(ginf, v);
+  }
+  *cost_out = cost; if (finf_out) *finf_out = finf; if (ginf_out) *ginf_out = ginf;
+  return c1;
+}
+
+// log_out (optional): 10 doubles per SQP iteration: alpha, mu, phi0, phi(alpha), c1, dl, armijo-accepted flag, then eq. 18 after the step: stat, |f|_inf, viol
+int sqp_ls_bicycle(const Cfg& cf_in, const SqpOpt& op, const double* D, const double* E, const double* q_, const double* x_init, const double* ref, double* xbar,
+                   double* zg, double* yf, double* yg, double* xi, double* info_out, double* log_out) {
+  Cfg c = cf_in; c.g_sel = 0; c.zg_given = 0;
+  const int N = c.N, T = N + 1, n = 6, nx = 4, ng = 3, nz = T * n, mf = nx + N * nx, mg = T * ng;
+  vec Am((size_t)N * nx * n), Ap((size_t)N * nx * n), b((size_t)N * nx), G((size_t)T * ng * n), lo(mg), hi(mg), q(q_, q_ + nz);
+  vec xs(nz), zs(mg), yfs(mf), ygs(mg), xis(mg), xc(nz), xic(mg), g(nz), Px(nz);
+  int fail = 0, it = 0, converged = 0;
+  double stat = 0, finf = 0, ginf = 0;
+  for (it = 0; it < op.max_sqp && !converged; ) {
+    bicycle_linearize(c, xbar, ref, Am.data(), Ap.data(), b.data(), G.data(), lo.data(), hi.data());
+    QP p = assemble(c, D, E, q.data(), Am.data(), Ap.data(), b.data(), x_init, G.data(), lo.data(), hi.data());
+    // QP solve (Alg. 3) warm-started at (xbar, y); the solution goes to (xs, xis, yfs, ygs)
+    std::copy(xbar, xbar + nz, xs.begin()); std::copy(yf, yf + mf, yfs.begin()); std::copy(yg, yg + mg, ygs.begin());
+    double inf4[4]; Info ai = admm(c, p, xs.data(), zs.data(), yfs.data(), ygs.data(), xis.data(), op.admm_iters); (void)inf4;
+    if (!(ai.min_pivot > 0)) fail = 1;
+    // linesearch (App. D)
+    double cost0, c1 = merit_parts(c, p.P, q, x_init, xbar, xi, G.data(), lo.data(), hi.data(), &cost0, nullptr, nullptr);
+    vec xb(xbar, xbar + nz); band_mul(p.P, xb, Px);
+    double dl = 0; for (int i = 0; i < nz; ++i) dl += (Px[i] + q[i]) * (xs[i] - xbar[i]);
+    for (int e = 0; e < mg; ++e) if (c.soft[e % ng]) { double dxi = xis[e] - xi[e]; double sg = xi[e] > 0 ? 1.0 : (xi[e] < 0 ? -1.0 : (dxi > 0 ? 1.0 : (dxi < 0 ? -1.0 : 0.0))); dl += (c.lam * sg + c.gamma * xi[e]) * dxi; }
+    const double mu = std::max(0.0, dl / (0.5 * std::max(c1, op.eps_c))), phi0 = cost0 + mu * c1, Dmu = dl - mu * c1;
+    double alpha = 0, best_phi = std::numeric_limits<double>::infinity(), best_alpha = 1.0, phi_a = 0; int accepted = 0;
+    for (int j = 0; j < op.n_alpha && !accepted; ++j) {
+      const double a = std::ldexp(1.0, -j);
+      for (int i = 0; i < nz; ++i) xc[i] = xbar[i] + a * (xs[i] - xbar[i]);
+      for (int e = 0; e < mg; ++e) xic[e] = xi[e] + a * (xis[e] - xi[e]);
+      double costa, c1a = merit_parts(c, p.P, q, x_init, xc.data(), xic.data(), G.data(), lo.data(), hi.data(), &costa, nullptr, nullptr);
+      const double phi = costa + mu * c1a;
+      if (phi < best_phi) { best_phi = phi; best_alpha = a; }
+      if (phi <= phi0 + op.eta * a * Dmu) { alpha = a; phi_a = phi; accepted = 1; }
+    }
+    if (!accepted) { alpha = best_alpha; phi_a = best_phi; }
+    for (int i = 0; i < nz; ++i) xbar[i] += alpha * (xs[i] - xbar[i]);
+    for (int e = 0; e < mg; ++e) { xi[e] += alpha * (xis[e] - xi[e]); yg[e] += alpha * (ygs[e] - yg[e]); zg[e] = zs[e]; }
+    for (int e = 0; e < mf; ++e) yf[e] += alpha * (yfs[e] - yf[e]);
+    ++it;
+    // eq. 18 at the new iterate (Jacobians re-linearised there)
+    bicycle_linearize(c, xbar, ref, Am.data(), Ap.data(), b.data(), G.data(), lo.data(), hi.data());
+    QP pn = assemble(c, D, E, q.data(), Am.data(), Ap.data(), b.data(), x_init, G.data(), lo.data(), hi.data());
+    vec xn(xbar, xbar + nz), yfv(yf, yf + mf), ygv(yg, yg + mg); band_mul(pn.P, xn, Px);
+    for (int i = 0; i < nz; ++i) g[i] = Px[i] + q[i];
+    pn.C.mulT_add(yfv, g); pn.G.mulT_add(ygv, g);
+    stat = 0; for (int i = 0; i < nz; ++i) stat = std::max(stat, std::fabs(g[i]));
+    double cdummy; merit_parts(c, pn.P, q, x_init, xbar, xi, G.data(), lo.data(), hi.data(), &cdummy, &finf, &ginf);
+    converged = stat <= op.eps_c && finf <= op.eps_c && ginf <= op.eps_c;
+    if (log_out) { double* l = log_out + 10 * (it - 1); l[0] = alpha; l[1] = mu; l[2] = phi0; l[3] = phi_a; l[4] = c1; l[5] = dl; l[6] = accepted; l[7] = stat; l[8] = finf; l[9] = ginf; }
+  }
+  info_out[0] = it; info_out[1] = converged; info_out[2] = stat; info_out[3] = finf; info_out[4] = ginf;
+  return fail;
+}
+
 }  // namespace
 
 extern "C" {
@@ -520,6 +602,13 @@ int orc_admm_adaptive(const Cfg* cf, const Adaptive* ad, const double* D, const 
   return admm_adaptive(*cf, p, *ad, x, zg, yf, yg, xi, info_out, log_out, max_log);
 }
 int orc_sizeof_adaptive() { return (int)sizeof(Adaptive); }
+
+// f2 for one problem.  info_out[5] = SQP iterations, converged, eq. 18 quantities (stationarity, |f|_inf, bound violation); log_out [max_sqp][10].
+int orc_sqp_ls_bicycle(const Cfg* cf, const SqpOpt* op, const double* D, const double* E, const double* q, const double* x_init, const double* ref, double* xbar,
+                       double* zg, double* yf, double* yg, double* xi, double* info_out, double* log_out) {
+  return sqp_ls_bicycle(*cf, *op, D, E, q, x_init, ref, xbar, zg, yf, yg, xi, info_out, log_out);
+}
+int orc_sizeof_sqpopt() { return (int)sizeof(SqpOpt); }
 
 int orc_sizeof_cfg() { return (int)sizeof(Cfg); }
 

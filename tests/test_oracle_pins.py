@@ -620,3 +620,82 @@ def test_sqp_driver_reduces_dynamics_residual_and_is_consistent_with_admm():
         for k in ("x", "zg", "yf", "yg", "xi"):
             assert np.abs(s[k][0] - st3[k][b]).max() < 1e-12 * max(1.0, np.abs(st3[k][b]).max()), k
         assert np.abs(st3["yf"][b]).max() > 1e-3                # the carried multipliers are not trivially zero
+
+
+# ----------------------------------------------------------------------------------------------- f2: SQP with linesearch (App. D) and eq. 18
+def _bicycle_f(w, x):
+    """Stacked equality residual (x_0 - x_init ; implicit-midpoint bicycle residuals), numpy, for one problem x [T,6]."""
+    vk, vk1 = x[:-1], x[1:]
+    psi, v = 0.5 * (vk[:, 2] + vk1[:, 2]), 0.5 * (vk[:, 3] + vk1[:, 3])
+    F = np.stack([v * np.cos(psi), v * np.sin(psi), v / w.wheelbase * np.tan(vk[:, 5]), vk[:, 4]], axis=1)
+    return x[0, :4].copy(), vk[:, :4] + w.dt * F - vk1[:, :4]
+
+
+def _merit_parts(w, b, P, q, x, xi, G, lo, hi):
+    """cost l(x~) and c1 = |f|_1 + |[g - hi]_+|_1 + |[lo - g]_+|_1 (App. D) in numpy."""
+    soft = np.array(w.soft, dtype=bool)
+    xf = x.ravel()
+    cost = 0.5 * xf @ P @ xf + q @ xf + (w.lam * np.abs(xi[:, soft]) + 0.5 * w.gamma * xi[:, soft] ** 2).sum()
+    f0, fk = _bicycle_f(w, x)
+    g = np.einsum("trn,tn->tr", G, x) + np.where(soft, xi, 0.0)
+    viol = np.maximum(0.0, g - hi) + np.maximum(0.0, lo - g)
+    return cost, np.abs(f0 - w.x_init[b]).sum() + np.abs(fk).sum() + viol.sum(), max(np.abs(f0 - w.x_init[b]).max(), np.abs(fk).max()), viol.max()
+
+
+def test_sqp_linesearch_steps_recomputed_in_numpy():
+    """Every SQP iteration of one run: the QP solution comes from the pinned pieces (bicycle_linearize + Alg. 3), the merit function,
+    mu, D_mu, the Armijo test over alpha = 2^-j (eta = 0.4), the fallback to the smallest merit and the update of (x, xi, y) are retyped
+    here from App. D; the convergence quantities of eq. 18 are recomputed with the Jacobians at the new iterate."""
+    import copy
+    w = W.config4(B=1, N=16, dtype="f64")
+    x0 = w.xbar0.copy(); x0[:, :, :2] += np.random.default_rng(0).normal(0, 1.5, x0[:, :, :2].shape); x0[:, :, 2] += 0.3
+    cfg = O.make_cfg(w)
+    K, eps_c, nA, eta, nsqp = 200, 1e-3, 8, 0.4, 30
+    st_all, info, log, rc = O.sqp_linesearch_bicycle(w, cfg, max_sqp=nsqp, admm_iters=K, eps_c=eps_c, n_alpha=nA, eta=eta, xbar0=x0)
+    assert rc == 0
+    soft = np.array(w.soft, dtype=bool)
+    cur = O.new_state(w); cur["x"] = x0.copy()
+    seen_backtrack = False
+    for it in range(int(info[0, 0])):
+        Am, Ap, bb, G, lo, hi = O.bicycle_linearize(w, cfg, cur["x"][0], 0)
+        wq = copy.copy(w)
+        wq.Am, wq.Ap, wq.b, wq.G, wq.lo, wq.hi, wq.model = Am[None], Ap[None], bb[None], G[None], lo[None], hi[None], 0
+        s0 = {k: v.copy() for k, v in cur.items()}
+        sol, _, _ = O.admm(wq, O.make_cfg(wq), iters=K, state=s0)
+        P, C, c, Gd = dense_PCG(wq, 0)
+        q = w.q[0].ravel()
+        x, xi = cur["x"][0], cur["xi"][0]
+        dx, dxi = sol["x"][0] - x, sol["xi"][0] - xi
+        cost0, c1, _, _ = _merit_parts(w, 0, P, q, x, xi, G, lo, hi)
+        sg = np.where(xi != 0, np.sign(xi), np.sign(dxi))
+        dl = (P @ x.ravel() + q) @ dx.ravel() + ((w.lam * sg + w.gamma * xi) * dxi)[:, soft].sum()
+        mu = max(0.0, dl / (0.5 * max(c1, eps_c)))
+        phi0, Dmu = cost0 + mu * c1, dl - mu * c1
+        phis = []
+        for j in range(nA):
+            a = 2.0 ** -j
+            ca, c1a, _, _ = _merit_parts(w, 0, P, q, x + a * dx, xi + a * dxi, G, lo, hi)
+            phis.append(ca + mu * c1a)
+        ok = [j for j in range(nA) if phis[j] <= phi0 + eta * 2.0 ** -j * Dmu]
+        jstar = ok[0] if ok else int(np.argmin(phis))
+        alpha = 2.0 ** -jstar
+        seen_backtrack |= alpha < 1.0
+        assert log[0, it, 0] == alpha and bool(log[0, it, 6]) == bool(ok), (it, log[0, it], alpha)
+        assert abs(log[0, it, 1] - mu) <= 1e-9 * max(1, abs(mu)) and abs(log[0, it, 2] - phi0) <= 1e-9 * abs(phi0) and abs(log[0, it, 4] - c1) <= 1e-9 * max(1, c1)
+        for k in ("x", "xi", "yf", "yg"):
+            cur[k] = cur[k] + alpha * (sol[k] - cur[k])
+        cur["zg"] = sol["zg"]
+        # eq. 18 at the new iterate
+        Am, Ap, bb, G, lo, hi = O.bicycle_linearize(w, cfg, cur["x"][0], 0)
+        wq.Am, wq.Ap, wq.b, wq.G, wq.lo, wq.hi = Am[None], Ap[None], bb[None], G[None], lo[None], hi[None]
+        P, C, c, Gd = dense_PCG(wq, 0)
+        stat = np.abs(P @ cur["x"][0].ravel() + q + C.T @ cur["yf"][0] + Gd.T @ cur["yg"][0].ravel()).max()
+        _, _, finf, ginf = _merit_parts(w, 0, P, q, cur["x"][0], cur["xi"][0], G, lo, hi)
+        for got, ref in ((log[0, it, 7], stat), (log[0, it, 8], finf), (log[0, it, 9], ginf)):
+            assert abs(got - ref) <= 1e-9 * max(1.0, abs(ref))
+        conv = stat <= eps_c and finf <= eps_c and ginf <= eps_c
+        assert conv == (it == int(info[0, 0]) - 1 and bool(info[0, 1]))
+    for k in ("x", "xi", "yf", "yg"):
+        assert np.abs(cur[k] - st_all[k]).max() <= 1e-10 * max(1.0, np.abs(st_all[k]).max()), k
+    assert info[0, 1] == 1 and info[0, 3] <= eps_c, "the run must converge by eq. 18"
+    print("alphas", log[0, :int(info[0, 0]), 0], "backtracked", seen_backtrack)
