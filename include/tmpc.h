@@ -124,6 +124,22 @@ typedef struct {
  * TMPC_E_UNSUPPORTED for the streamed class (stage blocks that do not fit in shared memory) and for cyclic reduction. */
 tmpc_status tmpc_admm_solve_adaptive(tmpc_handle h, const tmpc_qp* qp, tmpc_state* st, const tmpc_adaptive* ad, int32_t flags, tmpc_info* info,
                                      int32_t* iters_out, int32_t* converged_out, void* rho_out);
+/* f2 — the SQP outer loop of Alg. 1 for the built-in model: per iteration tmpc_linearize at the iterate st.x,
+ * tmpc_factor, `admm_iters` iterations of Alg. 3 warm-started there (y carried, z_g re-projected), then the backtracking linesearch of
+ * App. D on the l1 merit function with the candidates alpha = 2^-j, j < n_alpha, evaluated in parallel: the largest
+ * that satisfies the Armijo condition with eta, else the one with the smallest merit; (x, xi, y) move by alpha along the QP step.
+ * A problem stops when eq. 18 holds at its iterate: stationarity, |f|_inf and the bound violation all <= eps_c. */
+typedef struct {
+  int32_t max_sqp, admm_iters, n_alpha, reserved;   /* n_alpha <= 15 */
+  double eps_c, eta;                                /* eq. 18 tolerance; Armijo parameter (paper: 0.4) */
+} tmpc_sqp_opts;
+/* st.x holds the start iterate and receives the final one (st.yf, st.yg, st.xi likewise); qp->Am, Ap, b, G, lo, hi are written every
+ * iteration (as by tmpc_linearize).  Outputs (DEVICE, any may be NULL): SQP iterations per problem [B], eq. 18 met [B], the accepted alpha
+ * of every iteration [B][max_sqp] and the eq. 18 quantities of the last test [B][3] (working dtype).  Like tmpc_admm_solve_adaptive the
+ * call SYNCHRONISES once per iteration (count of live problems) and leaves the workspace factor unusable for a later tmpc_admm_solve.
+ * TMPC_E_UNSUPPORTED without a built-in model or with cyclic reduction. */
+tmpc_status tmpc_sqp_solve(tmpc_handle h, tmpc_qp* qp, tmpc_state* st, const void* stage_ref, const tmpc_sqp_opts* o, int32_t* iters_out,
+                           int32_t* converged_out, void* alpha_log, void* kkt_out);
 /* a10 (Alg. 2, eq. 59-65): dL/dq [B][T][n] and dL/dx_init [B][nx] from dL/dx [B][T][n] (and dL/dxi [B][T][ng] or NULL)
  * at the state st.  dL/dxi is the gradient with respect to the SIGNED slack st.xi that tmpc_admm_solve returns
  * (lo <= Gx + xi <= hi; App. E's xi_A of eq. 54 is |xi| = sign(xi) xi, so eq. 65's S dL/dxi_A is dL/dxi); only its

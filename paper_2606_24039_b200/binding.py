@@ -22,7 +22,7 @@ TMPC_BWD_REFACTOR_REFINE, TMPC_BWD_ADMM_REUSE_FACTOR = 0, 1
 TMPC_SOLVE_ZG_GIVEN = 1
 EXPORTS = ["tmpc_workspace_bytes", "tmpc_setup", "tmpc_linearize", "tmpc_factor", "tmpc_admm_solve", "tmpc_backward",
            "tmpc_kkt_solve", "tmpc_host_staging_bytes", "tmpc_admm_solve_host", "tmpc_destroy", "tmpc_status_string",
-           "tmpc_launch_count", "tmpc_measure_peak", "tmpc_admm_solve_adaptive"]
+           "tmpc_launch_count", "tmpc_measure_peak", "tmpc_admm_solve_adaptive", "tmpc_sqp_solve"]
 
 
 class TmpcConfig(C.Structure):
@@ -49,6 +49,10 @@ class TmpcState(C.Structure):
 class TmpcAdaptive(C.Structure):
     _fields_ = [("max_iters", C.c_int32), ("check_every", C.c_int32), ("adapt_rho", C.c_int32), ("reserved", C.c_int32),
                 ("eps_abs", C.c_double), ("eps_rel", C.c_double), ("rho_ratio", C.c_double), ("rho_min", C.c_double), ("rho_max", C.c_double)]
+
+
+class TmpcSqpOpts(C.Structure):
+    _fields_ = [("max_sqp", C.c_int32), ("admm_iters", C.c_int32), ("n_alpha", C.c_int32), ("reserved", C.c_int32), ("eps_c", C.c_double), ("eta", C.c_double)]
 
 
 class TmpcInfo(C.Structure):
@@ -79,6 +83,7 @@ def lib():
         L.tmpc_kkt_solve.argtypes = [C.c_void_p] * 3
         L.tmpc_admm_solve_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t]
         L.tmpc_destroy.argtypes = [C.c_void_p]
+        L.tmpc_sqp_solve.argtypes = [C.c_void_p] * 9
         L.tmpc_admm_solve_adaptive.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tmpc_measure_peak.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
         _LIB = L
@@ -180,3 +185,7 @@ def tmpc_measure_peak(what: int, scratch_ptr: int, stream_ptr: int, reps: int = 
 def tmpc_admm_solve_adaptive(h, qp, st, ad: TmpcAdaptive, flags=0, info=None, iters_ptr=None, converged_ptr=None, rho_ptr=None):
     _check(lib().tmpc_admm_solve_adaptive(h, C.byref(qp), C.byref(st), C.byref(ad), flags, C.byref(info) if info is not None else None,
                                           iters_ptr, converged_ptr, rho_ptr), "tmpc_admm_solve_adaptive")
+
+
+def tmpc_sqp_solve(h, qp, st, ref_ptr, opts: TmpcSqpOpts, iters_ptr=None, converged_ptr=None, alpha_ptr=None, kkt_ptr=None):
+    _check(lib().tmpc_sqp_solve(h, C.byref(qp), C.byref(st), ref_ptr, C.byref(opts), iters_ptr, converged_ptr, alpha_ptr, kkt_ptr), "tmpc_sqp_solve")

@@ -16,6 +16,7 @@
 #include "tmpc_cr.cuh"
 #include "tmpc_cr2.cuh"
 #include "tmpc_peak.cuh"
+#include "tmpc_sqp.cuh"
 
 using namespace tmpc;
 
@@ -397,6 +398,57 @@ tmpc_status do_solve_adaptive(tmpc_ctx* h, const tmpc_qp* qp, tmpc_state* st, co
   return TMPC_OK;
 }
 
+// ---- f2: SQP with linesearch and the eq. 18 stop (Alg. 1, App. D) for the built-in bicycle model.  One linearisation per iteration
+// serves both the convergence test of the previous step and the next QP; converged problems are frozen (activity flags of f1).
+template <typename T>
+tmpc_status do_sqp(tmpc_ctx* h, tmpc_qp* qp, tmpc_state* st, const void* stage_ref, const tmpc_sqp_opts* o, int32_t* iters_out, int32_t* conv_out,
+                   void* alpha_log, void* kkt_out) {
+  const Dims& d = h->d; const Layout& L = h->lay; unsigned char* ws = h->ws;
+  if (h->cfg.model != TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT) return TMPC_E_UNSUPPORTED;
+  int32_t* active = (int32_t*)(ws + L.ad_active); int32_t* mask = (int32_t*)(ws + L.ad_mask);
+  int32_t* iters = (int32_t*)(ws + L.ad_iters); int32_t* conv = (int32_t*)(ws + L.ad_conv); int32_t* count = (int32_t*)(ws + L.ad_count);
+  const unsigned nb = (unsigned)((d.B + 255) / 256);
+  adapt_init_kernel<T><<<nb, 256, 0, h->stream>>>(d.B, (T)h->cfg.rho_bar, (T*)(ws + L.ad_rho), active, mask, iters, conv, count); h->launches++;
+  if (!cuda_ok()) return TMPC_E_CUDA;
+  SqpArgs<T> a; memset(&a, 0, sizeof(a));
+  a.d = d; a.qp = view<T>(qp); a.Lwb = h->cfg.wheelbase; a.dt = h->cfg.dt; a.gamma = h->cfg.slack_gamma; a.lam = h->cfg.slack_lambda; a.eps_c = o->eps_c; a.eta = o->eta;
+  a.n_alpha = o->n_alpha; a.active = active; a.act_rw = active; a.iters = iters; a.converged = conv; a.n_active = count;
+  a.ox = (const T*)(ws + L.ax); a.oxi = (const T*)(ws + L.axi); a.oyf = (const T*)(ws + L.ayf); a.oyg = (const T*)(ws + L.ayg);
+  a.x = (T*)st->x; a.xi = (T*)st->xi; a.yf = (T*)st->yf; a.yg = (T*)st->yg; a.alpha_log = (T*)alpha_log; a.max_sqp = o->max_sqp; a.kkt = (T*)kkt_out;
+  const size_t es = sizeof(T);
+  tmpc_status rc = TMPC_OK;
+  for (int it = 0; it <= o->max_sqp && rc == TMPC_OK; ++it) {
+    rc = tmpc_linearize(h, st->x, stage_ref, qp); if (rc != TMPC_OK) break;
+    if (it > 0) {                                         // eq. 18 at the iterate the last step produced
+      if (cudaMemsetAsync(count, 0, sizeof(int32_t), h->stream) != cudaSuccess) { rc = TMPC_E_CUDA; break; }
+      a.it = it;
+      sqp_kkt_kernel<T><<<d.B, 128, 0, h->stream>>>(a); h->launches++;
+      int32_t live = 0;
+      if (!cuda_ok() || cudaMemcpyAsync(&live, count, sizeof(int32_t), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+          cudaStreamSynchronize(h->stream) != cudaSuccess) { rc = TMPC_E_CUDA; break; }
+      if (live == 0 || it == o->max_sqp) break;
+    }
+    // keep the iterate, solve the QP from it (y carried, z_g re-projected: reading A-26), search along the step
+    if (cudaMemcpyAsync(ws + L.ax, st->x, (size_t)d.B * d.nz * es, cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess ||
+        cudaMemcpyAsync(ws + L.axi, st->xi, (size_t)d.B * d.mg * es, cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess ||
+        cudaMemcpyAsync(ws + L.ayf, st->yf, (size_t)d.B * d.mf * es, cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess ||
+        cudaMemcpyAsync(ws + L.ayg, st->yg, (size_t)d.B * d.mg * es, cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess) { rc = TMPC_E_CUDA; break; }
+    h->cur_active = active; h->cur_mask = active;
+    rc = do_factor<T>(h, qp);
+    if (rc == TMPC_OK) { h->factored = true; rc = do_solve<T>(h, qp, st, o->admm_iters, 0, nullptr); }
+    h->cur_active = nullptr; h->cur_mask = nullptr;
+    if (rc != TMPC_OK) break;
+    a.it = it;
+    sqp_linesearch_kernel<T><<<d.B, 32 * (o->n_alpha + 1), 0, h->stream>>>(a); h->launches++;
+    if (!cuda_ok()) rc = TMPC_E_CUDA;
+  }
+  h->cur_active = nullptr; h->cur_mask = nullptr;
+  if (rc != TMPC_OK) return rc;
+  if (iters_out && cudaMemcpyAsync(iters_out, iters, (size_t)d.B * sizeof(int32_t), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess) return TMPC_E_CUDA;
+  if (conv_out && cudaMemcpyAsync(conv_out, conv, (size_t)d.B * sizeof(int32_t), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess) return TMPC_E_CUDA;
+  return TMPC_OK;
+}
+
 template <typename T>
 tmpc_status kkt_solve_t(tmpc_handle h, const void* eta, void* xt) {
   AdmmArgs<T> a; memset(&a, 0, sizeof(a));
@@ -521,6 +573,16 @@ tmpc_status tmpc_admm_solve_adaptive(tmpc_handle h, const tmpc_qp* qp, tmpc_stat
   if (!h->factored) return TMPC_E_STATE;
   return h->cfg.dtype == TMPC_F32 ? do_solve_adaptive<float>(h, qp, st, ad, flags, info, iters_out, converged_out, rho_out)
                                   : do_solve_adaptive<double>(h, qp, st, ad, flags, info, iters_out, converged_out, rho_out);
+}
+
+tmpc_status tmpc_sqp_solve(tmpc_handle h, tmpc_qp* qp, tmpc_state* st, const void* stage_ref, const tmpc_sqp_opts* o, int32_t* iters_out,
+                           int32_t* converged_out, void* alpha_log, void* kkt_out) {
+  if (!h || !qp || !st || !stage_ref || !o || !st->x || !st->zg || !st->yf || !st->yg || !st->xi) return TMPC_E_BADARG;
+  if (!qp->D || !qp->E || !qp->q || !qp->x_init || !qp->Am || !qp->Ap || !qp->b || !qp->G || !qp->lo || !qp->hi) return TMPC_E_BADARG;
+  if (o->max_sqp < 1 || o->admm_iters < 1 || o->n_alpha < 1 || o->n_alpha > SQP_MAX_ALPHA || !(o->eps_c > 0) || !(o->eta > 0 && o->eta < 1)) return TMPC_E_BADARG;
+  if (h->cr) return TMPC_E_UNSUPPORTED;
+  return h->cfg.dtype == TMPC_F32 ? do_sqp<float>(h, qp, st, stage_ref, o, iters_out, converged_out, alpha_log, kkt_out)
+                                  : do_sqp<double>(h, qp, st, stage_ref, o, iters_out, converged_out, alpha_log, kkt_out);
 }
 
 tmpc_status tmpc_kkt_solve(tmpc_handle h, const void* eta, void* xt) {

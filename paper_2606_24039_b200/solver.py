@@ -115,6 +115,16 @@ class Solver:
             self.factor()
             self.admm_solve(iters)
 
+    def sqp_linesearch(self, max_sqp=10, admm_iters=50, eps_c=1e-3, n_alpha=8, eta=0.4):
+        """f2: tmpc_sqp_solve from the current state.  Returns dict(iters, converged, alpha [B,max_sqp], kkt [B,3]) as numpy arrays."""
+        w = self.w
+        it = torch.zeros(w.B, dtype=torch.int32, device=self.dev); cv = torch.zeros(w.B, dtype=torch.int32, device=self.dev)
+        al = torch.zeros(w.B, max_sqp, dtype=self.td, device=self.dev); kk = torch.zeros(w.B, 3, dtype=self.td, device=self.dev)
+        B.tmpc_sqp_solve(self.h, self.qp, self.st, self.t["stage_ref"].data_ptr(), B.TmpcSqpOpts(max_sqp, admm_iters, n_alpha, 0, eps_c, eta),
+                         it.data_ptr(), cv.data_ptr(), al.data_ptr(), kk.data_ptr())
+        torch.cuda.synchronize(self.dev)
+        return dict(iters=it.cpu().numpy(), converged=cv.cpu().numpy(), alpha=al.cpu().double().numpy(), kkt=kk.cpu().double().numpy())
+
     def backward(self, dLdx, dLdxi=None, mode=B.TMPC_BWD_REFACTOR_REFINE, iters=None):
         w = self.w
         if iters is None:

@@ -624,3 +624,29 @@ def test_f4_linear_rl_sweep_shapes_fp32():
     run_pair(W.linear_rl(B=5, N=12, nx=4, nu=2, u_max=1.0), "f32", iters=60)
     run_pair(W.linear_rl(B=3, N=10, nx=16, nu=8, u_max=10.0), "f32", iters=60)
     run_pair(W.linear_rl(B=2, N=8, nx=32, nu=16, u_max=1.0), "f32", iters=60, band=1)
+
+
+# ----------------------------------------------------------------------------------------------- f2: SQP with linesearch + eq. 18
+def test_sqp_linesearch_matches_oracle_fp64():
+    """Alg. 1 with the App. D linesearch and the eq. 18 stop on perturbed bicycle starts: accepted
+    step sizes of every iteration, per-problem iteration counts, convergence flags and the final iterates equal the oracle's."""
+    from paper_2606_24039_b200.solver import Solver
+    w = W.config4(B=7, N=24, dtype="f64")
+    x0 = w.xbar0.copy(); x0[:, :, :2] += np.random.default_rng(0).normal(0, 1.5, x0[:, :, :2].shape); x0[:, :, 2] += 0.3
+    x0[5:] = w.xbar0[5:]                                   # two problems start from the reference (first steps: smallest candidate, fallback)
+    kw = dict(max_sqp=8, admm_iters=120, eps_c=1e-3, n_alpha=8, eta=0.4)
+    ref, rinfo, log, rc = O.sqp_linesearch_bicycle(w, O.make_cfg(w), xbar0=x0, **kw)
+    assert rc == 0
+    s = Solver(w, dtype="f64")
+    s.reset_state(x0)
+    out = s.sqp_linesearch(**kw)
+    got = s.state_numpy()
+    assert (out["iters"] == rinfo[:, 0].astype(int)).all(), (out["iters"], rinfo[:, 0])
+    assert (out["converged"] == rinfo[:, 1].astype(int)).all()
+    for b in range(w.B):
+        k = int(rinfo[b, 0])
+        assert (out["alpha"][b, :k] == log[b, :k, 0]).all(), (b, out["alpha"][b, :k], log[b, :k, 0])
+    assert (out["alpha"] < 1.0).any() and (out["alpha"] == 1.0).any(), "instance must exercise backtracking and full steps"
+    compare_states({k: got[k] for k in ("x", "yf", "yg", "xi")} | {"zg": ref["zg"]}, ref, 1e-9)
+    assert np.abs(out["kkt"] - rinfo[:, 2:5]).max() <= 1e-7
+    s.close()
