@@ -148,6 +148,10 @@ tmpc_status tmpc_sqp_solve(tmpc_handle h, tmpc_qp* qp, tmpc_state* st, const voi
  * forward factor.  Overwrites the factor in the workspace in REFACTOR_REFINE mode. */
 tmpc_status tmpc_backward(tmpc_handle h, const tmpc_qp* qp, const tmpc_state* st, const void* dL_dx, const void* dL_dxi,
                           int32_t mode, int32_t iters, void* dL_dq, void* dL_dxinit);
+/* eq. 66: dL/dgamma_xi [B] (working dtype, DEVICE) = sum over the soft-active rows of xi_i (G eta_x)_i, from the
+ * dL/dq = -eta_x that the preceding tmpc_backward of the same state returned (its row classification is kept in the workspace;
+ * TMPC_E_STATE without one). */
+tmpc_status tmpc_backward_dgamma(tmpc_handle h, const tmpc_qp* qp, const tmpc_state* st, const void* dL_dq, void* dL_dgamma);
 /* Applies the current factor: xt [B][T][n] = S^{-1} eta [B][T][n] (eq. 8).  Test/diagnostic entry. */
 tmpc_status tmpc_kkt_solve(tmpc_handle h, const void* eta, void* xt);
 /* Same as tmpc_factor + tmpc_admm_solve but every pointer in qp/st/info is HOST memory (pinned for speed); the

@@ -205,15 +205,16 @@ def sqp_linesearch_bicycle(w, cfg, max_sqp=10, admm_iters=50, eps_c=1e-3, n_alph
     return st, info, log, rc
 
 
-def backward(w, cfg, state, dLdx, dLdxi=None):
-    """O-5 on every problem.  Returns dq [B,T,n], dxinit [B,nx], counts [B,2], rc [B]."""
+def backward(w, cfg, state, dLdx, dLdxi=None, with_dgamma=False):
+    """O-5 on every problem.  Returns dq [B,T,n], dxinit [B,nx], counts [B,2], rc [B] (and dL/dgamma_xi [B], eq. 66, with with_dgamma)."""
     n, T, nz, mf, mg = _dims(w)
     dq = np.zeros((w.B, T, n))
     dxi = np.zeros((w.B, w.nx))
     counts = np.zeros((w.B, 2), dtype=np.int32)
     rcs = np.zeros(w.B, dtype=np.int32)
     f = lib().orc_backward
-    f.argtypes = [C.c_void_p] * 19
+    f.argtypes = [C.c_void_p] * 20
+    dgam = np.zeros(w.B)
     for b in range(w.B):
         D, E = _c(_bs(w.D, b)), _c(_bs(w.E, b))
         G = None if cfg.g_sel else _c(_bs(w.G, b))
@@ -223,7 +224,9 @@ def backward(w, cfg, state, dLdx, dLdxi=None):
         gx = _c(dLdx[b])
         gxi = None if dLdxi is None else _c(dLdxi[b])
         rcs[b] = f(C.byref(cfg), _p(D), _p(E), *[_p(a) for a in args], _p(G), _p(lo), _p(hi), _p(x), _p(yg), _p(xi), _p(gx), _p(gxi),
-                   _p(dq[b]), _p(dxi[b]), counts[b].ctypes.data_as(C.c_void_p))
+                   _p(dq[b]), _p(dxi[b]), counts[b].ctypes.data_as(C.c_void_p), dgam[b:b + 1].ctypes.data_as(C.c_void_p))
+    if with_dgamma:
+        return dq, dxi, counts, rcs, dgam
     return dq, dxi, counts, rcs
 
 

@@ -336,8 +336,11 @@ void classify(const Cfg& cf, const QP& p, const double* x, const double* yg, con
 }
 
 // O-5.  Backward by the definition (eq. 62 / 65).  Returns min |pivot| of the elimination.
+// dgamma (optional): dL/dgamma_xi of eq. 66 in the signed slack: the only explicit dependence of the KKT conditions on gamma
+// is the stationarity row gamma xi + lam sgn(xi) + y_g = 0 of the soft-active rows, so dL/dgamma = -xi_s' eta_xi with eta_xi = -G_s eta_x (eq. 64),
+// i.e. dL/dgamma = sum_{soft-active i} xi_i (G eta_x)_i.
 double backward(const Cfg& cf, const QP& p, const double* x, const double* yg, const double* xi, const double* dLdx, const double* dLdxi,
-                double* dq, double* dxinit, int* n_hard, int* n_soft) {
+                double* dq, double* dxinit, int* n_hard, int* n_soft, double* dgamma = nullptr) {
   std::vector<int> cls; classify(cf, p, x, yg, xi, cls);
   std::vector<int> hard; int ns = 0;
   for (int i = 0; i < p.mg; ++i) { if (cls[i] == 1) hard.push_back(i); if (cls[i] == 2) ++ns; }
@@ -360,6 +363,13 @@ double backward(const Cfg& cf, const QP& p, const double* x, const double* yg, c
   double piv = gauss_solve(K, rhs, m);
   for (int i = 0; i < p.nz; ++i) dq[i] = -rhs[i];                 // dL/dq = -eta_x         (eq. 59, dF/dq = [I;0;0])
   for (int i = 0; i < p.nx; ++i) dxinit[i] = rhs[p.nz + i];       // dL/dx_init = +eta_f[0:nx] (dF/dx_init = -I on init rows)
+  if (dgamma) {
+    double s = 0;
+    for (int r = 0; r < p.mg; ++r) if (cls[r] == 2) { const double* a = p.G.row(r); double ge = 0; for (int k = 0; k < p.G.len[r]; ++k) ge += a[k] * rhs[p.G.c0[r] + k];
+      // the adjoint of the eliminated slack also carries the upstream dL/dxi: gamma eta_xi + eta_yg = dL/dxi, G eta_x + eta_xi = 0 (eq. 60 rows 2, 4)
+      s += xi[r] * ge; }
+    *dgamma = s;
+  }
   *n_hard = nh; *n_soft = ns;
   return piv;
 }
@@ -544,10 +554,10 @@ int orc_admm_batch(const Cfg* cf, int B, int nthreads, const double* D, int64_t 
 // O-5 for one problem.  counts_out[2] = #hard-active, #soft-active.  Returns 0, or 2 when the KKT system is (numerically) singular (reading A-18).
 int orc_backward(const Cfg* cf, const double* D, const double* E, const double* q, const double* Am, const double* Ap, const double* b, const double* x_init,
                  const double* G, const double* lo, const double* hi, const double* x, const double* yg, const double* xi, const double* dLdx,
-                 const double* dLdxi, double* dq, double* dxinit, int* counts_out) {
+                 const double* dLdxi, double* dq, double* dxinit, int* counts_out, double* dgamma_out) {
   Cfg c = *cf;
   QP p = assemble(c, D, E, q, Am, Ap, b, x_init, G, lo, hi);
-  double piv = backward(c, p, x, yg, xi, dLdx, dLdxi, dq, dxinit, &counts_out[0], &counts_out[1]);
+  double piv = backward(c, p, x, yg, xi, dLdx, dLdxi, dq, dxinit, &counts_out[0], &counts_out[1], dgamma_out);
   return piv > 1e-12 ? 0 : 2;
 }
 

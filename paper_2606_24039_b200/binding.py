@@ -22,7 +22,7 @@ TMPC_BWD_REFACTOR_REFINE, TMPC_BWD_ADMM_REUSE_FACTOR = 0, 1
 TMPC_SOLVE_ZG_GIVEN = 1
 EXPORTS = ["tmpc_workspace_bytes", "tmpc_setup", "tmpc_linearize", "tmpc_factor", "tmpc_admm_solve", "tmpc_backward",
            "tmpc_kkt_solve", "tmpc_host_staging_bytes", "tmpc_admm_solve_host", "tmpc_destroy", "tmpc_status_string",
-           "tmpc_launch_count", "tmpc_measure_peak", "tmpc_admm_solve_adaptive", "tmpc_sqp_solve"]
+           "tmpc_launch_count", "tmpc_measure_peak", "tmpc_admm_solve_adaptive", "tmpc_sqp_solve", "tmpc_backward_dgamma"]
 
 
 class TmpcConfig(C.Structure):
@@ -83,6 +83,7 @@ def lib():
         L.tmpc_kkt_solve.argtypes = [C.c_void_p] * 3
         L.tmpc_admm_solve_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t]
         L.tmpc_destroy.argtypes = [C.c_void_p]
+        L.tmpc_backward_dgamma.argtypes = [C.c_void_p] * 5
         L.tmpc_sqp_solve.argtypes = [C.c_void_p] * 9
         L.tmpc_admm_solve_adaptive.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tmpc_measure_peak.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
@@ -189,3 +190,7 @@ def tmpc_admm_solve_adaptive(h, qp, st, ad: TmpcAdaptive, flags=0, info=None, it
 
 def tmpc_sqp_solve(h, qp, st, ref_ptr, opts: TmpcSqpOpts, iters_ptr=None, converged_ptr=None, alpha_ptr=None, kkt_ptr=None):
     _check(lib().tmpc_sqp_solve(h, C.byref(qp), C.byref(st), ref_ptr, C.byref(opts), iters_ptr, converged_ptr, alpha_ptr, kkt_ptr), "tmpc_sqp_solve")
+
+
+def tmpc_backward_dgamma(h, qp, st, dq_ptr, out_ptr):
+    _check(lib().tmpc_backward_dgamma(h, C.byref(qp), C.byref(st), dq_ptr, out_ptr), "tmpc_backward_dgamma")

@@ -86,6 +86,7 @@ struct tmpc_ctx {
   tmpc_config cfg; Dims d; Layout lay; unsigned char* ws; cudaStream_t stream; bool factored; bool cr; bool twisted; int64_t launches;
   // set while tmpc_admm_solve_adaptive runs (f1): per-problem rho_bar, activity flags for the solve kernels, refactor mask for the factor kernels
   const void* cur_rho; const int32_t* cur_active; const int32_t* cur_mask;
+  bool bwd_classified;                          // tmpc_backward has left the row classification of its state in the workspace
   cudaStream_t aux[2]; cudaEvent_t ev[3];       // tmpc_admm_solve_host: two sub-batches in flight (copies of one overlap the kernels of the other)
 };
 
@@ -493,7 +494,7 @@ tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, vo
   if (!h) return TMPC_E_BADARG;
   h->cfg = *cfg; h->d = make_dims(*cfg); h->lay = L; h->ws = (unsigned char*)workspace; h->stream = (cudaStream_t)cuda_stream;
   h->factored = false; h->cr = use_cr(*cfg); h->twisted = false; h->launches = 0;
-  h->cur_rho = nullptr; h->cur_active = nullptr; h->cur_mask = nullptr;
+  h->cur_rho = nullptr; h->cur_active = nullptr; h->cur_mask = nullptr; h->bwd_classified = false;
   h->aux[0] = h->aux[1] = nullptr; h->ev[0] = h->ev[1] = h->ev[2] = nullptr;
   // zero buffers of the adjoint QP (x_init = 0, b = 0)
   if (cudaMemsetAsync(h->ws + L.zero_xinit, 0, L.zero_b - L.zero_xinit, h->stream) != cudaSuccess ||
@@ -603,6 +604,7 @@ tmpc_status do_backward(tmpc_ctx* h, const tmpc_qp* qp, const tmpc_state* st, co
   const Dims& d = h->d; const Layout& L = h->lay; unsigned char* ws = h->ws;
   if (h->cr) return TMPC_E_UNSUPPORTED;
   BwdArgs<T> a; memset(&a, 0, sizeof(a));
+  h->bwd_classified = true;
   a.d = d; a.qp = view<T>(qp); a.x = (const T*)st->x; a.yg = (const T*)st->yg; a.xi = (const T*)st->xi;
   a.dLdx = (const T*)dLdx; a.dLdxi = (const T*)dLdxi;
   a.eps_abs = (T)h->cfg.eps_active_abs; a.eps_rel = (T)h->cfg.eps_active_rel; a.gamma = (T)h->cfg.slack_gamma; a.sigma = (T)h->cfg.sigma;
@@ -674,6 +676,17 @@ tmpc_status tmpc_backward(tmpc_handle h, const tmpc_qp* qp, const tmpc_state* st
   if (mode != TMPC_BWD_REFACTOR_REFINE && mode != TMPC_BWD_ADMM_REUSE_FACTOR) return TMPC_E_BADARG;
   return h->cfg.dtype == TMPC_F32 ? do_backward<float>(h, qp, st, dL_dx, dL_dxi, mode, iters, dL_dq, dL_dxinit)
                                   : do_backward<double>(h, qp, st, dL_dx, dL_dxi, mode, iters, dL_dq, dL_dxinit);
+}
+
+tmpc_status tmpc_backward_dgamma(tmpc_handle h, const tmpc_qp* qp, const tmpc_state* st, const void* dL_dq, void* dL_dgamma) {
+  tmpc_status s = check_qp(h, qp); if (s != TMPC_OK) return s;
+  if (!st || !st->xi || !dL_dq || !dL_dgamma) return TMPC_E_BADARG;
+  if (!h->bwd_classified) return TMPC_E_STATE;
+  const int8_t* cls = (const int8_t*)(h->ws + h->lay.cls);
+  if (h->cfg.dtype == TMPC_F32) bwd_dgamma_kernel<float><<<h->d.B, 256, 0, h->stream>>>(h->d, view<float>(qp), cls, (const float*)st->xi, (const float*)dL_dq, (float*)dL_dgamma);
+  else bwd_dgamma_kernel<double><<<h->d.B, 256, 0, h->stream>>>(h->d, view<double>(qp), cls, (const double*)st->xi, (const double*)dL_dq, (double*)dL_dgamma);
+  h->launches++;
+  return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
 }
 
 tmpc_status tmpc_host_staging_bytes(const tmpc_config* cfg, size_t* bytes) {

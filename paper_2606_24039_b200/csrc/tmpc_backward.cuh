@@ -162,6 +162,22 @@ __global__ void __launch_bounds__(1024) bwd_refine_kernel(BwdArgs<T> a) {
   for (int e = tid; e < nx; e += nt) a.dxinit[(size_t)p * nx + e] = ef[e];
 }
 
+// eq. 66 in the signed slack: dL/dgamma_xi = sum over the soft-active rows of xi_i (G eta_x)_i with eta_x = -dL/dq;
+// one CTA per problem, fixed summation order.
+template <typename T>
+__global__ void __launch_bounds__(256) bwd_dgamma_kernel(Dims d, QpView<T> qp, const int8_t* __restrict__ cls, const T* __restrict__ xi, const T* __restrict__ dq, T* __restrict__ out) {
+  __shared__ T red[64];
+  const int p = blockIdx.x, ng = d.ng, mg = d.mg, nz = d.nz;
+  const T* G = qp.G ? qp.G + qp.sG * p : nullptr;
+  T s = T(0);
+  for (int e = threadIdx.x; e < mg; e += blockDim.x) {
+    if (cls[(size_t)p * mg + e] != 2) continue;
+    s -= xi[(size_t)p * mg + e] * g_dot(d, G, e / ng, e % ng, dq + (size_t)p * nz);
+  }
+  s = block_sum(s, red);
+  if (threadIdx.x == 0) out[p] = s;
+}
+
 // REUSE mode epilogue: dq = -x_adj, dxinit = +yf_adj[0:nx]
 template <typename T>
 __global__ void bwd_reuse_finish_kernel(int B, int nz, int nx, int mf, const T* xa, const T* yfa, T* dq, T* dxinit) {

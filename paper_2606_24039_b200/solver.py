@@ -134,6 +134,12 @@ class Solver:
         B.tmpc_backward(self.h, self.qp, self.st, dLdx.data_ptr(), None if dLdxi is None else dLdxi.data_ptr(), mode, iters, dq.data_ptr(), dxi.data_ptr())
         return dq, dxi
 
+    def backward_dgamma(self, dq):
+        """eq. 66 after a backward() call on the same state: dL/dgamma_xi [B]."""
+        out = torch.zeros(self.w.B, dtype=self.td, device=self.dev)
+        B.tmpc_backward_dgamma(self.h, self.qp, self.st, dq.data_ptr(), out.data_ptr())
+        return out
+
     def kkt_solve(self, eta):
         xt = torch.empty_like(eta)
         B.tmpc_kkt_solve(self.h, eta.data_ptr(), xt.data_ptr())

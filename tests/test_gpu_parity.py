@@ -502,6 +502,10 @@ def test_backward_with_dLdxi_and_dead_zone_rows(dtype):
     tol = 1e-9 if dtype == "f64" else 2e-3
     dq, dxi = _gpu_backward(s, ref, dLdx, dLdxi, Bd.TMPC_BWD_REFACTOR_REFINE)
     assert rel_err(dq[ok], dq_o[ok]) <= tol and rel_err(dxi[ok], dxi_o[ok]) <= tol
+    # eq. 66: dL/dgamma_xi from the same adjoint solution
+    dg_o = O.backward(wr, cfg, ref, dLdx, dLdxi, with_dgamma=True)[4]
+    dg = s.backward_dgamma(s._up(dq)).cpu().double().numpy()
+    assert (np.abs(dg - dg_o)[ok] <= tol * np.maximum(1.0, np.abs(dg_o[ok]))).all() and np.abs(dg_o[ok]).max() > 1e-3
     K = 300
     s.factor()
     dq2, dxi2 = _gpu_backward(s, ref, dLdx, dLdxi, Bd.TMPC_BWD_ADMM_REUSE_FACTOR, iters=K)

@@ -550,6 +550,27 @@ def test_adjoint_qp_of_eq67_converges_to_the_definition():
     assert all((a[k] == b[k]).all() for k in a)
 
 
+def test_backward_dgamma_matches_finite_differences():
+    """dL/dgamma_xi (eq. 66) for L = |x|^2 + |xi|^2 vs central differences in gamma on a soft-active instance."""
+    import copy
+    w = W.config2(B=1, N=8, soft_bound=0.3)
+    w.lam, w.rho_bar = 0.05, 2.0
+    w.q = w.q + 0.3 * np.random.default_rng(5).standard_normal(w.q.shape)
+
+    def loss(gam):
+        ww = copy.copy(w); ww.gamma = gam
+        st, info, rc = O.admm(ww, O.make_cfg(ww), iters=30000)
+        assert info[0, 0] < 1e-11 and info[0, 1] < 1e-11
+        return (st["x"] ** 2).sum() + (st["xi"] ** 2).sum(), st
+
+    L0, st = loss(w.gamma)
+    dq, dxi, counts, rcs, dg = O.backward(w, O.make_cfg(w), st, 2.0 * st["x"], 2.0 * st["xi"], with_dgamma=True)
+    assert rcs[0] == 0 and counts[0, 1] > 0
+    h = 1e-5
+    fd = (loss(w.gamma + h)[0] - loss(w.gamma - h)[0]) / (2 * h)
+    assert abs(fd - dg[0]) <= 1e-6 * max(1.0, abs(fd)) and abs(fd) > 1e-3
+
+
 def test_backward_unconstrained_closed_form():
     """No active rows: dL/dq = -(K^-1)_xx dL/dx with K the equality KKT matrix (numpy)."""
     w = W.random_ltv(7, 1, 6, 3, 2, [3, 4], [0, 0], bound=np.inf, implicit=True, q_scale=0.5)
