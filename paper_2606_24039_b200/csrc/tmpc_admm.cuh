@@ -25,7 +25,7 @@ struct AdmmArgs {
   int32_t* status;
   int iters, zg_given;
   int kkt_only;                           // 1: x <- S^{-1} x and return (tmpc_kkt_solve)
-  const int8_t* soft_rows;                // optional [B][mg] per-row soft flag overriding d.soft_mask (adjoint QP, eq. 67)
+  const int8_t* soft_rows;                // optional [B][mg] per-row flag overriding d.soft_mask: 0 hard, 1 soft (adjoint QP, eq. 67), 2 = row switched off (resident class only)
   // f1 (adaptive step size): optional per-problem rho_bar [B] (rho_g = rho_bar, rho_f = rho_scale rho_bar) replacing
   // prm.rho_g / prm.rho_f, and an optional per-problem activity flag [B]: problems with active[p] == 0 (terminated by eq. 4) are left untouched
   const T* rho_bar; T rho_scale;

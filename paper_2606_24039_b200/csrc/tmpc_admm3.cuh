@@ -387,9 +387,10 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
       } else if (2 * s + h < ng) r = 2 * s + h;
       if (r < 0) continue;
       const size_t row = (size_t)p * mg + t * ng + r;
+      if (a.soft_rows && a.soft_rows[row] == 2) continue;      // row switched off (adjoint refinement: inactive rows, and soft-active rows that live in the factor only)
       qf[s] = Q_VALID | ((unsigned)r << Q_ROW_SH);
       lo[s] = a.qp.lo[row]; hi[s] = a.qp.hi[row]; yg[s] = a.yg[row];
-      if (a.soft_rows ? (a.soft_rows[row] != 0) : (((d.soft_mask >> r) & 1u) != 0)) qf[s] |= Q_SOFT;
+      if (a.soft_rows ? (a.soft_rows[row] == 1) : (((d.soft_mask >> r) & 1u) != 0)) qf[s] |= Q_SOFT;
       if (a.zg_given) zg[s] = a.zg[row];
       else {                                             // z_g^0 = clip(G x^0, lo, hi) (x-space, straight from the problem data)
         T gx;

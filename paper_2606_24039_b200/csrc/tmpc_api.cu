@@ -249,6 +249,7 @@ tmpc_status launch_admm3_shape(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return TMPC_E_CUDA;
     if ((h->d.B + PG - 1) / PG <= sms) return launch_admm3_inst<T, NC, NX, PG, 256, 1>(h, a, f);
+    if constexpr (sizeof(T) == 8) { if (f.nt <= 192 && f.ctas_per_sm == 2) return launch_admm3_inst<T, NC, NX, PG, 192, 2>(h, a, f); }   // 170 registers: no spills for double
     if (f.ctas_per_sm >= 3) return launch_admm3_inst<T, NC, NX, PG, 256, 3>(h, a, f);
     if (f.ctas_per_sm >= 2) return launch_admm3_inst<T, NC, NX, PG, 256, 2>(h, a, f);
     return launch_admm3_inst<T, NC, NX, PG, 256, 1>(h, a, f);
@@ -263,9 +264,9 @@ tmpc_status launch_resident(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f
   return TMPC_E_UNSUPPORTED;
 }
 template <typename T>
-tmpc_status launch_factor_tw(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_in, int32_t* status) {
-  FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = nullptr;
-  a.rho_bar = (const T*)h->cur_rho; a.rho_scale = h->cfg.rho_eq_scale; a.mask = h->cur_mask;
+tmpc_status launch_factor_tw(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_in, int32_t* status, const T* w_rows = nullptr) {
+  FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = w_rows;
+  a.rho_bar = w_rows ? nullptr : (const T*)h->cur_rho; a.rho_scale = h->cfg.rho_eq_scale; a.mask = w_rows ? nullptr : h->cur_mask;
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
   if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) factor_tw2_kernel<T, 8, 6, true><<<h->d.B, 64, 0, h->stream>>>(a);
   else if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) factor_tw2_kernel<T, 6, 4, true><<<h->d.B, 64, 0, h->stream>>>(a);
@@ -612,6 +613,32 @@ tmpc_status do_backward(tmpc_ctx* h, const tmpc_qp* qp, const tmpc_state* st, co
   a.cls = (int8_t*)(ws + L.cls); a.rhs = (T*)(ws + L.rhs);
   a.dq = (T*)dq; a.dxinit = (T*)dxinit; a.sweeps = iters;
   int ntp = ((d.nz + 31) / 32) * 32; if (ntp > 512) ntp = 512; if (ntp < 64) ntp = 64;
+  if (mode == TMPC_BWD_REFACTOR_REFINE && fast_plan<T>(d).ok) {
+    // Resident class: the refinement  e <- e + K_reg^{-1}(rhs - K e)  of the active-set system is, term by term, Alg. 3 with alpha = 1 on the
+    // equality-constrained adjoint QP  min 1/2 x'(P + gamma G_s'G_s)x - rhs'x  s.t. Cx = 0, G_h x = 0  with rho_f = rho_g = rho_adj:
+    //   x+ = S_adj^{-1}(sigma x + rhs - C'y_f - G_h'y_g),  y+ = y + rho_adj A_a x+      (z = 0 on every constraint row)
+    // so it runs on the twisted factor and the resident kernel: soft-active rows only weight the factor (gamma), inactive rows are off.
+    a.w_rows = (T*)(ws + L.w_rows); a.refine_codes = 1;
+    a.lo_adj = (T*)(ws + L.lo_adj); a.hi_adj = (T*)(ws + L.hi_adj); a.soft_adj = (int8_t*)(ws + L.soft_adj); a.q_adj = (T*)(ws + L.q_adj);
+    bwd_prepare_kernel<T><<<d.B, ntp, 0, h->stream>>>(a); h->launches++;
+    if (!cuda_ok()) return TMPC_E_CUDA;
+    tmpc_status s = launch_factor_tw<T>(h, qp, (double)a.rho_adj, 0.0, nullptr, a.w_rows);
+    h->factored = false; h->twisted = true;       // the forward factor has been overwritten
+    if (s != TMPC_OK) return s;
+    if (cudaMemsetAsync(ws + L.ax, 0, L.zero_xinit - L.ax, h->stream) != cudaSuccess) return TMPC_E_CUDA;
+    AdmmArgs<T> r; memset(&r, 0, sizeof(r));
+    r.d = d; r.prm = params<T>(h->cfg); r.prm.alpha = T(1); r.prm.rho_f = a.rho_adj; r.prm.rho_g = a.rho_adj; r.prm.lam = T(0); r.qp = view<T>(qp);
+    r.qp.q = a.q_adj; r.qp.b = (const T*)(ws + L.zero_b); r.qp.x_init = (const T*)(ws + L.zero_xinit); r.qp.lo = a.lo_adj; r.qp.hi = a.hi_adj;
+    r.Lam = (const T*)(ws + L.Lam); r.Sinv = (const T*)(ws + L.Sinv);
+    r.x = (T*)(ws + L.ax); r.zg = (T*)(ws + L.azg); r.yf = (T*)(ws + L.ayf); r.yg = (T*)(ws + L.ayg); r.xi = (T*)(ws + L.axi);
+    r.iters = iters; r.soft_rows = a.soft_adj;
+    s = launch_resident<T>(h, r, fast_plan<T>(d));
+    h->twisted = false;
+    if (s != TMPC_OK) return s;
+    const long long tot = (long long)d.B * d.nz;
+    bwd_reuse_finish_kernel<T><<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(d.B, d.nz, d.nx, d.mf, r.x, r.yf, (T*)dq, (T*)dxinit); h->launches++;
+    return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+  }
   if (mode == TMPC_BWD_REFACTOR_REFINE) {
     a.w_rows = (T*)(ws + L.w_rows);
     bwd_prepare_kernel<T><<<d.B, ntp, 0, h->stream>>>(a); h->launches++;

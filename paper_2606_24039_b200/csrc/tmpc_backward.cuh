@@ -27,6 +27,7 @@ struct BwdArgs {
   T* w_rows;                                // [B][mg] out (REFINE): row weights for the adjoint factor
   T* lo_adj; T* hi_adj; int8_t* soft_adj;   // [B][mg] out (REUSE): bounds and soft flags of the adjoint QP
   T* q_adj;                                 // [B][nz] out (REUSE): -rhs_x
+  int refine_codes;                         // 1: soft_adj holds the row codes of the resident-class refinement (see bwd_prepare_kernel)
   // refine
   const T* Lam; const T* Sinv;
   int sweeps;
@@ -71,7 +72,9 @@ __global__ void bwd_prepare_kernel(BwdArgs<T> a) {
     if (a.w_rows) a.w_rows[(size_t)p * mg + e] = c == 1 ? a.rho_adj : (c == 2 ? a.gamma : T(0));
     if (a.lo_adj) {
       a.lo_adj[(size_t)p * mg + e] = c ? T(0) : -INFINITY; a.hi_adj[(size_t)p * mg + e] = c ? T(0) : INFINITY;
-      a.soft_adj[(size_t)p * mg + e] = (int8_t)(c == 2);
+      // eq. 67 mode: soft-active rows are soft rows of the adjoint QP.  Refinement on the resident class (refine_codes): only the hard-active
+      // rows are constraint rows; soft-active rows enter through the factor (weight gamma), inactive rows not at all -> both switched off (2)
+      a.soft_adj[(size_t)p * mg + e] = a.refine_codes ? (int8_t)(c == 1 ? 0 : 2) : (int8_t)(c == 2);
     }
   }
   __syncthreads();
