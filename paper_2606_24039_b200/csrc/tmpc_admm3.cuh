@@ -39,7 +39,6 @@ struct Rec3 {
   static constexpr int up(int v) { return (v + V - 1) / V * V; }
   static constexpr int AM = 0, AP = AM + up(NX * NC), E0 = AP + up(NX * NC), E1A = E0 + up(NC), E1B = E1A + up(NC),
                        LAM = E1B + up(NC), SINV = LAM + up(NC * NC), G = SINV + up(NC * NC);
-  static constexpr int SKEW = 32 / (int)sizeof(T);      // 32 bytes: the down-chain records sit one 8-bank group off
   // record stride: 32 bytes (mod 128 bytes) for the 16-byte accesses of n = 8 (a quarter warp = four stages x two halves covers
   // the eight bank groups); 24 bytes (mod 128) for the 6-wide rows of n = 6, whose 8-byte pairs and single elements cannot all
   // be conflict free: this residue makes the single-element loads conflict free and the pair loads 2-way (simulated over all
@@ -51,7 +50,11 @@ struct Rec3 {
     return r;
   }
 };
-struct Admm3Plan { int R, per_problem; };
+// Placement of the records of one problem: stages 0..m (the up chain and the middle) at t R; stages m+1..N (the down chain) in REVERSE
+// order from `down0`, i.e. stage t at down0 + (N - t) R, so that step k of both chains sits at (k R) and (down0 + k R): with
+// down0 = 64 bytes (mod 128) and the second problem of a CTA another 32 bytes off, the four slots of the chain warp read four disjoint
+// 8-bank windows at every step, for any record stride (n = 6 and n = 8 alike).
+struct Admm3Plan { int R, down0, per_problem; };
 
 template <typename T, int NC, int NX>
 inline Admm3Plan admm3_plan(const Dims& d, int pg) {
@@ -59,8 +62,12 @@ inline Admm3Plan admm3_plan(const Dims& d, int pg) {
   Admm3Plan P;
   int R = d.g_sel ? RC::G : RC::G + ((d.ng * NC + RC::V - 1) / RC::V) * RC::V;
   P.R = RC::pad_stride(R);
-  int pp = d.T * P.R + RC::SKEW;
-  if (pg == 2) { const int w128 = 128 / (int)sizeof(T), w64 = 64 / (int)sizeof(T); pp = (pp + RC::V - 1) / RC::V * RC::V; while (pp % w128 != w64) pp += RC::V; }   // second problem: 16-byte aligned, two bank groups off
+  const int w128 = 128 / (int)sizeof(T), w64 = 64 / (int)sizeof(T), w32 = 32 / (int)sizeof(T), m = d.T / 2;
+  int d0 = ((m + 1) * P.R + RC::V - 1) / RC::V * RC::V;
+  while (d0 % w128 != w64) d0 += RC::V;
+  P.down0 = d0;
+  int pp = (d0 + (d.T - 1 - m) * P.R + RC::V - 1) / RC::V * RC::V;
+  if (pg == 2) { while (pp % w128 != w32) pp += RC::V; }
   P.per_problem = pp;
   return P;
 }
@@ -122,21 +129,24 @@ template <typename T, int H> __device__ __forceinline__ T dot2(const T (&a)[H], 
 // Row i >= n/2 takes its 16-byte chunks in the opposite order (`swb`; the data is not swizzled) so that the eight rows of a
 // slot cover the eight bank groups; the broadcast operand vector is read in the same order.
 template <typename T, int NC, int NX, int PG>
-__device__ __forceinline__ void chain3_solve(T* sm, int R, int PP, int T_, int lane, unsigned pmask) {   // pmask: bit g = problem g of the CTA is live
+__device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, int T_, int lane, unsigned pmask) {   // pmask: bit g = problem g of the CTA is live
   static_assert(NC == 8 || NC == 6, "chain lanes are written for n = 6 and n = 8");
   using RC = Rec3<T, NC, NX>;
   constexpr int n = NC;
   constexpr unsigned ES = sizeof(T);
   const unsigned sb = (unsigned)__cvta_generic_to_shared(sm);
   const int N = T_ - 1, m = T_ / 2;
-  const int slot = lane >> 3, i8 = lane & 7;
+  // Lanes without a chain of their own (rows >= n of a slot, the upper half warp when the CTA holds one problem, a terminated problem)
+  // still walk the records of a live-looking slot and load from them — the SAME addresses as that slot's lanes, i.e. pure broadcasts that
+  // cost no extra shared-memory wavefront (ncu: parked on the middle record they collided with the working lanes) — but never store.
+  const int slot = PG == 2 ? (lane >> 3) : ((lane >> 3) & 1), i8 = lane & 7;
   const int g = PG == 2 ? (slot >> 1) : 0, dir = slot & 1;
-  const bool act = (PG == 2 || slot < 2) && i8 < n && ((pmask >> g) & 1u);
+  const bool live = (PG == 2 || lane < 16) && i8 < n && ((pmask >> g) & 1u);
   const int ii = i8 < n ? i8 : 0;
   const unsigned swb = (unsigned)swz_x<T, NC>(ii) * ES;                 // chunk ORDER of my row (bytes)
-  const int cnt = act ? (dir ? T_ - 1 - m : m) : 0, t0 = dir ? N : 0;
-  const int dRb = (dir ? -R : R) * (int)ES;
-  auto rec = [&](int t) { return t * R + (t > m ? RC::SKEW : 0); };
+  const int cnt = dir ? T_ - 1 - m : m, t0 = dir ? N : 0;
+  const int dRb = R * (int)ES;                           // both chains advance by +R per step (the down half is stored in reverse order)
+  auto rec = [&](int t) { return t > m ? DOWN0 + (N - t) * R : t * R; };
   const unsigned pb = sb + (unsigned)(g * PP) * ES, bm = pb + (unsigned)rec(m) * ES;
   constexpr unsigned oE0 = RC::E0 * ES, oE1 = RC::E1A * ES, oE1B = RC::E1B * ES, oLAM = RC::LAM * ES;
   const unsigned me = (unsigned)ii * ES, myrow = oLAM + (unsigned)(ii * n) * ES;
@@ -147,21 +157,21 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int PP, int T_, int l
   lds_row<T, NC>(bt + myrow, swb, Br);
   const int cmin = T_ - 1 - m;                          // = the down chain's length <= the up chain's (m)
   const int kmain = cmin > 1 ? ((cmin - 1) & ~1) : 0;   // even: the main loop is unrolled by two
-  const int dRa = act ? dRb : 0;                        // idle lanes stay on record m
+  const int dRa = dRb;
   // Main loop: every active slot is on and none is at its last stage, so no predicates.  Two steps per trip with the row
   // buffers Br / Bn swapping roles (in admm2 the copies Br <- Bn sat in front of the final adds in program order and made
   // the in-order issue wait for the NEXT step's row load inside the dependent chain of THIS step).
 #pragma unroll 1
   for (int k = 0; k < kmain; k += 2) {
     T W[n], Bn[n], eta;
-    if (act) sts_1(bt + oE1 + me, wv);
+    if (live) sts_1(bt + oE1 + me, wv);
     __syncwarp();
     lds_row<T, NC>(bt + oE1, swb, W);
     bt += dRa;
     eta = ld_eta(bt);
     lds_row<T, NC>(bt + myrow, swb, Bn);
     wv = dotv_from<n>(Br, W, eta);
-    if (act) sts_1(bt + oE1 + me, wv);
+    if (live) sts_1(bt + oE1 + me, wv);
     __syncwarp();
     lds_row<T, NC>(bt + oE1, swb, W);
     bt += dRa;
@@ -172,7 +182,7 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int PP, int T_, int l
 #pragma unroll 1
   for (int k = kmain; k < m; ++k) {                    // w_next = eta~_next + (-B_t) w_t, with the per-slot end conditions
     const bool on = k < cnt, last = k == cnt - 1;
-    if (on) sts_1(bt + oE1 + me, wv);
+    if (on && live) sts_1(bt + oE1 + me, wv);
     __syncwarp();
     T W[n];
     lds_row<T, NC>(bt + oE1, swb, W);
@@ -189,7 +199,7 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int PP, int T_, int l
   }
   // middle stage: w_m = eta~_m + both contributions; y_m = w_m
   const T wm = wv + __shfl_xor_sync(0xffffffffu, wv, 8);
-  if (act) { sts_1(bm + oE1 + me, wm); sts_1(bm + oE0 + me, wm); }
+  if (live) { sts_1(bm + oE1 + me, wm); sts_1(bm + oE0 + me, wm); }
   __syncwarp();
   // outward sweep: y_t = w_t + (-B_t)' y_next.  The column of -B_t and w_t of the NEXT step are loaded while this step's
   // y vector is in flight; two steps per trip with the buffers swapping roles.
@@ -206,7 +216,7 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int PP, int T_, int l
     const unsigned bnx = (on && k > 0) ? bc - dRb : bc;
     ld_col(bnx, coln, wn);
     const T y = dotv_from<n>(col, Y, w);
-    if (on) { sts_1(bc + oE0 + me, y); bp = bc; bc = bnx; }
+    if (on) { if (live) sts_1(bc + oE0 + me, y); bp = bc; bc = bnx; }
     __syncwarp();
   };
   T colA[n], colB[n], wA, wB;
@@ -234,7 +244,8 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   const int ng = d.ng, N = d.N, T_ = d.T, nz = T_ * n, mf = d.mf, mg = d.mg;
   const int tid = threadIdx.x, nt = blockDim.x, it_tid = tid - 32;
   const int m = T_ / 2;
-  auto rec = [&](int t) { return t * R + (t > m ? RC::SKEW : 0); };
+  const int DOWN0 = A.pl.down0;
+  auto rec = [&](int t) { return t > m ? DOWN0 + (N - t) * R : t * R; };
 
   // ---- stage 1: X_t, -B_t and the raw constraint blocks of every problem of this CTA into the records (all threads)
 #pragma unroll 1
@@ -304,7 +315,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
 #ifdef TMPC_TIMING
       __syncwarp(); const T probe = sm[tid & 7]; const long long c1 = clock64() + (probe == T(12345.678) ? 1 : 0);   // the load makes the deferred barrier block first
 #endif
-      chain3_solve<T, NC, NX, PG>(sm, R, PP, T_, tid, pmask);
+      chain3_solve<T, NC, NX, PG>(sm, R, A.pl.down0, PP, T_, tid, pmask);
       __syncwarp();
 #ifdef TMPC_TIMING
       tch += clock64() - c1;
