@@ -38,8 +38,14 @@ NOMINAL_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1
 DEFAULT_DTYPE = {1: "f64", 2: "f32", 3: "f32", 4: "f32", 5: "f64"}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per tmpc_admm_solve call, from committed `ncu --set full`
 # captures: (bytes, profiles/ file).  Only quoted for the exact workload the capture was taken on; None otherwise.
-NCU_TRAFFIC = {}
-KERNEL_NAMES = {1: "admm2_kernel", 2: "admm2_kernel", 3: "admm_stream_kernel x chunk launches", 4: "admm2_kernel", 5: "cr2_admm_kernel"}
+NCU_TRAFFIC = {
+    (2, "f32", 1024): (57.05e6 + 0.38e6, "profiles/r02_ncu_full_admm3_kernel_config2_f32.md"),
+    (4, "f32", 4096): (275.5e6 + 25.7e6, "profiles/r02_ncu_full_admm3_kernel_config4_f32.md (one tmpc_admm_solve = one SQP step)"),
+    (5, "f64", 1): (13.38e6 + 0.003e6, "profiles/r02_ncu_full_cr2_admm_kernel_config5_f64.md"),
+    # config 3: one tmpc_admm_solve = 7 chunk launches; the capture is ONE full-wave launch (296 CTAs x 50 iterations), scaled to the 2048 chunk jobs of a call
+    (3, "f32", 512): ((65.42e9 + 0.572e9) * 2048 / 296, "profiles/r01_v3_ncu_full_admm_stream_kernel_config3_f32.md (kernel unchanged in round 2)"),
+}
+KERNEL_NAMES = {1: "admm3_kernel", 2: "admm3_kernel", 3: "admm_stream_kernel x chunk launches", 4: "admm3_kernel", 5: "cr2_admm_kernel"}
 STEPS_CAP = {3: 5, 5: 10}     # per_config legs of the all-configs run: the 95 ms / 6 ms steps need fewer repetitions for a stable mean
 
 
