@@ -77,10 +77,21 @@ __device__ __forceinline__ double lds_1(unsigned a, double) { double v; asm vola
 __device__ __forceinline__ void sts_1(unsigned a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
 __device__ __forceinline__ void sts_1(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
 // contiguous NC-vector at byte address a; for NC = 8 the 16-byte chunks are taken in the order of a row swizzled by swb bytes
+__device__ __forceinline__ void lds_chunk(unsigned a, float& r0, float& r1, float& r2, float& r3) { asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r0), "=f"(r1), "=f"(r2), "=f"(r3) : "r"(a)); }
+__device__ __forceinline__ void lds_chunk(unsigned a, double& r0, double& r1) { asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(r0), "=d"(r1) : "r"(a)); }
 template <typename T, int NC> __device__ __forceinline__ void lds_row(unsigned a, unsigned swb, T (&r)[NC]) {
   if constexpr (NC == 8 && sizeof(T) == 4) lds_vec8(a + swb, a + 16u - swb, r);     // swb in {0,16}: chunks (0,16) or (16,0), one add each
   else if constexpr (NC == 8) lds_vec8(a + (0u ^ swb), a + (16u ^ swb), a + (32u ^ swb), a + (48u ^ swb), r);
-  else lds_vec6(a, r);
+  else if constexpr (NC == 6) lds_vec6(a, r);
+  else if constexpr (sizeof(T) == 4) {                  // wider rows (n = 12, ...): 16-byte chunks in natural order
+    static_assert(NC % 4 == 0, "float rows in 16-byte chunks");
+#pragma unroll
+    for (int c = 0; c < NC / 4; ++c) lds_chunk(a + 16u * c, r[4 * c], r[4 * c + 1], r[4 * c + 2], r[4 * c + 3]);
+  } else {
+    static_assert(NC % 2 == 0, "double rows in 16-byte chunks");
+#pragma unroll
+    for (int c = 0; c < NC / 2; ++c) lds_chunk(a + 16u * c, r[2 * c], r[2 * c + 1]);
+  }
 }
 
 // empty asm that "uses" a whole register vector: keeps ptxas from splitting a multi-chunk load into load - use - load - use

@@ -90,21 +90,46 @@ template <int NC> __device__ __forceinline__ constexpr int slot_col(int h, int s
 struct HalfOff { int pair, single; };                                         // element offsets of a half inside a row
 template <int NC> __device__ __forceinline__ HalfOff half_off(int h) { HalfOff o; o.pair = NC == 6 ? 4 * h : h * (NC / 2); o.single = NC == 6 ? 2 + h : 0; return o; }
 
+//   other even n (n = 12): slots = columns h n/2 + s, loaded in the widest aligned vectors (8 bytes for a 24-byte half, else 16)
 template <int NC> __device__ __forceinline__ void ld_half(const float* __restrict__ row, const HalfOff& o, float (&r)[NC / 2]) {
-  if constexpr (NC == 8) { const float4 v = *reinterpret_cast<const float4*>(row + o.pair); r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w; }
-  else { const float2 v = *reinterpret_cast<const float2*>(row + o.pair); r[0] = v.x; r[1] = v.y; r[2] = row[o.single]; }
+  constexpr int H = NC / 2;
+  if constexpr (NC == 6) { const float2 v = *reinterpret_cast<const float2*>(row + o.pair); r[0] = v.x; r[1] = v.y; r[2] = row[o.single]; }
+  else if constexpr (H % 4 == 0) {
+#pragma unroll
+    for (int c = 0; c < H / 4; ++c) { const float4 v = reinterpret_cast<const float4*>(row + o.pair)[c]; r[4 * c] = v.x; r[4 * c + 1] = v.y; r[4 * c + 2] = v.z; r[4 * c + 3] = v.w; }
+  } else {
+    static_assert(H % 2 == 0, "half rows of floats in 8-byte vectors");
+#pragma unroll
+    for (int c = 0; c < H / 2; ++c) { const float2 v = reinterpret_cast<const float2*>(row + o.pair)[c]; r[2 * c] = v.x; r[2 * c + 1] = v.y; }
+  }
 }
 template <int NC> __device__ __forceinline__ void ld_half(const double* __restrict__ row, const HalfOff& o, double (&r)[NC / 2]) {
-  if constexpr (NC == 8) { const double2 v = *reinterpret_cast<const double2*>(row + o.pair), w = *reinterpret_cast<const double2*>(row + o.pair + 2); r[0] = v.x; r[1] = v.y; r[2] = w.x; r[3] = w.y; }
-  else { const double2 v = *reinterpret_cast<const double2*>(row + o.pair); r[0] = v.x; r[1] = v.y; r[2] = row[o.single]; }
+  constexpr int H = NC / 2;
+  if constexpr (NC == 6) { const double2 v = *reinterpret_cast<const double2*>(row + o.pair); r[0] = v.x; r[1] = v.y; r[2] = row[o.single]; }
+  else {
+    static_assert(H % 2 == 0, "half rows of doubles in 16-byte vectors");
+#pragma unroll
+    for (int c = 0; c < H / 2; ++c) { const double2 v = reinterpret_cast<const double2*>(row + o.pair)[c]; r[2 * c] = v.x; r[2 * c + 1] = v.y; }
+  }
 }
 template <int NC> __device__ __forceinline__ void st_half(float* __restrict__ row, const HalfOff& o, const float (&r)[NC / 2]) {
-  if constexpr (NC == 8) *reinterpret_cast<float4*>(row + o.pair) = make_float4(r[0], r[1], r[2], r[3]);
-  else { *reinterpret_cast<float2*>(row + o.pair) = make_float2(r[0], r[1]); row[o.single] = r[2]; }
+  constexpr int H = NC / 2;
+  if constexpr (NC == 6) { *reinterpret_cast<float2*>(row + o.pair) = make_float2(r[0], r[1]); row[o.single] = r[2]; }
+  else if constexpr (H % 4 == 0) {
+#pragma unroll
+    for (int c = 0; c < H / 4; ++c) reinterpret_cast<float4*>(row + o.pair)[c] = make_float4(r[4 * c], r[4 * c + 1], r[4 * c + 2], r[4 * c + 3]);
+  } else {
+#pragma unroll
+    for (int c = 0; c < H / 2; ++c) reinterpret_cast<float2*>(row + o.pair)[c] = make_float2(r[2 * c], r[2 * c + 1]);
+  }
 }
 template <int NC> __device__ __forceinline__ void st_half(double* __restrict__ row, const HalfOff& o, const double (&r)[NC / 2]) {
-  if constexpr (NC == 8) { *reinterpret_cast<double2*>(row + o.pair) = make_double2(r[0], r[1]); *reinterpret_cast<double2*>(row + o.pair + 2) = make_double2(r[2], r[3]); }
-  else { *reinterpret_cast<double2*>(row + o.pair) = make_double2(r[0], r[1]); row[o.single] = r[2]; }
+  constexpr int H = NC / 2;
+  if constexpr (NC == 6) { *reinterpret_cast<double2*>(row + o.pair) = make_double2(r[0], r[1]); row[o.single] = r[2]; }
+  else {
+#pragma unroll
+    for (int c = 0; c < H / 2; ++c) reinterpret_cast<double2*>(row + o.pair)[c] = make_double2(r[2 * c], r[2 * c + 1]);
+  }
 }
 // acc[s] += m[s] * w for a half (packed FFMA2 for float)
 template <int H> __device__ __forceinline__ void axpy_half(float (&acc)[H], const float (&m)[H], float w) {
@@ -130,7 +155,8 @@ template <typename T, int H> __device__ __forceinline__ T dot2(const T (&a)[H], 
 // slot cover the eight bank groups; the broadcast operand vector is read in the same order.
 template <typename T, int NC, int NX, int PG>
 __device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, int T_, int lane, unsigned pmask) {   // pmask: bit g = problem g of the CTA is live
-  static_assert(NC == 8 || NC == 6, "chain lanes are written for n = 6 and n = 8");
+  constexpr int SL = NC <= 8 ? 8 : 16;                   // lanes per slot (one per row)
+  static_assert(NC <= 16 && PG * 2 * SL <= 32, "the chain warp holds (problems x 2 directions) slots of SL lanes");
   using RC = Rec3<T, NC, NX>;
   constexpr int n = NC;
   constexpr unsigned ES = sizeof(T);
@@ -139,9 +165,9 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, in
   // Lanes without a chain of their own (rows >= n of a slot, the upper half warp when the CTA holds one problem, a terminated problem)
   // still walk the records of a live-looking slot and load from them — the SAME addresses as that slot's lanes, i.e. pure broadcasts that
   // cost no extra shared-memory wavefront (ncu: parked on the middle record they collided with the working lanes) — but never store.
-  const int slot = PG == 2 ? (lane >> 3) : ((lane >> 3) & 1), i8 = lane & 7;
+  const int slot = (lane / SL) % (2 * PG), i8 = lane % SL;
   const int g = PG == 2 ? (slot >> 1) : 0, dir = slot & 1;
-  const bool live = (PG == 2 || lane < 16) && i8 < n && ((pmask >> g) & 1u);
+  const bool live = lane < 2 * PG * SL && i8 < n && ((pmask >> g) & 1u);
   const int ii = i8 < n ? i8 : 0;
   const unsigned swb = (unsigned)swz_x<T, NC>(ii) * ES;                 // chunk ORDER of my row (bytes)
   const int cnt = dir ? T_ - 1 - m : m, t0 = dir ? N : 0;
@@ -198,7 +224,7 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, in
     for (int j = 0; j < n; ++j) Br[j] = Bn[j];
   }
   // middle stage: w_m = eta~_m + both contributions; y_m = w_m
-  const T wm = wv + __shfl_xor_sync(0xffffffffu, wv, 8);
+  const T wm = wv + __shfl_xor_sync(0xffffffffu, wv, SL);
   if (live) { sts_1(bm + oE1 + me, wm); sts_1(bm + oE0 + me, wm); }
   __syncwarp();
   // outward sweep: y_t = w_t + (-B_t)' y_next.  The column of -B_t and w_t of the NEXT step are loaded while this step's
@@ -236,7 +262,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* sm = reinterpret_cast<T*>(smem_raw);
   using RC = Rec3<T, NC, NX>;
-  static_assert(NC == 6 || NC == 8, "half-row loads are written for n = 6 and n = 8");
+  static_assert(NC % 2 == 0, "two lanes per stage own half a row each");
   const AdmmArgs<T>& a = A.a;
   const Dims& d = a.d;
   constexpr int n = NC, nx = NX, nn = NC * NC, H = NC / 2, KA = (NX + 1) / 2;

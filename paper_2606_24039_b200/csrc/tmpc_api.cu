@@ -215,10 +215,11 @@ constexpr size_t kSmemPerSM = 228 * 1024;
 template <typename T>
 FastPlan fast_plan(const Dims& d) {
   FastPlan f; f.ok = false; f.pg = 1; f.nt = 0; f.ctas_per_sm = 0; f.smem = 0;
-  const bool shape = (d.n == 8 && d.nx == 6) || (d.n == 6 && d.nx == 4);
+  const bool shape = (d.n == 8 && d.nx == 6) || (d.n == 6 && d.nx == 4) || (d.n == 12 && d.nx == 8);   // (12, 8): the nominal block size of the paper's scaling study (f4)
   if (!shape || d.ng > d.n || d.T < 2) return f;
   if (d.g_sel) for (int r = 0; r < d.ng; ++r) for (int q = 0; q < r; ++q) if (d.g_col[r] == d.g_col[q]) return f;   // one selection row per column
-  const size_t s1 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 1) : admm3_smem_bytes<T, 6, 4>(d, 1), s2 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 2) : admm3_smem_bytes<T, 6, 4>(d, 2);
+  const size_t s1 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 1) : d.n == 6 ? admm3_smem_bytes<T, 6, 4>(d, 1) : admm3_smem_bytes<T, 12, 8>(d, 1);
+  const size_t s2 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 2) : d.n == 6 ? admm3_smem_bytes<T, 6, 4>(d, 2) : kMaxSmem + 1;   // n = 12: one problem per CTA (16 chain lanes per slot)
   if (s1 > kMaxSmem) return f;
   const int c1 = (int)(kSmemPerSM / (s1 + 1024)), c2 = s2 <= kMaxSmem ? (int)(kSmemPerSM / (s2 + 1024)) : 0;
   f.pg = (d.B >= 2 && c2 >= 2 && 2 * c2 >= c1) ? 2 : 1;
@@ -261,6 +262,7 @@ tmpc_status launch_resident(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f
   const Dims& d = h->d;
   if (d.n == 8) return f.pg == 2 ? launch_admm3_shape<T, 8, 6, 2>(h, a, f) : launch_admm3_shape<T, 8, 6, 1>(h, a, f);
   if (d.n == 6) return f.pg == 2 ? launch_admm3_shape<T, 6, 4, 2>(h, a, f) : launch_admm3_shape<T, 6, 4, 1>(h, a, f);
+  if (d.n == 12) return launch_admm3_shape<T, 12, 8, 1>(h, a, f);
   return TMPC_E_UNSUPPORTED;
 }
 template <typename T>
@@ -270,6 +272,7 @@ tmpc_status launch_factor_tw(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
   if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) factor_tw2_kernel<T, 8, 6, true><<<h->d.B, 64, 0, h->stream>>>(a);
   else if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) factor_tw2_kernel<T, 6, 4, true><<<h->d.B, 64, 0, h->stream>>>(a);
+  else if (h->d.n == 12 && h->d.nx == 8 && h->d.ng <= 12) factor_tw2_kernel<T, 12, 8, true><<<h->d.B, 64, 0, h->stream>>>(a);
   else return TMPC_E_UNSUPPORTED;      // fast_plan() only admits the shapes above
   h->launches++;
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
