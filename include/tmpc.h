@@ -121,7 +121,7 @@ typedef struct {
  * is read back after every round so that the call returns when all have terminated.  Outputs (DEVICE, [B], any may be NULL): iterations
  * each problem ran, 1 if it met eq. 4, its final rho_bar (working dtype); info as in tmpc_admm_solve, at each problem's last check.
  * Afterwards the factor in the workspace belongs to the per-problem rho_bar values: call tmpc_factor before the next solve.
- * TMPC_E_UNSUPPORTED for the streamed class (stage blocks that do not fit in shared memory) and for cyclic reduction. */
+ * TMPC_E_UNSUPPORTED for cyclic reduction. */
 tmpc_status tmpc_admm_solve_adaptive(tmpc_handle h, const tmpc_qp* qp, tmpc_state* st, const tmpc_adaptive* ad, int32_t flags, tmpc_info* info,
                                      int32_t* iters_out, int32_t* converged_out, void* rho_out);
 /* f2 — the SQP outer loop of Alg. 1 for the built-in model: per iteration tmpc_linearize at the iterate st.x,

@@ -366,7 +366,6 @@ tmpc_status do_solve_adaptive(tmpc_ctx* h, const tmpc_qp* qp, tmpc_state* st, co
                               int32_t* iters_out, int32_t* conv_out, void* rho_out) {
   const Dims& d = h->d; const Layout& L = h->lay; unsigned char* ws = h->ws;
   if (h->cr) return TMPC_E_UNSUPPORTED;
-  if (!h->twisted && admm_smem_elems(d, true) * sizeof(T) > kMaxSmem) return TMPC_E_UNSUPPORTED;     // streamed class: fixed-count solves only
   T* rho = (T*)(ws + L.ad_rho); int32_t* active = (int32_t*)(ws + L.ad_active); int32_t* mask = (int32_t*)(ws + L.ad_mask);
   int32_t* iters = (int32_t*)(ws + L.ad_iters); int32_t* conv = (int32_t*)(ws + L.ad_conv); int32_t* count = (int32_t*)(ws + L.ad_count);
   tmpc_info li;

@@ -76,6 +76,7 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
   const int LD = S.LD, KS = S.slots, tid = threadIdx.x;
   const int gjob = S.g0 + (int)blockIdx.x, chunk = gjob / d.B, p = gjob - chunk * d.B;
   const int zg_given = chunk > 0 ? 1 : a.zg_given;                   // later chunks resume from the stored state
+  if (a.active && !a.active[p]) return;                              // terminated problem (f1): the whole CTA leaves before any barrier is set up
   unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_raw);            // full[KS], empty[KS]
   T* ring = reinterpret_cast<T*>(smem_raw + 256);
   // Only v / x~ is kept whole in shared memory.  The right-hand side eta lives in global memory (each element is written
@@ -162,7 +163,7 @@ __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant
     for (; k < rows; k += 4) acc[0] += M[(size_t)k * LD + col] * vec[k];
     return quad_sum(acc[0] + acc[1]);
   };
-  const T sigma = a.prm.sigma, rho_f = a.prm.rho_f, rho_g = a.prm.rho_g, alpha = a.prm.alpha;
+  const T sigma = a.prm.sigma, rho_g = a.rho_bar ? a.rho_bar[p] : a.prm.rho_g, rho_f = a.rho_bar ? a.rho_scale * rho_g : a.prm.rho_f, alpha = a.prm.alpha;   // per-problem step size under f1
   const T inv_rho_g = T(1) / rho_g, inv_rg = T(1) / (rho_g + a.prm.gamma), lam = a.prm.lam;
   const bool own_x = cq == 0 && ci < n, own_f = cq == 0 && ci < nx, own_g = cq == 0 && ci < ng;
   const size_t gx = (size_t)p * nz, gf = (size_t)p * mf, gg = (size_t)p * mg;

@@ -654,3 +654,19 @@ def test_sqp_linesearch_matches_oracle_fp64():
     compare_states({k: got[k] for k in ("x", "yf", "yg", "xi")} | {"zg": ref["zg"]}, ref, 1e-9)
     assert np.abs(out["kkt"] - rinfo[:, 2:5]).max() <= 1e-7
     s.close()
+
+
+def test_adaptive_on_the_streamed_class_fp64():
+    """f1 on the streamed class (blocks that do not fit in shared memory: admm_stream_kernel + factor3_kernel with per-problem rho_bar,
+    refactor mask and frozen terminated problems), on the f4 generator at (nx, nu) = (32, 16)."""
+    from paper_2606_24039_b200.solver import Solver
+    w = W.linear_rl(B=3, N=24, nx=32, nu=16, u_max=1.0)
+    ref, rinfo, log, rc = O.admm_adaptive(w, O.make_cfg(w, band=1), O.make_adaptive(400, 1e-4, 1e-4))
+    assert rc == 0
+    s = Solver(w, dtype="f64")
+    out = s.solve_adaptive(400, 1e-4, 1e-4)
+    assert (out["iters"] == rinfo[:, 4].astype(int)).all(), (out["iters"], rinfo[:, 4])
+    assert (out["converged"] == rinfo[:, 6].astype(int)).all()
+    assert (np.abs(out["rho"] - rinfo[:, 5]) <= 1e-6 * np.abs(rinfo[:, 5])).all()
+    compare_states(s.state_numpy(), ref, 1e-7)
+    s.close()
