@@ -1,7 +1,7 @@
 // tmpc_admm3.cuh — a4..a8 for the RESIDENT class, second generation (round 2): the fused ADMM loop of Alg. 3
 // on the twisted block factor of tmpc_factor2.cuh, all iterations in one launch.
 //
-// What changed against tmpc_admm2.cuh, and why (ncu of admm2 at config 2: 62 % of the warp samples wait at a barrier, the
+// What changed against round 1's admm2_kernel, and why (ncu of admm2 at config 2: 62 % of the warp samples wait at a barrier, the
 // LSU pipe carries 1435 shared-memory wavefronts per problem-iteration = 52 % of its peak, 23 % of them excess):
 //  * TWO lanes per stage instead of four.  Lane h of a stage owns the columns [h n/2, (h+1) n/2) of every block of
 //    the stage record, the same rows of the stage variable, and half of the dynamics / inequality rows.  Every matrix

@@ -1,7 +1,7 @@
 // tmpc_factor2.cuh — a2 + a3 for the resident fast path: twisted block Cholesky, one WARP per half chain with
 // compile-time block sizes.
 //
-// Twisted ("burn at both ends") block LDL' factor for the resident fast path (tmpc_admm2.cuh).
+// Twisted ("burn at both ends") block LDL' factor for the resident fast path (tmpc_admm3.cuh).
 //
 // The block-tridiagonal S is eliminated from BOTH ends towards the middle stage m = T/2: the up chain runs over
 // stages 0,1,..,m-1 and the down chain over N,N-1,..,m+1, independently; the middle pivot collects both Schur
@@ -27,7 +27,7 @@
 
 namespace tmpc {
 
-// TW = true: twisted factor (X_t, B_t) for admm2_kernel.  TW = false: the one-directional block LDL' of factor_kernel
+// TW = true: twisted factor (X_t, B_t) for admm3_kernel.  TW = false: the one-directional block LDL' of factor_kernel
 // (Lam_t = Phi_t Sigma_t^{-1}, Sinv_t = Sigma_t^{-1}; per-row weights w_rows supported) for the backward pass; one warp.
 template <typename T, int NC, int NX, bool TW>
 __global__ void __launch_bounds__(64, 12) factor_tw2_kernel(FactorArgs<T> a) {
