@@ -443,8 +443,14 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
     }
   }
 
+#ifdef TMPC_TIMING
+  long long tA = 0, tW = 0, tB = 0, qs = clock64();
+#endif
 #pragma unroll 1
   for (int it = 0; it < a.iters; ++it) {
+#ifdef TMPC_TIMING
+    if (it > 0) { const long long q0 = clock64(); tB += q0 - qs; qs = q0; }
+#endif
     // ---- a4 in scaled variables (eq. 51): eta~_t = X_t (sigma x - q + G's) + A~^-_t' r_t  [+ G~_t' s_t]  -> E1A of my record,
     //      and my block's share of the next stage's right-hand side, A~^+_t' r_t -> E1B of record t+1 (record 0 for t = N)
     T dn[H], dr[H], ro[KA], rr[KA];
@@ -500,8 +506,14 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
       st_half<NC>(sm + b + RC::E1A, mine, acc);
       st_half<NC>(sm + bn + RC::E1B, mine, accb);
     }
+#ifdef TMPC_TIMING
+    const long long qa = clock64();
+#endif
     bar_arrive(1, nt);
     bar_sync(2, nt);
+#ifdef TMPC_TIMING
+    { const T probe = sm[b + RC::E0]; const long long qb = clock64() + (probe == T(12345.678) ? 1 : 0); tA += qa - qs; tW += qb - qa; qs = qb; }
+#endif
     // ---- a7 + a8 on y: x~ = X_t' y_t, z~_f = A~^-_t y_t + A~^+_t y_{t+1}, z~_g = x~_col or G~_t y_t; relaxation (eq. 10),
     // projection (eq. 12-15), duals (eq. 16 / 44-45)
     if (valid) {
@@ -545,6 +557,9 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
     }
   }
 
+#ifdef TMPC_TIMING
+  if (blockIdx.x == 0 && (tid == 32 || tid == 160)) printf("item warp %d: phase A %lld, wait for chain %lld, phase B %lld cycles per iteration\n", tid >> 5, tA / a.iters, tW / a.iters, tB / a.iters);
+#endif
   // ---- write back the state
   if (valid) {
 #pragma unroll
