@@ -36,7 +36,8 @@ extern "C" {
 
 typedef struct tmpc_ctx* tmpc_handle; /* opaque; owns nothing the caller passed in */
 
-typedef enum { TMPC_OK = 0, TMPC_E_BADARG, TMPC_E_DIM, TMPC_E_UNSUPPORTED, TMPC_E_STATE, TMPC_E_WORKSPACE, TMPC_E_CUDA } tmpc_status;
+typedef enum { TMPC_OK = 0, TMPC_E_BADARG, TMPC_E_DIM, TMPC_E_UNSUPPORTED, TMPC_E_STATE, TMPC_E_WORKSPACE, TMPC_E_CUDA,
+               TMPC_E_STATIC_LIMIT /* tmpc_admm_solve_static: the problem needs more than TMPC_STATIC_SCRATCH_BYTES of scratch */ } tmpc_status;
 typedef enum { TMPC_F32 = 0, TMPC_F64 = 1 } tmpc_dtype;
 typedef enum { TMPC_MODEL_NONE = 0, TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT = 1 } tmpc_model;
 typedef enum { TMPC_LIN_SEQUENTIAL = 0, TMPC_LIN_CYCLIC_REDUCTION = 1, TMPC_LIN_AUTO = 2 } tmpc_linsolve;
@@ -168,6 +169,21 @@ tmpc_status tmpc_admm_solve_host(tmpc_handle h, const tmpc_qp* host_qp, tmpc_sta
 #define TMPC_PEAK_DFMA 2
 #define TMPC_PEAK_LDS 3
 tmpc_status tmpc_measure_peak(int32_t what, void* scratch, void* cuda_stream, int32_t reps, double* out);
+/* Allocation-free variant of tmpc_factor + tmpc_admm_solve for callers that cannot allocate device memory (CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): no handle, no caller workspace.  The scratch the kernels need (the block factor of S, the per-problem
+ * status word, residual partials) lives in ONE file-scope `static __device__` array of TMPC_STATIC_SCRATCH_BYTES inside the library, which every
+ * GPU that loads the library holds until the process exits.  cfg, qp, st, info, iters, flags as in tmpc_setup / tmpc_admm_solve (qp, st, info
+ * are DEVICE pointers owned by the caller); the kernels are enqueued on cuda_stream and the call returns without synchronising.
+ *  - a problem whose tmpc_workspace_bytes(cfg) exceeds TMPC_STATIC_SCRATCH_BYTES is rejected with TMPC_E_STATIC_LIMIT and nothing is enqueued;
+ *    TMPC_LIN_CYCLIC_REDUCTION (and AUTO where it would pick it) returns TMPC_E_UNSUPPORTED;
+ *  - the call makes no cudaMalloc / cudaFree / allocating library call (it uses cudaGetSymbolAddress once per device, cudaMemsetAsync and
+ *    kernel launches);
+ *  - ALL calls on a device share the one array, which keeps the contents of the previous call: the status words are cleared at the start of
+ *    every call, everything else is written before it is read.  Two calls that overlap on the GPU (different streams, or different host
+ *    threads without ordering) RACE on the array: serialise them on one stream or with events. */
+#define TMPC_STATIC_SCRATCH_BYTES (8u << 20)
+tmpc_status tmpc_admm_solve_static(const tmpc_config* cfg, const tmpc_qp* qp, tmpc_state* st, int32_t iters, int32_t flags, tmpc_info* info,
+                                   void* cuda_stream);
 tmpc_status tmpc_destroy(tmpc_handle h);
 const char* tmpc_status_string(tmpc_status s);
 /* Number of kernels this handle has launched so far (for bench.py's gpu_launches). */

@@ -22,7 +22,7 @@ TMPC_BWD_REFACTOR_REFINE, TMPC_BWD_ADMM_REUSE_FACTOR = 0, 1
 TMPC_SOLVE_ZG_GIVEN = 1
 EXPORTS = ["tmpc_workspace_bytes", "tmpc_setup", "tmpc_linearize", "tmpc_factor", "tmpc_admm_solve", "tmpc_backward",
            "tmpc_kkt_solve", "tmpc_host_staging_bytes", "tmpc_admm_solve_host", "tmpc_destroy", "tmpc_status_string",
-           "tmpc_launch_count", "tmpc_measure_peak", "tmpc_admm_solve_adaptive", "tmpc_sqp_solve", "tmpc_backward_dgamma"]
+           "tmpc_launch_count", "tmpc_measure_peak", "tmpc_admm_solve_adaptive", "tmpc_sqp_solve", "tmpc_backward_dgamma", "tmpc_admm_solve_static"]
 
 
 class TmpcConfig(C.Structure):
@@ -83,6 +83,7 @@ def lib():
         L.tmpc_kkt_solve.argtypes = [C.c_void_p] * 3
         L.tmpc_admm_solve_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t]
         L.tmpc_destroy.argtypes = [C.c_void_p]
+        L.tmpc_admm_solve_static.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         L.tmpc_backward_dgamma.argtypes = [C.c_void_p] * 5
         L.tmpc_sqp_solve.argtypes = [C.c_void_p] * 9
         L.tmpc_admm_solve_adaptive.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -194,3 +195,13 @@ def tmpc_sqp_solve(h, qp, st, ref_ptr, opts: TmpcSqpOpts, iters_ptr=None, conver
 
 def tmpc_backward_dgamma(h, qp, st, dq_ptr, out_ptr):
     _check(lib().tmpc_backward_dgamma(h, C.byref(qp), C.byref(st), dq_ptr, out_ptr), "tmpc_backward_dgamma")
+
+
+TMPC_STATIC_SCRATCH_BYTES = 8 << 20
+TMPC_E_STATIC_LIMIT = 7
+
+
+def tmpc_admm_solve_static(cfg: TmpcConfig, qp: TmpcQp, st: TmpcState, iters: int, flags: int = 0, info: TmpcInfo | None = None, stream_ptr=None):
+    """Allocation-free factor + solve on the library's static device scratch (see include/tmpc.h); no handle, no workspace."""
+    _check(lib().tmpc_admm_solve_static(C.byref(cfg), C.byref(qp), C.byref(st), iters, flags, C.byref(info) if info is not None else None, stream_ptr),
+           "tmpc_admm_solve_static")

@@ -475,6 +475,7 @@ const char* tmpc_status_string(tmpc_status s) {
     case TMPC_E_STATE: return "call order: tmpc_factor must precede tmpc_admm_solve / tmpc_backward / tmpc_kkt_solve";
     case TMPC_E_WORKSPACE: return "workspace missing, misaligned or too small";
     case TMPC_E_CUDA: return "CUDA error (or no CUDA device: there is no CPU fallback)";
+    case TMPC_E_STATIC_LIMIT: return "problem exceeds the static scratch of tmpc_admm_solve_static (tmpc_workspace_bytes > TMPC_STATIC_SCRATCH_BYTES = 8 MiB)";
   }
   return "unknown";
 }
@@ -794,3 +795,52 @@ tmpc_status tmpc_admm_solve_host(tmpc_handle h, const tmpc_qp* hq, tmpc_state* h
 }
 
 }  // extern "C"
+
+// =================================================================================================== allocation-free entry
+// Scratch of tmpc_admm_solve_static: one array per GPU that loads the library, held until the process exits.  In HOST code the name below is a
+// host-side stand-in, not a device address: the address the kernels get comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char g_tmpc_static_scratch[TMPC_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kMaxDevices = 64;
+unsigned char* g_static_ptr[kMaxDevices] = {};           // device address of g_tmpc_static_scratch on device d (nullptr: not looked up yet)
+
+tmpc_status static_scratch_ptr(unsigned char** out) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return TMPC_E_CUDA; }
+  if (dev < 0 || dev >= kMaxDevices) return TMPC_E_UNSUPPORTED;
+  if (!g_static_ptr[dev]) {                              // (a race between two host threads here stores the same value twice)
+    void* ptr = nullptr;
+    if (cudaGetSymbolAddress(&ptr, g_tmpc_static_scratch) != cudaSuccess || !ptr) { cudaGetLastError(); return TMPC_E_CUDA; }
+    g_static_ptr[dev] = (unsigned char*)ptr;
+  }
+  *out = g_static_ptr[dev];
+  return TMPC_OK;
+}
+}  // namespace
+
+extern "C" tmpc_status tmpc_admm_solve_static(const tmpc_config* cfg, const tmpc_qp* qp, tmpc_state* st, int32_t iters, int32_t flags, tmpc_info* info,
+                                              void* cuda_stream) {
+  tmpc_status s = check_cfg(cfg); if (s != TMPC_OK) return s;
+  if (!st || !st->x || !st->zg || !st->yf || !st->yg || !st->xi || iters < 0) return TMPC_E_BADARG;
+  if (use_cr(*cfg)) return TMPC_E_UNSUPPORTED;
+  const Layout L = make_layout(*cfg);
+  if (L.total > (size_t)TMPC_STATIC_SCRATCH_BYTES) return TMPC_E_STATIC_LIMIT;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return TMPC_E_CUDA; }
+  unsigned char* ws = nullptr;
+  s = static_scratch_ptr(&ws); if (s != TMPC_OK) return s;
+  tmpc_ctx c;                                             // a handle on the host stack: nothing is allocated, nothing outlives the call
+  c.cfg = *cfg; c.d = make_dims(*cfg); c.lay = L; c.ws = ws; c.stream = (cudaStream_t)cuda_stream;
+  c.factored = false; c.cr = false; c.twisted = false; c.launches = 0;
+  c.cur_rho = nullptr; c.cur_active = nullptr; c.cur_mask = nullptr; c.bwd_classified = false;
+  c.aux[0] = c.aux[1] = nullptr; c.ev[0] = c.ev[1] = c.ev[2] = nullptr;
+  s = check_qp(&c, qp); if (s != TMPC_OK) return s;
+  // the array keeps the previous call's contents: the per-problem status words must start at zero (the factor kernels overwrite them, this is
+  // belt and braces); the factor, the eta scratch of the streamed class and the residual partials are all written before they are read
+  if (cudaMemsetAsync(ws + L.fstatus, 0, (size_t)c.d.B * sizeof(int32_t), c.stream) != cudaSuccess) { cudaGetLastError(); return TMPC_E_CUDA; }
+  s = c.cfg.dtype == TMPC_F32 ? do_factor<float>(&c, qp) : do_factor<double>(&c, qp);
+  if (s != TMPC_OK) return s;
+  c.factored = true;
+  return c.cfg.dtype == TMPC_F32 ? do_solve<float>(&c, qp, st, iters, flags, info) : do_solve<double>(&c, qp, st, iters, flags, info);
+}
