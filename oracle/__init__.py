@@ -25,7 +25,7 @@ class Cfg(C.Structure):
         ("gamma", C.c_double), ("lam", C.c_double), ("eps_abs", C.c_double), ("eps_rel", C.c_double),
         ("wheelbase", C.c_double), ("dt", C.c_double),
         ("g_lo", C.c_double * MAXR), ("g_hi", C.c_double * MAXR),
-        ("g_col", C.c_int32 * MAXR), ("soft", C.c_uint8 * MAXR),
+        ("g_col", C.c_int32 * MAXR), ("soft", C.c_uint8 * MAXR), ("model_params", C.c_double * 16),
     ]
 
 
@@ -56,7 +56,7 @@ def make_cfg(w, band=None, zg_given=0, eps_abs=1e-8, eps_rel=1e-8, **over) -> Cf
     c.N, c.nx, c.nu, c.ng = w.N, w.nx, w.nu, w.ng
     nz = (w.N + 1) * (w.nx + w.nu)
     c.band = int(nz > 512) if band is None else int(band)
-    c.g_sel = int(w.g_col is not None and w.G is None and w.model == 0)
+    c.g_sel = int(w.g_col is not None and w.G is None and w.model != 1)      # (the bicycle model writes a dense G)
     c.zg_given = zg_given
     c.model = w.model
     c.sigma, c.rho_bar, c.rho_eq_scale, c.alpha = w.sigma, w.rho_bar, w.rho_eq_scale, w.alpha
@@ -69,6 +69,9 @@ def make_cfg(w, band=None, zg_given=0, eps_abs=1e-8, eps_rel=1e-8, **over) -> Cf
             c.g_col[r] = int(w.g_col[r])
         if w.g_lo is not None:
             c.g_lo[r], c.g_hi[r] = w.g_lo[r], w.g_hi[r]
+    if getattr(w, 'model_params', None) is not None:
+        for i, v in enumerate(w.model_params):
+            c.model_params[i] = float(v)
     for k, v in over.items():
         setattr(c, k, v)
     return c
@@ -282,4 +285,37 @@ def sqp_bicycle(w, cfg, n_sqp=None, iters=None, nthreads=1, with_fnorm=False):
     fn.argtypes = [C.c_void_p, C.c_int, C.c_int] + [C.c_void_p] * 10 + [C.c_int, C.c_int, C.c_void_p]
     rc = fn(C.byref(cfg), w.B, nthreads, _p(D), _p(E), _p(q), _p(x0), _p(ref), _p(st["x"]), _p(st["zg"]), _p(st["yf"]), _p(st["yg"]),
             _p(st["xi"]), n_sqp, iters, _p(info))
+    return st, info, rc
+
+
+def srb_step(cfg, x, u):
+    """x+ = Phi(x, u): one RK4 step of the SRB humanoid dynamics."""
+    out = np.zeros(12)
+    fn = lib().orc_srb_step
+    fn.argtypes = [C.c_void_p] * 4
+    fn(C.byref(cfg), _p(_c(x)), _p(_c(u)), _p(out))
+    return out
+
+
+def srb_linearize(w, cfg, xbar):
+    Am = np.zeros((w.N, 12, 18)); Ap = np.zeros((w.N, 12, 18)); b = np.zeros((w.N, 12))
+    fn = lib().orc_srb_linearize
+    fn.argtypes = [C.c_void_p] * 5
+    fn(C.byref(cfg), _p(_c(xbar)), _p(Am), _p(Ap), _p(b))
+    return Am, Ap, b
+
+
+def sqp_srb(w, cfg, n_sqp=None, iters=None):
+    """O-4 for the SRB model on every problem (selection rows with the workload's constant bounds).  Returns (state with x = final xbar, info, rc)."""
+    n_sqp = w.sqp_iters if n_sqp is None else n_sqp
+    iters = w.iters if iters is None else iters
+    st = new_state(w); st["x"] = _c(w.xbar0).copy()
+    info = np.zeros((w.B, 4))
+    D, E = _c(w.D[0]), _c(w.E[0])
+    fn = lib().orc_sqp_srb
+    fn.argtypes = [C.c_void_p] * 12 + [C.c_int, C.c_int, C.c_void_p]
+    rc = 0
+    for b in range(w.B):
+        rc |= fn(C.byref(cfg), _p(D), _p(E), _p(_c(w.q[b])), _p(_c(w.x_init[b])), _p(_c(w.lo[b])), _p(_c(w.hi[b])), _p(st["x"][b]), _p(st["zg"][b]),
+                 _p(st["yf"][b]), _p(st["yg"][b]), _p(st["xi"][b]), n_sqp, iters, _p(info[b]))
     return st, info, rc

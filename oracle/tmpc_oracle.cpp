@@ -19,6 +19,7 @@
 //                   by eq. 36-38.
 //   f1   adaptive   Alg. 3 with the adaptive step size of eq. 17 and the termination test eq. 4 (admm_adaptive).
 //   f2   SQP + linesearch   App. D l1-merit backtracking and the convergence test eq. 18 (sqp_ls_bicycle).
+//   f3   SRB model  single-rigid-body humanoid dynamics (eq. 68-69) + RK4 and its eq. 36-37 blocks by forward-mode dual numbers.
 //   O-5  backward   the definition: dense active-set KKT system eq. 62 / 65 solved by
 //                   Gaussian elimination with partial pivoting; dL/dq = -eta_x, dL/dx_init = +eta_f[0:nx].
 //
@@ -55,6 +56,7 @@ struct Cfg {              // mirrored field-by-field by oracle/__init__.py (ctyp
   double g_lo[64], g_hi[64];  // un-shifted bounds of g_t (model != 0)
   int32_t g_col[64];
   uint8_t soft[64];       // per-row delta_xi (reading A-13)
+  double model_params[16]; // model 2 (SRB humanoid): mass, g[3], diag(I)[3], foot_L[3], foot_R[3] (world positions)
 };
 
 // ---- symmetric band matrix, lower storage: element (i,j), i-bw <= j <= i, at a[i*(bw+1) + (j-i+bw)]
@@ -408,6 +410,81 @@ void bicycle_linearize(const Cfg& cf, const double* xbar, const double* ref, dou
   }
 }
 
+// ---- f3: single-rigid-body humanoid model (eq. 68-69), RK4 with step cf.dt: x = (p, Theta = (roll, pitch, yaw), v, omega),
+// u = (f_L, f_R) world-frame foot forces.  Readings (A-38): I = diag(model_params[4..6]) in the body frame; the contact vectors are
+// r_i = foot_i - p with fixed world foot positions (model_params[7..12]); the torque r x f enters eq. 68d as printed (no frame change).
+// Written once as a template over the scalar type so that the SAME lines give values (double) and exact directional derivatives (Dual).
+struct Dual { double v, d; };
+inline Dual operator+(Dual a, Dual b) { return {a.v + b.v, a.d + b.d}; }
+inline Dual operator-(Dual a, Dual b) { return {a.v - b.v, a.d - b.d}; }
+inline Dual operator*(Dual a, Dual b) { return {a.v * b.v, a.d * b.v + a.v * b.d}; }
+inline Dual operator/(Dual a, Dual b) { return {a.v / b.v, (a.d * b.v - a.v * b.d) / (b.v * b.v)}; }
+inline Dual operator*(double a, Dual b) { return {a * b.v, a * b.d}; }
+inline Dual operator+(Dual a, double b) { return {a.v + b, a.d}; }
+inline Dual operator-(double a, Dual b) { return {a - b.v, -b.d}; }
+inline Dual dsin(Dual a) { return {std::sin(a.v), std::cos(a.v) * a.d}; }
+inline Dual dcos(Dual a) { return {std::cos(a.v), -std::sin(a.v) * a.d}; }
+inline double dsin(double a) { return std::sin(a); }
+inline double dcos(double a) { return std::cos(a); }
+
+template <typename S>
+void srb_xdot(const double* mp, const S* x, const S* u, S* xd) {       // eq. 68a-d with T(Theta) of eq. 69
+  const double mass = mp[0];
+  const S phi = x[3], th = x[4];
+  const S sp = dsin(phi), cp = dcos(phi), st = dsin(th), ct = dcos(th), tt = st / ct;
+  for (int i = 0; i < 3; ++i) xd[i] = x[6 + i];                          // p' = v
+  const S w0 = x[9], w1 = x[10], w2 = x[11];
+  xd[3] = w0 + sp * tt * w1 + cp * tt * w2;                              // Theta' = T(Theta) omega
+  xd[4] = cp * w1 - sp * w2;
+  xd[5] = sp / ct * w1 + cp / ct * w2;
+  for (int i = 0; i < 3; ++i) xd[6 + i] = (1.0 / mass) * (u[i] + u[3 + i]) + mp[1 + i];     // v' = (f_L + f_R)/m + g
+  S tau[3];
+  for (int i = 0; i < 3; ++i) tau[i] = 0.0 * w0;
+  for (int f = 0; f < 2; ++f) {                                          // r x f, r = foot - p
+    S r[3]; for (int i = 0; i < 3; ++i) r[i] = mp[7 + 3 * f + i] - x[i];
+    const S* F = u + 3 * f;
+    tau[0] = tau[0] + (r[1] * F[2] - r[2] * F[1]); tau[1] = tau[1] + (r[2] * F[0] - r[0] * F[2]); tau[2] = tau[2] + (r[0] * F[1] - r[1] * F[0]);
+  }
+  const S Iw0 = mp[4] * w0, Iw1 = mp[5] * w1, Iw2 = mp[6] * w2;          // omega x (I omega)
+  xd[9] = (1.0 / mp[4]) * (tau[0] - (w1 * Iw2 - w2 * Iw1));
+  xd[10] = (1.0 / mp[5]) * (tau[1] - (w2 * Iw0 - w0 * Iw2));
+  xd[11] = (1.0 / mp[6]) * (tau[2] - (w0 * Iw1 - w1 * Iw0));
+}
+template <typename S>
+void srb_rk4(const double* mp, double dt, const S* x, const S* u, S* xn) {   // classical RK4: x+ = x + dt/6 (k1 + 2 k2 + 2 k3 + k4)
+  S k1[12], k2[12], k3[12], k4[12], xt[12];
+  srb_xdot(mp, x, u, k1);
+  for (int i = 0; i < 12; ++i) xt[i] = x[i] + (0.5 * dt) * k1[i];
+  srb_xdot(mp, xt, u, k2);
+  for (int i = 0; i < 12; ++i) xt[i] = x[i] + (0.5 * dt) * k2[i];
+  srb_xdot(mp, xt, u, k3);
+  for (int i = 0; i < 12; ++i) xt[i] = x[i] + dt * k3[i];
+  srb_xdot(mp, xt, u, k4);
+  for (int i = 0; i < 12; ++i) xn[i] = x[i] + (dt / 6.0) * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+}
+// eq. 36-37 for f_k(v_k, v_{k+1}) = Phi(x_k, u_k) - x_{k+1}: Am = [dPhi/dx dPhi/du] (one Dual sweep per column), Ap = [-I 0], b = Am v_k + Ap v_{k+1} - f_k
+void srb_linearize(const Cfg& cf, const double* xbar, double* Am, double* Ap, double* b) {
+  const int N = cf.N, n = 18, nx = 12;
+  for (int t = 0; t < N; ++t) {
+    const double* vk = xbar + (size_t)t * n; const double* vk1 = vk + n;
+    double* am = Am + (size_t)t * nx * n; double* ap = Ap + (size_t)t * nx * n;
+    for (int j = 0; j < n; ++j) {
+      Dual xd[12], ud[6], out[12];
+      for (int i = 0; i < 12; ++i) xd[i] = {vk[i], i == j ? 1.0 : 0.0};
+      for (int i = 0; i < 6; ++i) ud[i] = {vk[12 + i], 12 + i == j ? 1.0 : 0.0};
+      srb_rk4<Dual>(cf.model_params, cf.dt, xd, ud, out);
+      for (int i = 0; i < nx; ++i) am[i * n + j] = out[i].d;
+    }
+    for (int i = 0; i < nx; ++i) for (int j = 0; j < n; ++j) ap[i * n + j] = (i == j) ? -1.0 : 0.0;
+    double phi[12]; srb_rk4<double>(cf.model_params, cf.dt, vk, vk + 12, phi);
+    for (int i = 0; i < nx; ++i) {
+      double sacc = -(phi[i] - vk1[i]);
+      for (int j = 0; j < n; ++j) sacc += am[i * n + j] * vk[j] + ap[i * n + j] * vk1[j];
+      b[(size_t)t * nx + i] = sacc;
+    }
+  }
+}
+
 // ---- f2: SQP with the l1-merit backtracking linesearch of App. D and the convergence test eq. 18
 // (PAPER.md:305-314), for the bicycle model.  Readings (A-34..A-37):
 //   x~ = (x, xi); l(x~) = 1/2 x'Px + q'x + sum_soft (lam |xi| + gamma/2 xi^2); f(x~) = (x_0 - x_init ; f_k(v_k, v_{k+1}));
@@ -619,6 +696,22 @@ int orc_sqp_ls_bicycle(const Cfg* cf, const SqpOpt* op, const double* D, const d
   return sqp_ls_bicycle(*cf, *op, D, E, q, x_init, ref, xbar, zg, yf, yg, xi, info_out, log_out);
 }
 int orc_sizeof_sqpopt() { return (int)sizeof(SqpOpt); }
+
+// f3: SRB humanoid model.  orc_srb_step: x+ = Phi(x, u) (RK4 of eq. 68); orc_srb_linearize: eq. 36-37 blocks; orc_sqp_srb: the fixed-count full-step
+// SQP driver of O-4 (reading A-26) around them, inequality rows = selection rows with the caller's constant bounds (eq. 70d).
+void orc_srb_step(const Cfg* cf, const double* x, const double* u, double* xn) { srb_rk4<double>(cf->model_params, cf->dt, x, u, xn); }
+void orc_srb_linearize(const Cfg* cf, const double* xbar, double* Am, double* Ap, double* b) { srb_linearize(*cf, xbar, Am, Ap, b); }
+int orc_sqp_srb(const Cfg* cf, const double* D, const double* E, const double* q, const double* x_init, const double* lo, const double* hi, double* xbar,
+                double* zg, double* yf, double* yg, double* xi, int n_sqp, int K, double* info_out) {
+  const int N = cf->N, n = 18, nx = 12;
+  vec Am((size_t)N * nx * n), Ap((size_t)N * nx * n), b((size_t)N * nx);
+  Cfg c = *cf; c.g_sel = 1; c.zg_given = 0; int fail = 0;
+  for (int s = 0; s < n_sqp; ++s) {
+    srb_linearize(c, xbar, Am.data(), Ap.data(), b.data());
+    fail |= orc_admm(&c, D, E, q, Am.data(), Ap.data(), b.data(), x_init, nullptr, lo, hi, xbar, zg, yf, yg, xi, K, info_out);
+  }
+  return fail;
+}
 
 int orc_sizeof_cfg() { return (int)sizeof(Cfg); }
 

@@ -107,6 +107,7 @@ class QPData:
     wheelbase: float = 2.7
     dt: float = 0.05
     sqp_iters: int = 0
+    model_params: Optional[list] = None  # model 2 (SRB humanoid): mass, g[3], diag(I)[3], foot_L[3], foot_R[3]
 
     @property
     def n(self) -> int:
@@ -430,3 +431,36 @@ def linear_rl(seed: int = 0, B: int = 64, N: int = 40, nx: int = 8, nu: int = 4,
     hi = np.full((B, T, nu), u_max)
     return QPData(f"f4_linear_rl_umax{u_max:g}", B, N, nx, nu, nu, dtype, D, E, np.zeros((B, T, n)), Am, Ap, b, x0, None, lo, hi,
                   g_col=list(range(nx, n)), soft=[0] * nu, iters=100)
+
+
+# --------------------------------------------------------------------------- f3: SRB humanoid balancing OCP
+SRB_PARAMS = [33.34, 0.0, 0.0, -9.81, 1.2, 1.0, 0.4, 0.0, 0.1, 0.0, 0.0, -0.1, 0.0]   # m, g, diag(I) and foot positions: proposed (A-38)
+
+
+def srb_humanoid(seed: int = 0, B: int = 64, N: int = 20, dtype: str = "f64", sqp_iters: int = 4, iters: int = 60, first_problem: int = 0) -> QPData:
+    """Humanoid balancing OCP of the paper's imitation-learning experiment (eq. 68-70): single-rigid-body dynamics,
+    x = (p, Theta, v, omega) in R^12, u = (f_L, f_R) in R^6, RK4 with dt = 0.025, N = 20, cost dx'Q dx + du'R du with Q = diag(exp(theta)),
+    R = 1e-3 I, box bounds on u (eq. 70d).  The paper gives m = 33.34 kg and g; proposed here (reading A-38, the paper is silent): I = diag(1.2,
+    1.0, 0.4) kg m^2, feet at (0, +-0.1, 0) m, standing reference p_ref = (0, 0, 0.6), u_ref = (0, 0, m g / 2) per foot, log-weights theta =
+    log(100, 100, 100, 50, 50, 50, 1, 1, 1, 1, 1, 1), bounds f_xy in [-60, 60] N, f_z in [0, 400] N, and a perturbed start
+    x_init = x_ref + (N(0, 0.03^2) on p, N(0, 0.08^2) on Theta, N(0, 0.2^2) on v, N(0, 0.3^2) on omega).  Draw order: the 12 normals of x_init."""
+    nx, nu, n, T = 12, 6, 18, N + 1
+    mp = list(SRB_PARAMS)
+    mass, gz = mp[0], mp[3]
+    st = Streams(seed, 12, np.arange(first_problem, first_problem + B))
+    nrm = st.normal(12)
+    x_ref = np.zeros(12); x_ref[2] = 0.6
+    u_ref = np.array([0.0, 0.0, -mass * gz / 2.0] * 2)
+    sd = np.array([0.03] * 3 + [0.08] * 3 + [0.2] * 3 + [0.3] * 3)
+    x_init = x_ref[None, :] + sd[None, :] * nrm
+    Q = 2.0 * np.diag([100.0] * 3 + [50.0] * 3 + [1.0] * 6)           # dx'Q dx without 1/2 -> D = 2 Q in the 1/2-convention (A-9)
+    R = 2.0 * 1e-3 * np.eye(nu)
+    D, E = _rate_cost_blocks(T, nx, nu, Q, R, None)
+    ref = np.concatenate([x_ref, u_ref])
+    q = np.broadcast_to(-(D[0, 0] @ ref), (B, T, n)).copy()
+    stage_ref = np.broadcast_to(ref, (B, T, n)).copy()
+    xbar0 = stage_ref.copy(); xbar0[:, 0, :nx] = x_init
+    lo = np.broadcast_to(np.array([-60.0, -60.0, 0.0] * 2), (B, T, nu)).copy()
+    hi = np.broadcast_to(np.array([60.0, 60.0, 400.0] * 2), (B, T, nu)).copy()
+    return QPData("f3_srb_humanoid", B, N, nx, nu, nu, dtype, D, E, q, None, None, None, x_init, None, lo, hi, g_col=list(range(nx, n)),
+                  soft=[0] * nu, rho_bar=0.1, iters=iters, model=2, stage_ref=stage_ref, xbar0=xbar0, dt=0.025, sqp_iters=sqp_iters, model_params=mp)

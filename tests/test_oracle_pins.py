@@ -720,3 +720,84 @@ def test_sqp_linesearch_steps_recomputed_in_numpy():
         assert np.abs(cur[k] - st_all[k]).max() <= 1e-10 * max(1.0, np.abs(st_all[k]).max()), k
     assert info[0, 1] == 1 and info[0, 3] <= eps_c, "the run must converge by eq. 18"
     print("alphas", log[0, :int(info[0, 0]), 0], "backtracked", seen_backtrack)
+
+
+# ----------------------------------------------------------------------------------------------- f3: SRB humanoid model (eq. 68-69 + RK4)
+def test_srb_model_closed_forms_and_rk4_order():
+    """(i) no forces, no spin: free fall p(t) = p0 + v0 t + g t^2 / 2, v(t) = v0 + g t is a quadratic and RK4 integrates it exactly (eq. 68a, 68c);
+    (ii) standing reference with u_ref = m g / 2 per foot is an equilibrium (feet symmetric about the CoM: zero net torque);
+    (iii) torque-free spin about a principal axis keeps omega constant and turns the yaw at that rate (eq. 68b with T(0) = I, eq. 68d);
+    (iv) the one-step error against 64 sub-steps shrinks ~32x when dt is halved (local error of a 4th-order scheme)."""
+    import copy
+    w = W.srb_humanoid(B=1)
+    cfg = O.make_cfg(w)
+    x = np.array([0.1, -0.2, 0.7, 0, 0, 0, 0.3, -0.1, 0.5, 0, 0, 0.0]); u = np.zeros(6)
+    xn = O.srb_step(cfg, x, u)
+    g = np.array([0, 0, -9.81]); dt = w.dt
+    assert np.abs(xn[:3] - (x[:3] + dt * x[6:9] + 0.5 * dt * dt * g)).max() < 1e-14 and np.abs(xn[6:9] - (x[6:9] + dt * g)).max() < 1e-14
+    assert np.abs(xn[3:6]).max() == 0 and np.abs(xn[9:]).max() == 0
+    xr, ur = w.stage_ref[0, 0, :12], w.stage_ref[0, 0, 12:]
+    assert np.abs(O.srb_step(cfg, xr, ur) - xr).max() < 1e-14
+    xs = xr.copy(); xs[11] = 0.8                                             # spin about the body z axis, upright
+    xn = O.srb_step(cfg, xs, ur)
+    assert abs(xn[11] - 0.8) < 1e-14 and abs(xn[5] - 0.8 * dt) < 1e-14 and np.abs(xn[3:5]).max() < 1e-14
+
+    def fine(cfg_, x_, u_, dt_, sub=64):
+        c2 = copy.copy(cfg_); c2.dt = dt_ / sub
+        for _ in range(sub):
+            x_ = O.srb_step(c2, x_, u_)
+        return x_
+    rng = np.random.default_rng(0)
+    x = xr + np.concatenate([0.05 * rng.standard_normal(3), 0.2 * rng.standard_normal(3), 0.3 * rng.standard_normal(3), 0.5 * rng.standard_normal(3)])
+    u = ur + 5.0 * rng.standard_normal(6)
+    errs = []
+    for dt_ in (0.1, 0.05):
+        c1 = copy.copy(cfg); c1.dt = dt_
+        errs.append(np.abs(O.srb_step(c1, x, u) - fine(cfg, x, u, dt_)).max())
+    assert 20.0 < errs[0] / errs[1] < 45.0, errs
+
+
+def test_srb_jacobians_match_finite_differences_and_eq37():
+    """A^- = [dPhi/dx dPhi/du] (forward-mode dual numbers in the oracle) == central finite differences of the RK4 flow; A^+ = [-I 0];
+    b == A^- v_k + A^+ v_{k+1} - f_k (eq. 37); the torque term: d(omega+)/d(f) has the size dt r / I (the cross product is there)."""
+    w = W.srb_humanoid(B=2, N=6)
+    cfg = O.make_cfg(w)
+    rng = np.random.default_rng(1)
+    xbar = w.xbar0[1] + np.concatenate([0.05 * rng.standard_normal((w.T, 3)), 0.2 * rng.standard_normal((w.T, 3)), 0.3 * rng.standard_normal((w.T, 6)),
+                                        20.0 * rng.standard_normal((w.T, 6))], axis=1)
+    Am, Ap, b = O.srb_linearize(w, cfg, xbar)
+    h = 1e-6
+    for t in (0, 3, 5):
+        vk, vk1 = xbar[t], xbar[t + 1]
+        for j in range(18):
+            e = np.zeros(18); e[j] = h * max(1.0, abs(vk[j]))
+            fd = (O.srb_step(cfg, (vk + e)[:12], (vk + e)[12:]) - O.srb_step(cfg, (vk - e)[:12], (vk - e)[12:])) / (2 * e[j])
+            assert np.abs(fd - Am[t][:, j]).max() < 1e-7 * max(1.0, np.abs(Am[t][:, j]).max()), (t, j)
+        assert np.abs(Ap[t] - np.hstack([-np.eye(12), np.zeros((12, 6))])).max() == 0
+        f = O.srb_step(cfg, vk[:12], vk[12:]) - vk1[:12]
+        assert np.abs(b[t] - (Am[t] @ vk + Ap[t] @ vk1 - f)).max() < 1e-11
+    assert np.abs(Am[0][9:12, 12:]).max() > 1e-3            # forces torque the body
+
+
+def test_srb_sqp_driver_reaches_the_reference():
+    """Fixed-count SQP on the balancing OCP: the dynamics residual of the final iterate is small, the bounds on u hold, and one SQP step equals
+    linearise + Alg. 3 by hand (the pieces pinned above)."""
+    import copy
+    w = W.srb_humanoid(B=2, N=10)
+    cfg = O.make_cfg(w)
+    st, info, rc = O.sqp_srb(w, cfg, n_sqp=5, iters=150)
+    assert rc == 0
+    for b in range(w.B):
+        x = st["x"][b]
+        res = max(np.abs(O.srb_step(cfg, x[t, :12], x[t, 12:]) - x[t + 1, :12]).max() for t in range(w.N))
+        assert res < 1e-3
+        assert (x[:, 12:] >= w.lo[b] - 1e-3).all() and (x[:, 12:] <= w.hi[b] + 1e-3).all()
+    st1, _, _ = O.sqp_srb(w, cfg, n_sqp=1, iters=40)
+    for b in range(w.B):
+        Am, Ap, bb = O.srb_linearize(w, cfg, w.xbar0[b])
+        wq = copy.copy(w)
+        wq.B, wq.Am, wq.Ap, wq.b, wq.model = 1, Am[None], Ap[None], bb[None], 0
+        wq.q, wq.x_init, wq.lo, wq.hi = w.q[b:b + 1], w.x_init[b:b + 1], w.lo[b:b + 1], w.hi[b:b + 1]
+        s0 = O.new_state(wq); s0["x"] = w.xbar0[b:b + 1].copy()
+        s, _, _ = O.admm(wq, O.make_cfg(wq), iters=40, state=s0)
+        assert np.abs(s["x"][0] - st1["x"][b]).max() < 1e-12
