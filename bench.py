@@ -422,6 +422,30 @@ def f4_rows(ctx, args):
     return rows
 
 
+def f3_row(ctx, args):
+    """f3: the humanoid balancing OCP of the paper's imitation-learning experiment (SRB dynamics, RK4, nx = 12, nu = 6, N = 20) with
+    the second built-in model: n_sqp x (tmpc_linearize + tmpc_factor + tmpc_admm_solve), fp64 like the paper, B = 1024."""
+    import torch
+    from paper_2606_24039_b200 import workloads as W
+    from paper_2606_24039_b200.solver import Solver
+    dev = ctx["dev"]
+    w = W.srb_humanoid(B=1024)
+    s = Solver(w, dtype="f64", device=dev)
+    x0 = s._up(w.xbar0)
+    ts = []
+    for _ in range(6):
+        for k, v in s.s.items():
+            v.copy_(x0) if k == "x" else v.zero_()
+        torch.cuda.synchronize(dev)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); s.sqp(); b.record(); torch.cuda.synchronize(dev); ts.append(a.elapsed_time(b))
+    info = s.info_numpy()
+    s.close()
+    ms = float(np.median(ts[2:]))
+    return {"workload": workload_name(w, "f64"), "ms_per_batched_solve": ms, "qp_solves_per_s": w.B / (ms * 1e-3),
+            "admm_iters_per_s": w.B * total_iters(w) / (ms * 1e-3), "max_r_prim": float(np.max(info["r_prim"])), "kernels": "srb_linearize_kernel + factor_kernel + admm_kernel (generic class, n = 18)"}
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -445,9 +469,10 @@ def run_gpu(args):
         steps = args.steps if (args.config is not None or i == 0) else max(3, min(args.steps, STEPS_CAP.get(c, args.steps)))
         res.append((c, d, gpu_one(c, d, args, ctx, steps, world == 1 and not args.no_cpu_baseline)))
     f4 = f4_rows(ctx, args) if (args.config is None and world == 1 and not args.no_f4) or args.f4_only else None
+    f3 = f3_row(ctx, args) if f4 is not None else None
     if args.f4_only:
         if rank == 0:
-            print(json.dumps({"metric": "f4 linear-system RL workload (PAPER.md:414-416)", "rows": f4, "measured_peaks": ctx["peaks"]}))
+            print(json.dumps({"metric": "f4 linear-system RL workload (PAPER.md:414-416) and f3 humanoid OCP", "rows": f4, "f3_srb_humanoid": f3, "measured_peaks": ctx["peaks"]}))
         return
     if rank == 0:
         c0, d0, head = res[0]
@@ -459,6 +484,7 @@ def run_gpu(args):
             line["gpu_launches"] = int(sum(r["gpu_launches"] for _, _, r in res))
         if f4 is not None:
             line.setdefault("per_config", {})["f4_linear_rl"] = f4
+            line["per_config"]["f3_srb_humanoid"] = f3
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -39,7 +39,7 @@ typedef struct tmpc_ctx* tmpc_handle; /* opaque; owns nothing the caller passed 
 typedef enum { TMPC_OK = 0, TMPC_E_BADARG, TMPC_E_DIM, TMPC_E_UNSUPPORTED, TMPC_E_STATE, TMPC_E_WORKSPACE, TMPC_E_CUDA,
                TMPC_E_STATIC_LIMIT /* tmpc_admm_solve_static: the problem needs more than TMPC_STATIC_SCRATCH_BYTES of scratch */ } tmpc_status;
 typedef enum { TMPC_F32 = 0, TMPC_F64 = 1 } tmpc_dtype;
-typedef enum { TMPC_MODEL_NONE = 0, TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT = 1 } tmpc_model;
+typedef enum { TMPC_MODEL_NONE = 0, TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT = 1, TMPC_MODEL_SRB_HUMANOID_RK4 = 2 } tmpc_model;
 typedef enum { TMPC_LIN_SEQUENTIAL = 0, TMPC_LIN_CYCLIC_REDUCTION = 1, TMPC_LIN_AUTO = 2 } tmpc_linsolve;
 typedef enum { TMPC_BWD_REFACTOR_REFINE = 0, TMPC_BWD_ADMM_REUSE_FACTOR = 1 } tmpc_bwd_mode;
 
@@ -62,6 +62,8 @@ typedef struct { /* POD, copied at tmpc_setup */
   int32_t g_is_selection;                     /* 1: row r of every G_t is the unit vector e_{g_col[r]} and qp.G is NULL */
   int32_t g_col[TMPC_MAX_NG];
   uint8_t soft_row[TMPC_MAX_NG];              /* per-row delta_xi, same for every stage and problem */
+  double model_params[16];                    /* TMPC_MODEL_SRB_HUMANOID_RK4 (eq. 68-69; nx = 12, nu = 6, step `dt`): mass, g[3],
+                                                 diag of the body inertia [3], world positions of the left and the right foot [3] + [3] */
 } tmpc_config;
 
 typedef struct {
@@ -95,7 +97,9 @@ tmpc_status tmpc_workspace_bytes(const tmpc_config* cfg, size_t* bytes);
  * alive until tmpc_destroy.  cuda_stream: a cudaStream_t (NULL = default stream). */
 tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, void* cuda_stream, tmpc_handle* out);
 /* a1 (eq. 36-38): linearise the built-in model at xbar [B][T][n] against stage_ref [B][T][n]
- * (x_ref,u_ref per stage); writes qp->Am, Ap, b, G, lo, hi.  TMPC_E_UNSUPPORTED for TMPC_MODEL_NONE. */
+ * (x_ref,u_ref per stage); writes qp->Am, Ap, b, G, lo, hi.  TMPC_E_UNSUPPORTED for TMPC_MODEL_NONE.
+ * TMPC_MODEL_SRB_HUMANOID_RK4 has box bounds on u only (eq. 70d: selection rows, constant bounds): it writes Am, Ap, b and leaves qp->G, lo,
+ * hi alone (G may be NULL, stage_ref is not read). */
 tmpc_status tmpc_linearize(tmpc_handle h, const void* xbar, const void* stage_ref, tmpc_qp* qp);
 /* a2+a3: assemble Theta_t, Phi_t and factor S block by block into the workspace. */
 tmpc_status tmpc_factor(tmpc_handle h, const tmpc_qp* qp);

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtmpc.so")
 TMPC_MAX_NG = 32
 TMPC_F32, TMPC_F64 = 0, 1
-TMPC_MODEL_NONE, TMPC_MODEL_BICYCLE = 0, 1
+TMPC_MODEL_NONE, TMPC_MODEL_BICYCLE, TMPC_MODEL_SRB = 0, 1, 2
 TMPC_LIN_SEQUENTIAL, TMPC_LIN_CYCLIC_REDUCTION, TMPC_LIN_AUTO = 0, 1, 2
 TMPC_BWD_REFACTOR_REFINE, TMPC_BWD_ADMM_REUSE_FACTOR = 0, 1
 TMPC_SOLVE_ZG_GIVEN = 1
@@ -33,7 +33,8 @@ class TmpcConfig(C.Structure):
                 ("eps_active_abs", C.c_double), ("eps_active_rel", C.c_double),
                 ("wheelbase", C.c_double), ("dt", C.c_double),
                 ("g_lo", C.c_double * TMPC_MAX_NG), ("g_hi", C.c_double * TMPC_MAX_NG),
-                ("g_is_selection", C.c_int32), ("g_col", C.c_int32 * TMPC_MAX_NG), ("soft_row", C.c_uint8 * TMPC_MAX_NG)]
+                ("g_is_selection", C.c_int32), ("g_col", C.c_int32 * TMPC_MAX_NG), ("soft_row", C.c_uint8 * TMPC_MAX_NG),
+                ("model_params", C.c_double * 16)]
 
 
 class TmpcQp(C.Structure):
@@ -114,7 +115,10 @@ def make_config(w, batch=None, dtype=None, linsolve=TMPC_LIN_SEQUENTIAL, eps_abs
     c.eps_active_abs = tol if eps_abs is None else eps_abs
     c.eps_active_rel = tol if eps_rel is None else eps_rel
     c.wheelbase, c.dt = w.wheelbase, w.dt
-    c.g_is_selection = int(w.G is None and w.g_col is not None and w.model == 0)
+    c.g_is_selection = int(w.G is None and w.g_col is not None and w.model != 1)      # (the bicycle model writes a dense G)
+    if getattr(w, 'model_params', None) is not None:
+        for i, v in enumerate(w.model_params):
+            c.model_params[i] = float(v)
     for r in range(w.ng):
         c.soft_row[r] = int(w.soft[r])
         if c.g_is_selection:

@@ -17,6 +17,7 @@
 #include "tmpc_cr2.cuh"
 #include "tmpc_peak.cuh"
 #include "tmpc_sqp.cuh"
+#include "tmpc_srb.cuh"
 
 using namespace tmpc;
 
@@ -76,7 +77,9 @@ tmpc_status check_cfg(const tmpc_config* c) {
   if (!(c->slack_gamma >= 0) || !(c->slack_lambda >= 0)) return TMPC_E_BADARG;
   if (c->g_is_selection) for (int r = 0; r < c->ng; ++r) if (c->g_col[r] < 0 || c->g_col[r] >= c->nx + c->nu) return TMPC_E_BADARG;
   if (c->model == TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT && (c->nx != 4 || c->nu != 2 || c->ng != 3 || c->g_is_selection)) return TMPC_E_DIM;
-  if (c->model != TMPC_MODEL_NONE && c->model != TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT) return TMPC_E_BADARG;
+  if (c->model == TMPC_MODEL_SRB_HUMANOID_RK4 && (c->nx != 12 || c->nu != 6 || (c->ng > 0 && !c->g_is_selection) || !(c->model_params[0] > 0) ||
+                                                 !(c->model_params[4] > 0) || !(c->model_params[5] > 0) || !(c->model_params[6] > 0) || !(c->dt > 0))) return TMPC_E_DIM;
+  if (c->model != TMPC_MODEL_NONE && c->model != TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT && c->model != TMPC_MODEL_SRB_HUMANOID_RK4) return TMPC_E_BADARG;
   return TMPC_OK;
 }
 
@@ -527,7 +530,22 @@ tmpc_status tmpc_destroy(tmpc_handle h) {
 }
 int64_t tmpc_launch_count(tmpc_handle h) { return h ? h->launches : 0; }
 
+extern "C++" {
+template <typename T>
+static tmpc_status srb_linearize_launch(tmpc_handle h, const void* xbar, tmpc_qp* qp) {
+  SrbArgs<T> a; a.B = h->d.B; a.N = h->d.N; a.dt = (T)h->cfg.dt;
+  for (int k = 0; k < 13; ++k) a.mp[k] = (T)h->cfg.model_params[k];
+  a.xbar = (const T*)xbar; a.Am = (T*)qp->Am; a.Ap = (T*)qp->Ap; a.b = (T*)qp->b;
+  srb_linearize_kernel<T><<<(unsigned)((long long)h->d.B * h->d.N), 32, 0, h->stream>>>(a); h->launches++;
+  return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+}
+}  // extern "C++"
+
 tmpc_status tmpc_linearize(tmpc_handle h, const void* xbar, const void* stage_ref, tmpc_qp* qp) {
+  if (h && h->cfg.model == TMPC_MODEL_SRB_HUMANOID_RK4) {
+    if (!xbar || !qp || !qp->Am || !qp->Ap || !qp->b) return TMPC_E_BADARG;
+    return h->cfg.dtype == TMPC_F32 ? srb_linearize_launch<float>(h, xbar, qp) : srb_linearize_launch<double>(h, xbar, qp);
+  }
   if (!h || !xbar || !stage_ref || !qp || !qp->Am || !qp->Ap || !qp->b || !qp->G || !qp->lo || !qp->hi) return TMPC_E_BADARG;
   if (h->cfg.model != TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT) return TMPC_E_UNSUPPORTED;
   if (qp->G_bstride != (int64_t)h->d.T * 3 * 6 && h->d.B > 1) return TMPC_E_BADARG;

@@ -47,6 +47,11 @@ class Solver:
         if w.model == 0:
             t["Am"], t["Ap"], t["b"], t["lo"], t["hi"] = self._up(w.Am), self._up(w.Ap), self._up(w.b), self._up(w.lo), self._up(w.hi)
             t["G"] = self._up(w.G) if w.G is not None else None
+        elif w.model == B.TMPC_MODEL_SRB:                 # box bounds on u (selection rows): tmpc_linearize writes Am, Ap, b only
+            z = lambda *s: torch.zeros(*s, dtype=self.td, device=self.dev)
+            t["Am"], t["Ap"], t["b"] = z(Bn, N, nx, n), z(Bn, N, nx, n), z(Bn, N, nx)
+            t["G"], t["lo"], t["hi"] = None, self._up(w.lo), self._up(w.hi)
+            t["stage_ref"] = self._up(w.stage_ref)
         else:
             z = lambda *s: torch.zeros(*s, dtype=self.td, device=self.dev)
             t["Am"], t["Ap"], t["b"] = z(Bn, N, nx, n), z(Bn, N, nx, n), z(Bn, N, nx)

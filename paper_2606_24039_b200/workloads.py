@@ -442,7 +442,8 @@ def srb_humanoid(seed: int = 0, B: int = 64, N: int = 20, dtype: str = "f64", sq
     x = (p, Theta, v, omega) in R^12, u = (f_L, f_R) in R^6, RK4 with dt = 0.025, N = 20, cost dx'Q dx + du'R du with Q = diag(exp(theta)),
     R = 1e-3 I, box bounds on u (eq. 70d).  The paper gives m = 33.34 kg and g; proposed here (reading A-38, the paper is silent): I = diag(1.2,
     1.0, 0.4) kg m^2, feet at (0, +-0.1, 0) m, standing reference p_ref = (0, 0, 0.6), u_ref = (0, 0, m g / 2) per foot, log-weights theta =
-    log(100, 100, 100, 50, 50, 50, 1, 1, 1, 1, 1, 1), bounds f_xy in [-60, 60] N, f_z in [0, 400] N, and a perturbed start
+    log(100, 100, 100, 50, 50, 50, 1, 1, 1, 1, 1, 1), bounds f_xy in [-8, 8] N, f_z in [150, 170] N (tight enough to bind on the perturbed
+    starts: the unconstrained controller asks for +-15 N and 157..173 N), and a perturbed start
     x_init = x_ref + (N(0, 0.03^2) on p, N(0, 0.08^2) on Theta, N(0, 0.2^2) on v, N(0, 0.3^2) on omega).  Draw order: the 12 normals of x_init."""
     nx, nu, n, T = 12, 6, 18, N + 1
     mp = list(SRB_PARAMS)
@@ -460,7 +461,7 @@ def srb_humanoid(seed: int = 0, B: int = 64, N: int = 20, dtype: str = "f64", sq
     q = np.broadcast_to(-(D[0, 0] @ ref), (B, T, n)).copy()
     stage_ref = np.broadcast_to(ref, (B, T, n)).copy()
     xbar0 = stage_ref.copy(); xbar0[:, 0, :nx] = x_init
-    lo = np.broadcast_to(np.array([-60.0, -60.0, 0.0] * 2), (B, T, nu)).copy()
-    hi = np.broadcast_to(np.array([60.0, 60.0, 400.0] * 2), (B, T, nu)).copy()
+    lo = np.broadcast_to(np.array([-8.0, -8.0, 150.0] * 2), (B, T, nu)).copy()
+    hi = np.broadcast_to(np.array([8.0, 8.0, 170.0] * 2), (B, T, nu)).copy()
     return QPData("f3_srb_humanoid", B, N, nx, nu, nu, dtype, D, E, q, None, None, None, x_init, None, lo, hi, g_col=list(range(nx, n)),
                   soft=[0] * nu, rho_bar=0.1, iters=iters, model=2, stage_ref=stage_ref, xbar0=xbar0, dt=0.025, sqp_iters=sqp_iters, model_params=mp)

@@ -670,3 +670,45 @@ def test_adaptive_on_the_streamed_class_fp64():
     assert (np.abs(out["rho"] - rinfo[:, 5]) <= 1e-6 * np.abs(rinfo[:, 5])).all()
     compare_states(s.state_numpy(), ref, 1e-7)
     s.close()
+
+
+# ----------------------------------------------------------------------------------------------- f3: SRB humanoid model (second built-in model)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_srb_linearize_matches_oracle(dtype):
+    """tmpc_linearize for TMPC_MODEL_SRB_HUMANOID_RK4 (eq. 68-69 + RK4): A^- = [dPhi/dx dPhi/du], A^+ = [-I 0], b (eq. 36-37)
+    element-wise against the oracle at a perturbed iterate (large angles, forces and spins so that every term of eq. 68 is active)."""
+    from paper_2606_24039_b200.solver import Solver
+    w = W.srb_humanoid(B=4, N=9, dtype=dtype)
+    rng = np.random.default_rng(2)
+    w.xbar0 = w.xbar0 + np.concatenate([0.05 * rng.standard_normal((w.B, w.T, 3)), 0.3 * rng.standard_normal((w.B, w.T, 3)),
+                                        0.5 * rng.standard_normal((w.B, w.T, 6)), 30.0 * rng.standard_normal((w.B, w.T, 6))], axis=2)
+    wr = w.rounded(np.float32) if dtype == "f32" else w
+    s = Solver(wr, dtype=dtype)
+    s.reset_state(wr.xbar0)
+    s.linearize()
+    cfg = O.make_cfg(wr)
+    tol = 1e-12 if dtype == "f64" else 3e-5
+    for b in range(w.B):
+        ref = O.srb_linearize(wr, cfg, wr.xbar0[b])
+        for name, r in zip(("Am", "Ap", "b"), ref):
+            g = s.t[name][b].cpu().double().numpy()
+            assert np.abs(g - r).max() <= tol * max(1.0, np.abs(r).max()), (name, np.abs(g - r).max())
+    s.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_srb_sqp_matches_oracle(dtype):
+    """The humanoid balancing OCP (eq. 70; N = 20, nx = 12, nu = 6, box bounds on the foot forces): n_sqp x (tmpc_linearize + tmpc_factor +
+    tmpc_admm_solve) against the oracle's driver."""
+    from paper_2606_24039_b200.solver import Solver
+    w = W.srb_humanoid(B=5, dtype=dtype)
+    wr = w.rounded(np.float32) if dtype == "f32" else w
+    s = Solver(wr, dtype=dtype)
+    s.reset_state(wr.xbar0)
+    s.sqp()
+    got = s.state_numpy()
+    ref, info, rc = O.sqp_srb(wr, O.make_cfg(wr))
+    assert rc == 0
+    compare_states(got, ref, TOL[dtype])
+    assert (np.abs(ref["yg"]) > 1e-3).any(), "force bounds should be active on the perturbed starts"
+    s.close()

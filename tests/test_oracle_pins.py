@@ -785,7 +785,7 @@ def test_srb_sqp_driver_reaches_the_reference():
     import copy
     w = W.srb_humanoid(B=2, N=10)
     cfg = O.make_cfg(w)
-    st, info, rc = O.sqp_srb(w, cfg, n_sqp=5, iters=150)
+    st, info, rc = O.sqp_srb(w, cfg, n_sqp=6, iters=600)
     assert rc == 0
     for b in range(w.B):
         x = st["x"][b]
