@@ -142,7 +142,8 @@ typedef struct {
  * iteration (as by tmpc_linearize).  Outputs (DEVICE, any may be NULL): SQP iterations per problem [B], eq. 18 met [B], the accepted alpha
  * of every iteration [B][max_sqp] and the eq. 18 quantities of the last test [B][3] (working dtype).  Like tmpc_admm_solve_adaptive the
  * call SYNCHRONISES once per iteration (count of live problems) and leaves the workspace factor unusable for a later tmpc_admm_solve.
- * TMPC_E_UNSUPPORTED without a built-in model or with cyclic reduction. */
+ * TMPC_E_UNSUPPORTED for any model but TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT (the merit and eq. 18 kernels are written for it) and with cyclic
+ * reduction. */
 tmpc_status tmpc_sqp_solve(tmpc_handle h, tmpc_qp* qp, tmpc_state* st, const void* stage_ref, const tmpc_sqp_opts* o, int32_t* iters_out,
                            int32_t* converged_out, void* alpha_log, void* kkt_out);
 /* a10 (Alg. 2, eq. 59-65): dL/dq [B][T][n] and dL/dx_init [B][nx] from dL/dx [B][T][n] (and dL/dxi [B][T][ng] or NULL)
@@ -150,7 +151,8 @@ tmpc_status tmpc_sqp_solve(tmpc_handle h, tmpc_qp* qp, tmpc_state* st, const voi
  * (lo <= Gx + xi <= hi; App. E's xi_A of eq. 54 is |xi| = sign(xi) xi, so eq. 65's S dL/dxi_A is dL/dxi); only its
  * entries on soft-active rows (xi != 0) are read.  REFACTOR_REFINE factors the adjoint-weighted S and runs `iters` refinement sweeps of the
  * active-set KKT system; ADMM_REUSE_FACTOR runs `iters` ADMM iterations on the adjoint QP (eq. 67) with the
- * forward factor.  Overwrites the factor in the workspace in REFACTOR_REFINE mode. */
+ * forward factor.  Overwrites the factor in the workspace in REFACTOR_REFINE mode.  TMPC_E_UNSUPPORTED for handles that use cyclic reduction
+ * (TMPC_LIN_CYCLIC_REDUCTION, or AUTO where it picked it). */
 tmpc_status tmpc_backward(tmpc_handle h, const tmpc_qp* qp, const tmpc_state* st, const void* dL_dx, const void* dL_dxi,
                           int32_t mode, int32_t iters, void* dL_dq, void* dL_dxinit);
 /* eq. 66: dL/dgamma_xi [B] (working dtype, DEVICE) = sum over the soft-active rows of xi_i (G eta_x)_i, from the
