@@ -33,17 +33,21 @@ namespace tmpc {
 //   E0  y_t [n]      E1A  eta~_t (own part) -> w_t [n]      E1B  eta~_t (part of the block before) [n]
 //   LAM -B_t [n][n]  SINV X_t = L_t^{-1} [n][n]
 //   G   G~_t = G_t X_t' [ng][n]      (dense G only; s_t = rho_g z_g - y_g lives in the registers of the row owners)
-template <typename T, int NC, int NX>
+// XG ("X and A~ in global memory", long horizons): the record keeps only what the CHAIN warp reads — y, eta~ / w and -B_t — and the item
+// lanes take X_t, A~^-_t, A~^+_t from global memory (X from the factor in the workspace, A~ from the scratch atil_kernel fills), where
+// they are L2 hits: the chain is the latency-bound part, the item phases are throughput-bound and tolerate the longer loads.
+template <typename T, int NC, int NX, bool XG = false>
 struct Rec3 {
   static constexpr int V = 16 / (int)sizeof(T);
   static constexpr int up(int v) { return (v + V - 1) / V * V; }
-  static constexpr int AM = 0, AP = AM + up(NX * NC), E0 = AP + up(NX * NC), E1A = E0 + up(NC), E1B = E1A + up(NC),
-                       LAM = E1B + up(NC), SINV = LAM + up(NC * NC), G = SINV + up(NC * NC);
+  static constexpr int AM = 0, AP = AM + (XG ? 0 : up(NX * NC)), E0 = AP + (XG ? 0 : up(NX * NC)), E1A = E0 + up(NC), E1B = E1A + up(NC),
+                       LAM = E1B + up(NC), SINV = LAM + up(NC * NC), G = SINV + (XG ? 0 : up(NC * NC));
   // record stride: 32 bytes (mod 128 bytes) for the 16-byte accesses of n = 8 (a quarter warp = four stages x two halves covers
   // the eight bank groups); 24 bytes (mod 128) for the 6-wide rows of n = 6, whose 8-byte pairs and single elements cannot all
   // be conflict free: this residue makes the single-element loads conflict free and the pair loads 2-way (simulated over all
   // residues; 32 bytes gives 4-way and 8-way)
   static constexpr int pad_stride(int r) {
+    if (XG) return r;                                      // the item lanes touch only the three vectors of a record: no residue to protect
     constexpr bool SIX32 = NC == 6 && sizeof(T) == 4;      // (double keeps 32 bytes: its pairs are 16-byte loads)
     constexpr int W128 = 128 / (int)sizeof(T), WR = (SIX32 ? 24 : 32) / (int)sizeof(T), STEP = SIX32 ? 2 : V;
     while (r % W128 != WR) r += STEP;
@@ -56,11 +60,11 @@ struct Rec3 {
 // 8-bank windows at every step, for any record stride (n = 6 and n = 8 alike).
 struct Admm3Plan { int R, down0, per_problem; };
 
-template <typename T, int NC, int NX>
+template <typename T, int NC, int NX, bool XG = false>
 inline Admm3Plan admm3_plan(const Dims& d, int pg) {
-  using RC = Rec3<T, NC, NX>;
+  using RC = Rec3<T, NC, NX, XG>;
   Admm3Plan P;
-  int R = d.g_sel ? RC::G : RC::G + ((d.ng * NC + RC::V - 1) / RC::V) * RC::V;
+  int R = (d.g_sel || XG) ? RC::G : RC::G + ((d.ng * NC + RC::V - 1) / RC::V) * RC::V;
   P.R = RC::pad_stride(R);
   const int w128 = 128 / (int)sizeof(T), w64 = 64 / (int)sizeof(T), w32 = 32 / (int)sizeof(T), m = d.T / 2;
   int d0 = ((m + 1) * P.R + RC::V - 1) / RC::V * RC::V;
@@ -71,13 +75,14 @@ inline Admm3Plan admm3_plan(const Dims& d, int pg) {
   P.per_problem = pp;
   return P;
 }
-template <typename T, int NC, int NX>
-inline size_t admm3_smem_bytes(const Dims& d, int pg) { return (size_t)admm3_plan<T, NC, NX>(d, pg).per_problem * pg * sizeof(T); }
+template <typename T, int NC, int NX, bool XG = false>
+inline size_t admm3_smem_bytes(const Dims& d, int pg) { return (size_t)admm3_plan<T, NC, NX, XG>(d, pg).per_problem * pg * sizeof(T); }
 
 template <typename T>
 struct Admm3Args {
   AdmmArgs<T> a;
   Admm3Plan pl;
+  const T* atil;                      // XG only: A~ per stage, [B][T][2][nx][n] (atil_kernel)
   T rfa, oma, inv_rho_g, inv_rg;      // rho_f alpha, 1 - alpha, 1 / rho_g, 1 / (rho_g + gamma)
 };
 
@@ -153,11 +158,11 @@ template <typename T, int H> __device__ __forceinline__ T dot2(const T (&a)[H], 
 // read the vector back as a broadcast vector load, one row (inward sweep) or column (outward sweep) of -B_t, one dot.
 // Row i >= n/2 takes its 16-byte chunks in the opposite order (`swb`; the data is not swizzled) so that the eight rows of a
 // slot cover the eight bank groups; the broadcast operand vector is read in the same order.
-template <typename T, int NC, int NX, int PG>
+template <typename T, int NC, int NX, int PG, bool XG = false>
 __device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, int T_, int lane, unsigned pmask) {   // pmask: bit g = problem g of the CTA is live
   constexpr int SL = NC <= 8 ? 8 : 16;                   // lanes per slot (one per row)
   static_assert(NC <= 16 && PG * 2 * SL <= 32, "the chain warp holds (problems x 2 directions) slots of SL lanes");
-  using RC = Rec3<T, NC, NX>;
+  using RC = Rec3<T, NC, NX, XG>;
   constexpr int n = NC;
   constexpr unsigned ES = sizeof(T);
   const unsigned sb = (unsigned)__cvta_generic_to_shared(sm);
@@ -257,11 +262,11 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, in
 // order above), the dynamics rows [h KA, ...) of ITS stage's block (block t for t < N; the rows x_0 = x_init for t = N, whose
 // A^+ = [I 0] sits in record 0), and the inequality rows: for a selection G the rows whose column it owns, for a dense G the
 // rows 2 s + h.
-template <typename T, int NC, int NX, int PG, int MAXT, int MINB>
+template <typename T, int NC, int NX, int PG, int MAXT, int MINB, bool XG = false>
 __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant__ Admm3Args<T> A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* sm = reinterpret_cast<T*>(smem_raw);
-  using RC = Rec3<T, NC, NX>;
+  using RC = Rec3<T, NC, NX, XG>;
   static_assert(NC % 2 == 0, "two lanes per stage own half a row each");
   const AdmmArgs<T>& a = A.a;
   const Dims& d = a.d;
@@ -287,9 +292,9 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
       const int t = e / nn, rc = e - t * nn;
       const int o = rec(t) + rc;
       if (t != m) P[o + RC::LAM] = -gLam[e];
-      P[o + RC::SINV] = gX[e];
+      if constexpr (!XG) P[o + RC::SINV] = gX[e];
     }
-    if (!a.kkt_only) {
+    if (!XG && !a.kkt_only) {
       const T* gAm = a.qp.Am + (size_t)p * N * nx * n; const T* gAp = a.qp.Ap + (size_t)p * N * nx * n;
       for (int e = tid; e < T_ * nx * n; e += nt) {
         const int t = e / (nx * n), rc = e - t * nx * n, k = rc / n, j = rc - k * n;
@@ -305,7 +310,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   __syncthreads();
   // ---- stage 2: the constraint blocks in the scaled variables, row by row in place: M~[k][j] = sum_{l <= j} M[k][l] X_t[j][l]
   // (A~^-_t = A^-_t X_t', A~^+_{t-1} = A^+_{t-1} X_t', G~_t = G_t X_t'); a thread owns a whole row, so there is no hazard
-  if (!a.kkt_only) {
+  if (!XG && !a.kkt_only) {
     const int rows_t = 2 * nx + (d.g_sel ? 0 : ng);       // rows per stage: AM, AP, G
     for (int e = tid; e < PG * T_ * rows_t; e += nt) {
       const int g = e / (T_ * rows_t), r2 = e - g * T_ * rows_t, t = r2 / rows_t, k = r2 - t * rows_t;
@@ -341,7 +346,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
 #ifdef TMPC_TIMING
       __syncwarp(); const T probe = sm[tid & 7]; const long long c1 = clock64() + (probe == T(12345.678) ? 1 : 0);   // the load makes the deferred barrier block first
 #endif
-      chain3_solve<T, NC, NX, PG>(sm, R, A.pl.down0, PP, T_, tid, pmask);
+      chain3_solve<T, NC, NX, PG, XG>(sm, R, A.pl.down0, PP, T_, tid, pmask);
       __syncwarp();
 #ifdef TMPC_TIMING
       tch += clock64() - c1;
@@ -360,7 +365,11 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   const bool valid = g < PG && p < d.B && (!a.active || a.active[p]);      // a terminated problem (f1) is left untouched
   const HalfOff mine = half_off<NC>(h), other = half_off<NC>(1 - h);
   const int b = valid ? g * PP + rec(t) : 0, bn = valid ? g * PP + (t < N ? rec(t + 1) : rec(0)) : 0;
-  const T* Xb = sm + b + RC::SINV;
+  // the blocks the item lanes read: X_t, A~^-_t (my record) and A~^+_t (the next record) — shared memory, or global memory for XG
+  const size_t gst = valid ? (size_t)p * T_ + t : 0, gsn = valid ? (size_t)p * T_ + (t < N ? t + 1 : 0) : 0;
+  const T* Xb = XG ? a.Sinv + gst * nn : sm + b + RC::SINV;
+  const T* AMb = XG ? A.atil + gst * (2 * nx * n) : sm + b + RC::AM;
+  const T* APn = XG ? A.atil + gsn * (2 * nx * n) + nx * n : sm + bn + RC::AP;
 
   if (a.kkt_only) {                                      // xt <- S^{-1} eta : eta~ = X eta, solve, x = X' y
     T eo[H], er[H];
@@ -487,12 +496,12 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
       for (int s = 0; s < KA; ++s) {                   // my columns of A~^-_t (my record) and A~^+_t (next record), rows of my block half / the partner's
         T mk[H];
         if (s < nk) {
-          ld_half<NC>(sm + b + RC::AM + (k0 + s) * n, mine, mk); axpy_half<H>(acc, mk, ro[s]);
-          ld_half<NC>(sm + bn + RC::AP + (k0 + s) * n, mine, mk); axpy_half<H>(accb, mk, ro[s]);
+          ld_half<NC>(AMb + (k0 + s) * n, mine, mk); axpy_half<H>(acc, mk, ro[s]);
+          ld_half<NC>(APn + (k0 + s) * n, mine, mk); axpy_half<H>(accb, mk, ro[s]);
         }
         if (s < nkp) {
-          ld_half<NC>(sm + b + RC::AM + (k0p + s) * n, mine, mk); axpy_half<H>(acc, mk, rr[s]);
-          ld_half<NC>(sm + bn + RC::AP + (k0p + s) * n, mine, mk); axpy_half<H>(accb, mk, rr[s]);
+          ld_half<NC>(AMb + (k0p + s) * n, mine, mk); axpy_half<H>(acc, mk, rr[s]);
+          ld_half<NC>(APn + (k0p + s) * n, mine, mk); axpy_half<H>(accb, mk, rr[s]);
         }
       }
       if (!d.g_sel) {
@@ -532,9 +541,9 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
         for (int s = 0; s < KA; ++s) if (s < nk) {
           const int k = k0 + s;
           T f[H], f2[H];
-          ld_half<NC>(sm + b + RC::AM + k * n, mine, f); ld_half<NC>(sm + b + RC::AM + k * n, other, f2);
+          ld_half<NC>(AMb + k * n, mine, f); ld_half<NC>(AMb + k * n, other, f2);
           T zt = dot2<T, H>(f, yo, f2, yr);
-          ld_half<NC>(sm + bn + RC::AP + k * n, mine, f); ld_half<NC>(sm + bn + RC::AP + k * n, other, f2);
+          ld_half<NC>(APn + k * n, mine, f); ld_half<NC>(APn + k * n, other, f2);
           zt += dot2<T, H>(f, y2o, f2, y2r);
           yf[s] += rfa * (zt - cv[s]);
         }
@@ -571,6 +580,37 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
       const size_t row = (size_t)p * mg + t * ng + (qf[s] >> Q_ROW_SH);
       a.zg[row] = zg[s]; a.yg[row] = yg[s]; if (a.iters > 0) a.xi[row] = xi_last[s];
     }
+  }
+}
+
+// ---- XG: the constraint blocks in the scaled variables, once per launch of the solve: row k of stage t of
+//   atil[p][t][0] = A~^-_t = A^-_t X_t'  (zero for t = N)      atil[p][t][1] = A~^+_{t-1} = A^+_{t-1} X_t'  (A_init = [I 0] for t = 0),
+// M~[k][j] = sum_{l <= j} M[k][l] X_t[j][l] (X_t lower triangular).  One thread per row; n <= 16.
+template <typename T>
+__global__ void __launch_bounds__(128) atil_kernel(const AdmmArgs<T> a, T* __restrict__ atil) {
+  const Dims& d = a.d;
+  const int n = d.n, nx = d.nx, T_ = d.T, N = d.N, rows = 2 * nx;
+  const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= (long long)d.B * T_ * rows) return;
+  const int k2 = (int)(e % rows), t = (int)((e / rows) % T_), p = (int)(e / ((long long)rows * T_));
+  const bool plus = k2 >= nx; const int k = plus ? k2 - nx : k2;
+  T v[16];
+#pragma unroll
+  for (int l = 0; l < 16; ++l) {
+    T s = T(0);
+    if (l < n) {
+      if (!plus) { if (t < N) s = a.qp.Am[(((size_t)p * N + t) * nx + k) * n + l]; }
+      else s = t > 0 ? a.qp.Ap[(((size_t)p * N + t - 1) * nx + k) * n + l] : (l == k ? T(1) : T(0));
+    }
+    v[l] = s;
+  }
+  const T* X = a.Sinv + ((size_t)p * T_ + t) * n * n;
+  T* out = atil + (size_t)e * n;
+  for (int j = 0; j < n; ++j) {
+    T acc = T(0);
+#pragma unroll
+    for (int l = 0; l < 16; ++l) if (l <= j) acc += v[l] * X[j * n + l];
+    out[j] = acc;
   }
 }
 

@@ -28,7 +28,7 @@ inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 inline size_t esize(int dtype) { return dtype == TMPC_F64 ? 8 : 4; }
 
 struct Layout {   // byte offsets into the workspace
-  size_t Lam, Sinv, eta, fstatus, ad_rho, ad_np, ad_nd, ad_rp, ad_rd, ad_obj, ad_active, ad_mask, ad_iters, ad_conv, ad_count, cls, soft_adj, rhs, w_rows, lo_adj, hi_adj, q_adj, ax, azg, ayf, ayg, axi, zero_xinit, zero_b, res, cr, total;
+  size_t Lam, Sinv, atil, eta, fstatus, ad_rho, ad_np, ad_nd, ad_rp, ad_rd, ad_obj, ad_active, ad_mask, ad_iters, ad_conv, ad_count, cls, soft_adj, rhs, w_rows, lo_adj, hi_adj, q_adj, ax, azg, ayf, ayg, axi, zero_xinit, zero_b, res, cr, total;
 };
 
 // Cyclic reduction (tmpc_cr.cuh) exists for n = 6 and n = 8 and pays off for a few very long horizons; TMPC_LIN_AUTO picks it
@@ -48,11 +48,14 @@ Dims make_dims(const tmpc_config& c) {
   return d;
 }
 
+bool plan_xg(const tmpc_config& c);      // the resident kernel keeps X and A~ in global memory (long horizons of n = 12): defined beside fast_plan()
+
 Layout make_layout(const tmpc_config& c) {
   const Dims d = make_dims(c); const size_t es = esize(c.dtype), B = d.B, nn = (size_t)d.n * d.n;
   Layout L; size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
   L.Lam = take(B * d.T * nn * es); L.Sinv = take(B * d.T * nn * es); L.eta = take(B * d.nz * es);
+  L.atil = take(plan_xg(c) ? B * d.T * 2 * (size_t)d.nx * d.n * es : 0);       // A~ per stage (atil_kernel), only for the handles whose plan reads it
   L.fstatus = take(B * sizeof(int32_t));       // per-problem TMPC_ST_PIVOT word of the last tmpc_factor
   // f1 (tmpc_admm_solve_adaptive): per-problem rho_bar, eq. 4 scales, residuals / objective when the caller passes no info, flags, counters
   L.ad_rho = take(B * es); L.ad_np = take(B * es); L.ad_nd = take(B * es); L.ad_rp = take(B * es); L.ad_rd = take(B * es); L.ad_obj = take(B * es);
@@ -145,7 +148,7 @@ tmpc_status launch_admm_inst(tmpc_ctx* h, const AdmmArgs<T>& a, int nt, size_t s
   k<<<h->d.B, nt, smem, h->stream>>>(a); h->launches++;
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
 }
-struct FastPlan { bool ok; int pg, nt, ctas_per_sm; size_t smem; };
+struct FastPlan { bool ok, xg; int pg, nt, ctas_per_sm; size_t smem; };
 template <typename T> FastPlan fast_plan(const Dims& d);
 template <typename T> tmpc_status launch_resident(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f);
 template <typename T> tmpc_status launch_residual(tmpc_ctx* h, const AdmmArgs<T>& s);
@@ -217,13 +220,21 @@ tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
 constexpr size_t kSmemPerSM = 228 * 1024;
 template <typename T>
 FastPlan fast_plan(const Dims& d) {
-  FastPlan f; f.ok = false; f.pg = 1; f.nt = 0; f.ctas_per_sm = 0; f.smem = 0;
+  FastPlan f; f.ok = false; f.xg = false; f.pg = 1; f.nt = 0; f.ctas_per_sm = 0; f.smem = 0;
   const bool shape = (d.n == 8 && d.nx == 6) || (d.n == 6 && d.nx == 4) || (d.n == 12 && d.nx == 8);   // (12, 8): the nominal block size of the paper's scaling study (f4)
   if (!shape || d.ng > d.n || d.T < 2) return f;
   if (d.g_sel) for (int r = 0; r < d.ng; ++r) for (int q = 0; q < r; ++q) if (d.g_col[r] == d.g_col[q]) return f;   // one selection row per column
   const size_t s1 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 1) : d.n == 6 ? admm3_smem_bytes<T, 6, 4>(d, 1) : admm3_smem_bytes<T, 12, 8>(d, 1);
   const size_t s2 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 2) : d.n == 6 ? admm3_smem_bytes<T, 6, 4>(d, 2) : kMaxSmem + 1;   // n = 12: one problem per CTA (16 chain lanes per slot)
-  if (s1 > kMaxSmem) return f;
+  if (s1 > kMaxSmem) {
+    // long horizons of the (12, 8) block: only the chain's share of a record stays in shared memory (Rec3<.., XG>), one problem per SM
+    if (d.n != 12 || !(d.g_sel || d.ng == 0)) return f;
+    const size_t sx = admm3_smem_bytes<T, 12, 8, true>(d, 1);
+    const int ntx = 32 + (2 * d.T + 31) / 32 * 32;
+    if (sx > kMaxSmem || ntx > 704) return f;
+    f.ok = true; f.xg = true; f.pg = 1; f.nt = ntx; f.ctas_per_sm = 1; f.smem = sx;
+    return f;
+  }
   const int c1 = (int)(kSmemPerSM / (s1 + 1024)), c2 = s2 <= kMaxSmem ? (int)(kSmemPerSM / (s2 + 1024)) : 0;
   f.pg = (d.B >= 2 && c2 >= 2 && 2 * c2 >= c1) ? 2 : 1;
   const int ipt = d.n / 2;                                 // rows of a stage per item thread (admm3: two lanes per stage)
@@ -236,12 +247,24 @@ FastPlan fast_plan(const Dims& d) {
   return f;
 }
 
-template <typename T, int NC, int NX, int PG, int MAXT, int MINB>
+bool plan_xg(const tmpc_config& c) {
+  const Dims d = make_dims(c);
+  return c.dtype == TMPC_F64 ? fast_plan<double>(d).xg : fast_plan<float>(d).xg;
+}
+
+template <typename T, int NC, int NX, int PG, int MAXT, int MINB, bool XG = false>
 tmpc_status launch_admm3_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
-  auto k = admm3_kernel<T, NC, NX, PG, MAXT, MINB>;
+  auto k = admm3_kernel<T, NC, NX, PG, MAXT, MINB, XG>;
   if (f.smem > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem) != cudaSuccess) return TMPC_E_CUDA;
   const unsigned grid = (unsigned)((h->d.B + PG - 1) / PG);
-  Admm3Args<T> A; A.a = a; A.pl = admm3_plan<T, NC, NX>(h->d, PG);
+  Admm3Args<T> A; A.a = a; A.pl = admm3_plan<T, NC, NX, XG>(h->d, PG); A.atil = nullptr;
+  if constexpr (XG) {
+    T* atil = (T*)(h->ws + h->lay.atil); A.atil = atil;
+    if (!a.kkt_only) {
+      const long long rows = (long long)h->d.B * h->d.T * 2 * h->d.nx;
+      atil_kernel<T><<<(unsigned)((rows + 127) / 128), 128, 0, h->stream>>>(a, atil); h->launches++;
+    }
+  }
   A.rfa = a.prm.rho_f * a.prm.alpha; A.oma = T(1) - a.prm.alpha; A.inv_rho_g = T(1) / a.prm.rho_g; A.inv_rg = T(1) / (a.prm.rho_g + a.prm.gamma);
   k<<<grid, f.nt, f.smem, h->stream>>>(A); h->launches++;
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
@@ -265,6 +288,7 @@ tmpc_status launch_resident(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f
   const Dims& d = h->d;
   if (d.n == 8) return f.pg == 2 ? launch_admm3_shape<T, 8, 6, 2>(h, a, f) : launch_admm3_shape<T, 8, 6, 1>(h, a, f);
   if (d.n == 6) return f.pg == 2 ? launch_admm3_shape<T, 6, 4, 2>(h, a, f) : launch_admm3_shape<T, 6, 4, 1>(h, a, f);
+  if (d.n == 12 && f.xg) return f.nt <= 384 ? launch_admm3_inst<T, 12, 8, 1, 384, 1, true>(h, a, f) : launch_admm3_inst<T, 12, 8, 1, 704, 1, true>(h, a, f);
   if (d.n == 12) return launch_admm3_shape<T, 12, 8, 1>(h, a, f);
   return TMPC_E_UNSUPPORTED;
 }

@@ -630,6 +630,33 @@ def test_f4_linear_rl_sweep_shapes_fp32():
     run_pair(W.linear_rl(B=2, N=8, nx=32, nu=16, u_max=1.0), "f32", iters=60, band=1)
 
 
+def test_f4_linear_rl_long_horizons_chain_resident():
+    """The horizon sweep's long end at the nominal block (N = 160 and 320 at (nx, nu) = (8, 4)): the records no longer fit in
+    shared memory, admm3_kernel keeps only the chain's share there and reads X_t, A~_t from global memory (Rec3<.., XG>).  Fixed-count iterates
+    in both dtypes, the adaptive run and the backward pass against the oracle; N = 161 is the odd-length, ragged-warp case."""
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    w = W.linear_rl(B=3, N=160, u_max=1.0)
+    run_pair(w, "f64", iters=60)
+    run_pair(w, "f32", iters=60)
+    run_pair(W.linear_rl(B=2, N=161, u_max=10.0), "f64", iters=40)
+    run_pair(W.linear_rl(B=2, N=320, u_max=1.0), "f32", iters=40)
+    ref, rinfo, log, rc = O.admm_adaptive(w, O.make_cfg(w), O.make_adaptive(300, 1e-4, 1e-4))
+    s = Solver(w, dtype="f64")
+    out = s.solve_adaptive(300, 1e-4, 1e-4)
+    assert (out["iters"] == rinfo[:, 4].astype(int)).all() and (out["converged"] == rinfo[:, 6].astype(int)).all()
+    compare_states(s.state_numpy(), ref, 1e-7)
+    cfg = O.make_cfg(w)
+    ref, info, rc = O.admm(w, O.make_cfg(w, rho_bar=5.0), iters=3000)
+    dq_o, dxi_o, counts, rcs = O.backward(w, cfg, ref, 2.0 * ref["x"])
+    ok = rcs == 0
+    assert ok.sum() >= 2
+    s.set_state(ref)
+    dq, dxi = s.backward(s._up(2.0 * ref["x"]), mode=Bd.TMPC_BWD_REFACTOR_REFINE)
+    assert rel_err(dq.cpu().double().numpy()[ok], dq_o[ok]) <= 1e-9 and rel_err(dxi.cpu().double().numpy()[ok], dxi_o[ok]) <= 1e-9
+    s.close()
+
+
 # ----------------------------------------------------------------------------------------------- f2: SQP with linesearch + eq. 18
 def test_sqp_linesearch_matches_oracle_fp64():
     """Alg. 1 with the App. D linesearch and the eq. 18 stop on perturbed bicycle starts: accepted
