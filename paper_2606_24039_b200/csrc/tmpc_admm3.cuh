@@ -82,7 +82,7 @@ template <typename T>
 struct Admm3Args {
   AdmmArgs<T> a;
   Admm3Plan pl;
-  const T* atil;                      // XG only: A~ per stage, [B][T][2][nx][n] (atil_kernel)
+  const T* atil;                      // XG only: A~^-, A~^+ and (dense G) G~ per stage, [B][T][2 nx + ng][n] (atil_kernel)
   T rfa, oma, inv_rho_g, inv_rg;      // rho_f alpha, 1 - alpha, 1 / rho_g, 1 / (rho_g + gamma)
 };
 
@@ -368,8 +368,10 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   // the blocks the item lanes read: X_t, A~^-_t (my record) and A~^+_t (the next record) — shared memory, or global memory for XG
   const size_t gst = valid ? (size_t)p * T_ + t : 0, gsn = valid ? (size_t)p * T_ + (t < N ? t + 1 : 0) : 0;
   const T* Xb = XG ? a.Sinv + gst * nn : sm + b + RC::SINV;
-  const T* AMb = XG ? A.atil + gst * (2 * nx * n) : sm + b + RC::AM;
-  const T* APn = XG ? A.atil + gsn * (2 * nx * n) + nx * n : sm + bn + RC::AP;
+  const int arows = 2 * nx + (d.g_sel ? 0 : ng);        // rows of a stage in atil: A~^-, A~^+, G~ (dense G only)
+  const T* AMb = XG ? A.atil + gst * (arows * n) : sm + b + RC::AM;
+  const T* APn = XG ? A.atil + gsn * (arows * n) + nx * n : sm + bn + RC::AP;
+  const T* Gb = XG ? A.atil + gst * (arows * n) + 2 * nx * n : sm + b + RC::G;
 
   if (a.kkt_only) {                                      // xt <- S^{-1} eta : eta~ = X eta, solve, x = X' y
     T eo[H], er[H];
@@ -508,8 +510,8 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
 #pragma unroll
         for (int s = 0; s < H; ++s) {
           T mk[H];
-          if (2 * s + h < ng) { ld_half<NC>(sm + b + RC::G + (2 * s + h) * n, mine, mk); axpy_half<H>(acc, mk, sg[s]); }
-          if (2 * s + 1 - h < ng) { ld_half<NC>(sm + b + RC::G + (2 * s + 1 - h) * n, mine, mk); axpy_half<H>(acc, mk, sgr[s]); }
+          if (2 * s + h < ng) { ld_half<NC>(Gb + (2 * s + h) * n, mine, mk); axpy_half<H>(acc, mk, sg[s]); }
+          if (2 * s + 1 - h < ng) { ld_half<NC>(Gb + (2 * s + 1 - h) * n, mine, mk); axpy_half<H>(acc, mk, sgr[s]); }
         }
       }
       st_half<NC>(sm + b + RC::E1A, mine, acc);
@@ -552,7 +554,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
       for (int s = 0; s < H; ++s) {
         if (qf[s] & Q_VALID) {
           T ztg = xt[s];
-          if (!d.g_sel) { const T* row = sm + b + RC::G + (int)(qf[s] >> Q_ROW_SH) * n; T f[H], f2[H]; ld_half<NC>(row, mine, f); ld_half<NC>(row, other, f2); ztg = dot2<T, H>(f, yo, f2, yr); }
+          if (!d.g_sel) { const T* row = Gb + (int)(qf[s] >> Q_ROW_SH) * n; T f[H], f2[H]; ld_half<NC>(row, mine, f); ld_half<NC>(row, other, f2); ztg = dot2<T, H>(f, yo, f2, yr); }
           const T zh = a.prm.alpha * ztg + A.oma * zg[s];
           const T v = zh + yg[s] * inv_rho_g;
           T z, sl;
@@ -584,22 +586,24 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
 }
 
 // ---- XG: the constraint blocks in the scaled variables, once per launch of the solve: row k of stage t of
-//   atil[p][t][0] = A~^-_t = A^-_t X_t'  (zero for t = N)      atil[p][t][1] = A~^+_{t-1} = A^+_{t-1} X_t'  (A_init = [I 0] for t = 0),
+//   rows [0, nx): A~^-_t = A^-_t X_t' (zero for t = N);  rows [nx, 2 nx): A~^+_{t-1} = A^+_{t-1} X_t' (A_init = [I 0] for t = 0);
+//   rows [2 nx, 2 nx + ng): G~_t = G_t X_t' (dense G only),
 // M~[k][j] = sum_{l <= j} M[k][l] X_t[j][l] (X_t lower triangular).  One thread per row; n <= 16.
 template <typename T>
 __global__ void __launch_bounds__(128) atil_kernel(const AdmmArgs<T> a, T* __restrict__ atil) {
   const Dims& d = a.d;
-  const int n = d.n, nx = d.nx, T_ = d.T, N = d.N, rows = 2 * nx;
+  const int n = d.n, nx = d.nx, T_ = d.T, N = d.N, rows = 2 * nx + (d.g_sel ? 0 : d.ng);
   const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= (long long)d.B * T_ * rows) return;
   const int k2 = (int)(e % rows), t = (int)((e / rows) % T_), p = (int)(e / ((long long)rows * T_));
-  const bool plus = k2 >= nx; const int k = plus ? k2 - nx : k2;
+  const bool plus = k2 >= nx && k2 < 2 * nx, isg = k2 >= 2 * nx; const int k = isg ? k2 - 2 * nx : (plus ? k2 - nx : k2);
   T v[16];
 #pragma unroll
   for (int l = 0; l < 16; ++l) {
     T s = T(0);
     if (l < n) {
-      if (!plus) { if (t < N) s = a.qp.Am[(((size_t)p * N + t) * nx + k) * n + l]; }
+      if (isg) s = a.qp.G[a.qp.sG * p + ((size_t)t * d.ng + k) * n + l];
+      else if (!plus) { if (t < N) s = a.qp.Am[(((size_t)p * N + t) * nx + k) * n + l]; }
       else s = t > 0 ? a.qp.Ap[(((size_t)p * N + t - 1) * nx + k) * n + l] : (l == k ? T(1) : T(0));
     }
     v[l] = s;

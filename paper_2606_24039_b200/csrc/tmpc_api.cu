@@ -55,7 +55,7 @@ Layout make_layout(const tmpc_config& c) {
   Layout L; size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
   L.Lam = take(B * d.T * nn * es); L.Sinv = take(B * d.T * nn * es); L.eta = take(B * d.nz * es);
-  L.atil = take(plan_xg(c) ? B * d.T * 2 * (size_t)d.nx * d.n * es : 0);       // A~ per stage (atil_kernel), only for the handles whose plan reads it
+  L.atil = take(plan_xg(c) ? B * d.T * (2 * (size_t)d.nx + (d.g_sel ? 0 : d.ng)) * d.n * es : 0);       // A~ per stage (atil_kernel), only for the handles whose plan reads it
   L.fstatus = take(B * sizeof(int32_t));       // per-problem TMPC_ST_PIVOT word of the last tmpc_factor
   // f1 (tmpc_admm_solve_adaptive): per-problem rho_bar, eq. 4 scales, residuals / objective when the caller passes no info, flags, counters
   L.ad_rho = take(B * es); L.ad_np = take(B * es); L.ad_nd = take(B * es); L.ad_rp = take(B * es); L.ad_rd = take(B * es); L.ad_obj = take(B * es);
@@ -227,12 +227,11 @@ FastPlan fast_plan(const Dims& d) {
   const size_t s1 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 1) : d.n == 6 ? admm3_smem_bytes<T, 6, 4>(d, 1) : admm3_smem_bytes<T, 12, 8>(d, 1);
   const size_t s2 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 2) : d.n == 6 ? admm3_smem_bytes<T, 6, 4>(d, 2) : kMaxSmem + 1;   // n = 12: one problem per CTA (16 chain lanes per slot)
   if (s1 > kMaxSmem) {
-    // long horizons of the (12, 8) block: only the chain's share of a record stays in shared memory (Rec3<.., XG>), one problem per SM
-    if (d.n != 12 || !(d.g_sel || d.ng == 0)) return f;
-    const size_t sx = admm3_smem_bytes<T, 12, 8, true>(d, 1);
+    // long horizons: only the chain's share of a record stays in shared memory (Rec3<.., XG>), one problem per CTA, two item lanes per stage
+    const size_t sx = d.n == 8 ? admm3_smem_bytes<T, 8, 6, true>(d, 1) : d.n == 6 ? admm3_smem_bytes<T, 6, 4, true>(d, 1) : admm3_smem_bytes<T, 12, 8, true>(d, 1);
     const int ntx = 32 + (2 * d.T + 31) / 32 * 32;
-    if (sx > kMaxSmem || ntx > 704) return f;
-    f.ok = true; f.xg = true; f.pg = 1; f.nt = ntx; f.ctas_per_sm = 1; f.smem = sx;
+    if (sx > kMaxSmem || ntx > 1024) return f;
+    f.ok = true; f.xg = true; f.pg = 1; f.nt = ntx; f.ctas_per_sm = (int)(kSmemPerSM / (sx + 1024)); f.smem = sx;
     return f;
   }
   const int c1 = (int)(kSmemPerSM / (s1 + 1024)), c2 = s2 <= kMaxSmem ? (int)(kSmemPerSM / (s2 + 1024)) : 0;
@@ -261,7 +260,7 @@ tmpc_status launch_admm3_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan&
   if constexpr (XG) {
     T* atil = (T*)(h->ws + h->lay.atil); A.atil = atil;
     if (!a.kkt_only) {
-      const long long rows = (long long)h->d.B * h->d.T * 2 * h->d.nx;
+      const long long rows = (long long)h->d.B * h->d.T * (2 * h->d.nx + (h->d.g_sel ? 0 : h->d.ng));
       atil_kernel<T><<<(unsigned)((rows + 127) / 128), 128, 0, h->stream>>>(a, atil); h->launches++;
     }
   }
@@ -283,12 +282,22 @@ tmpc_status launch_admm3_shape(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan
   }
   return launch_admm3_inst<T, NC, NX, PG, 1024, 1>(h, a, f);
 }
+template <typename T, int NC, int NX>
+tmpc_status launch_admm3_xg(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {      // chain-resident variant: thread caps by horizon
+  if (f.nt <= 384) return launch_admm3_inst<T, NC, NX, 1, 384, 1, true>(h, a, f);
+  if (f.nt <= 704) return launch_admm3_inst<T, NC, NX, 1, 704, 1, true>(h, a, f);
+  return launch_admm3_inst<T, NC, NX, 1, 1024, 1, true>(h, a, f);
+}
 template <typename T>
 tmpc_status launch_resident(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
   const Dims& d = h->d;
+  if (f.xg) {
+    if (d.n == 12) return launch_admm3_xg<T, 12, 8>(h, a, f);
+    if (d.n == 8) return launch_admm3_xg<T, 8, 6>(h, a, f);
+    if (d.n == 6) return launch_admm3_xg<T, 6, 4>(h, a, f);
+  }
   if (d.n == 8) return f.pg == 2 ? launch_admm3_shape<T, 8, 6, 2>(h, a, f) : launch_admm3_shape<T, 8, 6, 1>(h, a, f);
   if (d.n == 6) return f.pg == 2 ? launch_admm3_shape<T, 6, 4, 2>(h, a, f) : launch_admm3_shape<T, 6, 4, 1>(h, a, f);
-  if (d.n == 12 && f.xg) return f.nt <= 384 ? launch_admm3_inst<T, 12, 8, 1, 384, 1, true>(h, a, f) : launch_admm3_inst<T, 12, 8, 1, 704, 1, true>(h, a, f);
   if (d.n == 12) return launch_admm3_shape<T, 12, 8, 1>(h, a, f);
   return TMPC_E_UNSUPPORTED;
 }

@@ -657,6 +657,25 @@ def test_f4_linear_rl_long_horizons_chain_resident():
     s.close()
 
 
+def test_long_horizons_chain_resident_small_blocks():
+    """The same variant for the (8, 6) and (6, 4) blocks once their records outgrow shared memory (fp64: N > ~190 resp. ~330): selection G with
+    soft rows (config 2's data at N = 260), dense G (config 4's bicycle QP at N = 400, G~ rows in global memory too), and the thread-cap
+    variants (384 / 704 / 1024 threads per CTA)."""
+    run_pair(W.config2(B=3, N=260, soft_bound=0.5), "f64", iters=60)
+    run_pair(W.config2(B=2, N=420).rounded(np.float32), "f32", iters=50)
+    run_pair(W.random_ltv(31, 3, 400, 4, 2, [4], [0, 1, 0], dense_g_rows=2, q_scale=0.3), "f64", iters=50)
+    run_pair(W.random_ltv(32, 2, 480, 4, 2, [5], [0, 0, 1], dense_g_rows=2, q_scale=0.3), "f32", iters=50)
+    from paper_2606_24039_b200.solver import Solver
+    w = W.config4(B=2, N=400, dtype="f64")               # SQP on the bicycle model: linearise + factor + solve, all on the long-horizon variant
+    s = Solver(w, dtype="f64")
+    s.reset_state(w.xbar0)
+    s.sqp()
+    ref, info, rc = O.sqp_bicycle(w, O.make_cfg(w), nthreads=8)
+    assert rc == 0
+    compare_states(s.state_numpy(), ref, TOL["f64"])
+    s.close()
+
+
 # ----------------------------------------------------------------------------------------------- f2: SQP with linesearch + eq. 18
 def test_sqp_linesearch_matches_oracle_fp64():
     """Alg. 1 with the App. D linesearch and the eq. 18 stop on perturbed bicycle starts: accepted
