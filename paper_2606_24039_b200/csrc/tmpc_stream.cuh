@@ -68,17 +68,16 @@ struct StreamArgs { AdmmArgs<T> a; int LD, slots, tile_elems; T* eta; int g0, ch
 //                t = N..0   : Lambda_t, A^-_t, A^+_t (t < N; the A blocks skipped for kkt_only)
 template <typename T>
 __global__ void __launch_bounds__(1024) admm_stream_kernel(const __grid_constant__ StreamArgs<T> S) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_ring_raw[];   // own name: the other kernels of this translation unit declare theirs 16-byte aligned
   const AdmmArgs<T>& a = S.a;
   const Dims& d = a.d;
-  constexpr int V = 16 / (int)sizeof(T);
   const int n = d.n, nx = d.nx, ng = d.ng, N = d.N, T_ = d.T, nn = n * n, an = nx * n, nz = d.nz, mf = d.mf, mg = d.mg;
   const int LD = S.LD, KS = S.slots, tid = threadIdx.x;
   const int gjob = S.g0 + (int)blockIdx.x, chunk = gjob / d.B, p = gjob - chunk * d.B;
   const int zg_given = chunk > 0 ? 1 : a.zg_given;                   // later chunks resume from the stored state
   if (a.active && !a.active[p]) return;                              // terminated problem (f1): the whole CTA leaves before any barrier is set up
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_raw);            // full[KS], empty[KS]
-  T* ring = reinterpret_cast<T*>(smem_raw + 256);
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_ring_raw);            // full[KS], empty[KS]
+  T* ring = reinterpret_cast<T*>(smem_ring_raw + 256);
   // Only v / x~ is kept whole in shared memory.  The right-hand side eta lives in global memory (each element is written
   // once and read once per iteration by the SAME thread, prefetched a step ahead), x is updated in place in global
   // memory, and w_t only needs a two-stage window: the small footprint leaves room for a deeper ring / more CTAs.
