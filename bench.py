@@ -422,6 +422,44 @@ def f4_rows(ctx, args):
     return rows
 
 
+def f4_sweep(ctx, args):
+    """The three sweeps of the paper's Fig. 3 around the nominal (B, N, nx, nu) = (64, 40, 8, 4): batch size, horizon and block size,
+    u_max in {1, 10}, tol = 1e-5 with at most 1000 ADMM iterations, fp64; forward = one batched adaptive solve (best of 3), backward = REFINE mode
+    (best of 3).  One seed per point (the paper averages ten)."""
+    import torch
+    from paper_2606_24039_b200 import binding as Bd
+    from paper_2606_24039_b200 import workloads as W
+    from paper_2606_24039_b200.solver import Solver
+    dev = ctx["dev"]
+    pts = [("B", (B, 40, 8, 4)) for B in (1, 8, 16, 32, 64, 128, 256, 512, 1024)]
+    pts += [("N", (64, N, 8, 4)) for N in (10, 20, 80, 160, 320)]
+    pts += [("n", (64, 40, nx, nx // 2)) for nx in (4, 16, 32, 64)]
+    rows = []
+    for axis, (B, N, nx, nu) in pts:
+        for u_max in (1.0, 10.0):
+            row = {"sweep": axis, "B": B, "N": N, "nx": nx, "nu": nu, "u_max": u_max, "dtype": "f64"}
+            try:
+                w = W.linear_rl(B=B, N=N, nx=nx, nu=nu, u_max=u_max)
+                s = Solver(w, dtype="f64", device=dev)
+                ts, out = [], None
+                for _ in range(3):
+                    s.reset_state(); torch.cuda.synchronize(dev)
+                    t0 = time.perf_counter(); out = s.solve_adaptive(1000, 1e-5, 1e-5); ts.append(time.perf_counter() - t0)
+                row.update({"forward_ms": 1e3 * min(ts), "iterations_median": float(np.median(out["iters"])), "iterations_max": int(out["iters"].max()),
+                            "converged_frac": float(out["converged"].mean())})
+                dLdx = 2.0 * s.s["x"]
+                ts = []
+                for _ in range(4):
+                    s.factor(); torch.cuda.synchronize(dev)
+                    t0 = time.perf_counter(); s.backward(dLdx); torch.cuda.synchronize(dev); ts.append(time.perf_counter() - t0)
+                row["backward_ms"] = 1e3 * min(ts[1:])
+                s.close()
+            except Bd.TmpcError as e:
+                row["error"] = str(e)
+            rows.append(row)
+    return rows
+
+
 def f3_row(ctx, args):
     """f3: the humanoid balancing OCP of the paper's imitation-learning experiment (SRB dynamics, RK4, nx = 12, nu = 6, N = 20) with
     the second built-in model: n_sqp x (tmpc_linearize + tmpc_factor + tmpc_admm_solve), fp64 like the paper, B = 1024."""
@@ -465,9 +503,14 @@ def run_gpu(args):
            "peaks": measure_peaks(dev, torch.cuda.current_stream(dev)),
            "kernel_names": KERNEL_NAMES}
     res = []
-    for i, (c, d) in enumerate([] if args.f4_only else config_list(args)):
+    for i, (c, d) in enumerate([] if (args.f4_only or args.f4_sweep) else config_list(args)):
         steps = args.steps if (args.config is not None or i == 0) else max(3, min(args.steps, STEPS_CAP.get(c, args.steps)))
         res.append((c, d, gpu_one(c, d, args, ctx, steps, world == 1 and not args.no_cpu_baseline)))
+    if args.f4_sweep:
+        rows = f4_sweep(ctx, args)
+        if rank == 0:
+            print(json.dumps({"metric": "f4 linear-system RL workload: the sweeps of PAPER.md Fig. 3 (tol 1e-5, fp64)", "rows": rows}))
+        return
     f4 = f4_rows(ctx, args) if (args.config is None and world == 1 and not args.no_f4) or args.f4_only else None
     f3 = f3_row(ctx, args) if f4 is not None else None
     if args.f4_only:
@@ -502,6 +545,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-f4", action="store_true", help="skip the f4 linear-system RL rows of the all-configs run")
     ap.add_argument("--f4-only", action="store_true", help="run only the f4 linear-system RL rows")
+    ap.add_argument("--f4-sweep", action="store_true", help="run only the batch / horizon / block-size sweeps of the paper's Fig. 3 on the f4 workload")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -78,6 +78,20 @@ inline Admm3Plan admm3_plan(const Dims& d, int pg) {
 template <typename T, int NC, int NX, bool XG = false>
 inline size_t admm3_smem_bytes(const Dims& d, int pg) { return (size_t)admm3_plan<T, NC, NX, XG>(d, pg).per_problem * pg * sizeof(T); }
 
+// Cluster variant (CL): per CTA the records of its half (+ the zero record that stands in for the middle stage in the down CTA), the mailbox of
+// the middle exchange and three mbarriers (mid, eta, y).  down0 = 0: each CTA stores its own half from offset 0.
+template <typename T, int NC, int NX>
+inline Admm3Plan admm3_cl_plan(const Dims& d) {
+  using RC = Rec3<T, NC, NX, true>;
+  Admm3Plan P;
+  P.R = RC::G; P.down0 = 0;
+  const int m = d.T / 2, nrecs = (m + 1 > d.T - m) ? m + 1 : d.T - m;
+  P.per_problem = RC::up(nrecs * P.R) + RC::up(NC);      // records + mailbox (zero-filled by the prologue); the mbarriers follow
+  return P;
+}
+template <typename T, int NC, int NX>
+inline size_t admm3_cl_smem_bytes(const Dims& d) { return (size_t)admm3_cl_plan<T, NC, NX>(d).per_problem * sizeof(T) + 32; }
+
 template <typename T>
 struct Admm3Args {
   AdmmArgs<T> a;
@@ -158,10 +172,30 @@ template <typename T, int H> __device__ __forceinline__ T dot2(const T (&a)[H], 
 // read the vector back as a broadcast vector load, one row (inward sweep) or column (outward sweep) of -B_t, one dot.
 // Row i >= n/2 takes its 16-byte chunks in the opposite order (`swb`; the data is not swizzled) so that the eight rows of a
 // slot cover the eight bank groups; the broadcast operand vector is read in the same order.
-template <typename T, int NC, int NX, int PG, bool XG = false>
-__device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, int T_, int lane, unsigned pmask) {   // pmask: bit g = problem g of the CTA is live
+// ---- CL ("cluster"): one problem on a thread-block CLUSTER of two CTAs, for horizons whose chain share outgrows one SM.  The twisted factor
+// splits the work by construction: CTA 0 holds the records of stages 0..m and runs the up chain, CTA 1 holds m+1..N (in reverse order) and runs
+// the down chain.  They meet three times per iteration, each time through distributed shared memory and an mbarrier in the RECEIVER's CTA:
+//   eta:  the item lanes of the boundary stage write their share of the neighbour's right-hand side (E1B of record m+1 resp. 0) remotely;
+//   mid:  the down chain sends its contribution to the middle stage into CTA 0's mailbox, CTA 0 returns y_m into CTA 1's mailbox;
+//   y:    each chain tells the neighbour's boundary lanes that its y's are complete (they read y_{m+1} resp. y_0 remotely in the second phase).
+struct ClCtx { int rank; unsigned box, mb_mid, r_box, r_mb_mid, parity; };   // shared-window addresses: my mailbox / mbarrier, the partner's (shared::cluster)
+__device__ __forceinline__ unsigned cl_rank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ unsigned cl_map(unsigned saddr, unsigned rank) { unsigned r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank)); return r; }
+__device__ __forceinline__ void cl_sync() { asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cl_mbar_init(unsigned a, unsigned cnt) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(a), "r"(cnt) : "memory"); }
+__device__ __forceinline__ void cl_arrive_remote(unsigned ra) { asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(ra) : "memory"); }
+__device__ __forceinline__ void cl_wait(unsigned a, unsigned parity) {
+  unsigned ok;
+  do { asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(a), "r"(parity) : "memory"); } while (!ok);
+}
+__device__ __forceinline__ void cl_sts(unsigned ra, float v) { asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(ra), "f"(v) : "memory"); }
+__device__ __forceinline__ void cl_sts(unsigned ra, double v) { asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(ra), "d"(v) : "memory"); }
+
+template <typename T, int NC, int NX, int PG, bool XG = false, bool CL = false>
+__device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, int T_, int lane, unsigned pmask, const ClCtx cl = ClCtx()) {   // pmask: bit g = problem g of the CTA is live
   constexpr int SL = NC <= 8 ? 8 : 16;                   // lanes per slot (one per row)
   static_assert(NC <= 16 && PG * 2 * SL <= 32, "the chain warp holds (problems x 2 directions) slots of SL lanes");
+  static_assert(!CL || (XG && PG == 1), "the cluster variant keeps the chain's share of one problem per CTA pair");
   using RC = Rec3<T, NC, NX, XG>;
   constexpr int n = NC;
   constexpr unsigned ES = sizeof(T);
@@ -171,14 +205,15 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, in
   // still walk the records of a live-looking slot and load from them — the SAME addresses as that slot's lanes, i.e. pure broadcasts that
   // cost no extra shared-memory wavefront (ncu: parked on the middle record they collided with the working lanes) — but never store.
   const int slot = (lane / SL) % (2 * PG), i8 = lane % SL;
-  const int g = PG == 2 ? (slot >> 1) : 0, dir = slot & 1;
-  const bool live = lane < 2 * PG * SL && i8 < n && ((pmask >> g) & 1u);
+  const int g = PG == 2 ? (slot >> 1) : 0, dir = CL ? cl.rank : (slot & 1);           // CL: every slot mirrors slot 0, which runs this CTA's direction
+  const bool live = (CL ? lane < SL : lane < 2 * PG * SL) && i8 < n && ((pmask >> g) & 1u);
   const int ii = i8 < n ? i8 : 0;
   const unsigned swb = (unsigned)swz_x<T, NC>(ii) * ES;                 // chunk ORDER of my row (bytes)
   const int cnt = dir ? T_ - 1 - m : m, t0 = dir ? N : 0;
   const int dRb = R * (int)ES;                           // both chains advance by +R per step (the down half is stored in reverse order)
   auto rec = [&](int t) { return t > m ? DOWN0 + (N - t) * R : t * R; };
-  const unsigned pb = sb + (unsigned)(g * PP) * ES, bm = pb + (unsigned)rec(m) * ES;
+  // CL, down CTA: the middle stage lives in the partner; a zero record behind the cnt records of this CTA stands in for it
+  const unsigned pb = sb + (unsigned)(g * PP) * ES, bm = pb + (unsigned)((CL && dir) ? cnt * R : rec(m)) * ES;
   constexpr unsigned oE0 = RC::E0 * ES, oE1 = RC::E1A * ES, oE1B = RC::E1B * ES, oLAM = RC::LAM * ES;
   const unsigned me = (unsigned)ii * ES, myrow = oLAM + (unsigned)(ii * n) * ES;
   auto ld_eta = [&](unsigned base) { return lds_1(base + oE1 + me, T(0)) + lds_1(base + oE1B + me, T(0)); };
@@ -186,7 +221,7 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, in
   T wv = cnt > 0 ? ld_eta(bt) : T(0);
   T Br[n];
   lds_row<T, NC>(bt + myrow, swb, Br);
-  const int cmin = T_ - 1 - m;                          // = the down chain's length <= the up chain's (m)
+  const int cmin = CL ? cnt : T_ - 1 - m;               // = the down chain's length <= the up chain's (m); CL: this CTA's own chain
   const int kmain = cmin > 1 ? ((cmin - 1) & ~1) : 0;   // even: the main loop is unrolled by two
   const int dRa = dRb;
   // Main loop: every active slot is on and none is at its last stage, so no predicates.  Two steps per trip with the row
@@ -210,8 +245,9 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, in
     lds_row<T, NC>(bt + myrow, swb, Br);
     wv = dotv_from<n>(Bn, W, eta);
   }
+  const int kend = CL ? cnt : m;
 #pragma unroll 1
-  for (int k = kmain; k < m; ++k) {                    // w_next = eta~_next + (-B_t) w_t, with the per-slot end conditions
+  for (int k = kmain; k < kend; ++k) {                 // w_next = eta~_next + (-B_t) w_t, with the per-slot end conditions
     const bool on = k < cnt, last = k == cnt - 1;
     if (on && live) sts_1(bt + oE1 + me, wv);
     __syncwarp();
@@ -229,12 +265,29 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, in
     for (int j = 0; j < n; ++j) Br[j] = Bn[j];
   }
   // middle stage: w_m = eta~_m + both contributions; y_m = w_m
-  const T wm = wv + __shfl_xor_sync(0xffffffffu, wv, SL);
-  if (live) { sts_1(bm + oE1 + me, wm); sts_1(bm + oE0 + me, wm); }
+  T wm;
+  unsigned bp0 = bm;                                    // where the outward sweep finds the y vector of its first step
+  if constexpr (CL) {
+    if (dir) {                                          // down chain: contribution -> CTA 0's mailbox; y_m comes back into mine
+      if (live) cl_sts(cl.r_box + me, wv);
+      cl_arrive_remote(cl.r_mb_mid);
+      cl_wait(cl.mb_mid, cl.parity);
+      wm = T(0);
+      bp0 = cl.box - oE0;
+    } else {
+      cl_wait(cl.mb_mid, cl.parity);
+      wm = wv + lds_1(cl.box + me, T(0));
+      if (live) { sts_1(bm + oE1 + me, wm); sts_1(bm + oE0 + me, wm); cl_sts(cl.r_box + me, wm); }
+      cl_arrive_remote(cl.r_mb_mid);
+    }
+  } else {
+    wm = wv + __shfl_xor_sync(0xffffffffu, wv, SL);
+    if (live) { sts_1(bm + oE1 + me, wm); sts_1(bm + oE0 + me, wm); }
+  }
   __syncwarp();
   // outward sweep: y_t = w_t + (-B_t)' y_next.  The column of -B_t and w_t of the NEXT step are loaded while this step's
   // y vector is in flight; two steps per trip with the buffers swapping roles.
-  unsigned bc = cnt > 0 ? pb + (unsigned)rec(t0 + (cnt - 1) * (dir ? -1 : 1)) * ES : bm, bp = bm;
+  unsigned bc = cnt > 0 ? pb + (unsigned)rec(t0 + (cnt - 1) * (dir ? -1 : 1)) * ES : bm, bp = bp0;
   auto ld_col = [&](unsigned base, T (&col)[n], T& w) {
 #pragma unroll
     for (int j = 0; j < n; ++j) col[j] = lds_1(base + oLAM + (unsigned)(j * n) * ES + me, T(0));
@@ -252,7 +305,7 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, in
   };
   T colA[n], colB[n], wA, wB;
   ld_col(bc, colA, wA);
-  int k = m - 1;
+  int k = kend - 1;
 #pragma unroll 1
   for (; k >= 1; k -= 2) { bstep(colA, wA, colB, wB, k); bstep(colB, wB, colA, wA, k - 1); }
   if (k == 0) bstep(colA, wA, colB, wB, 0);
@@ -262,7 +315,7 @@ __device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, in
 // order above), the dynamics rows [h KA, ...) of ITS stage's block (block t for t < N; the rows x_0 = x_init for t = N, whose
 // A^+ = [I 0] sits in record 0), and the inequality rows: for a selection G the rows whose column it owns, for a dense G the
 // rows 2 s + h.
-template <typename T, int NC, int NX, int PG, int MAXT, int MINB, bool XG = false>
+template <typename T, int NC, int NX, int PG, int MAXT, int MINB, bool XG = false, bool CL = false>
 __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant__ Admm3Args<T> A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* sm = reinterpret_cast<T*>(smem_raw);
@@ -277,21 +330,27 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   const int m = T_ / 2;
   const int DOWN0 = A.pl.down0;
   auto rec = [&](int t) { return t > m ? DOWN0 + (N - t) * R : t * R; };
+  // CL: CTA `crank` of the pair holds stages [cl_t0, cl_t0 + cl_cnt) of problem blockIdx.x / 2
+  const int crank = CL ? (int)cl_rank() : 0, cl_t0 = crank ? m + 1 : 0, cl_cnt = CL ? (crank ? T_ - 1 - m : m + 1) : T_;
+  const int pbase = CL ? (int)(blockIdx.x >> 1) : (int)blockIdx.x * PG;
+  if constexpr (CL) { if (a.active && !a.active[pbase]) return; }      // a terminated problem (f1): both CTAs of the pair leave before any cluster barrier
+  const unsigned cl_sb = (unsigned)__cvta_generic_to_shared(sm);
+  const unsigned cl_box = cl_sb + (unsigned)(PP - (NC + RC::V - 1) / RC::V * RC::V) * (unsigned)sizeof(T), cl_mb = cl_sb + (unsigned)PP * (unsigned)sizeof(T);   // mailbox; mbarriers mid, eta, y
 
   // ---- stage 1: X_t, -B_t and the raw constraint blocks of every problem of this CTA into the records (all threads)
 #pragma unroll 1
   for (int g = 0; g < PG; ++g) {
-    const int p = blockIdx.x * PG + g;
+    const int p = pbase + g;
     T* P = sm + g * PP;
     for (int e = tid; e < PP; e += nt) P[e] = T(0);
     __syncthreads();
     if (p >= d.B) continue;
     const T* gLam = a.Lam + (size_t)p * T_ * nn;
     const T* gX = a.Sinv + (size_t)p * T_ * nn;
-    for (int e = tid; e < T_ * nn; e += nt) {
-      const int t = e / nn, rc = e - t * nn;
+    for (int e = tid; e < cl_cnt * nn; e += nt) {
+      const int t = cl_t0 + e / nn, rc = e - (t - cl_t0) * nn;
       const int o = rec(t) + rc;
-      if (t != m) P[o + RC::LAM] = -gLam[e];
+      if (t != m) P[o + RC::LAM] = -gLam[(size_t)t * nn + rc];
       if constexpr (!XG) P[o + RC::SINV] = gX[e];
     }
     if (!XG && !a.kkt_only) {
@@ -331,12 +390,24 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
     __syncthreads();
   }
 
+  // CL: the three mbarriers of this CTA (mid: the partner's chain warp arrives; eta: the partner's two boundary lanes; y: the partner's chain warp),
+  // then a cluster barrier: nobody touches the partner's shared memory before it is set up
+  unsigned r_box = 0u, r_mb = 0u;
+  if constexpr (CL) {
+    if (tid == 0) {
+      cl_mbar_init(cl_mb, 32u); cl_mbar_init(cl_mb + 8u, 2u); cl_mbar_init(cl_mb + 16u, 32u);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    r_box = cl_map(cl_box, (unsigned)(crank ^ 1)); r_mb = cl_map(cl_mb, (unsigned)(crank ^ 1));
+    cl_sync();
+  }
+
   // ================================================================ chain warp
   if (tid < 32) {
     const int iters = a.kkt_only ? 1 : a.iters;
     unsigned pmask = 0u;
 #pragma unroll
-    for (int g = 0; g < PG; ++g) { const int p = blockIdx.x * PG + g; if (p < d.B && (!a.active || a.active[p])) pmask |= 1u << g; }
+    for (int g = 0; g < PG; ++g) { const int p = pbase + g; if (p < d.B && (!a.active || a.active[p])) pmask |= 1u << g; }
 #pragma unroll 1
 #ifdef TMPC_TIMING
     long long tch = 0; const long long tbeg = clock64();
@@ -346,13 +417,19 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
 #ifdef TMPC_TIMING
       __syncwarp(); const T probe = sm[tid & 7]; const long long c1 = clock64() + (probe == T(12345.678) ? 1 : 0);   // the load makes the deferred barrier block first
 #endif
-      chain3_solve<T, NC, NX, PG, XG>(sm, R, A.pl.down0, PP, T_, tid, pmask);
+      if constexpr (CL) {
+        if (!a.kkt_only) cl_wait(cl_mb + 8u, (unsigned)(it & 1));      // the partner's boundary lanes have delivered their share of my right-hand side
+        ClCtx cc; cc.rank = crank; cc.box = cl_box; cc.mb_mid = cl_mb; cc.r_box = r_box; cc.r_mb_mid = r_mb; cc.parity = (unsigned)(it & 1);
+        chain3_solve<T, NC, NX, PG, XG, true>(sm, R, A.pl.down0, PP, T_, tid, pmask, cc);
+      } else chain3_solve<T, NC, NX, PG, XG>(sm, R, A.pl.down0, PP, T_, tid, pmask);
       __syncwarp();
 #ifdef TMPC_TIMING
       tch += clock64() - c1;
 #endif
       bar_arrive(2, nt);
+      if constexpr (CL) cl_arrive_remote(r_mb + 16u);                  // my y's are complete: the partner's boundary lanes may read across
     }
+    if constexpr (CL) cl_sync();                                       // neither CTA leaves while the other may still reach into it
 #ifdef TMPC_TIMING
     if ((blockIdx.x == 0 || blockIdx.x == gridDim.x - 1) && tid == 0) printf("cta %d: %lld cycles per iteration, of which chain %lld\n", blockIdx.x, (clock64() - tbeg) / iters, tch / iters);
 #endif
@@ -360,11 +437,15 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   }
 
   // ================================================================ item warps
-  const int per_p = 2 * T_;                              // lanes per problem
-  const int g = it_tid / per_p, rem = it_tid - g * per_p, t = rem >> 1, h = rem & 1, p = blockIdx.x * PG + g;
+  const int per_p = 2 * cl_cnt;                          // lanes per problem (CL: of this CTA's half)
+  const int g = it_tid / per_p, rem = it_tid - g * per_p, t = cl_t0 + (rem >> 1), h = rem & 1, p = pbase + g;
   const bool valid = g < PG && p < d.B && (!a.active || a.active[p]);      // a terminated problem (f1) is left untouched
   const HalfOff mine = half_off<NC>(h), other = half_off<NC>(1 - h);
   const int b = valid ? g * PP + rec(t) : 0, bn = valid ? g * PP + (t < N ? rec(t + 1) : rec(0)) : 0;
+  // the record of the next stage (E1B written in the first phase, E0 read in the second): for the boundary stage of a CL half it is the partner's
+  const bool cross = CL && valid && (crank ? t == N : t == m);
+  T* nbp = sm + bn;
+  if constexpr (CL) { if (cross) { unsigned long long ga; asm volatile("mapa.u64 %0, %1, %2;" : "=l"(ga) : "l"((unsigned long long)(sm + bn)), "r"((unsigned)(crank ^ 1))); nbp = reinterpret_cast<T*>(ga); } }
   // the blocks the item lanes read: X_t, A~^-_t (my record) and A~^+_t (the next record) — shared memory, or global memory for XG
   const size_t gst = valid ? (size_t)p * T_ + t : 0, gsn = valid ? (size_t)p * T_ + (t < N ? t + 1 : 0) : 0;
   const T* Xb = XG ? a.Sinv + gst * nn : sm + b + RC::SINV;
@@ -399,6 +480,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
 #pragma unroll
       for (int s = 0; s < H; ++s) a.xi[(size_t)p * nz + t * n + slot_col<NC>(h, s)] = xt[s];
     }
+    if constexpr (CL) cl_sync();
     return;
   }
 
@@ -515,13 +597,15 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
         }
       }
       st_half<NC>(sm + b + RC::E1A, mine, acc);
-      st_half<NC>(sm + bn + RC::E1B, mine, accb);
+      st_half<NC>(nbp + RC::E1B, mine, accb);
+      if constexpr (CL) { if (cross) cl_arrive_remote(r_mb + 8u); }
     }
 #ifdef TMPC_TIMING
     const long long qa = clock64();
 #endif
     bar_arrive(1, nt);
     bar_sync(2, nt);
+    if constexpr (CL) { if (cross) cl_wait(cl_mb + 16u, (unsigned)(it & 1)); }   // the partner's chain has finished: y of the stage across the boundary is there
 #ifdef TMPC_TIMING
     { const T probe = sm[b + RC::E0]; const long long qb = clock64() + (probe == T(12345.678) ? 1 : 0); tA += qa - qs; tW += qb - qa; qs = qb; }
 #endif
@@ -538,7 +622,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
       for (int jj = 0; jj < H; ++jj) { T mk[H]; ld_half<NC>(Xb + slot_col<NC>(1 - h, jj) * n, mine, mk); axpy_half<H>(xt, mk, yr[jj]); }   // rows of the partner's half
       if (nk > 0) {
         T y2o[H], y2r[H];
-        ld_half<NC>(sm + bn + RC::E0, mine, y2o); ld_half<NC>(sm + bn + RC::E0, other, y2r);
+        ld_half<NC>(nbp + RC::E0, mine, y2o); ld_half<NC>(nbp + RC::E0, other, y2r);
 #pragma unroll
         for (int s = 0; s < KA; ++s) if (s < nk) {
           const int k = k0 + s;
@@ -583,6 +667,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
       a.zg[row] = zg[s]; a.yg[row] = yg[s]; if (a.iters > 0) a.xi[row] = xi_last[s];
     }
   }
+  if constexpr (CL) cl_sync();
 }
 
 // ---- XG: the constraint blocks in the scaled variables, once per launch of the solve: row k of stage t of

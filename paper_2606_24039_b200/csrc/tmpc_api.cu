@@ -148,7 +148,7 @@ tmpc_status launch_admm_inst(tmpc_ctx* h, const AdmmArgs<T>& a, int nt, size_t s
   k<<<h->d.B, nt, smem, h->stream>>>(a); h->launches++;
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
 }
-struct FastPlan { bool ok, xg; int pg, nt, ctas_per_sm; size_t smem; };
+struct FastPlan { bool ok, xg, cl; int pg, nt, ctas_per_sm; size_t smem; };   // xg: X / A~ in global memory; cl: one problem on a cluster of two CTAs
 template <typename T> FastPlan fast_plan(const Dims& d);
 template <typename T> tmpc_status launch_resident(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f);
 template <typename T> tmpc_status launch_residual(tmpc_ctx* h, const AdmmArgs<T>& s);
@@ -220,7 +220,7 @@ tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
 constexpr size_t kSmemPerSM = 228 * 1024;
 template <typename T>
 FastPlan fast_plan(const Dims& d) {
-  FastPlan f; f.ok = false; f.xg = false; f.pg = 1; f.nt = 0; f.ctas_per_sm = 0; f.smem = 0;
+  FastPlan f; f.ok = false; f.xg = false; f.cl = false; f.pg = 1; f.nt = 0; f.ctas_per_sm = 0; f.smem = 0;
   const bool shape = (d.n == 8 && d.nx == 6) || (d.n == 6 && d.nx == 4) || (d.n == 12 && d.nx == 8);   // (12, 8): the nominal block size of the paper's scaling study (f4)
   if (!shape || d.ng > d.n || d.T < 2) return f;
   if (d.g_sel) for (int r = 0; r < d.ng; ++r) for (int q = 0; q < r; ++q) if (d.g_col[r] == d.g_col[q]) return f;   // one selection row per column
@@ -230,7 +230,15 @@ FastPlan fast_plan(const Dims& d) {
     // long horizons: only the chain's share of a record stays in shared memory (Rec3<.., XG>), one problem per CTA, two item lanes per stage
     const size_t sx = d.n == 8 ? admm3_smem_bytes<T, 8, 6, true>(d, 1) : d.n == 6 ? admm3_smem_bytes<T, 6, 4, true>(d, 1) : admm3_smem_bytes<T, 12, 8, true>(d, 1);
     const int ntx = 32 + (2 * d.T + 31) / 32 * 32;
-    if (sx > kMaxSmem || ntx > 1024) return f;
+    if (sx > kMaxSmem || ntx > 1024) {
+      // longer still: the two half chains of the twisted factor on a cluster of two CTAs (tmpc_admm3.cuh, CL), (12, 8) block
+      if (d.n != 12 || d.T < 8) return f;
+      const size_t sc = admm3_cl_smem_bytes<T, 12, 8>(d);
+      const int half = d.T / 2 + 1, ntc = 32 + (2 * half + 31) / 32 * 32;
+      if (sc > kMaxSmem || ntc > 704) return f;
+      f.ok = true; f.xg = true; f.cl = true; f.pg = 1; f.nt = ntc; f.ctas_per_sm = 1; f.smem = sc;
+      return f;
+    }
     f.ok = true; f.xg = true; f.pg = 1; f.nt = ntx; f.ctas_per_sm = (int)(kSmemPerSM / (sx + 1024)); f.smem = sx;
     return f;
   }
@@ -251,12 +259,13 @@ bool plan_xg(const tmpc_config& c) {
   return c.dtype == TMPC_F64 ? fast_plan<double>(d).xg : fast_plan<float>(d).xg;
 }
 
-template <typename T, int NC, int NX, int PG, int MAXT, int MINB, bool XG = false>
+template <typename T, int NC, int NX, int PG, int MAXT, int MINB, bool XG = false, bool CL = false>
 tmpc_status launch_admm3_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
-  auto k = admm3_kernel<T, NC, NX, PG, MAXT, MINB, XG>;
+  auto k = admm3_kernel<T, NC, NX, PG, MAXT, MINB, XG, CL>;
   if (f.smem > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem) != cudaSuccess) return TMPC_E_CUDA;
   const unsigned grid = (unsigned)((h->d.B + PG - 1) / PG);
-  Admm3Args<T> A; A.a = a; A.pl = admm3_plan<T, NC, NX, XG>(h->d, PG); A.atil = nullptr;
+  Admm3Args<T> A; A.a = a; A.atil = nullptr;
+  if constexpr (CL) A.pl = admm3_cl_plan<T, NC, NX>(h->d); else A.pl = admm3_plan<T, NC, NX, XG>(h->d, PG);
   if constexpr (XG) {
     T* atil = (T*)(h->ws + h->lay.atil); A.atil = atil;
     if (!a.kkt_only) {
@@ -265,6 +274,15 @@ tmpc_status launch_admm3_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan&
     }
   }
   A.rfa = a.prm.rho_f * a.prm.alpha; A.oma = T(1) - a.prm.alpha; A.inv_rho_g = T(1) / a.prm.rho_g; A.inv_rg = T(1) / (a.prm.rho_g + a.prm.gamma);
+  if constexpr (CL) {                                   // two CTAs per problem, launched as a cluster
+    cudaLaunchConfig_t lc; memset(&lc, 0, sizeof(lc));
+    lc.gridDim = dim3(2u * (unsigned)h->d.B); lc.blockDim = dim3((unsigned)f.nt); lc.dynamicSmemBytes = f.smem; lc.stream = h->stream;
+    cudaLaunchAttribute at[1]; at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    lc.attrs = at; lc.numAttrs = 1;
+    if (cudaLaunchKernelEx(&lc, k, A) != cudaSuccess) { cudaGetLastError(); return TMPC_E_CUDA; }
+    h->launches++;
+    return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
+  }
   k<<<grid, f.nt, f.smem, h->stream>>>(A); h->launches++;
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
 }
@@ -291,6 +309,7 @@ tmpc_status launch_admm3_xg(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f
 template <typename T>
 tmpc_status launch_resident(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
   const Dims& d = h->d;
+  if (f.cl) return f.nt <= 384 ? launch_admm3_inst<T, 12, 8, 1, 384, 1, true, true>(h, a, f) : launch_admm3_inst<T, 12, 8, 1, 704, 1, true, true>(h, a, f);
   if (f.xg) {
     if (d.n == 12) return launch_admm3_xg<T, 12, 8>(h, a, f);
     if (d.n == 8) return launch_admm3_xg<T, 8, 6>(h, a, f);

@@ -657,6 +657,33 @@ def test_f4_linear_rl_long_horizons_chain_resident():
     s.close()
 
 
+def test_f4_linear_rl_cluster_pair_fp64():
+    """N = 320 in fp64 (the end of the paper's horizon sweep): the chain's share of the records no longer fits one SM, the two half
+    chains of the twisted factor run on a cluster of two CTAs that meet through distributed shared memory (admm3_kernel<.., CL>).  One iteration
+    (every exchange exactly once), fixed counts at even and odd T, the adaptive run with per-problem termination, and the REFINE backward."""
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    run_pair(W.linear_rl(B=1, N=320, u_max=1.0), "f64", iters=1)
+    w = W.linear_rl(B=3, N=320, u_max=1.0)
+    run_pair(w, "f64", iters=40)
+    run_pair(W.linear_rl(B=2, N=321, u_max=10.0), "f64", iters=40)
+    ref, rinfo, log, rc = O.admm_adaptive(w, O.make_cfg(w), O.make_adaptive(300, 1e-4, 1e-4))
+    s = Solver(w, dtype="f64")
+    out = s.solve_adaptive(300, 1e-4, 1e-4)
+    assert (out["iters"] == rinfo[:, 4].astype(int)).all() and (out["converged"] == rinfo[:, 6].astype(int)).all()
+    assert len(set(out["iters"].tolist())) > 1            # the problems stop at different checks: pairs leave while others go on
+    compare_states(s.state_numpy(), ref, 1e-7)
+    cfg = O.make_cfg(w)
+    ref, info, rc = O.admm(w, O.make_cfg(w, rho_bar=5.0), iters=3000)
+    dq_o, dxi_o, counts, rcs = O.backward(w, cfg, ref, 2.0 * ref["x"])
+    ok = rcs == 0
+    assert ok.sum() >= 2
+    s.set_state(ref)
+    dq, dxi = s.backward(s._up(2.0 * ref["x"]), mode=Bd.TMPC_BWD_REFACTOR_REFINE)
+    assert rel_err(dq.cpu().double().numpy()[ok], dq_o[ok]) <= 1e-9 and rel_err(dxi.cpu().double().numpy()[ok], dxi_o[ok]) <= 1e-9
+    s.close()
+
+
 def test_long_horizons_chain_resident_small_blocks():
     """The same variant for the (8, 6) and (6, 4) blocks once their records outgrow shared memory (fp64: N > ~190 resp. ~330): selection G with
     soft rows (config 2's data at N = 260), dense G (config 4's bicycle QP at N = 400, G~ rows in global memory too), and the thread-cap
