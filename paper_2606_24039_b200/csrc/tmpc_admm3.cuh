@@ -80,17 +80,17 @@ inline size_t admm3_smem_bytes(const Dims& d, int pg) { return (size_t)admm3_pla
 
 // Cluster variant (CL): per CTA the records of its half (+ the zero record that stands in for the middle stage in the down CTA), the mailbox of
 // the middle exchange and three mbarriers (mid, eta, y).  down0 = 0: each CTA stores its own half from offset 0.
-template <typename T, int NC, int NX>
+template <typename T, int NC, int NX, bool XG>
 inline Admm3Plan admm3_cl_plan(const Dims& d) {
-  using RC = Rec3<T, NC, NX, true>;
+  using RC = Rec3<T, NC, NX, XG>;
   Admm3Plan P;
-  P.R = RC::G; P.down0 = 0;
+  P.R = RC::pad_stride((d.g_sel || XG) ? RC::G : RC::G + RC::up(d.ng * NC)); P.down0 = 0;
   const int m = d.T / 2, nrecs = (m + 1 > d.T - m) ? m + 1 : d.T - m;
   P.per_problem = RC::up(nrecs * P.R) + RC::up(NC);      // records + mailbox (zero-filled by the prologue); the mbarriers follow
   return P;
 }
-template <typename T, int NC, int NX>
-inline size_t admm3_cl_smem_bytes(const Dims& d) { return (size_t)admm3_cl_plan<T, NC, NX>(d).per_problem * sizeof(T) + 32; }
+template <typename T, int NC, int NX, bool XG>
+inline size_t admm3_cl_smem_bytes(const Dims& d) { return (size_t)admm3_cl_plan<T, NC, NX, XG>(d).per_problem * sizeof(T) + 32; }
 
 template <typename T>
 struct Admm3Args {
@@ -195,7 +195,7 @@ template <typename T, int NC, int NX, int PG, bool XG = false, bool CL = false>
 __device__ __forceinline__ void chain3_solve(T* sm, int R, int DOWN0, int PP, int T_, int lane, unsigned pmask, const ClCtx cl = ClCtx()) {   // pmask: bit g = problem g of the CTA is live
   constexpr int SL = NC <= 8 ? 8 : 16;                   // lanes per slot (one per row)
   static_assert(NC <= 16 && PG * 2 * SL <= 32, "the chain warp holds (problems x 2 directions) slots of SL lanes");
-  static_assert(!CL || (XG && PG == 1), "the cluster variant keeps the chain's share of one problem per CTA pair");
+  static_assert(!CL || PG == 1, "the cluster variant keeps one problem per CTA pair");
   using RC = Rec3<T, NC, NX, XG>;
   constexpr int n = NC;
   constexpr unsigned ES = sizeof(T);
@@ -351,18 +351,18 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
       const int t = cl_t0 + e / nn, rc = e - (t - cl_t0) * nn;
       const int o = rec(t) + rc;
       if (t != m) P[o + RC::LAM] = -gLam[(size_t)t * nn + rc];
-      if constexpr (!XG) P[o + RC::SINV] = gX[e];
+      if constexpr (!XG) P[o + RC::SINV] = gX[(size_t)t * nn + rc];
     }
     if (!XG && !a.kkt_only) {
       const T* gAm = a.qp.Am + (size_t)p * N * nx * n; const T* gAp = a.qp.Ap + (size_t)p * N * nx * n;
-      for (int e = tid; e < T_ * nx * n; e += nt) {
-        const int t = e / (nx * n), rc = e - t * nx * n, k = rc / n, j = rc - k * n;
+      for (int e = tid; e < cl_cnt * nx * n; e += nt) {
+        const int t = cl_t0 + e / (nx * n), rc = e - (t - cl_t0) * nx * n, k = rc / n, j = rc - k * n;
         if (t < N) P[rec(t) + RC::AM + rc] = gAm[(size_t)t * nx * n + rc];
         P[rec(t) + RC::AP + rc] = t > 0 ? gAp[(size_t)(t - 1) * nx * n + rc] : (k == j ? T(1) : T(0));      // A_init = [I 0]
       }
       if (!d.g_sel) {
         const T* gG = a.qp.G + a.qp.sG * p;
-        for (int e = tid; e < T_ * ng * n; e += nt) { const int t = e / (ng * n), rc = e - t * ng * n; P[rec(t) + RC::G + rc] = gG[e]; }
+        for (int e = tid; e < cl_cnt * ng * n; e += nt) { const int t = cl_t0 + e / (ng * n), rc = e - (t - cl_t0) * ng * n; P[rec(t) + RC::G + rc] = gG[(size_t)t * ng * n + rc]; }
       }
     }
   }
@@ -371,9 +371,9 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   // (A~^-_t = A^-_t X_t', A~^+_{t-1} = A^+_{t-1} X_t', G~_t = G_t X_t'); a thread owns a whole row, so there is no hazard
   if (!XG && !a.kkt_only) {
     const int rows_t = 2 * nx + (d.g_sel ? 0 : ng);       // rows per stage: AM, AP, G
-    for (int e = tid; e < PG * T_ * rows_t; e += nt) {
-      const int g = e / (T_ * rows_t), r2 = e - g * T_ * rows_t, t = r2 / rows_t, k = r2 - t * rows_t;
-      if (blockIdx.x * PG + g >= d.B) continue;
+    for (int e = tid; e < PG * cl_cnt * rows_t; e += nt) {
+      const int g = e / (cl_cnt * rows_t), r2 = e - g * cl_cnt * rows_t, t = cl_t0 + r2 / rows_t, k = r2 - (t - cl_t0) * rows_t;
+      if (pbase + g >= d.B) continue;
       T* rowp = sm + g * PP + rec(t) + (k < nx ? RC::AM + k * n : (k < 2 * nx ? RC::AP + (k - nx) * n : RC::G + (k - 2 * nx) * n));
       const T* X = sm + g * PP + rec(t) + RC::SINV;
       T v[n], o[n];
@@ -442,7 +442,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   const bool valid = g < PG && p < d.B && (!a.active || a.active[p]);      // a terminated problem (f1) is left untouched
   const HalfOff mine = half_off<NC>(h), other = half_off<NC>(1 - h);
   const int b = valid ? g * PP + rec(t) : 0, bn = valid ? g * PP + (t < N ? rec(t + 1) : rec(0)) : 0;
-  // the record of the next stage (E1B written in the first phase, E0 read in the second): for the boundary stage of a CL half it is the partner's
+  // the record of the next stage (E1B written in the first phase, E0 and A~^+ read): for the boundary stage of a CL half it is the partner's
   const bool cross = CL && valid && (crank ? t == N : t == m);
   T* nbp = sm + bn;
   if constexpr (CL) { if (cross) { unsigned long long ga; asm volatile("mapa.u64 %0, %1, %2;" : "=l"(ga) : "l"((unsigned long long)(sm + bn)), "r"((unsigned)(crank ^ 1))); nbp = reinterpret_cast<T*>(ga); } }
@@ -451,7 +451,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   const T* Xb = XG ? a.Sinv + gst * nn : sm + b + RC::SINV;
   const int arows = 2 * nx + (d.g_sel ? 0 : ng);        // rows of a stage in atil: A~^-, A~^+, G~ (dense G only)
   const T* AMb = XG ? A.atil + gst * (arows * n) : sm + b + RC::AM;
-  const T* APn = XG ? A.atil + gsn * (arows * n) + nx * n : sm + bn + RC::AP;
+  const T* APn = XG ? A.atil + gsn * (arows * n) + nx * n : nbp + RC::AP;
   const T* Gb = XG ? A.atil + gst * (arows * n) + 2 * nx * n : sm + b + RC::G;
 
   if (a.kkt_only) {                                      // xt <- S^{-1} eta : eta~ = X eta, solve, x = X' y

@@ -218,6 +218,11 @@ tmpc_status launch_admm(tmpc_ctx* h, AdmmArgs<T>& a) {
 
 // ---- resident fast path (tmpc_admm3.cuh): eligibility and launch shape
 constexpr size_t kSmemPerSM = 228 * 1024;
+int sm_count() {
+  static int sms = 0;
+  if (sms == 0) { int dev = 0; if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) { cudaGetLastError(); sms = 148; } }
+  return sms;
+}
 template <typename T>
 FastPlan fast_plan(const Dims& d) {
   FastPlan f; f.ok = false; f.xg = false; f.cl = false; f.pg = 1; f.nt = 0; f.ctas_per_sm = 0; f.smem = 0;
@@ -227,18 +232,24 @@ FastPlan fast_plan(const Dims& d) {
   const size_t s1 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 1) : d.n == 6 ? admm3_smem_bytes<T, 6, 4>(d, 1) : admm3_smem_bytes<T, 12, 8>(d, 1);
   const size_t s2 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 2) : d.n == 6 ? admm3_smem_bytes<T, 6, 4>(d, 2) : kMaxSmem + 1;   // n = 12: one problem per CTA (16 chain lanes per slot)
   if (s1 > kMaxSmem) {
+    // The (12, 8) block first tries a CLUSTER of two CTAs per problem (tmpc_admm3.cuh, CL): with full records when the two halves fit two SMs
+    // (same throughput per SM as the single-CTA variant below at about half the latency per iteration), ...
+    const int half = d.T / 2 + 1, ntc = 32 + (2 * half + 31) / 32 * 32;
+    const bool cl_shape = d.n == 12 && d.T >= 8 && ntc <= 384;
+    if (cl_shape) {
+      const size_t sr = admm3_cl_smem_bytes<T, 12, 8, false>(d);
+      if (sr <= kMaxSmem) { f.ok = true; f.cl = true; f.nt = ntc; f.ctas_per_sm = 1; f.smem = sr; return f; }
+    }
     // long horizons: only the chain's share of a record stays in shared memory (Rec3<.., XG>), one problem per CTA, two item lanes per stage
     const size_t sx = d.n == 8 ? admm3_smem_bytes<T, 8, 6, true>(d, 1) : d.n == 6 ? admm3_smem_bytes<T, 6, 4, true>(d, 1) : admm3_smem_bytes<T, 12, 8, true>(d, 1);
     const int ntx = 32 + (2 * d.T + 31) / 32 * 32;
-    if (sx > kMaxSmem || ntx > 1024) {
-      // longer still: the two half chains of the twisted factor on a cluster of two CTAs (tmpc_admm3.cuh, CL), (12, 8) block
-      if (d.n != 12 || d.T < 8) return f;
-      const size_t sc = admm3_cl_smem_bytes<T, 12, 8>(d);
-      const int half = d.T / 2 + 1, ntc = 32 + (2 * half + 31) / 32 * 32;
-      if (sc > kMaxSmem || ntc > 704) return f;
-      f.ok = true; f.xg = true; f.cl = true; f.pg = 1; f.nt = ntc; f.ctas_per_sm = 1; f.smem = sc;
-      return f;
+    // ... and with the chain's share only when that no longer fits one SM, or when the batch leaves half of the SMs idle anyway
+    const bool one_fits = sx <= kMaxSmem && ntx <= 1024;
+    if (cl_shape && (!one_fits || 2 * d.B <= sm_count())) {
+      const size_t sc = admm3_cl_smem_bytes<T, 12, 8, true>(d);
+      if (sc <= kMaxSmem) { f.ok = true; f.xg = true; f.cl = true; f.nt = ntc; f.ctas_per_sm = 1; f.smem = sc; return f; }
     }
+    if (!one_fits) return f;
     f.ok = true; f.xg = true; f.pg = 1; f.nt = ntx; f.ctas_per_sm = (int)(kSmemPerSM / (sx + 1024)); f.smem = sx;
     return f;
   }
@@ -265,7 +276,7 @@ tmpc_status launch_admm3_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan&
   if (f.smem > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem) != cudaSuccess) return TMPC_E_CUDA;
   const unsigned grid = (unsigned)((h->d.B + PG - 1) / PG);
   Admm3Args<T> A; A.a = a; A.atil = nullptr;
-  if constexpr (CL) A.pl = admm3_cl_plan<T, NC, NX>(h->d); else A.pl = admm3_plan<T, NC, NX, XG>(h->d, PG);
+  if constexpr (CL) A.pl = admm3_cl_plan<T, NC, NX, XG>(h->d); else A.pl = admm3_plan<T, NC, NX, XG>(h->d, PG);
   if constexpr (XG) {
     T* atil = (T*)(h->ws + h->lay.atil); A.atil = atil;
     if (!a.kkt_only) {
@@ -309,7 +320,7 @@ tmpc_status launch_admm3_xg(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f
 template <typename T>
 tmpc_status launch_resident(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan& f) {
   const Dims& d = h->d;
-  if (f.cl) return f.nt <= 384 ? launch_admm3_inst<T, 12, 8, 1, 384, 1, true, true>(h, a, f) : launch_admm3_inst<T, 12, 8, 1, 704, 1, true, true>(h, a, f);
+  if (f.cl) return f.xg ? launch_admm3_inst<T, 12, 8, 1, 384, 1, true, true>(h, a, f) : launch_admm3_inst<T, 12, 8, 1, 384, 1, false, true>(h, a, f);
   if (f.xg) {
     if (d.n == 12) return launch_admm3_xg<T, 12, 8>(h, a, f);
     if (d.n == 8) return launch_admm3_xg<T, 8, 6>(h, a, f);

@@ -667,6 +667,12 @@ def test_f4_linear_rl_cluster_pair_fp64():
     w = W.linear_rl(B=3, N=320, u_max=1.0)
     run_pair(w, "f64", iters=40)
     run_pair(W.linear_rl(B=2, N=321, u_max=10.0), "f64", iters=40)
+    # the pair with FULL records (horizons between one and two SMs' worth: N = 80 in fp64, 160 in fp32), incl. dense A^+ (remote A~^+ rows)
+    run_pair(W.linear_rl(B=3, N=80, u_max=1.0), "f64", iters=60)
+    run_pair(W.with_dense_Ap(W.linear_rl(B=2, N=81, u_max=10.0)), "f64", iters=40)
+    run_pair(W.linear_rl(B=3, N=160, u_max=1.0), "f32", iters=60)
+    # a batch that fills the GPU keeps one CTA per problem (chain-resident, no cluster)
+    run_pair(W.linear_rl(B=80, N=160, u_max=1.0), "f64", iters=30)
     ref, rinfo, log, rc = O.admm_adaptive(w, O.make_cfg(w), O.make_adaptive(300, 1e-4, 1e-4))
     s = Solver(w, dtype="f64")
     out = s.solve_adaptive(300, 1e-4, 1e-4)
