@@ -178,6 +178,14 @@ template <typename T, int H> __device__ __forceinline__ T dot2(const T (&a)[H], 
 //   eta:  the item lanes of the boundary stage write their share of the neighbour's right-hand side (E1B of record m+1 resp. 0) remotely;
 //   mid:  the down chain sends its contribution to the middle stage into CTA 0's mailbox, CTA 0 returns y_m into CTA 1's mailbox;
 //   y:    each chain tells the neighbour's boundary lanes that its y's are complete (they read y_{m+1} resp. y_0 remotely in the second phase).
+// Ordering of the remote fields across iterations (each mbarrier completes one phase per iteration, parity = iteration & 1):
+//   * a boundary lane writes the neighbour's E1B for iteration k+1 only after its own second phase of iteration k, which waited for `y` of
+//     iteration k, i.e. for the neighbour's chain to have consumed iteration k's right-hand side;
+//   * a chain warp starts iteration k+1 (and overwrites its y's, its mailbox partner's contents) only after `eta` of iteration k+1, which the
+//     neighbour's boundary lanes send after their second phase of iteration k — their remote reads of y are done, and the neighbour's chain
+//     warp, having passed its named barrier 2 of iteration k before those lanes could, is done with both mailboxes;
+//   * the first remote access of the kernel comes after the cluster barrier that follows the prologue, the last one before the cluster barrier
+//     at exit.
 struct ClCtx { int rank; unsigned box, mb_mid, r_box, r_mb_mid, parity; };   // shared-window addresses: my mailbox / mbarrier, the partner's (shared::cluster)
 __device__ __forceinline__ unsigned cl_rank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
 __device__ __forceinline__ unsigned cl_map(unsigned saddr, unsigned rank) { unsigned r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank)); return r; }

@@ -108,3 +108,18 @@ def test_sharding_two_ranks_gloo():
     assert res[0][3] == full.x_init[0, 0] and res[1][3] == full.x_init[8, 0]     # disjoint, covering problem ranges
     assert all(r[4] == 11.0 and r[5] == 16.0 for r in res)                       # MAX of timings, SUM of units
     assert [(r[6], r[7]) for r in res] == [(0, 6), (6, 5)]
+
+
+def test_shared_memory_plans_of_the_resident_kernel(tmp_path):
+    """Host logic of tmpc_admm3.cuh: the record-stride / placement plans (plain, chain-resident, cluster pair) terminate, keep the alignments the
+    kernel's vector accesses assume and cover the records they place, for every horizon 2..700 of the three fast-path blocks in both dtypes; and the
+    two capacity claims of DESIGN.md 5.1 ((64,160,8,4) fp64 on one SM, (64,320,8,4) fp64 on a pair).  tests/plan_check.cu, host code only."""
+    import shutil
+    import subprocess
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    here = os.path.dirname(os.path.abspath(__file__))
+    exe = str(tmp_path / "plan_check")
+    subprocess.run([nvcc, "-std=c++17", "-O1", "-gencode", "arch=compute_100a,code=sm_100a", "-I", os.path.join(here, "..", "include"),
+                    "-o", exe, os.path.join(here, "plan_check.cu")], check=True, capture_output=True, timeout=300)
+    r = subprocess.run([exe], capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0 and "plan_check: ok" in r.stdout, r.stdout[-2000:]
