@@ -232,11 +232,12 @@ FastPlan fast_plan(const Dims& d) {
   const size_t s1 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 1) : d.n == 6 ? admm3_smem_bytes<T, 6, 4>(d, 1) : admm3_smem_bytes<T, 12, 8>(d, 1);
   const size_t s2 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 2) : d.n == 6 ? admm3_smem_bytes<T, 6, 4>(d, 2) : kMaxSmem + 1;   // n = 12: one problem per CTA (16 chain lanes per slot)
   if (s1 > kMaxSmem) {
-    // The (12, 8) block first tries a CLUSTER of two CTAs per problem (tmpc_admm3.cuh, CL): with full records when the two halves fit two SMs
-    // (same throughput per SM as the single-CTA variant below at about half the latency per iteration), ...
+    // The (12, 8) block first tries a CLUSTER of two CTAs per problem (tmpc_admm3.cuh, CL) when the batch leaves half of the SMs idle anyway: with
+    // full records when the two halves fit two SMs (about half the latency per iteration of the single-CTA variant below; for batches that fill
+    // the GPU one CTA per problem is ~8 % faster: 15.9 vs 17.4 ms per 100 iterations at (1024,80,8,4) fp64), ...
     const int half = d.T / 2 + 1, ntc = 32 + (2 * half + 31) / 32 * 32;
     const bool cl_shape = d.n == 12 && d.T >= 8 && ntc <= 384;
-    if (cl_shape) {
+    if (cl_shape && 2 * d.B <= sm_count()) {
       const size_t sr = admm3_cl_smem_bytes<T, 12, 8, false>(d);
       if (sr <= kMaxSmem) { f.ok = true; f.cl = true; f.nt = ntc; f.ctas_per_sm = 1; f.smem = sr; return f; }
     }
