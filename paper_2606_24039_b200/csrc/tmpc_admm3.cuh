@@ -96,7 +96,8 @@ template <typename T>
 struct Admm3Args {
   AdmmArgs<T> a;
   Admm3Plan pl;
-  const T* atil;                      // XG only: A~^-, A~^+ and (dense G) G~ per stage, [B][T][2 nx + ng][n] (atil_kernel)
+  const T* atil;                      // XG only: X, A~^-, A~^+ and (dense G) G~ of every stage in the stage-minor layout atil_kernel writes
+  int tpad;                           // ... whose chunk stride is tpad * V elements (tpad = T rounded up to 8 stages)
   T rfa, oma, inv_rho_g, inv_rg;      // rho_f alpha, 1 - alpha, 1 / rho_g, 1 / (rho_g + gamma)
 };
 
@@ -165,6 +166,31 @@ __device__ __forceinline__ double shfl_x1(double v) { return __shfl_xor_sync(0xf
 // full-row product: first half of the row with my half of the operand, second half with the partner's
 template <typename T, int H> __device__ __forceinline__ T dot2(const T (&a)[H], const T (&x)[H], const T (&b)[H], const T (&y)[H]) {
   return dotv<H>(a, x) + dotv<H>(b, y);
+}
+
+// ---- the same half rows from the STAGE-MINOR global scratch of the chain-resident variants (XG): element e of a row lives at
+// row + (e / V) cs + e % V with V = 16 / sizeof(T) elements per 16-byte chunk and cs the chunk stride (all stages of a problem side by side), so
+// that the lanes of a warp — consecutive stages — read consecutive 16-byte chunks: a warp-wide load is two contiguous runs (one per half)
+// instead of 32 scattered half rows (measured: the scattered form ran at one 32-byte sector per cycle and made the stage-parallel phases
+// 75 % of an iteration).
+template <int NC> __device__ __forceinline__ void ld_half_g(const float* __restrict__ row, const HalfOff& o, float (&r)[NC / 2], int cs) {
+  constexpr int H = NC / 2;
+  if constexpr (NC == 6) { const float2 v = *reinterpret_cast<const float2*>(row + (o.pair >> 2) * cs); r[0] = v.x; r[1] = v.y; r[2] = row[o.single]; }
+  else if constexpr (H % 4 == 0) {
+#pragma unroll
+    for (int c = 0; c < H / 4; ++c) { const float4 v = *reinterpret_cast<const float4*>(row + ((o.pair >> 2) + c) * cs); r[4 * c] = v.x; r[4 * c + 1] = v.y; r[4 * c + 2] = v.z; r[4 * c + 3] = v.w; }
+  } else {
+#pragma unroll
+    for (int c = 0; c < H / 2; ++c) { const int e = o.pair + 2 * c; const float2 v = *reinterpret_cast<const float2*>(row + (e >> 2) * cs + (e & 3)); r[2 * c] = v.x; r[2 * c + 1] = v.y; }
+  }
+}
+template <int NC> __device__ __forceinline__ void ld_half_g(const double* __restrict__ row, const HalfOff& o, double (&r)[NC / 2], int cs) {
+  constexpr int H = NC / 2;
+  if constexpr (NC == 6) { const double2 v = *reinterpret_cast<const double2*>(row + (o.pair >> 1) * cs); r[0] = v.x; r[1] = v.y; r[2] = row[(o.single >> 1) * cs + (o.single & 1)]; }
+  else {
+#pragma unroll
+    for (int c = 0; c < H / 2; ++c) { const double2 v = *reinterpret_cast<const double2*>(row + ((o.pair >> 1) + c) * cs); r[2 * c] = v.x; r[2 * c + 1] = v.y; }
+  }
 }
 
 // ---- x~ = S^{-1} eta on the scaled variables (tmpc_factor2.cuh): E1A + E1B hold eta~ on entry, E1A holds w on exit, E0
@@ -455,12 +481,17 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   T* nbp = sm + bn;
   if constexpr (CL) { if (cross) { unsigned long long ga; asm volatile("mapa.u64 %0, %1, %2;" : "=l"(ga) : "l"((unsigned long long)(sm + bn)), "r"((unsigned)(crank ^ 1))); nbp = reinterpret_cast<T*>(ga); } }
   // the blocks the item lanes read: X_t, A~^-_t (my record) and A~^+_t (the next record) — shared memory, or global memory for XG
-  const size_t gst = valid ? (size_t)p * T_ + t : 0, gsn = valid ? (size_t)p * T_ + (t < N ? t + 1 : 0) : 0;
-  const T* Xb = XG ? a.Sinv + gst * nn : sm + b + RC::SINV;
-  const int arows = 2 * nx + (d.g_sel ? 0 : ng);        // rows of a stage in atil: A~^-, A~^+, G~ (dense G only)
-  const T* AMb = XG ? A.atil + gst * (arows * n) : sm + b + RC::AM;
-  const T* APn = XG ? A.atil + gsn * (arows * n) + nx * n : nbp + RC::AP;
-  const T* Gb = XG ? A.atil + gst * (arows * n) + 2 * nx * n : sm + b + RC::G;
+  // XG: rows of X, A~^-, A~^+, G~ in that order, row r of stage t at gp + r RS + t V, its 16-byte chunks CS apart (atil_kernel)
+  constexpr int VV = RC::V, CCH = (NC + VV - 1) / VV;
+  const int CS = XG ? A.tpad * VV : VV, RS = XG ? CCH * CS : n;
+  const int arows = n + 2 * nx + (d.g_sel ? 0 : ng);
+  const T* gp = XG ? A.atil + (valid ? (size_t)p * arows * RS : 0) : nullptr;
+  const int tn = valid ? (t < N ? t + 1 : 0) : 0, tv = valid ? t : 0;
+  const T* Xb = XG ? gp + tv * VV : sm + b + RC::SINV;
+  const T* AMb = XG ? gp + (size_t)n * RS + tv * VV : sm + b + RC::AM;
+  const T* APn = XG ? gp + (size_t)(n + nx) * RS + tn * VV : nbp + RC::AP;
+  const T* Gb = XG ? gp + (size_t)(n + 2 * nx) * RS + tv * VV : sm + b + RC::G;
+  auto ldh = [&](const T* row, const HalfOff& o, T (&r)[H]) { if constexpr (XG) ld_half_g<NC>(row, o, r, CS); else ld_half<NC>(row, o, r); };
 
   if (a.kkt_only) {                                      // xt <- S^{-1} eta : eta~ = X eta, solve, x = X' y
     T eo[H], er[H];
@@ -471,7 +502,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
     if (valid) {
       T acc[H];
 #pragma unroll
-      for (int s = 0; s < H; ++s) { T f[H], f2[H]; const T* row = Xb + slot_col<NC>(h, s) * n; ld_half<NC>(row, mine, f); ld_half<NC>(row, other, f2); acc[s] = dot2<T, H>(f, eo, f2, er); }
+      for (int s = 0; s < H; ++s) { T f[H], f2[H]; const T* row = Xb + slot_col<NC>(h, s) * RS; ldh(row, mine, f); ldh(row, other, f2); acc[s] = dot2<T, H>(f, eo, f2, er); }
       st_half<NC>(sm + b + RC::E1A, mine, acc);
     }
     bar_arrive(1, nt);
@@ -482,9 +513,9 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
 #pragma unroll
       for (int s = 0; s < H; ++s) xt[s] = T(0);
 #pragma unroll
-      for (int jj = 0; jj < H; ++jj) { T mk[H]; ld_half<NC>(Xb + slot_col<NC>(h, jj) * n, mine, mk); axpy_half<H>(xt, mk, yo[jj]); }
+      for (int jj = 0; jj < H; ++jj) { T mk[H]; ldh(Xb + slot_col<NC>(h, jj) * RS, mine, mk); axpy_half<H>(xt, mk, yo[jj]); }
 #pragma unroll
-      for (int jj = 0; jj < H; ++jj) { T mk[H]; ld_half<NC>(Xb + slot_col<NC>(1 - h, jj) * n, mine, mk); axpy_half<H>(xt, mk, yr[jj]); }
+      for (int jj = 0; jj < H; ++jj) { T mk[H]; ldh(Xb + slot_col<NC>(1 - h, jj) * RS, mine, mk); axpy_half<H>(xt, mk, yr[jj]); }
 #pragma unroll
       for (int s = 0; s < H; ++s) a.xi[(size_t)p * nz + t * n + slot_col<NC>(h, s)] = xt[s];
     }
@@ -579,8 +610,8 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
 #pragma unroll
       for (int s = 0; s < H; ++s) {                    // my rows of X_t: my half first, then the partner's
         T f[H], f2[H];
-        const T* row = Xb + slot_col<NC>(h, s) * n;
-        ld_half<NC>(row, mine, f); ld_half<NC>(row, other, f2);
+        const T* row = Xb + slot_col<NC>(h, s) * RS;
+        ldh(row, mine, f); ldh(row, other, f2);
         acc[s] = dot2<T, H>(f, dn, f2, dr);
         accb[s] = T(0);
       }
@@ -588,20 +619,20 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
       for (int s = 0; s < KA; ++s) {                   // my columns of A~^-_t (my record) and A~^+_t (next record), rows of my block half / the partner's
         T mk[H];
         if (s < nk) {
-          ld_half<NC>(AMb + (k0 + s) * n, mine, mk); axpy_half<H>(acc, mk, ro[s]);
-          ld_half<NC>(APn + (k0 + s) * n, mine, mk); axpy_half<H>(accb, mk, ro[s]);
+          ldh(AMb + (k0 + s) * RS, mine, mk); axpy_half<H>(acc, mk, ro[s]);
+          ldh(APn + (k0 + s) * RS, mine, mk); axpy_half<H>(accb, mk, ro[s]);
         }
         if (s < nkp) {
-          ld_half<NC>(AMb + (k0p + s) * n, mine, mk); axpy_half<H>(acc, mk, rr[s]);
-          ld_half<NC>(APn + (k0p + s) * n, mine, mk); axpy_half<H>(accb, mk, rr[s]);
+          ldh(AMb + (k0p + s) * RS, mine, mk); axpy_half<H>(acc, mk, rr[s]);
+          ldh(APn + (k0p + s) * RS, mine, mk); axpy_half<H>(accb, mk, rr[s]);
         }
       }
       if (!d.g_sel) {
 #pragma unroll
         for (int s = 0; s < H; ++s) {
           T mk[H];
-          if (2 * s + h < ng) { ld_half<NC>(Gb + (2 * s + h) * n, mine, mk); axpy_half<H>(acc, mk, sg[s]); }
-          if (2 * s + 1 - h < ng) { ld_half<NC>(Gb + (2 * s + 1 - h) * n, mine, mk); axpy_half<H>(acc, mk, sgr[s]); }
+          if (2 * s + h < ng) { ldh(Gb + (2 * s + h) * RS, mine, mk); axpy_half<H>(acc, mk, sg[s]); }
+          if (2 * s + 1 - h < ng) { ldh(Gb + (2 * s + 1 - h) * RS, mine, mk); axpy_half<H>(acc, mk, sgr[s]); }
         }
       }
       st_half<NC>(sm + b + RC::E1A, mine, acc);
@@ -625,9 +656,9 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
 #pragma unroll
       for (int s = 0; s < H; ++s) xt[s] = T(0);
 #pragma unroll
-      for (int jj = 0; jj < H; ++jj) { T mk[H]; ld_half<NC>(Xb + slot_col<NC>(h, jj) * n, mine, mk); axpy_half<H>(xt, mk, yo[jj]); }       // rows of my half
+      for (int jj = 0; jj < H; ++jj) { T mk[H]; ldh(Xb + slot_col<NC>(h, jj) * RS, mine, mk); axpy_half<H>(xt, mk, yo[jj]); }       // rows of my half
 #pragma unroll
-      for (int jj = 0; jj < H; ++jj) { T mk[H]; ld_half<NC>(Xb + slot_col<NC>(1 - h, jj) * n, mine, mk); axpy_half<H>(xt, mk, yr[jj]); }   // rows of the partner's half
+      for (int jj = 0; jj < H; ++jj) { T mk[H]; ldh(Xb + slot_col<NC>(1 - h, jj) * RS, mine, mk); axpy_half<H>(xt, mk, yr[jj]); }   // rows of the partner's half
       if (nk > 0) {
         T y2o[H], y2r[H];
         ld_half<NC>(nbp + RC::E0, mine, y2o); ld_half<NC>(nbp + RC::E0, other, y2r);
@@ -635,9 +666,9 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
         for (int s = 0; s < KA; ++s) if (s < nk) {
           const int k = k0 + s;
           T f[H], f2[H];
-          ld_half<NC>(AMb + k * n, mine, f); ld_half<NC>(AMb + k * n, other, f2);
+          ldh(AMb + k * RS, mine, f); ldh(AMb + k * RS, other, f2);
           T zt = dot2<T, H>(f, yo, f2, yr);
-          ld_half<NC>(APn + k * n, mine, f); ld_half<NC>(APn + k * n, other, f2);
+          ldh(APn + k * RS, mine, f); ldh(APn + k * RS, other, f2);
           zt += dot2<T, H>(f, y2o, f2, y2r);
           yf[s] += rfa * (zt - cv[s]);
         }
@@ -646,7 +677,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
       for (int s = 0; s < H; ++s) {
         if (qf[s] & Q_VALID) {
           T ztg = xt[s];
-          if (!d.g_sel) { const T* row = Gb + (int)(qf[s] >> Q_ROW_SH) * n; T f[H], f2[H]; ld_half<NC>(row, mine, f); ld_half<NC>(row, other, f2); ztg = dot2<T, H>(f, yo, f2, yr); }
+          if (!d.g_sel) { const T* row = Gb + (int)(qf[s] >> Q_ROW_SH) * RS; T f[H], f2[H]; ldh(row, mine, f); ldh(row, other, f2); ztg = dot2<T, H>(f, yo, f2, yr); }
           const T zh = a.prm.alpha * ztg + A.oma * zg[s];
           const T v = zh + yg[s] * inv_rho_g;
           T z, sl;
@@ -678,17 +709,30 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   if constexpr (CL) cl_sync();
 }
 
-// ---- XG: the constraint blocks in the scaled variables, once per launch of the solve: row k of stage t of
-//   rows [0, nx): A~^-_t = A^-_t X_t' (zero for t = N);  rows [nx, 2 nx): A~^+_{t-1} = A^+_{t-1} X_t' (A_init = [I 0] for t = 0);
-//   rows [2 nx, 2 nx + ng): G~_t = G_t X_t' (dense G only),
-// M~[k][j] = sum_{l <= j} M[k][l] X_t[j][l] (X_t lower triangular).  One thread per row; n <= 16.
+// ---- XG: what the item lanes read, once per launch of the solve, in the STAGE-MINOR layout of ld_half_g: per problem the rows
+//   [0, n)                 X_t                                   (copied from the factor)
+//   [n, n + nx)            A~^-_t = A^-_t X_t'                    (zero for t = N)
+//   [n + nx, n + 2 nx)     A~^+_{t-1} = A^+_{t-1} X_t'            (A_init = [I 0] for t = 0)
+//   [n + 2 nx, .. + ng)    G~_t = G_t X_t'                        (dense G only)
+// with M~[k][j] = sum_{l <= j} M[k][l] X_t[j][l] (X_t lower triangular); element j of row r of stage t goes to
+// (p rows + r) RS + (j / V) CS + t V + j % V, CS = tpad V, RS = ceil(n / V) CS.  One thread per (problem, row, stage), stage fastest; n <= 16.
 template <typename T>
-__global__ void __launch_bounds__(128) atil_kernel(const AdmmArgs<T> a, T* __restrict__ atil) {
+__global__ void __launch_bounds__(128) atil_kernel(const AdmmArgs<T> a, T* __restrict__ atil, int tpad, int rows) {   // rows = n for kkt_only (X only)
   const Dims& d = a.d;
-  const int n = d.n, nx = d.nx, T_ = d.T, N = d.N, rows = 2 * nx + (d.g_sel ? 0 : d.ng);
+  constexpr int V = 16 / (int)sizeof(T);
+  const int n = d.n, nx = d.nx, T_ = d.T, N = d.N;
+  const int CS = tpad * V, RS = (n + V - 1) / V * CS;
+  const int rows_all = n + 2 * nx + (d.g_sel ? 0 : d.ng);
   const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (e >= (long long)d.B * T_ * rows) return;
-  const int k2 = (int)(e % rows), t = (int)((e / rows) % T_), p = (int)(e / ((long long)rows * T_));
+  if (e >= (long long)d.B * rows * T_) return;
+  const int t = (int)(e % T_), r = (int)((e / T_) % rows), p = (int)(e / ((long long)rows * T_));
+  const T* X = a.Sinv + ((size_t)p * T_ + t) * n * n;
+  T* out = atil + ((size_t)p * rows_all + r) * RS + (size_t)t * V;
+  if (r < n) {                                         // a row of X_t
+    for (int j = 0; j < n; ++j) out[(j / V) * CS + j % V] = X[r * n + j];
+    return;
+  }
+  const int k2 = r - n;
   const bool plus = k2 >= nx && k2 < 2 * nx, isg = k2 >= 2 * nx; const int k = isg ? k2 - 2 * nx : (plus ? k2 - nx : k2);
   T v[16];
 #pragma unroll
@@ -701,13 +745,11 @@ __global__ void __launch_bounds__(128) atil_kernel(const AdmmArgs<T> a, T* __res
     }
     v[l] = s;
   }
-  const T* X = a.Sinv + ((size_t)p * T_ + t) * n * n;
-  T* out = atil + (size_t)e * n;
   for (int j = 0; j < n; ++j) {
     T acc = T(0);
 #pragma unroll
     for (int l = 0; l < 16; ++l) if (l <= j) acc += v[l] * X[j * n + l];
-    out[j] = acc;
+    out[(j / V) * CS + j % V] = acc;
   }
 }
 

@@ -55,7 +55,8 @@ Layout make_layout(const tmpc_config& c) {
   Layout L; size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
   L.Lam = take(B * d.T * nn * es); L.Sinv = take(B * d.T * nn * es); L.eta = take(B * d.nz * es);
-  L.atil = take(plan_xg(c) ? B * d.T * (2 * (size_t)d.nx + (d.g_sel ? 0 : d.ng)) * d.n * es : 0);       // A~ per stage (atil_kernel), only for the handles whose plan reads it
+  // X, A~ and G~ rows in the stage-minor layout of atil_kernel (16-byte chunks, horizon padded to 8 stages), only for the handles whose plan reads it
+  L.atil = take(plan_xg(c) ? B * ((size_t)d.n + 2 * d.nx + (d.g_sel ? 0 : d.ng)) * ((d.n * es + 15) / 16) * (size_t)((d.T + 7) / 8 * 8) * 16 : 0);
   L.fstatus = take(B * sizeof(int32_t));       // per-problem TMPC_ST_PIVOT word of the last tmpc_factor
   // f1 (tmpc_admm_solve_adaptive): per-problem rho_bar, eq. 4 scales, residuals / objective when the caller passes no info, flags, counters
   L.ad_rho = take(B * es); L.ad_np = take(B * es); L.ad_nd = take(B * es); L.ad_rp = take(B * es); L.ad_rd = take(B * es); L.ad_obj = take(B * es);
@@ -244,9 +245,10 @@ FastPlan fast_plan(const Dims& d) {
     // long horizons: only the chain's share of a record stays in shared memory (Rec3<.., XG>), one problem per CTA, two item lanes per stage
     const size_t sx = d.n == 8 ? admm3_smem_bytes<T, 8, 6, true>(d, 1) : d.n == 6 ? admm3_smem_bytes<T, 6, 4, true>(d, 1) : admm3_smem_bytes<T, 12, 8, true>(d, 1);
     const int ntx = 32 + (2 * d.T + 31) / 32 * 32;
-    // ... and with the chain's share only when that no longer fits one SM, or when the batch leaves half of the SMs idle anyway
+    // ... and with the chain's share only when that no longer fits one SM (one CTA per problem is faster where it fits: 37 against 50 us per
+    // iteration at (64,160,8,4) fp64 once the global operands are laid out stage-minor)
     const bool one_fits = sx <= kMaxSmem && ntx <= 1024;
-    if (cl_shape && (!one_fits || 2 * d.B <= sm_count())) {
+    if (cl_shape && !one_fits) {
       const size_t sc = admm3_cl_smem_bytes<T, 12, 8, true>(d);
       if (sc <= kMaxSmem) { f.ok = true; f.xg = true; f.cl = true; f.nt = ntc; f.ctas_per_sm = 1; f.smem = sc; return f; }
     }
@@ -278,12 +280,12 @@ tmpc_status launch_admm3_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan&
   const unsigned grid = (unsigned)((h->d.B + PG - 1) / PG);
   Admm3Args<T> A; A.a = a; A.atil = nullptr;
   if constexpr (CL) A.pl = admm3_cl_plan<T, NC, NX, XG>(h->d); else A.pl = admm3_plan<T, NC, NX, XG>(h->d, PG);
+  A.tpad = (h->d.T + 7) / 8 * 8;
   if constexpr (XG) {
     T* atil = (T*)(h->ws + h->lay.atil); A.atil = atil;
-    if (!a.kkt_only) {
-      const long long rows = (long long)h->d.B * h->d.T * (2 * h->d.nx + (h->d.g_sel ? 0 : h->d.ng));
-      atil_kernel<T><<<(unsigned)((rows + 127) / 128), 128, 0, h->stream>>>(a, atil); h->launches++;
-    }
+    const int rows = a.kkt_only ? h->d.n : h->d.n + 2 * h->d.nx + (h->d.g_sel ? 0 : h->d.ng);      // tmpc_kkt_solve needs X only
+    const long long work = (long long)h->d.B * rows * h->d.T;
+    atil_kernel<T><<<(unsigned)((work + 127) / 128), 128, 0, h->stream>>>(a, atil, A.tpad, rows); h->launches++;
   }
   A.rfa = a.prm.rho_f * a.prm.alpha; A.oma = T(1) - a.prm.alpha; A.inv_rho_g = T(1) / a.prm.rho_g; A.inv_rg = T(1) / (a.prm.rho_g + a.prm.gamma);
   if constexpr (CL) {                                   // two CTAs per problem, launched as a cluster
