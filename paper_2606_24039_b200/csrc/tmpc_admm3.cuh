@@ -34,8 +34,8 @@ namespace tmpc {
 //   LAM -B_t [n][n]  SINV X_t = L_t^{-1} [n][n]
 //   G   G~_t = G_t X_t' [ng][n]      (dense G only; s_t = rho_g z_g - y_g lives in the registers of the row owners)
 // XG ("X and A~ in global memory", long horizons): the record keeps only what the CHAIN warp reads — y, eta~ / w and -B_t — and the item
-// lanes take X_t, A~^-_t, A~^+_t from global memory (X from the factor in the workspace, A~ from the scratch atil_kernel fills), where
-// they are L2 hits: the chain is the latency-bound part, the item phases are throughput-bound and tolerate the longer loads.
+// lanes take X_t, A~^-_t, A~^+_t (G~_t) from global memory, from the stage-minor scratch atil_kernel fills (ld_half_g), where they are L2
+// hits: the chain is the latency-bound part, the item phases are throughput-bound and tolerate the longer loads.
 template <typename T, int NC, int NX, bool XG = false>
 struct Rec3 {
   static constexpr int V = 16 / (int)sizeof(T);
