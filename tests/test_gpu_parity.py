@@ -115,6 +115,23 @@ def test_kkt_solve_matches_oracle_cholesky(dtype):
         s.close()
 
 
+def test_kkt_solve_long_horizon_variants_fp64():
+    """tmpc_kkt_solve (one S^{-1} eta, no ADMM state) through the long-horizon variants of the resident kernel: cluster pair with full records
+    (N = 80), one CTA with the chain's share (N = 160; and the (6, 4) block with dense G at N = 400), cluster pair with the chain's share (N = 320)."""
+    from paper_2606_24039_b200.solver import Solver
+    cases = [W.linear_rl(B=2, N=80, u_max=1.0), W.linear_rl(B=2, N=160, u_max=1.0), W.linear_rl(B=2, N=320, u_max=1.0),
+             W.random_ltv(31, 2, 400, 4, 2, [4], [0, 1, 0], dense_g_rows=2, q_scale=0.3)]
+    for w in cases:
+        s = Solver(w, dtype="f64")
+        s.factor()
+        eta = np.random.default_rng(1).standard_normal((w.B, w.T, w.n))
+        xt = s.kkt_solve(s._up(eta)).cpu().double().numpy()
+        cfg = O.make_cfg(w)
+        ref = np.stack([O.solve_S(w, cfg, eta[b].ravel(), b).reshape(w.T, w.n) for b in range(w.B)])
+        assert rel_err(xt, ref) <= 1e-9, (w.name, rel_err(xt, ref))
+        s.close()
+
+
 # ----------------------------------------------------------------------------------------------- a10 backward
 def _backward_case(dtype, soft_bound, rho_bar, iters, B=6, N=20):
     """Oracle forward output is fed to BOTH sides (reading A-20) so the classification cannot diverge by rounding."""
