@@ -305,6 +305,23 @@ def srb_linearize(w, cfg, xbar):
     return Am, Ap, b
 
 
+def sqp_linesearch_srb(w, cfg, max_sqp=10, admm_iters=50, eps_c=1e-3, n_alpha=8, eta=0.4, xbar0=None):
+    """f2 for the SRB model on every problem; same returns as sqp_linesearch_bicycle."""
+    n, T, nz, mf, mg = _dims(w)
+    assert lib().orc_sizeof_sqpopt() == C.sizeof(SqpOpt)
+    op = SqpOpt(max_sqp, admm_iters, n_alpha, 0, eps_c, eta)
+    st = new_state(w); st["x"] = _c(w.xbar0 if xbar0 is None else xbar0).copy()
+    info = np.zeros((w.B, 5)); log = np.zeros((w.B, max_sqp, 10))
+    D, E = _c(w.D[0]), _c(w.E[0])
+    fn = lib().orc_sqp_ls_srb
+    fn.argtypes = [C.c_void_p] * 15
+    rc = 0
+    for b in range(w.B):
+        rc |= fn(C.byref(cfg), C.byref(op), _p(D), _p(E), _p(_c(w.q[b])), _p(_c(w.x_init[b])), _p(_c(w.lo[b])), _p(_c(w.hi[b])), _p(st["x"][b]),
+                 _p(st["zg"][b]), _p(st["yf"][b]), _p(st["yg"][b]), _p(st["xi"][b]), _p(info[b]), _p(log[b]))
+    return st, info, log, rc
+
+
 def sqp_srb(w, cfg, n_sqp=None, iters=None):
     """O-4 for the SRB model on every problem (selection rows with the workload's constant bounds).  Returns (state with x = final xbar, info, rc)."""
     n_sqp = w.sqp_iters if n_sqp is None else n_sqp

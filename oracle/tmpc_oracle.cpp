@@ -18,7 +18,7 @@
 //   O-4  SQP        fixed-count full-step driver around O-1..O-3 with the bicycle model linearised
 //                   by eq. 36-38.
 //   f1   adaptive   Alg. 3 with the adaptive step size of eq. 17 and the termination test eq. 4 (admm_adaptive).
-//   f2   SQP + linesearch   App. D l1-merit backtracking and the convergence test eq. 18 (sqp_ls_bicycle).
+//   f2   SQP + linesearch   App. D l1-merit backtracking and the convergence test eq. 18 (sqp_ls_bicycle; sqp_ls_srb for the second model).
 //   f3   SRB model  single-rigid-body humanoid dynamics (eq. 68-69) + RK4 and its eq. 36-37 blocks by forward-mode dual numbers.
 //   O-5  backward   the definition: dense active-set KKT system eq. 62 / 65 solved by
 //                   Gaussian elimination with partial pivoting; dL/dq = -eta_x, dL/dx_init = +eta_f[0:nx].
@@ -566,6 +566,80 @@ int sqp_ls_bicycle(const Cfg& cf_in, const SqpOpt& op, const double* D, const do
   return fail;
 }
 
+// ---- f2 for the SRB humanoid model (second built-in model): the same App. D linesearch and eq. 18 test as sqp_ls_bicycle, with
+//   f(x~) = (x_0 - x_init ; Phi(x_k, u_k) - x_{k+1}) (RK4 of eq. 68), g(x~) = the selected components of v_t (+ xi on soft rows) against the
+//   caller's constant bounds (eq. 70d).  Kept apart from the bicycle routine so that its pinned arithmetic is not touched.
+double merit_parts_srb(const Cfg& c, const Band& P, const vec& q, const double* x_init, const double* x, const double* xi, const double* lo,
+                       const double* hi, double* cost_out, double* finf_out, double* ginf_out) {
+  const int N = c.N, T = N + 1, n = 18, nx = 12, ng = c.ng, nz = T * n;
+  vec xv(x, x + nz), Px(nz); band_mul(P, xv, Px);
+  double cost = 0; for (int i = 0; i < nz; ++i) cost += 0.5 * x[i] * Px[i] + q[i] * x[i];
+  double c1 = 0, finf = 0, ginf = 0, phi[12];
+  for (int i = 0; i < nx; ++i) { double r = x[i] - x_init[i]; c1 += std::fabs(r); finf = std::max(finf, std::fabs(r)); }
+  for (int t = 0; t < N; ++t) {
+    const double* vk = x + (size_t)t * n; const double* vk1 = vk + n;
+    srb_rk4<double>(c.model_params, c.dt, vk, vk + 12, phi);
+    for (int i = 0; i < nx; ++i) { const double f = phi[i] - vk1[i]; c1 += std::fabs(f); finf = std::max(finf, std::fabs(f)); }
+  }
+  for (int t = 0; t < T; ++t) for (int r = 0; r < ng; ++r) {
+    const int e = t * ng + r; double g = x[t * n + c.g_col[r]];
+    if (c.soft[r]) { g += xi[e]; cost += c.lam * std::fabs(xi[e]) + 0.5 * c.gamma * xi[e] * xi[e]; }
+    double v = std::max(0.0, g - hi[e]) + std::max(0.0, lo[e] - g);
+    c1 += v; ginf = std::max(ginf, v);
+  }
+  *cost_out = cost; if (finf_out) *finf_out = finf; if (ginf_out) *ginf_out = ginf;
+  return c1;
+}
+
+// log_out as in sqp_ls_bicycle
+int sqp_ls_srb(const Cfg& cf_in, const SqpOpt& op, const double* D, const double* E, const double* q_, const double* x_init, const double* lo, const double* hi,
+               double* xbar, double* zg, double* yf, double* yg, double* xi, double* info_out, double* log_out) {
+  Cfg c = cf_in; c.g_sel = 1; c.zg_given = 0;
+  const int N = c.N, T = N + 1, n = 18, nx = 12, ng = c.ng, nz = T * n, mf = nx + N * nx, mg = T * ng;
+  vec Am((size_t)N * nx * n), Ap((size_t)N * nx * n), b((size_t)N * nx), q(q_, q_ + nz);
+  vec xs(nz), zs(mg), yfs(mf), ygs(mg), xis(mg), xc(nz), xic(mg), g(nz), Px(nz);
+  int fail = 0, it = 0, converged = 0;
+  double stat = 0, finf = 0, ginf = 0;
+  for (it = 0; it < op.max_sqp && !converged; ) {
+    srb_linearize(c, xbar, Am.data(), Ap.data(), b.data());
+    QP p = assemble(c, D, E, q.data(), Am.data(), Ap.data(), b.data(), x_init, nullptr, lo, hi);
+    std::copy(xbar, xbar + nz, xs.begin()); std::copy(yf, yf + mf, yfs.begin()); std::copy(yg, yg + mg, ygs.begin());
+    Info ai = admm(c, p, xs.data(), zs.data(), yfs.data(), ygs.data(), xis.data(), op.admm_iters);
+    if (!(ai.min_pivot > 0)) fail = 1;
+    double cost0, c1 = merit_parts_srb(c, p.P, q, x_init, xbar, xi, lo, hi, &cost0, nullptr, nullptr);
+    vec xb(xbar, xbar + nz); band_mul(p.P, xb, Px);
+    double dl = 0; for (int i = 0; i < nz; ++i) dl += (Px[i] + q[i]) * (xs[i] - xbar[i]);
+    for (int e = 0; e < mg; ++e) if (c.soft[e % ng]) { double dxi = xis[e] - xi[e]; double sg = xi[e] > 0 ? 1.0 : (xi[e] < 0 ? -1.0 : (dxi > 0 ? 1.0 : (dxi < 0 ? -1.0 : 0.0))); dl += (c.lam * sg + c.gamma * xi[e]) * dxi; }
+    const double mu = std::max(0.0, dl / (0.5 * std::max(c1, op.eps_c))), phi0 = cost0 + mu * c1, Dmu = dl - mu * c1;
+    double alpha = 0, best_phi = std::numeric_limits<double>::infinity(), best_alpha = 1.0, phi_a = 0; int accepted = 0;
+    for (int j = 0; j < op.n_alpha && !accepted; ++j) {
+      const double a = std::ldexp(1.0, -j);
+      for (int i = 0; i < nz; ++i) xc[i] = xbar[i] + a * (xs[i] - xbar[i]);
+      for (int e = 0; e < mg; ++e) xic[e] = xi[e] + a * (xis[e] - xi[e]);
+      double costa, c1a = merit_parts_srb(c, p.P, q, x_init, xc.data(), xic.data(), lo, hi, &costa, nullptr, nullptr);
+      const double phi = costa + mu * c1a;
+      if (phi < best_phi) { best_phi = phi; best_alpha = a; }
+      if (phi <= phi0 + op.eta * a * Dmu) { alpha = a; phi_a = phi; accepted = 1; }
+    }
+    if (!accepted) { alpha = best_alpha; phi_a = best_phi; }
+    for (int i = 0; i < nz; ++i) xbar[i] += alpha * (xs[i] - xbar[i]);
+    for (int e = 0; e < mg; ++e) { xi[e] += alpha * (xis[e] - xi[e]); yg[e] += alpha * (ygs[e] - yg[e]); zg[e] = zs[e]; }
+    for (int e = 0; e < mf; ++e) yf[e] += alpha * (yfs[e] - yf[e]);
+    ++it;
+    srb_linearize(c, xbar, Am.data(), Ap.data(), b.data());
+    QP pn = assemble(c, D, E, q.data(), Am.data(), Ap.data(), b.data(), x_init, nullptr, lo, hi);
+    vec xn(xbar, xbar + nz), yfv(yf, yf + mf), ygv(yg, yg + mg); band_mul(pn.P, xn, Px);
+    for (int i = 0; i < nz; ++i) g[i] = Px[i] + q[i];
+    pn.C.mulT_add(yfv, g); pn.G.mulT_add(ygv, g);
+    stat = 0; for (int i = 0; i < nz; ++i) stat = std::max(stat, std::fabs(g[i]));
+    double cdummy; merit_parts_srb(c, pn.P, q, x_init, xbar, xi, lo, hi, &cdummy, &finf, &ginf);
+    converged = stat <= op.eps_c && finf <= op.eps_c && ginf <= op.eps_c;
+    if (log_out) { double* l = log_out + 10 * (it - 1); l[0] = alpha; l[1] = mu; l[2] = phi0; l[3] = phi_a; l[4] = c1; l[5] = dl; l[6] = accepted; l[7] = stat; l[8] = finf; l[9] = ginf; }
+  }
+  info_out[0] = it; info_out[1] = converged; info_out[2] = stat; info_out[3] = finf; info_out[4] = ginf;
+  return fail;
+}
+
 }  // namespace
 
 extern "C" {
@@ -711,6 +785,11 @@ int orc_sqp_srb(const Cfg* cf, const double* D, const double* E, const double* q
     fail |= orc_admm(&c, D, E, q, Am.data(), Ap.data(), b.data(), x_init, nullptr, lo, hi, xbar, zg, yf, yg, xi, K, info_out);
   }
   return fail;
+}
+
+int orc_sqp_ls_srb(const Cfg* cf, const SqpOpt* op, const double* D, const double* E, const double* q, const double* x_init, const double* lo, const double* hi,
+                   double* xbar, double* zg, double* yf, double* yg, double* xi, double* info_out, double* log_out) {
+  return sqp_ls_srb(*cf, *op, D, E, q, x_init, lo, hi, xbar, zg, yf, yg, xi, info_out, log_out);
 }
 
 int orc_sizeof_cfg() { return (int)sizeof(Cfg); }

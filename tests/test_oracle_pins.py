@@ -801,3 +801,84 @@ def test_srb_sqp_driver_reaches_the_reference():
         s0 = O.new_state(wq); s0["x"] = w.xbar0[b:b + 1].copy()
         s, _, _ = O.admm(wq, O.make_cfg(wq), iters=40, state=s0)
         assert np.abs(s["x"][0] - st1["x"][b]).max() < 1e-12
+
+
+def _srb_instance(B=1, N=10, seed=3):
+    """The balancing OCP with a perturbed start and the two f_y rows (the ones that bind) made soft, so that the slack terms of the merit function act."""
+    w = W.srb_humanoid(B=B, N=N)
+    w.soft = [0, 1, 0, 0, 1, 0]
+    w.lam, w.gamma = 0.01, 0.1
+    rng = np.random.default_rng(seed)
+    x0 = w.xbar0.copy()
+    x0[:, :, :3] += 0.03 * rng.standard_normal(x0[:, :, :3].shape); x0[:, :, 3:6] += 0.1 * rng.standard_normal(x0[:, :, 3:6].shape)
+    x0[:, :, 6:12] += 0.2 * rng.standard_normal(x0[:, :, 6:12].shape)
+    return w, x0
+
+
+def _merit_parts_srb(w, cfg, b, P, q, x, xi, lo, hi):
+    """cost and c1 of App. D for the SRB model: f_k = Phi(x_k, u_k) - x_{k+1} with the pinned RK4 step, g = selected components (+ xi on soft rows)."""
+    soft = np.array(w.soft, dtype=bool)
+    xf = x.ravel()
+    cost = 0.5 * xf @ P @ xf + q @ xf + (w.lam * np.abs(xi[:, soft]) + 0.5 * w.gamma * xi[:, soft] ** 2).sum()
+    fk = np.stack([O.srb_step(cfg, x[t, :12], x[t, 12:]) - x[t + 1, :12] for t in range(w.N)])
+    f0 = x[0, :12] - w.x_init[b]
+    g = x[:, w.g_col] + np.where(soft, xi, 0.0)
+    viol = np.maximum(0.0, g - hi) + np.maximum(0.0, lo - g)
+    return cost, np.abs(f0).sum() + np.abs(fk).sum() + viol.sum(), max(np.abs(f0).max(), np.abs(fk).max()), viol.max()
+
+
+def test_sqp_linesearch_srb_steps_recomputed_in_numpy():
+    """f2 for the second model: every SQP iteration of one run of sqp_ls_srb retyped from App. D (merit, mu, D_mu, Armijo over alpha = 2^-j, fallback,
+    update) around the pinned pieces (srb_linearize, srb_step, Alg. 3), and eq. 18 with the Jacobians at the new iterate.  The run backtracks, uses
+    the soft row's slack and converges."""
+    import copy
+    w, x0 = _srb_instance()
+    cfg = O.make_cfg(w)
+    K, eps_c, nA, eta, nsqp = 2000, 1e-3, 8, 0.4, 25
+    st_all, info, log, rc = O.sqp_linesearch_srb(w, cfg, max_sqp=nsqp, admm_iters=K, eps_c=eps_c, n_alpha=nA, eta=eta, xbar0=x0)
+    assert rc == 0
+    soft = np.array(w.soft, dtype=bool)
+    cur = O.new_state(w); cur["x"] = x0.copy()
+    seen_backtrack = seen_slack = False
+    q = w.q[0].ravel(); lo, hi = w.lo[0], w.hi[0]
+    for it in range(int(info[0, 0])):
+        Am, Ap, bb = O.srb_linearize(w, cfg, cur["x"][0])
+        wq = copy.copy(w)
+        wq.Am, wq.Ap, wq.b, wq.model = Am[None], Ap[None], bb[None], 0
+        s0 = {k: v.copy() for k, v in cur.items()}
+        sol, _, _ = O.admm(wq, O.make_cfg(wq), iters=K, state=s0)
+        P, C, c, Gd = dense_PCG(wq, 0)
+        x, xi = cur["x"][0], cur["xi"][0]
+        dx, dxi = sol["x"][0] - x, sol["xi"][0] - xi
+        seen_slack |= bool((sol["xi"] != 0).any())
+        cost0, c1, _, _ = _merit_parts_srb(w, cfg, 0, P, q, x, xi, lo, hi)
+        sg = np.where(xi != 0, np.sign(xi), np.sign(dxi))
+        dl = (P @ x.ravel() + q) @ dx.ravel() + ((w.lam * sg + w.gamma * xi) * dxi)[:, soft].sum()
+        mu = max(0.0, dl / (0.5 * max(c1, eps_c)))
+        phi0, Dmu = cost0 + mu * c1, dl - mu * c1
+        phis = []
+        for j in range(nA):
+            a = 2.0 ** -j
+            ca, c1a, _, _ = _merit_parts_srb(w, cfg, 0, P, q, x + a * dx, xi + a * dxi, lo, hi)
+            phis.append(ca + mu * c1a)
+        ok = [j for j in range(nA) if phis[j] <= phi0 + eta * 2.0 ** -j * Dmu]
+        jstar = ok[0] if ok else int(np.argmin(phis))
+        alpha = 2.0 ** -jstar
+        seen_backtrack |= alpha < 1.0
+        assert log[0, it, 0] == alpha and bool(log[0, it, 6]) == bool(ok), (it, log[0, it], alpha)
+        assert abs(log[0, it, 1] - mu) <= 1e-8 * max(1, abs(mu)) and abs(log[0, it, 2] - phi0) <= 1e-9 * abs(phi0) and abs(log[0, it, 4] - c1) <= 1e-9 * max(1, c1)
+        for k in ("x", "xi", "yf", "yg"):
+            cur[k] = cur[k] + alpha * (sol[k] - cur[k])
+        cur["zg"] = sol["zg"]
+        Am, Ap, bb = O.srb_linearize(w, cfg, cur["x"][0])
+        wq.Am, wq.Ap, wq.b = Am[None], Ap[None], bb[None]
+        P, C, c, Gd = dense_PCG(wq, 0)
+        stat = np.abs(P @ cur["x"][0].ravel() + q + C.T @ cur["yf"][0] + Gd.T @ cur["yg"][0].ravel()).max()
+        _, _, finf, ginf = _merit_parts_srb(w, cfg, 0, P, q, cur["x"][0], cur["xi"][0], lo, hi)
+        for got, ref in ((log[0, it, 7], stat), (log[0, it, 8], finf), (log[0, it, 9], ginf)):
+            assert abs(got - ref) <= 1e-9 * max(1.0, abs(ref))
+        conv = stat <= eps_c and finf <= eps_c and ginf <= eps_c
+        assert conv == (it == int(info[0, 0]) - 1 and bool(info[0, 1]))
+    for k in ("x", "xi", "yf", "yg"):
+        assert np.abs(cur[k] - st_all[k]).max() <= 1e-10 * max(1.0, np.abs(st_all[k]).max()), k
+    assert info[0, 1] == 1 and seen_backtrack and seen_slack, (info[0], seen_backtrack, seen_slack)
