@@ -142,8 +142,9 @@ typedef struct {
  * iteration (as by tmpc_linearize).  Outputs (DEVICE, any may be NULL): SQP iterations per problem [B], eq. 18 met [B], the accepted alpha
  * of every iteration [B][max_sqp] and the eq. 18 quantities of the last test [B][3] (working dtype).  Like tmpc_admm_solve_adaptive the
  * call SYNCHRONISES once per iteration (count of live problems) and leaves the workspace factor unusable for a later tmpc_admm_solve.
- * TMPC_E_UNSUPPORTED for any model but TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT (the merit and eq. 18 kernels are written for it) and with cyclic
- * reduction. */
+ * Both built-in models (for TMPC_MODEL_SRB_HUMANOID_RK4 the equality residual of the merit function is Phi(x_k, u_k) - x_{k+1}, the inequality
+ * rows are the handle's selection rows with the caller's constant qp->lo, qp->hi, and stage_ref is not read); TMPC_E_UNSUPPORTED for
+ * TMPC_MODEL_NONE and with cyclic reduction. */
 tmpc_status tmpc_sqp_solve(tmpc_handle h, tmpc_qp* qp, tmpc_state* st, const void* stage_ref, const tmpc_sqp_opts* o, int32_t* iters_out,
                            int32_t* converged_out, void* alpha_log, void* kkt_out);
 /* a10 (Alg. 2, eq. 59-65): dL/dq [B][T][n] and dL/dx_init [B][nx] from dL/dx [B][T][n] (and dL/dxi [B][T][ng] or NULL)

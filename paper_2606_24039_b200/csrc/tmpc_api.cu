@@ -477,7 +477,8 @@ template <typename T>
 tmpc_status do_sqp(tmpc_ctx* h, tmpc_qp* qp, tmpc_state* st, const void* stage_ref, const tmpc_sqp_opts* o, int32_t* iters_out, int32_t* conv_out,
                    void* alpha_log, void* kkt_out) {
   const Dims& d = h->d; const Layout& L = h->lay; unsigned char* ws = h->ws;
-  if (h->cfg.model != TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT) return TMPC_E_UNSUPPORTED;
+  const int model = h->cfg.model;
+  if (model != TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT && model != TMPC_MODEL_SRB_HUMANOID_RK4) return TMPC_E_UNSUPPORTED;
   int32_t* active = (int32_t*)(ws + L.ad_active); int32_t* mask = (int32_t*)(ws + L.ad_mask);
   int32_t* iters = (int32_t*)(ws + L.ad_iters); int32_t* conv = (int32_t*)(ws + L.ad_conv); int32_t* count = (int32_t*)(ws + L.ad_count);
   const unsigned nb = (unsigned)((d.B + 255) / 256);
@@ -485,6 +486,7 @@ tmpc_status do_sqp(tmpc_ctx* h, tmpc_qp* qp, tmpc_state* st, const void* stage_r
   if (!cuda_ok()) return TMPC_E_CUDA;
   SqpArgs<T> a; memset(&a, 0, sizeof(a));
   a.d = d; a.qp = view<T>(qp); a.Lwb = h->cfg.wheelbase; a.dt = h->cfg.dt; a.gamma = h->cfg.slack_gamma; a.lam = h->cfg.slack_lambda; a.eps_c = o->eps_c; a.eta = o->eta;
+  for (int i = 0; i < 13; ++i) a.mp[i] = h->cfg.model_params[i];
   a.n_alpha = o->n_alpha; a.active = active; a.act_rw = active; a.iters = iters; a.converged = conv; a.n_active = count;
   a.ox = (const T*)(ws + L.ax); a.oxi = (const T*)(ws + L.axi); a.oyf = (const T*)(ws + L.ayf); a.oyg = (const T*)(ws + L.ayg);
   a.x = (T*)st->x; a.xi = (T*)st->xi; a.yf = (T*)st->yf; a.yg = (T*)st->yg; a.alpha_log = (T*)alpha_log; a.max_sqp = o->max_sqp; a.kkt = (T*)kkt_out;
@@ -512,7 +514,9 @@ tmpc_status do_sqp(tmpc_ctx* h, tmpc_qp* qp, tmpc_state* st, const void* stage_r
     h->cur_active = nullptr; h->cur_mask = nullptr;
     if (rc != TMPC_OK) break;
     a.it = it;
-    sqp_linesearch_kernel<T><<<d.B, 32 * (o->n_alpha + 1), 0, h->stream>>>(a); h->launches++;
+    if (model == TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT) sqp_linesearch_kernel<T, 1><<<d.B, 32 * (o->n_alpha + 1), 0, h->stream>>>(a);
+    else sqp_linesearch_kernel<T, 2><<<d.B, 32 * (o->n_alpha + 1), 0, h->stream>>>(a);
+    h->launches++;
     if (!cuda_ok()) rc = TMPC_E_CUDA;
   }
   h->cur_active = nullptr; h->cur_mask = nullptr;
@@ -666,8 +670,10 @@ tmpc_status tmpc_admm_solve_adaptive(tmpc_handle h, const tmpc_qp* qp, tmpc_stat
 
 tmpc_status tmpc_sqp_solve(tmpc_handle h, tmpc_qp* qp, tmpc_state* st, const void* stage_ref, const tmpc_sqp_opts* o, int32_t* iters_out,
                            int32_t* converged_out, void* alpha_log, void* kkt_out) {
-  if (!h || !qp || !st || !stage_ref || !o || !st->x || !st->zg || !st->yf || !st->yg || !st->xi) return TMPC_E_BADARG;
-  if (!qp->D || !qp->E || !qp->q || !qp->x_init || !qp->Am || !qp->Ap || !qp->b || !qp->G || !qp->lo || !qp->hi) return TMPC_E_BADARG;
+  if (!h || !qp || !st || !o || !st->x || !st->zg || !st->yf || !st->yg || !st->xi) return TMPC_E_BADARG;
+  const bool bicycle = h->cfg.model == TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT;      // the bicycle model reads stage_ref and writes dense G rows
+  if (bicycle && (!stage_ref || !qp->G)) return TMPC_E_BADARG;
+  if (!qp->D || !qp->E || !qp->q || !qp->x_init || !qp->Am || !qp->Ap || !qp->b || !qp->lo || !qp->hi) return TMPC_E_BADARG;
   if (o->max_sqp < 1 || o->admm_iters < 1 || o->n_alpha < 1 || o->n_alpha > SQP_MAX_ALPHA || !(o->eps_c > 0) || !(o->eta > 0 && o->eta < 1)) return TMPC_E_BADARG;
   if (h->cr) return TMPC_E_UNSUPPORTED;
   return h->cfg.dtype == TMPC_F32 ? do_sqp<float>(h, qp, st, stage_ref, o, iters_out, converged_out, alpha_log, kkt_out)

@@ -1,4 +1,5 @@
-// tmpc_sqp.cuh — f2: the SQP outer loop of Alg. 1 around the ADMM solve for the built-in bicycle model:
+// tmpc_sqp.cuh — f2: the SQP outer loop of Alg. 1 around the ADMM solve for the two built-in models (MODEL = 1: kinematic
+// bicycle, implicit midpoint, dense G rows; MODEL = 2: SRB humanoid, RK4, f_k = Phi(x_k, u_k) - x_{k+1}, selection rows with constant bounds):
 // l1-merit backtracking linesearch with the step-size candidates evaluated in parallel (App. D) and the
 // convergence test eq. 18.  Readings A-34..A-37 of DESIGN.md:
 //   x~ = (x, xi);  l(x~) = 1/2 x'Px + q'x + sum_soft (lam |xi| + gamma/2 xi^2);  f(x~) = (x_0 - x_init ; f_k(v_k, v_{k+1}));
@@ -10,6 +11,7 @@
 // shuffle tree), so a run is reproducible.
 #pragma once
 #include "tmpc_common.cuh"
+#include "tmpc_srb.cuh"
 
 namespace tmpc {
 
@@ -19,6 +21,7 @@ template <typename T>
 struct SqpArgs {
   Dims d; QpView<T> qp;
   double Lwb, dt, gamma, lam, eps_c, eta;
+  double mp[13];                                               // SRB model parameters (tmpc_config.model_params)
   int n_alpha, it;
   const int32_t* active;
   const T* ox; const T* oxi; const T* oyf; const T* oyg;      // iterate before the QP solve  [B][nz], [B][mg], [B][mf], [B][mg]
@@ -48,19 +51,41 @@ __device__ __forceinline__ void bicycle_res(double Lwb, double dt, const double*
   f[2] = vk[2] + dt * vel / Lwb * tan(vk[5]) - vk1[2]; f[3] = vk[3] + dt * vk[4] - vk1[3];
 }
 
+// Phi(x, u) - x_next of the SRB model in double: the RK4 step of tmpc_srb.cuh on Fwd<double> numbers with zero derivative parts
+__device__ __forceinline__ void srb_res(const double* mp, double dt, const double* vk, const double* vk1, double* f) {
+  Fwd<double> x[12], u[6], k1[12], k2[12], k3[12], k4[12], xt[12];
+#pragma unroll
+  for (int i = 0; i < 12; ++i) x[i] = {vk[i], 0.0};
+#pragma unroll
+  for (int i = 0; i < 6; ++i) u[i] = {vk[12 + i], 0.0};
+  srb_rhs<double>(mp, x, u, k1);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) xt[i] = x[i] + scale(0.5 * dt, k1[i]);
+  srb_rhs<double>(mp, xt, u, k2);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) xt[i] = x[i] + scale(0.5 * dt, k2[i]);
+  srb_rhs<double>(mp, xt, u, k3);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) xt[i] = x[i] + scale(dt, k3[i]);
+  srb_rhs<double>(mp, xt, u, k4);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) f[i] = (x[i] + scale(dt / 6.0, k1[i] + scale(2.0, k2[i]) + scale(2.0, k3[i]) + k4[i])).v - vk1[i];
+}
+
 // grid = B, block = 32 (n_alpha + 1): warp j < n_alpha evaluates the merit parts at alpha = 2^-j, warp n_alpha at alpha = 0 (plus dl)
-template <typename T>
+template <typename T, int MODEL>
 __global__ void __launch_bounds__(32 * (SQP_MAX_ALPHA + 1)) sqp_linesearch_kernel(SqpArgs<T> a) {
   __shared__ double s_cost[SQP_MAX_ALPHA + 1], s_c1[SQP_MAX_ALPHA + 1], s_dl, s_alpha;
   const Dims& d = a.d;
   const int p = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nA = a.n_alpha;
   if (a.active && !a.active[p]) return;
-  constexpr int n = 6, nx = 4, ng = 3;
+  constexpr int n = MODEL == 1 ? 6 : 18, nx = MODEL == 1 ? 4 : 12;
+  const int ng = MODEL == 1 ? 3 : d.ng;
   const int N = d.N, T_ = d.T, nz = d.nz, mg = d.mg, mf = d.mf, nn = n * n;
   const T* ox = a.ox + (size_t)p * nz; const T* sx = a.x + (size_t)p * nz;
   const T* oxi = a.oxi + (size_t)p * mg; const T* sxi = a.xi + (size_t)p * mg;
   const T* Dp = a.qp.D + a.qp.sD * p; const T* Ep = a.qp.E + a.qp.sE * p; const T* q = a.qp.q + (size_t)p * nz;
-  const T* G = a.qp.G + a.qp.sG * p; const T* lo = a.qp.lo + (size_t)p * mg; const T* hi = a.qp.hi + (size_t)p * mg;
+  const T* G = MODEL == 1 ? a.qp.G + a.qp.sG * p : nullptr; const T* lo = a.qp.lo + (size_t)p * mg; const T* hi = a.qp.hi + (size_t)p * mg;
   const double al = warp < nA ? ldexp(1.0, -warp) : 0.0;
   double cost = 0, c1 = 0, dl = 0;
   for (int t = lane; t < T_; t += 32) {
@@ -108,14 +133,24 @@ __global__ void __launch_bounds__(32 * (SQP_MAX_ALPHA + 1)) sqp_linesearch_kerne
 #pragma unroll
       for (int i = 0; i < nx; ++i) c1 += fabs(v[i] - (double)a.qp.x_init[(size_t)p * nx + i]);
     }
-    if (t < N) { double f[4]; bicycle_res(a.Lwb, a.dt, v, v1, f); c1 += fabs(f[0]) + fabs(f[1]) + fabs(f[2]) + fabs(f[3]); }
-    // inequality rows with their slack
+    if (t < N) {
+      if constexpr (MODEL == 1) { double f[4]; bicycle_res(a.Lwb, a.dt, v, v1, f); c1 += fabs(f[0]) + fabs(f[1]) + fabs(f[2]) + fabs(f[3]); }
+      else { double f[12]; srb_res(a.mp, a.dt, v, v1, f);
 #pragma unroll
+        for (int i = 0; i < 12; ++i) c1 += fabs(f[i]); }
+    }
+    // inequality rows with their slack
     for (int r = 0; r < ng; ++r) {
       const int e = t * ng + r;
       double g = 0;
+      if constexpr (MODEL == 1) {
 #pragma unroll
-      for (int j = 0; j < n; ++j) g += (double)G[(size_t)e * n + j] * v[j];
+        for (int j = 0; j < n; ++j) g += (double)G[(size_t)e * n + j] * v[j];
+      } else {
+        const int col = d.g_col[r];
+#pragma unroll
+        for (int j = 0; j < n; ++j) if (j == col) g = v[j];
+      }
       if ((d.soft_mask >> r) & 1u) {
         const double xo = (double)oxi[e], dxi = (double)sxi[e] - xo, xc = xo + al * dxi;
         g += xc; cost += a.lam * fabs(xc) + 0.5 * a.gamma * xc * xc;
@@ -158,12 +193,12 @@ __global__ void __launch_bounds__(128) sqp_kkt_kernel(SqpArgs<T> a) {
   const Dims& d = a.d;
   const int p = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
   if (!a.act_rw[p]) return;
-  constexpr int n = 6, nx = 4, ng = 3;
+  const int n = d.n, nx = d.nx, ng = d.ng;
   const int N = d.N, nz = d.nz, mg = d.mg, mf = d.mf, nn = n * n;
   const T* x = a.x + (size_t)p * nz; const T* xi = a.xi + (size_t)p * mg; const T* yf = a.yf + (size_t)p * mf; const T* yg = a.yg + (size_t)p * mg;
   const T* Dp = a.qp.D + a.qp.sD * p; const T* Ep = a.qp.E + a.qp.sE * p; const T* q = a.qp.q + (size_t)p * nz;
   const T* Am = a.qp.Am + (size_t)p * N * nx * n; const T* Ap = a.qp.Ap + (size_t)p * N * nx * n; const T* bb = a.qp.b + (size_t)p * N * nx;
-  const T* G = a.qp.G + a.qp.sG * p; const T* lo = a.qp.lo + (size_t)p * mg; const T* hi = a.qp.hi + (size_t)p * mg;
+  const T* G = d.g_sel ? nullptr : a.qp.G + a.qp.sG * p; const T* lo = a.qp.lo + (size_t)p * mg; const T* hi = a.qp.hi + (size_t)p * mg;
   double stat = 0, finf = 0, ginf = 0;
   for (int e = tid; e < nz; e += nt) {
     const int t = e / n, i = e - t * n;
@@ -174,7 +209,8 @@ __global__ void __launch_bounds__(128) sqp_kkt_kernel(SqpArgs<T> a) {
     if (t == 0 && i < nx) g += (double)yf[i];
     if (t < N) for (int k = 0; k < nx; ++k) g += (double)Am[((size_t)t * nx + k) * n + i] * (double)yf[nx + t * nx + k];
     if (t > 0) for (int k = 0; k < nx; ++k) g += (double)Ap[((size_t)(t - 1) * nx + k) * n + i] * (double)yf[nx + (t - 1) * nx + k];
-    for (int r = 0; r < ng; ++r) g += (double)G[((size_t)t * ng + r) * n + i] * (double)yg[t * ng + r];
+    if (d.g_sel) { for (int r = 0; r < ng; ++r) if (d.g_col[r] == i) g += (double)yg[t * ng + r]; }
+    else for (int r = 0; r < ng; ++r) g += (double)G[((size_t)t * ng + r) * n + i] * (double)yg[t * ng + r];
     stat = fmax(stat, fabs(g));
   }
   for (int e = tid; e < mf; e += nt) {
@@ -190,7 +226,8 @@ __global__ void __launch_bounds__(128) sqp_kkt_kernel(SqpArgs<T> a) {
   for (int e = tid; e < mg; e += nt) {
     const int t = e / ng, r = e - t * ng;
     double g = ((d.soft_mask >> r) & 1u) ? (double)xi[e] : 0.0;
-    for (int j = 0; j < n; ++j) g += (double)G[(size_t)e * n + j] * (double)x[t * n + j];
+    if (d.g_sel) g += (double)x[t * n + d.g_col[r]];
+    else for (int j = 0; j < n; ++j) g += (double)G[(size_t)e * n + j] * (double)x[t * n + j];
     ginf = fmax(ginf, fmax(0.0, g - (double)hi[e]) + fmax(0.0, (double)lo[e] - g));
   }
   stat = warp_max(stat); finf = warp_max(finf); ginf = warp_max(ginf);

@@ -752,6 +752,35 @@ def test_sqp_linesearch_matches_oracle_fp64():
     s.close()
 
 
+def test_sqp_linesearch_srb_matches_oracle_fp64():
+    """f2 on the second built-in model (SRB humanoid, RK4: the merit function's equality residual is Phi(x_k, u_k) - x_{k+1}, selection rows with
+    two soft rows): accepted step sizes, iteration counts, convergence flags, eq. 18 quantities and final iterates equal the oracle's."""
+    from paper_2606_24039_b200.solver import Solver
+    w = W.srb_humanoid(B=4, N=10)
+    w.soft = [0, 1, 0, 0, 1, 0]; w.lam, w.gamma = 0.01, 0.1
+    rng = np.random.default_rng(3)
+    x0 = w.xbar0.copy()
+    x0[:, :, :3] += 0.03 * rng.standard_normal(x0[:, :, :3].shape); x0[:, :, 3:6] += 0.1 * rng.standard_normal(x0[:, :, 3:6].shape)
+    x0[:, :, 6:12] += 0.2 * rng.standard_normal(x0[:, :, 6:12].shape)
+    x0[3] = w.xbar0[3]                                     # one problem starts from the reference
+    kw = dict(max_sqp=20, admm_iters=2000, eps_c=1e-3, n_alpha=8, eta=0.4)
+    ref, rinfo, log, rc = O.sqp_linesearch_srb(w, O.make_cfg(w), xbar0=x0, **kw)
+    assert rc == 0
+    s = Solver(w, dtype="f64")
+    s.reset_state(x0)
+    out = s.sqp_linesearch(**kw)
+    got = s.state_numpy()
+    assert (out["iters"] == rinfo[:, 0].astype(int)).all(), (out["iters"], rinfo[:, 0])
+    assert (out["converged"] == rinfo[:, 1].astype(int)).all() and out["converged"].any()
+    for b in range(w.B):
+        k = int(rinfo[b, 0])
+        assert (out["alpha"][b, :k] == log[b, :k, 0]).all(), (b, out["alpha"][b, :k], log[b, :k, 0])
+    assert (out["alpha"] < 1.0).any() and (out["alpha"] == 1.0).any() and (ref["xi"] != 0).any()
+    compare_states({k: got[k] for k in ("x", "yf", "yg", "xi")} | {"zg": ref["zg"]}, ref, 1e-8)
+    assert np.abs(out["kkt"] - rinfo[:, 2:5]).max() <= 1e-6
+    s.close()
+
+
 def test_adaptive_on_the_streamed_class_fp64():
     """f1 on the streamed class (blocks that do not fit in shared memory: admm_stream_kernel + factor3_kernel with per-problem rho_bar,
     refactor mask and frozen terminated problems), on the f4 generator at (nx, nu) = (32, 16)."""
