@@ -339,9 +339,11 @@ tmpc_status launch_factor_tw(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double
   FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = w_rows;
   a.rho_bar = w_rows ? nullptr : (const T*)h->cur_rho; a.rho_scale = h->cfg.rho_eq_scale; a.mask = w_rows ? nullptr : h->cur_mask;
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
-  if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) factor_tw2_kernel<T, 8, 6, true><<<h->d.B, 64, 0, h->stream>>>(a);
-  else if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) factor_tw2_kernel<T, 6, 4, true><<<h->d.B, 64, 0, h->stream>>>(a);
-  else if (h->d.n == 12 && h->d.nx == 8 && h->d.ng <= 12) factor_tw2_kernel<T, 12, 8, true><<<h->d.B, 64, 0, h->stream>>>(a);
+  // small batches: the launch lasts as long as one problem's chain, so four warps per chain instead of one (tmpc_factor2.cuh)
+  const bool wide = h->d.B <= 2 * sm_count();
+  if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) { if (wide) factor_tw2_kernel<T, 8, 6, true, 4><<<h->d.B, 256, 0, h->stream>>>(a); else factor_tw2_kernel<T, 8, 6, true><<<h->d.B, 64, 0, h->stream>>>(a); }
+  else if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) { if (wide) factor_tw2_kernel<T, 6, 4, true, 4><<<h->d.B, 256, 0, h->stream>>>(a); else factor_tw2_kernel<T, 6, 4, true><<<h->d.B, 64, 0, h->stream>>>(a); }
+  else if (h->d.n == 12 && h->d.nx == 8 && h->d.ng <= 12) { if (h->d.B <= sm_count()) factor_tw2_kernel<T, 12, 8, true, 8><<<h->d.B, 512, 0, h->stream>>>(a); else if (wide) factor_tw2_kernel<T, 12, 8, true, 4><<<h->d.B, 256, 0, h->stream>>>(a); else factor_tw2_kernel<T, 12, 8, true><<<h->d.B, 64, 0, h->stream>>>(a); }
   else return TMPC_E_UNSUPPORTED;      // fast_plan() only admits the shapes above
   h->launches++;
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;

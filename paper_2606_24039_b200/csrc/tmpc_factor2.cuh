@@ -29,17 +29,24 @@ namespace tmpc {
 
 // TW = true: twisted factor (X_t, B_t) for admm3_kernel.  TW = false: the one-directional block LDL' of factor_kernel
 // (Lam_t = Phi_t Sigma_t^{-1}, Sinv_t = Sigma_t^{-1}; per-row weights w_rows supported) for the backward pass; one warp.
-template <typename T, int NC, int NX, bool TW>
-__global__ void __launch_bounds__(64, 12) factor_tw2_kernel(FactorArgs<T> a) {
+// WPC warps per chain: 1 for batches that fill the GPU (12 CTAs of two warps per SM, throughput bound); 4 (8 for n = 12) for small batches, where
+// the launch is as long as ONE problem's chain (2000+ dependent warp instructions per stage for n = 12 on one warp) — the element loops are then
+// spread over 128 (256) threads per chain and the phases are separated by a named barrier per chain instead of __syncwarp.  Same sums in the
+// same order.  Measured at (64,40,8,4) fp64: 341 -> 128 -> 108 us per launch; two warps per chain for mid-size batches (B = 1024) lost to the
+// register cap its eight CTAs per SM need (554 against 477 us).
+template <typename T, int NC, int NX, bool TW, int WPC = 1>
+__global__ void __launch_bounds__(64 * WPC, WPC == 1 ? 12 : (WPC <= 4 ? 2 : 1)) factor_tw2_kernel(FactorArgs<T> a) {
   constexpr int n = NC, nx = NX, nn = NC * NC, an = NX * NC;
-  constexpr int EPL = (nn + 31) / 32;                   // matrix elements per lane
+  constexpr int GT = 32 * WPC;                          // threads per chain
+  constexpr int EPL = (nn + GT - 1) / GT;               // matrix elements per lane
   constexpr int GMAX = NC * NC;                         // room for ng <= n rows of G
   constexpr int RAW = 2 * nn + 2 * an + GMAX;           // D, E, Am, Ap, G
-  constexpr int RPL = (RAW + 31) / 32;
+  constexpr int RPL = (RAW + GT - 1) / GT;
   __shared__ double sm[2][3 * nn + RAW + NC];
   const Dims& d = a.d;
   const int ng = d.ng, N = d.N, T_ = d.T;
-  const int half = threadIdx.x >> 5, lane = threadIdx.x & 31, p = blockIdx.x;
+  const int half = threadIdx.x / GT, lane = threadIdx.x % GT, p = blockIdx.x;
+  auto gsync = [&]() { if constexpr (WPC == 1) __syncwarp(); else asm volatile("bar.sync %0, %1;" ::"r"(1 + half), "r"(GT) : "memory"); };
   double* A = sm[half]; double* Bm = A + nn; double* C = Bm + nn;
   double* rD = C + nn; double* rE = rD + nn; double* rAm = rE + nn; double* rAp = rAm + an; double* rG = rAp + an;
   const T* Dp = a.qp.D + a.qp.sD * p;
@@ -70,17 +77,17 @@ __global__ void __launch_bounds__(64, 12) factor_tw2_kernel(FactorArgs<T> a) {
   T pre[RPL];
   auto prefetch = [&](int t) {
 #pragma unroll
-    for (int u = 0; u < RPL; ++u) { const int e = lane + 32 * u; pre[u] = e < RAW ? raw_src(t, e) : T(0); }
+    for (int u = 0; u < RPL; ++u) { const int e = lane + GT * u; pre[u] = e < RAW ? raw_src(t, e) : T(0); }
   };
   auto commit = [&]() {
 #pragma unroll
-    for (int u = 0; u < RPL; ++u) { const int e = lane + 32 * u; if (e < RAW) rD[e] = (double)pre[u]; }
+    for (int u = 0; u < RPL; ++u) { const int e = lane + GT * u; if (e < RAW) rD[e] = (double)pre[u]; }
   };
   // Theta_t (lower triangle) minus W W' of up to two finished neighbours, from the raw data in shared memory
   auto theta = [&](int t, double* dst, const double* W1, const double* W2) {
 #pragma unroll
     for (int u = 0; u < EPL; ++u) {
-      const int e = lane + 32 * u;
+      const int e = lane + GT * u;
       if (e >= nn) continue;
       const int i = e / n, j = e % n;
       if (j > i) continue;
@@ -117,39 +124,39 @@ __global__ void __launch_bounds__(64, 12) factor_tw2_kernel(FactorArgs<T> a) {
       rsk[k] = rs;
 #pragma unroll
       for (int u = 0; u < EPL; ++u) {
-        const int e = lane + 32 * u, i = e / n, j = e % n;
+        const int e = lane + GT * u, i = e / n, j = e % n;
         if (e < nn && j > k && j <= i) Am_[e] -= Am_[i * n + k] * Am_[j * n + k] * inv;
       }
-      __syncwarp();
+      gsync();
       if (lane < n && lane >= k) Am_[lane * n + k] = lane == k ? sq : Am_[lane * n + k] * rs;
       if (lane == 0) rsd[k] = rs;
-      __syncwarp();
+      gsync();
     }
 #pragma unroll
-    for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u; if (e < nn) Xo[e] = (e / n == e % n) ? 1.0 : 0.0; }
-    __syncwarp();
+    for (int u = 0; u < EPL; ++u) { const int e = lane + GT * u; if (e < nn) Xo[e] = (e / n == e % n) ? 1.0 : 0.0; }
+    gsync();
 #pragma unroll
     for (int k = 0; k < n - 1; ++k) {
       const double inv = rsk[k];
 #pragma unroll
       for (int u = 0; u < EPL; ++u) {
-        const int e = lane + 32 * u, i = e / n, j = e % n;
+        const int e = lane + GT * u, i = e / n, j = e % n;
         if (e < nn && i > k && j <= k) Xo[e] -= Am_[i * n + k] * Xo[k * n + j] * inv;
       }
-      __syncwarp();
+      gsync();
     }
 #pragma unroll
-    for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u; if (e < nn) Xo[e] = Xo[e] * rsd[e / n]; }
-    __syncwarp();
+    for (int u = 0; u < EPL; ++u) { const int e = lane + GT * u; if (e < nn) Xo[e] = Xo[e] * rsd[e / n]; }
+    gsync();
   };
   auto x_out = [&](int t, const double* X) {
 #pragma unroll
-    for (int u = 0; u < EPL; ++u) { const int e = lane + 32 * u; if (e < nn) Xp[(size_t)t * nn + e] = (T)X[e]; }
+    for (int u = 0; u < EPL; ++u) { const int e = lane + GT * u; if (e < nn) Xp[(size_t)t * nn + e] = (T)X[e]; }
   };
   auto b_out = [&](int tprev, const double* X, const double* W) {      // B = X_next W_prev
 #pragma unroll
     for (int u = 0; u < EPL; ++u) {
-      const int e = lane + 32 * u;
+      const int e = lane + GT * u;
       if (e >= nn) continue;
       const int i = e / n, j = e % n;
       double s = 0;
@@ -163,16 +170,16 @@ __global__ void __launch_bounds__(64, 12) factor_tw2_kernel(FactorArgs<T> a) {
   for (int k = 0; k < cnt; ++k) {
     const int t = half ? N - k : k;
     commit();
-    __syncwarp();
+    gsync();
     if (k + 1 < cnt) prefetch(half ? t - 1 : t + 1);
     theta(t, A, k > 0 ? C : nullptr, nullptr);
-    __syncwarp();
+    gsync();
     chol_inv(A, Bm);
     if constexpr (TW) { if (k > 0) b_out(half ? t + 1 : t - 1, Bm, C); x_out(t, Bm); }
     else {                                             // Sinv_t = X'X
 #pragma unroll
       for (int u = 0; u < EPL; ++u) {
-        const int e = lane + 32 * u;
+        const int e = lane + GT * u;
         if (e >= nn) continue;
         const int i = e / n, j = e % n;
         double s = 0;
@@ -182,7 +189,7 @@ __global__ void __launch_bounds__(64, 12) factor_tw2_kernel(FactorArgs<T> a) {
       }
       if (t == N) break;
     }
-    __syncwarp();
+    gsync();
     // A <- Psi_t: up Phi_t = E_t + w A^+_t' A^-_t ; down Phi_{t-1}' = E_{t-1}' + w A^-_{t-1}' A^+_{t-1}.
     // up needs A^+_t (not in this stage's raw data): read it from global; down has A^+_{t-1} (rAp) and needs A^-_{t-1}.
     {
@@ -190,7 +197,7 @@ __global__ void __launch_bounds__(64, 12) factor_tw2_kernel(FactorArgs<T> a) {
       const T* other = half ? Amp + (size_t)tc * an : App + (size_t)tc * an;
 #pragma unroll
       for (int u = 0; u < EPL; ++u) {
-        const int e = lane + 32 * u;
+        const int e = lane + GT * u;
         if (e >= nn) continue;
         const int i = e / n, j = e % n;
         const int ii = half ? j : i, jj = half ? i : j; // Phi[ii][jj] = E[ii][jj] + w sum_r A^+[r][ii] A^-[r][jj]
@@ -200,10 +207,10 @@ __global__ void __launch_bounds__(64, 12) factor_tw2_kernel(FactorArgs<T> a) {
         A[e] = rE[ii * n + jj] + w_eq * acc;
       }
     }
-    __syncwarp();
+    gsync();
 #pragma unroll
     for (int u = 0; u < EPL; ++u) {                     // C <- W = Psi X'
-      const int e = lane + 32 * u;
+      const int e = lane + GT * u;
       if (e >= nn) continue;
       const int i = e / n, j = e % n;
       double s = 0;
@@ -211,11 +218,11 @@ __global__ void __launch_bounds__(64, 12) factor_tw2_kernel(FactorArgs<T> a) {
       for (int kk = 0; kk < n; ++kk) if (kk <= j) s += A[i * n + kk] * Bm[j * n + kk];
       C[e] = s;
     }
-    __syncwarp();
+    gsync();
     if constexpr (!TW) {                                // Lambda_t = W X
 #pragma unroll
       for (int u = 0; u < EPL; ++u) {
-        const int e = lane + 32 * u;
+        const int e = lane + GT * u;
         if (e >= nn) continue;
         const int i = e / n, j = e % n;
         double s = 0;
@@ -230,9 +237,9 @@ __global__ void __launch_bounds__(64, 12) factor_tw2_kernel(FactorArgs<T> a) {
   if (TW && half == 0) {
     const double* Wup = sm[0] + 2 * nn; const double* Wdn = sm[1] + 2 * nn;
     prefetch(m); commit();
-    __syncwarp();
+    gsync();
     theta(m, A, m > 0 ? Wup : nullptr, (T_ - 1 - m) > 0 ? Wdn : nullptr);
-    __syncwarp();
+    gsync();
     chol_inv(A, Bm);
     if (m > 0) b_out(m - 1, Bm, Wup);
     if (T_ - 1 - m > 0) b_out(m + 1, Bm, Wdn);
