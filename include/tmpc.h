@@ -123,7 +123,8 @@ typedef struct {
   double rho_ratio, rho_min, rho_max; /* k_rho^ratio and the clip bounds of eq. 17 (paper: 5, 1e-6, 1e6) */
 } tmpc_adaptive;
 /* Needs tmpc_factor first (every problem starts from cfg.rho_bar) and, unlike the other calls, SYNCHRONISES: the count of live problems
- * is read back after every round so that the call returns when all have terminated.  Outputs (DEVICE, [B], any may be NULL): iterations
+ * of every round is read back (one round behind the launches, through a pinned page the library allocates once per process) so that the
+ * call returns when all have terminated; it returns with the stream idle.  Outputs (DEVICE, [B], any may be NULL): iterations
  * each problem ran, 1 if it met eq. 4, its final rho_bar (working dtype); info as in tmpc_admm_solve, at each problem's last check.
  * Afterwards the factor in the workspace belongs to the per-problem rho_bar values: call tmpc_factor before the next solve.
  * TMPC_E_UNSUPPORTED for cyclic reduction. */

@@ -2,6 +2,7 @@
 // No CPU fallback: every compute entry point needs a CUDA device and returns TMPC_E_CUDA otherwise.
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include "tmpc_common.cuh"
 #include "tmpc_factor.cuh"
@@ -95,6 +96,7 @@ struct tmpc_ctx {
   const void* cur_rho; const int32_t* cur_active; const int32_t* cur_mask;
   bool bwd_classified;                          // tmpc_backward has left the row classification of its state in the workspace
   cudaStream_t aux[2]; cudaEvent_t ev[3];       // tmpc_admm_solve_host: two sub-batches in flight (copies of one overlap the kernels of the other)
+  int32_t* pin_live; cudaEvent_t ad_ev[2];      // tmpc_admm_solve_adaptive: pinned landing slots of the per-round live counts and their events (created on first use)
 };
 
 namespace {
@@ -432,6 +434,16 @@ tmpc_status do_solve(tmpc_ctx* h, const tmpc_qp* qp, tmpc_state* st, int iters, 
 // Rounds of `check_every` iterations: [solve kernel on the live problems with their own rho_bar] -> [residuals + eq. 4 scales] ->
 // [adapt_kernel: terminate / new rho_bar / refactor mask] -> [masked refactor].  The number of live problems comes back to the host
 // after every round (4 bytes), so the call returns as soon as every problem has terminated.
+// Two pinned ints per handle for the live counts of tmpc_admm_solve_adaptive, handed out round-robin from ONE page-locked page per process
+// (cudaHostAlloc costs milliseconds, too much for a handle that lives for one solve; the page is never freed).  512 pairs: more handles than
+// that running the adaptive solve at the same time would share landing slots.
+int32_t* pinned_pair() {
+  static std::mutex mu; static int32_t* pool = nullptr; static unsigned next = 0;
+  std::lock_guard<std::mutex> lk(mu);
+  if (!pool && cudaHostAlloc((void**)&pool, 1024 * sizeof(int32_t), cudaHostAllocDefault) != cudaSuccess) { cudaGetLastError(); pool = nullptr; return nullptr; }
+  return pool + 2 * (next++ % 512u);
+}
+
 template <typename T>
 tmpc_status do_solve_adaptive(tmpc_ctx* h, const tmpc_qp* qp, tmpc_state* st, const tmpc_adaptive* ad, int flags, tmpc_info* info,
                               int32_t* iters_out, int32_t* conv_out, void* rho_out) {
@@ -445,25 +457,35 @@ tmpc_status do_solve_adaptive(tmpc_ctx* h, const tmpc_qp* qp, tmpc_state* st, co
   const unsigned nb = (unsigned)((d.B + 255) / 256);
   adapt_init_kernel<T><<<nb, 256, 0, h->stream>>>(d.B, (T)h->cfg.rho_bar, rho, active, mask, iters, conv, count); h->launches++;
   if (!cuda_ok()) return TMPC_E_CUDA;
+  // The host only needs the live count to stop launching: it reads round r's count AFTER round r + 1 has been enqueued (two counters, two pinned
+  // landing slots, two events), so the GPU never idles while the host waits.  A round enqueued after every problem has terminated finds all
+  // activity flags clear and changes nothing.
+  if (!h->pin_live) { h->pin_live = pinned_pair(); if (!h->pin_live) return TMPC_E_CUDA; }
+  for (int e = 0; e < 2; ++e) if (!h->ad_ev[e] && cudaEventCreateWithFlags(&h->ad_ev[e], cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return TMPC_E_CUDA; }
   h->cur_rho = rho; h->cur_active = active; h->cur_mask = mask;
   tmpc_status rc = TMPC_OK;
-  int k = 0, f = flags;
+  int k = 0, f = flags, round = 0;
   while (k < ad->max_iters && rc == TMPC_OK) {
     const int chunk = ad->max_iters - k < ad->check_every ? ad->max_iters - k : ad->check_every;
     rc = do_solve<T>(h, qp, st, chunk, f, &li);          // also runs residual_kernel with the eq. 4 scales (li is never null)
     if (rc != TMPC_OK) break;
     k += chunk; f |= TMPC_SOLVE_ZG_GIVEN;
-    if (cudaMemsetAsync(count, 0, sizeof(int32_t), h->stream) != cudaSuccess) { rc = TMPC_E_CUDA; break; }
+    int32_t* cnt_r = count + (round & 1);
+    if (cudaMemsetAsync(cnt_r, 0, sizeof(int32_t), h->stream) != cudaSuccess) { rc = TMPC_E_CUDA; break; }
     AdaptParams ap; ap.k = k; ap.last = k >= ad->max_iters; ap.adapt_rho = ad->adapt_rho; ap.eps_abs = ad->eps_abs; ap.eps_rel = ad->eps_rel;
     ap.ratio = ad->rho_ratio; ap.rho_min = ad->rho_min; ap.rho_max = ad->rho_max;
     adapt_kernel<T><<<nb, 256, 0, h->stream>>>(d.B, ap, (const T*)li.r_prim, (const T*)li.r_dual, (const T*)(ws + L.ad_np), (const T*)(ws + L.ad_nd), rho, active, mask,
-                                              iters, conv, count); h->launches++;
-    int32_t live = 0;
-    if (!cuda_ok() || cudaMemcpyAsync(&live, count, sizeof(int32_t), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
-        cudaStreamSynchronize(h->stream) != cudaSuccess) { rc = TMPC_E_CUDA; break; }
-    if (live == 0) break;
-    if (ad->adapt_rho) rc = do_factor<T>(h, qp);          // only the problems whose rho_bar changed (mask)
+                                              iters, conv, cnt_r); h->launches++;
+    if (!cuda_ok() || cudaMemcpyAsync(h->pin_live + (round & 1), cnt_r, sizeof(int32_t), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+        cudaEventRecord(h->ad_ev[round & 1], h->stream) != cudaSuccess) { rc = TMPC_E_CUDA; break; }
+    if (round > 0) {                                     // the count of the round before this one
+      if (cudaEventSynchronize(h->ad_ev[(round - 1) & 1]) != cudaSuccess) { rc = TMPC_E_CUDA; break; }
+      if (h->pin_live[(round - 1) & 1] == 0) break;
+    }
+    if (ad->adapt_rho && k < ad->max_iters) rc = do_factor<T>(h, qp);          // only the problems whose rho_bar changed (mask)
+    ++round;
   }
+  if (rc == TMPC_OK && cudaStreamSynchronize(h->stream) != cudaSuccess) rc = TMPC_E_CUDA;      // the call synchronises (tmpc.h)
   h->cur_rho = nullptr; h->cur_active = nullptr; h->cur_mask = nullptr;
   h->factored = false;                                   // the factor in the workspace now belongs to the per-problem rho_bar values
   if (rc != TMPC_OK) return rc;
@@ -575,6 +597,7 @@ tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, vo
   h->factored = false; h->cr = use_cr(*cfg); h->twisted = false; h->launches = 0;
   h->cur_rho = nullptr; h->cur_active = nullptr; h->cur_mask = nullptr; h->bwd_classified = false;
   h->aux[0] = h->aux[1] = nullptr; h->ev[0] = h->ev[1] = h->ev[2] = nullptr;
+  h->pin_live = nullptr; h->ad_ev[0] = h->ad_ev[1] = nullptr;
   // zero buffers of the adjoint QP (x_init = 0, b = 0)
   if (cudaMemsetAsync(h->ws + L.zero_xinit, 0, L.zero_b - L.zero_xinit, h->stream) != cudaSuccess ||
       cudaMemsetAsync(h->ws + L.zero_b, 0, L.cr - L.zero_b, h->stream) != cudaSuccess) { delete h; return TMPC_E_CUDA; }
@@ -597,6 +620,7 @@ tmpc_status tmpc_destroy(tmpc_handle h) {
   if (h) {
     for (int k = 0; k < 2; ++k) if (h->aux[k]) cudaStreamDestroy(h->aux[k]);
     for (int k = 0; k < 3; ++k) if (h->ev[k]) cudaEventDestroy(h->ev[k]);
+    for (int k = 0; k < 2; ++k) if (h->ad_ev[k]) cudaEventDestroy(h->ad_ev[k]);
   }
   delete h; return TMPC_OK;
 }
@@ -926,7 +950,7 @@ extern "C" tmpc_status tmpc_admm_solve_static(const tmpc_config* cfg, const tmpc
   c.cfg = *cfg; c.d = make_dims(*cfg); c.lay = L; c.ws = ws; c.stream = (cudaStream_t)cuda_stream;
   c.factored = false; c.cr = false; c.twisted = false; c.launches = 0;
   c.cur_rho = nullptr; c.cur_active = nullptr; c.cur_mask = nullptr; c.bwd_classified = false;
-  c.aux[0] = c.aux[1] = nullptr; c.ev[0] = c.ev[1] = c.ev[2] = nullptr;
+  c.aux[0] = c.aux[1] = nullptr; c.ev[0] = c.ev[1] = c.ev[2] = nullptr; c.pin_live = nullptr; c.ad_ev[0] = c.ad_ev[1] = nullptr;
   s = check_qp(&c, qp); if (s != TMPC_OK) return s;
   // the array keeps the previous call's contents: the per-problem status words must start at zero (the factor kernels overwrite them, this is
   // belt and braces); the factor, the eta scratch of the streamed class and the residual partials are all written before they are read
