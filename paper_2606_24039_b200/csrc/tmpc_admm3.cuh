@@ -368,6 +368,12 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
   const int crank = CL ? (int)cl_rank() : 0, cl_t0 = crank ? m + 1 : 0, cl_cnt = CL ? (crank ? T_ - 1 - m : m + 1) : T_;
   const int pbase = CL ? (int)(blockIdx.x >> 1) : (int)blockIdx.x * PG;
   if constexpr (CL) { if (a.active && !a.active[pbase]) return; }      // a terminated problem (f1): both CTAs of the pair leave before any cluster barrier
+  else if (a.active) {                                                 // a CTA whose problems have all terminated leaves before the prologue
+    bool any = false;
+#pragma unroll
+    for (int g = 0; g < PG; ++g) any |= pbase + g < d.B && a.active[pbase + g] != 0;
+    if (!any) return;
+  }
   const unsigned cl_sb = (unsigned)__cvta_generic_to_shared(sm);
   const unsigned cl_box = cl_sb + (unsigned)(PP - (NC + RC::V - 1) / RC::V * RC::V) * (unsigned)sizeof(T), cl_mb = cl_sb + (unsigned)PP * (unsigned)sizeof(T);   // mailbox; mbarriers mid, eta, y
 
