@@ -407,16 +407,19 @@ def f4_rows(ctx, args):
             row["backward_ms"] = 1e3 * min(ts[1:])
             if (B, N, nx, nu) == (64, 40, 8, 4):          # closed loop: H = 50 MPC solves, each warm-started from the previous solution
                 A = s.t["Am"][:, 0, :, :nx]; Bm = s.t["Am"][:, 0, :, nx:]; bv = -s.t["b"][:, 0, :]
-                s.reset_state(); s.t["x_init"].copy_(s._up(w.x_init)); torch.cuda.synchronize(dev)
-                t0 = time.perf_counter(); its = 0
-                for hstep in range(50):
-                    out = s.solve_adaptive(1000, 1e-3, 1e-3, flags=Bd.TMPC_SOLVE_ZG_GIVEN if hstep else 0)
-                    its += int(out["iters"].max())
-                    u0 = s.s["x"][:, 0, nx:]
-                    xn = torch.einsum("bij,bj->bi", A, s.t["x_init"]) + torch.einsum("bij,bj->bi", Bm, u0) + bv      # the environment step (not the solver)
-                    s.t["x_init"].copy_(xn)
-                torch.cuda.synchronize(dev)
-                row["closed_loop_H50_tol_1e-3"] = {"ms_total": 1e3 * (time.perf_counter() - t0), "max_iterations_summed": its}
+                tl = []
+                for _ in range(2):                        # best of two roll-outs (the first one also pays torch's one-time einsum set-up)
+                    s.reset_state(); s.t["x_init"].copy_(s._up(w.x_init)); torch.cuda.synchronize(dev)
+                    t0 = time.perf_counter(); its = 0
+                    for hstep in range(50):
+                        out = s.solve_adaptive(1000, 1e-3, 1e-3, flags=Bd.TMPC_SOLVE_ZG_GIVEN if hstep else 0)
+                        its += int(out["iters"].max())
+                        u0 = s.s["x"][:, 0, nx:]
+                        xn = torch.einsum("bij,bj->bi", A, s.t["x_init"]) + torch.einsum("bij,bj->bi", Bm, u0) + bv      # the environment step (not the solver)
+                        s.t["x_init"].copy_(xn)
+                    torch.cuda.synchronize(dev)
+                    tl.append(time.perf_counter() - t0)
+                row["closed_loop_H50_tol_1e-3"] = {"ms_total": 1e3 * min(tl), "max_iterations_summed": its}
             rows.append(row)
             s.close()
     return rows
