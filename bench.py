@@ -317,7 +317,7 @@ def gpu_one(cfg_id, dtype, args, ctx, steps, with_cpu):
                 t0 = time.perf_counter(); out = s.solve_adaptive(1000, eps, eps); ts.append(time.perf_counter() - t0)
             adaptive[f"eps_{eps:g}"] = {"ms_per_batched_solve": 1e3 * min(ts), "iterations_median": float(np.median(out["iters"])), "iterations_max": int(out["iters"].max()),
                                         "converged_frac": float(out["converged"].mean()), "rho_bar_final_median": float(np.median(out["rho"])),
-                                        "note": "tmpc_factor + tmpc_admm_solve_adaptive, wall clock (the call synchronises once per 25-iteration round)"}
+                                        "note": "tmpc_factor + tmpc_admm_solve_adaptive, wall clock (the call reads the live count back once per 25-iteration round)"}
 
     s.close()
     if rank != 0:
