@@ -235,20 +235,21 @@ FastPlan fast_plan(const Dims& d) {
   const size_t s1 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 1) : d.n == 6 ? admm3_smem_bytes<T, 6, 4>(d, 1) : admm3_smem_bytes<T, 12, 8>(d, 1);
   const size_t s2 = d.n == 8 ? admm3_smem_bytes<T, 8, 6>(d, 2) : d.n == 6 ? admm3_smem_bytes<T, 6, 4>(d, 2) : kMaxSmem + 1;   // n = 12: one problem per CTA (16 chain lanes per slot)
   if (s1 > kMaxSmem) {
-    // The (12, 8) block first tries a CLUSTER of two CTAs per problem (tmpc_admm3.cuh, CL) when the batch leaves half of the SMs idle anyway: with
-    // full records when the two halves fit two SMs (about half the latency per iteration of the single-CTA variant below; for batches that fill
-    // the GPU one CTA per problem is ~8 % faster: 15.9 vs 17.4 ms per 100 iterations at (1024,80,8,4) fp64), ...
+    // The full records of one problem do not fit one SM.  In order of preference:
+    // (1) (12, 8) block, batch that leaves half of the SMs idle anyway: a CLUSTER of two CTAs per problem (tmpc_admm3.cuh, CL) with full records,
+    //     if the two halves fit two SMs — about half the latency per iteration of (2); for batches that fill the GPU (2) is ~8 % faster
+    //     (15.9 vs 17.4 ms per 100 iterations at (1024,80,8,4) fp64);
     const int half = d.T / 2 + 1, ntc = 32 + (2 * half + 31) / 32 * 32;
     const bool cl_shape = d.n == 12 && d.T >= 8 && ntc <= 384;
     if (cl_shape && 2 * d.B <= sm_count()) {
       const size_t sr = admm3_cl_smem_bytes<T, 12, 8, false>(d);
       if (sr <= kMaxSmem) { f.ok = true; f.cl = true; f.nt = ntc; f.ctas_per_sm = 1; f.smem = sr; return f; }
     }
-    // long horizons: only the chain's share of a record stays in shared memory (Rec3<.., XG>), one problem per CTA, two item lanes per stage
+    // (2) one CTA per problem with only the chain's share of a record in shared memory (Rec3<.., XG>), the rest from the stage-minor global scratch;
     const size_t sx = d.n == 8 ? admm3_smem_bytes<T, 8, 6, true>(d, 1) : d.n == 6 ? admm3_smem_bytes<T, 6, 4, true>(d, 1) : admm3_smem_bytes<T, 12, 8, true>(d, 1);
     const int ntx = 32 + (2 * d.T + 31) / 32 * 32;
-    // ... and with the chain's share only when that no longer fits one SM (one CTA per problem is faster where it fits: 37 against 50 us per
-    // iteration at (64,160,8,4) fp64 once the global operands are laid out stage-minor)
+    // (3) (12, 8) block: the cluster pair with the chain's share, when even that does not fit one SM (where it fits, (2) is faster: 37 against
+    //     50 us per iteration at (64,160,8,4) fp64).
     const bool one_fits = sx <= kMaxSmem && ntx <= 1024;
     if (cl_shape && !one_fits) {
       const size_t sc = admm3_cl_smem_bytes<T, 12, 8, true>(d);
