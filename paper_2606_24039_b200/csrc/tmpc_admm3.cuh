@@ -723,7 +723,7 @@ __global__ void __launch_bounds__(MAXT, MINB) admm3_kernel(const __grid_constant
 // with M~[k][j] = sum_{l <= j} M[k][l] X_t[j][l] (X_t lower triangular); element j of row r of stage t goes to
 // (p rows + r) RS + (j / V) CS + t V + j % V, CS = tpad V, RS = ceil(n / V) CS.  One thread per (problem, row, stage), stage fastest; n <= 16.
 template <typename T>
-__global__ void __launch_bounds__(128) atil_kernel(const AdmmArgs<T> a, T* __restrict__ atil, int tpad, int rows) {   // rows = n for kkt_only (X only)
+__global__ void __launch_bounds__(128) atil_kernel(const AdmmArgs<T> a, T* __restrict__ atil, int tpad, int rows, const int32_t* __restrict__ mask) {   // rows = n for kkt_only (X only); mask: only the problems whose factor has changed
   const Dims& d = a.d;
   constexpr int V = 16 / (int)sizeof(T);
   const int n = d.n, nx = d.nx, T_ = d.T, N = d.N;
@@ -732,6 +732,7 @@ __global__ void __launch_bounds__(128) atil_kernel(const AdmmArgs<T> a, T* __res
   const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= (long long)d.B * rows * T_) return;
   const int t = (int)(e % T_), r = (int)((e / T_) % rows), p = (int)(e / ((long long)rows * T_));
+  if (mask && !mask[p]) return;
   const T* X = a.Sinv + ((size_t)p * T_ + t) * n * n;
   T* out = atil + ((size_t)p * rows_all + r) * RS + (size_t)t * V;
   if (r < n) {                                         // a row of X_t

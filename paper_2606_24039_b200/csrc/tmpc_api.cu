@@ -96,6 +96,7 @@ struct tmpc_ctx {
   const void* cur_rho; const int32_t* cur_active; const int32_t* cur_mask;
   bool bwd_classified;                          // tmpc_backward has left the row classification of its state in the workspace
   cudaStream_t aux[2]; cudaEvent_t ev[3];       // tmpc_admm_solve_host: two sub-batches in flight (copies of one overlap the kernels of the other)
+  bool atil_valid;                              // the stage-minor scratch of the chain-resident variants matches the factor in the workspace
   int32_t* pin_live; cudaEvent_t ad_ev[2];      // tmpc_admm_solve_adaptive: pinned landing slots of the per-round live counts and their events (created on first use)
 };
 
@@ -121,6 +122,7 @@ tmpc_status launch_factor(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_
   FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = w_rows;
   a.rho_bar = w_rows ? nullptr : (const T*)h->cur_rho; a.rho_scale = h->cfg.rho_eq_scale; a.mask = w_rows ? nullptr : h->cur_mask;
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
+  h->atil_valid = false;                                // another factor form takes the workspace
   // small compile-time shapes: the warp-level kernel in its one-directional form (tmpc_factor2.cuh)
   if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) { factor_tw2_kernel<T, 8, 6, false><<<h->d.B, 32, 0, h->stream>>>(a); h->launches++; return cuda_ok() ? TMPC_OK : TMPC_E_CUDA; }
   if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) { factor_tw2_kernel<T, 6, 4, false><<<h->d.B, 32, 0, h->stream>>>(a); h->launches++; return cuda_ok() ? TMPC_OK : TMPC_E_CUDA; }
@@ -286,9 +288,13 @@ tmpc_status launch_admm3_inst(tmpc_ctx* h, const AdmmArgs<T>& a, const FastPlan&
   A.tpad = (h->d.T + 7) / 8 * 8;
   if constexpr (XG) {
     T* atil = (T*)(h->ws + h->lay.atil); A.atil = atil;
+    // The scratch depends on the factor and the constraint blocks only: it is rebuilt in full after a full (or adjoint) factorisation, for the
+    // re-factored problems after a masked one (f1, SQP: cur_mask still holds the mask that factorisation took), and not at all otherwise.
     const int rows = a.kkt_only ? h->d.n : h->d.n + 2 * h->d.nx + (h->d.g_sel ? 0 : h->d.ng);      // tmpc_kkt_solve needs X only
     const long long work = (long long)h->d.B * rows * h->d.T;
-    atil_kernel<T><<<(unsigned)((work + 127) / 128), 128, 0, h->stream>>>(a, atil, A.tpad, rows); h->launches++;
+    const bool full = !h->atil_valid;
+    if (full || h->cur_mask) { atil_kernel<T><<<(unsigned)((work + 127) / 128), 128, 0, h->stream>>>(a, atil, A.tpad, rows, full ? nullptr : h->cur_mask); h->launches++; }
+    if (full && !a.kkt_only) h->atil_valid = true;
   }
   A.rfa = a.prm.rho_f * a.prm.alpha; A.oma = T(1) - a.prm.alpha; A.inv_rho_g = T(1) / a.prm.rho_g; A.inv_rg = T(1) / (a.prm.rho_g + a.prm.gamma);
   if constexpr (CL) {                                   // two CTAs per problem, launched as a cluster
@@ -341,6 +347,7 @@ template <typename T>
 tmpc_status launch_factor_tw(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double w_in, int32_t* status, const T* w_rows = nullptr) {
   FactorArgs<T> a; a.d = h->d; a.qp = view<T>(qp); a.sigma = h->cfg.sigma; a.w_eq = w_eq; a.w_in = w_in; a.w_rows = w_rows;
   a.rho_bar = w_rows ? nullptr : (const T*)h->cur_rho; a.rho_scale = h->cfg.rho_eq_scale; a.mask = w_rows ? nullptr : h->cur_mask;
+  if (!a.mask) h->atil_valid = false;                   // every problem's factor changes (a masked factorisation is followed by a masked atil_kernel)
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
   // small batches: the launch lasts as long as one problem's chain, so four warps per chain instead of one (tmpc_factor2.cuh)
   const bool wide = h->d.B <= 2 * sm_count();
@@ -598,7 +605,7 @@ tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, vo
   h->factored = false; h->cr = use_cr(*cfg); h->twisted = false; h->launches = 0;
   h->cur_rho = nullptr; h->cur_active = nullptr; h->cur_mask = nullptr; h->bwd_classified = false;
   h->aux[0] = h->aux[1] = nullptr; h->ev[0] = h->ev[1] = h->ev[2] = nullptr;
-  h->pin_live = nullptr; h->ad_ev[0] = h->ad_ev[1] = nullptr;
+  h->pin_live = nullptr; h->ad_ev[0] = h->ad_ev[1] = nullptr; h->atil_valid = false;
   // zero buffers of the adjoint QP (x_init = 0, b = 0)
   if (cudaMemsetAsync(h->ws + L.zero_xinit, 0, L.zero_b - L.zero_xinit, h->stream) != cudaSuccess ||
       cudaMemsetAsync(h->ws + L.zero_b, 0, L.cr - L.zero_b, h->stream) != cudaSuccess) { delete h; return TMPC_E_CUDA; }
@@ -951,7 +958,7 @@ extern "C" tmpc_status tmpc_admm_solve_static(const tmpc_config* cfg, const tmpc
   c.cfg = *cfg; c.d = make_dims(*cfg); c.lay = L; c.ws = ws; c.stream = (cudaStream_t)cuda_stream;
   c.factored = false; c.cr = false; c.twisted = false; c.launches = 0;
   c.cur_rho = nullptr; c.cur_active = nullptr; c.cur_mask = nullptr; c.bwd_classified = false;
-  c.aux[0] = c.aux[1] = nullptr; c.ev[0] = c.ev[1] = c.ev[2] = nullptr; c.pin_live = nullptr; c.ad_ev[0] = c.ad_ev[1] = nullptr;
+  c.aux[0] = c.aux[1] = nullptr; c.ev[0] = c.ev[1] = c.ev[2] = nullptr; c.pin_live = nullptr; c.ad_ev[0] = c.ad_ev[1] = nullptr; c.atil_valid = false;
   s = check_qp(&c, qp); if (s != TMPC_OK) return s;
   // the array keeps the previous call's contents: the per-problem status words must start at zero (the factor kernels overwrite them, this is
   // belt and braces); the factor, the eta scratch of the streamed class and the residual partials are all written before they are read

@@ -707,6 +707,37 @@ def test_f4_linear_rl_cluster_pair_fp64():
     s.close()
 
 
+def test_chain_resident_scratch_follows_the_factor_fp64():
+    """The stage-minor scratch of the chain-resident variants is rebuilt only when the factor changes (full, masked, adjoint).  Call sequences on
+    one handle at N = 160 (one CTA per problem) and N = 320 (cluster pair): kkt_solve before the first solve, a resumed solve that reuses the scratch,
+    a REFINE backward (adjoint factor) followed by a new factor + solve, and two adaptive runs in a row — each against a fresh handle or the oracle."""
+    from paper_2606_24039_b200.solver import Solver
+    from paper_2606_24039_b200 import binding as Bd
+    for N in (160, 320):
+        w = W.linear_rl(B=3, N=N, u_max=1.0)
+        cfg = O.make_cfg(w)
+        ref70, _, _ = O.admm(w, cfg, iters=70)
+        s = Solver(w, dtype="f64")
+        s.factor()
+        eta = np.random.default_rng(2).standard_normal((w.B, w.T, w.n))
+        xt = s.kkt_solve(s._up(eta)).cpu().double().numpy()                 # X rows only: the next solve must still build the whole scratch
+        ref = np.stack([O.solve_S(w, cfg, eta[b].ravel(), b).reshape(w.T, w.n) for b in range(w.B)])
+        assert rel_err(xt, ref) <= 1e-9
+        s.reset_state(); s.admm_solve(30); s.admm_solve(40, flags=Bd.TMPC_SOLVE_ZG_GIVEN)      # second call: scratch reused
+        compare_states(s.state_numpy(), ref70, 1e-9)
+        st = s.state_numpy()
+        dq, dxi = s.backward(2.0 * s.s["x"], mode=Bd.TMPC_BWD_REFACTOR_REFINE)                 # adjoint factor takes the workspace and the scratch
+        s.reset_state(); s.solve(70)                                                          # factor + solve again
+        compare_states(s.state_numpy(), ref70, 1e-9)
+        refa, rinfo, log, rc = O.admm_adaptive(w, cfg, O.make_adaptive(200, 1e-4, 1e-4))
+        for _ in range(2):                                                                    # masked refactorisations, twice on the same handle
+            s.factor(); s.reset_state()
+            out = s.solve_adaptive(200, 1e-4, 1e-4)
+            assert (out["iters"] == rinfo[:, 4].astype(int)).all()
+            compare_states(s.state_numpy(), refa, 1e-7)
+        s.close()
+
+
 def test_long_horizons_chain_resident_small_blocks():
     """The same variant for the (8, 6) and (6, 4) blocks once their records outgrow shared memory (fp64: N > ~190 resp. ~330): selection G with
     soft rows (config 2's data at N = 260), dense G (config 4's bicycle QP at N = 400, G~ rows in global memory too), and the thread-cap
