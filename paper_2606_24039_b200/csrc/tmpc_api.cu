@@ -4,6 +4,7 @@
 #include <cstring>
 #include <mutex>
 #include <new>
+#include <type_traits>
 #include "tmpc_common.cuh"
 #include "tmpc_factor.cuh"
 #include "tmpc_factor2.cuh"
@@ -96,6 +97,7 @@ struct tmpc_ctx {
   const void* cur_rho; const int32_t* cur_active; const int32_t* cur_mask;
   bool bwd_classified;                          // tmpc_backward has left the row classification of its state in the workspace
   cudaStream_t aux[2]; cudaEvent_t ev[3];       // tmpc_admm_solve_host: two sub-batches in flight (copies of one overlap the kernels of the other)
+  bool mask_sparse;                             // hint for the masked factor launch: few problems flagged (later rounds of f1)
   bool atil_valid;                              // the stage-minor scratch of the chain-resident variants matches the factor in the workspace
   int32_t* pin_live; cudaEvent_t ad_ev[2];      // tmpc_admm_solve_adaptive: pinned landing slots of the per-round live counts and their events (created on first use)
 };
@@ -349,11 +351,22 @@ tmpc_status launch_factor_tw(tmpc_ctx* h, const tmpc_qp* qp, double w_eq, double
   a.rho_bar = w_rows ? nullptr : (const T*)h->cur_rho; a.rho_scale = h->cfg.rho_eq_scale; a.mask = w_rows ? nullptr : h->cur_mask;
   if (!a.mask) h->atil_valid = false;                   // every problem's factor changes (a masked factorisation is followed by a masked atil_kernel)
   a.Lam = (T*)(h->ws + h->lay.Lam); a.Sinv = (T*)(h->ws + h->lay.Sinv); a.status = status;
-  // small batches: the launch lasts as long as one problem's chain, so four warps per chain instead of one (tmpc_factor2.cuh)
-  const bool wide = h->d.B <= 2 * sm_count();
-  if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) { if (wide) factor_tw2_kernel<T, 8, 6, true, 4><<<h->d.B, 256, 0, h->stream>>>(a); else factor_tw2_kernel<T, 8, 6, true><<<h->d.B, 64, 0, h->stream>>>(a); }
-  else if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) { if (wide) factor_tw2_kernel<T, 6, 4, true, 4><<<h->d.B, 256, 0, h->stream>>>(a); else factor_tw2_kernel<T, 6, 4, true><<<h->d.B, 64, 0, h->stream>>>(a); }
-  else if (h->d.n == 12 && h->d.nx == 8 && h->d.ng <= 12) { if (h->d.B <= sm_count()) factor_tw2_kernel<T, 12, 8, true, 8><<<h->d.B, 512, 0, h->stream>>>(a); else if (wide) factor_tw2_kernel<T, 12, 8, true, 4><<<h->d.B, 256, 0, h->stream>>>(a); else factor_tw2_kernel<T, 12, 8, true><<<h->d.B, 64, 0, h->stream>>>(a); }
+  // Warps per chain (tmpc_factor2.cuh): a launch that cannot fill the GPU lasts as long as ONE problem's chain, so small batches take four (n = 12:
+  // eight) warps per chain; MASKED launches after the first check of f1 (typically a few flagged problems, the other CTAs leave at once) and mid-size batches of
+  // the (12, 8) block (up to eight per SM) take four warps at four CTAs per SM; everything else keeps one warp per chain, twelve CTAs per SM
+  // (measured at B = 1024: n = 12 fp64 475 -> 459 us, but n = 8 config 2 1.05 -> 1.16 ms per step with four warps).
+  const int B = h->d.B, sms = sm_count();
+  const int wpc = B <= 2 * sms ? ((h->d.n == 12 && B <= sms) ? 8 : 4) : (((a.mask && h->mask_sparse) || (h->d.n == 12 && B <= 8 * sms)) ? 44 : 1);      // 44: four warps, four CTAs per SM
+  auto go = [&](auto nc, auto nx) {
+    constexpr int NC = decltype(nc)::value, NX = decltype(nx)::value;
+    if (wpc == 8) { if constexpr (NC == 12) factor_tw2_kernel<T, NC, NX, true, 8><<<B, 512, 0, h->stream>>>(a); }
+    else if (wpc == 4) factor_tw2_kernel<T, NC, NX, true, 4><<<B, 256, 0, h->stream>>>(a);
+    else if (wpc == 44) factor_tw2_kernel<T, NC, NX, true, 4, 4><<<B, 256, 0, h->stream>>>(a);
+    else factor_tw2_kernel<T, NC, NX, true><<<B, 64, 0, h->stream>>>(a);
+  };
+  if (h->d.n == 8 && h->d.nx == 6 && h->d.ng <= 8) go(std::integral_constant<int, 8>(), std::integral_constant<int, 6>());
+  else if (h->d.n == 6 && h->d.nx == 4 && h->d.ng <= 6) go(std::integral_constant<int, 6>(), std::integral_constant<int, 4>());
+  else if (h->d.n == 12 && h->d.nx == 8 && h->d.ng <= 12) go(std::integral_constant<int, 12>(), std::integral_constant<int, 8>());
   else return TMPC_E_UNSUPPORTED;      // fast_plan() only admits the shapes above
   h->launches++;
   return cuda_ok() ? TMPC_OK : TMPC_E_CUDA;
@@ -490,9 +503,11 @@ tmpc_status do_solve_adaptive(tmpc_ctx* h, const tmpc_qp* qp, tmpc_state* st, co
       if (cudaEventSynchronize(h->ad_ev[(round - 1) & 1]) != cudaSuccess) { rc = TMPC_E_CUDA; break; }
       if (h->pin_live[(round - 1) & 1] == 0) break;
     }
+    h->mask_sparse = round > 0;                          // the first check re-scales most problems, the later ones a few
     if (ad->adapt_rho && k < ad->max_iters) rc = do_factor<T>(h, qp);          // only the problems whose rho_bar changed (mask)
     ++round;
   }
+  h->mask_sparse = false;
   if (rc == TMPC_OK && cudaStreamSynchronize(h->stream) != cudaSuccess) rc = TMPC_E_CUDA;      // the call synchronises (tmpc.h)
   h->cur_rho = nullptr; h->cur_active = nullptr; h->cur_mask = nullptr;
   h->factored = false;                                   // the factor in the workspace now belongs to the per-problem rho_bar values
@@ -605,7 +620,7 @@ tmpc_status tmpc_setup(const tmpc_config* cfg, void* workspace, size_t bytes, vo
   h->factored = false; h->cr = use_cr(*cfg); h->twisted = false; h->launches = 0;
   h->cur_rho = nullptr; h->cur_active = nullptr; h->cur_mask = nullptr; h->bwd_classified = false;
   h->aux[0] = h->aux[1] = nullptr; h->ev[0] = h->ev[1] = h->ev[2] = nullptr;
-  h->pin_live = nullptr; h->ad_ev[0] = h->ad_ev[1] = nullptr; h->atil_valid = false;
+  h->pin_live = nullptr; h->ad_ev[0] = h->ad_ev[1] = nullptr; h->atil_valid = false; h->mask_sparse = false;
   // zero buffers of the adjoint QP (x_init = 0, b = 0)
   if (cudaMemsetAsync(h->ws + L.zero_xinit, 0, L.zero_b - L.zero_xinit, h->stream) != cudaSuccess ||
       cudaMemsetAsync(h->ws + L.zero_b, 0, L.cr - L.zero_b, h->stream) != cudaSuccess) { delete h; return TMPC_E_CUDA; }
@@ -958,7 +973,7 @@ extern "C" tmpc_status tmpc_admm_solve_static(const tmpc_config* cfg, const tmpc
   c.cfg = *cfg; c.d = make_dims(*cfg); c.lay = L; c.ws = ws; c.stream = (cudaStream_t)cuda_stream;
   c.factored = false; c.cr = false; c.twisted = false; c.launches = 0;
   c.cur_rho = nullptr; c.cur_active = nullptr; c.cur_mask = nullptr; c.bwd_classified = false;
-  c.aux[0] = c.aux[1] = nullptr; c.ev[0] = c.ev[1] = c.ev[2] = nullptr; c.pin_live = nullptr; c.ad_ev[0] = c.ad_ev[1] = nullptr; c.atil_valid = false;
+  c.aux[0] = c.aux[1] = nullptr; c.ev[0] = c.ev[1] = c.ev[2] = nullptr; c.pin_live = nullptr; c.ad_ev[0] = c.ad_ev[1] = nullptr; c.atil_valid = false; c.mask_sparse = false;
   s = check_qp(&c, qp); if (s != TMPC_OK) return s;
   // the array keeps the previous call's contents: the per-problem status words must start at zero (the factor kernels overwrite them, this is
   // belt and braces); the factor, the eta scratch of the streamed class and the residual partials are all written before they are read

@@ -34,8 +34,8 @@ namespace tmpc {
 // spread over 128 (256) threads per chain and the phases are separated by a named barrier per chain instead of __syncwarp.  Same sums in the
 // same order.  Measured at (64,40,8,4) fp64: 341 -> 128 -> 108 us per launch; two warps per chain for mid-size batches (B = 1024) lost to the
 // register cap its eight CTAs per SM need (554 against 477 us).
-template <typename T, int NC, int NX, bool TW, int WPC = 1>
-__global__ void __launch_bounds__(64 * WPC, WPC == 1 ? 12 : (WPC <= 4 ? 2 : 1)) factor_tw2_kernel(FactorArgs<T> a) {
+template <typename T, int NC, int NX, bool TW, int WPC = 1, int MB = 0>
+__global__ void __launch_bounds__(64 * WPC, MB ? MB : (WPC == 1 ? 12 : (WPC <= 4 ? 2 : 1))) factor_tw2_kernel(FactorArgs<T> a) {
   constexpr int n = NC, nx = NX, nn = NC * NC, an = NX * NC;
   constexpr int GT = 32 * WPC;                          // threads per chain
   constexpr int EPL = (nn + GT - 1) / GT;               // matrix elements per lane
