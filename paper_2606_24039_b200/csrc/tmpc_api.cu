@@ -461,7 +461,7 @@ tmpc_status do_solve(tmpc_ctx* h, const tmpc_qp* qp, tmpc_state* st, int iters, 
 int32_t* pinned_pair() {
   static std::mutex mu; static int32_t* pool = nullptr; static unsigned next = 0;
   std::lock_guard<std::mutex> lk(mu);
-  if (!pool && cudaHostAlloc((void**)&pool, 1024 * sizeof(int32_t), cudaHostAllocDefault) != cudaSuccess) { cudaGetLastError(); pool = nullptr; return nullptr; }
+  if (!pool && cudaHostAlloc((void**)&pool, 1024 * sizeof(int32_t), cudaHostAllocPortable) != cudaSuccess) { cudaGetLastError(); pool = nullptr; return nullptr; }
   return pool + 2 * (next++ % 512u);
 }
 
