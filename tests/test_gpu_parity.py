@@ -688,6 +688,7 @@ def test_f4_linear_rl_cluster_pair_fp64():
     run_pair(W.linear_rl(B=3, N=80, u_max=1.0), "f64", iters=60)
     run_pair(W.with_dense_Ap(W.linear_rl(B=2, N=81, u_max=10.0)), "f64", iters=40)
     run_pair(W.linear_rl(B=3, N=160, u_max=1.0), "f32", iters=60)
+    run_pair(W.linear_rl(B=2, N=340, u_max=1.0), "f32", iters=40)      # fp32 on the pair with the chain's share (322 <= N <= 350)
     # a batch that fills the GPU keeps one CTA per problem (chain-resident, no cluster)
     run_pair(W.linear_rl(B=80, N=160, u_max=1.0), "f64", iters=30)
     ref, rinfo, log, rc = O.admm_adaptive(w, O.make_cfg(w), O.make_adaptive(300, 1e-4, 1e-4))
