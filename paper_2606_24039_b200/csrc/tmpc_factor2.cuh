@@ -83,14 +83,34 @@ __global__ void __launch_bounds__(64 * WPC, MB ? MB : (WPC == 1 ? 12 : (WPC <= 4
 #pragma unroll
     for (int u = 0; u < RPL; ++u) { const int e = lane + GT * u; if (e < RAW) rD[e] = (double)pre[u]; }
   };
+  // The phases that touch the LOWER TRIANGLE only (Theta, the Cholesky updates, the triangular inverse) walk its n (n + 1) / 2 elements, TPL per
+  // lane, instead of all n^2 with half of them masked: for n = 6 that is one pass of 21 lanes instead of two passes (36 > 32).  The (row, column)
+  // of a lane's elements never changes, so it is worked out once.
+  // Used where it saves a pass (n = 6, n = 12; measured: config 4 22.0 -> 21.7 ms, (1024,40,8,4) factor 459 -> 377 us); for n = 8 both walks take
+  // two passes and the plain one is faster (config 2 1.053 vs 1.068 ms), so it keeps e = lane + GT u with the upper triangle masked.
+  constexpr int NTRI = n * (n + 1) / 2, TPT = (NTRI + GT - 1) / GT;
+  constexpr bool TRI = TPT < EPL;
+  constexpr int TPL = TRI ? TPT : EPL;
+  int tri_e[TRI ? TPL : 1];                             // triangular walk: i * n + j of my u-th element, -1 for none
+  if constexpr (TRI) {
+#pragma unroll
+    for (int u = 0; u < TPL; ++u) {
+      const int q = lane + GT * u;
+      int i = 0;
+#pragma unroll
+      for (int r = 1; r < n; ++r) if (q >= r * (r + 1) / 2) i = r;
+      tri_e[u] = q < NTRI ? i * n + (q - i * (i + 1) / 2) : -1;
+    }
+  }
   // Theta_t (lower triangle) minus W W' of up to two finished neighbours, from the raw data in shared memory
   auto theta = [&](int t, double* dst, const double* W1, const double* W2) {
 #pragma unroll
-    for (int u = 0; u < EPL; ++u) {
-      const int e = lane + GT * u;
-      if (e >= nn) continue;
+    for (int u = 0; u < TPL; ++u) {
+      int e;
+      if constexpr (TRI) { e = tri_e[u]; if (e < 0) continue; }
+      else { e = lane + GT * u; if (e >= nn) continue; }
       const int i = e / n, j = e % n;
-      if (j > i) continue;
+      if constexpr (!TRI) { if (j > i) continue; }
       double s = rD[e];
       if (i == j) s += sigma;
       double acc = 0;
@@ -123,9 +143,9 @@ __global__ void __launch_bounds__(64 * WPC, MB ? MB : (WPC == 1 ? 12 : (WPC <= 4
       const double rs = rsqrt(dk), sq = dk * rs, inv = rs * rs;
       rsk[k] = rs;
 #pragma unroll
-      for (int u = 0; u < EPL; ++u) {
-        const int e = lane + GT * u, i = e / n, j = e % n;
-        if (e < nn && j > k && j <= i) Am_[e] -= Am_[i * n + k] * Am_[j * n + k] * inv;
+      for (int u = 0; u < TPL; ++u) {
+        if constexpr (TRI) { const int e = tri_e[u], i = e / n, j = e % n; if (e >= 0 && j > k) Am_[e] -= Am_[i * n + k] * Am_[j * n + k] * inv; }
+        else { const int e = lane + GT * u, i = e / n, j = e % n; if (e < nn && j > k && j <= i) Am_[e] -= Am_[i * n + k] * Am_[j * n + k] * inv; }
       }
       gsync();
       if (lane < n && lane >= k) Am_[lane * n + k] = lane == k ? sq : Am_[lane * n + k] * rs;
@@ -139,9 +159,9 @@ __global__ void __launch_bounds__(64 * WPC, MB ? MB : (WPC == 1 ? 12 : (WPC <= 4
     for (int k = 0; k < n - 1; ++k) {
       const double inv = rsk[k];
 #pragma unroll
-      for (int u = 0; u < EPL; ++u) {
-        const int e = lane + GT * u, i = e / n, j = e % n;
-        if (e < nn && i > k && j <= k) Xo[e] -= Am_[i * n + k] * Xo[k * n + j] * inv;
+      for (int u = 0; u < TPL; ++u) {
+        if constexpr (TRI) { const int e = tri_e[u], i = e / n, j = e % n; if (e >= 0 && i > k && j <= k) Xo[e] -= Am_[i * n + k] * Xo[k * n + j] * inv; }
+        else { const int e = lane + GT * u, i = e / n, j = e % n; if (e < nn && i > k && j <= k) Xo[e] -= Am_[i * n + k] * Xo[k * n + j] * inv; }
       }
       gsync();
     }
