@@ -45,6 +45,15 @@ def main():
     s = Solver(w, dtype="f64"); s.solve(20)
     ref, _, _ = O.admm(w, O.make_cfg(w), iters=20)
     check(s.state_numpy(), ref, 1e-9, "generic n=5 f64"); s.close()
+    # long-horizon forms of the resident kernel, (12, 8) block, fp64: one CTA with the chain's share (N = 160, stage-minor global operands),
+    # the cluster pair with full records (N = 80) and with the chain's share (N = 320: distributed shared memory, remote mbarriers), each with
+    # the adaptive schedule on top (early exit of terminated CTAs / pairs, masked multi-warp factor)
+    for N in (160, 80, 320):
+        w = W.linear_rl(B=2, N=N, u_max=1.0)
+        s = Solver(w, dtype="f64"); s.solve(20)
+        ref, _, _ = O.admm(w, O.make_cfg(w), iters=20)
+        check(s.state_numpy(), ref, 1e-9, f"linear_rl B=2 N={N} f64")
+        s.reset_state(); s.solve_adaptive(100, 1e-3, 1e-3); s.close()
     # cyclic reduction (grid barrier), chunked form needs T >= 256
     w = W.config5(N=300)
     s = Solver(w, dtype="f64", linsolve=Bd.TMPC_LIN_CYCLIC_REDUCTION); s.reset_state(w.xbar0); s.sqp(1, 20)
