@@ -75,7 +75,8 @@ typedef struct {
   const void* x_init;               /* [B][nx]                                                                           */
   const void* G; int64_t G_bstride; /* [B|1][T][ng][n]  or NULL with g_is_selection (eq. 31)                             */
   const void* lo; const void* hi;   /* [B][T][ng]       +-INFINITY allowed (eq. 38)                                      */
-} tmpc_qp; /* tmpc_linearize WRITES Am, Ap, b, G, lo, hi (the caller passes writable buffers there) */
+} tmpc_qp; /* tmpc_linearize WRITES Am, Ap, b, G, lo, hi (the caller passes writable buffers there).  D, E, Am, Ap, b and G must be 16-byte
+            * aligned (bulk copies of the streamed class, vector stores of tmpc_linearize): TMPC_E_BADARG otherwise. */
 
 typedef struct { /* ADMM state, in/out = warm start (Alg. 3 'Initial guess') */
   void* x;  /* [B][T][n]   */

@@ -668,6 +668,7 @@ tmpc_status tmpc_linearize(tmpc_handle h, const void* xbar, const void* stage_re
   if (!h || !xbar || !stage_ref || !qp || !qp->Am || !qp->Ap || !qp->b || !qp->G || !qp->lo || !qp->hi) return TMPC_E_BADARG;
   if (h->cfg.model != TMPC_MODEL_BICYCLE_IMPLICIT_MIDPOINT) return TMPC_E_UNSUPPORTED;
   if (qp->G_bstride != (int64_t)h->d.T * 3 * 6 && h->d.B > 1) return TMPC_E_BADARG;
+  if (((uintptr_t)qp->Am | (uintptr_t)qp->Ap | (uintptr_t)qp->b | (uintptr_t)qp->G) & 15u) return TMPC_E_BADARG;      // vector stores (tmpc.h)
   const long long total = (long long)h->d.B * h->d.T; const int nt = 128; const unsigned nb = (unsigned)((total + nt - 1) / nt);
   const tmpc_config& c = h->cfg;
   if (c.dtype == TMPC_F32) {
@@ -689,6 +690,8 @@ static tmpc_status check_qp(tmpc_handle h, const tmpc_qp* qp) {
   if (!h || !qp || !qp->D || !qp->E || !qp->q || !qp->Am || !qp->Ap || !qp->b || !qp->x_init) return TMPC_E_BADARG;
   if (h->d.ng > 0 && (!qp->lo || !qp->hi)) return TMPC_E_BADARG;
   if (h->d.ng > 0 && !h->cfg.g_is_selection && !qp->G) return TMPC_E_BADARG;
+  const void* al[6] = {qp->D, qp->E, qp->Am, qp->Ap, qp->b, qp->G};          // 16-byte aligned (tmpc.h)
+  for (int k = 0; k < 6; ++k) if ((uintptr_t)al[k] & 15u) return TMPC_E_BADARG;
   return TMPC_OK;
 }
 

@@ -23,6 +23,24 @@ struct LinArgs {
   T* Am; T* Ap; T* b; T* G; T* lo; T* hi;
 };
 
+// contiguous run of CNT elements in 16-byte stores (dst 16-byte aligned, CNT a multiple of 16 / sizeof(T)) or 8-byte stores for floats
+template <int CNT> __device__ __forceinline__ void store_run16(float* dst, const float* v) {
+#pragma unroll
+  for (int c = 0; c < CNT / 4; ++c) reinterpret_cast<float4*>(dst)[c] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
+}
+template <int CNT> __device__ __forceinline__ void store_run16(double* dst, const double* v) {
+#pragma unroll
+  for (int c = 0; c < CNT / 2; ++c) reinterpret_cast<double2*>(dst)[c] = make_double2(v[2 * c], v[2 * c + 1]);
+}
+template <int CNT> __device__ __forceinline__ void store_run8(float* dst, const float* v) {      // 8-byte aligned run of floats
+#pragma unroll
+  for (int c = 0; c < CNT / 2; ++c) reinterpret_cast<float2*>(dst)[c] = make_float2(v[2 * c], v[2 * c + 1]);
+}
+template <int CNT> __device__ __forceinline__ void store_run8(double* dst, const double* v) {
+#pragma unroll
+  for (int c = 0; c < CNT; ++c) dst[c] = v[c];
+}
+
 template <typename T>
 __global__ void bicycle_linearize_kernel(LinArgs<T> a) {
   const int T_ = a.N + 1, n = 6, nx = 4;
@@ -32,9 +50,13 @@ __global__ void bicycle_linearize_kernel(LinArgs<T> a) {
   const T* r = a.ref + ((size_t)p * T_ + t) * n;
   T* g = a.G + ((size_t)p * T_ + t) * 3 * n;
   T sr, cr; tsincos(r[2], &sr, &cr);
+  {                                                      // the three G rows of a stage are 72 / 144 contiguous bytes: vector stores
+    T gv[18];
 #pragma unroll
-  for (int k = 0; k < 18; ++k) g[k] = T(0);
-  g[4] = T(1); g[n + 5] = T(1); g[2 * n] = -sr; g[2 * n + 1] = cr;
+    for (int k = 0; k < 18; ++k) gv[k] = T(0);
+    gv[4] = T(1); gv[n + 5] = T(1); gv[2 * n] = -sr; gv[2 * n + 1] = cr;
+    store_run8<18>(g, gv);
+  }
   const T off = -sr * r[0] + cr * r[1];
   T* lo = a.lo + ((size_t)p * T_ + t) * 3; T* hi = a.hi + ((size_t)p * T_ + t) * 3;
   lo[0] = a.glo[0]; lo[1] = a.glo[1]; lo[2] = a.glo[2] + off;
@@ -58,13 +80,15 @@ __global__ void bicycle_linearize_kernel(LinArgs<T> a) {
   am[2][5] = dt * Fu21; am[3][4] = dt;
   const T F[4] = {vel * c, vel * s, vel * iL * td, acc};
   T* Am = a.Am + ((size_t)p * a.N + t) * nx * n; T* Ap = a.Ap + ((size_t)p * a.N + t) * nx * n; T* b = a.b + ((size_t)p * a.N + t) * nx;
+  T bv[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     T sb = -(vk[i] + dt * F[i] - vk1[i]);
 #pragma unroll
-    for (int j = 0; j < 6; ++j) { Am[i * n + j] = am[i][j]; Ap[i * n + j] = ap[i][j]; sb += am[i][j] * vk[j] + ap[i][j] * vk1[j]; }
-    b[i] = sb;
+    for (int j = 0; j < 6; ++j) sb += am[i][j] * vk[j] + ap[i][j] * vk1[j];
+    bv[i] = sb;
   }
+  store_run16<24>(Am, &am[0][0]); store_run16<24>(Ap, &ap[0][0]); store_run16<4>(b, bv);      // 96 / 192 and 16 / 32 contiguous bytes per block
 }
 
 }  // namespace tmpc
